@@ -1,0 +1,274 @@
+"""Pins for the oracle's PDD / PPT statement and its 3-D sweeps.  CPU only.
+The printed matrices at PAPER.md:L116 / L136 come from tests/golden/Z_n12_p4.txt."""
+import os
+import re
+
+import numpy as np
+import pytest
+import scipy.linalg
+
+import oracle as orc
+from paper_1812_01178_b200 import configs, inputs
+
+GOLD = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+rng = np.random.default_rng(4321)
+
+
+def relerr(x, ref):
+    return np.max(np.abs(x - ref)) / np.max(np.abs(ref))
+
+
+def random_dominant(n, margin=0.5):
+    a = rng.uniform(-1, 1, n); c = rng.uniform(-1, 1, n)
+    b = (np.abs(a) + np.abs(c) + margin) * rng.choice([-1.0, 1.0], n)
+    a[0] = 0.0; c[-1] = 0.0
+    return a, b, c
+
+
+def parse_golden(section):
+    rows, on = [], False
+    for line in open(os.path.join(GOLD, "Z_n12_p4.txt")):
+        line = line.strip()
+        if not line or line.startswith("#"):
+            continue
+        if line.startswith("["):
+            on = line == "[%s]" % section
+            continue
+        if on:
+            rows.append(line.split())
+    return rows
+
+
+@pytest.mark.parametrize("section", ["Z", "Zbar"])
+def test_Z_structure_as_printed_in_paper(section):
+    """n = 12, p = 4, m = 3: every entry of Z (L116) and Z-bar (L136) sits where the paper prints it."""
+    n, P, m = 12, 4, 3
+    a, b, c = random_dominant(n)
+    d = rng.uniform(-1, 1, n)
+    _, v, w = orc.local_solves(P, a, b, c, d)
+    Z = orc.build_Z(n, P, v, w)
+    M = Z if section == "Z" else orc.build_Zbar(Z)
+    gold = parse_golden(section)
+    assert len(gold) == 6 and all(len(r) == 6 for r in gold)
+    for r in range(6):
+        for cidx in range(6):
+            s = gold[r][cidx]
+            if s in (".", "0"):
+                assert M[r, cidx] == 0.0, (r, cidx)
+            elif s == "1":
+                assert M[r, cidx] == 1.0, (r, cidx)
+            else:
+                kind, pos, part = re.match(r"([vw])([1m])\((\d)\)", s).groups()
+                vec = v if kind == "v" else w
+                idx = int(part) * m + (0 if pos == "1" else m - 1)
+                assert M[r, cidx] == vec[idx] and vec[idx] != 0.0, (r, cidx, s)
+
+
+def test_Zbar_is_tridiagonal_and_equals_P_plus_EtAinvVP():
+    n, P = 24, 6
+    a, b, c = random_dominant(n)
+    _, v, w = orc.local_solves(P, a, b, c, np.zeros(n))
+    Zb = orc.build_Zbar(orc.build_Z(n, P, v, w))
+    K = 2 * (P - 1)
+    for r in range(K):
+        for cidx in range(K):
+            if abs(r - cidx) > 1:
+                assert Zb[r, cidx] == 0.0
+    # independent dense construction of Z = I + E^T A~^{-1} V
+    st = orc.partition_bounds(n, P)
+    A = orc.dense_from_tridiag(a, b, c)
+    At = A.copy(); E = np.zeros((n, K)); V = np.zeros((n, K))
+    for i in range(1, P):
+        f, l = st[i], st[i] - 1
+        At[f, l] = 0.0; At[l, f] = 0.0
+        E[l, 2 * i - 2] = 1.0; E[f, 2 * i - 1] = 1.0
+        V[f, 2 * i - 2] = a[f]; V[l, 2 * i - 1] = c[l]
+    assert np.allclose(At + V @ E.T, A, atol=0)                      # dA = V E^T (L85-91)
+    Zd = np.eye(K) + E.T @ np.linalg.solve(At, V)
+    assert np.allclose(orc.build_Z(n, P, v, w), Zd, atol=1e-14)
+    Pm = np.zeros((K, K))
+    for k in range(0, K, 2):
+        Pm[k, k + 1] = Pm[k + 1, k] = 1.0
+    assert np.allclose(Zb, Pm + E.T @ np.linalg.solve(At, V @ Pm), atol=1e-14)      # Eq. for Z-bar, L136
+
+
+def test_spikes_and_xt_vs_dense_blocks():
+    n, P = 23, 4                                                     # ragged: sizes 6,6,6,5
+    a, b, c = random_dominant(n)
+    d = rng.uniform(-1, 1, n)
+    xt, v, w = orc.local_solves(P, a, b, c, d)
+    st = orc.partition_bounds(n, P)
+    A = orc.dense_from_tridiag(a, b, c)
+    for p in range(P):
+        s, e = st[p], st[p + 1]
+        Ap = A[s:e, s:e]
+        assert relerr(xt[s:e], np.linalg.solve(Ap, d[s:e])) < 1e-14
+        e1 = np.zeros(e - s); e1[0] = a[s]
+        em = np.zeros(e - s); em[-1] = c[e - 1]
+        if p > 0:
+            assert np.allclose(v[s:e], np.linalg.solve(Ap, e1), rtol=1e-13, atol=1e-300)
+        else:
+            assert np.all(v[s:e] == 0)
+        if p < P - 1:
+            assert np.allclose(w[s:e], np.linalg.solve(Ap, em), rtol=1e-13, atol=1e-300)
+        else:
+            assert np.all(w[s:e] == 0)
+
+
+@pytest.mark.parametrize("n,P", [(12, 4), (32, 4), (64, 8), (100, 7), (288, 16), (288, 32)])
+def test_ppt_equals_thomas_and_y_are_interface_values(n, P):
+    """PPT makes no approximation (L156); y_{2i-1} = x_{last_{i-1}}, y_{2i} = x_{first_i}."""
+    a, b, c = random_dominant(n, margin=0.05)
+    d = rng.uniform(-1, 1, n)
+    x_ref = orc.thomas(a, b, c, d)
+    x, y = orc.partitioned_line(P, orc.MODE_PPT, a, b, c, d, return_y=True)
+    assert relerr(x, x_ref) < 1e-13
+    assert relerr(x, np.linalg.solve(orc.dense_from_tridiag(a, b, c), d)) < 1e-13
+    st = orc.partition_bounds(n, P)
+    for i in range(1, P):
+        assert abs(y[2 * i - 2] - x_ref[st[i] - 1]) < 1e-13 * np.max(np.abs(x_ref))
+        assert abs(y[2 * i - 1] - x_ref[st[i]]) < 1e-13 * np.max(np.abs(x_ref))
+
+
+def test_P1_reduces_to_thomas_bitwise():
+    a, b, c = random_dominant(40)
+    d = rng.uniform(-1, 1, 40)
+    for mode in (orc.MODE_PDD, orc.MODE_PPT):
+        assert np.array_equal(orc.partitioned_line(1, mode, a, b, c, d), orc.thomas(a, b, c, d))
+
+
+def test_pdd_error_bounded_by_dropped_and_exact_when_decayed():
+    """L148-154: v_m, w_1 -> 0 when n >> p for strictly dominant systems; then PDD == PPT."""
+    n = 256
+    for margin, P in [(3.0, 4), (3.0, 8), (0.05, 4), (0.05, 16), (0.002, 8)]:
+        a, b, c = random_dominant(n, margin=margin)
+        d = rng.uniform(-1, 1, n)
+        x_ref = orc.thomas(a, b, c, d)
+        dropped = orc.pdd_dropped(P, a, b, c)
+        err = relerr(orc.partitioned_line(P, orc.MODE_PDD, a, b, c, d), x_ref)
+        assert err <= 50 * dropped + 1e-13, (margin, P, err, dropped)
+        if dropped < 1e-30:
+            assert err < 1e-13
+    # strongly dominant: dropped entries are below the rounding of the 2x2 blocks -> PDD and PPT agree to rounding
+    a, b, c = random_dominant(64, margin=50.0)
+    d = rng.uniform(-1, 1, 64)
+    assert relerr(orc.partitioned_line(4, orc.MODE_PDD, a, b, c, d), orc.partitioned_line(4, orc.MODE_PPT, a, b, c, d)) < 1e-15
+
+
+def test_pdd_dropped_matches_dense_definition():
+    n, P = 48, 6
+    a, b, c = random_dominant(n, margin=0.1)
+    _, v, w = orc.local_solves(P, a, b, c, np.zeros(n))
+    st = orc.partition_bounds(n, P)
+    ref = max(max(abs(v[st[i] - 1]) for i in range(2, P)), max(abs(w[st[i]]) for i in range(1, P - 1)))
+    assert orc.pdd_dropped(P, a, b, c) == ref
+    Zfull = orc.build_Z(n, P, v, w); Zpdd = orc.build_Z(n, P, v, w, pdd=True)
+    assert np.max(np.abs(Zfull - Zpdd)) == ref
+    for i in range(1, P):                      # PDD Z is block diagonal with 2x2 blocks (L152-154)
+        blk = Zpdd[2 * i - 2:2 * i, :].copy(); blk[:, 2 * i - 2:2 * i] = 0
+        assert np.all(blk == 0)
+
+
+def test_paper_claims_pdd_on_adi_and_helmholtz():
+    """L164: PDD matches the exact ADI solution to machine accuracy (n >> p); L172: PDD inaccurate on the weakly
+    dominant Poisson systems, while PPT stays exact (L156)."""
+    cfg = configs.get(2)
+    _, yf, _ = cfg.faces()
+    d = inputs.uniform_pm1(7, cfg.ny)
+    a, b, c = orc.adi_coeffs(yf, orc.BC_DIRICHLET, cfg.alpha)
+    assert relerr(orc.partitioned_line(4, orc.MODE_PDD, a, b, c, d), orc.thomas(a, b, c, d)) < 1e-14
+    kz2 = cfg.kz2()
+    a, b, c, _ = orc.helmholtz_coeffs(yf, kz2[1])
+    ref = orc.thomas(a, b, c, d, long_double=True)
+    assert relerr(orc.partitioned_line(4, orc.MODE_PDD, a, b, c, d), ref) > 1e-3
+    assert relerr(orc.partitioned_line(4, orc.MODE_PPT, a, b, c, d), ref) < 1e-12
+    assert relerr(orc.thomas(a, b, c, d), ref) < 1e-12
+
+
+@pytest.mark.parametrize("mode", [orc.MODE_PDD, orc.MODE_PPT])
+def test_cyclic_line_with_partitions(mode):
+    n, P = 64, 4
+    a = rng.uniform(-1, 0, n); c = rng.uniform(-1, 0, n); b = 1.0 - a - c + 6.0
+    d = rng.uniform(-1, 1, n)
+    ref = np.linalg.solve(orc.dense_from_tridiag(a, b, c, cyclic=True), d)
+    assert relerr(orc.cyclic_line(P, mode, a, b, c, d), ref) < 1e-13
+    assert relerr(orc.cyclic_thomas(a, b, c, d), ref) < 1e-14
+
+
+# ---------------------------------------------------------------- 3-D sweeps
+def sweep_reference(field, a, b, c, axis, cyclic):
+    """independent: move the axis last and solve every line with LAPACK."""
+    n = b.size
+    A = orc.dense_from_tridiag(a, b, c, cyclic=cyclic)
+    moved = np.moveaxis(field, axis, 0).reshape(n, -1)
+    sol = np.linalg.solve(A, moved)
+    return np.moveaxis(sol.reshape(np.moveaxis(field, axis, 0).shape), 0, axis)
+
+
+@pytest.mark.parametrize("direction", [0, 1, 2])
+@pytest.mark.parametrize("mode,P", [(orc.MODE_THOMAS, 1), (orc.MODE_PPT, 3), (orc.MODE_PDD, 2)])
+def test_adi_sweep_every_direction_vs_lapack(direction, mode, P):
+    nx, ny, nz = 12, 10, 8
+    xf = inputs.faces_uniform(nx, 1.5); yf = inputs.faces_tanh_two_sided(ny, 2.0); zf = inputs.faces_uniform(nz, 1.0)
+    bcs = (orc.BC_DIRICHLET, orc.BC_DIRICHLET, orc.BC_PERIODIC)
+    alpha = 2e-3
+    field = inputs.rhs_uniform((nz, ny, nx), 11)
+    f = (xf, yf, zf)[direction]
+    a, b, c = orc.adi_coeffs(f, bcs[direction], alpha)
+    ref = sweep_reference(field, a, b, c, axis=2 - direction, cyclic=(direction == 2))
+    out = orc.adi_sweep(field.copy(), xf, yf, zf, bcs, direction, mode, P, alpha)
+    assert relerr(out, ref) < 1e-13
+
+
+def test_sweep_one_hot_touches_only_its_line():
+    nx, ny, nz = 8, 6, 5
+    xf = inputs.faces_uniform(nx, 1.0); yf = inputs.faces_uniform(ny, 1.0); zf = inputs.faces_uniform(nz, 1.0)
+    bcs = (orc.BC_DIRICHLET, orc.BC_DIRICHLET, orc.BC_PERIODIC)
+    for direction in range(3):
+        field = np.zeros((nz, ny, nx)); field[2, 3, 4] = 1.0
+        out = orc.adi_sweep(field, xf, yf, zf, bcs, direction, orc.MODE_THOMAS, 1, 0.05)
+        mask = np.zeros_like(out, dtype=bool)
+        if direction == 0: mask[2, 3, :] = True
+        if direction == 1: mask[2, :, 4] = True
+        if direction == 2: mask[:, 3, 4] = True
+        assert np.all(out[~mask] == 0.0) and np.all(out[mask] != 0.0)
+
+
+@pytest.mark.parametrize("mode,P", [(orc.MODE_THOMAS, 1), (orc.MODE_PPT, 4), (orc.MODE_THOMAS_LD, 1)])
+def test_helmholtz_solve_residual_and_pin(mode, P):
+    nx, ny, nz = 6, 16, 8
+    nm = nz // 2 + 1
+    yf = inputs.faces_tanh_one_sided(ny, 2.0)
+    kz2 = inputs.modified_wavenumbers_z(nz)
+    kx2 = inputs.modified_wavenumbers_x(nx, 0.75)
+    rhs = inputs.rhs_complex_uniform((nm, ny, nx), 5)
+    sol = orc.helmholtz_solve(rhs.copy(), yf, kx2, kz2, mode, P)
+    lo, up = orc.metrics(yf, orc.BC_NEUMANN)
+    for m in range(nm):
+        for i in range(nx):
+            lam = kx2[i] + kz2[m]
+            L = np.zeros((ny, ny))
+            for j in range(ny):                                   # unpinned operator delta2_y - lambda, Neumann ends
+                if j > 0: L[j, j - 1] = lo[j]; L[j, j] -= lo[j]
+                if j < ny - 1: L[j, j + 1] = up[j]; L[j, j] -= up[j]
+                L[j, j] -= lam
+            phi = sol[m, :, i]; r = L @ phi - rhs[m, :, i]
+            scale = np.max(np.abs(L)) * np.max(np.abs(phi))
+            if lam == 0.0:
+                assert phi[0] == 0.0                               # pinned point
+                assert np.max(np.abs(r[1:])) < 1e-12 * scale
+            else:
+                assert np.max(np.abs(r)) < 1e-12 * scale
+    # kx2 = None means zeros: then the whole m = 0 plane is pinned
+    sol0 = orc.helmholtz_solve(rhs.copy(), yf, None, kz2, mode, P)
+    assert np.all(sol0[0, 0, :] == 0.0)
+
+
+def test_cyclic_solve_user_coefficients():
+    nx, ny, nz = 5, 4, 12
+    a = rng.uniform(-1, 0, nz); c = rng.uniform(-1, 0, nz); b = 2.5 - a - c
+    field = inputs.rhs_uniform((nz, ny, nx), 3)
+    ref = sweep_reference(field, a, b, c, axis=0, cyclic=True)
+    for mode, P in [(orc.MODE_THOMAS, 1), (orc.MODE_PPT, 3), (orc.MODE_PDD, 2)]:
+        out = orc.cyclic_solve(field.copy(), 2, mode, P, a, b, c)
+        assert relerr(out, ref) < 1e-13
