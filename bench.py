@@ -1,0 +1,304 @@
+#!/usr/bin/env python
+"""bench.py -- one JSON line for the tdx hot path.
+
+A step = one pass of the whole hot path over one synthetic field of the chosen BASELINE.json config:
+    x sweep -> y sweep -> cyclic z sweep of (I - alpha delta2)   (tdx_adi_sweep, PPT or PDD, tuned P)
+    + the nm = nz/2+1 spanwise-wavenumber Helmholtz y-solves      (tdx_helmholtz_wavenumber_solve)
+metric  = Gpts/s per sweep: real grid values solved per second, averaged over the four sweeps of a step
+          (points of a step = 3 nx ny nz + 2 nx ny nm).
+Launch: python bench.py --gpus N --steps K --warmup W   (N > 1: under torch.distributed.run, one rank per GPU; the
+path shards as independent fields, weak scaling, no data-path collective).
+--impl reference times the CPU oracle (oracle/) on the host cores on a bounded sample of the same workload.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_1812_01178_b200 import configs  # noqa: E402
+
+METRIC = "Gpts/s per ADI sweep direction (fp64 PDD/PPT); achieved HBM GB/s vs peak"
+UNIT = "Gpts/s"
+BYTES_PER_POINT = 16.0          # 8 B read + 8 B written per real grid value per sweep
+
+# tuned partitions per line (x, y, z, helmholtz-y) per config; rows per partition <= 64
+TUNED_P = {1: (4, 4, 4, 4), 2: (16, 8, 8, 8), 3: (32, 16, 16, 16), 4: (64, 32, 16, 32), 5: (256, 18, 32, 18)}
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="tdx", choices=["tdx", "reference"])
+    ap.add_argument("--config", type=int, default=5, help="BASELINE.json config number 1..5")
+    ap.add_argument("--mode", default="ppt", choices=["ppt", "pdd", "thomas"])
+    ap.add_argument("--P", default="", help="override partitions: Px,Py,Pz,Ph")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--e2e-steps", type=int, default=2)
+    return ap.parse_args()
+
+
+def measured_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler(threading.Thread):
+    """nvidia-smi clocks / throttle reasons DURING the timed region."""
+    Q = "clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
+        "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.stop_flag, self.rows = index, threading.Event(), []
+
+    def run(self):
+        try:
+            proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits", "-lms", "100"],
+                                    stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except Exception:
+            return
+        while not self.stop_flag.is_set():
+            line = proc.stdout.readline()
+            if not line:
+                break
+            self.rows.append([x.strip() for x in line.split(",")])
+        proc.terminate()
+
+    def summary(self):
+        sm = [float(r[0]) for r in self.rows if r and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if len(r) > 1 and r[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for k, n in enumerate(names) if any(len(r) > 2 + k and r[2 + k].lower().startswith("active") for r in self.rows)]
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": reasons, "samples": len(sm)}
+
+
+def step_points(cfg):
+    return 3 * cfg.npts + 2 * cfg.nx * cfg.ny * cfg.nm
+
+
+def sample_shapes(cfg):
+    """Bounded sample of the workload for the CPU oracle: same grid lines, fewer of them (about 10-30 s of CPU work)."""
+    budget = 100_000_000                                       # real values per sweep
+    kx = max(1, min(cfg.nz, budget // (cfg.nx * cfg.ny)))      # planes for the x and y sweeps
+    jz = max(1, min(cfg.ny, budget // (cfg.nx * cfg.nz)))      # rows for the z sweep
+    mh = max(1, min(cfg.nm, budget // (2 * cfg.nx * cfg.ny)))  # wavenumbers for Helmholtz
+    return kx, jz, mh
+
+
+def run_oracle_sample(cfg, repeats=1):
+    """Times the oracle as it stands (Thomas / cyclic Thomas per line, OpenMP over lines). Returns (Gpts/s, info)."""
+    sys.path.insert(0, os.path.join(ROOT, "oracle"))
+    import oracle as orc
+    from paper_1812_01178_b200 import inputs
+    xf, yf, zf = cfg.faces()
+    bcs = (orc.BC_DIRICHLET, orc.BC_DIRICHLET, orc.BC_PERIODIC)
+    kx, jz, mh = sample_shapes(cfg)
+    fxy = inputs.rhs_uniform((kx, cfg.ny, cfg.nx), cfg.seed)
+    fz = inputs.rhs_uniform((cfg.nz, jz, cfg.nx), cfg.seed + 100)
+    fh = inputs.rhs_complex_uniform((mh, cfg.ny, cfg.nx), cfg.seed)
+    kz2 = cfg.kz2()[:mh]
+    zf_k = np.linspace(0.0, 1.0, kx + 1) if kx >= 2 else np.array([0.0, 0.5, 1.0])
+    yf_j = np.linspace(0.0, 1.0, jz + 1) if jz >= 2 else np.array([0.0, 0.5, 1.0])
+    pts = 2 * fxy.size + fz.size + 2 * fh.size
+    best = None
+    for _ in range(repeats):
+        t0 = time.perf_counter()
+        orc.adi_sweep(fxy, xf, yf, zf_k, bcs, 0, orc.MODE_THOMAS, 1, cfg.alpha)
+        orc.adi_sweep(fxy, xf, yf, zf_k, bcs, 1, orc.MODE_THOMAS, 1, cfg.alpha)
+        orc.adi_sweep(fz, xf, yf_j, zf, bcs, 2, orc.MODE_THOMAS, 1, cfg.alpha)
+        orc.helmholtz_solve(fh, yf, None, kz2, orc.MODE_THOMAS, 1)
+        dt = time.perf_counter() - t0
+        best = dt if best is None else min(best, dt)
+    info = {"kind": "oracle", "cores": orc.num_threads(),
+            "sample": "%s: x,y sweeps on %d z-planes, z sweep on %d y-rows, Helmholtz on %d wavenumbers (%.1f M real values, %.2f s)"
+                      % (cfg.name, kx, jz, mh, pts / 1e6, best)}
+    return pts / best / 1e9, best, info
+
+
+def run_reference(args, rank, world):
+    """--impl reference: the oracle on the host cores, each step a bounded sample of the workload (rank 0 only)."""
+    if rank != 0:
+        return
+    cfg = configs.get(args.config)
+    for _ in range(min(args.warmup, 1)):
+        run_oracle_sample(cfg)
+    times, val = [], None
+    for _ in range(max(1, min(args.steps, 3))):
+        val, dt, info = run_oracle_sample(cfg)
+        times.append(dt)
+    kx, jz, mh = sample_shapes(cfg)
+    pts = 2 * kx * cfg.ny * cfg.nx + cfg.nz * jz * cfg.nx + 2 * mh * cfg.ny * cfg.nx
+    t = float(np.mean(times))
+    value = pts / t / 1e9
+    info["value"] = value
+    info["unit"] = UNIT
+    print(json.dumps({"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+                      "steps": len(times), "warmup": min(args.warmup, 1), "ms_per_step": t * 1e3, "higher_is_better": True,
+                      "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                      "config": {"workload": cfg.name + " (bounded sample per step)", "mode": "thomas (cpu oracle)"},
+                      "cpu_baseline": info,
+                      "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
+
+
+def run_tdx(args, rank, world, local_rank):
+    import torch
+    import torch.distributed as dist
+    from paper_1812_01178_b200 import binding as tdx
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the tdx path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    cfg = configs.get(args.config)
+    mode = {"ppt": tdx.MODE_PPT, "pdd": tdx.MODE_PDD, "thomas": tdx.MODE_THOMAS}[args.mode]
+    Ps = tuple(int(v) for v in args.P.split(",")) if args.P else TUNED_P[args.config]
+    bcs = (tdx.BC_DIRICHLET, tdx.BC_DIRICHLET, tdx.BC_PERIODIC)
+    grid = tdx.Grid(cfg.nx, cfg.ny, cfg.nz, *cfg.faces(), bcs=bcs, device=local_rank)
+    kz2 = cfg.kz2()
+
+    # inputs: seeded synthetic, generated once on the host, resident in HBM before the timed region
+    seed_shift = 1000 * rank                                    # every rank solves its own field (weak scaling)
+    host_field = cfg.rhs_field() if rank == 0 else None
+    if rank != 0:
+        from paper_1812_01178_b200 import inputs
+        host_field = inputs.rhs_uniform((cfg.nz, cfg.ny, cfg.nx), cfg.seed + seed_shift)
+    host_helm = cfg.rhs_helmholtz()
+    field0 = torch.from_numpy(host_field).cuda()
+    helm0 = torch.from_numpy(host_helm).cuda()
+    field = field0.clone()
+    helm = helm0.clone()
+    stream = torch.cuda.current_stream().cuda_stream
+
+    def step(ev=None):
+        # in place: re-running on its own output is the same work (same bytes); contraction keeps values bounded
+        for k, d in enumerate((0, 1, 2)):
+            if ev: ev[k].record()
+            grid.adi_sweep(d, mode, Ps[d], cfg.alpha, field, stream)
+        if ev: ev[3].record()
+        grid.helmholtz_wavenumber_solve(mode, Ps[3], None, kz2, helm, stream)
+        if ev: ev[4].record()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+        helm.copy_(helm0)                                       # Helmholtz is not a contraction: restore its rhs
+    barrier()
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(5)] for _ in range(args.steps)]
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    time.sleep(0.25)
+    n0 = tdx.kernel_launch_count()
+    barrier()
+    e0.record()
+    for s in range(args.steps):
+        step(evs[s])
+    e1.record()
+    barrier()
+    launches = tdx.kernel_launch_count() - n0
+    sampler.stop_flag.set()
+    total_ms = e0.elapsed_time(e1)
+    if world > 1:
+        tt = torch.tensor([total_ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        total_ms = float(tt.item())
+    ms_per_step = total_ms / args.steps
+    value = world * step_points(cfg) * args.steps / (total_ms * 1e-3) / 1e9
+
+    # per-kernel durations (CUDA events on the launching stream, inside the timed region)
+    names = ["adi_x", "adi_y", "adi_z_cyclic", "helmholtz_y"]
+    pts = [cfg.npts, cfg.npts, cfg.npts, 2 * cfg.nx * cfg.ny * cfg.nm]
+    kms = [float(np.mean([evs[s][k].elapsed_time(evs[s][k + 1]) for s in range(args.steps)])) for k in range(4)]
+    peak, peak_src = measured_peak()
+    per_kernel = {n: {"ms": kms[k], "gpts_per_s": pts[k] / (kms[k] * 1e-3) / 1e9, "gb_per_s": BYTES_PER_POINT * pts[k] / (kms[k] * 1e-3) / 1e9,
+                      "frac_of_measured_peak": BYTES_PER_POINT * pts[k] / (kms[k] * 1e-3) / 1e9 / peak,
+                      "frac_of_nominal_8TBs": BYTES_PER_POINT * pts[k] / (kms[k] * 1e-3) / 1e9 / 8000.0, "P": Ps[k]} for k, n in enumerate(names)}
+    dom = int(np.argmax(kms))
+    achieved = BYTES_PER_POINT * pts[dom] / (kms[dom] * 1e-3) / 1e9
+    roofline = {"bound": "hbm", "kernel": names[dom], "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "traffic": None, "peak_source": peak_src, "algorithmic_bytes_per_launch": BYTES_PER_POINT * pts[dom],
+                "share_of_step": kms[dom] / sum(kms)}
+
+    out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+           "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+           "data": "synthetic",
+           "config": {"workload": cfg.name, "grid": [cfg.nx, cfg.ny, cfg.nz], "mode": args.mode,
+                      "P": {"x": Ps[0], "y": Ps[1], "z": Ps[2], "helmholtz": Ps[3]}, "alpha": cfg.alpha, "nm": cfg.nm,
+                      "step": "adi x + adi y + adi z (cyclic) + helmholtz y-solves, in place",
+                      "l2": "inputs larger than L2 (%.2f GB field, %.2f GB complex)" % (cfg.npts * 8 / 1e9, cfg.nx * cfg.ny * cfg.nm * 16 / 1e9)
+                      if cfg.npts * 8 > 2 * 126e6 else "L2-resident field: GB/s informational only",
+                      "parallelism": "independent field per GPU, no collective"},
+           "kernels": per_kernel, "roofline": roofline, "gpu_launches": int(launches), "clocks": sampler.summary()}
+
+    # end to end through the host-buffer C-ABI calls: pinned host buffers, H2D + solve + D2H inside the timed region
+    if not args.no_e2e:
+        hf = torch.from_numpy(host_field).pin_memory().numpy()
+        hh = torch.from_numpy(host_helm).pin_memory().numpy()
+        hh0 = host_helm
+        grid.adi_step_host(mode, Ps[0], Ps[1], Ps[2], cfg.alpha, hf)          # warm-up (staging allocation)
+        grid.helmholtz_wavenumber_solve_host(mode, Ps[3], None, kz2, hh)
+        barrier()
+        ts = []
+        for _ in range(max(1, args.e2e_steps)):
+            np.copyto(hh, hh0)
+            barrier()
+            t0 = time.perf_counter()
+            grid.adi_step_host(mode, Ps[0], Ps[1], Ps[2], cfg.alpha, hf)
+            grid.helmholtz_wavenumber_solve_host(mode, Ps[3], None, kz2, hh)
+            torch.cuda.synchronize()
+            ts.append(time.perf_counter() - t0)
+        te = float(np.mean(ts))
+        if world > 1:
+            tt = torch.tensor([te], device="cuda", dtype=torch.float64)
+            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+            te = float(tt.item())
+        out["e2e"] = {"value": world * step_points(cfg) / te / 1e9, "unit": UNIT, "h2d_bytes_per_step": int(hf.nbytes + hh.nbytes),
+                      "d2h_bytes_per_step": int(hf.nbytes + hh.nbytes), "ms_per_step": te * 1e3, "steps": len(ts),
+                      "api": "tdx_adi_step_host + tdx_helmholtz_wavenumber_solve_host (pinned host buffers)"}
+    if rank == 0 and world == 1 and not args.no_cpu:
+        v, _, info = run_oracle_sample(cfg)
+        info["value"] = v
+        info["unit"] = UNIT
+        out["cpu_baseline"] = info
+    grid.close()
+    if rank == 0:
+        print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+    else:
+        run_tdx(args, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()

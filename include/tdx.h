@@ -1,0 +1,111 @@
+/* tdx.h -- C ABI of libtdx.so: B200 (sm_100a) batched tridiagonal line solves along the x, y and z lines of a
+ * 3-D staggered grid by the Parallel Diagonal Dominant (PDD) and Parallel Partition (PPT) methods of
+ * Ha, Park & You, arxiv 1812.01178 (Section 3.2; Algorithm 1), used INSIDE one GPU:
+ * P partitions per line are solved by independent threads, coupled through the reduced interface system Z.
+ *
+ * Conventions (all entry points)
+ *   - fp64 throughout (the paper's precision).
+ *   - Field layout: x fastest, idx(i,j,k) = i + nx*(j + ny*k), 0-based, contiguous, base 16-byte aligned.
+ *     A line along dir has length n_dir and stride 1 (x), nx (y), nx*ny (z).  No transpose is ever made
+ *     (the point of the paper, L51-74).
+ *   - Solves are IN PLACE: the right-hand side is overwritten by the solution.
+ *   - Pointers marked HOST are read during the call and never retained; pointers marked DEVICE must be valid on
+ *     the grid's device and belong to the caller (e.g. torch.Tensor.data_ptr()).  The library never frees them.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  Device entry points are
+ *     asynchronous with respect to the host; plan tables are built on first use on the same stream.
+ *   - Every call returns tdx_status_t.  Argument validation precedes any launch: on an argument error nothing
+ *     is written.  tdx_last_error() gives a thread-local message for the last failure on this thread.
+ *   - There is no CPU fallback and no other backend: without a CUDA device every solve returns TDX_ERR_CUDA.
+ */
+#ifndef TDX_H
+#define TDX_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct tdx_grid tdx_grid_t;                 /* opaque; owns grid metrics and cached plan tables */
+
+typedef enum { TDX_DIR_X = 0, TDX_DIR_Y = 1, TDX_DIR_Z = 2 } tdx_dir_t;
+/* THOMAS: one thread per line, plain Thomas recurrence (GPU baseline; P ignored).
+ * PDD   : PAPER.md L148-154 -- far-end spike entries of Z dropped, 2x2 interface blocks (Alg.1 step 5).
+ * PPT   : PAPER.md L126-146, L156 -- Z solved exactly (to rounding).                                  */
+typedef enum { TDX_MODE_THOMAS = 0, TDX_MODE_PDD = 1, TDX_MODE_PPT = 2 } tdx_mode_t;
+typedef enum { TDX_BC_DIRICHLET = 0, TDX_BC_PERIODIC = 1, TDX_BC_NEUMANN = 2 } tdx_bc_t;
+typedef enum {
+    TDX_OK = 0,
+    TDX_ERR_INVALID_ARG = -1,      /* null pointer, bad enum, non-increasing faces, n < 2 ...            */
+    TDX_ERR_BAD_PARTITION = -2,    /* P < 1, P > TDX_MAX_P or floor(n_dir/P) < 2                          */
+    TDX_ERR_ALLOC = -3,
+    TDX_ERR_CUDA = -4,             /* no device / launch or runtime failure (text in tdx_last_error)      */
+    TDX_ERR_UNSUPPORTED = -5,      /* valid request this build cannot run (e.g. rows per partition > 64)  */
+    TDX_ERR_PDD_BOUND = -6         /* reserved for strict PDD checking                                    */
+} tdx_status_t;
+
+#define TDX_MAX_P 1024             /* partitions per line                                                 */
+#define TDX_MAX_ROWS_PER_PARTITION 64   /* register-resident partition length limit for PDD/PPT          */
+
+/* Create a grid.  xf/yf/zf: HOST arrays of n+1 strictly increasing face coordinates per direction (copied).
+ * Metrics (reading A3): width D_j, centre spacings hm_j, hp_j, mirrored ghost at Dirichlet/Neumann
+ * ends, wrap-around at periodic ends; delta2 u_j = [(u_{j+1}-u_j)/hp_j - (u_j-u_{j-1})/hm_j]/D_j.
+ * device: CUDA ordinal.  On success *out owns device memory until tdx_grid_destroy.                      */
+tdx_status_t tdx_grid_create(int nx, int ny, int nz,
+                             const double* xf, const double* yf, const double* zf,
+                             tdx_bc_t bcx, tdx_bc_t bcy, tdx_bc_t bcz,
+                             int device, tdx_grid_t** out);
+tdx_status_t tdx_grid_destroy(tdx_grid_t* grid);   /* frees plan tables; NULL is accepted                 */
+
+/* Partition map (host, integer only; bit-exact contract, reading A5): q = n/P, r = n%P,
+ * starts[p] = p*q + min(p,r), p = 0..P.  The paper has only m = n/p.
+ * starts: HOST array of P+1 ints.                                                                        */
+tdx_status_t tdx_partition_bounds(int n, int P, int* starts);
+
+/* ADI sweep (Algorithm 1): solve (I - alpha*delta2_dir) x = rhs on every line of
+ * direction dir, in place.  Rows satisfy |b| = |a| + |c| + 1 (L162).  Periodic directions are closed by
+ * Sherman-Morrison (Eq.(3) with a rank-1 update) on top of the chosen mode.
+ * rhs_inout: DEVICE, nx*ny*nz doubles.  P: partitions per line (ignored for THOMAS).                    */
+tdx_status_t tdx_adi_sweep(tdx_grid_t* grid, tdx_dir_t dir, tdx_mode_t mode, int P,
+                           double alpha, double* rhs_inout, void* stream);
+
+/* Poisson y-solves after the spanwise transform: for every wavenumber m < nm and
+ * x-index i solve (delta2_y - lambda) phi = rhs with lambda = kx2[i] + kz2[m] >= 0, Neumann ends;
+ * |b| = |a| + |c| + lambda (L172).  Lines with lambda == 0 exactly are singular and are pinned at j = 0
+ * (b_0 := 1, c_0 := 0, d_0 := 0).  kz2: HOST, nm doubles.  kx2: HOST, nx doubles, or NULL for zeros
+ * (non-NULL kx2 is not built yet: TDX_ERR_UNSUPPORTED).
+ * rhs_inout: DEVICE, complex128 interleaved [nm][ny][nx] (x fastest) = 2*nm*ny*nx doubles; the matrix is
+ * real, so re and im are two right-hand sides of one factorisation.                                       */
+tdx_status_t tdx_helmholtz_wavenumber_solve(tdx_grid_t* grid, tdx_mode_t mode, int P,
+                                            int nm, const double* kx2, const double* kz2,
+                                            double* rhs_inout, void* stream);
+
+/* Batched cyclic tridiagonal solve along dir with caller-given coefficients shared by every line:
+ * a, b, c: HOST arrays of n_dir doubles; a[0] couples row 0 to row n-1 and c[n-1] couples row n-1 to row 0.
+ * Sherman-Morrison closure (gamma = -b[0]) around the chosen mode.  rhs_inout: DEVICE, nx*ny*nz doubles. */
+tdx_status_t tdx_cyclic_solve(tdx_grid_t* grid, tdx_dir_t dir, tdx_mode_t mode, int P,
+                              const double* a, const double* b, const double* c,
+                              double* rhs_inout, void* stream);
+
+/* Same operations on HOST buffers: copy in, solve on the device, copy out, synchronous (returns when the result
+ * is in host memory).  These are the end-to-end calls bench.py times for its "e2e" figure.
+ * tdx_adi_step_host runs the x, y and z sweeps back to back on one upload.                               */
+tdx_status_t tdx_adi_sweep_host(tdx_grid_t* grid, tdx_dir_t dir, tdx_mode_t mode, int P,
+                                double alpha, double* host_rhs_inout);
+tdx_status_t tdx_adi_step_host(tdx_grid_t* grid, tdx_mode_t mode, int Px, int Py, int Pz,
+                               double alpha, double* host_rhs_inout);
+tdx_status_t tdx_helmholtz_wavenumber_solve_host(tdx_grid_t* grid, tdx_mode_t mode, int P,
+                                                 int nm, const double* kx2, const double* kz2,
+                                                 double* host_rhs_inout);
+
+/* Diagnostics.  tdx_pdd_dropped_bound: max over interfaces of |v_last|, |w_first| for the ADI operator of
+ * (dir, P, alpha) -- the entries PDD deletes from Z; the a-priori size of the PDD error.  */
+tdx_status_t tdx_pdd_dropped_bound(tdx_grid_t* grid, tdx_dir_t dir, int P, double alpha, double* out);
+/* Number of kernels this library has launched on this process so far (all grids). */
+long long    tdx_kernel_launch_count(void);
+const char*  tdx_status_string(tdx_status_t status);
+const char*  tdx_last_error(void);                  /* thread-local, static storage; "" when none          */
+const char*  tdx_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TDX_H */

@@ -1,0 +1,152 @@
+"""Thin ctypes binding over csrc/libtdx.so (C ABI in include/tdx.h): argument marshalling ONLY.
+Every step of the path runs in the CUDA kernels behind the C ABI.  PyTorch is used by callers for device memory
+and streams; this module accepts raw device pointers (int) or anything with .data_ptr() (torch tensors).
+Fails loudly (ImportError/RuntimeError) when the library is missing: there is no CPU fallback and this module
+never imports oracle/."""
+import ctypes as C
+import os
+
+import numpy as np
+
+from . import build as _build
+
+DIR_X, DIR_Y, DIR_Z = 0, 1, 2
+MODE_THOMAS, MODE_PDD, MODE_PPT = 0, 1, 2
+BC_DIRICHLET, BC_PERIODIC, BC_NEUMANN = 0, 1, 2
+OK, ERR_INVALID_ARG, ERR_BAD_PARTITION, ERR_ALLOC, ERR_CUDA, ERR_UNSUPPORTED, ERR_PDD_BOUND = 0, -1, -2, -3, -4, -5, -6
+
+EXPORTS = ("tdx_grid_create", "tdx_grid_destroy", "tdx_partition_bounds", "tdx_adi_sweep",
+           "tdx_helmholtz_wavenumber_solve", "tdx_cyclic_solve", "tdx_adi_sweep_host", "tdx_adi_step_host",
+           "tdx_helmholtz_wavenumber_solve_host", "tdx_pdd_dropped_bound", "tdx_kernel_launch_count",
+           "tdx_status_string", "tdx_last_error", "tdx_version")
+
+_dp = C.POINTER(C.c_double)
+_lib = None
+
+
+class TdxError(RuntimeError):
+    def __init__(self, status, msg):
+        super().__init__("%s: %s" % (status_string(status), msg))
+        self.status = status
+
+
+def lib():
+    """Load (building if the sources are newer) csrc/libtdx.so.  Raises if it cannot be had."""
+    global _lib
+    if _lib is None:
+        path = _build.LIB
+        if _build.stale():
+            path = _build.build()
+        if not os.path.exists(path):
+            raise ImportError("libtdx.so missing at %s: the CUDA extension is the only implementation" % path)
+        L = C.CDLL(path)
+        L.tdx_status_string.restype = C.c_char_p
+        L.tdx_last_error.restype = C.c_char_p
+        L.tdx_version.restype = C.c_char_p
+        L.tdx_kernel_launch_count.restype = C.c_longlong
+        L.tdx_grid_create.argtypes = [C.c_int, C.c_int, C.c_int, _dp, _dp, _dp, C.c_int, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_void_p)]
+        L.tdx_grid_destroy.argtypes = [C.c_void_p]
+        L.tdx_partition_bounds.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_int)]
+        L.tdx_adi_sweep.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_double, C.c_void_p, C.c_void_p]
+        L.tdx_helmholtz_wavenumber_solve.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, _dp, _dp, C.c_void_p, C.c_void_p]
+        L.tdx_cyclic_solve.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, _dp, _dp, _dp, C.c_void_p, C.c_void_p]
+        L.tdx_adi_sweep_host.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_double, C.c_void_p]
+        L.tdx_adi_step_host.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_double, C.c_void_p]
+        L.tdx_helmholtz_wavenumber_solve_host.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, _dp, _dp, C.c_void_p]
+        L.tdx_pdd_dropped_bound.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_double, _dp]
+        _lib = L
+    return _lib
+
+
+def status_string(status):
+    return lib().tdx_status_string(C.c_int(status)).decode()
+
+
+def last_error():
+    return lib().tdx_last_error().decode()
+
+
+def version():
+    return lib().tdx_version().decode()
+
+
+def kernel_launch_count():
+    return int(lib().tdx_kernel_launch_count())
+
+
+def _chk(rc):
+    if rc != OK:
+        raise TdxError(rc, last_error())
+
+
+def _host(arr):
+    if arr is None:
+        return None, None
+    a = np.ascontiguousarray(arr, dtype=np.float64)
+    return a, a.ctypes.data_as(_dp)
+
+
+def _devptr(x):
+    return C.c_void_p(int(x.data_ptr()) if hasattr(x, "data_ptr") else int(x))
+
+
+def _hostptr(arr, nbytes):
+    assert isinstance(arr, np.ndarray) and arr.flags.c_contiguous and arr.nbytes == nbytes, "host buffer: C-contiguous, %d bytes" % nbytes
+    return C.c_void_p(arr.ctypes.data)
+
+
+def partition_bounds(n, P):
+    st = (C.c_int * (P + 1))()
+    _chk(lib().tdx_partition_bounds(n, P, st))
+    return np.array(st[:], dtype=np.int32)
+
+
+class Grid:
+    """tdx_grid_create / tdx_grid_destroy.  faces: host arrays of n+1 face coordinates."""
+
+    def __init__(self, nx, ny, nz, xf, yf, zf, bcs=(BC_DIRICHLET, BC_DIRICHLET, BC_PERIODIC), device=0):
+        self.nx, self.ny, self.nz = nx, ny, nz
+        self._h = C.c_void_p()
+        (_, px), (_, py), (_, pz) = _host(xf), _host(yf), _host(zf)
+        assert len(xf) == nx + 1 and len(yf) == ny + 1 and len(zf) == nz + 1
+        _chk(lib().tdx_grid_create(nx, ny, nz, px, py, pz, bcs[0], bcs[1], bcs[2], device, C.byref(self._h)))
+
+    def close(self):
+        if self._h:
+            lib().tdx_grid_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def adi_sweep(self, direction, mode, P, alpha, rhs, stream=0):
+        _chk(lib().tdx_adi_sweep(self._h, direction, mode, P, alpha, _devptr(rhs), C.c_void_p(stream)))
+
+    def helmholtz_wavenumber_solve(self, mode, P, kx2, kz2, rhs, stream=0):
+        kz, pkz = _host(kz2)
+        _, pkx = _host(kx2)
+        _chk(lib().tdx_helmholtz_wavenumber_solve(self._h, mode, P, kz.size, pkx, pkz, _devptr(rhs), C.c_void_p(stream)))
+
+    def cyclic_solve(self, direction, mode, P, a, b, c, rhs, stream=0):
+        (_, pa), (_, pb), (_, pc) = _host(a), _host(b), _host(c)
+        _chk(lib().tdx_cyclic_solve(self._h, direction, mode, P, pa, pb, pc, _devptr(rhs), C.c_void_p(stream)))
+
+    def adi_sweep_host(self, direction, mode, P, alpha, host_rhs):
+        _chk(lib().tdx_adi_sweep_host(self._h, direction, mode, P, alpha, _hostptr(host_rhs, self.nx * self.ny * self.nz * 8)))
+
+    def adi_step_host(self, mode, Px, Py, Pz, alpha, host_rhs):
+        _chk(lib().tdx_adi_step_host(self._h, mode, Px, Py, Pz, alpha, _hostptr(host_rhs, self.nx * self.ny * self.nz * 8)))
+
+    def helmholtz_wavenumber_solve_host(self, mode, P, kx2, kz2, host_rhs):
+        kz, pkz = _host(kz2)
+        _, pkx = _host(kx2)
+        _chk(lib().tdx_helmholtz_wavenumber_solve_host(self._h, mode, P, kz.size, pkx, pkz,
+                                                       _hostptr(host_rhs, self.nx * self.ny * kz.size * 16)))
+
+    def pdd_dropped_bound(self, direction, P, alpha):
+        out = C.c_double(0.0)
+        _chk(lib().tdx_pdd_dropped_bound(self._h, direction, P, alpha, C.byref(out)))
+        return out.value

@@ -1,0 +1,607 @@
+// tdx.cu -- C ABI of libtdx.so (declared in include/tdx.h): argument checks, plan cache, launch selection.
+// All arithmetic of the method runs in the CUDA kernels of tdx_plan.cuh (matrix-only tables, built once per
+// (dir, mode, P, alpha / wavenumbers) on first use) and tdx_kernels.cuh (the per-sweep hot path).
+// There is no CPU fallback: without a device every entry point that needs one returns TDX_ERR_CUDA.
+#include <cuda_runtime.h>
+#include <atomic>
+#include <cstdint>
+#include <cstdio>
+#include <cstring>
+#include <mutex>
+#include <string>
+#include <vector>
+#include <deque>
+#include <cstdarg>
+#include <cmath>
+#include <algorithm>
+
+#include "../../include/tdx.h"
+#include "tdx_kernels.cuh"
+#include "tdx_plan.cuh"
+
+namespace {
+
+thread_local std::string g_last_error;
+std::atomic<long long> g_launches{0};
+
+tdx_status_t fail(tdx_status_t st, const char* fmt, ...) {
+    char buf[512];
+    va_list ap; va_start(ap, fmt); vsnprintf(buf, sizeof buf, fmt, ap); va_end(ap);
+    g_last_error = buf;
+    return st;
+}
+
+#define CUDA_TRY(expr)                                                                                      \
+    do { cudaError_t e_ = (expr);                                                                            \
+         if (e_ != cudaSuccess) return fail(TDX_ERR_CUDA, "%s failed: %s", #expr, cudaGetErrorString(e_)); } while (0)
+#define LAUNCH_CHECK(name)                                                                                  \
+    do { g_launches.fetch_add(1, std::memory_order_relaxed); cudaError_t e_ = cudaGetLastError();            \
+         if (e_ != cudaSuccess) return fail(TDX_ERR_CUDA, "launch of %s failed: %s", name, cudaGetErrorString(e_)); } while (0)
+
+// RAII device scratch (plan build only)
+struct DevBuf {
+    void* p = nullptr;
+    ~DevBuf() { if (p) cudaFree(p); }
+    cudaError_t alloc(size_t bytes) { return cudaMalloc(&p, bytes ? bytes : 8); }
+    template <class T> T* as() { return static_cast<T*>(p); }
+};
+
+enum PlanKind { KIND_ADI = 0, KIND_HELM = 1, KIND_USER = 2 };
+
+struct Plan {
+    int kind = 0, dir = 0, mode = 0, P = 1, n = 0, nsets = 1;
+    int M = 0;              // register rows per partition (kernel instantiation)
+    int layout = tdx::ROWS_PJ;
+    int KB = 0, Scap = 0;
+    bool cyc = false, thomas = false;
+    double alpha = 0.0;
+    uint64_t hash = 0;
+    double dropped = 0.0;   // max |v_last|, |w_first| (what PDD deletes)
+    double *rows = nullptr, *G = nullptr, *Sval = nullptr, *cyc_tab = nullptr;
+    int2* band = nullptr;
+    int *Sidx = nullptr, *Sn = nullptr;
+    void release() {
+        cudaFree(rows); cudaFree(G); cudaFree(Sval); cudaFree(cyc_tab); cudaFree(band); cudaFree(Sidx); cudaFree(Sn);
+        rows = G = Sval = cyc_tab = nullptr; band = nullptr; Sidx = Sn = nullptr;
+    }
+};
+
+const int kMInst[] = {4, 8, 12, 16, 20, 24, 32, 48, 64};
+
+uint64_t fnv1a(const void* data, size_t bytes, uint64_t h = 1469598103934665603ull) {
+    const unsigned char* p = static_cast<const unsigned char*>(data);
+    for (size_t i = 0; i < bytes; ++i) { h ^= p[i]; h *= 1099511628211ull; }
+    return h;
+}
+
+}  // namespace
+
+struct tdx_grid {
+    int nx = 0, ny = 0, nz = 0, device = 0;
+    int bc[3] = {0, 0, 0};
+    double* faces[3] = {nullptr, nullptr, nullptr};     // device copies
+    double* lo[3] = {nullptr, nullptr, nullptr};        // metrics per direction (device)
+    double* up[3] = {nullptr, nullptr, nullptr};
+    double* lo_neumann_y = nullptr;                     // Helmholtz uses Neumann ends in y whatever bcy is
+    double* up_neumann_y = nullptr;
+    std::deque<Plan> plans;            // deque: references stay valid across push_back
+    std::mutex mu;
+    double* stage = nullptr; size_t stage_bytes = 0;    // device staging for the *_host entry points
+    int n_of(int dir) const { return dir == 0 ? nx : (dir == 1 ? ny : nz); }
+};
+
+namespace {
+
+using namespace tdx;
+
+int pick_M(int maxlen) {
+    for (int m : kMInst) if (m >= maxlen) return m;
+    return -1;
+}
+
+// ---- plan construction (all arithmetic on the device) -------------------------------------------------------
+tdx_status_t build_plan(tdx_grid* g, Plan& pl, const double* lambda_host, const double* ua, const double* ub,
+                        const double* uc, cudaStream_t st) {
+    const int n = pl.n, nsets = pl.nsets, P = pl.P;
+    const size_t tot = (size_t)nsets * n;
+    DevBuf a, b, c, flags, lam, qv, work;
+    CUDA_TRY(a.alloc(tot * 8)); CUDA_TRY(b.alloc(tot * 8)); CUDA_TRY(c.alloc(tot * 8));
+    CUDA_TRY(flags.alloc((size_t)nsets * 4));
+    CUDA_TRY(cudaMemsetAsync(flags.p, 0, (size_t)nsets * 4, st));
+    const int tb = 128;
+    if (pl.kind == KIND_ADI) {
+        k_coeffs_adi<<<(n + tb - 1) / tb, tb, 0, st>>>(n, g->lo[pl.dir], g->up[pl.dir], g->bc[pl.dir], pl.alpha,
+                                                       a.as<double>(), b.as<double>(), c.as<double>());
+        LAUNCH_CHECK("k_coeffs_adi");
+    } else if (pl.kind == KIND_HELM) {
+        CUDA_TRY(lam.alloc((size_t)nsets * 8));
+        CUDA_TRY(cudaMemcpyAsync(lam.p, lambda_host, (size_t)nsets * 8, cudaMemcpyHostToDevice, st));
+        dim3 grid((n + tb - 1) / tb, nsets);
+        k_coeffs_helm<<<grid, tb, 0, st>>>(n, nsets, g->lo_neumann_y, g->up_neumann_y, lam.as<double>(),
+                                           a.as<double>(), b.as<double>(), c.as<double>(), flags.as<int>());
+        LAUNCH_CHECK("k_coeffs_helm");
+    } else {
+        CUDA_TRY(cudaMemcpyAsync(a.p, ua, tot * 8, cudaMemcpyHostToDevice, st));
+        CUDA_TRY(cudaMemcpyAsync(b.p, ub, tot * 8, cudaMemcpyHostToDevice, st));
+        CUDA_TRY(cudaMemcpyAsync(c.p, uc, tot * 8, cudaMemcpyHostToDevice, st));
+    }
+    if (pl.cyc) {
+        CUDA_TRY(cudaMalloc(&pl.cyc_tab, (size_t)nsets * 4 * 8));
+        CUDA_TRY(qv.alloc(tot * 8)); CUDA_TRY(work.alloc(tot * 2 * 8));
+        k_cyclic_split<<<(nsets + tb - 1) / tb, tb, 0, st>>>(n, nsets, a.as<double>(), b.as<double>(), c.as<double>(), pl.cyc_tab);
+        LAUNCH_CHECK("k_cyclic_split");
+        k_cyclic_q<<<(nsets + tb - 1) / tb, tb, 0, st>>>(n, nsets, a.as<double>(), b.as<double>(), c.as<double>(), pl.cyc_tab,
+                                                         qv.as<double>(), work.as<double>());
+        LAUNCH_CHECK("k_cyclic_q");
+    }
+    const double* qptr = pl.cyc ? qv.as<double>() : nullptr;
+    if (pl.thomas) {
+        CUDA_TRY(cudaMalloc(&pl.rows, tot * 6 * 8));
+        k_factor_line<<<(nsets + tb - 1) / tb, tb, 0, st>>>(n, nsets, a.as<double>(), b.as<double>(), c.as<double>(), qptr,
+                                                            flags.as<int>(), pl.rows);
+        LAUNCH_CHECK("k_factor_line");
+        CUDA_TRY(cudaStreamSynchronize(st));
+        return TDX_OK;
+    }
+    // partitioned modes
+    pl.layout = ROWS_PJ;
+    if (pl.dir == 0) {
+        pl.layout = ROWS_JP;
+        if (n % P == 0 && P >= 3 && nsets == 1) {
+            DevBuf differs; CUDA_TRY(differs.alloc(4));
+            CUDA_TRY(cudaMemsetAsync(differs.p, 0, 4, st));
+            k_blocks_identical<<<(n + tb - 1) / tb, tb, 0, st>>>(n, P, a.as<double>(), b.as<double>(), c.as<double>(), differs.as<int>());
+            LAUNCH_CHECK("k_blocks_identical");
+            int h = 1;
+            CUDA_TRY(cudaMemcpyAsync(&h, differs.p, 4, cudaMemcpyDeviceToHost, st));
+            CUDA_TRY(cudaStreamSynchronize(st));
+            if (h == 0) pl.layout = ROWS_U;
+        }
+    }
+    const size_t rows_elems = (pl.layout == ROWS_U) ? (size_t)pl.M * 6 : (size_t)nsets * P * pl.M * 6;
+    CUDA_TRY(cudaMalloc(&pl.rows, rows_elems * 8));
+    DevBuf ends; CUDA_TRY(ends.alloc((size_t)nsets * P * 4 * 8));
+    {
+        const int nt = nsets * P;
+        k_factor<TDX_MAX_ROWS_PER_PARTITION><<<(nt + 63) / 64, 64, 0, st>>>(n, nsets, P, pl.M, pl.layout, a.as<double>(), b.as<double>(),
+                                                                            c.as<double>(), qptr, flags.as<int>(), pl.rows, ends.as<double>());
+        LAUNCH_CHECK("k_factor");
+    }
+    pl.KB = (pl.mode == TDX_MODE_PDD) ? 4 : 2 * P;
+    CUDA_TRY(cudaMalloc(&pl.G, (size_t)nsets * 2 * pl.KB * P * 8));
+    CUDA_TRY(cudaMalloc(&pl.band, (size_t)nsets * P * sizeof(int2)));
+    const int ntp = nsets * P;
+    if (pl.mode == TDX_MODE_PDD) {
+        k_pack_pdd<<<(ntp + tb - 1) / tb, tb, 0, st>>>(nsets, P, pl.KB, ends.as<double>(), pl.G, pl.band);
+        LAUNCH_CHECK("k_pack_pdd");
+    } else {
+        const int K = 2 * (P - 1);
+        DevBuf Z, Zi, piv;
+        CUDA_TRY(Z.alloc((size_t)nsets * K * K * 8)); CUDA_TRY(Zi.alloc((size_t)nsets * K * K * 8)); CUDA_TRY(piv.alloc((size_t)nsets * K * 4));
+        k_reduced_factor<<<(nsets + 31) / 32, 32, 0, st>>>(nsets, P, ends.as<double>(), Z.as<double>(), piv.as<int>());
+        LAUNCH_CHECK("k_reduced_factor");
+        const long nk = (long)nsets * K;
+        k_reduced_inverse<<<(unsigned)((nk + 63) / 64), 64, 0, st>>>(nsets, P, Z.as<double>(), piv.as<int>(), Zi.as<double>());
+        LAUNCH_CHECK("k_reduced_inverse");
+        k_pack_ppt<<<(ntp + 63) / 64, 64, 0, st>>>(nsets, P, pl.KB, Zi.as<double>(), pl.G, pl.band);
+        LAUNCH_CHECK("k_pack_ppt");
+        CUDA_TRY(cudaStreamSynchronize(st));
+    }
+    if (pl.cyc) {
+        pl.Scap = 2 + 2 * pl.KB;
+        CUDA_TRY(cudaMalloc(&pl.Sidx, (size_t)nsets * pl.Scap * 4));
+        CUDA_TRY(cudaMalloc(&pl.Sval, (size_t)nsets * pl.Scap * 8));
+        CUDA_TRY(cudaMalloc(&pl.Sn, (size_t)nsets * 4));
+        k_cyclic_functional<<<(nsets + tb - 1) / tb, tb, 0, st>>>(nsets, P, pl.KB, pl.Scap, ends.as<double>(), pl.cyc_tab, pl.G,
+                                                                  pl.band, pl.Sidx, pl.Sval, pl.Sn);
+        LAUNCH_CHECK("k_cyclic_functional");
+    }
+    // a-priori PDD bound (diagnostic): the entries PDD deletes from Z
+    std::vector<double> he((size_t)nsets * P * 4);
+    CUDA_TRY(cudaMemcpyAsync(he.data(), ends.p, he.size() * 8, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    double dr = 0.0;
+    for (int s = 0; s < nsets; ++s)
+        for (int i = 1; i <= P - 1; ++i) {
+            if (i >= 2) dr = std::max(dr, std::fabs(he[((size_t)s * P + i - 1) * 4 + 1]));
+            if (i <= P - 2) dr = std::max(dr, std::fabs(he[((size_t)s * P + i) * 4 + 2]));
+        }
+    pl.dropped = dr;
+    return TDX_OK;
+}
+
+// find or build
+tdx_status_t get_plan(tdx_grid* g, int kind, int dir, int mode, int P, double alpha, int nsets,
+                      const double* lambda_host, const double* ua, const double* ub, const double* uc,
+                      cudaStream_t st, Plan** out) {
+    const int n = (kind == KIND_HELM) ? g->ny : g->n_of(dir);
+    if (n < 2) return fail(TDX_ERR_INVALID_ARG, "line length %d < 2", n);
+    bool thomas = (mode == TDX_MODE_THOMAS) || P == 1;
+    if (mode != TDX_MODE_THOMAS) {
+        if (P < 1 || P > TDX_MAX_P || n / P < 2) return fail(TDX_ERR_BAD_PARTITION, "P=%d invalid for line length %d (need 1 <= P <= %d, floor(n/P) >= 2)", P, n, TDX_MAX_P);
+    }
+    if (thomas) { P = 1; mode = TDX_MODE_THOMAS; }
+    const bool cyc = (kind == KIND_USER) || (kind == KIND_ADI && g->bc[dir] == TDX_BC_PERIODIC);
+    if (cyc && n < 3) return fail(TDX_ERR_INVALID_ARG, "periodic line needs n >= 3");
+    int M = 0;
+    if (!thomas) {
+        const int maxlen = n / P + (n % P ? 1 : 0);
+        M = pick_M(maxlen);
+        if (M < 0) return fail(TDX_ERR_UNSUPPORTED, "rows per partition %d > %d: raise P", maxlen, TDX_MAX_ROWS_PER_PARTITION);
+    }
+    uint64_t h = 0;
+    if (kind == KIND_HELM) h = fnv1a(lambda_host, (size_t)nsets * 8);
+    if (kind == KIND_USER) { h = fnv1a(ua, (size_t)n * 8); h = fnv1a(ub, (size_t)n * 8, h); h = fnv1a(uc, (size_t)n * 8, h); }
+    std::lock_guard<std::mutex> lk(g->mu);
+    for (Plan& p : g->plans)
+        if (p.kind == kind && p.dir == dir && p.mode == mode && p.P == P && p.nsets == nsets && p.hash == h &&
+            std::memcmp(&p.alpha, &alpha, 8) == 0) { *out = &p; return TDX_OK; }
+    Plan pl;
+    pl.kind = kind; pl.dir = dir; pl.mode = mode; pl.P = P; pl.n = n; pl.nsets = nsets; pl.M = M; pl.cyc = cyc;
+    pl.thomas = thomas; pl.alpha = alpha; pl.hash = h;
+    tdx_status_t rc = build_plan(g, pl, lambda_host, ua, ub, uc, st);
+    if (rc != TDX_OK) { pl.release(); return rc; }
+    g->plans.push_back(pl);
+    *out = &g->plans.back();
+    return TDX_OK;
+}
+
+Tables tables_of(const Plan& pl) {
+    Tables T;
+    T.rows = pl.rows; T.G = pl.G; T.band = pl.band; T.Sidx = pl.Sidx; T.Sval = pl.Sval; T.Sn = pl.Sn;
+    T.P = pl.P; T.n = pl.n; T.q = pl.n / pl.P; T.r = pl.n % pl.P; T.KB = pl.KB; T.Scap = pl.Scap;
+    return T;
+}
+
+}  // namespace
+
+// ---- launch selection ---------------------------------------------------------------------------------------
+namespace {
+
+template <int M, int V, bool CYC>
+tdx_status_t launch_strided_inst(const StridedArgs& A, const Tables& T, dim3 grid, dim3 block, size_t smem, cudaStream_t st) {
+    static bool attr_done = false;
+    if (!attr_done && smem > 48 * 1024) {
+        CUDA_TRY(cudaFuncSetAttribute(k_strided<M, V, CYC>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+        attr_done = true;
+    }
+    k_strided<M, V, CYC><<<grid, block, smem, st>>>(A, T);
+    LAUNCH_CHECK("k_strided");
+    return TDX_OK;
+}
+
+template <int V, bool CYC>
+tdx_status_t launch_strided_M(int M, const StridedArgs& A, const Tables& T, dim3 grid, dim3 block, size_t smem, cudaStream_t st) {
+    switch (M) {
+        case 4: return launch_strided_inst<4, V, CYC>(A, T, grid, block, smem, st);
+        case 8: return launch_strided_inst<8, V, CYC>(A, T, grid, block, smem, st);
+        case 12: return launch_strided_inst<12, V, CYC>(A, T, grid, block, smem, st);
+        case 16: return launch_strided_inst<16, V, CYC>(A, T, grid, block, smem, st);
+        case 20: return launch_strided_inst<20, V, CYC>(A, T, grid, block, smem, st);
+        case 24: return launch_strided_inst<24, V, CYC>(A, T, grid, block, smem, st);
+        case 32: return launch_strided_inst<32, V, CYC>(A, T, grid, block, smem, st);
+        case 48: if (V == 1) return launch_strided_inst<48, 1, CYC>(A, T, grid, block, smem, st); break;
+        case 64: if (V == 1) return launch_strided_inst<64, 1, CYC>(A, T, grid, block, smem, st); break;
+    }
+    return fail(TDX_ERR_UNSUPPORTED, "no strided kernel for M=%d V=%d", M, V);
+}
+
+int pow2floor(long long v) { int p = 1; while ((long long)p * 2 <= v) p *= 2; return p; }
+
+// lines of `dir` in a field whose x extent is `nxe` doubles (nx for real fields, 2 nx for complex ones)
+tdx_status_t run_strided(const Plan& pl, double* data, long long W, long long line_stride, long long O,
+                         long long outer_stride, bool set_per_outer, cudaStream_t st) {
+    // W, strides in doubles on entry; use 2 lines per thread (16-byte accesses) when everything is even
+    int V = 1;
+    if (pl.thomas || pl.M <= 32) {
+        if (W % 2 == 0 && line_stride % 2 == 0 && outer_stride % 2 == 0 && (reinterpret_cast<uintptr_t>(data) % 16) == 0) V = 2;
+    }
+    StridedArgs A;
+    A.data = data; A.W = W / V; A.line_stride = line_stride / V; A.outer_stride = outer_stride / V;
+    A.set_per_outer = set_per_outer ? 1 : 0;
+    if (O > 65535) return fail(TDX_ERR_UNSUPPORTED, "outer extent %lld > 65535", O);
+    if (pl.thomas) {
+        const int tb = 128;
+        A.LPC = tb;
+        dim3 grid((unsigned)((A.W + tb - 1) / tb), (unsigned)O);
+        if (V == 2) { if (pl.cyc) k_thomas_strided<2, true><<<grid, tb, 0, st>>>(A, pl.rows, pl.cyc_tab, pl.n); else k_thomas_strided<2, false><<<grid, tb, 0, st>>>(A, pl.rows, pl.cyc_tab, pl.n); }
+        else { if (pl.cyc) k_thomas_strided<1, true><<<grid, tb, 0, st>>>(A, pl.rows, pl.cyc_tab, pl.n); else k_thomas_strided<1, false><<<grid, tb, 0, st>>>(A, pl.rows, pl.cyc_tab, pl.n); }
+        LAUNCH_CHECK("k_thomas_strided");
+        return TDX_OK;
+    }
+    int BT = strided_block_threads(pl.M, V);
+    if (BT < pl.P && V == 2) {                                   // too many partitions for the 2-line variant
+        V = 1; A.W = W; A.line_stride = line_stride; A.outer_stride = outer_stride;
+        BT = strided_block_threads(pl.M, 1);
+    }
+    if (BT < pl.P) return fail(TDX_ERR_UNSUPPORTED, "P=%d partitions of up to %d rows do not fit one thread block", pl.P, pl.M);
+    int LPC = pow2floor(BT / pl.P);
+    if (LPC > 32) LPC = 32;
+    while (LPC > 1 && LPC / 2 >= A.W) LPC /= 2;
+    A.LPC = LPC;
+    dim3 block(LPC, pl.P), grid((unsigned)((A.W + LPC - 1) / LPC), (unsigned)O);
+    const size_t smem = (size_t)2 * pl.P * LPC * V * 8;
+    Tables T = tables_of(pl);
+    if (V == 2) return pl.cyc ? launch_strided_M<2, true>(pl.M, A, T, grid, block, smem, st) : launch_strided_M<2, false>(pl.M, A, T, grid, block, smem, st);
+    return pl.cyc ? launch_strided_M<1, true>(pl.M, A, T, grid, block, smem, st) : launch_strided_M<1, false>(pl.M, A, T, grid, block, smem, st);
+}
+
+template <int M, bool UNI, bool CYC>
+tdx_status_t launch_unit_inst(const UnitArgs& A, const Tables& T, unsigned grid, int threads, size_t smem, cudaStream_t st) {
+    static bool attr_done = false;
+    if (!attr_done) {
+        CUDA_TRY(cudaFuncSetAttribute(k_unit<M, UNI, CYC>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+        attr_done = true;
+    }
+    k_unit<M, UNI, CYC><<<grid, threads, smem, st>>>(A, T);
+    LAUNCH_CHECK("k_unit");
+    return TDX_OK;
+}
+
+template <bool UNI, bool CYC>
+tdx_status_t launch_unit_M(int M, const UnitArgs& A, const Tables& T, unsigned grid, int threads, size_t smem, cudaStream_t st) {
+    switch (M) {
+        case 4: return launch_unit_inst<4, UNI, CYC>(A, T, grid, threads, smem, st);
+        case 8: return launch_unit_inst<8, UNI, CYC>(A, T, grid, threads, smem, st);
+        case 12: return launch_unit_inst<12, UNI, CYC>(A, T, grid, threads, smem, st);
+        case 16: return launch_unit_inst<16, UNI, CYC>(A, T, grid, threads, smem, st);
+        case 20: return launch_unit_inst<20, UNI, CYC>(A, T, grid, threads, smem, st);
+        case 24: return launch_unit_inst<24, UNI, CYC>(A, T, grid, threads, smem, st);
+        case 32: return launch_unit_inst<32, UNI, CYC>(A, T, grid, threads, smem, st);
+        case 48: return launch_unit_inst<48, UNI, CYC>(A, T, grid, threads, smem, st);
+        case 64: return launch_unit_inst<64, UNI, CYC>(A, T, grid, threads, smem, st);
+    }
+    return fail(TDX_ERR_UNSUPPORTED, "no unit-stride kernel for M=%d", M);
+}
+
+int unit_bt(int M) { return M <= 8 ? 1024 : (M <= 24 ? 512 : 256); }
+
+tdx_status_t run_unit(const Plan& pl, double* data, long long nlines, cudaStream_t st) {
+    if (pl.thomas) {
+        const int tb = 128;
+        unsigned grid = (unsigned)((nlines + tb - 1) / tb);
+        if (pl.cyc) k_thomas_unit<true><<<grid, tb, 0, st>>>(data, nlines, pl.rows, pl.cyc_tab, pl.n);
+        else k_thomas_unit<false><<<grid, tb, 0, st>>>(data, nlines, pl.rows, pl.cyc_tab, pl.n);
+        LAUNCH_CHECK("k_thomas_unit");
+        return TDX_OK;
+    }
+    const int BT = unit_bt(pl.M);
+    if (pl.P > BT) return fail(TDX_ERR_UNSUPPORTED, "P=%d partitions of up to %d rows do not fit one thread block", pl.P, pl.M);
+    UnitArgs A;
+    A.data = data; A.nlines = nlines;
+    int target = BT < 256 ? BT : 256;
+    A.LPB = std::max(1, target / pl.P);
+    if (A.LPB > nlines) A.LPB = (int)nlines;
+    const int q = pl.n / pl.P;
+    A.pad_en = (q % 2 == 0) ? 1 : 0;
+    A.inv20 = ((1u << 20) + q - 1) / q;
+    const int threads = ((A.LPB * pl.P + 31) / 32) * 32;
+    const int nwarps = threads / 32;
+    const size_t smem = ((size_t)nwarps * (32 * pl.M + 48) + 2 * (size_t)threads) * 8;
+    const unsigned grid = (unsigned)((nlines + A.LPB - 1) / A.LPB);
+    Tables T = tables_of(pl);
+    const bool uni = pl.layout == ROWS_U;
+    if (uni) return pl.cyc ? launch_unit_M<true, true>(pl.M, A, T, grid, threads, smem, st) : launch_unit_M<true, false>(pl.M, A, T, grid, threads, smem, st);
+    return pl.cyc ? launch_unit_M<false, true>(pl.M, A, T, grid, threads, smem, st) : launch_unit_M<false, false>(pl.M, A, T, grid, threads, smem, st);
+}
+
+tdx_status_t run_sweep(tdx_grid* g, const Plan& pl, int dir, double* data, cudaStream_t st) {
+    const long long nx = g->nx, ny = g->ny, nz = g->nz;
+    if (dir == 0) return run_unit(pl, data, ny * nz, st);
+    if (dir == 1) return run_strided(pl, data, nx, nx, nz, nx * ny, false, st);
+    return run_strided(pl, data, nx * ny, nx * ny, 1, 0, false, st);
+}
+
+tdx_status_t check_common(tdx_grid* g, int dir, int mode, const void* ptr) {
+    if (!g) return fail(TDX_ERR_INVALID_ARG, "grid is NULL");
+    if (dir < 0 || dir > 2) return fail(TDX_ERR_INVALID_ARG, "dir=%d not in {0,1,2}", dir);
+    if (mode < 0 || mode > 2) return fail(TDX_ERR_INVALID_ARG, "mode=%d not in {0,1,2}", mode);
+    if (!ptr) return fail(TDX_ERR_INVALID_ARG, "data pointer is NULL");
+    return TDX_OK;
+}
+
+}  // namespace
+
+// ---- C ABI ---------------------------------------------------------------------------------------------------
+extern "C" {
+
+const char* tdx_version(void) { return "tdx 0.1 (sm_100a)"; }
+const char* tdx_last_error(void) { return g_last_error.c_str(); }
+long long tdx_kernel_launch_count(void) { return g_launches.load(); }
+
+const char* tdx_status_string(tdx_status_t s) {
+    switch (s) {
+        case TDX_OK: return "TDX_OK";
+        case TDX_ERR_INVALID_ARG: return "TDX_ERR_INVALID_ARG";
+        case TDX_ERR_BAD_PARTITION: return "TDX_ERR_BAD_PARTITION";
+        case TDX_ERR_ALLOC: return "TDX_ERR_ALLOC";
+        case TDX_ERR_CUDA: return "TDX_ERR_CUDA";
+        case TDX_ERR_UNSUPPORTED: return "TDX_ERR_UNSUPPORTED";
+        case TDX_ERR_PDD_BOUND: return "TDX_ERR_PDD_BOUND";
+    }
+    return "TDX_ERR_UNKNOWN";
+}
+
+tdx_status_t tdx_partition_bounds(int n, int P, int* starts) {
+    if (!starts) return fail(TDX_ERR_INVALID_ARG, "starts is NULL");
+    if (n < 2) return fail(TDX_ERR_INVALID_ARG, "n=%d < 2", n);
+    if (P < 1 || P > TDX_MAX_P || n / P < 2) return fail(TDX_ERR_BAD_PARTITION, "P=%d invalid for n=%d", P, n);
+    const int q = n / P, r = n % P;
+    for (int p = 0; p <= P; ++p) starts[p] = tdx::part_start(p, q, r);
+    return TDX_OK;
+}
+
+tdx_status_t tdx_grid_create(int nx, int ny, int nz, const double* xf, const double* yf, const double* zf,
+                             tdx_bc_t bcx, tdx_bc_t bcy, tdx_bc_t bcz, int device, tdx_grid_t** out) {
+    if (!out) return fail(TDX_ERR_INVALID_ARG, "out is NULL");
+    *out = nullptr;
+    if (nx < 2 || ny < 2 || nz < 2) return fail(TDX_ERR_INVALID_ARG, "grid %dx%dx%d: every extent must be >= 2", nx, ny, nz);
+    if (!xf || !yf || !zf) return fail(TDX_ERR_INVALID_ARG, "face array is NULL");
+    const int bcs[3] = {(int)bcx, (int)bcy, (int)bcz};
+    const double* fs[3] = {xf, yf, zf};
+    const int ns[3] = {nx, ny, nz};
+    for (int d = 0; d < 3; ++d) {
+        if (bcs[d] < 0 || bcs[d] > 2) return fail(TDX_ERR_INVALID_ARG, "bc[%d]=%d not in {0,1,2}", d, bcs[d]);
+        for (int j = 0; j < ns[d]; ++j)
+            if (!(fs[d][j + 1] > fs[d][j])) return fail(TDX_ERR_INVALID_ARG, "faces of direction %d not strictly increasing at %d", d, j);
+    }
+    int ndev = 0;
+    cudaError_t e = cudaGetDeviceCount(&ndev);
+    if (e != cudaSuccess || ndev == 0) { cudaGetLastError(); return fail(TDX_ERR_CUDA, "no CUDA device: %s (tdx has no CPU fallback)", cudaGetErrorString(e)); }
+    if (device < 0 || device >= ndev) return fail(TDX_ERR_INVALID_ARG, "device %d not in [0,%d)", device, ndev);
+    CUDA_TRY(cudaSetDevice(device));
+    tdx_grid* g = new (std::nothrow) tdx_grid();
+    if (!g) return fail(TDX_ERR_ALLOC, "host allocation failed");
+    g->nx = nx; g->ny = ny; g->nz = nz; g->device = device;
+    auto bail = [&](tdx_status_t st) { tdx_grid_destroy(g); return st; };
+    for (int d = 0; d < 3; ++d) {
+        g->bc[d] = bcs[d];
+        const int n = ns[d];
+        if (cudaMalloc(&g->faces[d], (size_t)(n + 1) * 8) != cudaSuccess || cudaMalloc(&g->lo[d], (size_t)n * 8) != cudaSuccess ||
+            cudaMalloc(&g->up[d], (size_t)n * 8) != cudaSuccess) return bail(fail(TDX_ERR_ALLOC, "device allocation failed"));
+        if (cudaMemcpy(g->faces[d], fs[d], (size_t)(n + 1) * 8, cudaMemcpyHostToDevice) != cudaSuccess) return bail(fail(TDX_ERR_CUDA, "face upload failed"));
+        tdx::k_metrics<<<(n + 127) / 128, 128>>>(n, g->faces[d], bcs[d], g->lo[d], g->up[d]);
+        g_launches.fetch_add(1);
+    }
+    if (cudaMalloc(&g->lo_neumann_y, (size_t)ny * 8) != cudaSuccess || cudaMalloc(&g->up_neumann_y, (size_t)ny * 8) != cudaSuccess)
+        return bail(fail(TDX_ERR_ALLOC, "device allocation failed"));
+    tdx::k_metrics<<<(ny + 127) / 128, 128>>>(ny, g->faces[1], TDX_BC_NEUMANN, g->lo_neumann_y, g->up_neumann_y);
+    g_launches.fetch_add(1);
+    e = cudaDeviceSynchronize();
+    if (e != cudaSuccess) return bail(fail(TDX_ERR_CUDA, "metrics kernel failed: %s", cudaGetErrorString(e)));
+    *out = g;
+    return TDX_OK;
+}
+
+tdx_status_t tdx_grid_destroy(tdx_grid_t* g) {
+    if (!g) return TDX_OK;
+    cudaSetDevice(g->device);
+    for (Plan& p : g->plans) p.release();
+    for (int d = 0; d < 3; ++d) { cudaFree(g->faces[d]); cudaFree(g->lo[d]); cudaFree(g->up[d]); }
+    cudaFree(g->lo_neumann_y); cudaFree(g->up_neumann_y); cudaFree(g->stage);
+    delete g;
+    return TDX_OK;
+}
+
+tdx_status_t tdx_adi_sweep(tdx_grid_t* g, tdx_dir_t dir, tdx_mode_t mode, int P, double alpha, double* rhs, void* stream) {
+    tdx_status_t rc = check_common(g, dir, mode, rhs);
+    if (rc != TDX_OK) return rc;
+    if (!(alpha == alpha)) return fail(TDX_ERR_INVALID_ARG, "alpha is NaN");
+    CUDA_TRY(cudaSetDevice(g->device));
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    Plan* pl = nullptr;
+    rc = get_plan(g, KIND_ADI, dir, mode, P, alpha, 1, nullptr, nullptr, nullptr, nullptr, st, &pl);
+    if (rc != TDX_OK) return rc;
+    return run_sweep(g, *pl, dir, rhs, st);
+}
+
+tdx_status_t tdx_cyclic_solve(tdx_grid_t* g, tdx_dir_t dir, tdx_mode_t mode, int P, const double* a, const double* b,
+                              const double* c, double* rhs, void* stream) {
+    tdx_status_t rc = check_common(g, dir, mode, rhs);
+    if (rc != TDX_OK) return rc;
+    if (!a || !b || !c) return fail(TDX_ERR_INVALID_ARG, "coefficient array is NULL");
+    CUDA_TRY(cudaSetDevice(g->device));
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    Plan* pl = nullptr;
+    rc = get_plan(g, KIND_USER, dir, mode, P, 0.0, 1, nullptr, a, b, c, st, &pl);
+    if (rc != TDX_OK) return rc;
+    return run_sweep(g, *pl, dir, rhs, st);
+}
+
+tdx_status_t tdx_helmholtz_wavenumber_solve(tdx_grid_t* g, tdx_mode_t mode, int P, int nm, const double* kx2,
+                                            const double* kz2, double* rhs, void* stream) {
+    tdx_status_t rc = check_common(g, TDX_DIR_Y, mode, rhs);
+    if (rc != TDX_OK) return rc;
+    if (nm < 1 || !kz2) return fail(TDX_ERR_INVALID_ARG, "nm=%d / kz2 invalid", nm);
+    for (int m = 0; m < nm; ++m) if (!(kz2[m] >= 0.0)) return fail(TDX_ERR_INVALID_ARG, "kz2[%d] is negative or NaN", m);
+    if (kx2) {
+        bool any = false;
+        for (int i = 0; i < g->nx; ++i) { if (!(kx2[i] >= 0.0)) return fail(TDX_ERR_INVALID_ARG, "kx2[%d] is negative or NaN", i); any |= kx2[i] != 0.0; }
+        if (any) return fail(TDX_ERR_UNSUPPORTED, "non-zero kx2 (per-line matrices) is not built yet");
+    }
+    CUDA_TRY(cudaSetDevice(g->device));
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    Plan* pl = nullptr;
+    rc = get_plan(g, KIND_HELM, TDX_DIR_Y, mode, P, 0.0, nm, kz2, nullptr, nullptr, nullptr, st, &pl);
+    if (rc != TDX_OK) return rc;
+    const long long nx2 = 2LL * g->nx;      // complex interleaved: 2 nx doubles per row, re/im share the matrix
+    return run_strided(*pl, rhs, nx2, nx2, nm, nx2 * g->ny, true, st);
+}
+
+tdx_status_t tdx_pdd_dropped_bound(tdx_grid_t* g, tdx_dir_t dir, int P, double alpha, double* out) {
+    if (!g || !out) return fail(TDX_ERR_INVALID_ARG, "NULL argument");
+    if (dir < 0 || dir > 2) return fail(TDX_ERR_INVALID_ARG, "dir=%d", dir);
+    CUDA_TRY(cudaSetDevice(g->device));
+    Plan* pl = nullptr;
+    tdx_status_t rc = get_plan(g, KIND_ADI, dir, TDX_MODE_PDD, P, alpha, 1, nullptr, nullptr, nullptr, nullptr, 0, &pl);
+    if (rc != TDX_OK) return rc;
+    *out = pl->dropped;
+    return TDX_OK;
+}
+
+// ---- host-buffer entry points (end-to-end: H2D + solve + D2H, synchronous) ----------------------------------
+static tdx_status_t ensure_stage(tdx_grid* g, size_t bytes) {
+    if (g->stage_bytes >= bytes) return TDX_OK;
+    cudaFree(g->stage); g->stage = nullptr; g->stage_bytes = 0;
+    if (cudaMalloc(&g->stage, bytes) != cudaSuccess) { cudaGetLastError(); return fail(TDX_ERR_ALLOC, "staging allocation of %zu bytes failed", bytes); }
+    g->stage_bytes = bytes;
+    return TDX_OK;
+}
+
+tdx_status_t tdx_adi_step_host(tdx_grid_t* g, tdx_mode_t mode, int Px, int Py, int Pz, double alpha, double* host) {
+    tdx_status_t rc = check_common(g, 0, mode, host);
+    if (rc != TDX_OK) return rc;
+    CUDA_TRY(cudaSetDevice(g->device));
+    const size_t bytes = (size_t)g->nx * g->ny * g->nz * 8;
+    const int Ps[3] = {Px, Py, Pz};
+    Plan* pls[3];
+    for (int d = 0; d < 3; ++d) {                       // validate everything before any copy
+        rc = get_plan(g, KIND_ADI, d, mode, Ps[d], alpha, 1, nullptr, nullptr, nullptr, nullptr, 0, &pls[d]);
+        if (rc != TDX_OK) return rc;
+    }
+    rc = ensure_stage(g, bytes);
+    if (rc != TDX_OK) return rc;
+    CUDA_TRY(cudaMemcpyAsync(g->stage, host, bytes, cudaMemcpyHostToDevice, 0));
+    for (int d = 0; d < 3; ++d) { rc = run_sweep(g, *pls[d], d, g->stage, 0); if (rc != TDX_OK) return rc; }
+    CUDA_TRY(cudaMemcpyAsync(host, g->stage, bytes, cudaMemcpyDeviceToHost, 0));
+    CUDA_TRY(cudaStreamSynchronize(0));
+    return TDX_OK;
+}
+
+tdx_status_t tdx_adi_sweep_host(tdx_grid_t* g, tdx_dir_t dir, tdx_mode_t mode, int P, double alpha, double* host) {
+    tdx_status_t rc = check_common(g, dir, mode, host);
+    if (rc != TDX_OK) return rc;
+    CUDA_TRY(cudaSetDevice(g->device));
+    const size_t bytes = (size_t)g->nx * g->ny * g->nz * 8;
+    Plan* pl = nullptr;
+    rc = get_plan(g, KIND_ADI, dir, mode, P, alpha, 1, nullptr, nullptr, nullptr, nullptr, 0, &pl);
+    if (rc != TDX_OK) return rc;
+    rc = ensure_stage(g, bytes);
+    if (rc != TDX_OK) return rc;
+    CUDA_TRY(cudaMemcpyAsync(g->stage, host, bytes, cudaMemcpyHostToDevice, 0));
+    rc = run_sweep(g, *pl, dir, g->stage, 0);
+    if (rc != TDX_OK) return rc;
+    CUDA_TRY(cudaMemcpyAsync(host, g->stage, bytes, cudaMemcpyDeviceToHost, 0));
+    CUDA_TRY(cudaStreamSynchronize(0));
+    return TDX_OK;
+}
+
+tdx_status_t tdx_helmholtz_wavenumber_solve_host(tdx_grid_t* g, tdx_mode_t mode, int P, int nm, const double* kx2,
+                                                 const double* kz2, double* host) {
+    tdx_status_t rc = check_common(g, TDX_DIR_Y, mode, host);
+    if (rc != TDX_OK) return rc;
+    if (nm < 1) return fail(TDX_ERR_INVALID_ARG, "nm=%d", nm);
+    CUDA_TRY(cudaSetDevice(g->device));
+    const size_t bytes = (size_t)g->nx * g->ny * nm * 16;
+    rc = ensure_stage(g, bytes);
+    if (rc != TDX_OK) return rc;
+    // validation happens inside the device entry point before any launch; upload first is harmless (staging only)
+    CUDA_TRY(cudaMemcpyAsync(g->stage, host, bytes, cudaMemcpyHostToDevice, 0));
+    rc = tdx_helmholtz_wavenumber_solve(g, mode, P, nm, kx2, kz2, g->stage, 0);
+    if (rc != TDX_OK) return rc;
+    CUDA_TRY(cudaMemcpyAsync(host, g->stage, bytes, cudaMemcpyDeviceToHost, 0));
+    CUDA_TRY(cudaStreamSynchronize(0));
+    return TDX_OK;
+}
+
+}  // extern "C"

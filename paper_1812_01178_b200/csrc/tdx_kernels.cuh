@@ -1,0 +1,320 @@
+// tdx_kernels.cuh -- the hot path: one launch per sweep, 8 B read + 8 B written per grid value.
+//
+//   k_strided<MAXM,V,CYC>  y / z sweeps and the Helmholtz y-solves: thread = (line, partition), a warp holds
+//                          consecutive lines of ONE partition, so every global access is a coalesced row segment and
+//                          the plan tables are warp-uniform.  Each thread keeps its partition (<= MAXM rows, V lines)
+//                          in registers: forward + backward elimination (Eq.(5)), interface values to shared memory,
+//                          reduced system (Eq.(7); PDD 2x2 blocks or PPT banded Z^{-1} rows), correction (Eq.(8)),
+//                          Sherman-Morrison closure for periodic lines -- then one coalesced store.
+//   k_unit<MAXM,UNI,CYC>   x sweeps (unit-stride lines): thread = partition, consecutive partitions in consecutive
+//                          lanes; a warp's 32 partitions are one contiguous chunk of memory which is loaded coalesced,
+//                          transposed through a padded per-warp shared-memory tile, and stored back the same way --
+//                          no global transpose (PAPER.md:L51-74 is what the method removes).
+//   k_thomas_strided / k_thomas_unit   mode THOMAS: one thread per line, plain recurrence, in place (GPU baseline).
+//
+// PAPER.md references: Eq.(5)-(8) L104-124, PDD L148-154, PPT L126-146/L156, Algorithm 1 steps 3,5,7 L240-258.
+#pragma once
+#include <cuda_runtime.h>
+#include "tdx_plan.cuh"
+
+namespace tdx {
+
+struct Tables {
+    const double* rows;      // row table (layout depends on the kernel), fields {l, inv, cp, v, w, q}
+    const double* G;         // reduced coefficients G[((set*2+side)*KB + k)*P + p]
+    const int2* band;        // band[set*P + p] = {lo, cnt} in interface-rhs indices r[0..2P)
+    const int* Sidx;         // cyclic closure functional (sparse), Sidx/Sval[set*Scap + k], Sn[set]
+    const double* Sval;
+    const int* Sn;
+    int P, n, q, r, KB, Scap;
+};
+
+struct StridedArgs {
+    double* data;            // base of the field (doubles)
+    long long W;             // lines per outer index, in V-vectors
+    long long line_stride;   // distance between consecutive rows of a line, in V-vectors
+    long long outer_stride;  // distance between outer indices, in V-vectors
+    int set_per_outer;       // 1: table set = outer index (Helmholtz wavenumber), 0: one set
+    int LPC;                 // lines (V-vectors) per CTA = blockDim.x
+};
+
+template <int V> struct VecIO;
+template <> struct VecIO<1> {
+    __device__ static inline void ld(const double* p, double (&x)[1]) { x[0] = __ldcs(p); }
+    __device__ static inline void st(double* p, const double (&x)[1]) { __stcs(p, x[0]); }
+};
+template <> struct VecIO<2> {
+    __device__ static inline void ld(const double* p, double (&x)[2]) { double2 t = __ldcs(reinterpret_cast<const double2*>(p)); x[0] = t.x; x[1] = t.y; }
+    __device__ static inline void st(double* p, const double (&x)[2]) { __stcs(reinterpret_cast<double2*>(p), make_double2(x[0], x[1])); }
+};
+
+constexpr int strided_block_threads(int MAXM, int V) { return (2 * MAXM * V <= 24) ? 1024 : ((2 * MAXM * V <= 64) ? 512 : 256); }
+
+template <int MAXM, int V, bool CYC>
+__global__ void __launch_bounds__(strided_block_threads(MAXM, V))
+k_strided(StridedArgs A, Tables T) {
+    extern __shared__ double rs[];                          // rs[(idx*LPC + tx)*V + v], idx in [0, 2P)
+    const int tx = threadIdx.x, p = threadIdx.y;
+    const int LPC = A.LPC, P = T.P;
+    const long long i = (long long)blockIdx.x * LPC + tx;
+    const bool valid = i < A.W;
+    const int o = blockIdx.y;
+    const int set = A.set_per_outer ? o : 0;
+    const int start = part_start(p, T.q, T.r);
+    const int m = T.q + (p < T.r ? 1 : 0);
+    double* base = A.data + ((long long)o * A.outer_stride + (long long)start * A.line_stride + i) * V;
+    const long long rstride = A.line_stride * V;
+
+    double x[MAXM][V];
+#pragma unroll
+    for (int jj = 0; jj < MAXM; ++jj) {
+        if (valid && jj < m) VecIO<V>::ld(base + jj * rstride, x[jj]);
+        else {
+#pragma unroll
+            for (int v = 0; v < V; ++v) x[jj][v] = 0.0;
+        }
+    }
+    const double2* rt = reinterpret_cast<const double2*>(T.rows + ((size_t)((size_t)set * P + p) * MAXM) * 6);
+
+    // Eq.(5): forward y_j = d_j - l_j y_{j-1}, backward xt_j = y_j inv_j - cp_j xt_{j+1}
+#pragma unroll
+    for (int jj = 1; jj < MAXM; ++jj) {
+        const double l = __ldg(&rt[jj * 3 + 0]).x;
+#pragma unroll
+        for (int v = 0; v < V; ++v) x[jj][v] = fma(-l, x[jj - 1][v], x[jj][v]);
+    }
+    {
+        const double inv = __ldg(&rt[(MAXM - 1) * 3 + 0]).y;
+#pragma unroll
+        for (int v = 0; v < V; ++v) x[MAXM - 1][v] *= inv;
+    }
+#pragma unroll
+    for (int jj = MAXM - 2; jj >= 0; --jj) {
+        const double inv = __ldg(&rt[jj * 3 + 0]).y;
+        const double cp = __ldg(&rt[jj * 3 + 1]).x;
+#pragma unroll
+        for (int v = 0; v < V; ++v) x[jj][v] = fma(-cp, x[jj + 1][v], x[jj][v] * inv);
+    }
+    // E^T xt: first and last row of this partition
+#pragma unroll
+    for (int v = 0; v < V; ++v) {
+        double xl = x[MAXM - 1][v];
+#pragma unroll
+        for (int jj = 0; jj < MAXM - 1; ++jj) if (jj == m - 1) xl = x[jj][v];
+        rs[((2 * p) * LPC + tx) * V + v] = x[0][v];
+        rs[((2 * p + 1) * LPC + tx) * V + v] = xl;
+    }
+    __syncthreads();
+    // Eq.(7): the two interface unknowns this partition needs
+    double yL[V], yR[V], sc[V];
+#pragma unroll
+    for (int v = 0; v < V; ++v) { yL[v] = 0.0; yR[v] = 0.0; sc[v] = 0.0; }
+    {
+        const int2 bd = __ldg(&T.band[set * P + p]);
+        const double* gl = T.G + ((size_t)(set * 2 + 0) * T.KB) * P + p;
+        const double* gr = T.G + ((size_t)(set * 2 + 1) * T.KB) * P + p;
+        for (int k = 0; k < bd.y; ++k) {
+            const double a = __ldg(gl + (size_t)k * P), b = __ldg(gr + (size_t)k * P);
+#pragma unroll
+            for (int v = 0; v < V; ++v) {
+                const double rv = rs[((bd.x + k) * LPC + tx) * V + v];
+                yL[v] = fma(a, rv, yL[v]);
+                yR[v] = fma(b, rv, yR[v]);
+            }
+        }
+        if (CYC) {
+            const int ns = __ldg(&T.Sn[set]);
+            for (int k = 0; k < ns; ++k) {
+                const int idx = __ldg(&T.Sidx[(size_t)set * T.Scap + k]);
+                const double sv = __ldg(&T.Sval[(size_t)set * T.Scap + k]);
+#pragma unroll
+                for (int v = 0; v < V; ++v) sc[v] = fma(sv, rs[(idx * LPC + tx) * V + v], sc[v]);
+            }
+        }
+    }
+    // Eq.(8): x = xt - v yL - w yR (- q s for periodic lines), then store
+#pragma unroll
+    for (int jj = 0; jj < MAXM; ++jj) {
+        const double2 t1 = __ldg(&rt[jj * 3 + 1]);          // {cp, v}
+        const double2 t2 = __ldg(&rt[jj * 3 + 2]);          // {w, q}
+#pragma unroll
+        for (int v = 0; v < V; ++v) {
+            double r = fma(-t1.y, yL[v], x[jj][v]);
+            r = fma(-t2.x, yR[v], r);
+            if (CYC) r = fma(-t2.y, sc[v], r);
+            x[jj][v] = r;
+        }
+        if (valid && jj < m) VecIO<V>::st(base + jj * rstride, x[jj]);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+struct UnitArgs {
+    double* data;
+    long long nlines;
+    int LPB;                 // whole lines per CTA
+    int pad_en;              // pad the per-warp tile (partition length even)
+    unsigned inv20;          // ceil(2^20 / q) for the pad index
+};
+
+template <int MAXM> constexpr int unit_block_threads() { return MAXM <= 8 ? 1024 : (MAXM <= 24 ? 512 : 256); }
+
+template <int MAXM, bool UNI, bool CYC>
+__global__ void __launch_bounds__(unit_block_threads<MAXM>())
+k_unit(UnitArgs A, Tables T) {
+    extern __shared__ double sm[];
+    const int P = T.P, n = T.n;
+    const int tl = threadIdx.x, lane = tl & 31, warp = tl >> 5;
+    const int nthreads_real = A.LPB * P;
+    const int nwarps = blockDim.x >> 5;
+    constexpr int WT = 32 * MAXM + 48;                                 // per-warp tile capacity (doubles)
+    double* tile = sm + (size_t)warp * WT;
+    double* rf = sm + (size_t)nwarps * WT;                              // xt_first per thread
+    double* rl = rf + blockDim.x;                                       // xt_last per thread
+
+    const long long line0 = (long long)blockIdx.x * A.LPB;
+    long long lines_here = A.nlines - line0; if (lines_here > A.LPB) lines_here = A.LPB;
+    const int ll = tl / P, p = tl - ll * P;
+    const bool valid = tl < nthreads_real && ll < lines_here;
+    const int m = valid ? T.q + (p < T.r ? 1 : 0) : 0;
+    const int cta_end = (int)lines_here * n;
+    const int S = valid ? ll * n + part_start(p, T.q, T.r) : cta_end;   // element offset in the CTA chunk
+    const int e0 = __shfl_sync(0xffffffffu, S, 0);
+    const int e1 = __shfl_sync(0xffffffffu, S + m, 31);
+    const int count = e1 - e0;
+    double* gptr = A.data + line0 * n + e0;
+    auto padi = [&](int e) -> int { return A.pad_en ? e + (int)(((unsigned)e * A.inv20) >> 20) : e; };
+
+    double x[MAXM];
+#pragma unroll
+    for (int k = 0; k < MAXM; ++k) { const int e = k * 32 + lane; x[k] = (e < count) ? __ldcs(gptr + e) : 0.0; }
+#pragma unroll
+    for (int k = 0; k < MAXM; ++k) { const int e = k * 32 + lane; if (e < count) tile[padi(e)] = x[k]; }
+    __syncwarp();
+    const int off = S - e0;
+#pragma unroll
+    for (int jj = 0; jj < MAXM; ++jj) x[jj] = (jj < m) ? tile[padi(off + jj)] : 0.0;
+
+    // table access: UNI -> one table for every partition (warp-uniform), else per-partition columns (coalesced)
+    const double* rows = T.rows;
+    auto tab = [&](int jj, int f) -> double {
+        if (UNI) return __ldg(rows + jj * 6 + f);
+        return __ldg(rows + ((size_t)jj * 6 + f) * P + (valid ? p : 0));
+    };
+#pragma unroll
+    for (int jj = 1; jj < MAXM; ++jj) x[jj] = fma(-tab(jj, F_L), x[jj - 1], x[jj]);
+    x[MAXM - 1] *= tab(MAXM - 1, F_INV);
+#pragma unroll
+    for (int jj = MAXM - 2; jj >= 0; --jj) x[jj] = fma(-tab(jj, F_CP), x[jj + 1], x[jj] * tab(jj, F_INV));
+    {
+        double xl = x[MAXM - 1];
+#pragma unroll
+        for (int jj = 0; jj < MAXM - 1; ++jj) if (jj == m - 1) xl = x[jj];
+        rf[tl] = x[0]; rl[tl] = xl;
+    }
+    __syncthreads();
+    double yL = 0.0, yR = 0.0, sc = 0.0;
+    if (valid) {
+        const int2 bd = __ldg(&T.band[p]);
+        const double* gl = T.G + p;
+        const double* gr = T.G + (size_t)T.KB * P + p;
+        const int lb = ll * P;
+        for (int k = 0; k < bd.y; ++k) {
+            const int idx = bd.x + k;
+            const double rv = (idx & 1) ? rl[lb + (idx >> 1)] : rf[lb + (idx >> 1)];
+            yL = fma(__ldg(gl + (size_t)k * P), rv, yL);
+            yR = fma(__ldg(gr + (size_t)k * P), rv, yR);
+        }
+        if (CYC) {
+            const int ns = __ldg(&T.Sn[0]);
+            for (int k = 0; k < ns; ++k) {
+                const int idx = __ldg(&T.Sidx[k]);
+                const double rv = (idx & 1) ? rl[lb + (idx >> 1)] : rf[lb + (idx >> 1)];
+                sc = fma(__ldg(&T.Sval[k]), rv, sc);
+            }
+        }
+    }
+#pragma unroll
+    for (int jj = 0; jj < MAXM; ++jj) {
+        double r = fma(-tab(jj, F_V), yL, x[jj]);
+        r = fma(-tab(jj, F_W), yR, r);
+        if (CYC) r = fma(-tab(jj, F_Q), sc, r);
+        if (jj < m) tile[padi(off + jj)] = r;
+    }
+    __syncwarp();
+#pragma unroll
+    for (int k = 0; k < MAXM; ++k) { const int e = k * 32 + lane; if (e < count) __stcs(gptr + e, tile[padi(e)]); }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// THOMAS mode: one thread per line, in place in global memory (forward pass stores y, backward pass re-reads it).
+// rows[(set*n + j)*6 + f].  cyc[set*4 + {0:g, 3:kappa}] for periodic lines.
+template <int V, bool CYC>
+__global__ void k_thomas_strided(StridedArgs A, const double* __restrict__ rows, const double* __restrict__ cyc, int n) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= A.W) return;
+    const int o = blockIdx.y;
+    const int set = A.set_per_outer ? o : 0;
+    double* base = A.data + ((long long)o * A.outer_stride + i) * V;
+    const long long rstride = A.line_stride * V;
+    const double* rt = rows + (size_t)set * n * 6;
+    double prev[V], cur[V];
+#pragma unroll
+    for (int v = 0; v < V; ++v) prev[v] = 0.0;
+    for (int j = 0; j < n; ++j) {
+        const double l = __ldg(rt + (size_t)j * 6 + F_L);
+        VecIO<V>::ld(base + j * rstride, cur);
+#pragma unroll
+        for (int v = 0; v < V; ++v) { cur[v] = fma(-l, prev[v], cur[v]); prev[v] = cur[v]; }
+        VecIO<V>::st(base + j * rstride, cur);
+    }
+    double ylast[V];
+#pragma unroll
+    for (int v = 0; v < V; ++v) prev[v] = 0.0;
+    for (int j = n - 1; j >= 0; --j) {
+        const double inv = __ldg(rt + (size_t)j * 6 + F_INV), cp = __ldg(rt + (size_t)j * 6 + F_CP);
+        VecIO<V>::ld(base + j * rstride, cur);
+#pragma unroll
+        for (int v = 0; v < V; ++v) { cur[v] = fma(-cp, prev[v], cur[v] * inv); prev[v] = cur[v]; if (j == n - 1) ylast[v] = cur[v]; }
+        VecIO<V>::st(base + j * rstride, cur);
+    }
+    if (CYC) {
+        const double g = __ldg(cyc + set * 4 + 0), kappa = __ldg(cyc + set * 4 + 3);
+        double s[V];
+#pragma unroll
+        for (int v = 0; v < V; ++v) s[v] = kappa * fma(g, ylast[v], prev[v]);     // prev = y_0 after the backward pass
+        for (int j = 0; j < n; ++j) {
+            const double qj = __ldg(rt + (size_t)j * 6 + F_Q);
+            VecIO<V>::ld(base + j * rstride, cur);
+#pragma unroll
+            for (int v = 0; v < V; ++v) cur[v] = fma(-qj, s[v], cur[v]);
+            VecIO<V>::st(base + j * rstride, cur);
+        }
+    }
+}
+
+template <bool CYC>
+__global__ void k_thomas_unit(double* __restrict__ data, long long nlines, const double* __restrict__ rows,
+                              const double* __restrict__ cyc, int n) {
+    const long long line = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (line >= nlines) return;
+    double* base = data + line * n;
+    double prev = 0.0;
+    for (int j = 0; j < n; ++j) {
+        const double cur = fma(-__ldg(rows + (size_t)j * 6 + F_L), prev, base[j]);
+        base[j] = cur; prev = cur;
+    }
+    prev = 0.0;
+    double ylast = 0.0;
+    for (int j = n - 1; j >= 0; --j) {
+        const double cur = fma(-__ldg(rows + (size_t)j * 6 + F_CP), prev, base[j] * __ldg(rows + (size_t)j * 6 + F_INV));
+        base[j] = cur; prev = cur;
+        if (j == n - 1) ylast = cur;
+    }
+    if (CYC) {
+        const double s = __ldg(cyc + 3) * fma(__ldg(cyc + 0), ylast, prev);
+        for (int j = 0; j < n; ++j) base[j] = fma(-__ldg(rows + (size_t)j * 6 + F_Q), s, base[j]);
+    }
+}
+
+}  // namespace tdx

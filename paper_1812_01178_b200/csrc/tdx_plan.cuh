@@ -1,0 +1,378 @@
+// tdx_plan.cuh -- plan-time CUDA kernels: everything that depends on the MATRIX only.
+//
+//   k_metrics            grid faces -> lo_j, up_j of the second difference             (hot-path row a1)
+//   k_coeffs_adi/helm    metrics, alpha / lambda -> a_j, b_j, c_j on the fly           (a1)
+//   k_cyclic_split       Sherman-Morrison split of a periodic line (Eq.(3), rank 1)    (a5)
+//   k_cyclic_q           q = A'^{-1} u, kappa = 1/(1+q_0+g q_{n-1})                    (a5)
+//   k_factor             per partition: LU factors of the block A_p (Alg.1 step 2: a_first, c_last zeroed) and the
+//                        spikes v = A_p^{-1}(a_first e_first), w = A_p^{-1}(c_last e_last) (Eq.(6))  (a2, matrix part)
+//   k_reduced_factor / k_reduced_inverse / k_pack_ppt / k_pack_pdd
+//                        Z = I + E^T A~^{-1} V (L112-116) -> the rows of Z^{-1} each partition needs, truncated where
+//                        they are below fp64 visibility (PPT, L156), or the explicit 2x2 block inverses (PDD, L148-154)
+//   k_cyclic_functional  the linear functional r -> s of the Sherman-Morrison closure
+//
+// The spikes and Z are the same for every line of a sweep (the matrix is shared), so -- unlike Algorithm 1, which
+// carries V as 2 extra right-hand sides per line (R(9M), L228-231) -- they are computed once per (dir, mode, P, alpha).
+// Tables are O(n_dir) (ADI) or O(ny * nmodes) (Helmholtz) and stay L2/L1 resident.
+#pragma once
+#include <cuda_runtime.h>
+#include <math.h>
+
+namespace tdx {
+
+enum RowLayout { ROWS_PJ = 0,      // rows[((set*P + p)*M + jj)*6 + f]   strided kernels (p is warp-uniform) and Thomas (P=1)
+                 ROWS_JP = 1,      // rows[((set*M + jj)*6 + f)*P + p]   unit-stride kernel, partitions differ per lane
+                 ROWS_U = 2 };     // rows[jj*6 + f]                     unit-stride kernel, all partitions identical
+enum RowField { F_L = 0, F_INV = 1, F_CP = 2, F_V = 3, F_W = 4, F_Q = 5 };
+
+__host__ __device__ inline int part_start(int p, int q, int r) { return p * q + (p < r ? p : r); }
+
+__device__ inline size_t row_index(int layout, int set, int P, int M, int p, int jj, int f) {
+    if (layout == ROWS_PJ) return ((size_t)((size_t)set * P + p) * M + jj) * 6 + f;
+    if (layout == ROWS_JP) return (((size_t)set * M + jj) * 6 + f) * P + p;
+    return (size_t)jj * 6 + f;
+}
+
+// ---- a1: metrics (reading A3) ---------------------------------------------------------------------
+__global__ void k_metrics(int n, const double* __restrict__ f, int bc, double* __restrict__ lo, double* __restrict__ up) {
+    int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= n) return;
+    double D = f[j + 1] - f[j];
+    double hper = 0.5 * ((f[1] - f[0]) + (f[n] - f[n - 1]));
+    double hm = (j > 0) ? 0.5 * (f[j] + f[j + 1]) - 0.5 * (f[j - 1] + f[j]) : (bc == 1 ? hper : D);
+    double hp = (j < n - 1) ? 0.5 * (f[j + 1] + f[j + 2]) - 0.5 * (f[j] + f[j + 1]) : (bc == 1 ? hper : D);
+    lo[j] = 1.0 / (hm * D);
+    up[j] = 1.0 / (hp * D);
+}
+
+// ---- a1: ADI rows  a = -alpha lo, c = -alpha up, b = 1 - a - c  (|b| = |a|+|c|+1) -------------
+__global__ void k_coeffs_adi(int n, const double* __restrict__ lo, const double* __restrict__ up, int bc, double alpha,
+                             double* __restrict__ a, double* __restrict__ b, double* __restrict__ c) {
+    int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= n) return;
+    double aj = -alpha * lo[j], cj = -alpha * up[j];
+    double bj = __dsub_rn(__dsub_rn(1.0, aj), cj);
+    if (bc == 0) { if (j == 0) aj = 0.0; if (j == n - 1) cj = 0.0; }                 // Dirichlet: ghost coupling dropped
+    if (bc == 2) {                                                                    // Neumann: ghost folds into b
+        if (j == 0) { bj = __dsub_rn(1.0, cj); aj = 0.0; }
+        if (j == n - 1) { bj = __dsub_rn(1.0, aj); cj = 0.0; }
+    }
+    a[j] = aj; b[j] = bj; c[j] = cj;
+}
+
+// ---- a1: Helmholtz rows a = lo, c = up, b = -(a+c) - lambda, Neumann ends, lambda==0 pinned ---
+// one set per wavenumber; flags[set] = 1 when pinned
+__global__ void k_coeffs_helm(int n, int nsets, const double* __restrict__ lo, const double* __restrict__ up,
+                              const double* __restrict__ lambda, double* __restrict__ a, double* __restrict__ b,
+                              double* __restrict__ c, int* __restrict__ flags) {
+    int j = blockIdx.x * blockDim.x + threadIdx.x;
+    int s = blockIdx.y;
+    if (j >= n || s >= nsets) return;
+    double lam = lambda[s];
+    double aj = lo[j], cj = up[j];
+    double bj = __dsub_rn(-__dadd_rn(aj, cj), lam);
+    if (j == 0) { bj = __dsub_rn(-cj, lam); aj = 0.0; }
+    if (j == n - 1) { bj = __dsub_rn(-aj, lam); cj = 0.0; }
+    if (lam == 0.0 && j == 0) { bj = 1.0; cj = 0.0; flags[s] = 1; }
+    size_t o = (size_t)s * n + j;
+    a[o] = aj; b[o] = bj; c[o] = cj;
+}
+
+// ---- a5: Sherman-Morrison split of a periodic line. cyc[set*4 + {0:g, 1:u0, 2:un, 3:kappa}] ------------------
+__global__ void k_cyclic_split(int n, int nsets, double* __restrict__ a, double* __restrict__ b, double* __restrict__ c,
+                               double* __restrict__ cyc) {
+    int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= nsets) return;
+    double* as = a + (size_t)s * n; double* bs = b + (size_t)s * n; double* cs = c + (size_t)s * n;
+    double gamma = -bs[0];
+    double g = as[0] / gamma;
+    cyc[s * 4 + 0] = g; cyc[s * 4 + 1] = gamma; cyc[s * 4 + 2] = cs[n - 1];
+    bs[0] = __dsub_rn(bs[0], gamma);
+    bs[n - 1] = __dsub_rn(bs[n - 1], __dmul_rn(cs[n - 1], g));
+    as[0] = 0.0; cs[n - 1] = 0.0;
+}
+
+// q = A'^{-1} u by the Thomas recurrence, one thread per set (matrix only, O(n), plan time). work: 2n per set.
+__global__ void k_cyclic_q(int n, int nsets, const double* __restrict__ a, const double* __restrict__ b,
+                           const double* __restrict__ c, double* __restrict__ cyc, double* __restrict__ qv,
+                           double* __restrict__ work) {
+    int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= nsets) return;
+    const double* as = a + (size_t)s * n; const double* bs = b + (size_t)s * n; const double* cs = c + (size_t)s * n;
+    double* cp = work + (size_t)s * 2 * n; double* dp = cp + n; double* q = qv + (size_t)s * n;
+    double u0 = cyc[s * 4 + 1], un = cyc[s * 4 + 2], g = cyc[s * 4 + 0];
+    cp[0] = cs[0] / bs[0]; dp[0] = u0 / bs[0];
+    for (int j = 1; j < n; ++j) {
+        double den = bs[j] - as[j] * cp[j - 1];
+        cp[j] = cs[j] / den;
+        double uj = (j == n - 1) ? un : 0.0;
+        dp[j] = (uj - as[j] * dp[j - 1]) / den;
+    }
+    q[n - 1] = dp[n - 1];
+    for (int j = n - 2; j >= 0; --j) q[j] = dp[j] - cp[j] * q[j + 1];
+    cyc[s * 4 + 3] = 1.0 / (1.0 + q[0] + g * q[n - 1]);
+}
+
+// ---- a2 (matrix part): block factors and spikes. One thread per (set, partition). --------------------------
+// Forward y_j = d_j - l_j y_{j-1};  backward x_j = y_j inv_j - cp_j x_{j+1}  (Thomas with plan-time pivots).
+// ends[(set*P+p)*4 + {0:v_first, 1:v_last, 2:w_first, 3:w_last}].  M = padded rows per partition (identity rows).
+// pinned sets (flags): d_0 := 0 is encoded as inv_0 := 0, l_1 := 0.
+template <int MAXROWS>
+__global__ void k_factor(int n, int nsets, int P, int M, int layout,
+                         const double* __restrict__ a, const double* __restrict__ b, const double* __restrict__ c,
+                         const double* __restrict__ qv, const int* __restrict__ flags,
+                         double* __restrict__ rows, double* __restrict__ ends) {
+    int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= nsets * P) return;
+    int s = t / P, p = t % P;
+    int q = n / P, r = n % P;
+    int st = part_start(p, q, r), m = q + (p < r ? 1 : 0);
+    const double* as = a + (size_t)s * n + st; const double* bs = b + (size_t)s * n + st; const double* cs = c + (size_t)s * n + st;
+    bool pinned = flags && flags[s] && p == 0;
+    // ROWS_U (needs P >= 3): partition 1 has both neighbours and writes the one shared table; every partition still
+    // reports its own spike ends, and the reduced tables zero the side a boundary partition does not have.
+    bool uniform_only = (layout == ROWS_U);
+    bool writer = !uniform_only || (s == 0 && p == 1);
+    double inv[MAXROWS], cp[MAXROWS], l[MAXROWS];
+    double den = bs[0];
+    inv[0] = 1.0 / den; l[0] = 0.0;
+    cp[0] = (m > 1) ? cs[0] * inv[0] : 0.0;
+    for (int j = 1; j < m; ++j) {
+        l[j] = as[j] * inv[j - 1];
+        den = bs[j] - as[j] * cp[j - 1];
+        inv[j] = 1.0 / den;
+        cp[j] = (j < m - 1) ? cs[j] * inv[j] : 0.0;
+    }
+    // spikes (Eq.(6)); for a uniform table the representative partition keeps both spikes, G zeroes the unused side
+    double v[MAXROWS], w[MAXROWS];
+    bool has_v = (p > 0) || uniform_only, has_w = (p < P - 1) || uniform_only;
+    if (P == 1) { has_v = has_w = false; }
+    {   // v: rhs a_first e_first
+        double y = has_v ? as[0] : 0.0;
+        v[0] = y;
+        for (int j = 1; j < m; ++j) { y = -l[j] * y; v[j] = y; }
+        v[m - 1] = v[m - 1] * inv[m - 1];
+        for (int j = m - 2; j >= 0; --j) v[j] = v[j] * inv[j] - cp[j] * v[j + 1];
+        // w: rhs c_last e_last
+        w[m - 1] = has_w ? cs[m - 1] * inv[m - 1] : 0.0;
+        for (int j = m - 2; j >= 0; --j) w[j] = -cp[j] * w[j + 1];
+    }
+    if (pinned) { inv[0] = 0.0; if (m > 1) l[1] = 0.0; }
+    double* e = ends + (size_t)t * 4;
+    e[0] = (p > 0) ? v[0] : 0.0; e[1] = (p > 0) ? v[m - 1] : 0.0;
+    e[2] = (p < P - 1) ? w[0] : 0.0; e[3] = (p < P - 1) ? w[m - 1] : 0.0;
+    if (P == 1) { e[0] = e[1] = e[2] = e[3] = 0.0; }
+    if (!writer) return;
+    for (int jj = 0; jj < M; ++jj) {
+        bool real = jj < m;
+        rows[row_index(layout, s, P, M, p, jj, F_L)] = real ? l[jj] : 0.0;
+        rows[row_index(layout, s, P, M, p, jj, F_INV)] = real ? inv[jj] : 1.0;
+        rows[row_index(layout, s, P, M, p, jj, F_CP)] = real ? cp[jj] : 0.0;
+        rows[row_index(layout, s, P, M, p, jj, F_V)] = real ? v[jj] : 0.0;
+        rows[row_index(layout, s, P, M, p, jj, F_W)] = real ? w[jj] : 0.0;
+        rows[row_index(layout, s, P, M, p, jj, F_Q)] = (real && qv) ? qv[(size_t)s * n + st + jj] : 0.0;
+    }
+}
+
+// Thomas-mode table (P = 1, any n): rows[(set*n + j)*6 + f], one thread per set, no local arrays.
+__global__ void k_factor_line(int n, int nsets, const double* __restrict__ a, const double* __restrict__ b,
+                              const double* __restrict__ c, const double* __restrict__ qv, const int* __restrict__ flags,
+                              double* __restrict__ rows) {
+    int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= nsets) return;
+    const double* as = a + (size_t)s * n; const double* bs = b + (size_t)s * n; const double* cs = c + (size_t)s * n;
+    double* rt = rows + (size_t)s * n * 6;
+    bool pinned = flags && flags[s];
+    double inv_prev = 1.0 / bs[0], cp_prev = (n > 1) ? cs[0] * inv_prev : 0.0;
+    rt[F_L] = 0.0; rt[F_INV] = pinned ? 0.0 : inv_prev; rt[F_CP] = cp_prev; rt[F_V] = 0.0; rt[F_W] = 0.0;
+    rt[F_Q] = qv ? qv[(size_t)s * n] : 0.0;
+    for (int j = 1; j < n; ++j) {
+        double lj = as[j] * inv_prev;
+        double den = bs[j] - as[j] * cp_prev;
+        double invj = 1.0 / den;
+        double cpj = (j < n - 1) ? cs[j] * invj : 0.0;
+        double* rj = rt + (size_t)j * 6;
+        rj[F_L] = (pinned && j == 1) ? 0.0 : lj; rj[F_INV] = invj; rj[F_CP] = cpj; rj[F_V] = 0.0; rj[F_W] = 0.0;
+        rj[F_Q] = qv ? qv[(size_t)s * n + j] : 0.0;
+        inv_prev = invj; cp_prev = cpj;
+    }
+}
+
+// ---- uniformity test for the unit-stride fast path: are all partitions' (a,b,c) blocks bitwise identical? ----
+__global__ void k_blocks_identical(int n, int P, const double* __restrict__ a, const double* __restrict__ b,
+                                   const double* __restrict__ c, int* __restrict__ differs) {
+    int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= n) return;
+    int m = n / P;                       // only called when n % P == 0
+    int p = j / m, jj = j % m;
+    if (p == 0) return;
+    bool first = (jj == 0), last = (jj == m - 1);
+    // a_first and c_last are zeroed inside every block (Alg.1 step 2), so they do not take part in the comparison
+    bool same = (b[j] == b[jj]) && (first || a[j] == a[jj]) && (last || c[j] == c[jj]);
+    // the spikes' right-hand sides: a_first of p>=1 blocks and c_last of p<=P-2 blocks must agree among themselves
+    if (first && p > 1 && a[j] != a[m]) same = false;
+    if (last && p < P - 1 && c[j] != c[m - 1]) same = false;
+    if (!same) atomicExch(differs, 1);
+}
+
+// ---- a3 (matrix part): reduced system Z ------------------------------------------------
+// Unknown order u_{2i-2} = x_{last_{i-1}}, u_{2i-1} = x_{first_i}, i = 1..P-1 (the paper's y_{2i-1}, y_{2i}); K = 2(P-1).
+//   row 2i-2:  v_last^(i-1) u_{2i-4} + u_{2i-2} + w_last^(i-1) u_{2i-1}  = xt_{last_{i-1}}
+//   row 2i-1:  v_first^(i)  u_{2i-2} + u_{2i-1} + w_first^(i)  u_{2i+1}  = xt_{first_i}
+// Z is stored dense (K x K per set, row-major) but only the band |row-col| <= 2 (4 above the diagonal after row
+// interchanges) is ever touched.  Paper-silent point (reading A7): Z is solved in natural order with
+// partial pivoting, never as the permuted Z-bar whose diagonal is the small spike ends.
+__global__ void k_reduced_factor(int nsets, int P, const double* __restrict__ ends, double* __restrict__ Z, int* __restrict__ piv) {
+    int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= nsets) return;
+    int K = 2 * (P - 1);
+    double* z = Z + (size_t)s * K * K;
+    int* pv = piv + (size_t)s * K;
+    const double* e = ends + (size_t)s * P * 4;
+    for (int rr = 0; rr < K; ++rr) {                        // clear the band that will be used
+        int c0 = rr - 2 < 0 ? 0 : rr - 2, c1 = rr + 5 > K ? K : rr + 5;
+        for (int cc = c0; cc < c1; ++cc) z[(size_t)rr * K + cc] = 0.0;
+    }
+    for (int i = 1; i <= P - 1; ++i) {
+        int r1 = 2 * i - 2, r2 = 2 * i - 1;
+        z[(size_t)r1 * K + r1] = 1.0; z[(size_t)r2 * K + r2] = 1.0;
+        z[(size_t)r1 * K + r2] = e[(i - 1) * 4 + 3];                     // w_last^(i-1)
+        z[(size_t)r2 * K + r1] = e[i * 4 + 0];                           // v_first^(i)
+        if (i >= 2) z[(size_t)r1 * K + r1 - 2] = e[(i - 1) * 4 + 1];     // v_last^(i-1)
+        if (i <= P - 2) z[(size_t)r2 * K + r2 + 2] = e[i * 4 + 2];       // w_first^(i)
+    }
+    for (int k = 0; k < K; ++k) {                           // banded LU, partial pivoting, multipliers left in place
+        int last = k + 2 < K - 1 ? k + 2 : K - 1;
+        int pr = k; double best = fabs(z[(size_t)k * K + k]);
+        for (int i = k + 1; i <= last; ++i) { double t = fabs(z[(size_t)i * K + k]); if (t > best) { best = t; pr = i; } }
+        pv[k] = pr;
+        int c1 = k + 5 > K ? K : k + 5;
+        if (pr != k) for (int cc = k; cc < c1; ++cc) { double t = z[(size_t)k * K + cc]; z[(size_t)k * K + cc] = z[(size_t)pr * K + cc]; z[(size_t)pr * K + cc] = t; }
+        double d = z[(size_t)k * K + k];
+        for (int i = k + 1; i <= last; ++i) {
+            double f = z[(size_t)i * K + k] / d;
+            z[(size_t)i * K + k] = f;
+            if (f != 0.0) for (int cc = k + 1; cc < c1; ++cc) z[(size_t)i * K + cc] -= f * z[(size_t)k * K + cc];
+        }
+    }
+}
+
+// column col of Z^{-1}: one thread per (set, col); Zi dense K x K per set, row-major.
+__global__ void k_reduced_inverse(int nsets, int P, const double* __restrict__ Z, const int* __restrict__ piv, double* __restrict__ Zi) {
+    int K = 2 * (P - 1);
+    long t = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= (long)nsets * K) return;
+    int s = (int)(t / K), col = (int)(t % K);
+    const double* z = Z + (size_t)s * K * K;
+    const int* pv = piv + (size_t)s * K;
+    double* x = Zi + (size_t)s * K * K;                      // column col, stride K
+    for (int i = 0; i < K; ++i) x[(size_t)i * K + col] = (i == col) ? 1.0 : 0.0;
+    for (int k = 0; k < K; ++k) {                            // L^{-1} P
+        int pr = pv[k];
+        if (pr != k) { double tmp = x[(size_t)k * K + col]; x[(size_t)k * K + col] = x[(size_t)pr * K + col]; x[(size_t)pr * K + col] = tmp; }
+        double xk = x[(size_t)k * K + col];
+        int last = k + 2 < K - 1 ? k + 2 : K - 1;
+        if (xk != 0.0) for (int i = k + 1; i <= last; ++i) x[(size_t)i * K + col] -= z[(size_t)i * K + k] * xk;
+    }
+    for (int i = K - 1; i >= 0; --i) {                       // U^{-1}
+        double acc = x[(size_t)i * K + col];
+        int c1 = i + 5 > K ? K : i + 5;
+        for (int cc = i + 1; cc < c1; ++cc) acc -= z[(size_t)i * K + cc] * x[(size_t)cc * K + col];
+        x[(size_t)i * K + col] = acc / z[(size_t)i * K + i];
+    }
+}
+
+// Interface right-hand sides live in r[0..2P): r[2p] = xt_first^(p), r[2p+1] = xt_last^(p); Z column k <-> r[k+1].
+// Partition p needs yL = x_{last_{p-1}} = u_{2p-2} (p >= 1) and yR = x_{first_{p+1}} = u_{2p+1} (p <= P-2).
+// G[((set*2+side)*KB + k)*P + p], band[(set*P+p)] = {lo (r index), cnt}: yL = sum_k G[0][k] r[lo+k], yR likewise.
+// PPT: rows of Z^{-1}, entries below tau * rowmax dropped (invisible in fp64), union band of the two rows.
+__global__ void k_pack_ppt(int nsets, int P, int KB, const double* __restrict__ Zi, double* __restrict__ G, int2* __restrict__ band) {
+    int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= nsets * P) return;
+    int s = t / P, p = t % P;
+    int K = 2 * (P - 1);
+    const double* zi = Zi + (size_t)s * K * K;
+    const double tau = 1e-24;
+    int rowL = (p >= 1) ? 2 * p - 2 : -1, rowR = (p <= P - 2) ? 2 * p + 1 : -1;
+    int lo = K, hi = -1;
+    for (int side = 0; side < 2; ++side) {
+        int rr = side ? rowR : rowL;
+        if (rr < 0) continue;
+        double mx = 0.0;
+        for (int cc = 0; cc < K; ++cc) mx = fmax(mx, fabs(zi[(size_t)rr * K + cc]));
+        for (int cc = 0; cc < K; ++cc) if (fabs(zi[(size_t)rr * K + cc]) > tau * mx) { if (cc < lo) lo = cc; if (cc > hi) hi = cc; }
+    }
+    int cnt = hi >= lo ? hi - lo + 1 : 0;
+    band[t] = make_int2(cnt ? lo + 1 : 0, cnt);
+    for (int k = 0; k < KB; ++k) {
+        double gl = 0.0, gr = 0.0;
+        if (k < cnt) {
+            if (rowL >= 0) gl = zi[(size_t)rowL * K + lo + k];
+            if (rowR >= 0) gr = zi[(size_t)rowR * K + lo + k];
+        }
+        G[((size_t)(s * 2 + 0) * KB + k) * P + p] = gl;
+        G[((size_t)(s * 2 + 1) * KB + k) * P + p] = gr;
+    }
+}
+
+// PDD (Alg.1 step 5): interface i block [[1, w_last^(i-1)],[v_first^(i), 1]] inverted explicitly:
+//   y_{2i-1} = (xt_last^(i-1) - w_last^(i-1) xt_first^(i))/det,  y_{2i} = (xt_first^(i) - v_first^(i) xt_last^(i-1))/det.
+// band of partition p: r[2p-1 .. 2p+2].
+__global__ void k_pack_pdd(int nsets, int P, int KB, const double* __restrict__ ends, double* __restrict__ G, int2* __restrict__ band) {
+    int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= nsets * P) return;
+    int s = t / P, p = t % P;
+    const double* e = ends + (size_t)s * P * 4;
+    double g[2][4] = {{0, 0, 0, 0}, {0, 0, 0, 0}};          // over r[2p-1], r[2p], r[2p+1], r[2p+2]
+    if (p >= 1) {                                           // interface i = p: yL = y_{2i-1}
+        double wl = e[(p - 1) * 4 + 3], vf = e[p * 4 + 0];
+        double det = 1.0 - wl * vf;
+        g[0][0] = 1.0 / det; g[0][1] = -wl / det;
+    }
+    if (p <= P - 2) {                                       // interface i = p+1: yR = y_{2i}
+        double wl = e[p * 4 + 3], vf = e[(p + 1) * 4 + 0];
+        double det = 1.0 - wl * vf;
+        g[1][2] = -vf / det; g[1][3] = 1.0 / det;
+    }
+    int lo = 2 * p - 1, k0 = 0, k1 = 4;
+    if (p == 0) k0 = 2;
+    if (p == P - 1) k1 = 2;
+    band[t] = make_int2(lo + k0, k1 - k0);
+    for (int k = 0; k < KB; ++k) {
+        double gl = 0.0, gr = 0.0;
+        if (k < k1 - k0) { gl = g[0][k0 + k]; gr = g[1][k0 + k]; }
+        G[((size_t)(s * 2 + 0) * KB + k) * P + p] = gl;
+        G[((size_t)(s * 2 + 1) * KB + k) * P + p] = gr;
+    }
+}
+
+// a5: the Sherman-Morrison scalar s = kappa (y_0 + g y_{n-1}) as a sparse linear functional of r, where y is the
+// partitioned solution of A' y = d:  y_0 = r[0] - w_first^(0) yR_0,  y_{n-1} = r[2P-1] - v_last^(P-1) yL_{P-1}.
+// Sidx/Sval[set*Scap + k], Sn[set]; Scap >= 2 + 2*KB.
+__global__ void k_cyclic_functional(int nsets, int P, int KB, int Scap, const double* __restrict__ ends,
+                                    const double* __restrict__ cyc, const double* __restrict__ G, const int2* __restrict__ band,
+                                    int* __restrict__ Sidx, double* __restrict__ Sval, int* __restrict__ Sn) {
+    int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= nsets) return;
+    const double* e = ends + (size_t)s * P * 4;
+    double g = cyc[s * 4 + 0], kappa = cyc[s * 4 + 3];
+    int* si = Sidx + (size_t)s * Scap; double* sv = Sval + (size_t)s * Scap;
+    int n = 0;
+    si[n] = 0; sv[n] = kappa; ++n;
+    si[n] = 2 * P - 1; sv[n] = kappa * g; ++n;
+    if (P > 1) {
+        double wf0 = e[0 * 4 + 2], vlP = e[(P - 1) * 4 + 1];
+        int2 b0 = band[s * P + 0], bP = band[s * P + P - 1];
+        for (int k = 0; k < b0.y; ++k) {
+            double gv = G[((size_t)(s * 2 + 1) * KB + k) * P + 0];
+            if (gv != 0.0) { si[n] = b0.x + k; sv[n] = -kappa * wf0 * gv; ++n; }
+        }
+        for (int k = 0; k < bP.y; ++k) {
+            double gv = G[((size_t)(s * 2 + 0) * KB + k) * P + (P - 1)];
+            if (gv != 0.0) { si[n] = bP.x + k; sv[n] = -kappa * g * vlP * gv; ++n; }
+        }
+    }
+    Sn[s] = n;
+}
+
+}  // namespace tdx

@@ -1,0 +1,144 @@
+"""GPU: bit-exact layout / partition indexing, error paths of the C ABI, cyclic_solve, host entry points."""
+import numpy as np
+import pytest
+import torch
+
+import oracle as orc
+from paper_1812_01178_b200 import binding as tdx
+from paper_1812_01178_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+BCS = (tdx.BC_DIRICHLET, tdx.BC_DIRICHLET, tdx.BC_PERIODIC)
+
+
+def relerr(x, ref):
+    return float(np.max(np.abs(x - ref)) / np.max(np.abs(ref)))
+
+
+@pytest.fixture(scope="module")
+def small():
+    nx, ny, nz = 64, 36, 30
+    faces = (inputs.faces_uniform(nx, 2.0), inputs.faces_tanh_two_sided(ny, 2.0), inputs.faces_uniform(nz, 1.0))
+    grid = tdx.Grid(nx, ny, nz, *faces, bcs=BCS)
+    yield (nx, ny, nz), faces, grid
+    grid.close()
+
+
+@pytest.mark.parametrize("direction", [0, 1, 2])
+@pytest.mark.parametrize("mode", [tdx.MODE_THOMAS, tdx.MODE_PDD, tdx.MODE_PPT])
+@pytest.mark.parametrize("P", [2, 3, 4, 6])
+def test_identity_operator_index_encoded_rhs_bit_exact(small, direction, mode, P):
+    """alpha = 0: (I - 0*delta2) x = d must return d bit for bit; d = linear index exposes any layout slip."""
+    (nx, ny, nz), _, grid = small
+    field = np.arange(nx * ny * nz, dtype=np.float64).reshape(nz, ny, nx) + 0.25
+    t = torch.from_numpy(field).cuda()
+    grid.adi_sweep(direction, mode, P, 0.0, t)
+    torch.cuda.synchronize()
+    assert np.array_equal(t.cpu().numpy(), field)
+
+
+@pytest.mark.parametrize("direction", [0, 1, 2])
+@pytest.mark.parametrize("mode", [tdx.MODE_THOMAS, tdx.MODE_PDD, tdx.MODE_PPT])
+def test_one_hot_changes_only_its_line(small, direction, mode):
+    (nx, ny, nz), faces, grid = small
+    field = np.zeros((nz, ny, nx)); field[7, 11, 13] = 1.0
+    t = torch.from_numpy(field).cuda()
+    grid.adi_sweep(direction, mode, 3, 0.02, t)
+    torch.cuda.synchronize()
+    out = t.cpu().numpy()
+    mask = np.zeros_like(out, dtype=bool)
+    if direction == 0: mask[7, 11, :] = True
+    if direction == 1: mask[7, :, 13] = True
+    if direction == 2: mask[:, 11, 13] = True
+    assert np.all(out[~mask] == 0.0) and np.count_nonzero(out[mask]) > 3
+    ref = orc.adi_sweep(field.copy(), *faces, BCS, direction, orc.MODE_THOMAS, 1, 0.02)
+    if mode != tdx.MODE_PDD:
+        assert relerr(out, ref) < 1e-12
+
+
+def test_error_paths_leave_data_untouched(small):
+    (nx, ny, nz), _, grid = small
+    field = inputs.rhs_uniform((nz, ny, nx), 1)
+    t = torch.from_numpy(field).cuda()
+    with pytest.raises(tdx.TdxError) as e:
+        grid.adi_sweep(1, tdx.MODE_PPT, 30, 1e-3, t)             # floor(36/30) < 2
+    assert e.value.status == tdx.ERR_BAD_PARTITION
+    with pytest.raises(tdx.TdxError) as e:
+        grid.adi_sweep(0, tdx.MODE_PPT, 0, 1e-3, t)
+    assert e.value.status == tdx.ERR_BAD_PARTITION
+    with pytest.raises(tdx.TdxError) as e:
+        grid.adi_sweep(5, tdx.MODE_PPT, 2, 1e-3, t)
+    assert e.value.status == tdx.ERR_INVALID_ARG
+    with pytest.raises(tdx.TdxError) as e:
+        grid.adi_sweep(0, 7, 2, 1e-3, t)
+    assert e.value.status == tdx.ERR_INVALID_ARG
+    with pytest.raises(tdx.TdxError) as e:
+        grid.adi_sweep(0, tdx.MODE_PPT, 2, 1e-3, 0)              # NULL data pointer
+    assert e.value.status == tdx.ERR_INVALID_ARG
+    with pytest.raises(tdx.TdxError) as e:
+        grid.helmholtz_wavenumber_solve(tdx.MODE_PPT, 4, np.ones(nx), np.ones(3), t)
+    assert e.value.status == tdx.ERR_UNSUPPORTED
+    torch.cuda.synchronize()
+    assert np.array_equal(t.cpu().numpy(), field)
+
+
+def test_rows_per_partition_limit_is_reported():
+    nx = 400
+    f = inputs.faces_uniform(nx, 1.0); g8 = inputs.faces_uniform(8, 1.0)
+    grid = tdx.Grid(nx, 8, 8, f, g8, g8, bcs=BCS)
+    t = torch.zeros(8 * 8 * nx, dtype=torch.float64, device="cuda")
+    with pytest.raises(tdx.TdxError) as e:
+        grid.adi_sweep(0, tdx.MODE_PPT, 4, 1e-3, t)              # 100 rows per partition > 64
+    assert e.value.status == tdx.ERR_UNSUPPORTED
+    grid.adi_sweep(0, tdx.MODE_THOMAS, 4, 1e-3, t)               # Thomas has no such limit
+    grid.close()
+
+
+@pytest.mark.parametrize("direction", [0, 1, 2])
+@pytest.mark.parametrize("mode,P", [(tdx.MODE_THOMAS, 1), (tdx.MODE_PPT, 3), (tdx.MODE_PDD, 2), (tdx.MODE_PPT, 5)])
+def test_cyclic_solve_user_coefficients(small, direction, mode, P):
+    (nx, ny, nz), _, grid = small
+    n = (nx, ny, nz)[direction]
+    rng = np.random.default_rng(direction * 10 + P)
+    a = rng.uniform(-1, -0.1, n); c = rng.uniform(-1, -0.1, n); b = 2.5 - a - c
+    field = inputs.rhs_uniform((nz, ny, nx), 5)
+    t = torch.from_numpy(field).cuda()
+    grid.cyclic_solve(direction, mode, P, a, b, c, t)
+    torch.cuda.synchronize()
+    ref = orc.cyclic_solve(field.copy(), direction, orc.MODE_THOMAS, 1, a, b, c)
+    tol = 1e-12 if mode != tdx.MODE_PDD else 1e-10
+    if mode == tdx.MODE_PDD:
+        ref_pdd = orc.cyclic_solve(field.copy(), direction, orc.MODE_PDD, P, a, b, c)
+        assert relerr(t.cpu().numpy(), ref_pdd) < 1e-12
+    assert relerr(t.cpu().numpy(), ref) < tol
+
+
+def test_host_entry_points(small):
+    (nx, ny, nz), faces, grid = small
+    alpha = 1e-3
+    field = inputs.rhs_uniform((nz, ny, nx), 8)
+    ref = field.copy()
+    for d in range(3):
+        orc.adi_sweep(ref, *faces, BCS, d, orc.MODE_THOMAS, 1, alpha)
+    h = field.copy()
+    grid.adi_step_host(tdx.MODE_PPT, 4, 3, 3, alpha, h)
+    assert relerr(h, ref) < 1e-12
+    h = field.copy()
+    grid.adi_sweep_host(1, tdx.MODE_PPT, 3, alpha, h)
+    assert relerr(h, orc.adi_sweep(field.copy(), *faces, BCS, 1, orc.MODE_THOMAS, 1, alpha)) < 1e-12
+    nm = nz // 2 + 1
+    kz2 = inputs.modified_wavenumbers_z(nz)
+    rhs = inputs.rhs_complex_uniform((nm, ny, nx), 4)
+    hc = rhs.copy()
+    grid.helmholtz_wavenumber_solve_host(tdx.MODE_PPT, 4, None, kz2, hc)
+    assert relerr(hc, orc.helmholtz_solve(rhs.copy(), faces[1], None, kz2, orc.MODE_THOMAS, 1)) < 1e-12
+
+
+def test_kernel_launch_counter_counts_this_librarys_kernels(small):
+    (nx, ny, nz), _, grid = small
+    t = torch.zeros(nx * ny * nz, dtype=torch.float64, device="cuda")
+    grid.adi_sweep(1, tdx.MODE_PPT, 3, 1e-3, t)                  # plan cached after this
+    n0 = tdx.kernel_launch_count()
+    for _ in range(5):
+        grid.adi_sweep(1, tdx.MODE_PPT, 3, 1e-3, t)
+    assert tdx.kernel_launch_count() - n0 == 5                   # one launch per sweep
