@@ -95,7 +95,7 @@ def step_points(cfg):
 
 def sample_shapes(cfg):
     """Bounded sample of the workload for the CPU oracle: same grid lines, fewer of them (about 10-30 s of CPU work)."""
-    budget = 100_000_000                                       # real values per sweep
+    budget = 250_000_000                                       # real values per sweep
     kx = max(1, min(cfg.nz, budget // (cfg.nx * cfg.ny)))      # planes for the x and y sweeps
     jz = max(1, min(cfg.ny, budget // (cfg.nx * cfg.nz)))      # rows for the z sweep
     mh = max(1, min(cfg.nm, budget // (2 * cfg.nx * cfg.ny)))  # wavenumbers for Helmholtz
