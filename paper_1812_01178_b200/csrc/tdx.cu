@@ -54,6 +54,8 @@ struct Plan {
     int layout = tdx::ROWS_PJ;
     int KB = 0, Scap = 0;
     bool cyc = false, thomas = false;
+    int sms = 148;          // SM count of the grid's device
+    mutable int pf = -1;    // L2 prefetch distance of the strided kernel (CTAs), set at first launch
     double alpha = 0.0;
     uint64_t hash = 0;
     double dropped = 0.0;   // max |v_last|, |w_first| (what PDD deletes)
@@ -77,7 +79,7 @@ uint64_t fnv1a(const void* data, size_t bytes, uint64_t h = 1469598103934665603u
 }  // namespace
 
 struct tdx_grid {
-    int nx = 0, ny = 0, nz = 0, device = 0;
+    int nx = 0, ny = 0, nz = 0, device = 0, sms = 148;
     int bc[3] = {0, 0, 0};
     double* faces[3] = {nullptr, nullptr, nullptr};     // device copies
     double* lo[3] = {nullptr, nullptr, nullptr};        // metrics per direction (device)
@@ -238,7 +240,7 @@ tdx_status_t get_plan(tdx_grid* g, int kind, int dir, int mode, int P, double al
             std::memcmp(&p.alpha, &alpha, 8) == 0) { *out = &p; return TDX_OK; }
     Plan pl;
     pl.kind = kind; pl.dir = dir; pl.mode = mode; pl.P = P; pl.n = n; pl.nsets = nsets; pl.M = M; pl.cyc = cyc;
-    pl.thomas = thomas; pl.alpha = alpha; pl.hash = h;
+    pl.thomas = thomas; pl.alpha = alpha; pl.hash = h; pl.sms = g->sms;
     tdx_status_t rc = build_plan(g, pl, lambda_host, ua, ub, uc, st);
     if (rc != TDX_OK) { pl.release(); return rc; }
     g->plans.push_back(pl);
@@ -259,29 +261,36 @@ Tables tables_of(const Plan& pl) {
 namespace {
 
 template <int M, int V, bool CYC>
-tdx_status_t launch_strided_inst(const StridedArgs& A, const Tables& T, dim3 grid, dim3 block, size_t smem, cudaStream_t st) {
+tdx_status_t launch_strided_inst(const Plan& pl, StridedArgs& A, const Tables& T, dim3 grid, dim3 block, size_t smem, cudaStream_t st) {
     static bool attr_done = false;
     if (!attr_done && smem > 48 * 1024) {
         CUDA_TRY(cudaFuncSetAttribute(k_strided<M, V, CYC>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
         attr_done = true;
     }
+    if (pl.pf < 0) {                                               // prefetch one wave of resident CTAs ahead
+        int occ = 1;
+        CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_strided<M, V, CYC>, (int)(block.x * block.y), smem));
+        pl.pf = pl.sms * (occ < 1 ? 1 : occ);
+    }
+    A.pf = pl.pf;
     k_strided<M, V, CYC><<<grid, block, smem, st>>>(A, T);
     LAUNCH_CHECK("k_strided");
     return TDX_OK;
 }
 
 template <int V, bool CYC>
-tdx_status_t launch_strided_M(int M, const StridedArgs& A, const Tables& T, dim3 grid, dim3 block, size_t smem, cudaStream_t st) {
+tdx_status_t launch_strided_M(const Plan& pl, StridedArgs& A, const Tables& T, dim3 grid, dim3 block, size_t smem, cudaStream_t st) {
+    const int M = pl.M;
     switch (M) {
-        case 4: return launch_strided_inst<4, V, CYC>(A, T, grid, block, smem, st);
-        case 8: return launch_strided_inst<8, V, CYC>(A, T, grid, block, smem, st);
-        case 12: return launch_strided_inst<12, V, CYC>(A, T, grid, block, smem, st);
-        case 16: return launch_strided_inst<16, V, CYC>(A, T, grid, block, smem, st);
-        case 20: return launch_strided_inst<20, V, CYC>(A, T, grid, block, smem, st);
-        case 24: return launch_strided_inst<24, V, CYC>(A, T, grid, block, smem, st);
-        case 32: return launch_strided_inst<32, V, CYC>(A, T, grid, block, smem, st);
-        case 48: if (V == 1) return launch_strided_inst<48, 1, CYC>(A, T, grid, block, smem, st); break;
-        case 64: if (V == 1) return launch_strided_inst<64, 1, CYC>(A, T, grid, block, smem, st); break;
+        case 4: return launch_strided_inst<4, V, CYC>(pl, A, T, grid, block, smem, st);
+        case 8: return launch_strided_inst<8, V, CYC>(pl, A, T, grid, block, smem, st);
+        case 12: return launch_strided_inst<12, V, CYC>(pl, A, T, grid, block, smem, st);
+        case 16: return launch_strided_inst<16, V, CYC>(pl, A, T, grid, block, smem, st);
+        case 20: return launch_strided_inst<20, V, CYC>(pl, A, T, grid, block, smem, st);
+        case 24: return launch_strided_inst<24, V, CYC>(pl, A, T, grid, block, smem, st);
+        case 32: return launch_strided_inst<32, V, CYC>(pl, A, T, grid, block, smem, st);
+        case 48: if (V == 1) return launch_strided_inst<48, 1, CYC>(pl, A, T, grid, block, smem, st); break;
+        case 64: if (V == 1) return launch_strided_inst<64, 1, CYC>(pl, A, T, grid, block, smem, st); break;
     }
     return fail(TDX_ERR_UNSUPPORTED, "no strided kernel for M=%d V=%d", M, V);
 }
@@ -291,16 +300,14 @@ int pow2floor(long long v) { int p = 1; while ((long long)p * 2 <= v) p *= 2; re
 // lines of `dir` in a field whose x extent is `nxe` doubles (nx for real fields, 2 nx for complex ones)
 tdx_status_t run_strided(const Plan& pl, double* data, long long W, long long line_stride, long long O,
                          long long outer_stride, bool set_per_outer, cudaStream_t st) {
-    // W, strides in doubles on entry; use 2 lines per thread (16-byte accesses) when everything is even
-    int V = 1;
-    if (pl.thomas || pl.M <= 32) {
-        if (W % 2 == 0 && line_stride % 2 == 0 && outer_stride % 2 == 0 && (reinterpret_cast<uintptr_t>(data) % 16) == 0) V = 2;
-    }
-    StridedArgs A;
-    A.data = data; A.W = W / V; A.line_stride = line_stride / V; A.outer_stride = outer_stride / V;
-    A.set_per_outer = set_per_outer ? 1 : 0;
+    // W, strides in doubles on entry.  16-byte accesses (V = 2 lines per thread) when everything is even.
+    const bool even = W % 2 == 0 && line_stride % 2 == 0 && outer_stride % 2 == 0 && (reinterpret_cast<uintptr_t>(data) % 16) == 0;
     if (O > 65535) return fail(TDX_ERR_UNSUPPORTED, "outer extent %lld > 65535", O);
+    StridedArgs A;
+    A.data = data; A.set_per_outer = set_per_outer ? 1 : 0; A.pf = 0;
     if (pl.thomas) {
+        const int V = even ? 2 : 1;
+        A.W = W / V; A.line_stride = line_stride / V; A.outer_stride = outer_stride / V;
         const int tb = 128;
         A.LPC = tb;
         dim3 grid((unsigned)((A.W + tb - 1) / tb), (unsigned)O);
@@ -309,21 +316,31 @@ tdx_status_t run_strided(const Plan& pl, double* data, long long W, long long li
         LAUNCH_CHECK("k_thomas_strided");
         return TDX_OK;
     }
-    int BT = strided_block_threads(pl.M, V);
-    if (BT < pl.P && V == 2) {                                   // too many partitions for the 2-line variant
-        V = 1; A.W = W; A.line_stride = line_stride; A.outer_stride = outer_stride;
-        BT = strided_block_threads(pl.M, 1);
-    }
-    if (BT < pl.P) return fail(TDX_ERR_UNSUPPORTED, "P=%d partitions of up to %d rows do not fit one thread block", pl.P, pl.M);
-    int LPC = pow2floor(BT / pl.P);
-    if (LPC > 32) LPC = 32;
+    // CTA shape: LPC line-vectors x P partitions.  Row segments of 128 bytes (LPC*V = 16 doubles) and small CTAs (several
+    // resident per SM) measured best; LPC grows only to reach 128 threads, shrinks when the register budget says so.
+    auto pick = [&](int V, int& LPC) -> bool {
+        const int bt = strided_block_threads(pl.M, V);
+        if (bt < pl.P || (V == 2 && (!even || pl.M > 32))) return false;
+        int lmax = pow2floor(bt / pl.P); if (lmax > 32) lmax = 32;
+        int l = 16 / V;
+        while (l * pl.P < 128 && l < 32) l *= 2;
+        if (l > lmax) l = lmax;
+        LPC = l;
+        return true;
+    };
+    int V = 0, LPC = 0, l1 = 0, l2 = 0;
+    const bool ok2 = pick(2, l2), ok1 = pick(1, l1);
+    if (ok2 && (!ok1 || l2 * 2 >= l1)) { V = 2; LPC = l2; }
+    else if (ok1) { V = 1; LPC = l1; }
+    else return fail(TDX_ERR_UNSUPPORTED, "P=%d partitions of up to %d rows do not fit one thread block", pl.P, pl.M);
+    A.W = W / V; A.line_stride = line_stride / V; A.outer_stride = outer_stride / V;
     while (LPC > 1 && LPC / 2 >= A.W) LPC /= 2;
     A.LPC = LPC;
     dim3 block(LPC, pl.P), grid((unsigned)((A.W + LPC - 1) / LPC), (unsigned)O);
     const size_t smem = (size_t)2 * pl.P * LPC * V * 8;
     Tables T = tables_of(pl);
-    if (V == 2) return pl.cyc ? launch_strided_M<2, true>(pl.M, A, T, grid, block, smem, st) : launch_strided_M<2, false>(pl.M, A, T, grid, block, smem, st);
-    return pl.cyc ? launch_strided_M<1, true>(pl.M, A, T, grid, block, smem, st) : launch_strided_M<1, false>(pl.M, A, T, grid, block, smem, st);
+    if (V == 2) return pl.cyc ? launch_strided_M<2, true>(pl, A, T, grid, block, smem, st) : launch_strided_M<2, false>(pl, A, T, grid, block, smem, st);
+    return pl.cyc ? launch_strided_M<1, true>(pl, A, T, grid, block, smem, st) : launch_strided_M<1, false>(pl, A, T, grid, block, smem, st);
 }
 
 template <int M, bool UNI, bool CYC>
@@ -453,6 +470,7 @@ tdx_status_t tdx_grid_create(int nx, int ny, int nz, const double* xf, const dou
     tdx_grid* g = new (std::nothrow) tdx_grid();
     if (!g) return fail(TDX_ERR_ALLOC, "host allocation failed");
     g->nx = nx; g->ny = ny; g->nz = nz; g->device = device;
+    if (cudaDeviceGetAttribute(&g->sms, cudaDevAttrMultiProcessorCount, device) != cudaSuccess || g->sms < 1) g->sms = 148;
     auto bail = [&](tdx_status_t st) { tdx_grid_destroy(g); return st; };
     for (int d = 0; d < 3; ++d) {
         g->bc[d] = bcs[d];

@@ -20,7 +20,7 @@
 namespace tdx {
 
 struct Tables {
-    const double* rows;      // row table (layout depends on the kernel), fields {l, inv, cp, v, w, q}
+    const double* rows;      // row table (layout depends on the kernel), fields {l, q, inv, cp, v, w}
     const double* G;         // reduced coefficients G[((set*2+side)*KB + k)*P + p]
     const int2* band;        // band[set*P + p] = {lo, cnt} in interface-rhs indices r[0..2P)
     const int* Sidx;         // cyclic closure functional (sparse), Sidx/Sval[set*Scap + k], Sn[set]
@@ -36,6 +36,7 @@ struct StridedArgs {
     long long outer_stride;  // distance between outer indices, in V-vectors
     int set_per_outer;       // 1: table set = outer index (Helmholtz wavenumber), 0: one set
     int LPC;                 // lines (V-vectors) per CTA = blockDim.x
+    int pf;                  // L2 prefetch distance in CTAs (0 = off)
 };
 
 template <int V> struct VecIO;
@@ -48,10 +49,18 @@ template <> struct VecIO<2> {
     __device__ static inline void st(double* p, const double (&x)[2]) { __stcs(reinterpret_cast<double2*>(p), make_double2(x[0], x[1])); }
 };
 
-constexpr int strided_block_threads(int MAXM, int V) { return (2 * MAXM * V <= 24) ? 1024 : ((2 * MAXM * V <= 64) ? 512 : 256); }
+// Register budget per thread: the partition (MAXM x V doubles = 2 MAXM V registers) plus ~50 for addresses, table
+// values in flight and the interface unknowns.  Measured on B200 (profiles/r1_probe_strided.md): spills cost more than
+// occupancy, and 2-4 small co-resident CTAs per SM beat one large one.
+constexpr int strided_regs(int MAXM, int V) {
+    return (MAXM * V <= 8) ? 72 : ((MAXM * V <= 16) ? 104 : ((MAXM * V <= 32) ? 128 : ((MAXM * V <= 48) ? 168 : 232)));
+}
+constexpr int strided_block_threads(int MAXM, int V) {            // largest CTA the register budget allows
+    return (65536 / strided_regs(MAXM, V)) / 32 * 32 > 1024 ? 1024 : (65536 / strided_regs(MAXM, V)) / 32 * 32;
+}
 
 template <int MAXM, int V, bool CYC>
-__global__ void __launch_bounds__(strided_block_threads(MAXM, V))
+__global__ void __maxnreg__(strided_regs(MAXM, V))
 k_strided(StridedArgs A, Tables T) {
     extern __shared__ double rs[];                          // rs[(idx*LPC + tx)*V + v], idx in [0, 2P)
     const int tx = threadIdx.x, p = threadIdx.y;
@@ -62,16 +71,32 @@ k_strided(StridedArgs A, Tables T) {
     const int set = A.set_per_outer ? o : 0;
     const int start = part_start(p, T.q, T.r);
     const int m = T.q + (p < T.r ? 1 : 0);
+    const bool full = (T.r == 0) && (T.q == MAXM);          // every partition has exactly MAXM rows (warp-uniform)
     double* base = A.data + ((long long)o * A.outer_stride + (long long)start * A.line_stride + i) * V;
     const long long rstride = A.line_stride * V;
 
     double x[MAXM][V];
 #pragma unroll
     for (int jj = 0; jj < MAXM; ++jj) {
-        if (valid && jj < m) VecIO<V>::ld(base + jj * rstride, x[jj]);
+        if (valid && (full || jj < m)) VecIO<V>::ld(base + jj * rstride, x[jj]);
         else {
 #pragma unroll
             for (int v = 0; v < V; ++v) x[jj][v] = 0.0;
+        }
+    }
+    // L2 prefetch of the tile a CTA `pf` launches later will load: one lane per 128-byte line.  The CTA that needs
+    // the data then finds it in L2 (~300 cycles) instead of HBM, so a few resident CTAs per SM keep HBM busy.
+    if (A.pf > 0 && ((tx * V) & 15) == 0) {
+        const long long lin = (long long)blockIdx.y * gridDim.x + blockIdx.x + A.pf;
+        if (lin < (long long)gridDim.x * gridDim.y) {
+            const int by = (int)(lin / gridDim.x), bx = (int)(lin - (long long)by * gridDim.x);
+            const long long ip = (long long)bx * LPC + tx;
+            if (ip < A.W) {
+                const double* pb = A.data + ((long long)by * A.outer_stride + (long long)start * A.line_stride + ip) * V;
+#pragma unroll
+                for (int jj = 0; jj < MAXM; ++jj)
+                    if (full || jj < m) asm volatile("prefetch.global.L2 [%0];" ::"l"(pb + jj * rstride));
+            }
         }
     }
     const double2* rt = reinterpret_cast<const double2*>(T.rows + ((size_t)((size_t)set * P + p) * MAXM) * 6);
@@ -79,30 +104,26 @@ k_strided(StridedArgs A, Tables T) {
     // Eq.(5): forward y_j = d_j - l_j y_{j-1}, backward xt_j = y_j inv_j - cp_j xt_{j+1}
 #pragma unroll
     for (int jj = 1; jj < MAXM; ++jj) {
-        const double l = __ldg(&rt[jj * 3 + 0]).x;
+        const double l = __ldg(reinterpret_cast<const double*>(&rt[jj * 3 + 0]));
 #pragma unroll
         for (int v = 0; v < V; ++v) x[jj][v] = fma(-l, x[jj - 1][v], x[jj][v]);
     }
     {
-        const double inv = __ldg(&rt[(MAXM - 1) * 3 + 0]).y;
+        const double inv = __ldg(reinterpret_cast<const double*>(&rt[(MAXM - 1) * 3 + 1]));
 #pragma unroll
         for (int v = 0; v < V; ++v) x[MAXM - 1][v] *= inv;
     }
 #pragma unroll
     for (int jj = MAXM - 2; jj >= 0; --jj) {
-        const double inv = __ldg(&rt[jj * 3 + 0]).y;
-        const double cp = __ldg(&rt[jj * 3 + 1]).x;
+        const double2 ic = __ldg(&rt[jj * 3 + 1]);          // {inv, cp}
 #pragma unroll
-        for (int v = 0; v < V; ++v) x[jj][v] = fma(-cp, x[jj + 1][v], x[jj][v] * inv);
+        for (int v = 0; v < V; ++v) x[jj][v] = fma(-ic.y, x[jj + 1][v], x[jj][v] * ic.x);
     }
     // E^T xt: first and last row of this partition
 #pragma unroll
     for (int v = 0; v < V; ++v) {
-        double xl = x[MAXM - 1][v];
-#pragma unroll
-        for (int jj = 0; jj < MAXM - 1; ++jj) if (jj == m - 1) xl = x[jj][v];
         rs[((2 * p) * LPC + tx) * V + v] = x[0][v];
-        rs[((2 * p + 1) * LPC + tx) * V + v] = xl;
+        rs[((2 * p + 1) * LPC + tx) * V + v] = x[MAXM - 1][v];  // xt_last (padding rows carry it to the last slot)
     }
     __syncthreads();
     // Eq.(7): the two interface unknowns this partition needs
@@ -135,16 +156,17 @@ k_strided(StridedArgs A, Tables T) {
     // Eq.(8): x = xt - v yL - w yR (- q s for periodic lines), then store
 #pragma unroll
     for (int jj = 0; jj < MAXM; ++jj) {
-        const double2 t1 = __ldg(&rt[jj * 3 + 1]);          // {cp, v}
-        const double2 t2 = __ldg(&rt[jj * 3 + 2]);          // {w, q}
+        const double2 vw = __ldg(&rt[jj * 3 + 2]);          // {v, w}
+        double qj = 0.0;
+        if (CYC) qj = __ldg(reinterpret_cast<const double*>(&rt[jj * 3 + 0]) + 1);   // {l, q}
 #pragma unroll
         for (int v = 0; v < V; ++v) {
-            double r = fma(-t1.y, yL[v], x[jj][v]);
-            r = fma(-t2.x, yR[v], r);
-            if (CYC) r = fma(-t2.y, sc[v], r);
+            double r = fma(-vw.x, yL[v], x[jj][v]);
+            r = fma(-vw.y, yR[v], r);
+            if (CYC) r = fma(-qj, sc[v], r);
             x[jj][v] = r;
         }
-        if (valid && jj < m) VecIO<V>::st(base + jj * rstride, x[jj]);
+        if (valid && (full || jj < m)) VecIO<V>::st(base + jj * rstride, x[jj]);
     }
 }
 

@@ -23,7 +23,8 @@ namespace tdx {
 enum RowLayout { ROWS_PJ = 0,      // rows[((set*P + p)*M + jj)*6 + f]   strided kernels (p is warp-uniform) and Thomas (P=1)
                  ROWS_JP = 1,      // rows[((set*M + jj)*6 + f)*P + p]   unit-stride kernel, partitions differ per lane
                  ROWS_U = 2 };     // rows[jj*6 + f]                     unit-stride kernel, all partitions identical
-enum RowField { F_L = 0, F_INV = 1, F_CP = 2, F_V = 3, F_W = 4, F_Q = 5 };
+// field order: 16-byte pairs {l, q}, {inv, cp}, {v, w} -- forward, backward and correction each read one pair per row
+enum RowField { F_L = 0, F_Q = 1, F_INV = 2, F_CP = 3, F_V = 4, F_W = 5 };
 
 __host__ __device__ inline int part_start(int p, int q, int r) { return p * q + (p < r ? p : r); }
 
@@ -163,10 +164,13 @@ __global__ void k_factor(int n, int nsets, int P, int M, int layout,
     e[2] = (p < P - 1) ? w[0] : 0.0; e[3] = (p < P - 1) ? w[m - 1] : 0.0;
     if (P == 1) { e[0] = e[1] = e[2] = e[3] = 0.0; }
     if (!writer) return;
+    // Padding rows jj >= m (never loaded or stored: their d is 0) carry the partition's last value along:
+    // l = -1 copies y_{m-1} forward, inv = inv_{m-1} and cp = 0 turn it into xt_{m-1} in the backward pass, so that
+    // xt_last is always slot M-1 and no kernel indexes its register-resident partition with a run-time row number.
     for (int jj = 0; jj < M; ++jj) {
         bool real = jj < m;
-        rows[row_index(layout, s, P, M, p, jj, F_L)] = real ? l[jj] : 0.0;
-        rows[row_index(layout, s, P, M, p, jj, F_INV)] = real ? inv[jj] : 1.0;
+        rows[row_index(layout, s, P, M, p, jj, F_L)] = real ? l[jj] : -1.0;
+        rows[row_index(layout, s, P, M, p, jj, F_INV)] = real ? inv[jj] : inv[m - 1];
         rows[row_index(layout, s, P, M, p, jj, F_CP)] = real ? cp[jj] : 0.0;
         rows[row_index(layout, s, P, M, p, jj, F_V)] = real ? v[jj] : 0.0;
         rows[row_index(layout, s, P, M, p, jj, F_W)] = real ? w[jj] : 0.0;
