@@ -18,6 +18,7 @@
 #include "../../include/tdx.h"
 #include "tdx_kernels.cuh"
 #include "tdx_plan.cuh"
+#include "tdx_tma.cuh"
 
 namespace {
 
@@ -55,7 +56,10 @@ struct Plan {
     int KB = 0, Scap = 0;
     bool cyc = false, thomas = false;
     int sms = 148;          // SM count of the grid's device
-    mutable int pf = -1;    // L2 prefetch distance of the strided kernel (CTAs), set at first launch
+    mutable int pf = -1;    // L2 prefetch distance of the sweep kernel (CTAs), set at first launch
+    mutable CUtensorMap tmap;             // x sweeps: tensor map of the field as [lines*P, M] partition rows
+    mutable const void* tmap_ptr = nullptr;   // field the cached tensor map was encoded for
+    mutable int tmap_box = 0;
     double alpha = 0.0;
     uint64_t hash = 0;
     double dropped = 0.0;   // max |v_last|, |w_first| (what PDD deletes)
@@ -371,6 +375,84 @@ tdx_status_t launch_unit_M(int M, const UnitArgs& A, const Tables& T, unsigned g
     return fail(TDX_ERR_UNSUPPORTED, "no unit-stride kernel for M=%d", M);
 }
 
+// ---- x sweeps through TMA (tdx_tma.cuh) ---------------------------------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+EncodeTiledFn encode_tiled_fn() {
+    static EncodeTiledFn fn = [] {
+        void* f = nullptr;
+        cudaDriverEntryPointQueryResult qr;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &f, cudaEnableDefault, &qr) != cudaSuccess) { cudaGetLastError(); f = nullptr; }
+        return reinterpret_cast<EncodeTiledFn>(f);
+    }();
+    return fn;
+}
+
+template <int M, bool UNI, bool CYC>
+tdx_status_t launch_unit_tma_inst(const Plan& pl, UnitTmaArgs& A, const Tables& T, unsigned grid, int threads, size_t smem, cudaStream_t st) {
+    static bool attr_done = false;
+    if (!attr_done) {
+        CUDA_TRY(cudaFuncSetAttribute(k_unit_tma<M, UNI, CYC>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+        attr_done = true;
+    }
+    if (pl.pf < 0) {
+        int occ = 1;
+        CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_unit_tma<M, UNI, CYC>, threads, smem));
+        pl.pf = pl.sms * (occ < 1 ? 1 : occ);
+    }
+    A.pf = pl.pf;
+    k_unit_tma<M, UNI, CYC><<<grid, threads, smem, st>>>(pl.tmap, A, T);
+    LAUNCH_CHECK("k_unit_tma");
+    return TDX_OK;
+}
+
+// returns TDX_ERR_UNSUPPORTED (without setting an error text) when the shape does not fit the TMA path
+tdx_status_t run_unit_tma(const Plan& pl, double* data, long long nlines, cudaStream_t st, bool* taken) {
+    *taken = false;
+    const int q = pl.n / pl.P;
+    if (pl.n % pl.P != 0 || (q != 8 && q != 16) || pl.M != q) return TDX_OK;
+    if (reinterpret_cast<uintptr_t>(data) % 16 != 0) return TDX_OK;
+    EncodeTiledFn enc = encode_tiled_fn();
+    if (!enc) return TDX_OK;
+    UnitTmaArgs A;
+    A.total_rows = nlines * pl.P;
+    if (A.total_rows >= (1LL << 31)) return TDX_OK;
+    int lpb = 256 / pl.P; if (lpb < 1) lpb = 1; if (lpb > nlines) lpb = (int)nlines;
+    A.rows_per_cta = lpb * pl.P;
+    A.nbox = (A.rows_per_cta + 255) / 256;
+    if (A.rows_per_cta % A.nbox != 0) return TDX_OK;
+    A.box_rows = A.rows_per_cta / A.nbox;
+    if (A.nbox > 1 && A.box_rows % 8 != 0) return TDX_OK;
+    const int threads = (A.rows_per_cta + 31) / 32 * 32;
+    if (threads > 1024 || threads * unit_tma_regs(q) > 65536) return TDX_OK;
+    if (pl.tmap_ptr != data || pl.tmap_box != A.box_rows) {
+        cuuint64_t gdim[2] = {(cuuint64_t)q, (cuuint64_t)A.total_rows};
+        cuuint64_t gstr[1] = {(cuuint64_t)q * 8};
+        cuuint32_t box[2] = {(cuuint32_t)q, (cuuint32_t)A.box_rows}, es[2] = {1, 1};
+        CUresult cr = enc(&pl.tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, data, gdim, gstr, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                          q == 16 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_64B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                          CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (cr != CUDA_SUCCESS) return fail(TDX_ERR_CUDA, "cuTensorMapEncodeTiled failed (%d)", (int)cr);
+        pl.tmap_ptr = data; pl.tmap_box = A.box_rows;
+    }
+    const size_t smem = (size_t)threads * q * 8 + (size_t)2 * threads * 8 + 16;
+    const unsigned grid = (unsigned)((A.total_rows + A.rows_per_cta - 1) / A.rows_per_cta);
+    Tables T = tables_of(pl);
+    const bool uni = pl.layout == ROWS_U;
+    *taken = true;
+#define TDX_TMA_CASE(MM) \
+    if (q == MM) { \
+        if (uni) return pl.cyc ? launch_unit_tma_inst<MM, true, true>(pl, A, T, grid, threads, smem, st) : launch_unit_tma_inst<MM, true, false>(pl, A, T, grid, threads, smem, st); \
+        return pl.cyc ? launch_unit_tma_inst<MM, false, true>(pl, A, T, grid, threads, smem, st) : launch_unit_tma_inst<MM, false, false>(pl, A, T, grid, threads, smem, st); \
+    }
+    TDX_TMA_CASE(16)
+    TDX_TMA_CASE(8)
+#undef TDX_TMA_CASE
+    *taken = false;
+    return TDX_OK;
+}
+
 int unit_bt(int M) { return M <= 8 ? 1024 : (M <= 24 ? 512 : 256); }
 
 tdx_status_t run_unit(const Plan& pl, double* data, long long nlines, cudaStream_t st) {
@@ -381,6 +463,11 @@ tdx_status_t run_unit(const Plan& pl, double* data, long long nlines, cudaStream
         else k_thomas_unit<false><<<grid, tb, 0, st>>>(data, nlines, pl.rows, pl.cyc_tab, pl.n);
         LAUNCH_CHECK("k_thomas_unit");
         return TDX_OK;
+    }
+    {
+        bool taken = false;
+        tdx_status_t rc = run_unit_tma(pl, data, nlines, st, &taken);
+        if (rc != TDX_OK || taken) return rc;
     }
     const int BT = unit_bt(pl.M);
     if (pl.P > BT) return fail(TDX_ERR_UNSUPPORTED, "P=%d partitions of up to %d rows do not fit one thread block", pl.P, pl.M);
