@@ -30,7 +30,7 @@ UNIT = "Gpts/s"
 BYTES_PER_POINT = 16.0          # 8 B read + 8 B written per real grid value per sweep
 
 # tuned partitions per line (x, y, z, helmholtz-y) per config; rows per partition <= 64
-TUNED_P = {1: (4, 4, 4, 4), 2: (16, 16, 16, 16), 3: (32, 32, 32, 32), 4: (64, 32, 32, 32), 5: (256, 36, 32, 36)}
+TUNED_P = {1: (4, 4, 4, 4), 2: (16, 16, 16, 16), 3: (32, 32, 32, 32), 4: (64, 32, 32, 32), 5: (256, 24, 16, 12)}
 
 
 def parse():

@@ -60,6 +60,8 @@ struct Plan {
     mutable CUtensorMap tmap;             // x sweeps: tensor map of the field as [lines*P, M] partition rows
     mutable const void* tmap_ptr = nullptr;   // field the cached tensor map was encoded for
     mutable int tmap_box = 0;
+    mutable double uni_host[16 * 6];      // host copy of the uniform row table (kernel parameter of k_unit_tma)
+    mutable bool uni_host_ok = false;
     double alpha = 0.0;
     uint64_t hash = 0;
     double dropped = 0.0;   // max |v_last|, |w_first| (what PDD deletes)
@@ -402,7 +404,16 @@ tdx_status_t launch_unit_tma_inst(const Plan& pl, UnitTmaArgs& A, const Tables& 
         pl.pf = pl.sms * (occ < 1 ? 1 : occ);
     }
     A.pf = pl.pf;
-    k_unit_tma<M, UNI, CYC><<<grid, threads, smem, st>>>(pl.tmap, A, T);
+    UniTable<M> U;
+    if (UNI) {
+        if (!pl.uni_host_ok) {
+            CUDA_TRY(cudaMemcpyAsync(pl.uni_host, pl.rows, sizeof(double) * M * 6, cudaMemcpyDeviceToHost, st));
+            CUDA_TRY(cudaStreamSynchronize(st));
+            pl.uni_host_ok = true;
+        }
+        std::memcpy(U.v, pl.uni_host, sizeof(double) * M * 6);
+    } else std::memset(U.v, 0, sizeof(U.v));
+    k_unit_tma<M, UNI, CYC><<<grid, threads, smem, st>>>(pl.tmap, A, T, U);
     LAUNCH_CHECK("k_unit_tma");
     return TDX_OK;
 }

@@ -70,11 +70,15 @@ struct UnitTmaArgs {
 
 constexpr int unit_tma_regs(int M) { return M <= 8 ? 56 : 80; }
 
+// The uniform row table (all partitions identical: uniform grid in x) travels as a kernel parameter: with the row loops
+// fully unrolled every table value is a constant-bank operand of its DFMA -- no load instruction, no L1 wavefront.
+template <int M> struct UniTable { double v[M * 6]; };
+
 // M = rows per partition = doubles per partition row (16 -> 128-byte rows / SWIZZLE_128B, 8 -> 64-byte / SWIZZLE_64B).
 // UNI: one table for every partition (rows[jj*6+f], warp-uniform); else per-partition columns (rows[(jj*6+f)*P + p]).
 template <int M, bool UNI, bool CYC>
 __global__ void __maxnreg__(unit_tma_regs(M))
-k_unit_tma(const __grid_constant__ CUtensorMap tmap, UnitTmaArgs A, Tables T) {
+k_unit_tma(const __grid_constant__ CUtensorMap tmap, UnitTmaArgs A, Tables T, const __grid_constant__ UniTable<M> U) {
     extern __shared__ __align__(1024) unsigned char tma_smem[];
     constexpr int CH = M / 2;                                         // 16-byte chunks per partition row
     double2* tile = reinterpret_cast<double2*>(tma_smem);             // [blockDim.x][CH] 16-byte chunks, hardware-swizzled
@@ -103,7 +107,7 @@ k_unit_tma(const __grid_constant__ CUtensorMap tmap, UnitTmaArgs A, Tables T) {
     const bool valid = r < A.rows_per_cta;
     const double* rows = T.rows;
     auto tab = [&](int jj, int f) -> double {
-        if (UNI) return __ldg(rows + jj * 6 + f);
+        if (UNI) return U.v[jj * 6 + f];
         return __ldg(rows + ((size_t)jj * 6 + f) * P + (valid ? p : 0));
     };
     mbar_wait(bar, 0);
