@@ -30,7 +30,7 @@ UNIT = "Gpts/s"
 BYTES_PER_POINT = 16.0          # 8 B read + 8 B written per real grid value per sweep
 
 # tuned partitions per line (x, y, z, helmholtz-y) per config; rows per partition <= 64
-TUNED_P = {1: (4, 4, 4, 4), 2: (16, 16, 16, 16), 3: (32, 32, 32, 32), 4: (64, 32, 32, 32), 5: (256, 24, 16, 12)}
+TUNED_P = {1: (4, 4, 4, 4), 2: (16, 8, 8, 8), 3: (32, 8, 8, 8), 4: (64, 16, 8, 16), 5: (256, 24, 16, 12)}
 
 
 def parse():
@@ -45,7 +45,59 @@ def parse():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--selftest-ranks", action="store_true",
+                    help="CPU-only check of the N>1 host logic over gloo (used by tests/test_bench_ranks_gloo.py)")
     return ap.parse_args()
+
+
+# ---- N > 1 host logic (one process per GPU; the path shards as independent fields, no data-path collective) ----------
+def init_dist(world, backend, local_rank=0):
+    """Process group for the barrier and the max-over-ranks reduction only. MASTER_ADDR/PORT, RANK, WORLD_SIZE from env."""
+    if world <= 1:
+        return None
+    import torch
+    import torch.distributed as dist
+    if backend == "nccl":
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    else:
+        dist.init_process_group(backend)
+    return dist
+
+
+def max_over_ranks(value, dist, device="cpu"):
+    """Every multi-GPU number is the MAX over ranks of a device-side time."""
+    if dist is None:
+        return float(value)
+    import torch
+    t = torch.tensor([float(value)], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def rank_seed(cfg, rank):
+    """Rank r solves its own field: same shape and recipe, seed shifted (weak scaling)."""
+    return cfg.seed + 1000 * rank
+
+
+def whole_job_value(cfg, world, steps, total_ms):
+    return world * step_points(cfg) * steps / (total_ms * 1e-3) / 1e9
+
+
+def selftest_ranks(args, rank, world):
+    dist = init_dist(world, "gloo")
+    cfg = configs.get(1)
+    seeds = [rank_seed(cfg, r) for r in range(world)]
+    assert len(set(seeds)) == world and seeds[0] == cfg.seed
+    fake_ms = 10.0 * (rank + 1)                                   # slowest rank = world-1
+    mx = max_over_ranks(fake_ms, dist)
+    assert mx == 10.0 * world, (mx, world)
+    val = whole_job_value(cfg, world, 2, mx)
+    if dist is not None:
+        dist.barrier()
+    if rank == 0:
+        print(json.dumps({"selftest": "ok", "world": world, "max_ms": mx, "value": val, "seeds": seeds}))
+    if dist is not None:
+        dist.destroy_process_group()
 
 
 def measured_peak():
@@ -159,14 +211,12 @@ def run_reference(args, rank, world):
 
 def run_tdx(args, rank, world, local_rank):
     import torch
-    import torch.distributed as dist
     from paper_1812_01178_b200 import binding as tdx
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device; the tdx path has no CPU fallback")
     torch.cuda.set_device(local_rank)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    dist = init_dist(world, "nccl", local_rank)
     cfg = configs.get(args.config)
     mode = {"ppt": tdx.MODE_PPT, "pdd": tdx.MODE_PDD, "thomas": tdx.MODE_THOMAS}[args.mode]
     Ps = tuple(int(v) for v in args.P.split(",")) if args.P else TUNED_P[args.config]
@@ -175,11 +225,10 @@ def run_tdx(args, rank, world, local_rank):
     kz2 = cfg.kz2()
 
     # inputs: seeded synthetic, generated once on the host, resident in HBM before the timed region
-    seed_shift = 1000 * rank                                    # every rank solves its own field (weak scaling)
-    host_field = cfg.rhs_field() if rank == 0 else None
+    host_field = cfg.rhs_field() if rank == 0 else None         # every rank solves its own field (weak scaling)
     if rank != 0:
         from paper_1812_01178_b200 import inputs
-        host_field = inputs.rhs_uniform((cfg.nz, cfg.ny, cfg.nx), cfg.seed + seed_shift)
+        host_field = inputs.rhs_uniform((cfg.nz, cfg.ny, cfg.nx), rank_seed(cfg, rank))
     host_helm = cfg.rhs_helmholtz()
     field0 = torch.from_numpy(host_field).cuda()
     helm0 = torch.from_numpy(host_helm).cuda()
@@ -219,13 +268,9 @@ def run_tdx(args, rank, world, local_rank):
     barrier()
     launches = tdx.kernel_launch_count() - n0
     sampler.stop_flag.set()
-    total_ms = e0.elapsed_time(e1)
-    if world > 1:
-        tt = torch.tensor([total_ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        total_ms = float(tt.item())
+    total_ms = max_over_ranks(e0.elapsed_time(e1), dist, "cuda")
     ms_per_step = total_ms / args.steps
-    value = world * step_points(cfg) * args.steps / (total_ms * 1e-3) / 1e9
+    value = whole_job_value(cfg, world, args.steps, total_ms)
 
     # per-kernel durations (CUDA events on the launching stream, inside the timed region)
     names = ["adi_x", "adi_y", "adi_z_cyclic", "helmholtz_y"]
@@ -269,11 +314,7 @@ def run_tdx(args, rank, world, local_rank):
             grid.helmholtz_wavenumber_solve_host(mode, Ps[3], None, kz2, hh)
             torch.cuda.synchronize()
             ts.append(time.perf_counter() - t0)
-        te = float(np.mean(ts))
-        if world > 1:
-            tt = torch.tensor([te], device="cuda", dtype=torch.float64)
-            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-            te = float(tt.item())
+        te = max_over_ranks(float(np.mean(ts)), dist, "cuda")
         out["e2e"] = {"value": world * step_points(cfg) / te / 1e9, "unit": UNIT, "h2d_bytes_per_step": int(hf.nbytes + hh.nbytes),
                       "d2h_bytes_per_step": int(hf.nbytes + hh.nbytes), "ms_per_step": te * 1e3, "steps": len(ts),
                       "api": "tdx_adi_step_host + tdx_helmholtz_wavenumber_solve_host (pinned host buffers)"}
@@ -294,7 +335,9 @@ def main():
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
-    if args.impl == "reference":
+    if args.selftest_ranks:
+        selftest_ranks(args, rank, world)
+    elif args.impl == "reference":
         run_reference(args, rank, world)
     else:
         run_tdx(args, rank, world, local_rank)

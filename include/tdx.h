@@ -61,8 +61,9 @@ tdx_status_t tdx_grid_destroy(tdx_grid_t* grid);   /* frees plan tables; NULL is
 tdx_status_t tdx_partition_bounds(int n, int P, int* starts);
 
 /* ADI sweep (Algorithm 1): solve (I - alpha*delta2_dir) x = rhs on every line of
- * direction dir, in place.  Rows satisfy |b| = |a| + |c| + 1 (L162).  Periodic directions are closed by
- * Sherman-Morrison (Eq.(3) with a rank-1 update) on top of the chosen mode.
+ * direction dir, in place.  Rows satisfy |b| = |a| + |c| + 1 (L162).  Periodic directions: THOMAS and PDD close the
+ * line by Sherman-Morrison (Eq.(3) with a rank-1 update) around the chosen mode; PPT (P <= 128) puts the two wrap-around
+ * corner entries into Delta A (L78-91), i.e. P interfaces and a cyclic reduced system Z -- Woodbury, Eq.(3)-(4), exact.
  * rhs_inout: DEVICE, nx*ny*nz doubles.  P: partitions per line (ignored for THOMAS).                    */
 tdx_status_t tdx_adi_sweep(tdx_grid_t* grid, tdx_dir_t dir, tdx_mode_t mode, int P,
                            double alpha, double* rhs_inout, void* stream);
@@ -80,7 +81,8 @@ tdx_status_t tdx_helmholtz_wavenumber_solve(tdx_grid_t* grid, tdx_mode_t mode, i
 
 /* Batched cyclic tridiagonal solve along dir with caller-given coefficients shared by every line:
  * a, b, c: HOST arrays of n_dir doubles; a[0] couples row 0 to row n-1 and c[n-1] couples row n-1 to row 0.
- * Sherman-Morrison closure (gamma = -b[0]) around the chosen mode.  rhs_inout: DEVICE, nx*ny*nz doubles. */
+ * Closure as for tdx_adi_sweep on a periodic direction (Sherman-Morrison with gamma = -b[0] for THOMAS / PDD, cyclic
+ * reduced system for PPT).  rhs_inout: DEVICE, nx*ny*nz doubles. */
 tdx_status_t tdx_cyclic_solve(tdx_grid_t* grid, tdx_dir_t dir, tdx_mode_t mode, int P,
                               const double* a, const double* b, const double* c,
                               double* rhs_inout, void* stream);

@@ -7,6 +7,7 @@
 #include <cstdint>
 #include <cstdio>
 #include <cstring>
+#include <cstdlib>
 #include <mutex>
 #include <string>
 #include <vector>
@@ -55,6 +56,7 @@ struct Plan {
     int layout = tdx::ROWS_PJ;
     int KB = 0, Scap = 0;
     bool cyc = false, thomas = false;
+    bool wrap = false;      // periodic line closed inside the reduced system (PPT, P <= 128) instead of Sherman-Morrison
     int sms = 148;          // SM count of the grid's device
     mutable int pf = -1;    // L2 prefetch distance of the sweep kernel (CTAs), set at first launch
     mutable CUtensorMap tmap;             // x sweeps: tensor map of the field as [lines*P, M] partition rows
@@ -75,6 +77,13 @@ struct Plan {
 };
 
 const int kMInst[] = {4, 8, 12, 16, 20, 24, 32, 48, 64};
+
+// L2 prefetch distance in waves of resident CTAs: environment TDX_L2_PREFETCH (default 1; 0 switches the prefetch off).
+// A measurement knob (profiles/ compare on/off); it never changes results.
+int prefetch_waves() {
+    static int w = [] { const char* e = std::getenv("TDX_L2_PREFETCH"); int v = e ? std::atoi(e) : 1; return v < 0 ? 0 : (v > 64 ? 64 : v); }();
+    return w;
+}
 
 uint64_t fnv1a(const void* data, size_t bytes, uint64_t h = 1469598103934665603ull) {
     const unsigned char* p = static_cast<const unsigned char*>(data);
@@ -155,7 +164,7 @@ tdx_status_t build_plan(tdx_grid* g, Plan& pl, const double* lambda_host, const 
     pl.layout = ROWS_PJ;
     if (pl.dir == 0) {
         pl.layout = ROWS_JP;
-        if (n % P == 0 && P >= 3 && nsets == 1) {
+        if (n % P == 0 && P >= 3 && nsets == 1 && !pl.wrap) {
             DevBuf differs; CUDA_TRY(differs.alloc(4));
             CUDA_TRY(cudaMemsetAsync(differs.p, 0, 4, st));
             k_blocks_identical<<<(n + tb - 1) / tb, tb, 0, st>>>(n, P, a.as<double>(), b.as<double>(), c.as<double>(), differs.as<int>());
@@ -171,7 +180,7 @@ tdx_status_t build_plan(tdx_grid* g, Plan& pl, const double* lambda_host, const 
     DevBuf ends; CUDA_TRY(ends.alloc((size_t)nsets * P * 4 * 8));
     {
         const int nt = nsets * P;
-        k_factor<TDX_MAX_ROWS_PER_PARTITION><<<(nt + 63) / 64, 64, 0, st>>>(n, nsets, P, pl.M, pl.layout, a.as<double>(), b.as<double>(),
+        k_factor<TDX_MAX_ROWS_PER_PARTITION><<<(nt + 63) / 64, 64, 0, st>>>(n, nsets, P, pl.M, pl.layout, pl.wrap ? 1 : 0, a.as<double>(), b.as<double>(),
                                                                             c.as<double>(), qptr, flags.as<int>(), pl.rows, ends.as<double>());
         LAUNCH_CHECK("k_factor");
     }
@@ -182,6 +191,18 @@ tdx_status_t build_plan(tdx_grid* g, Plan& pl, const double* lambda_host, const 
     if (pl.mode == TDX_MODE_PDD) {
         k_pack_pdd<<<(ntp + tb - 1) / tb, tb, 0, st>>>(nsets, P, pl.KB, ends.as<double>(), pl.G, pl.band);
         LAUNCH_CHECK("k_pack_pdd");
+    } else if (pl.wrap) {
+        const int K = 2 * P;
+        DevBuf Z, Zi, piv;
+        CUDA_TRY(Z.alloc((size_t)nsets * K * K * 8)); CUDA_TRY(Zi.alloc((size_t)nsets * K * K * 8)); CUDA_TRY(piv.alloc((size_t)nsets * K * 4));
+        k_reduced_cyclic_factor<<<(nsets + 31) / 32, 32, 0, st>>>(nsets, P, ends.as<double>(), Z.as<double>(), piv.as<int>());
+        LAUNCH_CHECK("k_reduced_cyclic_factor");
+        const long nk = (long)nsets * K;
+        k_reduced_cyclic_inverse<<<(unsigned)((nk + 63) / 64), 64, 0, st>>>(nsets, P, Z.as<double>(), piv.as<int>(), Zi.as<double>());
+        LAUNCH_CHECK("k_reduced_cyclic_inverse");
+        k_pack_ppt_cyclic<<<(ntp + 63) / 64, 64, 0, st>>>(nsets, P, pl.KB, Zi.as<double>(), pl.G, pl.band);
+        LAUNCH_CHECK("k_pack_ppt_cyclic");
+        CUDA_TRY(cudaStreamSynchronize(st));
     } else {
         const int K = 2 * (P - 1);
         DevBuf Z, Zi, piv;
@@ -229,8 +250,11 @@ tdx_status_t get_plan(tdx_grid* g, int kind, int dir, int mode, int P, double al
         if (P < 1 || P > TDX_MAX_P || n / P < 2) return fail(TDX_ERR_BAD_PARTITION, "P=%d invalid for line length %d (need 1 <= P <= %d, floor(n/P) >= 2)", P, n, TDX_MAX_P);
     }
     if (thomas) { P = 1; mode = TDX_MODE_THOMAS; }
-    const bool cyc = (kind == KIND_USER) || (kind == KIND_ADI && g->bc[dir] == TDX_BC_PERIODIC);
-    if (cyc && n < 3) return fail(TDX_ERR_INVALID_ARG, "periodic line needs n >= 3");
+    const bool periodic = (kind == KIND_USER) || (kind == KIND_ADI && g->bc[dir] == TDX_BC_PERIODIC);
+    if (periodic && n < 3) return fail(TDX_ERR_INVALID_ARG, "periodic line needs n >= 3");
+    // PPT closes a periodic line inside the (then cyclic) reduced system; PDD and Thomas use Sherman-Morrison (Eq.(3), rank 1)
+    const bool wrap = periodic && !thomas && mode == TDX_MODE_PPT && P >= 2 && P <= 128;
+    const bool cyc = periodic && !wrap;
     int M = 0;
     if (!thomas) {
         const int maxlen = n / P + (n % P ? 1 : 0);
@@ -245,7 +269,7 @@ tdx_status_t get_plan(tdx_grid* g, int kind, int dir, int mode, int P, double al
         if (p.kind == kind && p.dir == dir && p.mode == mode && p.P == P && p.nsets == nsets && p.hash == h &&
             std::memcmp(&p.alpha, &alpha, 8) == 0) { *out = &p; return TDX_OK; }
     Plan pl;
-    pl.kind = kind; pl.dir = dir; pl.mode = mode; pl.P = P; pl.n = n; pl.nsets = nsets; pl.M = M; pl.cyc = cyc;
+    pl.kind = kind; pl.dir = dir; pl.mode = mode; pl.P = P; pl.n = n; pl.nsets = nsets; pl.M = M; pl.cyc = cyc; pl.wrap = wrap;
     pl.thomas = thomas; pl.alpha = alpha; pl.hash = h; pl.sms = g->sms;
     tdx_status_t rc = build_plan(g, pl, lambda_host, ua, ub, uc, st);
     if (rc != TDX_OK) { pl.release(); return rc; }
@@ -276,7 +300,7 @@ tdx_status_t launch_strided_inst(const Plan& pl, StridedArgs& A, const Tables& T
     if (pl.pf < 0) {                                               // prefetch one wave of resident CTAs ahead
         int occ = 1;
         CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_strided<M, V, CYC>, (int)(block.x * block.y), smem));
-        pl.pf = pl.sms * (occ < 1 ? 1 : occ);
+        pl.pf = pl.sms * (occ < 1 ? 1 : occ) * prefetch_waves();
     }
     A.pf = pl.pf;
     k_strided<M, V, CYC><<<grid, block, smem, st>>>(A, T);
@@ -324,11 +348,15 @@ tdx_status_t run_strided(const Plan& pl, double* data, long long W, long long li
     }
     // CTA shape: LPC line-vectors x P partitions.  Row segments of 128 bytes (LPC*V = 16 doubles) and small CTAs (several
     // resident per SM) measured best; LPC grows only to reach 128 threads, shrinks when the register budget says so.
+    // Rows far apart in memory (z lines: stride = one xy-plane) like longer row segments; measured on cfg5 z.
+    static const int env_row = [] { const char* e = std::getenv("TDX_ROW_DOUBLES"); return e ? std::atoi(e) : 0; }();
+    int row_doubles = (line_stride * 8 >= (1 << 20)) ? 32 : 16;
+    if (env_row == 16 || env_row == 32 || env_row == 64) row_doubles = env_row;
     auto pick = [&](int V, int& LPC) -> bool {
         const int bt = strided_block_threads(pl.M, V);
         if (bt < pl.P || (V == 2 && (!even || pl.M > 32))) return false;
         int lmax = pow2floor(bt / pl.P); if (lmax > 32) lmax = 32;
-        int l = 16 / V;
+        int l = row_doubles / V;
         while (l * pl.P < 128 && l < 32) l *= 2;
         if (l > lmax) l = lmax;
         LPC = l;
@@ -401,7 +429,7 @@ tdx_status_t launch_unit_tma_inst(const Plan& pl, UnitTmaArgs& A, const Tables& 
     if (pl.pf < 0) {
         int occ = 1;
         CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_unit_tma<M, UNI, CYC>, threads, smem));
-        pl.pf = pl.sms * (occ < 1 ? 1 : occ);
+        pl.pf = pl.sms * (occ < 1 ? 1 : occ) * prefetch_waves();
     }
     A.pf = pl.pf;
     UniTable<M> U;

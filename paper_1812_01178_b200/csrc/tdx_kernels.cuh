@@ -136,9 +136,11 @@ k_strided(StridedArgs A, Tables T) {
         const double* gr = T.G + ((size_t)(set * 2 + 1) * T.KB) * P + p;
         for (int k = 0; k < bd.y; ++k) {
             const double a = __ldg(gl + (size_t)k * P), b = __ldg(gr + (size_t)k * P);
+            int idx = bd.x + k;                             // band may wrap around (periodic line closed inside Z)
+            if (idx >= 2 * P) idx -= 2 * P;
 #pragma unroll
             for (int v = 0; v < V; ++v) {
-                const double rv = rs[((bd.x + k) * LPC + tx) * V + v];
+                const double rv = rs[(idx * LPC + tx) * V + v];
                 yL[v] = fma(a, rv, yL[v]);
                 yR[v] = fma(b, rv, yR[v]);
             }
@@ -242,7 +244,8 @@ k_unit(UnitArgs A, Tables T) {
         const double* gr = T.G + (size_t)T.KB * P + p;
         const int lb = ll * P;
         for (int k = 0; k < bd.y; ++k) {
-            const int idx = bd.x + k;
+            int idx = bd.x + k;
+            if (idx >= 2 * P) idx -= 2 * P;                              // band may wrap (periodic line closed inside Z)
             const double rv = (idx & 1) ? rl[lb + (idx >> 1)] : rf[lb + (idx >> 1)];
             yL = fma(__ldg(gl + (size_t)k * P), rv, yL);
             yR = fma(__ldg(gr + (size_t)k * P), rv, yR);

@@ -119,7 +119,7 @@ __global__ void k_cyclic_q(int n, int nsets, const double* __restrict__ a, const
 // ends[(set*P+p)*4 + {0:v_first, 1:v_last, 2:w_first, 3:w_last}].  M = padded rows per partition (identity rows).
 // pinned sets (flags): d_0 := 0 is encoded as inv_0 := 0, l_1 := 0.
 template <int MAXROWS>
-__global__ void k_factor(int n, int nsets, int P, int M, int layout,
+__global__ void k_factor(int n, int nsets, int P, int M, int layout, int wrap,
                          const double* __restrict__ a, const double* __restrict__ b, const double* __restrict__ c,
                          const double* __restrict__ qv, const int* __restrict__ flags,
                          double* __restrict__ rows, double* __restrict__ ends) {
@@ -146,8 +146,9 @@ __global__ void k_factor(int n, int nsets, int P, int M, int layout,
     }
     // spikes (Eq.(6)); for a uniform table the representative partition keeps both spikes, G zeroes the unused side
     double v[MAXROWS], w[MAXROWS];
-    bool has_v = (p > 0) || uniform_only, has_w = (p < P - 1) || uniform_only;
-    if (P == 1) { has_v = has_w = false; }
+    // wrap: periodic line closed inside the reduced system -- partition 0 couples to row n-1 through a_0, partition P-1 to row 0
+    bool has_v = (p > 0) || uniform_only || wrap, has_w = (p < P - 1) || uniform_only || wrap;
+    if (P == 1 && !wrap) { has_v = has_w = false; }
     {   // v: rhs a_first e_first
         double y = has_v ? as[0] : 0.0;
         v[0] = y;
@@ -160,9 +161,9 @@ __global__ void k_factor(int n, int nsets, int P, int M, int layout,
     }
     if (pinned) { inv[0] = 0.0; if (m > 1) l[1] = 0.0; }
     double* e = ends + (size_t)t * 4;
-    e[0] = (p > 0) ? v[0] : 0.0; e[1] = (p > 0) ? v[m - 1] : 0.0;
-    e[2] = (p < P - 1) ? w[0] : 0.0; e[3] = (p < P - 1) ? w[m - 1] : 0.0;
-    if (P == 1) { e[0] = e[1] = e[2] = e[3] = 0.0; }
+    e[0] = (p > 0 || wrap) ? v[0] : 0.0; e[1] = (p > 0 || wrap) ? v[m - 1] : 0.0;
+    e[2] = (p < P - 1 || wrap) ? w[0] : 0.0; e[3] = (p < P - 1 || wrap) ? w[m - 1] : 0.0;
+    if (P == 1 && !wrap) { e[0] = e[1] = e[2] = e[3] = 0.0; }
     if (!writer) return;
     // Padding rows jj >= m (never loaded or stored: their d is 0) carry the partition's last value along:
     // l = -1 copies y_{m-1} forward, inv = inv_{m-1} and cp = 0 turn it into xt_{m-1} in the backward pass, so that
@@ -313,6 +314,96 @@ __global__ void k_pack_ppt(int nsets, int P, int KB, const double* __restrict__ 
         if (k < cnt) {
             if (rowL >= 0) gl = zi[(size_t)rowL * K + lo + k];
             if (rowR >= 0) gr = zi[(size_t)rowR * K + lo + k];
+        }
+        G[((size_t)(s * 2 + 0) * KB + k) * P + p] = gl;
+        G[((size_t)(s * 2 + 1) * KB + k) * P + p] = gr;
+    }
+}
+
+
+// ---- a3 + a5 for PPT on periodic lines: the wrap-around corner entries a_0, c_{n-1} join Delta A, so
+// there are P interfaces instead of P-1 and Z (L112-116) becomes a cyclic 2P x 2P matrix; Woodbury (Eq.(3)-(4)) is still
+// exact and the sweep kernel needs no separate Sherman-Morrison correction.  Unknowns: u_{2p} = x_{last_p},
+// u_{(2p-1) mod K} = x_{first_p}, K = 2P; the right-hand side of row k is r[(k+1) mod K] (r[2p] = xt_first^(p),
+// r[2p+1] = xt_last^(p)).  Dense LU with partial pivoting, one thread per set (plan time, K <= 256).
+__global__ void k_reduced_cyclic_factor(int nsets, int P, const double* __restrict__ ends, double* __restrict__ Z, int* __restrict__ piv) {
+    int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= nsets) return;
+    const int K = 2 * P;
+    double* z = Z + (size_t)s * K * K;
+    int* pv = piv + (size_t)s * K;
+    const double* e = ends + (size_t)s * P * 4;
+    for (int i = 0; i < K * K; ++i) z[i] = 0.0;
+    for (int p = 0; p < P; ++p) {
+        const int rl = 2 * p, rf = (2 * p - 1 + K) % K;
+        const int cL = (2 * p - 2 + K) % K, cR = (2 * p + 1) % K;          // x_last_{p-1}, x_first_{p+1}
+        z[(size_t)rl * K + rl] += 1.0; z[(size_t)rl * K + cL] += e[p * 4 + 1]; z[(size_t)rl * K + cR] += e[p * 4 + 3];
+        z[(size_t)rf * K + rf] += 1.0; z[(size_t)rf * K + cL] += e[p * 4 + 0]; z[(size_t)rf * K + cR] += e[p * 4 + 2];
+    }
+    for (int k = 0; k < K; ++k) {
+        int pr = k; double best = fabs(z[(size_t)k * K + k]);
+        for (int i = k + 1; i < K; ++i) { double t = fabs(z[(size_t)i * K + k]); if (t > best) { best = t; pr = i; } }
+        pv[k] = pr;
+        if (pr != k) for (int cc = 0; cc < K; ++cc) { double t = z[(size_t)k * K + cc]; z[(size_t)k * K + cc] = z[(size_t)pr * K + cc]; z[(size_t)pr * K + cc] = t; }
+        const double d = z[(size_t)k * K + k];
+        for (int i = k + 1; i < K; ++i) {
+            const double f = z[(size_t)i * K + k] / d;
+            z[(size_t)i * K + k] = f;
+            if (f != 0.0) for (int cc = k + 1; cc < K; ++cc) z[(size_t)i * K + cc] -= f * z[(size_t)k * K + cc];
+        }
+    }
+}
+
+// column col of Z^{-1} from the dense LU (rows were swapped in full, LAPACK style); one thread per (set, col)
+__global__ void k_reduced_cyclic_inverse(int nsets, int P, const double* __restrict__ Z, const int* __restrict__ piv, double* __restrict__ Zi) {
+    const int K = 2 * P;
+    long t = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= (long)nsets * K) return;
+    int s = (int)(t / K), col = (int)(t % K);
+    const double* z = Z + (size_t)s * K * K;
+    const int* pv = piv + (size_t)s * K;
+    double* x = Zi + (size_t)s * K * K;
+    for (int i = 0; i < K; ++i) x[(size_t)i * K + col] = (i == col) ? 1.0 : 0.0;
+    for (int k = 0; k < K; ++k) {                            // apply the row interchanges, then L^{-1}
+        int pr = pv[k];
+        if (pr != k) { double tmp = x[(size_t)k * K + col]; x[(size_t)k * K + col] = x[(size_t)pr * K + col]; x[(size_t)pr * K + col] = tmp; }
+    }
+    for (int k = 0; k < K; ++k) {
+        const double xk = x[(size_t)k * K + col];
+        if (xk != 0.0) for (int i = k + 1; i < K; ++i) x[(size_t)i * K + col] -= z[(size_t)i * K + k] * xk;
+    }
+    for (int i = K - 1; i >= 0; --i) {
+        double acc = x[(size_t)i * K + col];
+        for (int cc = i + 1; cc < K; ++cc) acc -= z[(size_t)i * K + cc] * x[(size_t)cc * K + col];
+        x[(size_t)i * K + col] = acc / z[(size_t)i * K + i];
+    }
+}
+
+// Partition p needs yL = x_{last_{p-1}} = u_{(2p-2) mod K} and yR = x_{first_{p+1}} = u_{(2p+1) mod K}.  The band is a
+// cyclic window of r indices around 2p: band = {lo, cnt}, entry k <-> r[(lo + k) mod K] <-> Z^{-1} column (lo + k - 1) mod K.
+__global__ void k_pack_ppt_cyclic(int nsets, int P, int KB, const double* __restrict__ Zi, double* __restrict__ G, int2* __restrict__ band) {
+    int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= nsets * P) return;
+    int s = t / P, p = t % P;
+    const int K = 2 * P;
+    const double* zi = Zi + (size_t)s * K * K;
+    const double tau = 1e-24;
+    const int rowL = (2 * p - 2 + K) % K, rowR = (2 * p + 1) % K;
+    double mxL = 0.0, mxR = 0.0;
+    for (int cc = 0; cc < K; ++cc) { mxL = fmax(mxL, fabs(zi[(size_t)rowL * K + cc])); mxR = fmax(mxR, fabs(zi[(size_t)rowR * K + cc])); }
+    int dl = 0, dr = 0;
+    for (int d = -(K / 2); d < K - K / 2; ++d) {
+        const int ri = ((2 * p + d) % K + K) % K, cc = (ri - 1 + K) % K;
+        if (fabs(zi[(size_t)rowL * K + cc]) > tau * mxL || fabs(zi[(size_t)rowR * K + cc]) > tau * mxR) { if (-d > dl) dl = -d; if (d > dr) dr = d; }
+    }
+    int cnt = dl + dr + 1; if (cnt > K) cnt = K;
+    const int lo = ((2 * p - dl) % K + K) % K;
+    band[t] = make_int2(lo, cnt);
+    for (int k = 0; k < KB; ++k) {
+        double gl = 0.0, gr = 0.0;
+        if (k < cnt) {
+            const int cc = ((lo + k) % K - 1 + K) % K;
+            gl = zi[(size_t)rowL * K + cc]; gr = zi[(size_t)rowR * K + cc];
         }
         G[((size_t)(s * 2 + 0) * KB + k) * P + p] = gl;
         G[((size_t)(s * 2 + 1) * KB + k) * P + p] = gr;

@@ -137,7 +137,8 @@ k_unit_tma(const __grid_constant__ CUtensorMap tmap, UnitTmaArgs A, Tables T, co
         const double* gr = T.G + (size_t)T.KB * P + p;
         const int lb = ll * P;
         for (int k = 0; k < bd.y; ++k) {
-            const int idx = bd.x + k;
+            int idx = bd.x + k;
+            if (idx >= 2 * P) idx -= 2 * P;                              // band may wrap (periodic line closed inside Z)
             const double rv = (idx & 1) ? rl[lb + (idx >> 1)] : rf[lb + (idx >> 1)];
             yL = fma(__ldg(gl + (size_t)k * P), rv, yL);
             yR = fma(__ldg(gr + (size_t)k * P), rv, yR);
