@@ -21,7 +21,7 @@ namespace tdx {
 
 struct Tables {
     const double* rows;      // row table (layout depends on the kernel), fields {l, q, inv, cp, v, w}
-    const double* G;         // reduced coefficients G[((set*2+side)*KB + k)*P + p]
+    const double* G;         // reduced coefficients, pairs {gL, gR}: G[g_index(set, side, k, p, KB, P)]
     const int2* band;        // band[set*P + p] = {lo, cnt} in interface-rhs indices r[0..2P)
     const int* Sidx;         // cyclic closure functional (sparse), Sidx/Sval[set*Scap + k], Sn[set]
     const double* Sval;
@@ -99,6 +99,18 @@ k_strided(StridedArgs A, Tables T) {
             }
         }
     }
+    // One table set per outer index (Helmholtz: a set per wavenumber): this CTA's set is cold in L1, so pull its lines
+    // in now, one prefetch per thread, while the data loads are in flight -- otherwise every table load on the
+    // dependent chain and in the band loop pays L2 latency.
+    if (A.set_per_outer) {
+        const int tid = p * LPC + tx, nth = LPC * P;
+        const char* rb = reinterpret_cast<const char*>(T.rows + (size_t)set * P * MAXM * 6);
+        const int rlines = (P * MAXM * 48 + 127) >> 7;
+        for (int k = tid; k < rlines; k += nth) asm volatile("prefetch.global.L1 [%0];" ::"l"(rb + ((size_t)k << 7)));
+        const char* gb = reinterpret_cast<const char*>(T.G + (size_t)set * 2 * T.KB * P);
+        const int glines = (2 * T.KB * P * 8 + 127) >> 7;
+        for (int k = tid; k < glines; k += nth) asm volatile("prefetch.global.L1 [%0];" ::"l"(gb + ((size_t)k << 7)));
+    }
     const double2* rt = reinterpret_cast<const double2*>(T.rows + ((size_t)((size_t)set * P + p) * MAXM) * 6);
 
     // Eq.(5): forward y_j = d_j - l_j y_{j-1}, backward xt_j = y_j inv_j - cp_j xt_{j+1}
@@ -132,10 +144,10 @@ k_strided(StridedArgs A, Tables T) {
     for (int v = 0; v < V; ++v) { yL[v] = 0.0; yR[v] = 0.0; sc[v] = 0.0; }
     {
         const int2 bd = __ldg(&T.band[set * P + p]);
-        const double* gl = T.G + ((size_t)(set * 2 + 0) * T.KB) * P + p;
-        const double* gr = T.G + ((size_t)(set * 2 + 1) * T.KB) * P + p;
+        const double2* g2 = reinterpret_cast<const double2*>(T.G) + (size_t)set * T.KB * P + p;
         for (int k = 0; k < bd.y; ++k) {
-            const double a = __ldg(gl + (size_t)k * P), b = __ldg(gr + (size_t)k * P);
+            const double2 ab = __ldg(g2 + (size_t)k * P);   // {gL, gR}
+            const double a = ab.x, b = ab.y;
             int idx = bd.x + k;                             // band may wrap around (periodic line closed inside Z)
             if (idx >= 2 * P) idx -= 2 * P;
 #pragma unroll
@@ -240,15 +252,15 @@ k_unit(UnitArgs A, Tables T) {
     double yL = 0.0, yR = 0.0, sc = 0.0;
     if (valid) {
         const int2 bd = __ldg(&T.band[p]);
-        const double* gl = T.G + p;
-        const double* gr = T.G + (size_t)T.KB * P + p;
+        const double2* g2 = reinterpret_cast<const double2*>(T.G) + p;
         const int lb = ll * P;
         for (int k = 0; k < bd.y; ++k) {
             int idx = bd.x + k;
             if (idx >= 2 * P) idx -= 2 * P;                              // band may wrap (periodic line closed inside Z)
             const double rv = (idx & 1) ? rl[lb + (idx >> 1)] : rf[lb + (idx >> 1)];
-            yL = fma(__ldg(gl + (size_t)k * P), rv, yL);
-            yR = fma(__ldg(gr + (size_t)k * P), rv, yR);
+            const double2 ab = __ldg(g2 + (size_t)k * P);                // {gL, gR}
+            yL = fma(ab.x, rv, yL);
+            yR = fma(ab.y, rv, yR);
         }
         if (CYC) {
             const int ns = __ldg(&T.Sn[0]);

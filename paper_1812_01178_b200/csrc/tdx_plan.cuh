@@ -27,6 +27,8 @@ enum RowLayout { ROWS_PJ = 0,      // rows[((set*P + p)*M + jj)*6 + f]   strided
 enum RowField { F_L = 0, F_Q = 1, F_INV = 2, F_CP = 3, F_V = 4, F_W = 5 };
 
 __host__ __device__ inline int part_start(int p, int q, int r) { return p * q + (p < r ? p : r); }
+// reduced-system coefficients: pairs {gL, gR} per (set, band entry k, partition p) -- one 16-byte load per band entry
+__host__ __device__ inline size_t g_index(int set, int side, int k, int p, int KB, int P) { return ((((size_t)set * KB + k) * P + p) << 1) + side; }
 
 __device__ inline size_t row_index(int layout, int set, int P, int M, int p, int jj, int f) {
     if (layout == ROWS_PJ) return ((size_t)((size_t)set * P + p) * M + jj) * 6 + f;
@@ -289,7 +291,7 @@ __global__ void k_reduced_inverse(int nsets, int P, const double* __restrict__ Z
 
 // Interface right-hand sides live in r[0..2P): r[2p] = xt_first^(p), r[2p+1] = xt_last^(p); Z column k <-> r[k+1].
 // Partition p needs yL = x_{last_{p-1}} = u_{2p-2} (p >= 1) and yR = x_{first_{p+1}} = u_{2p+1} (p <= P-2).
-// G[((set*2+side)*KB + k)*P + p], band[(set*P+p)] = {lo (r index), cnt}: yL = sum_k G[0][k] r[lo+k], yR likewise.
+// G[g_index(set, side, k, p)] (pairs {gL, gR}), band[(set*P+p)] = {lo (r index), cnt}: yL = sum_k G[0][k] r[lo+k], yR likewise.
 // PPT: rows of Z^{-1}, entries below tau * rowmax dropped (invisible in fp64), union band of the two rows.
 __global__ void k_pack_ppt(int nsets, int P, int KB, const double* __restrict__ Zi, double* __restrict__ G, int2* __restrict__ band) {
     int t = blockIdx.x * blockDim.x + threadIdx.x;
@@ -315,8 +317,8 @@ __global__ void k_pack_ppt(int nsets, int P, int KB, const double* __restrict__ 
             if (rowL >= 0) gl = zi[(size_t)rowL * K + lo + k];
             if (rowR >= 0) gr = zi[(size_t)rowR * K + lo + k];
         }
-        G[((size_t)(s * 2 + 0) * KB + k) * P + p] = gl;
-        G[((size_t)(s * 2 + 1) * KB + k) * P + p] = gr;
+        G[g_index(s, 0, k, p, KB, P)] = gl;
+        G[g_index(s, 1, k, p, KB, P)] = gr;
     }
 }
 
@@ -405,8 +407,8 @@ __global__ void k_pack_ppt_cyclic(int nsets, int P, int KB, const double* __rest
             const int cc = ((lo + k) % K - 1 + K) % K;
             gl = zi[(size_t)rowL * K + cc]; gr = zi[(size_t)rowR * K + cc];
         }
-        G[((size_t)(s * 2 + 0) * KB + k) * P + p] = gl;
-        G[((size_t)(s * 2 + 1) * KB + k) * P + p] = gr;
+        G[g_index(s, 0, k, p, KB, P)] = gl;
+        G[g_index(s, 1, k, p, KB, P)] = gr;
     }
 }
 
@@ -436,8 +438,8 @@ __global__ void k_pack_pdd(int nsets, int P, int KB, const double* __restrict__ 
     for (int k = 0; k < KB; ++k) {
         double gl = 0.0, gr = 0.0;
         if (k < k1 - k0) { gl = g[0][k0 + k]; gr = g[1][k0 + k]; }
-        G[((size_t)(s * 2 + 0) * KB + k) * P + p] = gl;
-        G[((size_t)(s * 2 + 1) * KB + k) * P + p] = gr;
+        G[g_index(s, 0, k, p, KB, P)] = gl;
+        G[g_index(s, 1, k, p, KB, P)] = gr;
     }
 }
 
@@ -459,11 +461,11 @@ __global__ void k_cyclic_functional(int nsets, int P, int KB, int Scap, const do
         double wf0 = e[0 * 4 + 2], vlP = e[(P - 1) * 4 + 1];
         int2 b0 = band[s * P + 0], bP = band[s * P + P - 1];
         for (int k = 0; k < b0.y; ++k) {
-            double gv = G[((size_t)(s * 2 + 1) * KB + k) * P + 0];
+            double gv = G[g_index(s, 1, k, 0, KB, P)];
             if (gv != 0.0) { si[n] = b0.x + k; sv[n] = -kappa * wf0 * gv; ++n; }
         }
         for (int k = 0; k < bP.y; ++k) {
-            double gv = G[((size_t)(s * 2 + 0) * KB + k) * P + (P - 1)];
+            double gv = G[g_index(s, 0, k, P - 1, KB, P)];
             if (gv != 0.0) { si[n] = bP.x + k; sv[n] = -kappa * g * vlP * gv; ++n; }
         }
     }

@@ -133,15 +133,15 @@ k_unit_tma(const __grid_constant__ CUtensorMap tmap, UnitTmaArgs A, Tables T, co
     double yL = 0.0, yR = 0.0, sc = 0.0;
     if (valid) {
         const int2 bd = __ldg(&T.band[p]);
-        const double* gl = T.G + p;
-        const double* gr = T.G + (size_t)T.KB * P + p;
+        const double2* g2 = reinterpret_cast<const double2*>(T.G) + p;
         const int lb = ll * P;
         for (int k = 0; k < bd.y; ++k) {
             int idx = bd.x + k;
             if (idx >= 2 * P) idx -= 2 * P;                              // band may wrap (periodic line closed inside Z)
             const double rv = (idx & 1) ? rl[lb + (idx >> 1)] : rf[lb + (idx >> 1)];
-            yL = fma(__ldg(gl + (size_t)k * P), rv, yL);
-            yR = fma(__ldg(gr + (size_t)k * P), rv, yR);
+            const double2 ab = __ldg(g2 + (size_t)k * P);                // {gL, gR}
+            yL = fma(ab.x, rv, yL);
+            yR = fma(ab.y, rv, yR);
         }
         if (CYC) {
             const int ns = __ldg(&T.Sn[0]);
