@@ -29,6 +29,13 @@ METRIC = "Gpts/s per ADI sweep direction (fp64 PDD/PPT); achieved HBM GB/s vs pe
 UNIT = "Gpts/s"
 BYTES_PER_POINT = 16.0          # 8 B read + 8 B written per real grid value per sweep
 
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures
+# (profiles/r1_ncu_cfg5_summary.md), valid for mode ppt with the tuned P of the config; bytes.
+NCU_TRAFFIC = {
+    "cfg5_4096x288x512": {"adi_x": 9.607577e9, "adi_y": 9.604446e9, "adi_z_cyclic": 9.623135e9, "helmholtz_y": 9.654605e9},
+    "cfg4_1024x512x256": {"adi_x": 2.088804e9, "adi_y": 2.089366e9, "adi_z_cyclic": 2.099430e9, "helmholtz_y": 2.110119e9},
+}
+
 # tuned partitions per line (x, y, z, helmholtz-y) per config; rows per partition <= 64
 TUNED_P = {1: (4, 4, 4, 4), 2: (16, 8, 8, 8), 3: (32, 8, 8, 8), 4: (64, 16, 8, 16), 5: (256, 24, 16, 12)}
 
@@ -282,8 +289,11 @@ def run_tdx(args, rank, world, local_rank):
                       "frac_of_nominal_8TBs": BYTES_PER_POINT * pts[k] / (kms[k] * 1e-3) / 1e9 / 8000.0, "P": Ps[k]} for k, n in enumerate(names)}
     dom = int(np.argmax(kms))
     achieved = BYTES_PER_POINT * pts[dom] / (kms[dom] * 1e-3) / 1e9
+    tuned = (Ps == TUNED_P[args.config]) and args.mode == "ppt"
+    traffic = NCU_TRAFFIC.get(cfg.name, {}).get(names[dom]) if tuned else None
     roofline = {"bound": "hbm", "kernel": names[dom], "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": None, "peak_source": peak_src, "algorithmic_bytes_per_launch": BYTES_PER_POINT * pts[dom],
+                "traffic": traffic, "traffic_source": "profiles/r1_ncu_cfg5_summary.md (ncu --set full, per launch)" if traffic else None,
+                "peak_source": peak_src, "algorithmic_bytes_per_launch": BYTES_PER_POINT * pts[dom],
                 "share_of_step": kms[dom] / sum(kms)}
 
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
