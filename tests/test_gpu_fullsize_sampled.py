@@ -1,0 +1,112 @@
+"""Parity at BASELINE.json's full sizes, in the launch configuration bench.py times (its TUNED_P, mode PPT and PDD):
+the whole sweep runs on the GPU; randomly sampled lines are checked one by one against the oracle's single-line
+solvers (Thomas / cyclic Thomas on the oracle's own coefficients).  Tolerances as in test_gpu_parity.py; error norm =
+max over the sampled lines relative to the max of the sampled exact solutions (A14)."""
+import importlib.util
+import os
+
+import numpy as np
+import pytest
+import torch
+
+import oracle as orc
+from paper_1812_01178_b200 import binding as tdx
+from paper_1812_01178_b200 import configs
+
+pytestmark = pytest.mark.gpu
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+_spec = importlib.util.spec_from_file_location("bench_module", os.path.join(ROOT, "bench.py"))
+bench = importlib.util.module_from_spec(_spec)
+_spec.loader.exec_module(bench)
+
+BCS = (tdx.BC_DIRICHLET, tdx.BC_DIRICHLET, tdx.BC_PERIODIC)
+NSAMPLE = 96
+
+
+def _need(nbytes):
+    free, _ = torch.cuda.mem_get_info()
+    if free < nbytes:
+        pytest.skip("not enough free device memory for this full-size case")
+
+
+def _sample_lines(t, direction, picks):
+    """t: [nz, ny, nx] device tensor; returns host array [len(picks), n_dir] of the picked lines."""
+    a, b = picks[:, 0], picks[:, 1]
+    ia, ib = torch.from_numpy(a).cuda(), torch.from_numpy(b).cuda()
+    if direction == 0:
+        return t[ia, ib, :].cpu().numpy()                       # picks = (k, j)
+    if direction == 1:
+        return t[ia, :, ib].cpu().numpy()                       # picks = (k, i)
+    return t[:, ia, ib].t().contiguous().cpu().numpy()          # picks = (j, i)
+
+
+def _picks(rng, direction, nx, ny, nz):
+    dims = {0: (nz, ny), 1: (nz, nx), 2: (ny, nx)}[direction]
+    p = np.stack([rng.integers(0, dims[0], NSAMPLE), rng.integers(0, dims[1], NSAMPLE)], axis=1)
+    p[0] = (0, 0); p[1] = (dims[0] - 1, dims[1] - 1)            # corners: first and last line of the field
+    return p
+
+
+@pytest.mark.parametrize("cfg_no", [4, 5])
+@pytest.mark.parametrize("mode_name", ["ppt", "pdd"])
+def test_adi_sweeps_fullsize_sampled_lines(cfg_no, mode_name):
+    c = configs.get(cfg_no)
+    _need(int(c.npts * 8 * 1.3))
+    Ps = bench.TUNED_P[cfg_no]
+    mode = {"ppt": tdx.MODE_PPT, "pdd": tdx.MODE_PDD}[mode_name]
+    faces = c.faces()
+    grid = tdx.Grid(c.nx, c.ny, c.nz, *faces, bcs=BCS)
+    t = torch.from_numpy(c.rhs_field()).cuda()
+    rng = np.random.default_rng(100 + cfg_no)
+    for direction in (0, 1, 2):
+        picks = _picks(rng, direction, c.nx, c.ny, c.nz)
+        din = _sample_lines(t, direction, picks)
+        grid.adi_sweep(direction, mode, Ps[direction], c.alpha, t)
+        torch.cuda.synchronize()
+        got = _sample_lines(t, direction, picks)
+        a, b, cc = orc.adi_coeffs(faces[direction], BCS[direction], c.alpha)
+        solve = orc.cyclic_thomas if BCS[direction] == orc.BC_PERIODIC else orc.thomas
+        ref = np.stack([solve(a, b, cc, d) for d in din])
+        err = float(np.max(np.abs(got - ref)) / np.max(np.abs(ref)))
+        if mode_name == "ppt":
+            assert err < 1e-12, (cfg_no, direction, err)
+        else:
+            dropped = grid.pdd_dropped_bound(direction, Ps[direction], c.alpha)
+            assert err < (1e-10 if dropped <= 1e-11 else 100 * dropped + 1e-10), (cfg_no, direction, err, dropped)
+    grid.close()
+
+
+@pytest.mark.parametrize("cfg_no", [4, 5])
+def test_helmholtz_fullsize_sampled_lines(cfg_no):
+    c = configs.get(cfg_no)
+    _need(int(c.nx * c.ny * c.nm * 16 * 1.3))
+    P = bench.TUNED_P[cfg_no][3]
+    faces = c.faces()
+    kz2 = c.kz2()
+    grid = tdx.Grid(c.nx, c.ny, c.nz, *faces, bcs=BCS)
+    t = torch.from_numpy(c.rhs_helmholtz()).cuda()              # [nm, ny, nx] complex128
+    tv = torch.view_as_real(t)                                  # [nm, ny, nx, 2]
+    rng = np.random.default_rng(200 + cfg_no)
+    ms = np.concatenate([[0, 1, 2, c.nm - 1], rng.integers(0, c.nm, NSAMPLE - 4)])
+    xs = np.concatenate([[0, c.nx - 1, 5, 7], rng.integers(0, c.nx, NSAMPLE - 4)])
+    im_, ix_ = torch.from_numpy(ms).cuda(), torch.from_numpy(xs).cuda()
+    din = tv[im_, :, ix_, :].cpu().numpy()                      # [S, ny, 2]
+    grid.helmholtz_wavenumber_solve(tdx.MODE_PPT, P, None, kz2, t)
+    torch.cuda.synchronize()
+    got = tv[im_, :, ix_, :].cpu().numpy()
+    ref = np.empty_like(got)
+    for s, m in enumerate(ms):
+        a, b, cc, pinned = orc.helmholtz_coeffs(faces[1], float(kz2[m]))
+        for part in (0, 1):
+            d = din[s, :, part].copy()
+            if pinned:
+                d[0] = 0.0
+            ref[s, :, part] = orc.thomas(a, b, cc, d)
+    for s, m in enumerate(ms):                                  # per line: low modes are large and must not hide the rest
+        e = float(np.max(np.abs(got[s] - ref[s])) / np.max(np.abs(ref[s])))
+        assert e < 1e-11, (cfg_no, int(m), int(xs[s]), e)
+    err = float(np.max(np.abs(got - ref)) / np.max(np.abs(ref)))
+    assert err < 1e-12, (cfg_no, err)
+    assert np.all(got[ms == 0][:, 0, :] == 0.0)                 # pinned points of the zero mode
+    grid.close()
