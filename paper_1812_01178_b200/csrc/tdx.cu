@@ -302,7 +302,8 @@ tdx_status_t launch_strided_inst(const Plan& pl, StridedArgs& A, const Tables& T
         CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_strided<M, V, CYC>, (int)(block.x * block.y), smem));
         pl.pf = pl.sms * (occ < 1 ? 1 : occ) * prefetch_waves();
     }
-    A.pf = pl.pf;
+    // one tile per CTA: pf = CTAs ahead; looping CTAs (grid.x < tiles_x): pf = sets ahead for the first tile of a later CTA
+    A.pf = ((int)grid.x == A.tiles_x) ? pl.pf : (pl.pf > 0 ? (pl.pf + (int)grid.x - 1) / (int)grid.x : 0);
     k_strided<M, V, CYC><<<grid, block, smem, st>>>(A, T);
     LAUNCH_CHECK("k_strided");
     return TDX_OK;
@@ -339,8 +340,8 @@ tdx_status_t run_strided(const Plan& pl, double* data, long long W, long long li
         const int V = even ? 2 : 1;
         A.W = W / V; A.line_stride = line_stride / V; A.outer_stride = outer_stride / V;
         const int tb = 128;
-        A.LPC = tb;
-        dim3 grid((unsigned)((A.W + tb - 1) / tb), (unsigned)O);
+        A.LPC = tb; A.tiles_x = (int)((A.W + tb - 1) / tb);
+        dim3 grid((unsigned)A.tiles_x, (unsigned)O);
         if (V == 2) { if (pl.cyc) k_thomas_strided<2, true><<<grid, tb, 0, st>>>(A, pl.rows, pl.cyc_tab, pl.n); else k_thomas_strided<2, false><<<grid, tb, 0, st>>>(A, pl.rows, pl.cyc_tab, pl.n); }
         else { if (pl.cyc) k_thomas_strided<1, true><<<grid, tb, 0, st>>>(A, pl.rows, pl.cyc_tab, pl.n); else k_thomas_strided<1, false><<<grid, tb, 0, st>>>(A, pl.rows, pl.cyc_tab, pl.n); }
         LAUNCH_CHECK("k_thomas_strided");
@@ -370,7 +371,18 @@ tdx_status_t run_strided(const Plan& pl, double* data, long long W, long long li
     A.W = W / V; A.line_stride = line_stride / V; A.outer_stride = outer_stride / V;
     while (LPC > 1 && LPC / 2 >= A.W) LPC /= 2;
     A.LPC = LPC;
-    dim3 block(LPC, pl.P), grid((unsigned)((A.W + LPC - 1) / LPC), (unsigned)O);
+    A.tiles_x = (int)((A.W + LPC - 1) / LPC);
+    // One table set per outer index (Helmholtz): a CTA works through several column tiles of its set, so the set's tables
+    // are fetched from L2 once per CTA instead of once per tile; keep >= ~16 waves of CTAs for balance.
+    int loops = 1;
+    if (set_per_outer) {
+        const long long total = (long long)A.tiles_x * O;
+        long long l = total / (16LL * pl.sms * 2);
+        loops = (int)(l < 1 ? 1 : (l > 4 ? 4 : l));                // measured: 4 tiles per CTA best on cfg4 and cfg5, 8+ loses balance
+        static const int env_loops = [] { const char* e = std::getenv("TDX_TILES_PER_CTA"); return e ? std::atoi(e) : 0; }();
+        if (env_loops >= 1 && env_loops <= 64) loops = env_loops;
+    }
+    dim3 block(LPC, pl.P), grid((unsigned)((A.tiles_x + loops - 1) / loops), (unsigned)O);
     const size_t smem = (size_t)2 * pl.P * LPC * V * 8;
     Tables T = tables_of(pl);
     if (V == 2) return pl.cyc ? launch_strided_M<2, true>(pl, A, T, grid, block, smem, st) : launch_strided_M<2, false>(pl, A, T, grid, block, smem, st);

@@ -36,7 +36,8 @@ struct StridedArgs {
     long long outer_stride;  // distance between outer indices, in V-vectors
     int set_per_outer;       // 1: table set = outer index (Helmholtz wavenumber), 0: one set
     int LPC;                 // lines (V-vectors) per CTA = blockDim.x
-    int pf;                  // L2 prefetch distance in CTAs (0 = off)
+    int pf;                  // L2 prefetch distance: CTAs ahead (one tile per CTA) or sets ahead (looping CTAs); 0 = off
+    int tiles_x;             // column tiles per outer index
 };
 
 template <int V> struct VecIO;
@@ -65,43 +66,15 @@ k_strided(StridedArgs A, Tables T) {
     extern __shared__ double rs[];                          // rs[(idx*LPC + tx)*V + v], idx in [0, 2P)
     const int tx = threadIdx.x, p = threadIdx.y;
     const int LPC = A.LPC, P = T.P;
-    const long long i = (long long)blockIdx.x * LPC + tx;
-    const bool valid = i < A.W;
     const int o = blockIdx.y;
     const int set = A.set_per_outer ? o : 0;
     const int start = part_start(p, T.q, T.r);
     const int m = T.q + (p < T.r ? 1 : 0);
     const bool full = (T.r == 0) && (T.q == MAXM);          // every partition has exactly MAXM rows (warp-uniform)
-    double* base = A.data + ((long long)o * A.outer_stride + (long long)start * A.line_stride + i) * V;
     const long long rstride = A.line_stride * V;
-
-    double x[MAXM][V];
-#pragma unroll
-    for (int jj = 0; jj < MAXM; ++jj) {
-        if (valid && (full || jj < m)) VecIO<V>::ld(base + jj * rstride, x[jj]);
-        else {
-#pragma unroll
-            for (int v = 0; v < V; ++v) x[jj][v] = 0.0;
-        }
-    }
-    // L2 prefetch of the tile a CTA `pf` launches later will load: one lane per 128-byte line.  The CTA that needs
-    // the data then finds it in L2 (~300 cycles) instead of HBM, so a few resident CTAs per SM keep HBM busy.
-    if (A.pf > 0 && ((tx * V) & 15) == 0) {
-        const long long lin = (long long)blockIdx.y * gridDim.x + blockIdx.x + A.pf;
-        if (lin < (long long)gridDim.x * gridDim.y) {
-            const int by = (int)(lin / gridDim.x), bx = (int)(lin - (long long)by * gridDim.x);
-            const long long ip = (long long)bx * LPC + tx;
-            if (ip < A.W) {
-                const double* pb = A.data + ((long long)by * A.outer_stride + (long long)start * A.line_stride + ip) * V;
-#pragma unroll
-                for (int jj = 0; jj < MAXM; ++jj)
-                    if (full || jj < m) asm volatile("prefetch.global.L2 [%0];" ::"l"(pb + jj * rstride));
-            }
-        }
-    }
     // One table set per outer index (Helmholtz: a set per wavenumber): this CTA's set is cold in L1, so pull its lines
-    // in now, one prefetch per thread, while the data loads are in flight -- otherwise every table load on the
-    // dependent chain and in the band loop pays L2 latency.
+    // in now, one prefetch per thread -- otherwise every table load on the dependent chain and in the band loop pays
+    // L2 latency.  Such a CTA then works through several column tiles of its set (the loop below) with warm tables.
     if (A.set_per_outer) {
         const int tid = p * LPC + tx, nth = LPC * P;
         const char* rb = reinterpret_cast<const char*>(T.rows + (size_t)set * P * MAXM * 6);
@@ -112,6 +85,43 @@ k_strided(StridedArgs A, Tables T) {
         for (int k = tid; k < glines; k += nth) asm volatile("prefetch.global.L1 [%0];" ::"l"(gb + ((size_t)k << 7)));
     }
     const double2* rt = reinterpret_cast<const double2*>(T.rows + ((size_t)((size_t)set * P + p) * MAXM) * 6);
+    const int tiles_x = A.tiles_x;
+
+  // column tiles of this CTA: exactly one when gridDim.x == tiles_x, else blockIdx.x, blockIdx.x + gridDim.x, ...
+  for (int xt = blockIdx.x; xt < tiles_x; xt += gridDim.x) {
+    const long long i = (long long)xt * LPC + tx;
+    const bool valid = i < A.W;
+    double* base = A.data + ((long long)o * A.outer_stride + (long long)start * A.line_stride + i) * V;
+
+    double x[MAXM][V];
+#pragma unroll
+    for (int jj = 0; jj < MAXM; ++jj) {
+        if (valid && (full || jj < m)) VecIO<V>::ld(base + jj * rstride, x[jj]);
+        else {
+#pragma unroll
+            for (int v = 0; v < V; ++v) x[jj][v] = 0.0;
+        }
+    }
+    // L2 prefetch of a tile that is loaded later -- by the CTA `pf` launches ahead (one tile per CTA), or by this CTA
+    // in its next iteration / by the CTA `pf` sets ahead (looping CTAs): one lane per 128-byte line.  Whoever needs the
+    // data then finds it in L2 (~300 cycles) instead of HBM, so a few resident CTAs per SM keep HBM busy.
+    if (A.pf > 0 && ((tx * V) & 15) == 0) {
+        int nbx, nby;
+        if ((int)gridDim.x == tiles_x) {
+            const long long lin = (long long)o * tiles_x + xt + A.pf;
+            nby = (int)(lin / tiles_x); nbx = (int)(lin - (long long)nby * tiles_x);
+        } else {
+            nbx = xt + gridDim.x; nby = o;
+            if (nbx >= tiles_x) { nbx = blockIdx.x; nby = o + A.pf; }
+        }
+        const long long ip = (long long)nbx * LPC + tx;
+        if (nby < (int)gridDim.y && ip < A.W) {
+            const double* pb = A.data + ((long long)nby * A.outer_stride + (long long)start * A.line_stride + ip) * V;
+#pragma unroll
+            for (int jj = 0; jj < MAXM; ++jj)
+                if (full || jj < m) asm volatile("prefetch.global.L2 [%0];" ::"l"(pb + jj * rstride));
+        }
+    }
 
     // Eq.(5): forward y_j = d_j - l_j y_{j-1}, backward xt_j = y_j inv_j - cp_j xt_{j+1}
 #pragma unroll
@@ -182,6 +192,8 @@ k_strided(StridedArgs A, Tables T) {
         }
         if (valid && (full || jj < m)) VecIO<V>::st(base + jj * rstride, x[jj]);
     }
+    if (xt + (int)gridDim.x < tiles_x) __syncthreads();     // rs is reused by the next tile
+  }
 }
 
 // ---------------------------------------------------------------------------------------------------------
