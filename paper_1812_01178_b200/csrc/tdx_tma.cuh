@@ -90,6 +90,7 @@ k_unit_tma(const __grid_constant__ CUtensorMap tmap, UnitTmaArgs A, Tables T, co
     const long long row0 = (long long)blockIdx.x * A.rows_per_cta;
 
     if (r == 0) {
+        if (smem_u32(tma_smem) & 1023u) __trap();                     // the hardware swizzle pattern assumes a 1024-byte aligned tile
         prefetch_tmap(&tmap);
         mbar_init(bar, 1);
         mbar_fence_init();
