@@ -91,6 +91,45 @@ int oracle_adi_coeffs(int n, const double *f, int bc, double alpha, double *a, d
 }
 
 /* ---------------------------------------------------------------------------------------------
+ * Face-located unknowns ("velocity components at cell faces": the wall-normal
+ * component of the ADI step lives on the y-faces).  Row i of a line holds the value at face f_{i+1}, i = 0..n-1.
+ * Second difference at a face from the two adjacent CELL widths Db = f_{i+1}-f_i (below), Da = f_{i+2}-f_{i+1}
+ * (above) and the distance between the adjacent cell centres hc = (Db+Da)/2:
+ *   delta2 v_i = [ (v_{i+1}-v_i)/Da - (v_i-v_{i-1})/Db ] / hc,   lo_i = 1/(Db hc), up_i = 1/(Da hc)
+ * (exact for quadratics on any grid).  Dirichlet: the walls f_0 and f_n carry v = 0; row n-1 IS the wall face f_n and
+ * is an identity row (lo = up = 0), rows 0 and n-2 lose their wall coupling (b unchanged).  Periodic: face f_n is
+ * face f_0, every row is regular, Da of row n-1 wraps to f_1-f_0.  Neumann is not defined for face unknowns.
+ * ------------------------------------------------------------------------------------------- */
+int oracle_metrics_face(int n, const double *f, int bc, double *lo, double *up) {
+    if (n < 3 || bc == BC_NEUMANN) return ORACLE_ERR;
+    for (int i = 0; i < n; ++i) {
+        if (bc == BC_DIRICHLET && i == n - 1) { lo[i] = 0.0; up[i] = 0.0; continue; }
+        double Db = f[i + 1] - f[i];
+        double Da = (i + 2 <= n) ? f[i + 2] - f[i + 1] : f[1] - f[0];
+        if (!(Db > 0.0) || !(Da > 0.0)) return ORACLE_ERR;
+        double hc = 0.5 * (Db + Da);
+        lo[i] = 1.0 / (Db * hc);
+        up[i] = 1.0 / (Da * hc);
+    }
+    return ORACLE_OK;
+}
+
+/* ADI rows for face unknowns: a = -alpha lo, c = -alpha up, b = 1 - a - c; Dirichlet: a_0 := 0, c_{n-2} := 0 (wall
+ * values are 0), row n-1 is the identity. */
+int oracle_adi_coeffs_face(int n, const double *f, int bc, double alpha, double *a, double *b, double *c) {
+    double *lo = (double *)malloc(sizeof(double) * n), *up = (double *)malloc(sizeof(double) * n);
+    if (oracle_metrics_face(n, f, bc, lo, up) != ORACLE_OK) { free(lo); free(up); return ORACLE_ERR; }
+    for (int j = 0; j < n; ++j) {
+        a[j] = -alpha * lo[j];
+        c[j] = -alpha * up[j];
+        b[j] = 1.0 - a[j] - c[j];
+    }
+    if (bc == BC_DIRICHLET) { a[0] = 0.0; c[n - 2] = 0.0; }
+    free(lo); free(up);
+    return ORACLE_OK;
+}
+
+/* ---------------------------------------------------------------------------------------------
  * Helmholtz operator (delta2_y - lambda), lambda >= 0 (main diagonal = off-diagonal sum
  * plus modified wavenumbers, |b_j| = |a_j|+|c_j|+eps with eps = lambda).
  * a_j = lo_j, c_j = up_j, b_j = -(a_j+c_j) - lambda.  Neumann ends (pseudo-pressure):
@@ -417,6 +456,20 @@ int oracle_adi_sweep(int nx, int ny, int nz, const double *xf, const double *yf,
     int bc = dir == 0 ? bcx : (dir == 1 ? bcy : bcz);
     double *a = (double *)malloc(sizeof(double) * n * 3), *b = a + n, *c = a + 2 * n;
     int rc = oracle_adi_coeffs(n, f, bc, alpha, a, b, c);
+    if (rc == ORACLE_OK) rc = oracle_sweep_coeffs(nx, ny, nz, dir, mode, P, bc == BC_PERIODIC, a, b, c, field);
+    free(a);
+    return rc;
+}
+
+/* The same with the unknowns of direction dir at cell centres (loc = 0) or at faces (loc = 1): tdx_adi_sweep_at. */
+int oracle_adi_sweep_at(int nx, int ny, int nz, const double *xf, const double *yf, const double *zf,
+                        int bcx, int bcy, int bcz, int dir, int loc, int mode, int P, double alpha, double *field) {
+    if (loc == 0) return oracle_adi_sweep(nx, ny, nz, xf, yf, zf, bcx, bcy, bcz, dir, mode, P, alpha, field);
+    int n = dir == 0 ? nx : (dir == 1 ? ny : nz);
+    const double *f = dir == 0 ? xf : (dir == 1 ? yf : zf);
+    int bc = dir == 0 ? bcx : (dir == 1 ? bcy : bcz);
+    double *a = (double *)malloc(sizeof(double) * n * 3), *b = a + n, *c = a + 2 * n;
+    int rc = oracle_adi_coeffs_face(n, f, bc, alpha, a, b, c);
     if (rc == ORACLE_OK) rc = oracle_sweep_coeffs(nx, ny, nz, dir, mode, P, bc == BC_PERIODIC, a, b, c, field);
     free(a);
     return rc;

@@ -64,6 +64,13 @@ def adi_coeffs(faces, bc, alpha):
     return a, b, c
 
 
+def adi_coeffs_face(faces, bc, alpha):
+    f = _c(faces); n = f.size - 1
+    a = np.empty(n); b = np.empty(n); c = np.empty(n)
+    _chk(_lib.oracle_adi_coeffs_face(C.c_int(n), _p(f), C.c_int(bc), C.c_double(alpha), _p(a), _p(b), _p(c)), "adi_coeffs_face")
+    return a, b, c
+
+
 def helmholtz_coeffs(faces, lam):
     f = _c(faces); n = f.size - 1
     a = np.empty(n); b = np.empty(n); c = np.empty(n); pinned = C.c_int(0)
@@ -156,6 +163,17 @@ def adi_sweep(field_zyx, xf, yf, zf, bcs, direction, mode, P, alpha):
     _chk(_lib.oracle_adi_sweep(C.c_int(nx), C.c_int(ny), C.c_int(nz), _p(xf), _p(yf), _p(zf),
                                C.c_int(bcs[0]), C.c_int(bcs[1]), C.c_int(bcs[2]), C.c_int(direction), C.c_int(mode),
                                C.c_int(P), C.c_double(alpha), _p(field_zyx)), "adi_sweep")
+    return field_zyx
+
+
+def adi_sweep_at(field_zyx, xf, yf, zf, bcs, direction, loc, mode, P, alpha):
+    """As adi_sweep with the unknowns of `direction` at cell centres (loc 0) or faces (loc 1)."""
+    nz, ny, nx = field_zyx.shape
+    _field(field_zyx, (nz, ny, nx))
+    xf, yf, zf = _c(xf), _c(yf), _c(zf)
+    _chk(_lib.oracle_adi_sweep_at(C.c_int(nx), C.c_int(ny), C.c_int(nz), _p(xf), _p(yf), _p(zf),
+                                  C.c_int(bcs[0]), C.c_int(bcs[1]), C.c_int(bcs[2]), C.c_int(direction), C.c_int(loc),
+                                  C.c_int(mode), C.c_int(P), C.c_double(alpha), _p(field_zyx)), "adi_sweep_at")
     return field_zyx
 
 
