@@ -32,6 +32,8 @@ typedef enum { TDX_DIR_X = 0, TDX_DIR_Y = 1, TDX_DIR_Z = 2 } tdx_dir_t;
  * PPT   : PAPER.md L126-146, L156 -- Z solved exactly (to rounding).                                  */
 typedef enum { TDX_MODE_THOMAS = 0, TDX_MODE_PDD = 1, TDX_MODE_PPT = 2 } tdx_mode_t;
 typedef enum { TDX_BC_DIRICHLET = 0, TDX_BC_PERIODIC = 1, TDX_BC_NEUMANN = 2 } tdx_bc_t;
+/* Where the unknowns of a direction sit on the staggered grid (velocities at faces, pressure at centres). */
+typedef enum { TDX_LOC_CENTER = 0, TDX_LOC_FACE = 1 } tdx_loc_t;
 typedef enum {
     TDX_OK = 0,
     TDX_ERR_INVALID_ARG = -1,      /* null pointer, bad enum, non-increasing faces, n < 2 ...            */
@@ -67,6 +69,23 @@ tdx_status_t tdx_partition_bounds(int n, int P, int* starts);
  * rhs_inout: DEVICE, nx*ny*nz doubles.  P: partitions per line (ignored for THOMAS).                    */
 tdx_status_t tdx_adi_sweep(tdx_grid_t* grid, tdx_dir_t dir, tdx_mode_t mode, int P,
                            double alpha, double* rhs_inout, void* stream);
+
+/* The same sweep with the unknowns of direction dir at cell centres (TDX_LOC_CENTER: identical to tdx_adi_sweep) or at
+ * cell faces (TDX_LOC_FACE; SURVEY 8(f) N1 -- the wall-normal velocity component of the ADI step).
+ * Face unknowns: row i of a line is the value at face f_{i+1}; delta2 v_i = [(v_{i+1}-v_i)/Da - (v_i-v_{i-1})/Db]/hc with
+ * the adjacent cell widths Db, Da and hc = (Db+Da)/2.  Dirichlet: both walls carry 0, row n-1 is the wall face and is an
+ * identity row (its right-hand side passes through); periodic: every row regular.  Neumann ends or n < 3:
+ * TDX_ERR_UNSUPPORTED.  rhs_inout: DEVICE, nx*ny*nz doubles. */
+tdx_status_t tdx_adi_sweep_at(tdx_grid_t* grid, tdx_dir_t dir, tdx_loc_t loc, tdx_mode_t mode, int P,
+                              double alpha, double* rhs_inout, void* stream);
+
+/* One ADI step for ncomp fields stored back to back ([ncomp][nz][ny][nx], e.g. the three velocity components that
+ * Algorithm 1 batches): x sweep, then y sweep, then z sweep of (I - alpha*delta2) over all components,
+ * one launch per direction for each run of consecutive components with the same location.  loc: HOST, ncomp*3 ints
+ * loc[c*3 + dir] in {TDX_LOC_CENTER, TDX_LOC_FACE}, or NULL for all centres (staggered velocities: u = face in x,
+ * v = face in y, w = face in z).  All plans are validated before the first launch.  rhs_inout: DEVICE. */
+tdx_status_t tdx_adi_step(tdx_grid_t* grid, tdx_mode_t mode, int Px, int Py, int Pz, double alpha,
+                          int ncomp, const int* loc, double* rhs_inout, void* stream);
 
 /* Poisson y-solves after the spanwise transform: for every wavenumber m < nm and
  * x-index i solve (delta2_y - lambda) phi = rhs with lambda = kx2[i] + kz2[m] >= 0, Neumann ends;

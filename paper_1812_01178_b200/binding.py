@@ -13,9 +13,10 @@ from . import build as _build
 DIR_X, DIR_Y, DIR_Z = 0, 1, 2
 MODE_THOMAS, MODE_PDD, MODE_PPT = 0, 1, 2
 BC_DIRICHLET, BC_PERIODIC, BC_NEUMANN = 0, 1, 2
+LOC_CENTER, LOC_FACE = 0, 1
 OK, ERR_INVALID_ARG, ERR_BAD_PARTITION, ERR_ALLOC, ERR_CUDA, ERR_UNSUPPORTED, ERR_PDD_BOUND = 0, -1, -2, -3, -4, -5, -6
 
-EXPORTS = ("tdx_grid_create", "tdx_grid_destroy", "tdx_partition_bounds", "tdx_adi_sweep",
+EXPORTS = ("tdx_grid_create", "tdx_grid_destroy", "tdx_partition_bounds", "tdx_adi_sweep", "tdx_adi_sweep_at", "tdx_adi_step",
            "tdx_helmholtz_wavenumber_solve", "tdx_cyclic_solve", "tdx_adi_sweep_host", "tdx_adi_step_host",
            "tdx_helmholtz_wavenumber_solve_host", "tdx_pdd_dropped_bound", "tdx_kernel_launch_count",
            "tdx_status_string", "tdx_last_error", "tdx_version")
@@ -48,6 +49,8 @@ def lib():
         L.tdx_grid_destroy.argtypes = [C.c_void_p]
         L.tdx_partition_bounds.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_int)]
         L.tdx_adi_sweep.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_double, C.c_void_p, C.c_void_p]
+        L.tdx_adi_sweep_at.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_double, C.c_void_p, C.c_void_p]
+        L.tdx_adi_step.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_double, C.c_int, C.POINTER(C.c_int), C.c_void_p, C.c_void_p]
         L.tdx_helmholtz_wavenumber_solve.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, _dp, _dp, C.c_void_p, C.c_void_p]
         L.tdx_cyclic_solve.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, _dp, _dp, _dp, C.c_void_p, C.c_void_p]
         L.tdx_adi_sweep_host.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_double, C.c_void_p]
@@ -124,6 +127,18 @@ class Grid:
 
     def adi_sweep(self, direction, mode, P, alpha, rhs, stream=0):
         _chk(lib().tdx_adi_sweep(self._h, direction, mode, P, alpha, _devptr(rhs), C.c_void_p(stream)))
+
+    def adi_sweep_at(self, direction, loc, mode, P, alpha, rhs, stream=0):
+        _chk(lib().tdx_adi_sweep_at(self._h, direction, loc, mode, P, alpha, _devptr(rhs), C.c_void_p(stream)))
+
+    def adi_step(self, mode, Px, Py, Pz, alpha, ncomp, loc, rhs, stream=0):
+        """loc: None or ncomp*3 ints (loc[c*3+dir]); rhs: device buffer of ncomp fields stored back to back."""
+        arr = None
+        if loc is not None:
+            flat = [int(v) for v in np.asarray(loc).reshape(-1)]
+            assert len(flat) == ncomp * 3
+            arr = (C.c_int * len(flat))(*flat)
+        _chk(lib().tdx_adi_step(self._h, mode, Px, Py, Pz, alpha, ncomp, arr, _devptr(rhs), C.c_void_p(stream)))
 
     def helmholtz_wavenumber_solve(self, mode, P, kx2, kz2, rhs, stream=0):
         kz, pkz = _host(kz2)

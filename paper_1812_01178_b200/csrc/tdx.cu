@@ -52,6 +52,7 @@ enum PlanKind { KIND_ADI = 0, KIND_HELM = 1, KIND_USER = 2 };
 
 struct Plan {
     int kind = 0, dir = 0, mode = 0, P = 1, n = 0, nsets = 1;
+    int loc = 0;            // unknowns of this direction at cell centres (0) or faces (1); ADI only
     int M = 0;              // register rows per partition (kernel instantiation)
     int layout = tdx::ROWS_PJ;
     int KB = 0, Scap = 0;
@@ -97,8 +98,10 @@ struct tdx_grid {
     int nx = 0, ny = 0, nz = 0, device = 0, sms = 148;
     int bc[3] = {0, 0, 0};
     double* faces[3] = {nullptr, nullptr, nullptr};     // device copies
-    double* lo[3] = {nullptr, nullptr, nullptr};        // metrics per direction (device)
+    double* lo[3] = {nullptr, nullptr, nullptr};        // metrics per direction (device), unknowns at cell centres
     double* up[3] = {nullptr, nullptr, nullptr};
+    double* lo_face[3] = {nullptr, nullptr, nullptr};   // metrics for face-located unknowns (nullptr: not defined, Neumann)
+    double* up_face[3] = {nullptr, nullptr, nullptr};
     double* lo_neumann_y = nullptr;                     // Helmholtz uses Neumann ends in y whatever bcy is
     double* up_neumann_y = nullptr;
     std::deque<Plan> plans;            // deque: references stay valid across push_back
@@ -127,7 +130,8 @@ tdx_status_t build_plan(tdx_grid* g, Plan& pl, const double* lambda_host, const 
     CUDA_TRY(cudaMemsetAsync(flags.p, 0, (size_t)nsets * 4, st));
     const int tb = 128;
     if (pl.kind == KIND_ADI) {
-        k_coeffs_adi<<<(n + tb - 1) / tb, tb, 0, st>>>(n, g->lo[pl.dir], g->up[pl.dir], g->bc[pl.dir], pl.alpha,
+        k_coeffs_adi<<<(n + tb - 1) / tb, tb, 0, st>>>(n, pl.loc ? g->lo_face[pl.dir] : g->lo[pl.dir], pl.loc ? g->up_face[pl.dir] : g->up[pl.dir],
+                                                       g->bc[pl.dir], pl.loc, pl.alpha,
                                                        a.as<double>(), b.as<double>(), c.as<double>());
         LAUNCH_CHECK("k_coeffs_adi");
     } else if (pl.kind == KIND_HELM) {
@@ -242,7 +246,7 @@ tdx_status_t build_plan(tdx_grid* g, Plan& pl, const double* lambda_host, const 
 // find or build
 tdx_status_t get_plan(tdx_grid* g, int kind, int dir, int mode, int P, double alpha, int nsets,
                       const double* lambda_host, const double* ua, const double* ub, const double* uc,
-                      cudaStream_t st, Plan** out) {
+                      cudaStream_t st, Plan** out, int loc = 0) {
     const int n = (kind == KIND_HELM) ? g->ny : g->n_of(dir);
     if (n < 2) return fail(TDX_ERR_INVALID_ARG, "line length %d < 2", n);
     bool thomas = (mode == TDX_MODE_THOMAS) || P == 1;
@@ -266,11 +270,11 @@ tdx_status_t get_plan(tdx_grid* g, int kind, int dir, int mode, int P, double al
     if (kind == KIND_USER) { h = fnv1a(ua, (size_t)n * 8); h = fnv1a(ub, (size_t)n * 8, h); h = fnv1a(uc, (size_t)n * 8, h); }
     std::lock_guard<std::mutex> lk(g->mu);
     for (Plan& p : g->plans)
-        if (p.kind == kind && p.dir == dir && p.mode == mode && p.P == P && p.nsets == nsets && p.hash == h &&
+        if (p.kind == kind && p.dir == dir && p.loc == loc && p.mode == mode && p.P == P && p.nsets == nsets && p.hash == h &&
             std::memcmp(&p.alpha, &alpha, 8) == 0) { *out = &p; return TDX_OK; }
     Plan pl;
     pl.kind = kind; pl.dir = dir; pl.mode = mode; pl.P = P; pl.n = n; pl.nsets = nsets; pl.M = M; pl.cyc = cyc; pl.wrap = wrap;
-    pl.thomas = thomas; pl.alpha = alpha; pl.hash = h; pl.sms = g->sms;
+    pl.thomas = thomas; pl.alpha = alpha; pl.hash = h; pl.sms = g->sms; pl.loc = loc;
     tdx_status_t rc = build_plan(g, pl, lambda_host, ua, ub, uc, st);
     if (rc != TDX_OK) { pl.release(); return rc; }
     g->plans.push_back(pl);
@@ -540,11 +544,13 @@ tdx_status_t run_unit(const Plan& pl, double* data, long long nlines, cudaStream
     return pl.cyc ? launch_unit_M<false, true>(pl.M, A, T, grid, threads, smem, st) : launch_unit_M<false, false>(pl.M, A, T, grid, threads, smem, st);
 }
 
-tdx_status_t run_sweep(tdx_grid* g, const Plan& pl, int dir, double* data, cudaStream_t st) {
+// ncomp fields of the grid's shape stored back to back are just a longer batch: more x lines, more outer planes for
+// the y sweep, `ncomp` outer indices for the z sweep.
+tdx_status_t run_sweep(tdx_grid* g, const Plan& pl, int dir, double* data, cudaStream_t st, int ncomp = 1) {
     const long long nx = g->nx, ny = g->ny, nz = g->nz;
-    if (dir == 0) return run_unit(pl, data, ny * nz, st);
-    if (dir == 1) return run_strided(pl, data, nx, nx, nz, nx * ny, false, st);
-    return run_strided(pl, data, nx * ny, nx * ny, 1, 0, false, st);
+    if (dir == 0) return run_unit(pl, data, ny * nz * ncomp, st);
+    if (dir == 1) return run_strided(pl, data, nx, nx, nz * ncomp, nx * ny, false, st);
+    return run_strided(pl, data, nx * ny, nx * ny, ncomp, ncomp > 1 ? nx * ny * nz : 0, false, st);
 }
 
 tdx_status_t check_common(tdx_grid* g, int dir, int mode, const void* ptr) {
@@ -618,6 +624,12 @@ tdx_status_t tdx_grid_create(int nx, int ny, int nz, const double* xf, const dou
         if (cudaMemcpy(g->faces[d], fs[d], (size_t)(n + 1) * 8, cudaMemcpyHostToDevice) != cudaSuccess) return bail(fail(TDX_ERR_CUDA, "face upload failed"));
         tdx::k_metrics<<<(n + 127) / 128, 128>>>(n, g->faces[d], bcs[d], g->lo[d], g->up[d]);
         g_launches.fetch_add(1);
+        if (bcs[d] != TDX_BC_NEUMANN && n >= 3) {
+            if (cudaMalloc(&g->lo_face[d], (size_t)n * 8) != cudaSuccess || cudaMalloc(&g->up_face[d], (size_t)n * 8) != cudaSuccess)
+                return bail(fail(TDX_ERR_ALLOC, "device allocation failed"));
+            tdx::k_metrics_face<<<(n + 127) / 128, 128>>>(n, g->faces[d], bcs[d], g->lo_face[d], g->up_face[d]);
+            g_launches.fetch_add(1);
+        }
     }
     if (cudaMalloc(&g->lo_neumann_y, (size_t)ny * 8) != cudaSuccess || cudaMalloc(&g->up_neumann_y, (size_t)ny * 8) != cudaSuccess)
         return bail(fail(TDX_ERR_ALLOC, "device allocation failed"));
@@ -633,7 +645,7 @@ tdx_status_t tdx_grid_destroy(tdx_grid_t* g) {
     if (!g) return TDX_OK;
     cudaSetDevice(g->device);
     for (Plan& p : g->plans) p.release();
-    for (int d = 0; d < 3; ++d) { cudaFree(g->faces[d]); cudaFree(g->lo[d]); cudaFree(g->up[d]); }
+    for (int d = 0; d < 3; ++d) { cudaFree(g->faces[d]); cudaFree(g->lo[d]); cudaFree(g->up[d]); cudaFree(g->lo_face[d]); cudaFree(g->up_face[d]); }
     cudaFree(g->lo_neumann_y); cudaFree(g->up_neumann_y); cudaFree(g->stage);
     delete g;
     return TDX_OK;
@@ -649,6 +661,54 @@ tdx_status_t tdx_adi_sweep(tdx_grid_t* g, tdx_dir_t dir, tdx_mode_t mode, int P,
     rc = get_plan(g, KIND_ADI, dir, mode, P, alpha, 1, nullptr, nullptr, nullptr, nullptr, st, &pl);
     if (rc != TDX_OK) return rc;
     return run_sweep(g, *pl, dir, rhs, st);
+}
+
+tdx_status_t tdx_adi_sweep_at(tdx_grid_t* g, tdx_dir_t dir, tdx_loc_t loc, tdx_mode_t mode, int P, double alpha, double* rhs, void* stream) {
+    tdx_status_t rc = check_common(g, dir, mode, rhs);
+    if (rc != TDX_OK) return rc;
+    if (loc != TDX_LOC_CENTER && loc != TDX_LOC_FACE) return fail(TDX_ERR_INVALID_ARG, "loc=%d not in {0,1}", (int)loc);
+    if (!(alpha == alpha)) return fail(TDX_ERR_INVALID_ARG, "alpha is NaN");
+    if (loc == TDX_LOC_FACE && !g->lo_face[dir]) return fail(TDX_ERR_UNSUPPORTED, "face-located unknowns need Dirichlet or periodic ends and n >= 3 in direction %d", (int)dir);
+    CUDA_TRY(cudaSetDevice(g->device));
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    Plan* pl = nullptr;
+    rc = get_plan(g, KIND_ADI, dir, mode, P, alpha, 1, nullptr, nullptr, nullptr, nullptr, st, &pl, (int)loc);
+    if (rc != TDX_OK) return rc;
+    return run_sweep(g, *pl, dir, rhs, st);
+}
+
+tdx_status_t tdx_adi_step(tdx_grid_t* g, tdx_mode_t mode, int Px, int Py, int Pz, double alpha, int ncomp, const int* loc,
+                          double* rhs, void* stream) {
+    tdx_status_t rc = check_common(g, 0, mode, rhs);
+    if (rc != TDX_OK) return rc;
+    if (ncomp < 1 || ncomp > 64) return fail(TDX_ERR_INVALID_ARG, "ncomp=%d not in [1,64]", ncomp);
+    if (!(alpha == alpha)) return fail(TDX_ERR_INVALID_ARG, "alpha is NaN");
+    if ((long long)g->nz * ncomp > 65535) return fail(TDX_ERR_UNSUPPORTED, "nz*ncomp > 65535");
+    CUDA_TRY(cudaSetDevice(g->device));
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const int Ps[3] = {Px, Py, Pz};
+    const size_t npts = (size_t)g->nx * g->ny * g->nz;
+    // validate every (direction, location) plan before the first launch: no partial step on an argument error
+    Plan* pls[3][2] = {{nullptr, nullptr}, {nullptr, nullptr}, {nullptr, nullptr}};
+    for (int d = 0; d < 3; ++d)
+        for (int c = 0; c < ncomp; ++c) {
+            const int l = loc ? loc[c * 3 + d] : 0;
+            if (l != 0 && l != 1) return fail(TDX_ERR_INVALID_ARG, "loc[%d][%d]=%d not in {0,1}", c, d, l);
+            if (l == 1 && !g->lo_face[d]) return fail(TDX_ERR_UNSUPPORTED, "face-located unknowns need Dirichlet or periodic ends in direction %d", d);
+            if (!pls[d][l]) { rc = get_plan(g, KIND_ADI, d, mode, Ps[d], alpha, 1, nullptr, nullptr, nullptr, nullptr, st, &pls[d][l], l); if (rc != TDX_OK) return rc; }
+        }
+    for (int d = 0; d < 3; ++d) {
+        int c = 0;
+        while (c < ncomp) {                                       // runs of consecutive components with the same location share a launch
+            const int l = loc ? loc[c * 3 + d] : 0;
+            int e = c + 1;
+            while (e < ncomp && (loc ? loc[e * 3 + d] : 0) == l) ++e;
+            rc = run_sweep(g, *pls[d][l], d, rhs + (size_t)c * npts, st, e - c);
+            if (rc != TDX_OK) return rc;
+            c = e;
+        }
+    }
+    return TDX_OK;
 }
 
 tdx_status_t tdx_cyclic_solve(tdx_grid_t* g, tdx_dir_t dir, tdx_mode_t mode, int P, const double* a, const double* b,

@@ -48,14 +48,29 @@ __global__ void k_metrics(int n, const double* __restrict__ f, int bc, double* _
     up[j] = 1.0 / (hp * D);
 }
 
+// ---- a1 for face-located unknowns (velocities at cell faces).  Row i holds the value
+// at face f_{i+1}: lo_i = 1/(Db hc), up_i = 1/(Da hc) with the adjacent cell widths Db = f_{i+1}-f_i, Da = f_{i+2}-f_{i+1}
+// and hc = (Db+Da)/2.  Dirichlet: row n-1 is the wall face (identity row, lo = up = 0); periodic: Da of row n-1 wraps.
+__global__ void k_metrics_face(int n, const double* __restrict__ f, int bc, double* __restrict__ lo, double* __restrict__ up) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    if (bc == 0 && i == n - 1) { lo[i] = 0.0; up[i] = 0.0; return; }
+    double Db = f[i + 1] - f[i];
+    double Da = (i + 2 <= n) ? f[i + 2] - f[i + 1] : f[1] - f[0];
+    double hc = 0.5 * (Db + Da);
+    lo[i] = 1.0 / (Db * hc);
+    up[i] = 1.0 / (Da * hc);
+}
+
 // ---- a1: ADI rows  a = -alpha lo, c = -alpha up, b = 1 - a - c  (|b| = |a|+|c|+1) -------------
-__global__ void k_coeffs_adi(int n, const double* __restrict__ lo, const double* __restrict__ up, int bc, double alpha,
+__global__ void k_coeffs_adi(int n, const double* __restrict__ lo, const double* __restrict__ up, int bc, int loc, double alpha,
                              double* __restrict__ a, double* __restrict__ b, double* __restrict__ c) {
     int j = blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= n) return;
     double aj = -alpha * lo[j], cj = -alpha * up[j];
     double bj = __dsub_rn(__dsub_rn(1.0, aj), cj);
-    if (bc == 0) { if (j == 0) aj = 0.0; if (j == n - 1) cj = 0.0; }                 // Dirichlet: ghost coupling dropped
+    if (bc == 0 && loc == 1) { if (j == 0) aj = 0.0; if (j == n - 2) cj = 0.0; }     // faces: walls carry 0, row n-1 is the wall
+    if (bc == 0 && loc == 0) { if (j == 0) aj = 0.0; if (j == n - 1) cj = 0.0; }     // Dirichlet: ghost coupling dropped
     if (bc == 2) {                                                                    // Neumann: ghost folds into b
         if (j == 0) { bj = __dsub_rn(1.0, cj); aj = 0.0; }
         if (j == n - 1) { bj = __dsub_rn(1.0, aj); cj = 0.0; }
