@@ -334,22 +334,20 @@ def run_tdx(args, rank, world, local_rank):
         hf = torch.from_numpy(host_field).pin_memory().numpy()
         hh = torch.from_numpy(host_helm).pin_memory().numpy()
         hh0 = host_helm
-        grid.adi_step_host(mode, Ps[0], Ps[1], Ps[2], cfg.alpha, hf)          # warm-up (staging allocation)
-        grid.helmholtz_wavenumber_solve_host(mode, Ps[3], None, kz2, hh)
+        grid.step_host(mode, Ps[0], Ps[1], Ps[2], cfg.alpha, hf, Ps[3], kz2, hh)   # warm-up (staging allocation, streams)
         barrier()
         ts = []
         for _ in range(max(1, args.e2e_steps)):
             np.copyto(hh, hh0)
             barrier()
             t0 = time.perf_counter()
-            grid.adi_step_host(mode, Ps[0], Ps[1], Ps[2], cfg.alpha, hf)
-            grid.helmholtz_wavenumber_solve_host(mode, Ps[3], None, kz2, hh)
+            grid.step_host(mode, Ps[0], Ps[1], Ps[2], cfg.alpha, hf, Ps[3], kz2, hh)
             torch.cuda.synchronize()
             ts.append(time.perf_counter() - t0)
         te = max_over_ranks(float(np.mean(ts)), dist, "cuda")
         out["e2e"] = {"value": world * step_points(cfg) / te / 1e9, "unit": UNIT, "h2d_bytes_per_step": int(hf.nbytes + hh.nbytes),
                       "d2h_bytes_per_step": int(hf.nbytes + hh.nbytes), "ms_per_step": te * 1e3, "steps": len(ts),
-                      "api": "tdx_adi_step_host + tdx_helmholtz_wavenumber_solve_host (pinned host buffers)"}
+                      "api": "tdx_step_host (pinned host buffers; slabs pipelined over upload/compute/download streams)"}
     if rank == 0 and world == 1 and not args.no_cpu:
         v, _, info = run_oracle_sample(cfg)
         info["value"] = v

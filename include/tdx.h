@@ -117,6 +117,14 @@ tdx_status_t tdx_helmholtz_wavenumber_solve_host(tdx_grid_t* grid, tdx_mode_t mo
                                                  int nm, const double* kx2, const double* kz2,
                                                  double* host_rhs_inout);
 
+/* One whole step on HOST buffers, pipelined: x, y and z sweeps of host_field (nx*ny*nz doubles; NULL skips it) and the
+ * nm Helmholtz y-solves of host_helm (complex128 [nm][ny][nx]; NULL skips it).  The buffers travel in slabs over three
+ * streams (upload, compute, download), so both PCIe directions are busy at once and the kernels hide behind the copies;
+ * page-locked (pinned) host memory is needed for the overlap, pageable memory works but serialises.  Synchronous:
+ * returns when both results are in host memory.  All plans are validated before the first copy. */
+tdx_status_t tdx_step_host(tdx_grid_t* grid, tdx_mode_t mode, int Px, int Py, int Pz, double alpha, double* host_field,
+                           int Ph, int nm, const double* kz2, double* host_helm);
+
 /* Diagnostics.  tdx_pdd_dropped_bound: max over interfaces of |v_last|, |w_first| for the ADI operator of
  * (dir, P, alpha) -- the entries PDD deletes from Z; the a-priori size of the PDD error.  */
 tdx_status_t tdx_pdd_dropped_bound(tdx_grid_t* grid, tdx_dir_t dir, int P, double alpha, double* out);

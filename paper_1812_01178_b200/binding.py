@@ -18,7 +18,7 @@ OK, ERR_INVALID_ARG, ERR_BAD_PARTITION, ERR_ALLOC, ERR_CUDA, ERR_UNSUPPORTED, ER
 
 EXPORTS = ("tdx_grid_create", "tdx_grid_destroy", "tdx_partition_bounds", "tdx_adi_sweep", "tdx_adi_sweep_at", "tdx_adi_step",
            "tdx_helmholtz_wavenumber_solve", "tdx_cyclic_solve", "tdx_adi_sweep_host", "tdx_adi_step_host",
-           "tdx_helmholtz_wavenumber_solve_host", "tdx_pdd_dropped_bound", "tdx_kernel_launch_count",
+           "tdx_helmholtz_wavenumber_solve_host", "tdx_step_host", "tdx_pdd_dropped_bound", "tdx_kernel_launch_count",
            "tdx_status_string", "tdx_last_error", "tdx_version")
 
 _dp = C.POINTER(C.c_double)
@@ -56,6 +56,7 @@ def lib():
         L.tdx_adi_sweep_host.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_double, C.c_void_p]
         L.tdx_adi_step_host.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_double, C.c_void_p]
         L.tdx_helmholtz_wavenumber_solve_host.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, _dp, _dp, C.c_void_p]
+        L.tdx_step_host.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_double, C.c_void_p, C.c_int, C.c_int, _dp, C.c_void_p]
         L.tdx_pdd_dropped_bound.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_double, _dp]
         _lib = L
     return _lib
@@ -160,6 +161,13 @@ class Grid:
         _, pkx = _host(kx2)
         _chk(lib().tdx_helmholtz_wavenumber_solve_host(self._h, mode, P, kz.size, pkx, pkz,
                                                        _hostptr(host_rhs, self.nx * self.ny * kz.size * 16)))
+
+    def step_host(self, mode, Px, Py, Pz, alpha, host_field, Ph, kz2, host_helm):
+        """Pipelined whole step on host buffers (either may be None)."""
+        kz, pkz = _host(kz2) if host_helm is not None else (None, None)
+        pf = _hostptr(host_field, self.nx * self.ny * self.nz * 8) if host_field is not None else None
+        ph = _hostptr(host_helm, self.nx * self.ny * kz.size * 16) if host_helm is not None else None
+        _chk(lib().tdx_step_host(self._h, mode, Px, Py, Pz, alpha, pf, Ph, kz.size if kz is not None else 0, pkz, ph))
 
     def pdd_dropped_bound(self, direction, P, alpha):
         out = C.c_double(0.0)

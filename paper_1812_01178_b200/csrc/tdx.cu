@@ -107,6 +107,8 @@ struct tdx_grid {
     std::deque<Plan> plans;            // deque: references stay valid across push_back
     std::mutex mu;
     double* stage = nullptr; size_t stage_bytes = 0;    // device staging for the *_host entry points
+    double* stage2 = nullptr; size_t stage2_bytes = 0;  // second staging buffer (Helmholtz part of tdx_step_host)
+    cudaStream_t s_up = nullptr, s_comp = nullptr, s_down = nullptr;   // pipeline streams of tdx_step_host
     int n_of(int dir) const { return dir == 0 ? nx : (dir == 1 ? ny : nz); }
 };
 
@@ -334,12 +336,12 @@ int pow2floor(long long v) { int p = 1; while ((long long)p * 2 <= v) p *= 2; re
 
 // lines of `dir` in a field whose x extent is `nxe` doubles (nx for real fields, 2 nx for complex ones)
 tdx_status_t run_strided(const Plan& pl, double* data, long long W, long long line_stride, long long O,
-                         long long outer_stride, bool set_per_outer, cudaStream_t st) {
+                         long long outer_stride, bool set_per_outer, cudaStream_t st, int set0 = 0) {
     // W, strides in doubles on entry.  16-byte accesses (V = 2 lines per thread) when everything is even.
     const bool even = W % 2 == 0 && line_stride % 2 == 0 && outer_stride % 2 == 0 && (reinterpret_cast<uintptr_t>(data) % 16) == 0;
     if (O > 65535) return fail(TDX_ERR_UNSUPPORTED, "outer extent %lld > 65535", O);
     StridedArgs A;
-    A.data = data; A.set_per_outer = set_per_outer ? 1 : 0; A.pf = 0;
+    A.data = data; A.set_per_outer = set_per_outer ? 1 : 0; A.set0 = set0; A.pf = 0;
     if (pl.thomas) {
         const int V = even ? 2 : 1;
         A.W = W / V; A.line_stride = line_stride / V; A.outer_stride = outer_stride / V;
@@ -646,7 +648,10 @@ tdx_status_t tdx_grid_destroy(tdx_grid_t* g) {
     cudaSetDevice(g->device);
     for (Plan& p : g->plans) p.release();
     for (int d = 0; d < 3; ++d) { cudaFree(g->faces[d]); cudaFree(g->lo[d]); cudaFree(g->up[d]); cudaFree(g->lo_face[d]); cudaFree(g->up_face[d]); }
-    cudaFree(g->lo_neumann_y); cudaFree(g->up_neumann_y); cudaFree(g->stage);
+    cudaFree(g->lo_neumann_y); cudaFree(g->up_neumann_y); cudaFree(g->stage); cudaFree(g->stage2);
+    if (g->s_up) cudaStreamDestroy(g->s_up);
+    if (g->s_comp) cudaStreamDestroy(g->s_comp);
+    if (g->s_down) cudaStreamDestroy(g->s_down);
     delete g;
     return TDX_OK;
 }
@@ -799,6 +804,105 @@ tdx_status_t tdx_adi_sweep_host(tdx_grid_t* g, tdx_dir_t dir, tdx_mode_t mode, i
     if (rc != TDX_OK) return rc;
     CUDA_TRY(cudaMemcpyAsync(host, g->stage, bytes, cudaMemcpyDeviceToHost, 0));
     CUDA_TRY(cudaStreamSynchronize(0));
+    return TDX_OK;
+}
+
+// One whole step on HOST buffers, pipelined over three streams (upload / compute / download) so that PCIe runs in both
+// directions at once and the kernels hide behind the copies:
+//   field: z-slabs go up; each slab is swept in x and y as soon as it has arrived; when the last one is in, the z sweep
+//          runs y-slab by y-slab and every finished y-slab goes down (strided 2-D copy) while
+//   helm : the wavenumber slabs go up behind the field, are solved as they arrive and go down behind the field.
+tdx_status_t tdx_step_host(tdx_grid_t* g, tdx_mode_t mode, int Px, int Py, int Pz, double alpha, double* host_field,
+                           int Ph, int nm, const double* kz2, double* host_helm) {
+    if (!g) return fail(TDX_ERR_INVALID_ARG, "grid is NULL");
+    if (mode < 0 || mode > 2) return fail(TDX_ERR_INVALID_ARG, "mode=%d not in {0,1,2}", (int)mode);
+    if (!host_field && !host_helm) return fail(TDX_ERR_INVALID_ARG, "both host buffers are NULL");
+    if (host_helm && (nm < 1 || !kz2)) return fail(TDX_ERR_INVALID_ARG, "nm=%d / kz2 invalid", nm);
+    if (host_helm) for (int m = 0; m < nm; ++m) if (!(kz2[m] >= 0.0)) return fail(TDX_ERR_INVALID_ARG, "kz2[%d] is negative or NaN", m);
+    CUDA_TRY(cudaSetDevice(g->device));
+    if (!g->s_up) {
+        CUDA_TRY(cudaStreamCreateWithFlags(&g->s_up, cudaStreamNonBlocking));
+        CUDA_TRY(cudaStreamCreateWithFlags(&g->s_comp, cudaStreamNonBlocking));
+        CUDA_TRY(cudaStreamCreateWithFlags(&g->s_down, cudaStreamNonBlocking));
+    }
+    const long long nx = g->nx, ny = g->ny, nz = g->nz;
+    tdx_status_t rc;
+    Plan* pls[3] = {nullptr, nullptr, nullptr};
+    Plan* plh = nullptr;
+    if (host_field) {
+        const int Ps[3] = {Px, Py, Pz};
+        for (int d = 0; d < 3; ++d) {                       // validate and build every plan before any copy
+            rc = get_plan(g, KIND_ADI, d, mode, Ps[d], alpha, 1, nullptr, nullptr, nullptr, nullptr, g->s_comp, &pls[d]);
+            if (rc != TDX_OK) return rc;
+        }
+        rc = ensure_stage(g, (size_t)nx * ny * nz * 8);
+        if (rc != TDX_OK) return rc;
+    }
+    if (host_helm) {
+        rc = get_plan(g, KIND_HELM, TDX_DIR_Y, mode, Ph, 0.0, nm, kz2, nullptr, nullptr, nullptr, g->s_comp, &plh);
+        if (rc != TDX_OK) return rc;
+        const size_t hb = (size_t)nx * ny * nm * 16;
+        if (g->stage2_bytes < hb) {
+            cudaFree(g->stage2); g->stage2 = nullptr; g->stage2_bytes = 0;
+            if (cudaMalloc(&g->stage2, hb) != cudaSuccess) { cudaGetLastError(); return fail(TDX_ERR_ALLOC, "staging allocation of %zu bytes failed", hb); }
+            g->stage2_bytes = hb;
+        }
+    }
+    std::vector<cudaEvent_t> evs;
+    auto new_event = [&]() -> cudaEvent_t { cudaEvent_t e = nullptr; cudaEventCreateWithFlags(&e, cudaEventDisableTiming); evs.push_back(e); return e; };
+    auto cleanup = [&]() { for (cudaEvent_t e : evs) if (e) cudaEventDestroy(e); };
+#define STEP_TRY(expr) do { cudaError_t e_ = (expr); if (e_ != cudaSuccess) { cudaDeviceSynchronize(); cleanup(); return fail(TDX_ERR_CUDA, "%s failed: %s", #expr, cudaGetErrorString(e_)); } } while (0)
+#define STEP_RC(expr) do { rc = (expr); if (rc != TDX_OK) { cudaDeviceSynchronize(); cleanup(); return rc; } } while (0)
+    const int kSlabs = 16;
+    if (host_field) {
+        double* dev = g->stage;
+        const int sz = (int)std::min<long long>(kSlabs, nz);
+        for (int s = 0; s < sz; ++s) {                      // z-slabs up; x and y sweeps as they arrive
+            const long long k0 = nz * s / sz, k1 = nz * (s + 1) / sz;
+            const size_t off = (size_t)k0 * nx * ny;
+            STEP_TRY(cudaMemcpyAsync(dev + off, host_field + off, (size_t)(k1 - k0) * nx * ny * 8, cudaMemcpyHostToDevice, g->s_up));
+            cudaEvent_t e = new_event();
+            STEP_TRY(cudaEventRecord(e, g->s_up));
+            STEP_TRY(cudaStreamWaitEvent(g->s_comp, e, 0));
+            STEP_RC(run_unit(*pls[0], dev + off, ny * (k1 - k0), g->s_comp));
+            STEP_RC(run_strided(*pls[1], dev + off, nx, nx, k1 - k0, nx * ny, false, g->s_comp));
+        }
+        const int sy = (int)std::min<long long>(kSlabs, ny);
+        for (int s = 0; s < sy; ++s) {                      // z sweep y-slab by y-slab; each finished slab goes down
+            const long long j0 = ny * s / sy, j1 = ny * (s + 1) / sy;
+            const size_t off = (size_t)j0 * nx;
+            STEP_RC(run_strided(*pls[2], dev + off, nx * (j1 - j0), nx * ny, 1, 0, false, g->s_comp));
+            cudaEvent_t e = new_event();
+            STEP_TRY(cudaEventRecord(e, g->s_comp));
+            STEP_TRY(cudaStreamWaitEvent(g->s_down, e, 0));
+            STEP_TRY(cudaMemcpy2DAsync(host_field + off, (size_t)nx * ny * 8, dev + off, (size_t)nx * ny * 8,
+                                       (size_t)nx * (j1 - j0) * 8, (size_t)nz, cudaMemcpyDeviceToHost, g->s_down));
+        }
+    }
+    if (host_helm) {
+        double* dev = g->stage2;
+        const int sm = std::min(kSlabs, nm);
+        for (int s = 0; s < sm; ++s) {
+            const long long m0 = (long long)nm * s / sm, m1 = (long long)nm * (s + 1) / sm;
+            const size_t off = (size_t)m0 * ny * nx * 2;
+            const size_t bytes = (size_t)(m1 - m0) * ny * nx * 16;
+            STEP_TRY(cudaMemcpyAsync(dev + off, host_helm + off, bytes, cudaMemcpyHostToDevice, g->s_up));
+            cudaEvent_t e = new_event();
+            STEP_TRY(cudaEventRecord(e, g->s_up));
+            STEP_TRY(cudaStreamWaitEvent(g->s_comp, e, 0));
+            STEP_RC(run_strided(*plh, dev + off, 2 * nx, 2 * nx, m1 - m0, 2 * nx * ny, true, g->s_comp, (int)m0));
+            cudaEvent_t e2 = new_event();
+            STEP_TRY(cudaEventRecord(e2, g->s_comp));
+            STEP_TRY(cudaStreamWaitEvent(g->s_down, e2, 0));
+            STEP_TRY(cudaMemcpyAsync(host_helm + off, dev + off, bytes, cudaMemcpyDeviceToHost, g->s_down));
+        }
+    }
+    STEP_TRY(cudaStreamSynchronize(g->s_down));
+    STEP_TRY(cudaStreamSynchronize(g->s_comp));
+    STEP_TRY(cudaStreamSynchronize(g->s_up));
+#undef STEP_TRY
+#undef STEP_RC
+    cleanup();
     return TDX_OK;
 }
 

@@ -34,7 +34,8 @@ struct StridedArgs {
     long long W;             // lines per outer index, in V-vectors
     long long line_stride;   // distance between consecutive rows of a line, in V-vectors
     long long outer_stride;  // distance between outer indices, in V-vectors
-    int set_per_outer;       // 1: table set = outer index (Helmholtz wavenumber), 0: one set
+    int set_per_outer;       // 1: table set = set0 + outer index (Helmholtz wavenumber), 0: one set
+    int set0;                // first set of this launch (a launch may cover a sub-range of the wavenumbers)
     int LPC;                 // lines (V-vectors) per CTA = blockDim.x
     int pf;                  // L2 prefetch distance: CTAs ahead (one tile per CTA) or sets ahead (looping CTAs); 0 = off
     int tiles_x;             // column tiles per outer index
@@ -67,7 +68,7 @@ k_strided(StridedArgs A, Tables T) {
     const int tx = threadIdx.x, p = threadIdx.y;
     const int LPC = A.LPC, P = T.P;
     const int o = blockIdx.y;
-    const int set = A.set_per_outer ? o : 0;
+    const int set = A.set_per_outer ? A.set0 + o : 0;
     const int start = part_start(p, T.q, T.r);
     const int m = T.q + (p < T.r ? 1 : 0);
     const bool full = (T.r == 0) && (T.q == MAXM);          // every partition has exactly MAXM rows (warp-uniform)
@@ -303,7 +304,7 @@ __global__ void k_thomas_strided(StridedArgs A, const double* __restrict__ rows,
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= A.W) return;
     const int o = blockIdx.y;
-    const int set = A.set_per_outer ? o : 0;
+    const int set = A.set_per_outer ? A.set0 + o : 0;
     double* base = A.data + ((long long)o * A.outer_stride + i) * V;
     const long long rstride = A.line_stride * V;
     const double* rt = rows + (size_t)set * n * 6;

@@ -142,3 +142,32 @@ def test_kernel_launch_counter_counts_this_librarys_kernels(small):
     for _ in range(5):
         grid.adi_sweep(1, tdx.MODE_PPT, 3, 1e-3, t)
     assert tdx.kernel_launch_count() - n0 == 5                   # one launch per sweep
+
+
+def test_pipelined_step_host_equals_device_path_bit_exact():
+    """tdx_step_host (slabs over three streams, sub-range launches) must give exactly what the whole-field device calls give."""
+    nx, ny, nz = 96, 40, 36
+    faces = (inputs.faces_uniform(nx, 2.0), inputs.faces_tanh_two_sided(ny, 2.0), inputs.faces_uniform(nz, 1.0))
+    grid = tdx.Grid(nx, ny, nz, *faces, bcs=BCS)
+    field = inputs.rhs_uniform((nz, ny, nx), 41)
+    nm = nz // 2 + 1
+    helm = inputs.rhs_complex_uniform((nm, ny, nx), 42)
+    kz2 = inputs.modified_wavenumbers_z(nz, 1.0)
+    alpha = 3e-4
+    for mode in (tdx.MODE_PPT, tdx.MODE_PDD, tdx.MODE_THOMAS):
+        t = torch.from_numpy(field).cuda(); th = torch.from_numpy(helm).cuda()
+        for d, P in ((0, 6), (1, 5), (2, 4)):
+            grid.adi_sweep(d, mode, P, alpha, t)
+        grid.helmholtz_wavenumber_solve(mode, 4, None, kz2, th)
+        torch.cuda.synchronize()
+        hf = torch.from_numpy(field.copy()).pin_memory().numpy()
+        hh = torch.from_numpy(helm.copy()).pin_memory().numpy()
+        grid.step_host(mode, 6, 5, 4, alpha, hf, 4, kz2, hh)
+        assert np.array_equal(hf, t.cpu().numpy())
+        assert np.array_equal(hh, th.cpu().numpy())
+        hf2 = field.copy()                                       # pageable memory and one part only
+        grid.step_host(mode, 6, 5, 4, alpha, hf2, 4, None, None)
+        assert np.array_equal(hf2, hf)
+    with pytest.raises(tdx.TdxError):
+        grid.step_host(tdx.MODE_PPT, 6, 5, 999, alpha, hf, 4, kz2, hh)
+    grid.close()
