@@ -53,6 +53,8 @@ def parse():
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-step3", action="store_true", help="skip the extra 3-component staggered ADI step figure")
+    ap.add_argument("--psweep", default="", help="P sweep table (e.g. 8,16,32,64): per direction and mode, time, GB/s, PDD bound, "
+                                                 "error of sampled lines vs the oracle; prints a markdown table, not the JSON line")
     ap.add_argument("--selftest-ranks", action="store_true",
                     help="CPU-only check of the N>1 host logic over gloo (used by tests/test_bench_ranks_gloo.py)")
     return ap.parse_args()
@@ -360,12 +362,62 @@ def run_tdx(args, rank, world, local_rank):
         dist.destroy_process_group()
 
 
+def run_psweep(args):
+    """BASELINE.json config 3's purpose: PDD vs PPT over P -- throughput and accuracy per sweep direction."""
+    import torch
+    sys.path.insert(0, os.path.join(ROOT, "oracle"))
+    import oracle as orc
+    from paper_1812_01178_b200 import binding as tdx
+    cfg = configs.get(args.config)
+    bcs = (tdx.BC_DIRICHLET, tdx.BC_DIRICHLET, tdx.BC_PERIODIC)
+    faces = cfg.faces()
+    grid = tdx.Grid(cfg.nx, cfg.ny, cfg.nz, *faces, bcs=bcs)
+    field0 = torch.from_numpy(cfg.rhs_field()).cuda()
+    rng = np.random.default_rng(7)
+    ns = 48
+    print("| dir | mode | P | rows/partition | ms | GB/s | PDD dropped bound | rel. error of %d sampled lines vs oracle |" % ns)
+    print("|---|---|---|---|---|---|---|---|")
+    for d, name in enumerate("xyz"):
+        n = (cfg.nx, cfg.ny, cfg.nz)[d]
+        dims = {0: (cfg.nz, cfg.ny), 1: (cfg.nz, cfg.nx), 2: (cfg.ny, cfg.nx)}[d]
+        ia = torch.from_numpy(rng.integers(0, dims[0], ns)).cuda(); ib = torch.from_numpy(rng.integers(0, dims[1], ns)).cuda()
+        take = {0: lambda t: t[ia, ib, :], 1: lambda t: t[ia, :, ib], 2: lambda t: t[:, ia, ib].t()}[d]
+        a, b, c = orc.adi_coeffs(faces[d], bcs[d], cfg.alpha)
+        solve = orc.cyclic_thomas if bcs[d] == orc.BC_PERIODIC else orc.thomas
+        ref = np.stack([solve(a, b, c, row) for row in take(field0).cpu().numpy()])
+        for mode_name, mode in (("pdd", tdx.MODE_PDD), ("ppt", tdx.MODE_PPT)):
+            for P in [int(v) for v in args.psweep.split(",")]:
+                if n // P < 2:
+                    continue
+                try:
+                    t = field0.clone()
+                    grid.adi_sweep(d, mode, P, cfg.alpha, t)
+                    torch.cuda.synchronize()
+                    err = float(np.max(np.abs(take(t).cpu().numpy() - ref)) / np.max(np.abs(ref)))
+                    for _ in range(3):
+                        grid.adi_sweep(d, mode, P, cfg.alpha, t)
+                    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    torch.cuda.synchronize(); e0.record()
+                    for _ in range(10):
+                        grid.adi_sweep(d, mode, P, cfg.alpha, t)
+                    e1.record(); torch.cuda.synchronize()
+                    ms = e0.elapsed_time(e1) / 10
+                    drop = grid.pdd_dropped_bound(d, P, cfg.alpha)
+                    print("| %s | %s | %d | %d | %.3f | %.0f | %.1e | %.1e |" % (name, mode_name, P, -(-n // P), ms, BYTES_PER_POINT * cfg.npts / ms / 1e6, drop, err))
+                except tdx.TdxError as e:
+                    print("| %s | %s | %d | %d | - | - | - | %s |" % (name, mode_name, P, -(-n // P), tdx.status_string(e.status)))
+    grid.close()
+
+
 def main():
     args = parse()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
-    if args.selftest_ranks:
+    if args.psweep:
+        if rank == 0:
+            run_psweep(args)
+    elif args.selftest_ranks:
         selftest_ranks(args, rank, world)
     elif args.impl == "reference":
         run_reference(args, rank, world)

@@ -55,7 +55,7 @@ template <> struct VecIO<2> {
 // values in flight and the interface unknowns.  Measured on B200 (profiles/r1_probe_strided.md): spills cost more than
 // occupancy, and 2-4 small co-resident CTAs per SM beat one large one.
 constexpr int strided_regs(int MAXM, int V) {
-    return (MAXM * V <= 8) ? 72 : ((MAXM * V <= 16) ? 104 : ((MAXM * V <= 32) ? 128 : ((MAXM * V <= 48) ? 168 : 232)));
+    return (MAXM * V <= 8) ? 72 : ((MAXM * V <= 16) ? 104 : ((MAXM * V <= 32) ? 128 : ((MAXM * V <= 48) ? 168 : 255)));
 }
 constexpr int strided_block_threads(int MAXM, int V) {            // largest CTA the register budget allows
     return (65536 / strided_regs(MAXM, V)) / 32 * 32 > 1024 ? 1024 : (65536 / strided_regs(MAXM, V)) / 32 * 32;
