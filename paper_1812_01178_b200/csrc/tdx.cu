@@ -63,7 +63,8 @@ struct Plan {
     mutable CUtensorMap tmap;             // x sweeps: tensor map of the field as [lines*P, M] partition rows
     mutable const void* tmap_ptr = nullptr;   // field the cached tensor map was encoded for
     mutable int tmap_box = 0;
-    mutable double uni_host[16 * 6];      // host copy of the uniform row table (kernel parameter of k_unit_tma)
+    mutable long long tmap_rows = 0;
+    mutable double uni_host[32 * 6];      // host copy of the uniform row table (kernel parameter of k_unit_tma)
     mutable bool uni_host_ok = false;
     double alpha = 0.0;
     uint64_t hash = 0;
@@ -468,33 +469,37 @@ tdx_status_t launch_unit_tma_inst(const Plan& pl, UnitTmaArgs& A, const Tables& 
 tdx_status_t run_unit_tma(const Plan& pl, double* data, long long nlines, cudaStream_t st, bool* taken) {
     *taken = false;
     const int q = pl.n / pl.P;
-    if (pl.n % pl.P != 0 || (q != 8 && q != 16) || pl.M != q) return TDX_OK;
+    if (pl.n % pl.P != 0 || (q != 8 && q != 16 && q != 32) || pl.M != q) return TDX_OK;
     if (reinterpret_cast<uintptr_t>(data) % 16 != 0) return TDX_OK;
     EncodeTiledFn enc = encode_tiled_fn();
     if (!enc) return TDX_OK;
+    const int rpp = q > 16 ? q / 16 : 1;                    // 128-byte tile rows per partition
+    const int inner = q > 16 ? 16 : q;                      // doubles per tile row
     UnitTmaArgs A;
-    A.total_rows = nlines * pl.P;
+    A.total_rows = nlines * pl.P * rpp;
     if (A.total_rows >= (1LL << 31)) return TDX_OK;
-    int lpb = 256 / pl.P; if (lpb < 1) lpb = 1; if (lpb > nlines) lpb = (int)nlines;
+    const int cap = 256 / rpp;                              // partitions per CTA: 32 KB of tile
+    int lpb = cap / pl.P; if (lpb < 1) lpb = 1; if (lpb > nlines) lpb = (int)nlines;
     A.rows_per_cta = lpb * pl.P;
-    A.nbox = (A.rows_per_cta + 255) / 256;
-    if (A.rows_per_cta % A.nbox != 0) return TDX_OK;
-    A.box_rows = A.rows_per_cta / A.nbox;
+    const int tile_rows = A.rows_per_cta * rpp;
+    A.nbox = (tile_rows + 255) / 256;
+    if (tile_rows % A.nbox != 0) return TDX_OK;
+    A.box_rows = tile_rows / A.nbox;
     if (A.nbox > 1 && A.box_rows % 8 != 0) return TDX_OK;
     const int threads = (A.rows_per_cta + 31) / 32 * 32;
     if (threads > 1024 || threads * unit_tma_regs(q) > 65536) return TDX_OK;
-    if (pl.tmap_ptr != data || pl.tmap_box != A.box_rows) {
-        cuuint64_t gdim[2] = {(cuuint64_t)q, (cuuint64_t)A.total_rows};
-        cuuint64_t gstr[1] = {(cuuint64_t)q * 8};
-        cuuint32_t box[2] = {(cuuint32_t)q, (cuuint32_t)A.box_rows}, es[2] = {1, 1};
+    if (pl.tmap_ptr != data || pl.tmap_box != A.box_rows || pl.tmap_rows != A.total_rows) {
+        cuuint64_t gdim[2] = {(cuuint64_t)inner, (cuuint64_t)A.total_rows};
+        cuuint64_t gstr[1] = {(cuuint64_t)inner * 8};
+        cuuint32_t box[2] = {(cuuint32_t)inner, (cuuint32_t)A.box_rows}, es[2] = {1, 1};
         CUresult cr = enc(&pl.tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, data, gdim, gstr, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                          q == 16 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_64B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                          q >= 16 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_64B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
         if (cr != CUDA_SUCCESS) return fail(TDX_ERR_CUDA, "cuTensorMapEncodeTiled failed (%d)", (int)cr);
-        pl.tmap_ptr = data; pl.tmap_box = A.box_rows;
+        pl.tmap_ptr = data; pl.tmap_box = A.box_rows; pl.tmap_rows = A.total_rows;
     }
     const size_t smem = (size_t)threads * q * 8 + (size_t)2 * threads * 8 + 16;
-    const unsigned grid = (unsigned)((A.total_rows + A.rows_per_cta - 1) / A.rows_per_cta);
+    const unsigned grid = (unsigned)((nlines * pl.P + A.rows_per_cta - 1) / A.rows_per_cta);
     Tables T = tables_of(pl);
     const bool uni = pl.layout == ROWS_U;
     *taken = true;
@@ -505,6 +510,7 @@ tdx_status_t run_unit_tma(const Plan& pl, double* data, long long nlines, cudaSt
     }
     TDX_TMA_CASE(16)
     TDX_TMA_CASE(8)
+    TDX_TMA_CASE(32)
 #undef TDX_TMA_CASE
     *taken = false;
     return TDX_OK;

@@ -61,43 +61,47 @@ __device__ __forceinline__ void prefetch_tmap(const CUtensorMap* tm) {
 
 // ---- unit-stride direction ------------------------------------------------------------------------------------
 struct UnitTmaArgs {
-    long long total_rows;    // lines * P partition rows in the field
-    int rows_per_cta;        // LPB * P (whole lines), <= TDX_TMA_MAX_BOXES * 256
-    int box_rows;            // rows per TMA box (<= 256); a CTA moves ceil(rows_per_cta / box_rows) boxes
+    long long total_rows;    // tile rows in the field: lines * P * (tile rows per partition)
+    int rows_per_cta;        // partitions per CTA = LPB * P (whole lines)
+    int box_rows;            // tile rows per TMA box (<= 256); a CTA moves nbox boxes
     int nbox;
     int pf;                  // L2 prefetch distance in CTAs (0 = off)
 };
 
-constexpr int unit_tma_regs(int M) { return M <= 8 ? 56 : 80; }
+constexpr int unit_tma_regs(int M) { return M <= 8 ? 56 : (M <= 16 ? 80 : 128); }
 
 // The uniform row table (all partitions identical: uniform grid in x) travels as a kernel parameter: with the row loops
 // fully unrolled every table value is a constant-bank operand of its DFMA -- no load instruction, no L1 wavefront.
 template <int M> struct UniTable { double v[M * 6]; };
 
-// M = rows per partition = doubles per partition row (16 -> 128-byte rows / SWIZZLE_128B, 8 -> 64-byte / SWIZZLE_64B).
+// M = rows per partition = doubles per partition row (16 -> 128-byte rows / SWIZZLE_128B, 8 -> 64-byte / SWIZZLE_64B,
+// 32 -> two 128-byte tile rows per partition: eight lanes then hit four distinct swizzle keys, a 2-way bank conflict that
+// the otherwise idle shared-memory pipe absorbs).
 // UNI: one table for every partition (rows[jj*6+f], warp-uniform); else per-partition columns (rows[(jj*6+f)*P + p]).
 template <int M, bool UNI, bool CYC>
 __global__ void __maxnreg__(unit_tma_regs(M))
 k_unit_tma(const __grid_constant__ CUtensorMap tmap, UnitTmaArgs A, Tables T, const __grid_constant__ UniTable<M> U) {
     extern __shared__ __align__(1024) unsigned char tma_smem[];
-    constexpr int CH = M / 2;                                         // 16-byte chunks per partition row
-    double2* tile = reinterpret_cast<double2*>(tma_smem);             // [blockDim.x][CH] 16-byte chunks, hardware-swizzled
-    const int rows_alloc = blockDim.x;                                 // >= nbox * box_rows (multiple of 32)
-    double* rf = reinterpret_cast<double*>(tile + (size_t)rows_alloc * CH);   // xt_first per row
-    double* rl = rf + rows_alloc;                                              // xt_last per row
+    constexpr int CH = M / 2;                                         // 16-byte chunks per partition
+    constexpr int RPP = (M > 16) ? M / 16 : 1;                        // 128-byte tile rows per partition
+    constexpr int CHR = CH / RPP;                                     // chunks per tile row (8, or 4 for M = 8)
+    double2* tile = reinterpret_cast<double2*>(tma_smem);             // [blockDim.x * RPP][CHR] 16-byte chunks, hardware-swizzled
+    const int rows_alloc = blockDim.x;                                 // partitions; >= rows_per_cta (multiple of 32)
+    double* rf = reinterpret_cast<double*>(tile + (size_t)rows_alloc * CH);   // xt_first per partition
+    double* rl = rf + rows_alloc;                                              // xt_last per partition
     uint64_t* bar = reinterpret_cast<uint64_t*>(rl + rows_alloc);
     const int r = threadIdx.x;
-    const long long row0 = (long long)blockIdx.x * A.rows_per_cta;
+    const long long row0 = (long long)blockIdx.x * A.rows_per_cta * RPP;       // first tile row of this CTA
 
     if (r == 0) {
         if (smem_u32(tma_smem) & 1023u) __trap();                     // the hardware swizzle pattern assumes a 1024-byte aligned tile
         prefetch_tmap(&tmap);
         mbar_init(bar, 1);
         mbar_fence_init();
-        mbar_arrive_expect_tx(bar, (uint32_t)(A.nbox * A.box_rows) * M * 8u);
-        for (int b = 0; b < A.nbox; ++b) tma_load_2d(tile + (size_t)b * A.box_rows * CH, &tmap, 0, (int)(row0 + (long long)b * A.box_rows), bar);
+        mbar_arrive_expect_tx(bar, (uint32_t)(A.nbox * A.box_rows) * CHR * 16u);
+        for (int b = 0; b < A.nbox; ++b) tma_load_2d(tile + (size_t)b * A.box_rows * CHR, &tmap, 0, (int)(row0 + (long long)b * A.box_rows), bar);
         if (A.pf > 0) {
-            const long long prow = row0 + (long long)A.pf * A.rows_per_cta;
+            const long long prow = row0 + (long long)A.pf * A.rows_per_cta * RPP;
             if (prow < A.total_rows)
                 for (int b = 0; b < A.nbox; ++b) tma_prefetch_2d(&tmap, 0, (int)(prow + (long long)b * A.box_rows));
         }
@@ -115,11 +119,15 @@ k_unit_tma(const __grid_constant__ CUtensorMap tmap, UnitTmaArgs A, Tables T, co
 
     double x[M];
     double2* myrow = tile + (size_t)r * CH;
-    // SWIZZLE_128B: chunk ^= row & 7 (128-byte rows); SWIZZLE_64B: chunk ^= (row >> 1) & 3 (64-byte rows)
-    const int key = (M == 16) ? (r & 7) : ((r >> 1) & 3);
+    // SWIZZLE_128B: chunk ^= tile row & 7 (128-byte rows); SWIZZLE_64B: chunk ^= (tile row >> 1) & 3 (64-byte rows)
+    auto slot = [&](int c) -> int {
+        const int trow = r * RPP + c / CHR;
+        const int key = (M == 8) ? ((trow >> 1) & 3) : (trow & 7);
+        return (c / CHR) * CHR + ((c % CHR) ^ key);
+    };
 #pragma unroll
     for (int c = 0; c < CH; ++c) {
-        const double2 t = myrow[c ^ key];
+        const double2 t = myrow[slot(c)];
         x[2 * c] = t.x; x[2 * c + 1] = t.y;
     }
     // Eq.(5): forward y_j = d_j - l_j y_{j-1}, backward xt_j = y_j inv_j - cp_j xt_{j+1}
@@ -162,11 +170,11 @@ k_unit_tma(const __grid_constant__ CUtensorMap tmap, UnitTmaArgs A, Tables T, co
         x[jj] = v;
     }
 #pragma unroll
-    for (int c = 0; c < CH; ++c) myrow[c ^ key] = make_double2(x[2 * c], x[2 * c + 1]);
+    for (int c = 0; c < CH; ++c) myrow[slot(c)] = make_double2(x[2 * c], x[2 * c + 1]);
     fence_proxy_async();                                              // generic-proxy writes -> visible to the TMA store
     __syncthreads();
     if (r == 0) {
-        for (int b = 0; b < A.nbox; ++b) tma_store_2d(&tmap, tile + (size_t)b * A.box_rows * CH, 0, (int)(row0 + (long long)b * A.box_rows));
+        for (int b = 0; b < A.nbox; ++b) tma_store_2d(&tmap, tile + (size_t)b * A.box_rows * CHR, 0, (int)(row0 + (long long)b * A.box_rows));
         tma_commit();
         tma_wait_read<0>();                                           // shared memory must outlive the store's reads
     }
