@@ -91,7 +91,8 @@ tdx_status_t tdx_adi_step(tdx_grid_t* grid, tdx_mode_t mode, int Px, int Py, int
  * x-index i solve (delta2_y - lambda) phi = rhs with lambda = kx2[i] + kz2[m] >= 0, Neumann ends;
  * |b| = |a| + |c| + lambda (L172).  Lines with lambda == 0 exactly are singular and are pinned at j = 0
  * (b_0 := 1, c_0 := 0, d_0 := 0).  kz2: HOST, nm doubles.  kx2: HOST, nx doubles, or NULL for zeros
- * (non-NULL kx2 is not built yet: TDX_ERR_UNSUPPORTED).
+ * A kx2 with non-zero entries gives every line its own matrix: that case is built for mode THOMAS only (on-the-fly
+ * factorisation, device workspace of nx*ny*nm doubles owned by the grid, synchronous); PDD/PPT: TDX_ERR_UNSUPPORTED.
  * rhs_inout: DEVICE, complex128 interleaved [nm][ny][nx] (x fastest) = 2*nm*ny*nx doubles; the matrix is
  * real, so re and im are two right-hand sides of one factorisation.                                       */
 tdx_status_t tdx_helmholtz_wavenumber_solve(tdx_grid_t* grid, tdx_mode_t mode, int P,

@@ -108,6 +108,7 @@ struct tdx_grid {
     std::deque<Plan> plans;            // deque: references stay valid across push_back
     std::mutex mu;
     double* stage = nullptr; size_t stage_bytes = 0;    // device staging for the *_host entry points
+    double* ws = nullptr; size_t ws_bytes = 0;          // per-line Helmholtz (kx2 != 0): c' workspace + device copies of kx2, kz2
     double* stage2 = nullptr; size_t stage2_bytes = 0;  // second staging buffer (Helmholtz part of tdx_step_host)
     cudaStream_t s_up = nullptr, s_comp = nullptr, s_down = nullptr;   // pipeline streams of tdx_step_host
     int n_of(int dir) const { return dir == 0 ? nx : (dir == 1 ? ny : nz); }
@@ -654,7 +655,7 @@ tdx_status_t tdx_grid_destroy(tdx_grid_t* g) {
     cudaSetDevice(g->device);
     for (Plan& p : g->plans) p.release();
     for (int d = 0; d < 3; ++d) { cudaFree(g->faces[d]); cudaFree(g->lo[d]); cudaFree(g->up[d]); cudaFree(g->lo_face[d]); cudaFree(g->up_face[d]); }
-    cudaFree(g->lo_neumann_y); cudaFree(g->up_neumann_y); cudaFree(g->stage); cudaFree(g->stage2);
+    cudaFree(g->lo_neumann_y); cudaFree(g->up_neumann_y); cudaFree(g->stage); cudaFree(g->stage2); cudaFree(g->ws);
     if (g->s_up) cudaStreamDestroy(g->s_up);
     if (g->s_comp) cudaStreamDestroy(g->s_comp);
     if (g->s_down) cudaStreamDestroy(g->s_down);
@@ -744,7 +745,28 @@ tdx_status_t tdx_helmholtz_wavenumber_solve(tdx_grid_t* g, tdx_mode_t mode, int 
     if (kx2) {
         bool any = false;
         for (int i = 0; i < g->nx; ++i) { if (!(kx2[i] >= 0.0)) return fail(TDX_ERR_INVALID_ARG, "kx2[%d] is negative or NaN", i); any |= kx2[i] != 0.0; }
-        if (any) return fail(TDX_ERR_UNSUPPORTED, "non-zero kx2 (per-line matrices) is not built yet");
+        if (any) {
+            // per-line matrices: only the on-the-fly Thomas baseline is built (PPT/PDD per line: SURVEY 8(f) N2/N4)
+            if (mode != TDX_MODE_THOMAS) return fail(TDX_ERR_UNSUPPORTED, "non-zero kx2 (a different matrix per line) is built for mode THOMAS only");
+            CUDA_TRY(cudaSetDevice(g->device));
+            cudaStream_t st = static_cast<cudaStream_t>(stream);
+            const size_t wsb = (size_t)g->nx * g->ny * nm * 8;
+            std::lock_guard<std::mutex> lk(g->mu);
+            if (g->ws_bytes < wsb + (size_t)(g->nx + nm) * 8) {
+                cudaFree(g->ws); g->ws = nullptr; g->ws_bytes = 0;
+                if (cudaMalloc(&g->ws, wsb + (size_t)(g->nx + nm) * 8) != cudaSuccess) { cudaGetLastError(); return fail(TDX_ERR_ALLOC, "workspace allocation of %zu bytes failed", wsb); }
+                g->ws_bytes = wsb + (size_t)(g->nx + nm) * 8;
+            }
+            double* dkx = g->ws + (size_t)g->nx * g->ny * nm;
+            double* dkz = dkx + g->nx;
+            CUDA_TRY(cudaMemcpyAsync(dkx, kx2, (size_t)g->nx * 8, cudaMemcpyHostToDevice, st));
+            CUDA_TRY(cudaMemcpyAsync(dkz, kz2, (size_t)nm * 8, cudaMemcpyHostToDevice, st));
+            dim3 grid((g->nx + 127) / 128, nm);
+            k_thomas_helm_lines<<<grid, 128, 0, st>>>(reinterpret_cast<double2*>(rhs), g->ws, g->nx, g->ny, g->lo_neumann_y, g->up_neumann_y, dkx, dkz);
+            LAUNCH_CHECK("k_thomas_helm_lines");
+            CUDA_TRY(cudaStreamSynchronize(st));               // kx2/kz2 are read from host memory during the call
+            return TDX_OK;
+        }
     }
     CUDA_TRY(cudaSetDevice(g->device));
     cudaStream_t st = static_cast<cudaStream_t>(stream);

@@ -343,6 +343,47 @@ __global__ void k_thomas_strided(StridedArgs A, const double* __restrict__ rows,
     }
 }
 
+// THOMAS mode of the Helmholtz y-solves when the shift differs from line to line (lambda = kx2[i] + kz2[m], the paper's
+// cosine-x / Fourier-z Poisson solve): no table can be shared, so the thread that owns complex
+// line (i, m) factorises on the fly -- a_j = lo_j, c_j = up_j, b_j = -(a_j + c_j) - lambda, Neumann ends, lambda == 0
+// pinned at j = 0 (L172) -- stores the scaled forward-eliminated right-hand side in place and the scaled
+// super-diagonal c'_j in the workspace ws[m][j][i], and substitutes back.  Two passes over HBM: the GPU baseline.
+__global__ void k_thomas_helm_lines(double2* __restrict__ data, double* __restrict__ ws, int nx, int ny,
+                                    const double* __restrict__ lo, const double* __restrict__ up,
+                                    const double* __restrict__ kx2, const double* __restrict__ kz2) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= nx) return;
+    const int m = blockIdx.y;
+    const double lam = __dadd_rn(__ldg(kx2 + i), __ldg(kz2 + m));
+    const bool pinned = lam == 0.0;
+    double2* base = data + (size_t)m * ny * nx + i;
+    double* wb = ws + (size_t)m * ny * nx + i;
+    double cp = 0.0;
+    double2 prev = make_double2(0.0, 0.0);
+    for (int j = 0; j < ny; ++j) {
+        double aj = __ldg(lo + j), cj = __ldg(up + j);
+        double bj = __dsub_rn(-__dadd_rn(aj, cj), lam);
+        if (j == 0) { bj = __dsub_rn(-cj, lam); aj = 0.0; }
+        if (j == ny - 1) { bj = __dsub_rn(-aj, lam); cj = 0.0; }
+        double2 d = base[(size_t)j * nx];
+        if (pinned && j == 0) { bj = 1.0; cj = 0.0; d = make_double2(0.0, 0.0); }
+        const double den = bj - aj * cp;                    // Thomas: c'_j = c_j/den, d'_j = (d_j - a_j d'_{j-1})/den
+        cp = cj / den;
+        prev.x = (d.x - aj * prev.x) / den;
+        prev.y = (d.y - aj * prev.y) / den;
+        base[(size_t)j * nx] = prev;
+        wb[(size_t)j * nx] = cp;
+    }
+    double2 nxt = prev;                                      // x_{n-1} = d'_{n-1}
+    for (int j = ny - 2; j >= 0; --j) {
+        const double c1 = wb[(size_t)j * nx];
+        double2 d = base[(size_t)j * nx];
+        d.x = d.x - c1 * nxt.x; d.y = d.y - c1 * nxt.y;
+        base[(size_t)j * nx] = d;
+        nxt = d;
+    }
+}
+
 template <bool CYC>
 __global__ void k_thomas_unit(double* __restrict__ data, long long nlines, const double* __restrict__ rows,
                               const double* __restrict__ cyc, int n) {

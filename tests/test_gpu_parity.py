@@ -201,3 +201,32 @@ def test_tile_and_partition_extremes(nx, ny, nz, P):
         for mode_name in ("ppt", "pdd"):
             check_sweep(grid, faces, BCS, field, direction, mode_name, P, 2e-4)
     grid.close()
+
+
+def test_helmholtz_per_line_shift_kx2_thomas(cfg2):
+    """lambda = kx'^2(i) + kz'^2(m) (the paper's cosine-x / Fourier-z Poisson solve): every line has its own
+    matrix; built for mode THOMAS (on-the-fly factorisation).  Only the (i = 0, m = 0) line is singular and pinned."""
+    c, faces, grid, _ = cfg2
+    rhs = c.rhs_helmholtz()
+    kz2 = c.kz2()
+    kx2 = inputs.modified_wavenumbers_x(c.nx, c.lx)
+    assert kx2[0] == 0.0 and np.all(kx2[1:] > 0)
+    t = torch.from_numpy(rhs).cuda()
+    grid.helmholtz_wavenumber_solve(tdx.MODE_THOMAS, 1, kx2, kz2, t)
+    torch.cuda.synchronize()
+    out = t.cpu().numpy()
+    ref = orc.helmholtz_solve(rhs.copy(), faces[1], kx2, kz2, orc.MODE_THOMAS, 1)
+    assert out[0, 0, 0] == 0.0                                   # the one pinned point
+    assert np.all(out[0, 0, 1:] != 0.0)
+    for m in range(0, c.nm, 4):                                  # per wavenumber: large low modes must not hide the rest
+        assert relerr(out[m], ref[m]) < TOL_EXACT, (m, relerr(out[m], ref[m]))
+    assert relerr(out, ref) < TOL_EXACT
+    with pytest.raises(tdx.TdxError) as e:                       # per-line PPT is a NEXT row
+        grid.helmholtz_wavenumber_solve(tdx.MODE_PPT, 8, kx2, kz2, t)
+    assert e.value.status == tdx.ERR_UNSUPPORTED
+    # kx2 given but all zero is the shared-matrix fast path
+    t2 = torch.from_numpy(rhs).cuda(); t3 = torch.from_numpy(rhs).cuda()
+    grid.helmholtz_wavenumber_solve(tdx.MODE_PPT, 8, np.zeros(c.nx), kz2, t2)
+    grid.helmholtz_wavenumber_solve(tdx.MODE_PPT, 8, None, kz2, t3)
+    torch.cuda.synchronize()
+    assert torch.equal(t2, t3)
