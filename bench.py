@@ -29,6 +29,9 @@ METRIC = "Gpts/s per ADI sweep direction (fp64 PDD/PPT); achieved HBM GB/s vs pe
 UNIT = "Gpts/s"
 BYTES_PER_POINT = 16.0          # 8 B read + 8 B written per real grid value per sweep
 
+# partitions per line for the per-line-shift Helmholtz solve (kx2 != 0): ny = P*M with M in {8, 12, 16}
+TUNED_P_LINE = {1: 4, 2: 16, 3: 32, 4: 32, 5: 24}
+
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures
 # (profiles/r1_ncu_cfg5_summary.md), valid for mode ppt with the tuned P of the config; bytes.
 NCU_TRAFFIC = {
@@ -330,6 +333,29 @@ def run_tdx(args, rank, world, local_rank):
                                  "frac_of_measured_peak": BYTES_PER_POINT * 9 * cfg.npts / (ms3 * 1e-3) / 1e9 / peak,
                                  "what": "tdx_adi_step: 3 staggered components x (x, y, z) sweeps, 9 field sweeps in 3+ launches"}
         del comps
+
+    # Helmholtz y-solves with a different shift per line (lambda = kx'^2(i) + kz'^2(m), the paper's
+    # cosine-x / Fourier-z Poisson solve): factorisation, spikes and reduced system on the fly.  The call synchronises
+    # (kx2/kz2 are host arrays), so these times include one host round trip.  Reported beside the headline.
+    if not args.no_step3:
+        from paper_1812_01178_b200 import inputs as _inp
+        kx2 = _inp.modified_wavenumbers_x(cfg.nx, cfg.lx)
+        Pl = TUNED_P_LINE[args.config]
+        per_line = {}
+        for mname, mval in (("ppt", tdx.MODE_PPT), ("pdd", tdx.MODE_PDD)):
+            helm.copy_(helm0)
+            for _ in range(2):
+                grid.helmholtz_wavenumber_solve(mval, Pl, kx2, kz2, helm, stream)
+            barrier()
+            s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            s0.record()
+            for _ in range(args.steps):
+                grid.helmholtz_wavenumber_solve(mval, Pl, kx2, kz2, helm, stream)
+            s1.record()
+            barrier()
+            msl = max_over_ranks(s0.elapsed_time(s1) / args.steps, dist, "cuda")
+            per_line[mname] = {"ms": msl, "gb_per_s": BYTES_PER_POINT * pts[3] / (msl * 1e-3) / 1e9, "P": Pl}
+        out["helmholtz_per_line_shift"] = per_line
 
     # end to end through the host-buffer C-ABI calls: pinned host buffers, H2D + solve + D2H inside the timed region
     if not args.no_e2e:

@@ -91,8 +91,10 @@ tdx_status_t tdx_adi_step(tdx_grid_t* grid, tdx_mode_t mode, int Px, int Py, int
  * x-index i solve (delta2_y - lambda) phi = rhs with lambda = kx2[i] + kz2[m] >= 0, Neumann ends;
  * |b| = |a| + |c| + lambda (L172).  Lines with lambda == 0 exactly are singular and are pinned at j = 0
  * (b_0 := 1, c_0 := 0, d_0 := 0).  kz2: HOST, nm doubles.  kx2: HOST, nx doubles, or NULL for zeros
- * A kx2 with non-zero entries gives every line its own matrix: that case is built for mode THOMAS only (on-the-fly
- * factorisation, device workspace of nx*ny*nm doubles owned by the grid, synchronous); PDD/PPT: TDX_ERR_UNSUPPORTED.
+ * A kx2 with non-zero entries gives every line its own matrix (the paper's cosine-x / Fourier-z solve): factorisation,
+ * spikes and reduced system are then computed on the fly per line; THOMAS takes any shape (device workspace of nx*ny*nm
+ * doubles owned by the grid), PDD/PPT need ny = P*M with M in {8,12,16} (else TDX_ERR_UNSUPPORTED).  This case is
+ * synchronous (kx2/kz2 are read during the call).
  * rhs_inout: DEVICE, complex128 interleaved [nm][ny][nx] (x fastest) = 2*nm*ny*nx doubles; the matrix is
  * real, so re and im are two right-hand sides of one factorisation.                                       */
 tdx_status_t tdx_helmholtz_wavenumber_solve(tdx_grid_t* grid, tdx_mode_t mode, int P,

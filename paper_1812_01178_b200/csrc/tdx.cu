@@ -747,20 +747,51 @@ tdx_status_t tdx_helmholtz_wavenumber_solve(tdx_grid_t* g, tdx_mode_t mode, int 
         for (int i = 0; i < g->nx; ++i) { if (!(kx2[i] >= 0.0)) return fail(TDX_ERR_INVALID_ARG, "kx2[%d] is negative or NaN", i); any |= kx2[i] != 0.0; }
         if (any) {
             // per-line matrices: only the on-the-fly Thomas baseline is built (PPT/PDD per line: SURVEY 8(f) N2/N4)
-            if (mode != TDX_MODE_THOMAS) return fail(TDX_ERR_UNSUPPORTED, "non-zero kx2 (a different matrix per line) is built for mode THOMAS only");
+            const int ny = g->ny;
+            const int Mh = (mode != TDX_MODE_THOMAS && P >= 2 && ny % P == 0) ? ny / P : 0;
+            if (mode != TDX_MODE_THOMAS) {
+                if (P < 2 || P > TDX_MAX_P || ny / P < 2) return fail(TDX_ERR_BAD_PARTITION, "P=%d invalid for line length %d", P, ny);
+                if (Mh != 8 && Mh != 12 && Mh != 16)
+                    return fail(TDX_ERR_UNSUPPORTED, "per-line shifts (non-zero kx2) in PDD/PPT mode need ny = P*M with M in {8,12,16}; ny=%d P=%d", ny, P);
+            }
             CUDA_TRY(cudaSetDevice(g->device));
             cudaStream_t st = static_cast<cudaStream_t>(stream);
-            const size_t wsb = (size_t)g->nx * g->ny * nm * 8;
+            const size_t wsb = (mode == TDX_MODE_THOMAS) ? (size_t)g->nx * g->ny * nm * 8 : 0;
             std::lock_guard<std::mutex> lk(g->mu);
             if (g->ws_bytes < wsb + (size_t)(g->nx + nm) * 8) {
                 cudaFree(g->ws); g->ws = nullptr; g->ws_bytes = 0;
                 if (cudaMalloc(&g->ws, wsb + (size_t)(g->nx + nm) * 8) != cudaSuccess) { cudaGetLastError(); return fail(TDX_ERR_ALLOC, "workspace allocation of %zu bytes failed", wsb); }
                 g->ws_bytes = wsb + (size_t)(g->nx + nm) * 8;
             }
-            double* dkx = g->ws + (size_t)g->nx * g->ny * nm;
+            double* dkx = g->ws + wsb / 8;
             double* dkz = dkx + g->nx;
             CUDA_TRY(cudaMemcpyAsync(dkx, kx2, (size_t)g->nx * 8, cudaMemcpyHostToDevice, st));
             CUDA_TRY(cudaMemcpyAsync(dkz, kz2, (size_t)nm * 8, cudaMemcpyHostToDevice, st));
+            if (mode != TDX_MODE_THOMAS) {
+                const int regs = Mh <= 8 ? 128 : (Mh <= 12 ? 168 : 208);
+                int lpc = 8;
+                while (lpc > 1 && (lpc * P > 1024 || lpc * P * regs > 65536)) lpc /= 2;
+                if (lpc * P > 1024 || lpc * P * regs > 65536) return fail(TDX_ERR_UNSUPPORTED, "P=%d partitions do not fit one thread block", P);
+                dim3 block(lpc, P), grid((g->nx + lpc - 1) / lpc, nm);
+                if (grid.y > 65535) return fail(TDX_ERR_UNSUPPORTED, "nm > 65535");
+                const size_t smem = (size_t)14 * P * lpc * 8;
+                const int ppt = mode == TDX_MODE_PPT ? 1 : 0;
+                const int pf = g->sms * 2 * prefetch_waves();
+                double2* d2 = reinterpret_cast<double2*>(rhs);
+                static bool attr_done = false;
+                if (!attr_done) {
+                    CUDA_TRY(cudaFuncSetAttribute(k_helm_lines<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024));
+                    CUDA_TRY(cudaFuncSetAttribute(k_helm_lines<12>, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024));
+                    CUDA_TRY(cudaFuncSetAttribute(k_helm_lines<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024));
+                    attr_done = true;
+                }
+                if (Mh == 8) k_helm_lines<8><<<grid, block, smem, st>>>(d2, g->nx, ny, P, ppt, pf, g->lo_neumann_y, g->up_neumann_y, dkx, dkz);
+                else if (Mh == 12) k_helm_lines<12><<<grid, block, smem, st>>>(d2, g->nx, ny, P, ppt, pf, g->lo_neumann_y, g->up_neumann_y, dkx, dkz);
+                else k_helm_lines<16><<<grid, block, smem, st>>>(d2, g->nx, ny, P, ppt, pf, g->lo_neumann_y, g->up_neumann_y, dkx, dkz);
+                LAUNCH_CHECK("k_helm_lines");
+                CUDA_TRY(cudaStreamSynchronize(st));
+                return TDX_OK;
+            }
             dim3 grid((g->nx + 127) / 128, nm);
             k_thomas_helm_lines<<<grid, 128, 0, st>>>(reinterpret_cast<double2*>(rhs), g->ws, g->nx, g->ny, g->lo_neumann_y, g->up_neumann_y, dkx, dkz);
             LAUNCH_CHECK("k_thomas_helm_lines");

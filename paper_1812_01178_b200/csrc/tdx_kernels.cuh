@@ -384,6 +384,166 @@ __global__ void k_thomas_helm_lines(double2* __restrict__ data, double* __restri
     }
 }
 
+// ---------------------------------------------------------------------------------------------------------
+// PDD / PPT for the Helmholtz y-solves when every line has its own shift lambda = kx2[i] + kz2[m] (
+// the paper's TDMA-C workload after the cosine-x and Fourier-z transforms).  Nothing is
+// matrix-only any more, so the thread that owns (complex line, partition) does the whole of Eq.(5)-(6) on the fly:
+//   forward  : pivots, c'_j, the scaled right-hand side (re, im) and the scaled left spike, one division per row;
+//   backward : xt, the left spike v and the right spike w (w takes the slot of c'_j, which is dead by then);
+// the interface values and spike ends go to shared memory; PDD solves its two 2x2 blocks per thread (Alg.1 step 5), PPT
+// lets the first partition's thread of each line run the block-tridiagonal elimination of Z in natural order (2x2
+// diagonal blocks [[1, w_last],[v_first, 1]]; reading A7) and the others read their two unknowns back;
+// then Eq.(8).  Requires n = P*M exactly.  HBM traffic: 32 B per complex point; lo/up/kx2/kz2 come from L1.
+template <int M>
+__global__ void __maxnreg__(M <= 8 ? 128 : (M <= 12 ? 168 : 208))
+k_helm_lines(double2* __restrict__ data, int nx, int ny, int P, int ppt, int pf,
+             const double* __restrict__ lo, const double* __restrict__ up,
+             const double* __restrict__ kx2, const double* __restrict__ kz2) {
+    extern __shared__ double hs[];
+    const int tx = threadIdx.x, p = threadIdx.y, LPC = blockDim.x;
+    const int i = blockIdx.x * LPC + tx;
+    const bool valid = i < nx;
+    const int m = blockIdx.y;
+    const double lam = valid ? __dadd_rn(__ldg(kx2 + i), __ldg(kz2 + m)) : 1.0;
+    const bool pinned = lam == 0.0;
+    const int start = p * M;
+    double2* base = data + ((size_t)m * ny + start) * nx + i;
+    // shared layout, all indexed [p][tx]: xf, xl (double2), vf, vl, wf, wl; PPT adds beta, idet, r0, r1 (double2 r)
+    const int S = P * LPC;
+    double2* s_xf = reinterpret_cast<double2*>(hs);
+    double2* s_xl = s_xf + S;
+    double* s_vf = reinterpret_cast<double*>(s_xl + S);
+    double* s_vl = s_vf + S;
+    double* s_wf = s_vl + S;
+    double* s_wl = s_wf + S;
+    double2* s_y0 = reinterpret_cast<double2*>(s_wl + S);          // PPT: x_last_{i-1} of interface i at [i][tx]
+    double2* s_y1 = s_y0 + S;                                      // PPT: x_first_i
+    double* s_beta = reinterpret_cast<double*>(s_y1 + S);
+    double* s_idet = s_beta + S;
+    const int me = p * LPC + tx;
+
+    double2 y[M];
+    double f[M], cp[M];
+#pragma unroll
+    for (int jj = 0; jj < M; ++jj) y[jj] = valid ? __ldcs(base + (size_t)jj * nx) : make_double2(0.0, 0.0);
+    if (pf > 0 && (tx & 7) == 0) {                                   // L2 prefetch of the tile `pf` CTAs ahead, one lane per 128-byte line
+        const long long lin = (long long)blockIdx.y * gridDim.x + blockIdx.x + pf;
+        if (lin < (long long)gridDim.x * gridDim.y) {
+            const int by = (int)(lin / gridDim.x), bx = (int)(lin - (long long)by * gridDim.x);
+            if (bx * LPC + tx < nx) {
+                const double2* pb = data + ((size_t)by * ny + start) * nx + bx * LPC + tx;
+#pragma unroll
+                for (int jj = 0; jj < M; ++jj) asm volatile("prefetch.global.L2 [%0];" ::"l"(pb + (size_t)jj * nx));
+            }
+        }
+    }
+    double wl = 0.0;
+    {   // forward elimination of the block (a_first and c_last of the block are zeroed: Alg.1 step 2)
+        double cprev = 0.0, fprev = 0.0;
+        double2 yprev = make_double2(0.0, 0.0);
+#pragma unroll
+        for (int jj = 0; jj < M; ++jj) {
+            const int j = start + jj;
+            double aj = __ldg(lo + j), cj = __ldg(up + j);
+            double bj = __dsub_rn(-__dadd_rn(aj, cj), lam);
+            if (j == 0) { bj = __dsub_rn(-cj, lam); aj = 0.0; }
+            if (j == ny - 1) { bj = __dsub_rn(-aj, lam); cj = 0.0; }
+            if (pinned && j == 0) { bj = 1.0; cj = 0.0; y[0] = make_double2(0.0, 0.0); }
+            const double ae = (jj == 0) ? 0.0 : aj, ce = (jj == M - 1) ? 0.0 : cj;
+            const double inv = 1.0 / (bj - ae * cprev);
+            cp[jj] = ce * inv;
+            y[jj].x = (y[jj].x - ae * yprev.x) * inv;
+            y[jj].y = (y[jj].y - ae * yprev.y) * inv;
+            f[jj] = (jj == 0) ? aj * inv : -ae * fprev * inv;       // left spike: rhs a_first e_first
+            if (jj == M - 1) wl = cj * inv;                          // right spike: rhs c_last e_last
+            cprev = cp[jj]; fprev = f[jj]; yprev = y[jj];
+        }
+    }
+    {   // backward substitution: xt, v, w (w overwrites c')
+        double wn = wl;
+        cp[M - 1] = wl;
+#pragma unroll
+        for (int jj = M - 2; jj >= 0; --jj) {
+            const double c1 = cp[jj];
+            y[jj].x = y[jj].x - c1 * y[jj + 1].x;
+            y[jj].y = y[jj].y - c1 * y[jj + 1].y;
+            f[jj] = f[jj] - c1 * f[jj + 1];
+            wn = -c1 * wn;
+            cp[jj] = wn;
+        }
+    }
+    s_xf[me] = y[0]; s_xl[me] = y[M - 1];
+    s_vf[me] = f[0]; s_vl[me] = f[M - 1];
+    s_wf[me] = cp[0]; s_wl[me] = cp[M - 1];
+    __syncthreads();
+    double2 yL = make_double2(0.0, 0.0), yR = make_double2(0.0, 0.0);
+    if (!ppt) {
+        // PDD: interface blocks [[1, w_last^(i-1)],[v_first^(i), 1]] only
+        if (p >= 1) {
+            const int lft = me - LPC;
+            const double w = s_wl[lft], v = s_vf[me];
+            const double idet = 1.0 / (1.0 - w * v);
+            yL.x = (s_xl[lft].x - w * s_xf[me].x) * idet;
+            yL.y = (s_xl[lft].y - w * s_xf[me].y) * idet;
+        }
+        if (p <= P - 2) {
+            const int rgt = me + LPC;
+            const double w = s_wl[me], v = s_vf[rgt];
+            const double idet = 1.0 / (1.0 - w * v);
+            yR.x = (s_xf[rgt].x - v * s_xl[me].x) * idet;
+            yR.y = (s_xf[rgt].y - v * s_xl[me].y) * idet;
+        }
+    } else {
+        if (p == 0) {
+            // PPT (L126-146, L156): block-tridiagonal elimination of Z, unknown block i = (x_last_{i-1}, x_first_i), i = 1..P-1
+            //   row A_i: v_last^(i-1) s_{i-1} + s_i + w_last^(i-1) t_i = xt_last^(i-1);  row B_i: v_first^(i) s_i + t_i + w_first^(i) t_{i+1} = xt_first^(i)
+            double x01 = 0.0;                                   // (0,1) entry of the previous block's inverse
+            double2 r0p = make_double2(0.0, 0.0), r1p = make_double2(0.0, 0.0);
+            double x00 = 0.0;
+            for (int it = 1; it <= P - 1; ++it) {
+                const int a = (it - 1) * LPC + tx, b = it * LPC + tx;            // partitions it-1 and it
+                const double vlp = s_vl[a];                                      // v_last^(it-1) (0 for partition 0)
+                double beta = s_wl[a];
+                double2 r0 = s_xl[a], r1 = s_xf[b];
+                if (it >= 2) {
+                    const double wfp = s_wf[a];                                  // w_first^(it-1): U_{it-1}
+                    beta -= vlp * x01 * wfp;
+                    const double2 t = make_double2(x00 * r0p.x + x01 * r1p.x, x00 * r0p.y + x01 * r1p.y);
+                    r0.x -= vlp * t.x; r0.y -= vlp * t.y;
+                }
+                const double gamma = s_vf[b];
+                const double idet = 1.0 / (1.0 - beta * gamma);
+                s_beta[b] = beta; s_idet[b] = idet;
+                s_y0[b] = r0; s_y1[b] = r1;
+                x00 = idet; x01 = -beta * idet;
+                r0p = r0; r1p = r1;
+            }
+            double2 tn = make_double2(0.0, 0.0);                                 // t_{i+1}
+            for (int it = P - 1; it >= 1; --it) {
+                const int b = it * LPC + tx;
+                const double beta = s_beta[b], idet = s_idet[b], gamma = s_vf[b];
+                double2 r0 = s_y0[b], r1 = s_y1[b];
+                if (it <= P - 2) { const double wf = s_wf[b]; r1.x -= wf * tn.x; r1.y -= wf * tn.y; }
+                const double2 s = make_double2((r0.x - beta * r1.x) * idet, (r0.y - beta * r1.y) * idet);
+                const double2 t = make_double2((r1.x - gamma * r0.x) * idet, (r1.y - gamma * r0.y) * idet);
+                s_y0[b] = s; s_y1[b] = t;
+                tn = t;
+            }
+        }
+        __syncthreads();
+        if (p >= 1) yL = s_y0[me];                               // x_last_{p-1}
+        if (p <= P - 2) yR = s_y1[me + LPC];                     // x_first_{p+1}
+    }
+    // Eq.(8): x = xt - v yL - w yR
+#pragma unroll
+    for (int jj = 0; jj < M; ++jj) {
+        double2 r = y[jj];
+        r.x = fma(-f[jj], yL.x, r.x); r.y = fma(-f[jj], yL.y, r.y);
+        r.x = fma(-cp[jj], yR.x, r.x); r.y = fma(-cp[jj], yR.y, r.y);
+        if (valid) __stcs(base + (size_t)jj * nx, r);
+    }
+}
+
 template <bool CYC>
 __global__ void k_thomas_unit(double* __restrict__ data, long long nlines, const double* __restrict__ rows,
                               const double* __restrict__ cyc, int n) {

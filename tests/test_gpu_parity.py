@@ -221,8 +221,8 @@ def test_helmholtz_per_line_shift_kx2_thomas(cfg2):
     for m in range(0, c.nm, 4):                                  # per wavenumber: large low modes must not hide the rest
         assert relerr(out[m], ref[m]) < TOL_EXACT, (m, relerr(out[m], ref[m]))
     assert relerr(out, ref) < TOL_EXACT
-    with pytest.raises(tdx.TdxError) as e:                       # per-line PPT is a NEXT row
-        grid.helmholtz_wavenumber_solve(tdx.MODE_PPT, 8, kx2, kz2, t)
+    with pytest.raises(tdx.TdxError) as e:                       # per-line PDD/PPT needs ny = P*M, M in {8,12,16}
+        grid.helmholtz_wavenumber_solve(tdx.MODE_PPT, 4, kx2, kz2, t)
     assert e.value.status == tdx.ERR_UNSUPPORTED
     # kx2 given but all zero is the shared-matrix fast path
     t2 = torch.from_numpy(rhs).cuda(); t3 = torch.from_numpy(rhs).cuda()
@@ -230,3 +230,50 @@ def test_helmholtz_per_line_shift_kx2_thomas(cfg2):
     grid.helmholtz_wavenumber_solve(tdx.MODE_PPT, 8, None, kz2, t3)
     torch.cuda.synchronize()
     assert torch.equal(t2, t3)
+
+
+@pytest.mark.parametrize("P", [8, 16])
+def test_helmholtz_per_line_shift_kx2_ppt_and_pdd(cfg2, P):
+    """Per-line PPT/PDD (k_helm_lines: factorisation, spikes and the reduced system on the fly per line)."""
+    c, faces, grid, _ = cfg2
+    rhs = c.rhs_helmholtz()
+    kz2 = c.kz2()
+    kx2 = inputs.modified_wavenumbers_x(c.nx, c.lx)
+    exact = orc.helmholtz_solve(rhs.copy(), faces[1], kx2, kz2, orc.MODE_THOMAS, 1)
+    t = torch.from_numpy(rhs).cuda()
+    grid.helmholtz_wavenumber_solve(tdx.MODE_PPT, P, kx2, kz2, t)
+    torch.cuda.synchronize()
+    out = t.cpu().numpy()
+    assert out[0, 0, 0] == 0.0
+    err = relerr(out, exact)
+    if err >= TOL_EXACT:
+        ld = orc.helmholtz_solve(rhs.copy(), faces[1], kx2, kz2, orc.MODE_THOMAS_LD, 1)
+        raise AssertionError("gpu-vs-fp64 oracle %.2e; gpu-vs-long double %.2e; fp64 oracle-vs-long double %.2e" % (err, relerr(out, ld), relerr(exact, ld)))
+    for m in range(0, c.nm, 4):
+        assert relerr(out[m], exact[m]) < 1e-11, (m, relerr(out[m], exact[m]))
+    # PDD: equals the oracle's step-by-step PDD; accurate only where the spikes have decayed (high modes), PAPER.md:L172
+    t = torch.from_numpy(rhs).cuda()
+    grid.helmholtz_wavenumber_solve(tdx.MODE_PDD, P, kx2, kz2, t)
+    torch.cuda.synchronize()
+    out = t.cpu().numpy()
+    pdd = orc.helmholtz_solve(rhs.copy(), faces[1], kx2, kz2, orc.MODE_PDD, P)
+    for m in (0, 1, 5, 33, c.nm - 1):
+        assert relerr(out[m], pdd[m]) < 1e-11, (m, relerr(out[m], pdd[m]))
+
+
+def test_helmholtz_per_line_ragged_tile_and_12_row_partitions():
+    """nx not a multiple of the 8-line tile, ny = 96 = 8 x 12."""
+    nx, ny, nz = 50, 96, 12
+    faces = (inputs.faces_uniform(nx, 1.0), inputs.faces_tanh_one_sided(ny, 2.5), inputs.faces_uniform(nz, 1.0))
+    grid = tdx.Grid(nx, ny, nz, *faces, bcs=BCS)
+    nm = nz // 2 + 1
+    rhs = inputs.rhs_complex_uniform((nm, ny, nx), 55)
+    kz2 = inputs.modified_wavenumbers_z(nz, 1.0)
+    kx2 = inputs.modified_wavenumbers_x(nx, 1.0)
+    exact = orc.helmholtz_solve(rhs.copy(), faces[1], kx2, kz2, orc.MODE_THOMAS, 1)
+    for P in (8, 12, 6):                                         # M = 12, 8, 16
+        t = torch.from_numpy(rhs).cuda()
+        grid.helmholtz_wavenumber_solve(tdx.MODE_PPT, P, kx2, kz2, t)
+        torch.cuda.synchronize()
+        assert relerr(t.cpu().numpy(), exact) < TOL_EXACT, P
+    grid.close()
