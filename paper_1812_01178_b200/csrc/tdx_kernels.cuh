@@ -494,40 +494,108 @@ k_helm_lines(double2* __restrict__ data, int nx, int ny, int P, int ppt, int pf,
             yR.y = (s_xf[rgt].y - v * s_xl[me].y) * idet;
         }
     } else {
+        // PPT (L126-146, L156): block-tridiagonal elimination of Z in natural order, unknown block i = (s_i, t_i) =
+        // (x_last_{i-1}, x_first_i), i = 1..K, K = P-1:
+        //   row A_i: v_last^(i-1) s_{i-1} + s_i + w_last^(i-1) t_i = xt_last^(i-1)
+        //   row B_i: v_first^(i) s_i + t_i + w_first^(i) t_{i+1} = xt_first^(i)
+        // i.e. D_i = [[1, beta_i],[gamma_i, 1]], L_i = v_last^(i-1) e0 e0^T, U_i = w_first^(i) e1 e1^T.  Two threads per line
+        // work towards each other: partition 0's thread eliminates downwards through blocks 1..h, partition P-1's thread
+        // upwards through blocks K..h+1; both then solve the 4x4 meeting system and substitute back on their own side.
+        const int K = P - 1;
+        const int h = (K >= 4) ? (K + 1) / 2 : K;               // short systems: one-sided
         if (p == 0) {
-            // PPT (L126-146, L156): block-tridiagonal elimination of Z, unknown block i = (x_last_{i-1}, x_first_i), i = 1..P-1
-            //   row A_i: v_last^(i-1) s_{i-1} + s_i + w_last^(i-1) t_i = xt_last^(i-1);  row B_i: v_first^(i) s_i + t_i + w_first^(i) t_{i+1} = xt_first^(i)
-            double x01 = 0.0;                                   // (0,1) entry of the previous block's inverse
+            double x00 = 0.0, x01 = 0.0;                        // first row of the previous block's inverse
             double2 r0p = make_double2(0.0, 0.0), r1p = make_double2(0.0, 0.0);
-            double x00 = 0.0;
-            for (int it = 1; it <= P - 1; ++it) {
+            for (int it = 1; it <= h; ++it) {
                 const int a = (it - 1) * LPC + tx, b = it * LPC + tx;            // partitions it-1 and it
-                const double vlp = s_vl[a];                                      // v_last^(it-1) (0 for partition 0)
+                const double vlp = s_vl[a];
                 double beta = s_wl[a];
                 double2 r0 = s_xl[a], r1 = s_xf[b];
                 if (it >= 2) {
-                    const double wfp = s_wf[a];                                  // w_first^(it-1): U_{it-1}
-                    beta -= vlp * x01 * wfp;
-                    const double2 t = make_double2(x00 * r0p.x + x01 * r1p.x, x00 * r0p.y + x01 * r1p.y);
-                    r0.x -= vlp * t.x; r0.y -= vlp * t.y;
+                    beta -= vlp * x01 * s_wf[a];
+                    r0.x -= vlp * (x00 * r0p.x + x01 * r1p.x); r0.y -= vlp * (x00 * r0p.y + x01 * r1p.y);
                 }
-                const double gamma = s_vf[b];
-                const double idet = 1.0 / (1.0 - beta * gamma);
+                const double idet = 1.0 / (1.0 - beta * s_vf[b]);
                 s_beta[b] = beta; s_idet[b] = idet;
                 s_y0[b] = r0; s_y1[b] = r1;
                 x00 = idet; x01 = -beta * idet;
                 r0p = r0; r1p = r1;
             }
-            double2 tn = make_double2(0.0, 0.0);                                 // t_{i+1}
-            for (int it = P - 1; it >= 1; --it) {
-                const int b = it * LPC + tx;
-                const double beta = s_beta[b], idet = s_idet[b], gamma = s_vf[b];
-                double2 r0 = s_y0[b], r1 = s_y1[b];
-                if (it <= P - 2) { const double wf = s_wf[b]; r1.x -= wf * tn.x; r1.y -= wf * tn.y; }
-                const double2 s = make_double2((r0.x - beta * r1.x) * idet, (r0.y - beta * r1.y) * idet);
-                const double2 t = make_double2((r1.x - gamma * r0.x) * idet, (r1.y - gamma * r0.y) * idet);
-                s_y0[b] = s; s_y1[b] = t;
-                tn = t;
+        } else if (p == P - 1 && h < K) {
+            double x10 = 0.0, x11 = 0.0;                        // second row of the next block's inverse
+            double2 r0n = make_double2(0.0, 0.0), r1n = make_double2(0.0, 0.0);
+            for (int it = K; it >= h + 1; --it) {
+                const int a = (it - 1) * LPC + tx, b = it * LPC + tx;
+                const double beta = s_wl[a];
+                double gamma = s_vf[b];
+                double2 r0 = s_xl[a], r1 = s_xf[b];
+                if (it <= K - 1) {
+                    const double wf = s_wf[b];                                   // U_it couples t_{it+1}; L_{it+1} = v_last^(it)
+                    gamma -= wf * x10 * s_vl[b];
+                    r1.x -= wf * (x10 * r0n.x + x11 * r1n.x); r1.y -= wf * (x10 * r0n.y + x11 * r1n.y);
+                }
+                const double idet = 1.0 / (1.0 - beta * gamma);
+                s_beta[b] = gamma; s_idet[b] = idet;                             // upper half stores the modified gamma
+                s_y0[b] = r0; s_y1[b] = r1;
+                x10 = -gamma * idet; x11 = idet;
+                r0n = r0; r1n = r1;
+            }
+        }
+        if (h < K) __syncthreads();
+        if (p == 0 || (p == P - 1 && h < K)) {
+            double2 sm = make_double2(0.0, 0.0), tm = make_double2(0.0, 0.0);     // block h
+            double2 sn = make_double2(0.0, 0.0), tn = make_double2(0.0, 0.0);     // block h+1
+            const int bh = h * LPC + tx;
+            const double betah = s_beta[bh], gammah = s_vf[bh];
+            const double2 r0h = s_y0[bh], r1h = s_y1[bh];
+            if (h < K) {
+                const int bn = (h + 1) * LPC + tx;
+                const double betan = s_wl[bh], gamman = s_beta[bn];               // block h+1: original beta, modified gamma
+                const double wfh = s_wf[bh], vlh = s_vl[bh];
+                const double2 r0n = s_y0[bn], r1n = s_y1[bn];
+                const double a11 = 1.0 - gammah * betah, a12 = wfh;
+                const double a21 = gamman * vlh * betah, a22 = 1.0 - gamman * betan;
+                const double idet = 1.0 / (a11 * a22 - a12 * a21);
+                const double2 q1 = make_double2(r1h.x - gammah * r0h.x, r1h.y - gammah * r0h.y);
+                const double2 q2 = make_double2(r1n.x - gamman * (r0n.x - vlh * r0h.x), r1n.y - gamman * (r0n.y - vlh * r0h.y));
+                tm = make_double2((a22 * q1.x - a12 * q2.x) * idet, (a22 * q1.y - a12 * q2.y) * idet);
+                tn = make_double2((a11 * q2.x - a21 * q1.x) * idet, (a11 * q2.y - a21 * q1.y) * idet);
+                sm = make_double2(r0h.x - betah * tm.x, r0h.y - betah * tm.y);
+                sn = make_double2(r0n.x - vlh * sm.x - betan * tn.x, r0n.y - vlh * sm.y - betan * tn.y);
+            } else {                                            // one-sided: block K is the last one
+                const double idet = s_idet[bh];
+                sm = make_double2((r0h.x - betah * r1h.x) * idet, (r0h.y - betah * r1h.y) * idet);
+                tm = make_double2((r1h.x - gammah * r0h.x) * idet, (r1h.y - gammah * r0h.y) * idet);
+            }
+            if (p == 0) {
+                s_y0[bh] = sm; s_y1[bh] = tm;
+                double2 tnx = tm;                                // t_{i+1}
+                for (int it = h - 1; it >= 1; --it) {
+                    const int b = it * LPC + tx;
+                    const double beta = s_beta[b], idet = s_idet[b], gamma = s_vf[b], wf = s_wf[b];
+                    const double2 r0 = s_y0[b];
+                    double2 r1 = s_y1[b];
+                    r1.x -= wf * tnx.x; r1.y -= wf * tnx.y;
+                    const double2 sv = make_double2((r0.x - beta * r1.x) * idet, (r0.y - beta * r1.y) * idet);
+                    const double2 tv = make_double2((r1.x - gamma * r0.x) * idet, (r1.y - gamma * r0.y) * idet);
+                    s_y0[b] = sv; s_y1[b] = tv;
+                    tnx = tv;
+                }
+            } else {
+                const int bn = (h + 1) * LPC + tx;
+                s_y0[bn] = sn; s_y1[bn] = tn;
+                double2 spv = sn;                                // s_{i-1}
+                for (int it = h + 2; it <= K; ++it) {
+                    const int a = (it - 1) * LPC + tx, b = it * LPC + tx;
+                    const double beta = s_wl[a], gamma = s_beta[b], idet = s_idet[b], vlp = s_vl[a];
+                    double2 r0 = s_y0[b];
+                    const double2 r1 = s_y1[b];
+                    r0.x -= vlp * spv.x; r0.y -= vlp * spv.y;
+                    const double2 sv = make_double2((r0.x - beta * r1.x) * idet, (r0.y - beta * r1.y) * idet);
+                    const double2 tv = make_double2((r1.x - gamma * r0.x) * idet, (r1.y - gamma * r0.y) * idet);
+                    s_y0[b] = sv; s_y1[b] = tv;
+                    spv = sv;
+                }
             }
         }
         __syncthreads();
