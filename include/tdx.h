@@ -16,6 +16,8 @@
  *   - Every call returns tdx_status_t.  Argument validation precedes any launch: on an argument error nothing
  *     is written.  tdx_last_error() gives a thread-local message for the last failure on this thread.
  *   - There is no CPU fallback and no other backend: without a CUDA device every solve returns TDX_ERR_CUDA.
+ *   - A grid object caches its plans (at most 64; the oldest are dropped) and is NOT safe for concurrent calls from
+ *     several host threads: use one grid per thread.  Different grids are independent.
  */
 #ifndef TDX_H
 #define TDX_H

@@ -562,8 +562,19 @@ tdx_status_t run_sweep(tdx_grid* g, const Plan& pl, int dir, double* data, cudaS
     return run_strided(pl, data, nx * ny, nx * ny, ncomp, ncomp > 1 ? nx * ny * nz : 0, false, st);
 }
 
+// The plan cache is keyed by (kind, dir, loc, mode, P, alpha / coefficient hash): a caller that keeps changing alpha (variable
+// time step) would grow it without bound, so every public solve entry first drops the oldest plans beyond a cap.  cudaFree
+// waits for the device, so tables of kernels still in flight are safe.  Never called while a plan pointer is held.
+void trim_plans(tdx_grid* g) {
+    std::lock_guard<std::mutex> lk(g->mu);
+    const size_t kMaxPlans = 64, kKeep = 48;
+    if (g->plans.size() <= kMaxPlans) return;
+    while (g->plans.size() > kKeep) { g->plans.front().release(); g->plans.pop_front(); }
+}
+
 tdx_status_t check_common(tdx_grid* g, int dir, int mode, const void* ptr) {
     if (!g) return fail(TDX_ERR_INVALID_ARG, "grid is NULL");
+    trim_plans(g);
     if (dir < 0 || dir > 2) return fail(TDX_ERR_INVALID_ARG, "dir=%d not in {0,1,2}", dir);
     if (mode < 0 || mode > 2) return fail(TDX_ERR_INVALID_ARG, "mode=%d not in {0,1,2}", mode);
     if (!ptr) return fail(TDX_ERR_INVALID_ARG, "data pointer is NULL");
@@ -874,6 +885,7 @@ tdx_status_t tdx_adi_sweep_host(tdx_grid_t* g, tdx_dir_t dir, tdx_mode_t mode, i
 tdx_status_t tdx_step_host(tdx_grid_t* g, tdx_mode_t mode, int Px, int Py, int Pz, double alpha, double* host_field,
                            int Ph, int nm, const double* kz2, double* host_helm) {
     if (!g) return fail(TDX_ERR_INVALID_ARG, "grid is NULL");
+    trim_plans(g);
     if (mode < 0 || mode > 2) return fail(TDX_ERR_INVALID_ARG, "mode=%d not in {0,1,2}", (int)mode);
     if (!host_field && !host_helm) return fail(TDX_ERR_INVALID_ARG, "both host buffers are NULL");
     if (host_helm && (nm < 1 || !kz2)) return fail(TDX_ERR_INVALID_ARG, "nm=%d / kz2 invalid", nm);

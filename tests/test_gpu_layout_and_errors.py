@@ -171,3 +171,24 @@ def test_pipelined_step_host_equals_device_path_bit_exact():
     with pytest.raises(tdx.TdxError):
         grid.step_host(tdx.MODE_PPT, 6, 5, 999, alpha, hf, 4, kz2, hh)
     grid.close()
+
+
+def test_plan_cache_is_bounded_and_rebuilds_evicted_plans(small):
+    """A caller that keeps changing alpha (variable time step) must not grow the plan cache without bound, and a plan
+    that was dropped is rebuilt to the same bits."""
+    (nx, ny, nz), faces, grid = small
+    field = inputs.rhs_uniform((nz, ny, nx), 77)
+    t = torch.from_numpy(field).cuda()
+    grid.adi_sweep(1, tdx.MODE_PPT, 4, 1e-3, t)
+    torch.cuda.synchronize()
+    first = t.clone()
+    free0 = torch.cuda.mem_get_info()[0]
+    for k in range(200):
+        s = torch.from_numpy(field).cuda()
+        grid.adi_sweep(1, tdx.MODE_PPT, 4, 1e-3 * (1.0 + 1e-3 * (k + 1)), s)
+    torch.cuda.synchronize()
+    t2 = torch.from_numpy(field).cuda()
+    grid.adi_sweep(1, tdx.MODE_PPT, 4, 1e-3, t2)                 # evicted by now: rebuilt
+    torch.cuda.synchronize()
+    assert torch.equal(t2, first)
+    assert free0 - torch.cuda.mem_get_info()[0] < 64 * 1024 * 1024   # 200 plans of this grid would be far below this anyway; no leak growth
