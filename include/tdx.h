@@ -103,6 +103,34 @@ tdx_status_t tdx_helmholtz_wavenumber_solve(tdx_grid_t* grid, tdx_mode_t mode, i
                                             int nm, const double* kx2, const double* kz2,
                                             double* rhs_inout, void* stream);
 
+/* Transforms around the Poisson y-solves ("half-range cosine transform in the streamwise x-direction and
+ * Fourier transform in the spanwise z-direction ... after which the pseudo-pressure is obtained via inverse
+ * transforms").  All DEVICE buffers, 16-byte aligned, fp64, no transpose, asynchronous on `stream`.
+ *
+ * tdx_dct_x: in place on field [nz][ny][nx].  inverse == 0: X_k = sum_n x_n cos(pi k (n + 1/2) / nx), k < nx
+ * (cell-centred values, Neumann walls; unnormalised).  inverse != 0: x_n = (1/nx)[X_0 + 2 sum_{k>=1} X_k cos(...)],
+ * the exact inverse.  nx a power of two in [16, 4096], else TDX_ERR_UNSUPPORTED.
+ *
+ * tdx_rfft_z: field_in real [nz][ny][nx] -> spec_out complex128 interleaved [nz/2+1][ny][nx] (the layout
+ * tdx_helmholtz_wavenumber_solve takes), F_m = sum_k f_k exp(-2 pi i m k / nz).  tdx_irfft_z: the inverse including
+ * the 1/nz (imaginary parts of F_0 and F_{nz/2} do not enter).  Out of place (in == out is TDX_ERR_INVALID_ARG); the
+ * input is not modified.  nz a power of two in [16, 1024] and nx even, else TDX_ERR_UNSUPPORTED.               */
+tdx_status_t tdx_dct_x(tdx_grid_t* grid, int inverse, double* field_inout, void* stream);
+tdx_status_t tdx_rfft_z(tdx_grid_t* grid, const double* field_in, double* spec_out, void* stream);
+tdx_status_t tdx_irfft_z(tdx_grid_t* grid, const double* spec_in, double* field_out, void* stream);
+
+/* Direct Poisson solve of PAPER.md:L45 / L170-174 in the paper's order: cosine transform in x, Fourier transform in z,
+ * the y-solves (delta2_y - kx2[i] - kz2[m]) phi^ = f^ (Neumann ends, mode (0,0) pinned at j = 0), inverse Fourier,
+ * inverse cosine: five passes over the field.  field_inout: DEVICE [nz][ny][nx], f in, phi out.  spec_work: DEVICE
+ * scratch of 2*(nz/2+1)*ny*nx doubles (caller-owned).  kx2 (HOST, nx) / kz2 (HOST, nz/2+1): the modified wavenumbers,
+ * or NULL for kx2[i] = 2(1-cos(pi i/nx))/dx^2, kz2[m] = 2(1-cos(2 pi m/nz))/dz^2 of the grid's uniform x / z spacing
+ * (TDX_ERR_UNSUPPORTED if that direction is not uniform).  mode / P: as tdx_helmholtz_wavenumber_solve with per-line
+ * shifts (PDD/PPT need ny = P*M, M in {8,12,16}; the paper uses PPT here because PDD is inaccurate on the weakly
+ * dominant low modes, L172).  Every argument check of every stage precedes the first launch.  Synchronous
+ * (returns when the solve has finished on `stream`).                                                          */
+tdx_status_t tdx_poisson_solve(tdx_grid_t* grid, tdx_mode_t mode, int P, const double* kx2, const double* kz2,
+                               double* field_inout, double* spec_work, void* stream);
+
 /* Batched cyclic tridiagonal solve along dir with caller-given coefficients shared by every line:
  * a, b, c: HOST arrays of n_dir doubles; a[0] couples row 0 to row n-1 and c[n-1] couples row n-1 to row 0.
  * Closure as for tdx_adi_sweep on a periodic direction (Sherman-Morrison with gamma = -b[0] for THOMAS / PDD, cyclic

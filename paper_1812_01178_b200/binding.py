@@ -17,7 +17,7 @@ LOC_CENTER, LOC_FACE = 0, 1
 OK, ERR_INVALID_ARG, ERR_BAD_PARTITION, ERR_ALLOC, ERR_CUDA, ERR_UNSUPPORTED, ERR_PDD_BOUND = 0, -1, -2, -3, -4, -5, -6
 
 EXPORTS = ("tdx_grid_create", "tdx_grid_destroy", "tdx_partition_bounds", "tdx_adi_sweep", "tdx_adi_sweep_at", "tdx_adi_step",
-           "tdx_helmholtz_wavenumber_solve", "tdx_cyclic_solve", "tdx_adi_sweep_host", "tdx_adi_step_host",
+           "tdx_helmholtz_wavenumber_solve", "tdx_dct_x", "tdx_rfft_z", "tdx_irfft_z", "tdx_poisson_solve", "tdx_cyclic_solve", "tdx_adi_sweep_host", "tdx_adi_step_host",
            "tdx_helmholtz_wavenumber_solve_host", "tdx_step_host", "tdx_pdd_dropped_bound", "tdx_kernel_launch_count",
            "tdx_status_string", "tdx_last_error", "tdx_version")
 
@@ -57,6 +57,10 @@ def lib():
         L.tdx_adi_step_host.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_double, C.c_void_p]
         L.tdx_helmholtz_wavenumber_solve_host.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, _dp, _dp, C.c_void_p]
         L.tdx_step_host.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_double, C.c_void_p, C.c_int, C.c_int, _dp, C.c_void_p]
+        L.tdx_dct_x.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p]
+        L.tdx_rfft_z.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.tdx_irfft_z.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.tdx_poisson_solve.argtypes = [C.c_void_p, C.c_int, C.c_int, _dp, _dp, C.c_void_p, C.c_void_p, C.c_void_p]
         L.tdx_pdd_dropped_bound.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_double, _dp]
         _lib = L
     return _lib
@@ -145,6 +149,20 @@ class Grid:
         kz, pkz = _host(kz2)
         _, pkx = _host(kx2)
         _chk(lib().tdx_helmholtz_wavenumber_solve(self._h, mode, P, kz.size, pkx, pkz, _devptr(rhs), C.c_void_p(stream)))
+
+    def dct_x(self, inverse, field, stream=0):
+        _chk(lib().tdx_dct_x(self._h, int(inverse), _devptr(field), C.c_void_p(stream)))
+
+    def rfft_z(self, field_in, spec_out, stream=0):
+        _chk(lib().tdx_rfft_z(self._h, _devptr(field_in), _devptr(spec_out), C.c_void_p(stream)))
+
+    def irfft_z(self, spec_in, field_out, stream=0):
+        _chk(lib().tdx_irfft_z(self._h, _devptr(spec_in), _devptr(field_out), C.c_void_p(stream)))
+
+    def poisson_solve(self, mode, P, kx2, kz2, field, spec_work, stream=0):
+        _, pkx = _host(kx2)
+        _, pkz = _host(kz2)
+        _chk(lib().tdx_poisson_solve(self._h, mode, P, pkx, pkz, _devptr(field), _devptr(spec_work), C.c_void_p(stream)))
 
     def cyclic_solve(self, direction, mode, P, a, b, c, rhs, stream=0):
         (_, pa), (_, pb), (_, pc) = _host(a), _host(b), _host(c)

@@ -20,6 +20,7 @@
 #include "tdx_kernels.cuh"
 #include "tdx_plan.cuh"
 #include "tdx_tma.cuh"
+#include "tdx_fft.cuh"
 
 namespace {
 
@@ -111,6 +112,10 @@ struct tdx_grid {
     double* ws = nullptr; size_t ws_bytes = 0;          // per-line Helmholtz (kx2 != 0): c' workspace + device copies of kx2, kz2
     double* stage2 = nullptr; size_t stage2_bytes = 0;  // second staging buffer (Helmholtz part of tdx_step_host)
     cudaStream_t s_up = nullptr, s_comp = nullptr, s_down = nullptr;   // pipeline streams of tdx_step_host
+    double length[3] = {0, 0, 0};                       // domain length per direction (host copy of faces[n] - faces[0])
+    bool uniform[3] = {false, false, false};            // spacing uniform to 1e-12 relative (the transforms need it in x, z)
+    double2* fft_tw[3] = {nullptr, nullptr, nullptr};   // W_N^q tables of the x / z transforms (tdx_fft.cuh), built on first use
+    double2* fft_w4 = nullptr;                          // exp(-i pi k / 2nx), k <= nx/2 (cosine transform)
     int n_of(int dir) const { return dir == 0 ? nx : (dir == 1 ? ny : nz); }
 };
 
@@ -584,6 +589,114 @@ tdx_status_t check_common(tdx_grid* g, int dir, int mode, const void* ptr) {
 }  // namespace
 
 // ---- C ABI ---------------------------------------------------------------------------------------------------
+// ---- transforms around the Poisson y-solves (tdx_fft.cuh) and the direct Poisson solve --------------------------
+namespace {
+
+bool pow2(int n) { return n > 0 && (n & (n - 1)) == 0; }
+
+tdx_status_t fft_tables(tdx_grid* g, int dir, cudaStream_t st) {
+    std::lock_guard<std::mutex> lk(g->mu);
+    if (g->fft_tw[dir]) return TDX_OK;
+    const int N = g->n_of(dir);
+    double2 *tw = nullptr, *w4 = nullptr;
+    if (cudaMalloc(&tw, (size_t)N * 16) != cudaSuccess) { cudaGetLastError(); return fail(TDX_ERR_ALLOC, "twiddle table allocation failed"); }
+    if (dir == 0 && cudaMalloc(&w4, (size_t)(N / 2 + 1) * 16) != cudaSuccess) { cudaGetLastError(); cudaFree(tw); return fail(TDX_ERR_ALLOC, "twiddle table allocation failed"); }
+    tdx::k_fft_tables<<<(N + 127) / 128, 128, 0, st>>>(tw, w4, N);
+    LAUNCH_CHECK("k_fft_tables");
+    g->fft_tw[dir] = tw;
+    if (dir == 0) g->fft_w4 = w4;
+    return TDX_OK;
+}
+
+template <int N, int C>
+tdx_status_t launch_rfft_z(tdx_grid* g, const double* in, double* out, bool inverse, cudaStream_t st) {
+    const size_t smem = (size_t)N * C * 16;
+    dim3 block(C, N / 8), grid((g->nx + 2 * C - 1) / (2 * C), g->ny);
+    const int resident = std::max(1, std::min((int)(220 * 1024 / smem), 2048 / (C * N / 8)));
+    const int pf = g->sms * resident * prefetch_waves();
+    if (!inverse) {
+        static bool done = false;
+        if (!done) { CUDA_TRY(cudaFuncSetAttribute(k_rfft_z<N, C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); done = true; }
+        k_rfft_z<N, C><<<grid, block, smem, st>>>(in, reinterpret_cast<double2*>(out), g->nx, g->ny, g->fft_tw[2], pf);
+        LAUNCH_CHECK("k_rfft_z");
+    } else {
+        static bool done = false;
+        if (!done) { CUDA_TRY(cudaFuncSetAttribute(k_irfft_z<N, C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); done = true; }
+        k_irfft_z<N, C><<<grid, block, smem, st>>>(reinterpret_cast<const double2*>(in), out, g->nx, g->ny, g->fft_tw[2], pf);
+        LAUNCH_CHECK("k_irfft_z");
+    }
+    return TDX_OK;
+}
+
+tdx_status_t run_fft_z(tdx_grid* g, const double* in, double* out, bool inverse, cudaStream_t st) {
+    if (!g) return fail(TDX_ERR_INVALID_ARG, "grid is NULL");
+    if (!in || !out) return fail(TDX_ERR_INVALID_ARG, "data pointer is NULL");
+    if (in == out) return fail(TDX_ERR_INVALID_ARG, "the z transform is out of place (real nz planes <-> nz/2+1 complex planes)");
+    if ((reinterpret_cast<uintptr_t>(in) | reinterpret_cast<uintptr_t>(out)) & 15) return fail(TDX_ERR_INVALID_ARG, "buffers must be 16-byte aligned");
+    const int N = g->nz;
+    if (!pow2(N) || N < 16 || N > 1024) return fail(TDX_ERR_UNSUPPORTED, "z transform needs nz a power of two in [16, 1024]; nz=%d", N);
+    if (g->nx % 2) return fail(TDX_ERR_UNSUPPORTED, "z transform pairs adjacent x values: nx=%d must be even", g->nx);
+    if (g->ny > 65535) return fail(TDX_ERR_UNSUPPORTED, "ny > 65535");
+    CUDA_TRY(cudaSetDevice(g->device));
+    tdx_status_t rc = fft_tables(g, 2, st);
+    if (rc != TDX_OK) return rc;
+    switch (N) {
+        case 16:   return launch_rfft_z<16, 16>(g, in, out, inverse, st);
+        case 32:   return launch_rfft_z<32, 16>(g, in, out, inverse, st);
+        case 64:   return launch_rfft_z<64, 16>(g, in, out, inverse, st);
+        case 128:  return launch_rfft_z<128, 16>(g, in, out, inverse, st);
+        case 256:  return launch_rfft_z<256, 16>(g, in, out, inverse, st);
+        case 512:  return launch_rfft_z<512, 16>(g, in, out, inverse, st);
+        default:   return launch_rfft_z<1024, 8>(g, in, out, inverse, st);
+    }
+}
+
+template <int N, int LP>
+tdx_status_t launch_dct_x(tdx_grid* g, double* field, bool inverse, cudaStream_t st) {
+    const long long lines = (long long)g->ny * g->nz;
+    const size_t smem = (size_t)LP * (N + N / 8) * 16 + 16;
+    const long long ctas = (lines + 2 * LP - 1) / (2 * LP);
+    if (ctas > 2147483647LL) return fail(TDX_ERR_UNSUPPORTED, "too many lines");
+    const int resident = std::max(1, std::min((int)(220 * 1024 / smem), 2048 / (LP * N / 8)));
+    const int pf = g->sms * resident * prefetch_waves();
+    if (!inverse) {
+        static bool done = false;
+        if (!done) { CUDA_TRY(cudaFuncSetAttribute(k_dct_x<N, LP, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); done = true; }
+        k_dct_x<N, LP, 0><<<(unsigned)ctas, LP * N / 8, smem, st>>>(field, lines, g->fft_tw[0], g->fft_w4, pf);
+    } else {
+        static bool done = false;
+        if (!done) { CUDA_TRY(cudaFuncSetAttribute(k_dct_x<N, LP, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); done = true; }
+        k_dct_x<N, LP, 1><<<(unsigned)ctas, LP * N / 8, smem, st>>>(field, lines, g->fft_tw[0], g->fft_w4, pf);
+    }
+    LAUNCH_CHECK("k_dct_x");
+    return TDX_OK;
+}
+
+tdx_status_t run_dct_x(tdx_grid* g, double* field, bool inverse, cudaStream_t st) {
+    if (!g) return fail(TDX_ERR_INVALID_ARG, "grid is NULL");
+    if (!field) return fail(TDX_ERR_INVALID_ARG, "data pointer is NULL");
+    if (reinterpret_cast<uintptr_t>(field) & 15) return fail(TDX_ERR_INVALID_ARG, "field must be 16-byte aligned");
+    const int N = g->nx;
+    if (!pow2(N) || N < 16 || N > 4096) return fail(TDX_ERR_UNSUPPORTED, "x transform needs nx a power of two in [16, 4096]; nx=%d", N);
+    CUDA_TRY(cudaSetDevice(g->device));
+    tdx_status_t rc = fft_tables(g, 0, st);
+    if (rc != TDX_OK) return rc;
+    switch (N) {
+        case 16:   return launch_dct_x<16, 128>(g, field, inverse, st);
+        case 32:   return launch_dct_x<32, 64>(g, field, inverse, st);
+        case 64:   return launch_dct_x<64, 32>(g, field, inverse, st);
+        case 128:  return launch_dct_x<128, 16>(g, field, inverse, st);
+        case 256:  return launch_dct_x<256, 8>(g, field, inverse, st);
+        case 512:  return launch_dct_x<512, 4>(g, field, inverse, st);
+        case 1024: return launch_dct_x<1024, 2>(g, field, inverse, st);
+        case 2048: return launch_dct_x<2048, 1>(g, field, inverse, st);
+        default:   return launch_dct_x<4096, 1>(g, field, inverse, st);
+    }
+}
+
+}  // namespace
+
+
 extern "C" {
 
 const char* tdx_version(void) { return "tdx 0.1 (sm_100a)"; }
@@ -639,6 +752,11 @@ tdx_status_t tdx_grid_create(int nx, int ny, int nz, const double* xf, const dou
     for (int d = 0; d < 3; ++d) {
         g->bc[d] = bcs[d];
         const int n = ns[d];
+        g->length[d] = fs[d][n] - fs[d][0];
+        const double h = g->length[d] / n;
+        bool uni = true;
+        for (int j = 0; j <= n; ++j) uni = uni && std::fabs(fs[d][j] - (fs[d][0] + j * h)) <= 1e-12 * std::fabs(g->length[d]);
+        g->uniform[d] = uni;
         if (cudaMalloc(&g->faces[d], (size_t)(n + 1) * 8) != cudaSuccess || cudaMalloc(&g->lo[d], (size_t)n * 8) != cudaSuccess ||
             cudaMalloc(&g->up[d], (size_t)n * 8) != cudaSuccess) return bail(fail(TDX_ERR_ALLOC, "device allocation failed"));
         if (cudaMemcpy(g->faces[d], fs[d], (size_t)(n + 1) * 8, cudaMemcpyHostToDevice) != cudaSuccess) return bail(fail(TDX_ERR_CUDA, "face upload failed"));
@@ -667,6 +785,8 @@ tdx_status_t tdx_grid_destroy(tdx_grid_t* g) {
     for (Plan& p : g->plans) p.release();
     for (int d = 0; d < 3; ++d) { cudaFree(g->faces[d]); cudaFree(g->lo[d]); cudaFree(g->up[d]); cudaFree(g->lo_face[d]); cudaFree(g->up_face[d]); }
     cudaFree(g->lo_neumann_y); cudaFree(g->up_neumann_y); cudaFree(g->stage); cudaFree(g->stage2); cudaFree(g->ws);
+    for (int d = 0; d < 3; ++d) cudaFree(g->fft_tw[d]);
+    cudaFree(g->fft_w4);
     if (g->s_up) cudaStreamDestroy(g->s_up);
     if (g->s_comp) cudaStreamDestroy(g->s_comp);
     if (g->s_down) cudaStreamDestroy(g->s_down);
@@ -817,6 +937,58 @@ tdx_status_t tdx_helmholtz_wavenumber_solve(tdx_grid_t* g, tdx_mode_t mode, int 
     if (rc != TDX_OK) return rc;
     const long long nx2 = 2LL * g->nx;      // complex interleaved: 2 nx doubles per row, re/im share the matrix
     return run_strided(*pl, rhs, nx2, nx2, nm, nx2 * g->ny, true, st);
+}
+
+tdx_status_t tdx_dct_x(tdx_grid_t* g, int inverse, double* field, void* stream) {
+    return run_dct_x(g, field, inverse != 0, static_cast<cudaStream_t>(stream));
+}
+
+tdx_status_t tdx_rfft_z(tdx_grid_t* g, const double* field_in, double* spec_out, void* stream) {
+    return run_fft_z(g, field_in, spec_out, false, static_cast<cudaStream_t>(stream));
+}
+
+tdx_status_t tdx_irfft_z(tdx_grid_t* g, const double* spec_in, double* field_out, void* stream) {
+    return run_fft_z(g, spec_in, field_out, true, static_cast<cudaStream_t>(stream));
+}
+
+tdx_status_t tdx_poisson_solve(tdx_grid_t* g, tdx_mode_t mode, int P, const double* kx2, const double* kz2,
+                               double* field, double* spec_work, void* stream) {
+    tdx_status_t rc = check_common(g, TDX_DIR_Y, mode, field);
+    if (rc != TDX_OK) return rc;
+    if (!spec_work) return fail(TDX_ERR_INVALID_ARG, "spec_work is NULL");
+    if (field == spec_work) return fail(TDX_ERR_INVALID_ARG, "field and spec_work must differ");
+    const int nx = g->nx, nz = g->nz, nm = nz / 2 + 1;
+    // every check of the five stages first: nothing is written on an argument error
+    if (!pow2(nx) || nx < 16 || nx > 4096) return fail(TDX_ERR_UNSUPPORTED, "x transform needs nx a power of two in [16, 4096]; nx=%d", nx);
+    if (!pow2(nz) || nz < 16 || nz > 1024) return fail(TDX_ERR_UNSUPPORTED, "z transform needs nz a power of two in [16, 1024]; nz=%d", nz);
+    if ((reinterpret_cast<uintptr_t>(field) | reinterpret_cast<uintptr_t>(spec_work)) & 15) return fail(TDX_ERR_INVALID_ARG, "buffers must be 16-byte aligned");
+    if (mode != TDX_MODE_THOMAS) {
+        if (P < 2 || P > TDX_MAX_P || g->ny / P < 2) return fail(TDX_ERR_BAD_PARTITION, "P=%d invalid for line length %d", P, g->ny);
+        const int Mh = (g->ny % P == 0) ? g->ny / P : 0;
+        if (Mh != 8 && Mh != 12 && Mh != 16)
+            return fail(TDX_ERR_UNSUPPORTED, "per-line shifts in PDD/PPT mode need ny = P*M with M in {8,12,16}; ny=%d P=%d", g->ny, P);
+    }
+    std::vector<double> kx, kz;
+    if (!kx2) {
+        if (!g->uniform[0]) return fail(TDX_ERR_UNSUPPORTED, "cosine transform in x needs uniform x spacing (PAPER.md:L41) or caller-given kx2");
+        kx.resize(nx);
+        const double dx = g->length[0] / nx;
+        for (int i = 0; i < nx; ++i) { const double s = std::sin(0.5 * M_PI * i / nx); kx[i] = 4.0 * s * s / (dx * dx); }   // = 2(1-cos(pi i/nx))/dx^2
+        kx2 = kx.data();
+    }
+    if (!kz2) {
+        if (!g->uniform[2]) return fail(TDX_ERR_UNSUPPORTED, "Fourier transform in z needs uniform z spacing (PAPER.md:L41) or caller-given kz2");
+        kz.resize(nm);
+        const double dz = g->length[2] / nz;
+        for (int m = 0; m < nm; ++m) { const double s = std::sin(M_PI * m / nz); kz[m] = 4.0 * s * s / (dz * dz); }          // = 2(1-cos(2 pi m/nz))/dz^2
+        kz2 = kz.data();
+    }
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    rc = run_dct_x(g, field, false, st);                                       if (rc != TDX_OK) return rc;
+    rc = run_fft_z(g, field, spec_work, false, st);                            if (rc != TDX_OK) return rc;
+    rc = tdx_helmholtz_wavenumber_solve(g, mode, P, nm, kx2, kz2, spec_work, stream);   if (rc != TDX_OK) return rc;
+    rc = run_fft_z(g, spec_work, field, true, st);                             if (rc != TDX_OK) return rc;
+    return run_dct_x(g, field, true, st);
 }
 
 tdx_status_t tdx_pdd_dropped_bound(tdx_grid_t* g, tdx_dir_t dir, int P, double alpha, double* out) {
