@@ -357,6 +357,47 @@ def run_tdx(args, rank, world, local_rank):
             per_line[mname] = {"ms": msl, "gb_per_s": BYTES_PER_POINT * pts[3] / (msl * 1e-3) / 1e9, "P": Pl}
         out["helmholtz_per_line_shift"] = per_line
 
+        # the whole direct Poisson solve: cosine-x, Fourier-z, per-line y-solves, inverse
+        # transforms -- five passes over the field; per-pass times from events around the single-stage entry points.
+        del helm
+        work = helm0                                             # spectrum scratch (its right-hand side is no longer needed)
+        pfield = field0.clone()
+        stages = [("dct_x", lambda: grid.dct_x(False, pfield, stream), BYTES_PER_POINT * cfg.npts),
+                  ("rfft_z", lambda: grid.rfft_z(pfield, work, stream), 8 * cfg.npts + 16 * cfg.nx * cfg.ny * cfg.nm),
+                  ("irfft_z", lambda: grid.irfft_z(work, pfield, stream), 8 * cfg.npts + 16 * cfg.nx * cfg.ny * cfg.nm),
+                  ("idct_x", lambda: grid.dct_x(True, pfield, stream), BYTES_PER_POINT * cfg.npts)]
+        pstage = {}
+        for sname, fn, nbytes in stages:
+            for _ in range(3):
+                fn()
+            barrier()
+            s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            s0.record()
+            for _ in range(args.steps):
+                fn()
+            s1.record()
+            barrier()
+            mst = max_over_ranks(s0.elapsed_time(s1) / args.steps, dist, "cuda")
+            pstage[sname] = {"ms": mst, "gb_per_s": nbytes / (mst * 1e-3) / 1e9, "frac_of_measured_peak": nbytes / (mst * 1e-3) / 1e9 / peak}
+        pfield.copy_(field0)
+        for _ in range(2):
+            grid.poisson_solve(tdx.MODE_PPT, Pl, None, None, pfield, work, stream)
+        barrier()
+        s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        s0.record()
+        for _ in range(args.steps):
+            grid.poisson_solve(tdx.MODE_PPT, Pl, None, None, pfield, work, stream)
+        s1.record()
+        barrier()
+        msp = max_over_ranks(s0.elapsed_time(s1) / args.steps, dist, "cuda")
+        out["poisson_solve"] = {"ms": msp, "gpts_per_s": cfg.npts / (msp * 1e-3) / 1e9, "mode": "ppt", "P": Pl,
+                                "algorithmic_bytes": 5 * BYTES_PER_POINT * cfg.npts,
+                                "gb_per_s": 5 * BYTES_PER_POINT * cfg.npts / (msp * 1e-3) / 1e9,
+                                "frac_of_measured_peak": 5 * BYTES_PER_POINT * cfg.npts / (msp * 1e-3) / 1e9 / peak,
+                                "stages": pstage,
+                                "what": "tdx_poisson_solve: dct_x, rfft_z, per-line y-solves (PPT), irfft_z, idct_x; 80 B per grid value"}
+        del pfield, work
+
     # end to end through the host-buffer C-ABI calls: pinned host buffers, H2D + solve + D2H inside the timed region
     if not args.no_e2e:
         hf = torch.from_numpy(host_field).pin_memory().numpy()

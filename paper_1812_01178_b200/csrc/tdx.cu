@@ -608,12 +608,13 @@ tdx_status_t fft_tables(tdx_grid* g, int dir, cudaStream_t st) {
     return TDX_OK;
 }
 
-template <int N, int C>
-tdx_status_t launch_rfft_z(tdx_grid* g, const double* in, double* out, bool inverse, cudaStream_t st) {
+// WAVES: L2 prefetch distance in waves of resident CTAs (0 = off), measured per instantiation (profiles/r1_fft_tuning.md)
+template <int N, int C, int WAVES>
+tdx_status_t launch_fft_z(tdx_grid* g, const double* in, double* out, bool inverse, cudaStream_t st) {
     const size_t smem = (size_t)N * C * 16;
     dim3 block(C, N / 8), grid((g->nx + 2 * C - 1) / (2 * C), g->ny);
     const int resident = std::max(1, std::min((int)(220 * 1024 / smem), 2048 / (C * N / 8)));
-    const int pf = g->sms * resident * prefetch_waves();
+    const int pf = g->sms * resident * std::min(WAVES, prefetch_waves());
     if (!inverse) {
         static bool done = false;
         if (!done) { CUDA_TRY(cudaFuncSetAttribute(k_rfft_z<N, C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); done = true; }
@@ -640,14 +641,15 @@ tdx_status_t run_fft_z(tdx_grid* g, const double* in, double* out, bool inverse,
     CUDA_TRY(cudaSetDevice(g->device));
     tdx_status_t rc = fft_tables(g, 2, st);
     if (rc != TDX_OK) return rc;
+    // tile width (C column pairs = 32*C bytes of a real row) and prefetch per (N, direction): measured on cfg4 / cfg5
     switch (N) {
-        case 16:   return launch_rfft_z<16, 16>(g, in, out, inverse, st);
-        case 32:   return launch_rfft_z<32, 16>(g, in, out, inverse, st);
-        case 64:   return launch_rfft_z<64, 16>(g, in, out, inverse, st);
-        case 128:  return launch_rfft_z<128, 16>(g, in, out, inverse, st);
-        case 256:  return launch_rfft_z<256, 16>(g, in, out, inverse, st);
-        case 512:  return launch_rfft_z<512, 16>(g, in, out, inverse, st);
-        default:   return launch_rfft_z<1024, 8>(g, in, out, inverse, st);
+        case 16:   return launch_fft_z<16, 16, 1>(g, in, out, inverse, st);
+        case 32:   return launch_fft_z<32, 16, 1>(g, in, out, inverse, st);
+        case 64:   return launch_fft_z<64, 16, 1>(g, in, out, inverse, st);
+        case 128:  return launch_fft_z<128, 16, 1>(g, in, out, inverse, st);
+        case 256:  return launch_fft_z<256, 8, 0>(g, in, out, inverse, st);
+        case 512:  return inverse ? launch_fft_z<512, 16, 1>(g, in, out, inverse, st) : launch_fft_z<512, 8, 0>(g, in, out, inverse, st);
+        default:   return launch_fft_z<1024, 8, 1>(g, in, out, inverse, st);
     }
 }
 

@@ -139,8 +139,9 @@ def test_poisson_solve_cfg2(cfg2, mode, P):
     """Whole direct solve on config 2 (256x128x128) against the oracle's composition, same wavenumber arrays on both sides.
     Tolerance: the y-systems of the lowest modes are nearly singular (|b| = |a| + |c| + lambda with lambda down to
     kx'^2(1) ~ (pi/Lx)^2 against off-diagonals ~ 1/dy_min^2), so rounding differences between two
-    correct fp64 solvers are amplified by kappa ~ 1e6-1e7 there: 1e-10 relative max-norm on phi, with the long-double
-    arbiter reported if it is exceeded, and 1e-12 on the residual of the equation."""
+    correct fp64 solvers are amplified there.  Measured on B200: 3e-14 (THOMAS) to 1e-13 (PPT) on phi, 6e-13 on the
+    residual (the oracle's own residual: 3e-12); gates: 2e-12 on phi (north_star's 1e-12 for one solve, doubled for the
+    four transforms around it), 1e-11 on the residual."""
     c, faces, grid = cfg2
     f = c.rhs_field()
     kx2, kz2 = otr.modified_wavenumbers(c.nx, c.nz, c.lx, 1.0)
@@ -151,15 +152,15 @@ def test_poisson_solve_cfg2(cfg2, mode, P):
     torch.cuda.synchronize()
     phi = t.cpu().numpy()
     err = relerr(phi, ref)
-    assert err < 1e-10, err
+    assert err < 2e-12, err
     r = otr.laplacian(phi, faces[1], c.lx, 1.0) - f
     r[:, 0, :] -= np.mean(r[:, 0, :])                        # the pinned row of the mean mode carries the compatibility defect
-    assert np.max(np.abs(r)) < 1e-9 * np.max(np.abs(f)), np.max(np.abs(r)) / np.max(np.abs(f))
+    assert np.max(np.abs(r)) < 1e-11 * np.max(np.abs(f)), np.max(np.abs(r)) / np.max(np.abs(f))
     # wavenumbers computed by the library (NULL): same answer to rounding of lambda
     t2 = torch.from_numpy(f).cuda()
     grid.poisson_solve(mode, P, None, None, t2, work)
     torch.cuda.synchronize()
-    assert relerr(t2.cpu().numpy(), ref) < 1e-10
+    assert relerr(t2.cpu().numpy(), ref) < 2e-12
 
 
 def test_poisson_solve_manufactured_small_every_element():
@@ -176,5 +177,5 @@ def test_poisson_solve_manufactured_small_every_element():
         torch.cuda.synchronize()
         got = t.cpu().numpy()
         assert relerr(got, phi - np.mean(phi[:, 0, :])) < 1e-9, (mode, P)
-        assert relerr(got, otr.poisson_solve(f, faces[1], 2.0, 1.0)) < 1e-10, (mode, P)
+        assert relerr(got, otr.poisson_solve(f, faces[1], 2.0, 1.0)) < 2e-12, (mode, P)
     grid.close()
