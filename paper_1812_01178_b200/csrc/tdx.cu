@@ -907,7 +907,7 @@ tdx_status_t tdx_helmholtz_wavenumber_solve(tdx_grid_t* g, tdx_mode_t mode, int 
                 if (lpc * P > 1024 || lpc * P * regs > 65536) return fail(TDX_ERR_UNSUPPORTED, "P=%d partitions do not fit one thread block", P);
                 dim3 block(lpc, P), grid((g->nx + lpc - 1) / lpc, nm);
                 if (grid.y > 65535) return fail(TDX_ERR_UNSUPPORTED, "nm > 65535");
-                const size_t smem = (size_t)14 * P * lpc * 8;
+                const size_t smem = (size_t)30 * P * lpc * 8;          // interface values 8, y0/y1 4, PCR buffers 2 x 9 (tdx_kernels.cuh)
                 const int ppt = mode == TDX_MODE_PPT ? 1 : 0;
                 const int pf = g->sms * 2 * prefetch_waves();
                 double2* d2 = reinterpret_cast<double2*>(rhs);

@@ -391,8 +391,8 @@ __global__ void k_thomas_helm_lines(double2* __restrict__ data, double* __restri
 //   forward  : pivots, c'_j, the scaled right-hand side (re, im) and the scaled left spike, one division per row;
 //   backward : xt, the left spike v and the right spike w (w takes the slot of c'_j, which is dead by then);
 // the interface values and spike ends go to shared memory; PDD solves its two 2x2 blocks per thread (Alg.1 step 5), PPT
-// lets the first partition's thread of each line run the block-tridiagonal elimination of Z in natural order (2x2
-// diagonal blocks [[1, w_last],[v_first, 1]]; reading A7) and the others read their two unknowns back;
+// solves the block-tridiagonal Z in natural order (2x2 diagonal blocks [[1, w_last],[v_first, 1]]; DESIGN.md reading
+// A7) by block parallel cyclic reduction over the line's P threads, ceil(log2(P-1)) steps of one division each;
 // then Eq.(8).  Requires n = P*M exactly.  HBM traffic: 32 B per complex point; lo/up/kx2/kz2 come from L1.
 template <int M>
 __global__ void __maxnreg__(M <= 8 ? 128 : (M <= 12 ? 168 : 208))
@@ -416,10 +416,8 @@ k_helm_lines(double2* __restrict__ data, int nx, int ny, int P, int ppt, int pf,
     double* s_vl = s_vf + S;
     double* s_wf = s_vl + S;
     double* s_wl = s_wf + S;
-    double2* s_y0 = reinterpret_cast<double2*>(s_wl + S);          // PPT: x_last_{i-1} of interface i at [i][tx]
-    double2* s_y1 = s_y0 + S;                                      // PPT: x_first_i
-    double* s_beta = reinterpret_cast<double*>(s_y1 + S);
-    double* s_idet = s_beta + S;
+    double2* s_y0 = reinterpret_cast<double2*>(s_wl + S);          // (spare)
+    double2* s_y1 = s_y0 + S;                                      // PPT: x_first_i; the PCR buffers follow it
     const int me = p * LPC + tx;
 
     double2 y[M];
@@ -494,113 +492,65 @@ k_helm_lines(double2* __restrict__ data, int nx, int ny, int P, int ppt, int pf,
             yR.y = (s_xf[rgt].y - v * s_xl[me].y) * idet;
         }
     } else {
-        // PPT (L126-146, L156): block-tridiagonal elimination of Z in natural order, unknown block i = (s_i, t_i) =
+        // PPT (L126-146, L156): the reduced system Z in natural order, unknown block i = (s_i, t_i) =
         // (x_last_{i-1}, x_first_i), i = 1..K, K = P-1:
-        //   row A_i: v_last^(i-1) s_{i-1} + s_i + w_last^(i-1) t_i = xt_last^(i-1)
-        //   row B_i: v_first^(i) s_i + t_i + w_first^(i) t_{i+1} = xt_first^(i)
-        // i.e. D_i = [[1, beta_i],[gamma_i, 1]], L_i = v_last^(i-1) e0 e0^T, U_i = w_first^(i) e1 e1^T.  Two threads per line
-        // work towards each other: partition 0's thread eliminates downwards through blocks 1..h, partition P-1's thread
-        // upwards through blocks K..h+1; both then solve the 4x4 meeting system and substitute back on their own side.
+        //   row A_i: l_i s_{i-1} + s_i + beta_i t_i = r0_i      l_i = v_last^(i-1), beta_i = w_last^(i-1)
+        //   row B_i: gamma_i s_i + t_i + u_i t_{i+1} = r1_i     gamma_i = v_first^(i), u_i = w_first^(i)
+        // i.e. block tridiagonal with D_i = [[1, beta_i],[gamma_i, 1]] and rank-one couplings L_i = l_i e0 e0^T,
+        // U_i = u_i e1 e1^T.  Solved by block parallel cyclic reduction across the line's P threads (thread p owns block
+        // p): a step of distance d substitutes blocks i-d and i+d into block i,
+        //   beta_i += l_i u_{i-d} e01_{i-d},  r0_i -= l_i (D^-1 r)_{i-d,0},  l_i <- -l_i l_{i-d} idet_{i-d},
+        //   gamma_i += u_i l_{i+d} e10_{i+d}, r1_i -= u_i (D^-1 r)_{i+d,1},  u_i <- -u_i u_{i+d} idet_{i+d},
+        // (idet = 1/(1 - beta gamma), e01 = beta idet, e10 = gamma idet) which keeps the form of D, L and U; after
+        // ceil(log2 K) steps the blocks are decoupled and (s_i, t_i) = D_i^-1 r_i.  No pivoting is needed in this order
+        // (unit diagonal, |spikes| < 1; reading A7 -- the permuted Z-bar of Eq.(10) would need it).
         const int K = P - 1;
-        const int h = (K >= 4) ? (K + 1) / 2 : K;               // short systems: one-sided
-        if (p == 0) {
-            double x00 = 0.0, x01 = 0.0;                        // first row of the previous block's inverse
-            double2 r0p = make_double2(0.0, 0.0), r1p = make_double2(0.0, 0.0);
-            for (int it = 1; it <= h; ++it) {
-                const int a = (it - 1) * LPC + tx, b = it * LPC + tx;            // partitions it-1 and it
-                const double vlp = s_vl[a];
-                double beta = s_wl[a];
-                double2 r0 = s_xl[a], r1 = s_xf[b];
-                if (it >= 2) {
-                    beta -= vlp * x01 * s_wf[a];
-                    r0.x -= vlp * (x00 * r0p.x + x01 * r1p.x); r0.y -= vlp * (x00 * r0p.y + x01 * r1p.y);
-                }
-                const double idet = 1.0 / (1.0 - beta * s_vf[b]);
-                s_beta[b] = beta; s_idet[b] = idet;
-                s_y0[b] = r0; s_y1[b] = r1;
-                x00 = idet; x01 = -beta * idet;
-                r0p = r0; r1p = r1;
-            }
-        } else if (p == P - 1 && h < K) {
-            double x10 = 0.0, x11 = 0.0;                        // second row of the next block's inverse
-            double2 r0n = make_double2(0.0, 0.0), r1n = make_double2(0.0, 0.0);
-            for (int it = K; it >= h + 1; --it) {
-                const int a = (it - 1) * LPC + tx, b = it * LPC + tx;
-                const double beta = s_wl[a];
-                double gamma = s_vf[b];
-                double2 r0 = s_xl[a], r1 = s_xf[b];
-                if (it <= K - 1) {
-                    const double wf = s_wf[b];                                   // U_it couples t_{it+1}; L_{it+1} = v_last^(it)
-                    gamma -= wf * x10 * s_vl[b];
-                    r1.x -= wf * (x10 * r0n.x + x11 * r1n.x); r1.y -= wf * (x10 * r0n.y + x11 * r1n.y);
-                }
-                const double idet = 1.0 / (1.0 - beta * gamma);
-                s_beta[b] = gamma; s_idet[b] = idet;                             // upper half stores the modified gamma
-                s_y0[b] = r0; s_y1[b] = r1;
-                x10 = -gamma * idet; x11 = idet;
-                r0n = r0; r1n = r1;
-            }
+        double beta = 0.0, gamma = 0.0, l = 0.0, u = 0.0;
+        double2 r0 = make_double2(0.0, 0.0), r1 = make_double2(0.0, 0.0);
+        if (p >= 1) {
+            const int a = me - LPC;                                  // partition p-1
+            beta = s_wl[a]; gamma = s_vf[me];
+            l = (p >= 2) ? s_vl[a] : 0.0;
+            u = (p <= K - 1) ? s_wf[me] : 0.0;
+            r0 = s_xl[a]; r1 = s_xf[me];
         }
-        if (h < K) __syncthreads();
-        if (p == 0 || (p == P - 1 && h < K)) {
-            double2 sm = make_double2(0.0, 0.0), tm = make_double2(0.0, 0.0);     // block h
-            double2 sn = make_double2(0.0, 0.0), tn = make_double2(0.0, 0.0);     // block h+1
-            const int bh = h * LPC + tx;
-            const double betah = s_beta[bh], gammah = s_vf[bh];
-            const double2 r0h = s_y0[bh], r1h = s_y1[bh];
-            if (h < K) {
-                const int bn = (h + 1) * LPC + tx;
-                const double betan = s_wl[bh], gamman = s_beta[bn];               // block h+1: original beta, modified gamma
-                const double wfh = s_wf[bh], vlh = s_vl[bh];
-                const double2 r0n = s_y0[bn], r1n = s_y1[bn];
-                const double a11 = 1.0 - gammah * betah, a12 = wfh;
-                const double a21 = gamman * vlh * betah, a22 = 1.0 - gamman * betan;
-                const double idet = 1.0 / (a11 * a22 - a12 * a21);
-                const double2 q1 = make_double2(r1h.x - gammah * r0h.x, r1h.y - gammah * r0h.y);
-                const double2 q2 = make_double2(r1n.x - gamman * (r0n.x - vlh * r0h.x), r1n.y - gamman * (r0n.y - vlh * r0h.y));
-                tm = make_double2((a22 * q1.x - a12 * q2.x) * idet, (a22 * q1.y - a12 * q2.y) * idet);
-                tn = make_double2((a11 * q2.x - a21 * q1.x) * idet, (a11 * q2.y - a21 * q1.y) * idet);
-                sm = make_double2(r0h.x - betah * tm.x, r0h.y - betah * tm.y);
-                sn = make_double2(r0n.x - vlh * sm.x - betan * tn.x, r0n.y - vlh * sm.y - betan * tn.y);
-            } else {                                            // one-sided: block K is the last one
-                const double idet = s_idet[bh];
-                sm = make_double2((r0h.x - betah * r1h.x) * idet, (r0h.y - betah * r1h.y) * idet);
-                tm = make_double2((r1h.x - gammah * r0h.x) * idet, (r1h.y - gammah * r0h.y) * idet);
-            }
-            if (p == 0) {
-                s_y0[bh] = sm; s_y1[bh] = tm;
-                double2 tnx = tm;                                // t_{i+1}
-                for (int it = h - 1; it >= 1; --it) {
-                    const int b = it * LPC + tx;
-                    const double beta = s_beta[b], idet = s_idet[b], gamma = s_vf[b], wf = s_wf[b];
-                    const double2 r0 = s_y0[b];
-                    double2 r1 = s_y1[b];
-                    r1.x -= wf * tnx.x; r1.y -= wf * tnx.y;
-                    const double2 sv = make_double2((r0.x - beta * r1.x) * idet, (r0.y - beta * r1.y) * idet);
-                    const double2 tv = make_double2((r1.x - gamma * r0.x) * idet, (r1.y - gamma * r0.y) * idet);
-                    s_y0[b] = sv; s_y1[b] = tv;
-                    tnx = tv;
+        double* pc = reinterpret_cast<double*>(s_y1 + S);            // 2 buffers x {idet, e01, e10, l, u, q0 (2), q1 (2)} x S
+        int buf = 0;
+        double2 q0, q1;
+        for (int d = 1;; d <<= 1) {
+            const double idet = 1.0 / (1.0 - beta * gamma);
+            q0 = make_double2((r0.x - beta * r1.x) * idet, (r0.y - beta * r1.y) * idet);
+            q1 = make_double2((r1.x - gamma * r0.x) * idet, (r1.y - gamma * r0.y) * idet);
+            if (d >= K) break;                                       // uniform over the CTA
+            double* B = pc + (size_t)buf * 9 * S;
+            B[me] = idet; B[S + me] = beta * idet; B[2 * S + me] = gamma * idet; B[3 * S + me] = l; B[4 * S + me] = u;
+            reinterpret_cast<double2*>(B + 5 * S)[me] = q0;
+            reinterpret_cast<double2*>(B + 7 * S)[me] = q1;
+            __syncthreads();
+            if (p >= 1) {
+                double ln = 0.0, un = 0.0;
+                if (p - d >= 1) {
+                    const int L = me - d * LPC;
+                    const double2 qL = reinterpret_cast<const double2*>(B + 5 * S)[L];
+                    beta = fma(l * B[4 * S + L], B[S + L], beta);
+                    r0.x = fma(-l, qL.x, r0.x); r0.y = fma(-l, qL.y, r0.y);
+                    ln = -l * B[3 * S + L] * B[L];
                 }
-            } else {
-                const int bn = (h + 1) * LPC + tx;
-                s_y0[bn] = sn; s_y1[bn] = tn;
-                double2 spv = sn;                                // s_{i-1}
-                for (int it = h + 2; it <= K; ++it) {
-                    const int a = (it - 1) * LPC + tx, b = it * LPC + tx;
-                    const double beta = s_wl[a], gamma = s_beta[b], idet = s_idet[b], vlp = s_vl[a];
-                    double2 r0 = s_y0[b];
-                    const double2 r1 = s_y1[b];
-                    r0.x -= vlp * spv.x; r0.y -= vlp * spv.y;
-                    const double2 sv = make_double2((r0.x - beta * r1.x) * idet, (r0.y - beta * r1.y) * idet);
-                    const double2 tv = make_double2((r1.x - gamma * r0.x) * idet, (r1.y - gamma * r0.y) * idet);
-                    s_y0[b] = sv; s_y1[b] = tv;
-                    spv = sv;
+                if (p + d <= K) {
+                    const int R = me + d * LPC;
+                    const double2 qR = reinterpret_cast<const double2*>(B + 7 * S)[R];
+                    gamma = fma(u * B[3 * S + R], B[2 * S + R], gamma);
+                    r1.x = fma(-u, qR.x, r1.x); r1.y = fma(-u, qR.y, r1.y);
+                    un = -u * B[4 * S + R] * B[R];
                 }
+                l = ln; u = un;
             }
+            buf ^= 1;
         }
+        s_y1[me] = q1;                                               // t_p = x_first_p
         __syncthreads();
-        if (p >= 1) yL = s_y0[me];                               // x_last_{p-1}
-        if (p <= P - 2) yR = s_y1[me + LPC];                     // x_first_{p+1}
+        if (p >= 1) yL = q0;                                         // s_p = x_last_{p-1}
+        if (p <= P - 2) yR = s_y1[me + LPC];                         // t_{p+1} = x_first_{p+1}
     }
     // Eq.(8): x = xt - v yL - w yR
 #pragma unroll
