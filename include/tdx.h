@@ -131,6 +131,38 @@ tdx_status_t tdx_irfft_z(tdx_grid_t* grid, const double* spec_in, double* field_
 tdx_status_t tdx_poisson_solve(tdx_grid_t* grid, tdx_mode_t mode, int P, const double* kx2, const double* kz2,
                                double* field_inout, double* spec_work, void* stream);
 
+/* The paper's decomposition one level up (Algorithm 1 L222-258, L156/L174): the field is
+ * cut into slabs along `dir` (y in the paper; z also taken), one slab per GPU / rank, and every rank is ONE partition
+ * of the PDD or PPT method; inside the rank the slab's lines are solved by the intra-GPU sweeps above.
+ *
+ * tdx_slab_create: `slab_grid` describes this rank's slab (its extent along dir = the rank's share of n_global under
+ * the partition map of tdx_partition_bounds(n_global, nranks); the other two extents are the whole domain's; the
+ * grid's own faces / boundary condition along dir are not used).  faces_global: HOST, n_global+1 face coordinates of
+ * the whole line; bc_global: Dirichlet or Neumann (a periodic slab direction is TDX_ERR_UNSUPPORTED); alpha as in
+ * tdx_adi_sweep; across: PDD (neighbour exchange, exact where the spikes have decayed, L148-154) or PPT (all-gather,
+ * exact, L126-146); local_mode / P_local: how the rank solves its own slab (THOMAS, or PDD / PPT with P_local
+ * partitions per line).  The slab borrows slab_grid (destroy the slab first).  Plan-time work (global operator rows,
+ * the cut slab operator, the rank's spikes, the rank-level reduced system) runs in CUDA kernels at creation.
+ *
+ * One sweep = three calls, all asynchronous on `stream`, all DEVICE buffers, 16-byte aligned:
+ *   tdx_slab_eliminate  field_inout [slab] d -> xt = A_r^-1 d in place (Alg.1 steps 2-3) and iface_out[2][plane] =
+ *                       (row 0, row n_loc-1) of xt; plane = the slab's other two extents (x fastest).
+ *   (caller)            exchange: PDD -- send iface_out[0] to rank-1 and iface_out[1] to rank+1 (steps 4, 6);
+ *                       PPT -- all-gather every rank's iface_out into [nranks][2][plane] (L156, L174).
+ *   tdx_slab_correct    iface_own = this rank's iface_out; iface_nbr = PDD: [2][plane] = (xt_last of rank-1, xt_first
+ *                       of rank+1), entries of a missing neighbour are not read; PPT: the gathered [nranks][2][plane].
+ *                       Solves the interface unknowns per line (step 5 / Eq.(7)) and applies Eq.(8) (step 7) in place.
+ * tdx_slab_dropped_bound: max |v_last|, |w_first| over interior ranks, the entries PDD across ranks deletes (L152). */
+typedef struct tdx_slab tdx_slab_t;
+tdx_status_t tdx_slab_create(tdx_grid_t* slab_grid, tdx_dir_t dir, int rank, int nranks, int n_global,
+                             const double* faces_global, tdx_bc_t bc_global, double alpha, tdx_mode_t across,
+                             tdx_mode_t local_mode, int P_local, tdx_slab_t** out);
+tdx_status_t tdx_slab_destroy(tdx_slab_t* slab);
+tdx_status_t tdx_slab_eliminate(tdx_slab_t* slab, double* field_inout, double* iface_out, void* stream);
+tdx_status_t tdx_slab_correct(tdx_slab_t* slab, double* field_inout, const double* iface_own, const double* iface_nbr,
+                              void* stream);
+tdx_status_t tdx_slab_dropped_bound(tdx_slab_t* slab, double* out);
+
 /* Batched cyclic tridiagonal solve along dir with caller-given coefficients shared by every line:
  * a, b, c: HOST arrays of n_dir doubles; a[0] couples row 0 to row n-1 and c[n-1] couples row n-1 to row 0.
  * Closure as for tdx_adi_sweep on a periodic direction (Sherman-Morrison with gamma = -b[0] for THOMAS / PDD, cyclic

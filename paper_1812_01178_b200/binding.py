@@ -17,7 +17,7 @@ LOC_CENTER, LOC_FACE = 0, 1
 OK, ERR_INVALID_ARG, ERR_BAD_PARTITION, ERR_ALLOC, ERR_CUDA, ERR_UNSUPPORTED, ERR_PDD_BOUND = 0, -1, -2, -3, -4, -5, -6
 
 EXPORTS = ("tdx_grid_create", "tdx_grid_destroy", "tdx_partition_bounds", "tdx_adi_sweep", "tdx_adi_sweep_at", "tdx_adi_step",
-           "tdx_helmholtz_wavenumber_solve", "tdx_dct_x", "tdx_rfft_z", "tdx_irfft_z", "tdx_poisson_solve", "tdx_cyclic_solve", "tdx_adi_sweep_host", "tdx_adi_step_host",
+           "tdx_helmholtz_wavenumber_solve", "tdx_dct_x", "tdx_rfft_z", "tdx_irfft_z", "tdx_poisson_solve", "tdx_slab_create", "tdx_slab_destroy", "tdx_slab_eliminate", "tdx_slab_correct", "tdx_slab_dropped_bound", "tdx_cyclic_solve", "tdx_adi_sweep_host", "tdx_adi_step_host",
            "tdx_helmholtz_wavenumber_solve_host", "tdx_step_host", "tdx_pdd_dropped_bound", "tdx_kernel_launch_count",
            "tdx_status_string", "tdx_last_error", "tdx_version")
 
@@ -61,6 +61,11 @@ def lib():
         L.tdx_rfft_z.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.tdx_irfft_z.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.tdx_poisson_solve.argtypes = [C.c_void_p, C.c_int, C.c_int, _dp, _dp, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.tdx_slab_create.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, _dp, C.c_int, C.c_double, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_void_p)]
+        L.tdx_slab_destroy.argtypes = [C.c_void_p]
+        L.tdx_slab_eliminate.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.tdx_slab_correct.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.tdx_slab_dropped_bound.argtypes = [C.c_void_p, _dp]
         L.tdx_pdd_dropped_bound.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_double, _dp]
         _lib = L
     return _lib
@@ -190,4 +195,38 @@ class Grid:
     def pdd_dropped_bound(self, direction, P, alpha):
         out = C.c_double(0.0)
         _chk(lib().tdx_pdd_dropped_bound(self._h, direction, P, alpha, C.byref(out)))
+        return out.value
+
+
+class Slab:
+    """tdx_slab_t: one rank's share of a slab-decomposed sweep (include/tdx.h).  Holds a reference to its grid."""
+
+    def __init__(self, slab_grid, direction, rank, nranks, faces_global, bc_global, alpha, across, local_mode, P_local):
+        f, pf = _host(faces_global)
+        self._grid = slab_grid
+        self._h = C.c_void_p()
+        self.rank, self.nranks, self.direction = rank, nranks, direction
+        _chk(lib().tdx_slab_create(slab_grid._h, direction, rank, nranks, f.size - 1, pf, bc_global, float(alpha), across,
+                                   local_mode, P_local, C.byref(self._h)))
+
+    def close(self):
+        if self._h:
+            lib().tdx_slab_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def eliminate(self, field, iface_out, stream=0):
+        _chk(lib().tdx_slab_eliminate(self._h, _devptr(field), _devptr(iface_out), C.c_void_p(stream)))
+
+    def correct(self, field, iface_own, iface_nbr, stream=0):
+        _chk(lib().tdx_slab_correct(self._h, _devptr(field), _devptr(iface_own), _devptr(iface_nbr) if iface_nbr is not None else None, C.c_void_p(stream)))
+
+    def dropped_bound(self):
+        out = C.c_double(0.0)
+        _chk(lib().tdx_slab_dropped_bound(self._h, C.byref(out)))
         return out.value

@@ -21,6 +21,7 @@
 #include "tdx_plan.cuh"
 #include "tdx_tma.cuh"
 #include "tdx_fft.cuh"
+#include "tdx_slab.cuh"
 
 namespace {
 
@@ -49,7 +50,7 @@ struct DevBuf {
     template <class T> T* as() { return static_cast<T*>(p); }
 };
 
-enum PlanKind { KIND_ADI = 0, KIND_HELM = 1, KIND_USER = 2 };
+enum PlanKind { KIND_ADI = 0, KIND_HELM = 1, KIND_USER = 2, KIND_USERNP = 3 };   // USER: cyclic caller coefficients; USERNP: the same, not periodic
 
 struct Plan {
     int kind = 0, dir = 0, mode = 0, P = 1, n = 0, nsets = 1;
@@ -276,7 +277,7 @@ tdx_status_t get_plan(tdx_grid* g, int kind, int dir, int mode, int P, double al
     }
     uint64_t h = 0;
     if (kind == KIND_HELM) h = fnv1a(lambda_host, (size_t)nsets * 8);
-    if (kind == KIND_USER) { h = fnv1a(ua, (size_t)n * 8); h = fnv1a(ub, (size_t)n * 8, h); h = fnv1a(uc, (size_t)n * 8, h); }
+    if (kind == KIND_USER || kind == KIND_USERNP) { h = fnv1a(ua, (size_t)n * 8); h = fnv1a(ub, (size_t)n * 8, h); h = fnv1a(uc, (size_t)n * 8, h); }
     std::lock_guard<std::mutex> lk(g->mu);
     for (Plan& p : g->plans)
         if (p.kind == kind && p.dir == dir && p.loc == loc && p.mode == mode && p.P == P && p.nsets == nsets && p.hash == h &&
@@ -699,6 +700,28 @@ tdx_status_t run_dct_x(tdx_grid* g, double* field, bool inverse, cudaStream_t st
 }  // namespace
 
 
+
+// ---- multi-GPU slab decomposition (tdx_slab.cuh) ---------------------------------------------------
+struct tdx_slab {
+    tdx_grid* g = nullptr;             // the slab's own grid (not owned)
+    int dir = 1, rank = 0, R = 1, n_loc = 0, across = TDX_MODE_PPT, local_mode = TDX_MODE_PPT, P_local = 1;
+    long long inner = 0, outer = 0;
+    std::vector<double> a, b, c;       // the slab's cut operator (host): user coefficients of the local plan
+    double *v = nullptr, *w = nullptr, *coef = nullptr;   // device: spikes of this rank, interface coefficients
+    double dropped = 0.0;              // max |v_last|, |w_first| over interior ranks: what PDD across ranks deletes
+};
+
+namespace {
+
+tdx_status_t slab_check(tdx_slab* s, const void* p1, const void* p2) {
+    if (!s) return fail(TDX_ERR_INVALID_ARG, "slab is NULL");
+    if (!p1 || !p2) return fail(TDX_ERR_INVALID_ARG, "data pointer is NULL");
+    if ((reinterpret_cast<uintptr_t>(p1) | reinterpret_cast<uintptr_t>(p2)) & 15) return fail(TDX_ERR_INVALID_ARG, "buffers must be 16-byte aligned");
+    return TDX_OK;
+}
+
+}  // namespace
+
 extern "C" {
 
 const char* tdx_version(void) { return "tdx 0.1 (sm_100a)"; }
@@ -991,6 +1014,137 @@ tdx_status_t tdx_poisson_solve(tdx_grid_t* g, tdx_mode_t mode, int P, const doub
     rc = tdx_helmholtz_wavenumber_solve(g, mode, P, nm, kx2, kz2, spec_work, stream);   if (rc != TDX_OK) return rc;
     rc = run_fft_z(g, spec_work, field, true, st);                             if (rc != TDX_OK) return rc;
     return run_dct_x(g, field, true, st);
+}
+
+tdx_status_t tdx_slab_create(tdx_grid_t* g, tdx_dir_t dir, int rank, int nranks, int n_global, const double* faces_global,
+                             tdx_bc_t bc_global, double alpha, tdx_mode_t across, tdx_mode_t local_mode, int P_local,
+                             tdx_slab_t** out) {
+    if (!out) return fail(TDX_ERR_INVALID_ARG, "out is NULL");
+    *out = nullptr;
+    if (!g || !faces_global) return fail(TDX_ERR_INVALID_ARG, "NULL argument");
+    if (dir != TDX_DIR_Y && dir != TDX_DIR_Z) return fail(TDX_ERR_UNSUPPORTED, "slabs are cut along y (the paper's choice, L74) or z; dir=%d", (int)dir);
+    if (nranks < 1 || nranks > 512 || rank < 0 || rank >= nranks) return fail(TDX_ERR_INVALID_ARG, "rank %d of %d", rank, nranks);
+    if (across != TDX_MODE_PDD && across != TDX_MODE_PPT) return fail(TDX_ERR_INVALID_ARG, "across-rank mode must be PDD or PPT");
+    if (local_mode < 0 || local_mode > 2) return fail(TDX_ERR_INVALID_ARG, "local mode=%d", (int)local_mode);
+    if (bc_global != TDX_BC_DIRICHLET && bc_global != TDX_BC_NEUMANN) return fail(TDX_ERR_UNSUPPORTED, "the slab direction must not be periodic");
+    if (!(alpha == alpha)) return fail(TDX_ERR_INVALID_ARG, "alpha is NaN");
+    if (n_global / nranks < 2) return fail(TDX_ERR_BAD_PARTITION, "%d rows over %d ranks: every slab needs >= 2 rows", n_global, nranks);
+    for (int j = 0; j < n_global; ++j) if (!(faces_global[j + 1] > faces_global[j])) return fail(TDX_ERR_INVALID_ARG, "global faces not strictly increasing at %d", j);
+    const int q = n_global / nranks, rem = n_global % nranks;
+    std::vector<int> starts(nranks + 1);
+    for (int p = 0; p <= nranks; ++p) starts[p] = tdx::part_start(p, q, rem);      // the partition map of tdx_partition_bounds
+    const int n_loc = starts[rank + 1] - starts[rank];
+    if (g->n_of(dir) != n_loc) return fail(TDX_ERR_INVALID_ARG, "slab grid has %d rows in direction %d, rank %d of %d owns %d of %d", g->n_of(dir), (int)dir, rank, nranks, n_loc, n_global);
+    const long long inner = dir == TDX_DIR_Y ? g->nx : (long long)g->nx * g->ny, outer = dir == TDX_DIR_Y ? g->nz : 1;
+    if (inner % 2) return fail(TDX_ERR_UNSUPPORTED, "nx must be even");
+    CUDA_TRY(cudaSetDevice(g->device));
+    // global operator rows with the library's own coefficient kernels, then the cut slab operator and the spikes
+    const int tb = 128, nmax = q + (rem ? 1 : 0);
+    DevBuf f, lo, up, a, b, c, dst, scratch, ends;
+    CUDA_TRY(f.alloc((size_t)(n_global + 1) * 8)); CUDA_TRY(lo.alloc((size_t)n_global * 8)); CUDA_TRY(up.alloc((size_t)n_global * 8));
+    CUDA_TRY(a.alloc((size_t)n_global * 8)); CUDA_TRY(b.alloc((size_t)n_global * 8)); CUDA_TRY(c.alloc((size_t)n_global * 8));
+    CUDA_TRY(dst.alloc((size_t)(nranks + 1) * 4)); CUDA_TRY(scratch.alloc((size_t)nranks * 3 * nmax * 8)); CUDA_TRY(ends.alloc((size_t)nranks * 4 * 8));
+    CUDA_TRY(cudaMemcpy(f.p, faces_global, (size_t)(n_global + 1) * 8, cudaMemcpyHostToDevice));
+    CUDA_TRY(cudaMemcpy(dst.p, starts.data(), (size_t)(nranks + 1) * 4, cudaMemcpyHostToDevice));
+    tdx::k_metrics<<<(n_global + tb - 1) / tb, tb>>>(n_global, f.as<double>(), (int)bc_global, lo.as<double>(), up.as<double>());
+    LAUNCH_CHECK("k_metrics");
+    tdx::k_coeffs_adi<<<(n_global + tb - 1) / tb, tb>>>(n_global, lo.as<double>(), up.as<double>(), (int)bc_global, 0, alpha, a.as<double>(), b.as<double>(), c.as<double>());
+    LAUNCH_CHECK("k_coeffs_adi");
+    tdx_slab* s = new (std::nothrow) tdx_slab();
+    if (!s) return fail(TDX_ERR_ALLOC, "host allocation failed");
+    auto bail = [&](tdx_status_t st) { tdx_slab_destroy(s); return st; };
+    s->g = g; s->dir = dir; s->rank = rank; s->R = nranks; s->n_loc = n_loc; s->across = across; s->local_mode = local_mode; s->P_local = P_local;
+    s->inner = inner; s->outer = outer;
+    const int K = 2 * (nranks - 1);
+    if (cudaMalloc(&s->v, (size_t)n_loc * 8) != cudaSuccess || cudaMalloc(&s->w, (size_t)n_loc * 8) != cudaSuccess ||
+        cudaMalloc(&s->coef, (size_t)std::max(4, 2 * K) * 8) != cudaSuccess) { cudaGetLastError(); return bail(fail(TDX_ERR_ALLOC, "device allocation failed")); }
+    tdx::k_slab_spikes<<<(nranks + 31) / 32, 32>>>(nranks, dst.as<int>(), a.as<double>(), b.as<double>(), c.as<double>(), rank, nmax,
+                                                    scratch.as<double>(), ends.as<double>(), s->v, s->w);
+    g_launches.fetch_add(1);
+    std::vector<double> he((size_t)nranks * 4), ha(n_global), hb(n_global), hc(n_global);
+    if (cudaMemcpy(he.data(), ends.p, he.size() * 8, cudaMemcpyDeviceToHost) != cudaSuccess || cudaMemcpy(ha.data(), a.p, (size_t)n_global * 8, cudaMemcpyDeviceToHost) != cudaSuccess ||
+        cudaMemcpy(hb.data(), b.p, (size_t)n_global * 8, cudaMemcpyDeviceToHost) != cudaSuccess || cudaMemcpy(hc.data(), c.p, (size_t)n_global * 8, cudaMemcpyDeviceToHost) != cudaSuccess)
+        return bail(fail(TDX_ERR_CUDA, "slab plan kernels failed: %s", cudaGetErrorString(cudaGetLastError())));
+    s->a.assign(ha.begin() + starts[rank], ha.begin() + starts[rank + 1]);
+    s->b.assign(hb.begin() + starts[rank], hb.begin() + starts[rank + 1]);
+    s->c.assign(hc.begin() + starts[rank], hc.begin() + starts[rank + 1]);
+    s->a.front() = 0.0; s->c.back() = 0.0;                                        // Alg.1 step 2: couplings across the slab ends are cut
+    for (int i = 1; i <= nranks - 1; ++i) {
+        if (i >= 2) s->dropped = std::max(s->dropped, std::fabs(he[(size_t)(i - 1) * 4 + 1]));
+        if (i <= nranks - 2) s->dropped = std::max(s->dropped, std::fabs(he[(size_t)i * 4 + 2]));
+    }
+    std::vector<double> hcoef(std::max(4, 2 * K), 0.0);
+    if (across == TDX_MODE_PDD || nranks == 1) {
+        if (rank >= 1) { hcoef[0] = he[(size_t)(rank - 1) * 4 + 3]; hcoef[1] = he[(size_t)rank * 4 + 0]; }               // w_last^(r-1), v_first^(r)
+        if (rank <= nranks - 2) { hcoef[2] = he[(size_t)rank * 4 + 3]; hcoef[3] = he[(size_t)(rank + 1) * 4 + 0]; }     // w_last^(r), v_first^(r+1)
+    } else {
+        DevBuf Z, Zi, piv;                                                           // rank-level reduced system: the plan kernels of the intra-GPU PPT
+        CUDA_TRY(Z.alloc((size_t)K * K * 8)); CUDA_TRY(Zi.alloc((size_t)K * K * 8)); CUDA_TRY(piv.alloc((size_t)K * 4));
+        tdx::k_reduced_factor<<<1, 32>>>(1, nranks, ends.as<double>(), Z.as<double>(), piv.as<int>());
+        g_launches.fetch_add(1);
+        tdx::k_reduced_inverse<<<(K + 63) / 64, 64>>>(1, nranks, Z.as<double>(), piv.as<int>(), Zi.as<double>());
+        g_launches.fetch_add(1);
+        std::vector<double> hz((size_t)K * K);
+        if (cudaMemcpy(hz.data(), Zi.p, hz.size() * 8, cudaMemcpyDeviceToHost) != cudaSuccess) return bail(fail(TDX_ERR_CUDA, "reduced system kernels failed"));
+        if (rank >= 1) for (int k = 0; k < K; ++k) hcoef[k] = hz[(size_t)(2 * rank - 2) * K + k];                        // yL = x_last of rank-1 = u_{2r-2}
+        if (rank <= nranks - 2) for (int k = 0; k < K; ++k) hcoef[K + k] = hz[(size_t)(2 * rank + 1) * K + k];          // yR = x_first of rank+1 = u_{2r+1}
+    }
+    if (cudaMemcpy(s->coef, hcoef.data(), hcoef.size() * 8, cudaMemcpyHostToDevice) != cudaSuccess) return bail(fail(TDX_ERR_CUDA, "coefficient upload failed"));
+    // build the local plan now so that argument errors (P_local) surface here
+    Plan* pl = nullptr;
+    tdx_status_t rc = get_plan(g, KIND_USERNP, dir, local_mode, P_local, 0.0, 1, nullptr, s->a.data(), s->b.data(), s->c.data(), 0, &pl);
+    if (rc != TDX_OK) return bail(rc);
+    *out = s;
+    return TDX_OK;
+}
+
+tdx_status_t tdx_slab_destroy(tdx_slab_t* s) {
+    if (!s) return TDX_OK;
+    cudaFree(s->v); cudaFree(s->w); cudaFree(s->coef);
+    delete s;
+    return TDX_OK;
+}
+
+tdx_status_t tdx_slab_eliminate(tdx_slab_t* s, double* field, double* iface_out, void* stream) {
+    tdx_status_t rc = slab_check(s, field, iface_out);
+    if (rc != TDX_OK) return rc;
+    tdx_grid* g = s->g;
+    trim_plans(g);
+    CUDA_TRY(cudaSetDevice(g->device));
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    Plan* pl = nullptr;
+    rc = get_plan(g, KIND_USERNP, s->dir, s->local_mode, s->P_local, 0.0, 1, nullptr, s->a.data(), s->b.data(), s->c.data(), st, &pl);
+    if (rc != TDX_OK) return rc;
+    rc = run_sweep(g, *pl, s->dir, field, st);
+    if (rc != TDX_OK) return rc;
+    const long long tot = 2 * s->inner * s->outer;
+    tdx::k_slab_pack<<<(unsigned)((tot + 255) / 256), 256, 0, st>>>(field, iface_out, s->n_loc, s->inner, s->outer);
+    LAUNCH_CHECK("k_slab_pack");
+    return TDX_OK;
+}
+
+tdx_status_t tdx_slab_correct(tdx_slab_t* s, double* field, const double* iface_own, const double* iface_nbr, void* stream) {
+    tdx_status_t rc = slab_check(s, field, iface_own);
+    if (rc != TDX_OK) return rc;
+    if (s->R == 1) return TDX_OK;                                                   // one rank: xt is the solution
+    if (!iface_nbr || (reinterpret_cast<uintptr_t>(iface_nbr) & 15)) return fail(TDX_ERR_INVALID_ARG, "iface_nbr is NULL or not 16-byte aligned");
+    CUDA_TRY(cudaSetDevice(s->g->device));
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const int JT = std::max(8, (s->n_loc + 7) / 8);
+    dim3 block(128), grid((unsigned)((s->inner / 2 + 127) / 128), (s->n_loc + JT - 1) / JT, (unsigned)s->outer);
+    if (s->outer > 65535) return fail(TDX_ERR_UNSUPPORTED, "outer extent > 65535");
+    if (s->across == TDX_MODE_PPT)
+        tdx::k_slab_correct<true><<<grid, block, 0, st>>>(field, iface_own, iface_nbr, s->coef, s->v, s->w, s->rank, s->R, s->n_loc, s->inner, s->outer, JT);
+    else
+        tdx::k_slab_correct<false><<<grid, block, 0, st>>>(field, iface_own, iface_nbr, s->coef, s->v, s->w, s->rank, s->R, s->n_loc, s->inner, s->outer, JT);
+    LAUNCH_CHECK("k_slab_correct");
+    return TDX_OK;
+}
+
+tdx_status_t tdx_slab_dropped_bound(tdx_slab_t* s, double* out) {
+    if (!s || !out) return fail(TDX_ERR_INVALID_ARG, "NULL argument");
+    *out = s->dropped;
+    return TDX_OK;
 }
 
 tdx_status_t tdx_pdd_dropped_bound(tdx_grid_t* g, tdx_dir_t dir, int P, double alpha, double* out) {
