@@ -398,6 +398,53 @@ def run_tdx(args, rank, world, local_rank):
                                 "what": "tdx_poisson_solve: dct_x, rfft_z, per-line y-solves (PPT), irfft_z, idct_x; 80 B per grid value"}
         del pfield, work
 
+        # the y sweep with the field cut into y-slabs, one per rank (the paper's decomposition, L74): local
+        # elimination (the slab's own sweep kernel) + interface exchange + one correction pass = 32 B per grid value.
+        # world == 1: the compute part of an interior rank of a 4-rank job (a quarter slab; the exchange is a device copy);
+        # world > 1: the real thing over NCCL (strong scaling of ONE field), max over ranks.
+        try:
+            from paper_1812_01178_b200 import parallel
+            Rk = world if world > 1 else 4
+            rk = rank if world > 1 else 1
+            y0, y1 = parallel.slab_bounds(cfg.ny, Rk)[rk]
+            fs = cfg.faces()
+            sg = tdx.Grid(cfg.nx, y1 - y0, cfg.nz, fs[0], fs[1][y0:y1 + 1], fs[2], bcs=bcs, device=local_rank)
+            Ploc = max(p for p in range(1, (y1 - y0) // 2 + 1) if (y1 - y0) % p == 0 and (y1 - y0) // p >= 8) if (y1 - y0) >= 16 else 1
+            slab_out = {"ranks": Rk, "rows_per_rank": y1 - y0, "P_local": Ploc}
+            sfield = field0[:, y0:y1, :].contiguous()
+            for aname, across in (("ppt", tdx.MODE_PPT), ("pdd", tdx.MODE_PDD)):
+                sw = parallel.SlabSweep(sg, 1, rk, Rk, fs[1], bcs[1], cfg.alpha, across, tdx.MODE_PPT if Ploc > 1 else tdx.MODE_THOMAS, Ploc)
+                if world > 1:
+                    run = lambda: sw.sweep(sfield)
+                else:
+                    iface = torch.zeros((2, cfg.nx * cfg.nz), dtype=torch.float64, device=sfield.device)
+                    gathered = torch.zeros((Rk, 2, cfg.nx * cfg.nz), dtype=torch.float64, device=sfield.device)
+                    def run():
+                        sw.slab.eliminate(sfield, iface, stream)
+                        gathered[rk].copy_(iface)                # stands in for the exchange
+                        sw.slab.correct(sfield, iface, gathered if across == tdx.MODE_PPT else gathered[rk], stream)
+                for _ in range(3):
+                    run()
+                barrier()
+                s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                s0.record()
+                for _ in range(args.steps):
+                    run()
+                s1.record()
+                barrier()
+                mss = max_over_ranks(s0.elapsed_time(s1) / args.steps, dist, "cuda")
+                npt = cfg.npts if world > 1 else sfield.numel()
+                slab_out[aname] = {"ms": mss, "gpts_per_s": npt / (mss * 1e-3) / 1e9, "gb_per_s": 2 * BYTES_PER_POINT * npt / (mss * 1e-3) / 1e9 / (world if world > 1 else 1),
+                                   "dropped_bound": sw.slab.dropped_bound()}
+                sw.close()
+            slab_out["what"] = ("y sweep of the whole field over %d ranks (NCCL exchange), whole-job Gpts/s, per-GPU GB/s at 32 B/value" % world) if world > 1 else \
+                               "compute part of one interior rank of a 4-rank y-slab sweep (eliminate + correct, exchange replaced by a device copy)"
+            out["slab_y_sweep"] = slab_out
+            sg.close()
+            del sfield
+        except Exception as exc:                                 # an extra figure must never take the headline down
+            out["slab_y_sweep"] = {"error": repr(exc)[:300]}
+
     # end to end through the host-buffer C-ABI calls: pinned host buffers, H2D + solve + D2H inside the timed region
     if not args.no_e2e:
         hf = torch.from_numpy(host_field).pin_memory().numpy()
