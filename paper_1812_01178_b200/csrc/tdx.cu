@@ -610,21 +610,21 @@ tdx_status_t fft_tables(tdx_grid* g, int dir, cudaStream_t st) {
 }
 
 // WAVES: L2 prefetch distance in waves of resident CTAs (0 = off), measured per instantiation (profiles/r1_fft_tuning.md)
-template <int N, int C, int WAVES>
+template <int N, int C, int WAVES, int K = 8>
 tdx_status_t launch_fft_z(tdx_grid* g, const double* in, double* out, bool inverse, cudaStream_t st) {
     const size_t smem = (size_t)N * C * 16;
-    dim3 block(C, N / 8), grid((g->nx + 2 * C - 1) / (2 * C), g->ny);
-    const int resident = std::max(1, std::min((int)(220 * 1024 / smem), 2048 / (C * N / 8)));
+    dim3 block(C, N / K), grid((g->nx + 2 * C - 1) / (2 * C), g->ny);
+    const int resident = std::max(1, std::min((int)(220 * 1024 / smem), 2048 / (C * N / K)));
     const int pf = g->sms * resident * std::min(WAVES, prefetch_waves());
     if (!inverse) {
         static bool done = false;
-        if (!done) { CUDA_TRY(cudaFuncSetAttribute(k_rfft_z<N, C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); done = true; }
-        k_rfft_z<N, C><<<grid, block, smem, st>>>(in, reinterpret_cast<double2*>(out), g->nx, g->ny, g->fft_tw[2], pf);
+        if (!done) { CUDA_TRY(cudaFuncSetAttribute(k_rfft_z<N, C, K>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); done = true; }
+        k_rfft_z<N, C, K><<<grid, block, smem, st>>>(in, reinterpret_cast<double2*>(out), g->nx, g->ny, g->fft_tw[2], pf);
         LAUNCH_CHECK("k_rfft_z");
     } else {
         static bool done = false;
-        if (!done) { CUDA_TRY(cudaFuncSetAttribute(k_irfft_z<N, C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); done = true; }
-        k_irfft_z<N, C><<<grid, block, smem, st>>>(reinterpret_cast<const double2*>(in), out, g->nx, g->ny, g->fft_tw[2], pf);
+        if (!done) { CUDA_TRY(cudaFuncSetAttribute(k_irfft_z<N, C, K>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); done = true; }
+        k_irfft_z<N, C, K><<<grid, block, smem, st>>>(reinterpret_cast<const double2*>(in), out, g->nx, g->ny, g->fft_tw[2], pf);
         LAUNCH_CHECK("k_irfft_z");
     }
     return TDX_OK;
@@ -648,28 +648,28 @@ tdx_status_t run_fft_z(tdx_grid* g, const double* in, double* out, bool inverse,
         case 32:   return launch_fft_z<32, 16, 1>(g, in, out, inverse, st);
         case 64:   return launch_fft_z<64, 16, 1>(g, in, out, inverse, st);
         case 128:  return launch_fft_z<128, 16, 1>(g, in, out, inverse, st);
-        case 256:  return launch_fft_z<256, 8, 0>(g, in, out, inverse, st);
-        case 512:  return inverse ? launch_fft_z<512, 16, 1>(g, in, out, inverse, st) : launch_fft_z<512, 8, 0>(g, in, out, inverse, st);
+        case 256:  return inverse ? launch_fft_z<256, 8, 0, 16>(g, in, out, inverse, st) : launch_fft_z<256, 16, 1, 16>(g, in, out, inverse, st);
+        case 512:  return inverse ? launch_fft_z<512, 8, 1, 16>(g, in, out, inverse, st) : launch_fft_z<512, 8, 0, 8>(g, in, out, inverse, st);
         default:   return launch_fft_z<1024, 8, 1>(g, in, out, inverse, st);
     }
 }
 
-template <int N, int LP>
+template <int N, int LP, int K = 8>
 tdx_status_t launch_dct_x(tdx_grid* g, double* field, bool inverse, cudaStream_t st) {
     const long long lines = (long long)g->ny * g->nz;
-    const size_t smem = (size_t)LP * (N + N / 8) * 16 + 16;
+    const size_t smem = (size_t)LP * (N + N / K) * 16 + 16;
     const long long ctas = (lines + 2 * LP - 1) / (2 * LP);
     if (ctas > 2147483647LL) return fail(TDX_ERR_UNSUPPORTED, "too many lines");
-    const int resident = std::max(1, std::min((int)(220 * 1024 / smem), 2048 / (LP * N / 8)));
+    const int resident = std::max(1, std::min((int)(220 * 1024 / smem), 2048 / (LP * N / K)));
     const int pf = g->sms * resident * prefetch_waves();
     if (!inverse) {
         static bool done = false;
-        if (!done) { CUDA_TRY(cudaFuncSetAttribute(k_dct_x<N, LP, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); done = true; }
-        k_dct_x<N, LP, 0><<<(unsigned)ctas, LP * N / 8, smem, st>>>(field, lines, g->fft_tw[0], g->fft_w4, pf);
+        if (!done) { CUDA_TRY(cudaFuncSetAttribute(k_dct_x<N, LP, 0, K>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); done = true; }
+        k_dct_x<N, LP, 0, K><<<(unsigned)ctas, LP * N / K, smem, st>>>(field, lines, g->fft_tw[0], g->fft_w4, pf);
     } else {
         static bool done = false;
-        if (!done) { CUDA_TRY(cudaFuncSetAttribute(k_dct_x<N, LP, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); done = true; }
-        k_dct_x<N, LP, 1><<<(unsigned)ctas, LP * N / 8, smem, st>>>(field, lines, g->fft_tw[0], g->fft_w4, pf);
+        if (!done) { CUDA_TRY(cudaFuncSetAttribute(k_dct_x<N, LP, 1, K>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); done = true; }
+        k_dct_x<N, LP, 1, K><<<(unsigned)ctas, LP * N / K, smem, st>>>(field, lines, g->fft_tw[0], g->fft_w4, pf);
     }
     LAUNCH_CHECK("k_dct_x");
     return TDX_OK;
@@ -690,10 +690,10 @@ tdx_status_t run_dct_x(tdx_grid* g, double* field, bool inverse, cudaStream_t st
         case 64:   return launch_dct_x<64, 32>(g, field, inverse, st);
         case 128:  return launch_dct_x<128, 16>(g, field, inverse, st);
         case 256:  return launch_dct_x<256, 8>(g, field, inverse, st);
-        case 512:  return launch_dct_x<512, 4>(g, field, inverse, st);
-        case 1024: return launch_dct_x<1024, 2>(g, field, inverse, st);
-        case 2048: return launch_dct_x<2048, 1>(g, field, inverse, st);
-        default:   return launch_dct_x<4096, 1>(g, field, inverse, st);
+        case 512:  return launch_dct_x<512, 4, 16>(g, field, inverse, st);       // 16 points per thread from here on: one exchange less
+        case 1024: return launch_dct_x<1024, 2, 16>(g, field, inverse, st);
+        case 2048: return launch_dct_x<2048, 1, 16>(g, field, inverse, st);
+        default:   return launch_dct_x<4096, 1, 16>(g, field, inverse, st);
     }
 }
 

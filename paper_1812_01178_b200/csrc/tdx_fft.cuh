@@ -54,56 +54,89 @@ __device__ __forceinline__ void dft8(double2 (&v)[8]) {
     v[1] = b4; v[3] = b5; v[5] = b6; v[7] = b7;
 }
 
-// One Stockham pass of radix R on the 8 register points of thread t (slot kk = point t + kk*N/8).  NS = product of
-// the radices of the earlier passes.  Butterfly s (of B = 8/R) takes slots s + r*B, r < R; its index is j = t + s*N/8.
+// 16-point DFT as 4 x 4 (Cooley-Tukey): inner DFT4 over n1 of x[4 n1 + q], twiddle W16^(q k1), outer DFT4 over q.
+__device__ __forceinline__ void dft16(double2 (&v)[16]) {
+    const double h = 0.70710678118654752440, c1 = 0.92387953251128675613, s1 = 0.38268343236508977173;
+#pragma unroll
+    for (int q = 0; q < 4; ++q) dft4(v[q], v[q + 4], v[q + 8], v[q + 12]);          // v[q + 4 k1] = inner output k1 of column q
+    // twiddles W16^(q k1), q, k1 in 1..3
+    v[1 + 4] = cmul(v[1 + 4], make_double2(c1, -s1));                                // W^1
+    v[1 + 8] = make_double2((v[1 + 8].x + v[1 + 8].y) * h, (v[1 + 8].y - v[1 + 8].x) * h);   // W^2
+    v[1 + 12] = cmul(v[1 + 12], make_double2(s1, -c1));                              // W^3
+    v[2 + 4] = make_double2((v[2 + 4].x + v[2 + 4].y) * h, (v[2 + 4].y - v[2 + 4].x) * h);   // W^2
+    v[2 + 8] = cmul_mi(v[2 + 8]);                                                    // W^4 = -i
+    v[2 + 12] = make_double2((v[2 + 12].y - v[2 + 12].x) * h, -(v[2 + 12].x + v[2 + 12].y) * h);   // W^6
+    v[3 + 4] = cmul(v[3 + 4], make_double2(s1, -c1));                                // W^3
+    v[3 + 8] = make_double2((v[3 + 8].y - v[3 + 8].x) * h, -(v[3 + 8].x + v[3 + 8].y) * h);   // W^6
+    v[3 + 12] = cmul(v[3 + 12], make_double2(-c1, s1));                              // W^9
+#pragma unroll
+    for (int k1 = 0; k1 < 4; ++k1) dft4(v[4 * k1], v[4 * k1 + 1], v[4 * k1 + 2], v[4 * k1 + 3]);   // slot 4 k1 + k2 = X[k1 + 4 k2]
+    // to natural order: X[k] sits in slot 4 (k & 3) + (k >> 2)
+    double2 o[16];
+#pragma unroll
+    for (int k = 0; k < 16; ++k) o[k] = v[4 * (k & 3) + (k >> 2)];
+#pragma unroll
+    for (int k = 0; k < 16; ++k) v[k] = o[k];
+}
+
+// One Stockham pass of radix R on the K register points of thread t (slot kk = point t + kk*N/K).  NS = product of
+// the radices of the earlier passes.  Butterfly s (of B = K/R) takes slots s + r*B, r < R; its index is j = t + s*N/K.
 // pos[kk] receives the position the slot's value has after the pass: (j - j%NS)*R + j%NS + r*NS.
-template <int N, int R, int NS>
-__device__ __forceinline__ void fft_pass(double2 (&v)[8], int (&pos)[8], int t, const double2* __restrict__ tw) {
-    constexpr int T = N / 8, B = 8 / R;
+template <int N, int K, int R, int NS>
+__device__ __forceinline__ void fft_pass(double2 (&v)[K], int (&pos)[K], int t, const double2* __restrict__ tw) {
+    constexpr int T = N / K, B = K / R;
 #pragma unroll
     for (int s = 0; s < B; ++s) {
         const int j = t + s * T;
         const int jm = j & (NS - 1);
+        double2 x[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) x[r] = v[s + r * B];
         if (NS > 1) {
             const double2 w1 = __ldg(tw + jm * (N / (NS * R)));
-            if (R == 2) {
-                v[s + B] = cmul(v[s + B], w1);
-            } else if (R == 4) {
+            x[1] = cmul(x[1], w1);
+            if constexpr (R >= 4) {
                 const double2 w2 = cmul(w1, w1), w3 = cmul(w2, w1);
-                v[s + B] = cmul(v[s + B], w1); v[s + 2 * B] = cmul(v[s + 2 * B], w2); v[s + 3 * B] = cmul(v[s + 3 * B], w3);
-            } else {
-                const double2 w2 = cmul(w1, w1), w3 = cmul(w2, w1), w4 = cmul(w2, w2);
-                const double2 w5 = cmul(w4, w1), w6 = cmul(w3, w3), w7 = cmul(w4, w3);
-                v[1] = cmul(v[1], w1); v[2] = cmul(v[2], w2); v[3] = cmul(v[3], w3); v[4] = cmul(v[4], w4);
-                v[5] = cmul(v[5], w5); v[6] = cmul(v[6], w6); v[7] = cmul(v[7], w7);
+                x[2] = cmul(x[2], w2); x[3] = cmul(x[3], w3);
+                if constexpr (R >= 8) {
+                    const double2 w4 = cmul(w2, w2), w5 = cmul(w4, w1), w6 = cmul(w4, w2), w7 = cmul(w4, w3);
+                    x[4] = cmul(x[4], w4); x[5] = cmul(x[5], w5); x[6] = cmul(x[6], w6); x[7] = cmul(x[7], w7);
+                    if constexpr (R >= 16) {
+                        const double2 w8 = cmul(w4, w4);
+                        x[8] = cmul(x[8], w8); x[9] = cmul(x[9], cmul(w8, w1)); x[10] = cmul(x[10], cmul(w8, w2));
+                        x[11] = cmul(x[11], cmul(w8, w3)); x[12] = cmul(x[12], cmul(w8, w4)); x[13] = cmul(x[13], cmul(w8, w5));
+                        x[14] = cmul(x[14], cmul(w8, w6)); x[15] = cmul(x[15], cmul(w8, w7));
+                    }
+                }
             }
         }
-        if (R == 2) dft2(v[s], v[s + B]);
-        else if (R == 4) dft4(v[s], v[s + B], v[s + 2 * B], v[s + 3 * B]);
-        else dft8(v);
+        if constexpr (R == 2) dft2(x[0], x[1]);
+        else if constexpr (R == 4) dft4(x[0], x[1], x[2], x[3]);
+        else if constexpr (R == 8) dft8(x);
+        else dft16(x);
         const int base = (j - jm) * R + jm;
 #pragma unroll
-        for (int r = 0; r < R; ++r) pos[s + r * B] = base + r * NS;
+        for (int r = 0; r < R; ++r) { v[s + r * B] = x[r]; pos[s + r * B] = base + r * NS; }
     }
 }
 
-// Whole transform: passes of radix 8 while they fit, then the remaining 4 or 2.  SM maps a position to a shared-memory
-// slot (SM::at(pos)).  On return v[kk] = X[t + kk*N/8] (the last pass leaves its outputs in the slots they came from).
+// Whole transform: passes of radix K while they fit, then the remaining factor.  SM maps a position to a shared-memory
+// slot (SM::at(pos)).  On return v[kk] = X[t + kk*N/K] (the last pass leaves its outputs in the slots they came from).
 // Every pass but the last ends with: scatter to shared, barrier, gather, barrier.
-template <int N, int NS, class SM>
-__device__ __forceinline__ void fft_regs(double2 (&v)[8], int t, const double2* __restrict__ tw, const SM& sm) {
-    constexpr int T = N / 8;
-    constexpr int R = (N / NS >= 8) ? 8 : (N / NS);
-    int pos[8];
-    fft_pass<N, R, NS>(v, pos, t, tw);
+template <int N, int K, int NS, class SM>
+__device__ __forceinline__ void fft_regs(double2 (&v)[K], int t, const double2* __restrict__ tw, const SM& sm) {
+    constexpr int T = N / K;
+    constexpr int R = (N / NS >= K) ? K : (N / NS);
+    int pos[K];
+    fft_pass<N, K, R, NS>(v, pos, t, tw);
     if constexpr (NS * R < N) {
 #pragma unroll
-        for (int kk = 0; kk < 8; ++kk) *sm.at(pos[kk]) = v[kk];
+        for (int kk = 0; kk < K; ++kk) *sm.at(pos[kk]) = v[kk];
         __syncthreads();
 #pragma unroll
-        for (int kk = 0; kk < 8; ++kk) v[kk] = *sm.at(t + kk * T);
+        for (int kk = 0; kk < K; ++kk) v[kk] = *sm.at(t + kk * T);
         __syncthreads();
-        fft_regs<N, NS * R, SM>(v, t, tw, sm);
+        fft_regs<N, K, NS * R, SM>(v, t, tw, sm);
     }
 }
 
@@ -112,9 +145,10 @@ struct SmCols {      // z transforms: [pos][C columns], column fastest
     double2* base; int C;
     __device__ __forceinline__ double2* at(int pos) const { return base + pos * C; }
 };
-struct SmPad {       // x transforms: one line pair, one pad slot per 8 (the first pass writes with stride 8)
+template <int K>
+struct SmPad {       // x transforms: one line pair, one pad slot per K (the first pass writes with stride K)
     double2* base;
-    __device__ __forceinline__ double2* at(int pos) const { return base + pos + (pos >> 3); }
+    __device__ __forceinline__ double2* at(int pos) const { return base + pos + (pos >> (K == 16 ? 4 : 3)); }
 };
 
 // ---- plan-time tables ---------------------------------------------------------------------------------------------
@@ -127,10 +161,10 @@ __global__ void k_fft_tables(double2* __restrict__ tw, double2* __restrict__ w4,
 
 // ---- Fourier transform along z --------------------------------------------------------------------------------------
 // in: real [nz=N][ny][nx]; out: complex128 [N/2+1][ny][nx].  grid (ceil(nx / 2C), ny), block (C, N/8).  nx even.
-template <int N, int C>
-__global__ void __launch_bounds__(C * N / 8) k_rfft_z(const double* __restrict__ in, double2* __restrict__ out, int nx, int ny,
+template <int N, int C, int K>
+__global__ void __launch_bounds__(C * N / K) k_rfft_z(const double* __restrict__ in, double2* __restrict__ out, int nx, int ny,
                                                        const double2* __restrict__ tw, int pf) {
-    constexpr int T = N / 8;
+    constexpr int T = N / K, H = K / 2;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     double2* smb = reinterpret_cast<double2*>(smem_raw);
     const int c = threadIdx.x, t = threadIdx.y;
@@ -139,9 +173,9 @@ __global__ void __launch_bounds__(C * N / 8) k_rfft_z(const double* __restrict__
     const bool act = i0 < nx;
     const size_t plane = (size_t)nx * ny;
     const double* src = in + (size_t)j * nx + i0;
-    double2 v[8];
+    double2 v[K];
 #pragma unroll
-    for (int kk = 0; kk < 8; ++kk)
+    for (int kk = 0; kk < K; ++kk)
         v[kk] = act ? __ldcs(reinterpret_cast<const double2*>(src + (size_t)(t + kk * T) * plane)) : make_double2(0.0, 0.0);
     if (pf > 0 && (c & 7) == 0) {                  // L2 prefetch of the tile the CTA `pf` launches ahead will load (one lane per 128 B)
         const long long lin = (long long)blockIdx.y * gridDim.x + blockIdx.x + pf;
@@ -150,17 +184,17 @@ __global__ void __launch_bounds__(C * N / 8) k_rfft_z(const double* __restrict__
         if (by < ny && pi < nx) {
             const double* pb = in + (size_t)by * nx + pi;
 #pragma unroll
-            for (int kk = 0; kk < 8; ++kk) asm volatile("prefetch.global.L2 [%0];" ::"l"(pb + (size_t)(t + kk * T) * plane));
+            for (int kk = 0; kk < K; ++kk) asm volatile("prefetch.global.L2 [%0];" ::"l"(pb + (size_t)(t + kk * T) * plane));
         }
     }
     const SmCols sm{smb + c, C};
-    fft_regs<N, 1, SmCols>(v, t, tw, sm);
+    fft_regs<N, K, 1, SmCols>(v, t, tw, sm);
 #pragma unroll
-    for (int kk = 0; kk < 8; ++kk) *sm.at(t + kk * T) = v[kk];
+    for (int kk = 0; kk < K; ++kk) *sm.at(t + kk * T) = v[kk];
     __syncthreads();
     double2* dst = out + (size_t)j * nx + i0;
 #pragma unroll
-    for (int kk = 0; kk < 4; ++kk) {
+    for (int kk = 0; kk < H; ++kk) {
         const int m = t + kk * T;
         const double2 zm = *sm.at(m), zn = *sm.at((N - m) & (N - 1));
         if (act) {
@@ -178,10 +212,10 @@ __global__ void __launch_bounds__(C * N / 8) k_rfft_z(const double* __restrict__
 }
 
 // in: complex128 [N/2+1][ny][nx]; out: real [N][ny][nx] (includes the 1/N).  Same launch shape as k_rfft_z.
-template <int N, int C>
-__global__ void __launch_bounds__(C * N / 8) k_irfft_z(const double2* __restrict__ in, double* __restrict__ out, int nx, int ny,
+template <int N, int C, int K>
+__global__ void __launch_bounds__(C * N / K) k_irfft_z(const double2* __restrict__ in, double* __restrict__ out, int nx, int ny,
                                                         const double2* __restrict__ tw, int pf) {
-    constexpr int T = N / 8;
+    constexpr int T = N / K, H = K / 2;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     double2* smb = reinterpret_cast<double2*>(smem_raw);
     const int c = threadIdx.x, t = threadIdx.y;
@@ -191,17 +225,17 @@ __global__ void __launch_bounds__(C * N / 8) k_irfft_z(const double2* __restrict
     const size_t plane = (size_t)nx * ny;
     const double2* src = in + (size_t)j * nx + i0;
     const SmCols sm{smb + c, C};
-    double2 a[5], b[5];
+    double2 a[H + 1], b[H + 1];
 #pragma unroll
-    for (int kk = 0; kk < 4; ++kk) {
+    for (int kk = 0; kk < H; ++kk) {
         const double2* p = src + (size_t)(t + kk * T) * plane;
         a[kk] = act ? __ldcs(p) : make_double2(0.0, 0.0);
         b[kk] = act ? __ldcs(p + 1) : make_double2(0.0, 0.0);
     }
     if (t == 0) {
         const double2* p = src + (size_t)(N / 2) * plane;
-        a[4] = act ? __ldcs(p) : make_double2(0.0, 0.0);
-        b[4] = act ? __ldcs(p + 1) : make_double2(0.0, 0.0);
+        a[H] = act ? __ldcs(p) : make_double2(0.0, 0.0);
+        b[H] = act ? __ldcs(p + 1) : make_double2(0.0, 0.0);
     }
     if (pf > 0 && (c & 3) == 0) {                  // spectrum rows are 32 B per column pair: one lane per 128 B
         const long long lin = (long long)blockIdx.y * gridDim.x + blockIdx.x + pf;
@@ -210,13 +244,13 @@ __global__ void __launch_bounds__(C * N / 8) k_irfft_z(const double2* __restrict
         if (by < ny && pi < nx) {
             const double2* pb = in + (size_t)by * nx + pi;
 #pragma unroll
-            for (int kk = 0; kk < 4; ++kk) asm volatile("prefetch.global.L2 [%0];" ::"l"(pb + (size_t)(t + kk * T) * plane));
+            for (int kk = 0; kk < H; ++kk) asm volatile("prefetch.global.L2 [%0];" ::"l"(pb + (size_t)(t + kk * T) * plane));
             if (t == 0) asm volatile("prefetch.global.L2 [%0];" ::"l"(pb + (size_t)(N / 2) * plane));
         }
     }
     // Z_m = A + iB, Z_{N-m} = conj A + i conj B; stored with re/im swapped (inverse transform by the swap identity)
 #pragma unroll
-    for (int kk = 0; kk < 4; ++kk) {
+    for (int kk = 0; kk < H; ++kk) {
         const int m = t + kk * T;
         if (m == 0) {
             *sm.at(0) = make_double2(b[kk].x, a[kk].x);
@@ -225,18 +259,18 @@ __global__ void __launch_bounds__(C * N / 8) k_irfft_z(const double2* __restrict
             *sm.at(N - m) = make_double2(b[kk].x - a[kk].y, a[kk].x + b[kk].y);
         }
     }
-    if (t == 0) *sm.at(N / 2) = make_double2(b[4].x, a[4].x);
+    if (t == 0) *sm.at(N / 2) = make_double2(b[H].x, a[H].x);
     __syncthreads();
-    double2 v[8];
+    double2 v[K];
 #pragma unroll
-    for (int kk = 0; kk < 8; ++kk) v[kk] = *sm.at(t + kk * T);
+    for (int kk = 0; kk < K; ++kk) v[kk] = *sm.at(t + kk * T);
     __syncthreads();
-    fft_regs<N, 1, SmCols>(v, t, tw, sm);
+    fft_regs<N, K, 1, SmCols>(v, t, tw, sm);
     const double sc = 1.0 / (double)N;
     double* dst = out + (size_t)j * nx + i0;
     if (act) {
 #pragma unroll
-        for (int kk = 0; kk < 8; ++kk)
+        for (int kk = 0; kk < K; ++kk)
             __stcs(reinterpret_cast<double2*>(dst + (size_t)(t + kk * T) * plane), make_double2(v[kk].y * sc, v[kk].x * sc));
     }
 }
@@ -256,11 +290,11 @@ __device__ __forceinline__ void bulk_prefetch_1d(const void* src, uint32_t bytes
 
 // field: [lines][N] doubles, in place.  CTA = LP line pairs (2*LP*N contiguous doubles) x N/8 threads per pair.
 // Shared memory: LP * (N + N/8) double2 (the raw lines occupy the first LP*2N doubles of it) + one mbarrier.
-template <int N, int LP, int INV>
-__global__ void __launch_bounds__(LP * N / 8) k_dct_x(double* __restrict__ field, long long lines,
+template <int N, int LP, int INV, int K>
+__global__ void __launch_bounds__(LP * N / K) k_dct_x(double* __restrict__ field, long long lines,
                                                        const double2* __restrict__ tw, const double2* __restrict__ w4, int pf) {
-    constexpr int T = N / 8;
-    constexpr int PSTR = N + N / 8;                           // double2 slots per pair in the exchange layout
+    constexpr int T = N / K, H = K / 2;
+    constexpr int PSTR = N + N / K;                           // double2 slots per pair in the exchange layout
     extern __shared__ __align__(16) unsigned char smem_raw[];
     double2* smb = reinterpret_cast<double2*>(smem_raw);
     double* raw = reinterpret_cast<double*>(smem_raw);
@@ -285,31 +319,31 @@ __global__ void __launch_bounds__(LP * N / 8) k_dct_x(double* __restrict__ field
     const bool has_a = 2 * p < nl, has_b = 2 * p + 1 < nl;
     const double* la = raw + (size_t)p * 2 * N;
     const double* lb = la + N;
-    const SmPad sm{smb + (size_t)p * PSTR};
-    double2 v[8];
+    const SmPad<K> sm{smb + (size_t)p * PSTR};
+    double2 v[K];
     if (!INV) {
 #pragma unroll
-        for (int kk = 0; kk < 8; ++kk) {
+        for (int kk = 0; kk < K; ++kk) {
             const int n = t + kk * T;
             const int idx = (n < N / 2) ? 2 * n : 2 * (N - 1 - n) + 1;
             v[kk] = make_double2(has_a ? la[idx] : 0.0, has_b ? lb[idx] : 0.0);
         }
         __syncthreads();                                                       // raw lines consumed; the buffer becomes the exchange area
-        fft_regs<N, 1, SmPad>(v, t, tw, sm);
+        fft_regs<N, K, 1, SmPad<K>>(v, t, tw, sm);
 #pragma unroll
-        for (int kk = 0; kk < 8; ++kk) *sm.at(t + kk * T) = v[kk];
+        for (int kk = 0; kk < K; ++kk) *sm.at(t + kk * T) = v[kk];
         __syncthreads();
-        double2 zk[5], zn[5];
+        double2 zk[H + 1], zn[H + 1];
 #pragma unroll
-        for (int kk = 0; kk < 4; ++kk) { const int k = t + kk * T; zk[kk] = *sm.at(k); zn[kk] = *sm.at((N - k) & (N - 1)); }
-        if (t == 0) { zk[4] = *sm.at(N / 2); zn[4] = zk[4]; }
+        for (int kk = 0; kk < H; ++kk) { const int k = t + kk * T; zk[kk] = *sm.at(k); zn[kk] = *sm.at((N - k) & (N - 1)); }
+        if (t == 0) { zk[H] = *sm.at(N / 2); zn[H] = zk[H]; }
         __syncthreads();                                                       // spectrum consumed; the buffer becomes the raw lines again
         double* oa = raw + (size_t)p * 2 * N;
         double* ob = oa + N;
 #pragma unroll
-        for (int kk = 0; kk < 5; ++kk) {
-            if (kk == 4 && t != 0) break;
-            const int k = (kk == 4) ? N / 2 : t + kk * T;
+        for (int kk = 0; kk <= H; ++kk) {
+            if (kk == H && t != 0) break;
+            const int k = (kk == H) ? N / 2 : t + kk * T;
             // V_a = (Z_k + conj Z_{N-k})/2, V_b = (Z_k - conj Z_{N-k})/(2i)
             const double2 va = make_double2(0.5 * (zk[kk].x + zn[kk].x), 0.5 * (zk[kk].y - zn[kk].y));
             const double2 vb = make_double2(0.5 * (zk[kk].y + zn[kk].y), 0.5 * (zn[kk].x - zk[kk].x));
@@ -319,11 +353,11 @@ __global__ void __launch_bounds__(LP * N / 8) k_dct_x(double* __restrict__ field
             if (k != 0 && k != N / 2) { oa[N - k] = -ya.y; ob[N - k] = -yb.y; }   // X_{N-k} = -Im(w_k V_k)
         }
     } else {
-        double xa[5], xan[5], xb[5], xbn[5];
+        double xa[H + 1], xan[H + 1], xb[H + 1], xbn[H + 1];
 #pragma unroll
-        for (int kk = 0; kk < 5; ++kk) {
-            if (kk == 4 && t != 0) break;
-            const int k = (kk == 4) ? N / 2 : t + kk * T;
+        for (int kk = 0; kk <= H; ++kk) {
+            if (kk == H && t != 0) break;
+            const int k = (kk == H) ? N / 2 : t + kk * T;
             xa[kk] = has_a ? la[k] : 0.0; xb[kk] = has_b ? lb[k] : 0.0;
             xan[kk] = (k == 0 || !has_a) ? 0.0 : la[N - k];
             xbn[kk] = (k == 0 || !has_b) ? 0.0 : lb[N - k];
@@ -331,9 +365,9 @@ __global__ void __launch_bounds__(LP * N / 8) k_dct_x(double* __restrict__ field
         __syncthreads();
         // V_k = conj(w_k)(X_k - i X_{N-k}); Z_k = Va_k + i Vb_k; Z_{N-k} = conj(Va_k) + i conj(Vb_k); stored swapped
 #pragma unroll
-        for (int kk = 0; kk < 5; ++kk) {
-            if (kk == 4 && t != 0) break;
-            const int k = (kk == 4) ? N / 2 : t + kk * T;
+        for (int kk = 0; kk <= H; ++kk) {
+            if (kk == H && t != 0) break;
+            const int k = (kk == H) ? N / 2 : t + kk * T;
             const double2 w = __ldg(w4 + k);
             const double2 wc = make_double2(w.x, -w.y);
             const double2 va = cmul(wc, make_double2(xa[kk], -xan[kk]));
@@ -343,15 +377,15 @@ __global__ void __launch_bounds__(LP * N / 8) k_dct_x(double* __restrict__ field
         }
         __syncthreads();
 #pragma unroll
-        for (int kk = 0; kk < 8; ++kk) v[kk] = *sm.at(t + kk * T);
+        for (int kk = 0; kk < K; ++kk) v[kk] = *sm.at(t + kk * T);
         __syncthreads();
-        fft_regs<N, 1, SmPad>(v, t, tw, sm);
+        fft_regs<N, K, 1, SmPad<K>>(v, t, tw, sm);
         __syncthreads();                                                       // (fft_regs ends on a gather barrier only if it had > 1 pass)
         const double sc = 1.0 / (double)N;
         double* oa = raw + (size_t)p * 2 * N;
         double* ob = oa + N;
 #pragma unroll
-        for (int kk = 0; kk < 8; ++kk) {
+        for (int kk = 0; kk < K; ++kk) {
             const int n = t + kk * T;
             const int idx = (n < N / 2) ? 2 * n : 2 * (N - 1 - n) + 1;
             oa[idx] = v[kk].y * sc; ob[idx] = v[kk].x * sc;                    // un-swap: re of the inverse is the stored im
