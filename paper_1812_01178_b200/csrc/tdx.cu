@@ -609,7 +609,7 @@ tdx_status_t fft_tables(tdx_grid* g, int dir, cudaStream_t st) {
     return TDX_OK;
 }
 
-// WAVES: L2 prefetch distance in waves of resident CTAs (0 = off), measured per instantiation (profiles/r1_fft_tuning.md)
+// WAVES: L2 prefetch distance in waves of resident CTAs (0 = off), measured per instantiation
 template <int N, int C, int WAVES, int K = 8>
 tdx_status_t launch_fft_z(tdx_grid* g, const double* in, double* out, bool inverse, cudaStream_t st) {
     const size_t smem = (size_t)N * C * 16;
