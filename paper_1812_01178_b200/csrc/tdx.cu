@@ -366,6 +366,8 @@ tdx_status_t run_strided(const Plan& pl, double* data, long long W, long long li
     // Rows far apart in memory (z lines: stride = one xy-plane) like longer row segments; measured on cfg5 z.
     static const int env_row = [] { const char* e = std::getenv("TDX_ROW_DOUBLES"); return e ? std::atoi(e) : 0; }();
     int row_doubles = (line_stride * 8 >= (1 << 20)) ? 32 : 16;
+    const bool fat = set_per_outer && pl.M >= 32;             // 255-register instantiation, one table set per outer index: measured on cfg4 Helmholtz
+    if (fat) row_doubles = 32;                                //   256-byte rows + 8 tiles per CTA 0.389 ms against 0.406 (128-byte rows, 4 tiles)
     if (env_row == 16 || env_row == 32 || env_row == 64) row_doubles = env_row;
     auto pick = [&](int V, int& LPC) -> bool {
         const int bt = strided_block_threads(pl.M, V);
@@ -392,7 +394,8 @@ tdx_status_t run_strided(const Plan& pl, double* data, long long W, long long li
     if (set_per_outer) {
         const long long total = (long long)A.tiles_x * O;
         long long l = total / (16LL * pl.sms * 2);
-        loops = (int)(l < 1 ? 1 : (l > 4 ? 4 : l));                // measured: 4 tiles per CTA best on cfg4 and cfg5, 8+ loses balance
+        loops = (int)(l < 1 ? 1 : (l > 4 ? 4 : l));
+        if (fat) loops = A.tiles_x < 8 ? A.tiles_x : 8;             // one 256-thread CTA per SM: table reuse beats wave count here                // measured: 4 tiles per CTA best on cfg4 and cfg5, 8+ loses balance
         static const int env_loops = [] { const char* e = std::getenv("TDX_TILES_PER_CTA"); return e ? std::atoi(e) : 0; }();
         if (env_loops >= 1 && env_loops <= 64) loops = env_loops;
     }
