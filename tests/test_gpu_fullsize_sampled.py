@@ -110,3 +110,67 @@ def test_helmholtz_fullsize_sampled_lines(cfg_no):
     assert err < 1e-12, (cfg_no, err)
     assert np.all(got[ms == 0][:, 0, :] == 0.0)                 # pinned points of the zero mode
     grid.close()
+
+
+@pytest.mark.parametrize("cfg_no", [4, 5])
+def test_transforms_and_poisson_fullsize_sampled(cfg_no):
+    """SURVEY 8(f) N2 at the full sizes, in bench.py's launch configuration (TUNED_P_LINE, PPT): sampled x-lines of the
+    cosine transform and sampled z-columns of the Fourier transform against the oracle's dense sums, the round trips on
+    the whole field, and -- a property that holds at any size -- the residual of the discrete Poisson equation on
+    sampled z-planes of the solution, applied in physical space by the oracle's Laplacian."""
+    import transforms as otr
+    c = configs.get(cfg_no)
+    _need(int(c.npts * 8 * 3.4))
+    faces = c.faces()
+    grid = tdx.Grid(c.nx, c.ny, c.nz, *faces, bcs=BCS)
+    f_host = c.rhs_field()
+    t = torch.from_numpy(f_host).cuda()
+    rng = np.random.default_rng(300 + cfg_no)
+    # cosine transform: 12 sampled lines (the oracle's table is nx x nx)
+    picks = _picks(rng, 0, c.nx, c.ny, c.nz)[:12]
+    din = _sample_lines(t, 0, picks)
+    grid.dct_x(False, t)
+    torch.cuda.synchronize()
+    got = _sample_lines(t, 0, picks)
+    ref = otr.dct_x(din.reshape(1, len(picks), c.nx))[0]
+    assert float(np.max(np.abs(got - ref)) / np.max(np.abs(ref))) < 1e-12
+    # Fourier transform of the cosine-transformed field: 32 sampled (j, i) columns and their partners
+    spec = torch.empty((c.nm, c.ny, c.nx), dtype=torch.complex128, device="cuda")
+    pz = _picks(rng, 2, c.nx, c.ny, c.nz)[:32]
+    pz = np.concatenate([pz, np.stack([pz[:, 0], pz[:, 1] ^ 1], axis=1)])    # + the partner of every column: x-values 2c and 2c+1
+    zin = _sample_lines(t, 2, pz)                                # [64][nz]            are the re / im parts of ONE complex transform
+    grid.rfft_z(t, spec)
+    torch.cuda.synchronize()
+    ja, ia = torch.from_numpy(pz[:, 0]).cuda(), torch.from_numpy(pz[:, 1]).cuda()
+    zgot = spec[:, ja, ia].t().contiguous().cpu().numpy()        # [64][nm]
+    zref = otr.rfft_z(np.ascontiguousarray(zin.T).reshape(c.nz, 1, len(pz)))[:, 0, :].T
+    # error norm per column PAIR: rounding of the shared complex transform is relative to the larger of the two spectra
+    # (on this smooth field column i = 1 carries a mode 1e5 times larger than column i = 0)
+    amp = np.max(np.abs(zref), axis=1)
+    pair_scale = np.maximum(amp[:32], amp[32:])
+    err = np.max(np.abs(zgot - zref), axis=1)
+    assert np.max(np.maximum(err[:32], err[32:]) / pair_scale) < 1e-12
+    # round trips on the whole field
+    back = torch.empty_like(t)
+    grid.irfft_z(spec, back)
+    grid.dct_x(True, back)
+    torch.cuda.synchronize()
+    f_dev = torch.from_numpy(f_host).cuda()
+    scale = float(f_dev.abs().max())
+    assert float((back - f_dev).abs().max()) / scale < 1e-12
+    del back, t
+    # whole solve, PPT with bench.py's P; residual on 3 interior planes of a 5-plane window (and the wrap-around window)
+    P = bench.TUNED_P_LINE[cfg_no]
+    grid.poisson_solve(tdx.MODE_PPT, P, None, None, f_dev, spec)
+    torch.cuda.synchronize()
+    fmax = float(np.max(np.abs(f_host)))
+    for k0 in (int(rng.integers(1, c.nz - 5)), c.nz - 2):
+        ks = [(k0 + d) % c.nz for d in range(5)]
+        phi = f_dev[torch.tensor(ks, device="cuda")].cpu().numpy()          # 5 consecutive planes (periodic)
+        r = otr.laplacian(phi, faces[1], c.lx, 1.0 * 5 / c.nz)[1:4] - f_host[ks[1:4]]   # lz scaled so that dz is the grid's
+        r[:, 0, :] = 0.0                                         # row j = 0 carries the pinned mean mode's compatibility defect
+        # applying the Laplacian to phi in fp64 costs about eps * |phi| * 4 / dy_min^2 (dy_min ~ 6e-5 on these grids:
+        # ~1e-8 relative to max|f|; measured 2e-9), so that, not the solver, sets the gate; a wrong solve leaves O(1)
+        assert float(np.max(np.abs(r))) / fmax < 1e-7, (cfg_no, k0, float(np.max(np.abs(r))) / fmax)
+    assert abs(float(f_dev[:, 0, :].mean())) < 1e-12 * float(f_dev.abs().max()) + 1e-300   # the pin: mode (0,0) vanishes at j = 0
+    grid.close()
