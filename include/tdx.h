@@ -163,6 +163,18 @@ tdx_status_t tdx_slab_correct(tdx_slab_t* slab, double* field_inout, const doubl
                               void* stream);
 tdx_status_t tdx_slab_dropped_bound(tdx_slab_t* slab, double* out);
 
+/* Batched tridiagonal solve with PER-LINE coefficients and diagonal pivoting ("a parallel tridiagonal
+ * solver with diagonal pivoting is used [3]") -- for systems that are not diagonally dominant.
+ * a, b, c: DEVICE, nx*ny*nz doubles each, laid out like the field: row j of the line through (i, k) [dir = y] holds
+ * a = coupling to row j-1, b = diagonal, c = coupling to row j+1; a of a line's first row and c of its last row are
+ * not read.  pivoting != 0: 1x1 / 2x2 diagonal pivots without row interchanges (criterion: tdx_general.cuh);
+ * pivoting == 0: plain Thomas on the same data (breaks down on a zero pivot: inf / nan in that line, no error).
+ * rhs_inout: DEVICE, in place.  work: DEVICE scratch of 9*nx*ny*nz BYTES (modified diagonal + pivot types), 8-byte
+ * aligned, caller-owned.  dir = y or z (x lines: TDX_ERR_UNSUPPORTED).  A singular line yields inf / nan in that line.
+ * Thread-per-line baseline, two passes over HBM (about 100 B per value); asynchronous on `stream`.               */
+tdx_status_t tdx_general_solve(tdx_grid_t* grid, tdx_dir_t dir, int pivoting, const double* a, const double* b,
+                               const double* c, double* rhs_inout, void* work, void* stream);
+
 /* Batched cyclic tridiagonal solve along dir with caller-given coefficients shared by every line:
  * a, b, c: HOST arrays of n_dir doubles; a[0] couples row 0 to row n-1 and c[n-1] couples row n-1 to row 0.
  * Closure as for tdx_adi_sweep on a periodic direction (Sherman-Morrison with gamma = -b[0] for THOMAS / PDD, cyclic

@@ -6,7 +6,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(CSRC, "libtdx.so")
 SOURCES = ["tdx.cu"]
-DEPS = ["tdx.cu", "tdx_kernels.cuh", "tdx_plan.cuh", "tdx_tma.cuh", "tdx_fft.cuh", os.path.join("..", "..", "include", "tdx.h")]
+DEPS = ["tdx.cu", "tdx_kernels.cuh", "tdx_plan.cuh", "tdx_tma.cuh", "tdx_fft.cuh", "tdx_slab.cuh", "tdx_general.cuh", os.path.join("..", "..", "include", "tdx.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared", "-cudart", "static"]
 

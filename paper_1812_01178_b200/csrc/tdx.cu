@@ -22,6 +22,7 @@
 #include "tdx_tma.cuh"
 #include "tdx_fft.cuh"
 #include "tdx_slab.cuh"
+#include "tdx_general.cuh"
 
 namespace {
 
@@ -1147,6 +1148,29 @@ tdx_status_t tdx_slab_correct(tdx_slab_t* s, double* field, const double* iface_
 tdx_status_t tdx_slab_dropped_bound(tdx_slab_t* s, double* out) {
     if (!s || !out) return fail(TDX_ERR_INVALID_ARG, "NULL argument");
     *out = s->dropped;
+    return TDX_OK;
+}
+
+tdx_status_t tdx_general_solve(tdx_grid_t* g, tdx_dir_t dir, int pivoting, const double* a, const double* b, const double* c,
+                               double* rhs, void* work, void* stream) {
+    if (!g) return fail(TDX_ERR_INVALID_ARG, "grid is NULL");
+    if (!a || !b || !c || !rhs || !work) return fail(TDX_ERR_INVALID_ARG, "NULL argument");
+    if (dir != TDX_DIR_Y && dir != TDX_DIR_Z) return fail(TDX_ERR_UNSUPPORTED, "per-line coefficients are taken along y (the paper's case, L174) or z; dir=%d", (int)dir);
+    if (reinterpret_cast<uintptr_t>(work) & 7) return fail(TDX_ERR_INVALID_ARG, "work must be 8-byte aligned");
+    CUDA_TRY(cudaSetDevice(g->device));
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const int n = g->n_of(dir);
+    const long long inner = dir == TDX_DIR_Y ? g->nx : (long long)g->nx * g->ny, outer = dir == TDX_DIR_Y ? g->nz : 1;
+    if (outer > 65535) return fail(TDX_ERR_UNSUPPORTED, "outer extent > 65535");
+    const size_t npts = (size_t)g->nx * g->ny * g->nz;
+    double* bm = static_cast<double*>(work);
+    unsigned char* flag = reinterpret_cast<unsigned char*>(bm + npts);
+    dim3 block(128), grid((unsigned)((inner + 127) / 128), (unsigned)outer);
+    if (pivoting) tdx::k_general_forward<true><<<grid, block, 0, st>>>(a, b, c, rhs, bm, flag, n, inner, outer);
+    else tdx::k_general_forward<false><<<grid, block, 0, st>>>(a, b, c, rhs, bm, flag, n, inner, outer);
+    LAUNCH_CHECK("k_general_forward");
+    tdx::k_general_backward<<<grid, block, 0, st>>>(a, c, rhs, bm, flag, n, inner, outer);
+    LAUNCH_CHECK("k_general_backward");
     return TDX_OK;
 }
 
