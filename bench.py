@@ -398,6 +398,34 @@ def run_tdx(args, rank, world, local_rank):
                                 "what": "tdx_poisson_solve: dct_x, rfft_z, per-line y-solves (PPT), irfft_z, idct_x; 80 B per grid value"}
         del pfield, work
 
+        # per-line coefficients with diagonal pivoting along y (thread-per-line baseline, two passes):
+        # algorithmic bytes 82 per value (forward: a, b, c, d in; d, modified diagonal, pivot byte out; backward: d,
+        # diagonal, byte, c in; x out).  Random non-dominant systems (|b| <= 0.3, |a|, |c| <= 1).
+        try:
+            if torch.cuda.mem_get_info()[0] > 6.5 * cfg.npts * 8:
+                gen = torch.Generator(device=field0.device); gen.manual_seed(1234)
+                ga, gc = (torch.rand(field0.shape, dtype=torch.float64, device=field0.device, generator=gen) * 2 - 1 for _ in range(2))
+                gb = (torch.rand(field0.shape, dtype=torch.float64, device=field0.device, generator=gen) * 2 - 1) * 0.3
+                gd = field0.clone()
+                gwork = torch.empty(9 * cfg.npts + 64, dtype=torch.uint8, device=field0.device)
+                for _ in range(2):
+                    gd.copy_(field0); grid.general_solve(1, True, ga, gb, gc, gd, gwork, stream)
+                barrier()
+                tot = 0.0
+                for _ in range(args.steps):
+                    gd.copy_(field0)
+                    s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    s0.record(); grid.general_solve(1, True, ga, gb, gc, gd, gwork, stream); s1.record()
+                    torch.cuda.synchronize()
+                    tot += s0.elapsed_time(s1)
+                msg = max_over_ranks(tot / args.steps, dist, "cuda")
+                out["general_solve_pivoting"] = {"ms": msg, "gpts_per_s": cfg.npts / (msg * 1e-3) / 1e9, "gb_per_s": 82 * cfg.npts / (msg * 1e-3) / 1e9,
+                                                 "frac_of_measured_peak": 82 * cfg.npts / (msg * 1e-3) / 1e9 / peak, "finite": bool(torch.isfinite(gd).all()),
+                                                 "what": "tdx_general_solve along y, per-line a, b, c, diagonal pivoting; 82 B per value over two passes"}
+                del ga, gb, gc, gd, gwork
+        except Exception as exc:
+            out["general_solve_pivoting"] = {"error": repr(exc)[:300]}
+
         # the y sweep with the field cut into y-slabs, one per rank (the paper's decomposition, L74): local
         # elimination (the slab's own sweep kernel) + interface exchange + one correction pass = 32 B per grid value.
         # world == 1: the compute part of an interior rank of a 4-rank job (a quarter slab; the exchange is a device copy);
