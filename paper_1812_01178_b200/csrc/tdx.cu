@@ -1012,6 +1012,8 @@ tdx_status_t tdx_poisson_solve(tdx_grid_t* g, tdx_mode_t mode, int P, const doub
         for (int m = 0; m < nm; ++m) { const double s = std::sin(M_PI * m / nz); kz[m] = 4.0 * s * s / (dz * dz); }          // = 2(1-cos(2 pi m/nz))/dz^2
         kz2 = kz.data();
     }
+    for (int i = 0; i < nx; ++i) if (!(kx2[i] >= 0.0)) return fail(TDX_ERR_INVALID_ARG, "kx2[%d] is negative or NaN", i);
+    for (int m = 0; m < nm; ++m) if (!(kz2[m] >= 0.0)) return fail(TDX_ERR_INVALID_ARG, "kz2[%d] is negative or NaN", m);
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     rc = run_dct_x(g, field, false, st);                                       if (rc != TDX_OK) return rc;
     rc = run_fft_z(g, field, spec_work, false, st);                            if (rc != TDX_OK) return rc;

@@ -122,6 +122,13 @@ def test_transform_error_paths_leave_data_untouched():
     with pytest.raises(tdx.TdxError) as e:
         grid.poisson_solve(tdx.MODE_PPT, 3, None, None, t, spec)   # 16 rows / 3 partitions: not P*M
     assert e.value.status in (tdx.ERR_UNSUPPORTED, tdx.ERR_BAD_PARTITION)
+    t.fill_(1.5)
+    bad = np.full(32, 1.0); bad[7] = float("nan")
+    with pytest.raises(tdx.TdxError) as e:                       # a bad wavenumber is caught before the first transform runs
+        grid.poisson_solve(tdx.MODE_THOMAS, 1, bad, None, t, spec)
+    assert e.value.status == tdx.ERR_INVALID_ARG
+    torch.cuda.synchronize()
+    assert bool((t == 1.5).all())
     grid.close()
 
 
