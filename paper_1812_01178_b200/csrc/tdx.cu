@@ -634,13 +634,36 @@ tdx_status_t launch_fft_z(tdx_grid* g, const double* in, double* out, bool inver
     return TDX_OK;
 }
 
+bool fft_len_ok(int N, int lo, int hi) {      // 2^k or 3 * 2^k
+    if (N < lo || N > hi) return false;
+    return pow2(N) || (N % 3 == 0 && pow2(N / 3) && N / 3 >= 16);
+}
+
+template <int N, int C>
+tdx_status_t launch_fft_z3(tdx_grid* g, const double* in, double* out, bool inverse, cudaStream_t st) {
+    const size_t smem = (size_t)N * C * 16;
+    dim3 block(C, N / 24), grid((g->nx + 2 * C - 1) / (2 * C), g->ny);
+    if (!inverse) {
+        static bool done = false;
+        if (!done) { CUDA_TRY(cudaFuncSetAttribute(k_rfft_z3<N, C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); done = true; }
+        k_rfft_z3<N, C><<<grid, block, smem, st>>>(in, reinterpret_cast<double2*>(out), g->nx, g->ny, g->fft_tw[2]);
+        LAUNCH_CHECK("k_rfft_z3");
+    } else {
+        static bool done = false;
+        if (!done) { CUDA_TRY(cudaFuncSetAttribute(k_irfft_z3<N, C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); done = true; }
+        k_irfft_z3<N, C><<<grid, block, smem, st>>>(reinterpret_cast<const double2*>(in), out, g->nx, g->ny, g->fft_tw[2]);
+        LAUNCH_CHECK("k_irfft_z3");
+    }
+    return TDX_OK;
+}
+
 tdx_status_t run_fft_z(tdx_grid* g, const double* in, double* out, bool inverse, cudaStream_t st) {
     if (!g) return fail(TDX_ERR_INVALID_ARG, "grid is NULL");
     if (!in || !out) return fail(TDX_ERR_INVALID_ARG, "data pointer is NULL");
     if (in == out) return fail(TDX_ERR_INVALID_ARG, "the z transform is out of place (real nz planes <-> nz/2+1 complex planes)");
     if ((reinterpret_cast<uintptr_t>(in) | reinterpret_cast<uintptr_t>(out)) & 15) return fail(TDX_ERR_INVALID_ARG, "buffers must be 16-byte aligned");
     const int N = g->nz;
-    if (!pow2(N) || N < 16 || N > 1024) return fail(TDX_ERR_UNSUPPORTED, "z transform needs nz a power of two in [16, 1024]; nz=%d", N);
+    if (!fft_len_ok(N, 16, 1536)) return fail(TDX_ERR_UNSUPPORTED, "z transform needs nz = 2^k in [16, 1024] or 3*2^k in [48, 1536]; nz=%d", N);
     if (g->nx % 2) return fail(TDX_ERR_UNSUPPORTED, "z transform pairs adjacent x values: nx=%d must be even", g->nx);
     if (g->ny > 65535) return fail(TDX_ERR_UNSUPPORTED, "ny > 65535");
     CUDA_TRY(cudaSetDevice(g->device));
@@ -648,6 +671,12 @@ tdx_status_t run_fft_z(tdx_grid* g, const double* in, double* out, bool inverse,
     if (rc != TDX_OK) return rc;
     // tile width (C column pairs = 32*C bytes of a real row) and prefetch per (N, direction): measured on cfg4 / cfg5
     switch (N) {
+        case 48:   return launch_fft_z3<48, 16>(g, in, out, inverse, st);
+        case 96:   return launch_fft_z3<96, 16>(g, in, out, inverse, st);
+        case 192:  return launch_fft_z3<192, 16>(g, in, out, inverse, st);
+        case 384:  return launch_fft_z3<384, 8>(g, in, out, inverse, st);
+        case 768:  return launch_fft_z3<768, 8>(g, in, out, inverse, st);
+        case 1536: return launch_fft_z3<1536, 8>(g, in, out, inverse, st);
         case 16:   return launch_fft_z<16, 16, 1>(g, in, out, inverse, st);
         case 32:   return launch_fft_z<32, 16, 1>(g, in, out, inverse, st);
         case 64:   return launch_fft_z<64, 16, 1>(g, in, out, inverse, st);
@@ -679,16 +708,44 @@ tdx_status_t launch_dct_x(tdx_grid* g, double* field, bool inverse, cudaStream_t
     return TDX_OK;
 }
 
+template <int N, int LP>
+tdx_status_t launch_dct_x3(tdx_grid* g, double* field, bool inverse, cudaStream_t st) {
+    const long long lines = (long long)g->ny * g->nz;
+    const size_t smem = (size_t)LP * (N + N / 8) * 16 + 16;
+    const long long ctas = (lines + 2 * LP - 1) / (2 * LP);
+    if (ctas > 2147483647LL) return fail(TDX_ERR_UNSUPPORTED, "too many lines");
+    const int resident = std::max(1, std::min((int)(220 * 1024 / smem), 2048 / (LP * N / 24)));
+    const int pf = g->sms * resident * prefetch_waves();
+    if (!inverse) {
+        static bool done = false;
+        if (!done) { CUDA_TRY(cudaFuncSetAttribute(k_dct_x3<N, LP, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); done = true; }
+        k_dct_x3<N, LP, 0><<<(unsigned)ctas, LP * N / 24, smem, st>>>(field, lines, g->fft_tw[0], g->fft_w4, pf);
+    } else {
+        static bool done = false;
+        if (!done) { CUDA_TRY(cudaFuncSetAttribute(k_dct_x3<N, LP, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); done = true; }
+        k_dct_x3<N, LP, 1><<<(unsigned)ctas, LP * N / 24, smem, st>>>(field, lines, g->fft_tw[0], g->fft_w4, pf);
+    }
+    LAUNCH_CHECK("k_dct_x3");
+    return TDX_OK;
+}
+
 tdx_status_t run_dct_x(tdx_grid* g, double* field, bool inverse, cudaStream_t st) {
     if (!g) return fail(TDX_ERR_INVALID_ARG, "grid is NULL");
     if (!field) return fail(TDX_ERR_INVALID_ARG, "data pointer is NULL");
     if (reinterpret_cast<uintptr_t>(field) & 15) return fail(TDX_ERR_INVALID_ARG, "field must be 16-byte aligned");
     const int N = g->nx;
-    if (!pow2(N) || N < 16 || N > 4096) return fail(TDX_ERR_UNSUPPORTED, "x transform needs nx a power of two in [16, 4096]; nx=%d", N);
+    if (!fft_len_ok(N, 16, 4096)) return fail(TDX_ERR_UNSUPPORTED, "x transform needs nx = 2^k in [16, 4096] or 3*2^k in [48, 3072]; nx=%d", N);
     CUDA_TRY(cudaSetDevice(g->device));
     tdx_status_t rc = fft_tables(g, 0, st);
     if (rc != TDX_OK) return rc;
     switch (N) {
+        case 48:   return launch_dct_x3<48, 64>(g, field, inverse, st);
+        case 96:   return launch_dct_x3<96, 32>(g, field, inverse, st);
+        case 192:  return launch_dct_x3<192, 16>(g, field, inverse, st);
+        case 384:  return launch_dct_x3<384, 8>(g, field, inverse, st);
+        case 768:  return launch_dct_x3<768, 4>(g, field, inverse, st);
+        case 1536: return launch_dct_x3<1536, 2>(g, field, inverse, st);
+        case 3072: return launch_dct_x3<3072, 1>(g, field, inverse, st);
         case 16:   return launch_dct_x<16, 128>(g, field, inverse, st);
         case 32:   return launch_dct_x<32, 64>(g, field, inverse, st);
         case 64:   return launch_dct_x<64, 32>(g, field, inverse, st);
@@ -988,8 +1045,8 @@ tdx_status_t tdx_poisson_solve(tdx_grid_t* g, tdx_mode_t mode, int P, const doub
     if (field == spec_work) return fail(TDX_ERR_INVALID_ARG, "field and spec_work must differ");
     const int nx = g->nx, nz = g->nz, nm = nz / 2 + 1;
     // every check of the five stages first: nothing is written on an argument error
-    if (!pow2(nx) || nx < 16 || nx > 4096) return fail(TDX_ERR_UNSUPPORTED, "x transform needs nx a power of two in [16, 4096]; nx=%d", nx);
-    if (!pow2(nz) || nz < 16 || nz > 1024) return fail(TDX_ERR_UNSUPPORTED, "z transform needs nz a power of two in [16, 1024]; nz=%d", nz);
+    if (!fft_len_ok(nx, 16, 4096)) return fail(TDX_ERR_UNSUPPORTED, "x transform needs nx = 2^k in [16, 4096] or 3*2^k in [48, 3072]; nx=%d", nx);
+    if (!fft_len_ok(nz, 16, 1536)) return fail(TDX_ERR_UNSUPPORTED, "z transform needs nz = 2^k in [16, 1024] or 3*2^k in [48, 1536]; nz=%d", nz);
     if ((reinterpret_cast<uintptr_t>(field) | reinterpret_cast<uintptr_t>(spec_work)) & 15) return fail(TDX_ERR_INVALID_ARG, "buffers must be 16-byte aligned");
     if (mode != TDX_MODE_THOMAS) {
         if (P < 2 || P > TDX_MAX_P || g->ny / P < 2) return fail(TDX_ERR_BAD_PARTITION, "P=%d invalid for line length %d", P, g->ny);

@@ -82,7 +82,7 @@ __device__ __forceinline__ void dft16(double2 (&v)[16]) {
 // One Stockham pass of radix R on the K register points of thread t (slot kk = point t + kk*N/K).  NS = product of
 // the radices of the earlier passes.  Butterfly s (of B = K/R) takes slots s + r*B, r < R; its index is j = t + s*N/K.
 // pos[kk] receives the position the slot's value has after the pass: (j - j%NS)*R + j%NS + r*NS.
-template <int N, int K, int R, int NS>
+template <int N, int K, int R, int NS, int TWS = 1>
 __device__ __forceinline__ void fft_pass(double2 (&v)[K], int (&pos)[K], int t, const double2* __restrict__ tw) {
     constexpr int T = N / K, B = K / R;
 #pragma unroll
@@ -93,7 +93,7 @@ __device__ __forceinline__ void fft_pass(double2 (&v)[K], int (&pos)[K], int t, 
 #pragma unroll
         for (int r = 0; r < R; ++r) x[r] = v[s + r * B];
         if (NS > 1) {
-            const double2 w1 = __ldg(tw + jm * (N / (NS * R)));
+            const double2 w1 = __ldg(tw + TWS * (jm * (N / (NS * R))));      // TWS: stride into a table of TWS*N roots
             x[1] = cmul(x[1], w1);
             if constexpr (R >= 4) {
                 const double2 w2 = cmul(w1, w1), w3 = cmul(w2, w1);
@@ -138,6 +138,43 @@ __device__ __forceinline__ void fft_regs(double2 (&v)[K], int t, const double2* 
         __syncthreads();
         fft_regs<N, K, NS * R, SM>(v, t, tw, sm);
     }
+}
+
+// Three transforms of length M side by side in one thread (the sub-sequences x_{3m+r}, r = 0, 1, 2, of a transform of
+// length N = 3M): the same passes in lockstep, sharing the barriers.  tw is the table of N-th roots (stride 3 gives the
+// M-th roots).  sm[r] maps positions of sub-transform r.
+template <int M, int K, int NS, class SM>
+__device__ __forceinline__ void fft_regs3(double2 (&v)[3][K], int t, const double2* __restrict__ tw, const SM (&sm)[3]) {
+    constexpr int T = M / K;
+    constexpr int R = (M / NS >= K) ? K : (M / NS);
+    int pos[K];
+#pragma unroll
+    for (int r = 0; r < 3; ++r) fft_pass<M, K, R, NS, 3>(v[r], pos, t, tw);
+    if constexpr (NS * R < M) {
+#pragma unroll
+        for (int r = 0; r < 3; ++r)
+#pragma unroll
+            for (int kk = 0; kk < K; ++kk) *sm[r].at(pos[kk]) = v[r][kk];
+        __syncthreads();
+#pragma unroll
+        for (int r = 0; r < 3; ++r)
+#pragma unroll
+            for (int kk = 0; kk < K; ++kk) v[r][kk] = *sm[r].at(t + kk * T);
+        __syncthreads();
+        fft_regs3<M, K, NS * R, SM>(v, t, tw, sm);
+    }
+}
+
+// Radix-3 recombination X[k + s M] = sum_r W_3^{r s} W_N^{r k} F_r[k] (decimation in time by 3); in place: f_r -> X_s.
+__device__ __forceinline__ void combine3(double2& f0, double2& f1, double2& f2, double2 w1, double2 w2) {
+    const double hs = 0.86602540378443864676;                   // sqrt(3)/2
+    const double2 b = cmul(f1, w1), c = cmul(f2, w2);
+    const double2 s = cadd(b, c), d = csub(b, c);
+    const double2 m = make_double2(f0.x - 0.5 * s.x, f0.y - 0.5 * s.y);
+    const double2 rot = make_double2(hs * d.y, -hs * d.x);       // -i sqrt(3)/2 (b - c)
+    f0 = cadd(f0, s);
+    f1 = cadd(m, rot);                                           // a + w b + w^2 c, w = exp(-2 pi i / 3)
+    f2 = csub(m, rot);
 }
 
 // shared-memory maps
@@ -389,6 +426,221 @@ __global__ void __launch_bounds__(LP * N / K) k_dct_x(double* __restrict__ field
             const int n = t + kk * T;
             const int idx = (n < N / 2) ? 2 * n : 2 * (N - 1 - n) + 1;
             oa[idx] = v[kk].y * sc; ob[idx] = v[kk].x * sc;                    // un-swap: re of the inverse is the stored im
+        }
+    }
+    fence_proxy_async();
+    __syncthreads();
+    if (tid == 0) {
+        bulk_store_1d(gsrc, raw, bytes);
+        tma_commit();
+        tma_wait_read<0>();
+    }
+}
+
+// ---- lengths N = 3 * 2^k (the paper's own grid is 3072 x 256 x 768) ------------------------------
+// Decimation in time by 3: every thread runs the three M-point sub-transforms of its points side by side (8 points each)
+// and recombines them in registers (combine3); loads, stores and the pairing of the two real transforms are as above.
+template <int N, int C>
+__global__ void __launch_bounds__(C * N / 24) k_rfft_z3(const double* __restrict__ in, double2* __restrict__ out, int nx, int ny,
+                                                         const double2* __restrict__ tw) {
+    constexpr int K = 8, M = N / 3, T = M / K;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    double2* smb = reinterpret_cast<double2*>(smem_raw);
+    const int c = threadIdx.x, t = threadIdx.y, j = blockIdx.y;
+    const long long i0 = (long long)blockIdx.x * 2 * C + 2 * c;
+    const bool act = i0 < nx;
+    const size_t plane = (size_t)nx * ny;
+    const double* src = in + (size_t)j * nx + i0;
+    double2 v[3][K];
+#pragma unroll
+    for (int r = 0; r < 3; ++r)
+#pragma unroll
+        for (int kk = 0; kk < K; ++kk)
+            v[r][kk] = act ? __ldcs(reinterpret_cast<const double2*>(src + (size_t)(3 * (t + kk * T) + r) * plane)) : make_double2(0.0, 0.0);
+    const SmCols sm[3] = {{smb + c, C}, {smb + (size_t)M * C + c, C}, {smb + (size_t)2 * M * C + c, C}};
+    fft_regs3<M, K, 1, SmCols>(v, t, tw, sm);
+    const SmCols all{smb + c, C};
+#pragma unroll
+    for (int kk = 0; kk < K; ++kk) {
+        const int k = t + kk * T;
+        combine3(v[0][kk], v[1][kk], v[2][kk], __ldg(tw + k), __ldg(tw + 2 * k));
+        *all.at(k) = v[0][kk]; *all.at(k + M) = v[1][kk]; *all.at(k + 2 * M) = v[2][kk];
+    }
+    __syncthreads();
+    double2* dst = out + (size_t)j * nx + i0;
+#pragma unroll
+    for (int kk = 0; kk < 3 * K / 2; ++kk) {
+        const int m = t + kk * T;
+        const double2 zm = *all.at(m), zn = *all.at(m == 0 ? 0 : N - m);
+        if (act) {
+            double2* o = dst + (size_t)m * plane;
+            __stcs(o, make_double2(0.5 * (zm.x + zn.x), 0.5 * (zm.y - zn.y)));
+            __stcs(o + 1, make_double2(0.5 * (zm.y + zn.y), 0.5 * (zn.x - zm.x)));
+        }
+    }
+    if (t == 0 && act) {
+        const double2 z = *all.at(N / 2);
+        double2* o = dst + (size_t)(N / 2) * plane;
+        __stcs(o, make_double2(z.x, 0.0));
+        __stcs(o + 1, make_double2(z.y, 0.0));
+    }
+}
+
+template <int N, int C>
+__global__ void __launch_bounds__(C * N / 24) k_irfft_z3(const double2* __restrict__ in, double* __restrict__ out, int nx, int ny,
+                                                          const double2* __restrict__ tw) {
+    constexpr int K = 8, M = N / 3, T = M / K;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    double2* smb = reinterpret_cast<double2*>(smem_raw);
+    const int c = threadIdx.x, t = threadIdx.y, j = blockIdx.y;
+    const long long i0 = (long long)blockIdx.x * 2 * C + 2 * c;
+    const bool act = i0 < nx;
+    const size_t plane = (size_t)nx * ny;
+    const double2* src = in + (size_t)j * nx + i0;
+    const SmCols all{smb + c, C};
+#pragma unroll
+    for (int kk = 0; kk <= 3 * K / 2; ++kk) {
+        if (kk == 3 * K / 2 && t != 0) break;
+        const int m = (kk == 3 * K / 2) ? N / 2 : t + kk * T;
+        const double2* p = src + (size_t)m * plane;
+        const double2 a = act ? __ldcs(p) : make_double2(0.0, 0.0), b = act ? __ldcs(p + 1) : make_double2(0.0, 0.0);
+        if (m == 0 || m == N / 2) {
+            *all.at(m) = make_double2(b.x, a.x);
+        } else {
+            *all.at(m) = make_double2(a.y + b.x, a.x - b.y);
+            *all.at(N - m) = make_double2(b.x - a.y, a.x + b.y);
+        }
+    }
+    __syncthreads();
+    double2 v[3][K];
+#pragma unroll
+    for (int r = 0; r < 3; ++r)
+#pragma unroll
+        for (int kk = 0; kk < K; ++kk) v[r][kk] = *all.at(3 * (t + kk * T) + r);
+    __syncthreads();
+    const SmCols sm[3] = {{smb + c, C}, {smb + (size_t)M * C + c, C}, {smb + (size_t)2 * M * C + c, C}};
+    fft_regs3<M, K, 1, SmCols>(v, t, tw, sm);
+    const double sc = 1.0 / (double)N;
+    double* dst = out + (size_t)j * nx + i0;
+#pragma unroll
+    for (int kk = 0; kk < K; ++kk) {
+        const int k = t + kk * T;
+        combine3(v[0][kk], v[1][kk], v[2][kk], __ldg(tw + k), __ldg(tw + 2 * k));
+        if (act) {
+#pragma unroll
+            for (int s = 0; s < 3; ++s)
+                __stcs(reinterpret_cast<double2*>(dst + (size_t)(k + s * M) * plane), make_double2(v[s][kk].y * sc, v[s][kk].x * sc));
+        }
+    }
+}
+
+template <int N, int LP, int INV>
+__global__ void __launch_bounds__(LP * N / 24) k_dct_x3(double* __restrict__ field, long long lines,
+                                                         const double2* __restrict__ tw, const double2* __restrict__ w4, int pf) {
+    constexpr int K = 8, M = N / 3, T = M / K, H3 = 3 * K / 2;
+    constexpr int PSTR = N + N / 8;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    double2* smb = reinterpret_cast<double2*>(smem_raw);
+    double* raw = reinterpret_cast<double*>(smem_raw);
+    uint64_t* bar = reinterpret_cast<uint64_t*>(smem_raw + (size_t)LP * PSTR * 16);
+    const int tid = threadIdx.x;
+    const int p = tid / T, t = tid - p * T;
+    const long long line0 = (long long)blockIdx.x * 2 * LP;
+    const long long nl = min((long long)2 * LP, lines - line0);
+    const uint32_t bytes = (uint32_t)(nl * N * 8);
+    double* gsrc = field + (size_t)line0 * N;
+    if (tid == 0) { mbar_init(bar, 1); mbar_fence_init(); }
+    __syncthreads();
+    if (tid == 0) {
+        mbar_arrive_expect_tx(bar, bytes);
+        bulk_load_1d(raw, gsrc, bytes, bar);
+        if (pf > 0) {
+            const long long l2 = line0 + (long long)pf * 2 * LP;
+            if (l2 < lines) bulk_prefetch_1d(field + (size_t)l2 * N, (uint32_t)(min((long long)2 * LP, lines - l2) * N * 8));
+        }
+    }
+    mbar_wait(bar, 0);
+    const bool has_a = 2 * p < nl, has_b = 2 * p + 1 < nl;
+    double* la = raw + (size_t)p * 2 * N;
+    double* lb = la + N;
+    const SmPad<8> all{smb + (size_t)p * PSTR};
+    const SmPad<8> sm[3] = {{smb + (size_t)p * PSTR}, {smb + (size_t)p * PSTR + (M + M / 8)}, {smb + (size_t)p * PSTR + 2 * (M + M / 8)}};
+    double2 v[3][K];
+    if (!INV) {
+#pragma unroll
+        for (int r = 0; r < 3; ++r)
+#pragma unroll
+            for (int kk = 0; kk < K; ++kk) {
+                const int n = 3 * (t + kk * T) + r;
+                const int idx = (n < N / 2) ? 2 * n : 2 * (N - 1 - n) + 1;
+                v[r][kk] = make_double2(has_a ? la[idx] : 0.0, has_b ? lb[idx] : 0.0);
+            }
+        __syncthreads();
+        fft_regs3<M, K, 1, SmPad<8>>(v, t, tw, sm);
+#pragma unroll
+        for (int kk = 0; kk < K; ++kk) {
+            const int k = t + kk * T;
+            combine3(v[0][kk], v[1][kk], v[2][kk], __ldg(tw + k), __ldg(tw + 2 * k));
+            *all.at(k) = v[0][kk]; *all.at(k + M) = v[1][kk]; *all.at(k + 2 * M) = v[2][kk];
+        }
+        __syncthreads();
+        double2 zk[H3 + 1], zn[H3 + 1];
+#pragma unroll
+        for (int kk = 0; kk < H3; ++kk) { const int k = t + kk * T; zk[kk] = *all.at(k); zn[kk] = *all.at(k == 0 ? 0 : N - k); }
+        if (t == 0) { zk[H3] = *all.at(N / 2); zn[H3] = zk[H3]; }
+        __syncthreads();
+#pragma unroll
+        for (int kk = 0; kk <= H3; ++kk) {
+            if (kk == H3 && t != 0) break;
+            const int k = (kk == H3) ? N / 2 : t + kk * T;
+            const double2 va = make_double2(0.5 * (zk[kk].x + zn[kk].x), 0.5 * (zk[kk].y - zn[kk].y));
+            const double2 vb = make_double2(0.5 * (zk[kk].y + zn[kk].y), 0.5 * (zn[kk].x - zk[kk].x));
+            const double2 w = __ldg(w4 + k);
+            const double2 ya = cmul(w, va), yb = cmul(w, vb);
+            la[k] = ya.x; lb[k] = yb.x;
+            if (k != 0 && k != N / 2) { la[N - k] = -ya.y; lb[N - k] = -yb.y; }
+        }
+    } else {
+        double xa[H3 + 1], xan[H3 + 1], xb[H3 + 1], xbn[H3 + 1];
+#pragma unroll
+        for (int kk = 0; kk <= H3; ++kk) {
+            if (kk == H3 && t != 0) break;
+            const int k = (kk == H3) ? N / 2 : t + kk * T;
+            xa[kk] = has_a ? la[k] : 0.0; xb[kk] = has_b ? lb[k] : 0.0;
+            xan[kk] = (k == 0 || !has_a) ? 0.0 : la[N - k];
+            xbn[kk] = (k == 0 || !has_b) ? 0.0 : lb[N - k];
+        }
+        __syncthreads();
+#pragma unroll
+        for (int kk = 0; kk <= H3; ++kk) {
+            if (kk == H3 && t != 0) break;
+            const int k = (kk == H3) ? N / 2 : t + kk * T;
+            const double2 w = __ldg(w4 + k);
+            const double2 wc = make_double2(w.x, -w.y);
+            const double2 va = cmul(wc, make_double2(xa[kk], -xan[kk]));
+            const double2 vb = cmul(wc, make_double2(xb[kk], -xbn[kk]));
+            *all.at(k) = make_double2(va.y + vb.x, va.x - vb.y);
+            if (k != 0 && k != N / 2) *all.at(N - k) = make_double2(vb.x - va.y, va.x + vb.y);
+        }
+        __syncthreads();
+#pragma unroll
+        for (int r = 0; r < 3; ++r)
+#pragma unroll
+            for (int kk = 0; kk < K; ++kk) v[r][kk] = *all.at(3 * (t + kk * T) + r);
+        __syncthreads();
+        fft_regs3<M, K, 1, SmPad<8>>(v, t, tw, sm);
+        __syncthreads();
+        const double sc = 1.0 / (double)N;
+#pragma unroll
+        for (int kk = 0; kk < K; ++kk) {
+            const int k = t + kk * T;
+            combine3(v[0][kk], v[1][kk], v[2][kk], __ldg(tw + k), __ldg(tw + 2 * k));
+#pragma unroll
+            for (int s = 0; s < 3; ++s) {
+                const int n = k + s * M;
+                const int idx = (n < N / 2) ? 2 * n : 2 * (N - 1 - n) + 1;
+                la[idx] = v[s][kk].y * sc; lb[idx] = v[s][kk].x * sc;
+            }
         }
     }
     fence_proxy_async();

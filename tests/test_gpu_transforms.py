@@ -27,7 +27,8 @@ def make_grid(nx, ny, nz, lx=2.0):
 
 # every kernel instantiation: nx = 16 .. 4096; line counts that leave a partial last CTA (ny*nz not a multiple of 2*LP)
 @pytest.mark.parametrize("nx,ny,nz", [(16, 5, 16), (32, 3, 16), (64, 5, 16), (128, 7, 16), (256, 9, 16), (512, 3, 16),
-                                      (1024, 3, 16), (2048, 3, 16), (4096, 3, 16)])
+                                      (1024, 3, 16), (2048, 3, 16), (4096, 3, 16),
+                                      (48, 5, 16), (96, 3, 16), (192, 5, 16), (384, 3, 16), (768, 3, 16), (1536, 3, 16), (3072, 3, 16)])
 def test_dct_x_forward_and_inverse(nx, ny, nz):
     faces, grid = make_grid(nx, ny, nz)
     x = inputs.rhs_uniform((nz, ny, nx), 100 + nx)
@@ -68,7 +69,8 @@ def test_dct_x_one_hot_touches_only_its_line_and_is_the_cosine_row():
     grid.close()
 
 
-@pytest.mark.parametrize("nx,ny,nz", [(16, 3, 16), (50, 4, 32), (64, 3, 64), (34, 2, 128), (32, 3, 256), (36, 2, 512), (18, 2, 1024)])
+@pytest.mark.parametrize("nx,ny,nz", [(16, 3, 16), (50, 4, 32), (64, 3, 64), (34, 2, 128), (32, 3, 256), (36, 2, 512), (18, 2, 1024),
+                                      (34, 3, 48), (16, 2, 96), (50, 2, 192), (18, 3, 384), (36, 2, 768), (20, 2, 1536)])
 def test_rfft_z_forward_and_inverse(nx, ny, nz):
     """nx even but not a multiple of the 32-wide column tile: ragged last tile."""
     faces = (inputs.faces_uniform(nx, 1.0), inputs.faces_tanh_one_sided(ny, 2.5), inputs.faces_uniform(nz, 1.0))
@@ -99,7 +101,7 @@ def test_rfft_z_forward_and_inverse(nx, ny, nz):
 
 
 def test_transform_error_paths_leave_data_untouched():
-    nx, ny, nz = 48, 4, 24                                   # not powers of two
+    nx, ny, nz = 40, 4, 24                                   # neither 2^k nor 3 * 2^k (k >= 4)
     faces = (inputs.faces_uniform(nx, 1.0), inputs.faces_tanh_one_sided(ny, 2.5), inputs.faces_uniform(nz, 1.0))
     grid = tdx.Grid(nx, ny, nz, *faces, bcs=BCS)
     x = inputs.rhs_uniform((nz, ny, nx), 7)
@@ -168,6 +170,24 @@ def test_poisson_solve_cfg2(cfg2, mode, P):
     grid.poisson_solve(mode, P, None, None, t2, work)
     torch.cuda.synchronize()
     assert relerr(t2.cpu().numpy(), ref) < 2e-12
+
+
+def test_poisson_solve_factor_three_sizes():
+    """nx = 96 = 3 * 32, nz = 48 = 3 * 16 (the paper's own grid, 3072 x 256 x 768, has a factor 3 in x and z: L182, L314)."""
+    nx, ny, nz = 96, 32, 48
+    faces, grid = make_grid(nx, ny, nz, lx=2.0)
+    phi = inputs.rhs_uniform((nz, ny, nx), 33)
+    f = otr.laplacian(phi, faces[1], 2.0, 1.0)
+    work = torch.empty((nz // 2 + 1, ny, nx), dtype=torch.complex128, device="cuda")
+    ref = otr.poisson_solve(f, faces[1], 2.0, 1.0)
+    for mode, P in ((tdx.MODE_THOMAS, 1), (tdx.MODE_PPT, 4)):
+        t = torch.from_numpy(f).cuda()
+        grid.poisson_solve(mode, P, None, None, t, work)
+        torch.cuda.synchronize()
+        got = t.cpu().numpy()
+        assert relerr(got, ref) < 2e-12, (mode, P, relerr(got, ref))
+        assert relerr(got, phi - np.mean(phi[:, 0, :])) < 1e-9
+    grid.close()
 
 
 def test_poisson_solve_manufactured_small_every_element():
