@@ -30,7 +30,7 @@ UNIT = "Gpts/s"
 BYTES_PER_POINT = 16.0          # 8 B read + 8 B written per real grid value per sweep
 
 # partitions per line for the per-line-shift Helmholtz solve (kx2 != 0): ny = P*M with M in {8, 12, 16}
-TUNED_P_LINE = {1: 4, 2: 16, 3: 32, 4: 32, 5: 24}
+TUNED_P_LINE = {1: 4, 2: 16, 3: 32, 4: 32, 5: 24, 6: 16}
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures
 # (profiles/r1_ncu_cfg5_summary.md), valid for mode ppt with the tuned P of the config; bytes.
@@ -40,7 +40,7 @@ NCU_TRAFFIC = {
 }
 
 # tuned partitions per line (x, y, z, helmholtz-y) per config; rows per partition <= 64
-TUNED_P = {1: (4, 4, 4, 4), 2: (16, 8, 8, 8), 3: (32, 8, 8, 8), 4: (64, 16, 8, 16), 5: (256, 24, 16, 12)}
+TUNED_P = {1: (4, 4, 4, 4), 2: (16, 8, 8, 8), 3: (32, 8, 8, 8), 4: (64, 16, 8, 16), 5: (256, 24, 16, 12), 6: (192, 8, 24, 8)}
 
 
 def parse():
@@ -49,7 +49,7 @@ def parse():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="tdx", choices=["tdx", "reference"])
-    ap.add_argument("--config", type=int, default=5, help="BASELINE.json config number 1..5")
+    ap.add_argument("--config", type=int, default=5, help="BASELINE.json config number 1..5; 6 = the paper's own 3072x256x768 grid")
     ap.add_argument("--mode", default="ppt", choices=["ppt", "pdd", "thomas"])
     ap.add_argument("--P", default="", help="override partitions: Px,Py,Pz,Ph")
     ap.add_argument("--no-e2e", action="store_true")

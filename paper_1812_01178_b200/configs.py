@@ -1,4 +1,4 @@
-"""The five BASELINE.json workloads as plain data.
+"""The five BASELINE.json workloads (+ the paper's own 607M grid as number 6) as plain data.
 Only dimensions, stretching, alpha = dt/(2 Re), seeds and RHS kind: no arithmetic of the method."""
 from dataclasses import dataclass
 import numpy as np
@@ -62,6 +62,9 @@ CONFIGS = (
     Config("cfg3_512x256x256", 512, 256, 256, "two", 2.5, 5e-4 / (2 * 5000.0), "gaussian", 3, (8, 16, 32, 64)),
     Config("cfg4_1024x512x256", 1024, 512, 256, "one", 3.0, 5e-4 / (2 * 5000.0), "smooth", 4, (16, 32)),
     Config("cfg5_4096x288x512", 4096, 288, 512, "one", 3.0, 2e-4 / (2 * 20000.0), "smooth", 5, (16, 18)),
+    # not a BASELINE.json config: the grid of the paper's own ~607M flat-plate run, 3072 x 256 x 768 cells (PAPER.md:L182,
+    # L314) -- a factor 3 in x and z; cfg5's operator and right-hand side recipe.  `bench.py --config 6`.
+    Config("paper607_3072x256x768", 3072, 256, 768, "one", 3.0, 2e-4 / (2 * 20000.0), "smooth", 6, (16, 32)),
 )
 
 

@@ -489,7 +489,8 @@ tdx_status_t run_unit_tma(const Plan& pl, double* data, long long nlines, cudaSt
     UnitTmaArgs A;
     A.total_rows = nlines * pl.P * rpp;
     if (A.total_rows >= (1LL << 31)) return TDX_OK;
-    const int cap = 256 / rpp;                              // partitions per CTA: 32 KB of tile
+    static const int env_cap = [] { const char* e = std::getenv("TDX_TMA_CAP"); return e ? std::atoi(e) : 0; }();
+    const int cap = (env_cap > 0 ? env_cap : 256) / rpp;    // partitions per CTA: 32 KB of tile
     int lpb = cap / pl.P; if (lpb < 1) lpb = 1; if (lpb > nlines) lpb = (int)nlines;
     A.rows_per_cta = lpb * pl.P;
     const int tile_rows = A.rows_per_cta * rpp;

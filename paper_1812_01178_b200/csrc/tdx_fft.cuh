@@ -441,7 +441,7 @@ __global__ void __launch_bounds__(LP * N / K) k_dct_x(double* __restrict__ field
 // Decimation in time by 3: every thread runs the three M-point sub-transforms of its points side by side (8 points each)
 // and recombines them in registers (combine3); loads, stores and the pairing of the two real transforms are as above.
 template <int N, int C>
-__global__ void __launch_bounds__(C * N / 24) k_rfft_z3(const double* __restrict__ in, double2* __restrict__ out, int nx, int ny,
+__global__ void __launch_bounds__(C * N / 24, (C * N / 24 <= 256) ? 2 : 1) k_rfft_z3(const double* __restrict__ in, double2* __restrict__ out, int nx, int ny,
                                                          const double2* __restrict__ tw) {
     constexpr int K = 8, M = N / 3, T = M / K;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -487,7 +487,7 @@ __global__ void __launch_bounds__(C * N / 24) k_rfft_z3(const double* __restrict
 }
 
 template <int N, int C>
-__global__ void __launch_bounds__(C * N / 24) k_irfft_z3(const double2* __restrict__ in, double* __restrict__ out, int nx, int ny,
+__global__ void __launch_bounds__(C * N / 24, (C * N / 24 <= 256) ? 2 : 1) k_irfft_z3(const double2* __restrict__ in, double* __restrict__ out, int nx, int ny,
                                                           const double2* __restrict__ tw) {
     constexpr int K = 8, M = N / 3, T = M / K;
     extern __shared__ __align__(16) unsigned char smem_raw[];

@@ -1,4 +1,4 @@
-"""Parity at BASELINE.json's full sizes, in the launch configuration bench.py times (its TUNED_P, mode PPT and PDD):
+"""Parity at BASELINE.json's full sizes (configs 4 and 5; 6 is the paper's own 3072x256x768 grid, factor 3 in x and z), in the launch configuration bench.py times (its TUNED_P, mode PPT and PDD):
 the whole sweep runs on the GPU; randomly sampled lines are checked one by one against the oracle's single-line
 solvers (Thomas / cyclic Thomas on the oracle's own coefficients).  Tolerances as in test_gpu_parity.py; error norm =
 max over the sampled lines relative to the max of the sampled exact solutions (A14)."""
@@ -48,7 +48,7 @@ def _picks(rng, direction, nx, ny, nz):
     return p
 
 
-@pytest.mark.parametrize("cfg_no", [4, 5])
+@pytest.mark.parametrize("cfg_no", [4, 5, 6])
 @pytest.mark.parametrize("mode_name", ["ppt", "pdd"])
 def test_adi_sweeps_fullsize_sampled_lines(cfg_no, mode_name):
     c = configs.get(cfg_no)
@@ -112,7 +112,7 @@ def test_helmholtz_fullsize_sampled_lines(cfg_no):
     grid.close()
 
 
-@pytest.mark.parametrize("cfg_no", [4, 5])
+@pytest.mark.parametrize("cfg_no", [4, 5, 6])
 def test_transforms_and_poisson_fullsize_sampled(cfg_no):
     """SURVEY 8(f) N2 at the full sizes, in bench.py's launch configuration (TUNED_P_LINE, PPT): sampled x-lines of the
     cosine transform and sampled z-columns of the Fourier transform against the oracle's dense sums, the round trips on
