@@ -56,6 +56,8 @@ def parse():
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-step3", action="store_true", help="skip the extra 3-component staggered ADI step figure")
+    ap.add_argument("--slab", action="store_true", help="with --gpus N > 1: also time the y sweep of ONE field cut into y-slabs over the "
+                    "ranks (NCCL neighbour exchange / all-gather; SURVEY 8(f) N3).  At N = 1 the per-rank compute figure is always reported.")
     ap.add_argument("--psweep", default="", help="P sweep table (e.g. 8,16,32,64): per direction and mode, time, GB/s, PDD bound, "
                                                  "error of sampled lines vs the oracle; prints a markdown table, not the JSON line")
     ap.add_argument("--selftest-ranks", action="store_true",
@@ -431,6 +433,8 @@ def run_tdx(args, rank, world, local_rank):
         # world == 1: the compute part of an interior rank of a 4-rank job (a quarter slab; the exchange is a device copy);
         # world > 1: the real thing over NCCL (strong scaling of ONE field), max over ranks.
         try:
+            if world > 1 and not args.slab:
+                raise RuntimeError("skipped: pass --slab to time the NCCL slab sweep at N > 1")
             from paper_1812_01178_b200 import parallel
             Rk = world if world > 1 else 4
             rk = rank if world > 1 else 1
