@@ -182,7 +182,8 @@ tdx_status_t build_plan(tdx_grid* g, Plan& pl, const double* lambda_host, const 
         if (n % P == 0 && P >= 3 && nsets == 1 && !pl.wrap) {
             DevBuf differs; CUDA_TRY(differs.alloc(4));
             CUDA_TRY(cudaMemsetAsync(differs.p, 0, 4, st));
-            k_blocks_identical<<<(n + tb - 1) / tb, tb, 0, st>>>(n, P, a.as<double>(), b.as<double>(), c.as<double>(), differs.as<int>());
+            k_blocks_identical<<<(n + tb - 1) / tb, tb, 0, st>>>(n, P, a.as<double>(), b.as<double>(), c.as<double>(),
+                                                                  pl.kind == KIND_ADI ? 1e-13 : 0.0, differs.as<int>());
             LAUNCH_CHECK("k_blocks_identical");
             int h = 1;
             CUDA_TRY(cudaMemcpyAsync(&h, differs.p, 4, cudaMemcpyDeviceToHost, st));
