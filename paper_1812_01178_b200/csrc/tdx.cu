@@ -771,6 +771,7 @@ struct tdx_slab {
     long long inner = 0, outer = 0;
     std::vector<double> a, b, c;       // the slab's cut operator (host): user coefficients of the local plan
     double *v = nullptr, *w = nullptr, *coef = nullptr;   // device: spikes of this rank, interface coefficients
+    double* ylr = nullptr;             // device [2][plane]: interface unknowns of the current sweep
     double dropped = 0.0;              // max |v_last|, |w_first| over interior ranks: what PDD across ranks deletes
 };
 
@@ -1122,7 +1123,7 @@ tdx_status_t tdx_slab_create(tdx_grid_t* g, tdx_dir_t dir, int rank, int nranks,
     s->inner = inner; s->outer = outer;
     const int K = 2 * (nranks - 1);
     if (cudaMalloc(&s->v, (size_t)n_loc * 8) != cudaSuccess || cudaMalloc(&s->w, (size_t)n_loc * 8) != cudaSuccess ||
-        cudaMalloc(&s->coef, (size_t)std::max(4, 2 * K) * 8) != cudaSuccess) { cudaGetLastError(); return bail(fail(TDX_ERR_ALLOC, "device allocation failed")); }
+        cudaMalloc(&s->coef, (size_t)std::max(4, 2 * K) * 8) != cudaSuccess || cudaMalloc(&s->ylr, (size_t)2 * inner * outer * 8) != cudaSuccess) { cudaGetLastError(); return bail(fail(TDX_ERR_ALLOC, "device allocation failed")); }
     tdx::k_slab_spikes<<<(nranks + 31) / 32, 32>>>(nranks, dst.as<int>(), a.as<double>(), b.as<double>(), c.as<double>(), rank, nmax,
                                                     scratch.as<double>(), ends.as<double>(), s->v, s->w);
     g_launches.fetch_add(1);
@@ -1165,7 +1166,7 @@ tdx_status_t tdx_slab_create(tdx_grid_t* g, tdx_dir_t dir, int rank, int nranks,
 
 tdx_status_t tdx_slab_destroy(tdx_slab_t* s) {
     if (!s) return TDX_OK;
-    cudaFree(s->v); cudaFree(s->w); cudaFree(s->coef);
+    cudaFree(s->v); cudaFree(s->w); cudaFree(s->coef); cudaFree(s->ylr);
     delete s;
     return TDX_OK;
 }
@@ -1198,10 +1199,12 @@ tdx_status_t tdx_slab_correct(tdx_slab_t* s, double* field, const double* iface_
     const int JT = std::max(8, (s->n_loc + 7) / 8);
     dim3 block(128), grid((unsigned)((s->inner / 2 + 127) / 128), (s->n_loc + JT - 1) / JT, (unsigned)s->outer);
     if (s->outer > 65535) return fail(TDX_ERR_UNSUPPORTED, "outer extent > 65535");
-    if (s->across == TDX_MODE_PPT)
-        tdx::k_slab_correct<true><<<grid, block, 0, st>>>(field, iface_own, iface_nbr, s->coef, s->v, s->w, s->rank, s->R, s->n_loc, s->inner, s->outer, JT);
-    else
-        tdx::k_slab_correct<false><<<grid, block, 0, st>>>(field, iface_own, iface_nbr, s->coef, s->v, s->w, s->rank, s->R, s->n_loc, s->inner, s->outer, JT);
+    const long long plane = s->inner * s->outer;
+    const unsigned ib = (unsigned)((plane / 2 + 255) / 256);
+    if (s->across == TDX_MODE_PPT) tdx::k_slab_interface<true><<<ib, 256, 0, st>>>(iface_own, iface_nbr, s->coef, s->ylr, s->rank, s->R, plane);
+    else tdx::k_slab_interface<false><<<ib, 256, 0, st>>>(iface_own, iface_nbr, s->coef, s->ylr, s->rank, s->R, plane);
+    LAUNCH_CHECK("k_slab_interface");
+    tdx::k_slab_correct<<<grid, block, 0, st>>>(field, s->ylr, s->v, s->w, s->n_loc, s->inner, s->outer, JT);
     LAUNCH_CHECK("k_slab_correct");
     return TDX_OK;
 }
