@@ -5,6 +5,8 @@ they are not safely dominant (L172).  What such a solver must return has a plain
 so the oracle is that definition: every line's matrix is assembled densely and handed to LAPACK's general solver
 (numpy.linalg.solve: LU with partial pivoting, fp64).  Nothing of the GPU's pivoting strategy is restated here.
 Only tests/ may import this.  It imports nothing from paper_1812_01178_b200.
+Pinned by tests/test_oracle_general_pins.py (manufactured solutions through an independent mat-vec, the C Thomas on
+dominant systems, an exact rational zero-pivot system); nothing here is "parity unpinned".
 """
 import numpy as np
 

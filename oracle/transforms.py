@@ -10,6 +10,8 @@ Every transform here is its plain definition written out as a dense sum (a matri
 applied with a library matmul, fp64; arguments reduced exactly in integer arithmetic before cos/sin); nothing is blocked,
 factored or reordered.  Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
 import this.  It imports nothing from paper_1812_01178_b200 and shares no code or table with csrc/.
+Every function is pinned by tests/test_oracle_transform_pins.py (independent library FFTs, closed forms, eigen-relations
+with the second differences, manufactured Poisson solutions); nothing here is "parity unpinned".
 
 Readings (T1-T3):
   T1  half-range cosine transform of cell-centred values (pressure sits at cell centres, L41; Neumann walls):
