@@ -224,6 +224,63 @@ def run_reference(args, rank, world):
                       "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
 
 
+def grid_table(tdx, torch, cfg_no, local_rank, steps, peak):
+    """north_star: throughput on every BASELINE.json grid, per sweep direction, PPT and PDD, tuned P.  Fields that fit in
+    L2 (cfg1, cfg2) are rotated through enough distinct copies to exceed 2 x L2, and still flagged informational (the
+    launches are latency-bound there).  One event pair around each round of launches; Helmholtz right-hand sides are
+    restored between rounds (that solve is not a contraction)."""
+    cfg = configs.get(cfg_no)
+    Ps = TUNED_P[cfg_no]
+    bcs = (tdx.BC_DIRICHLET, tdx.BC_DIRICHLET, tdx.BC_PERIODIC)
+    grid = tdx.Grid(cfg.nx, cfg.ny, cfg.nz, *cfg.faces(), bcs=bcs, device=local_rank)
+    kz2 = cfg.kz2()
+    stream = torch.cuda.current_stream().cuda_stream
+    fbytes = cfg.npts * 8
+    K = 1 if fbytes > 2 * 126e6 else int(min(512, -(-2 * 126e6 // fbytes)))
+    f0 = torch.from_numpy(cfg.rhs_field()).cuda()
+    h0 = torch.from_numpy(cfg.rhs_helmholtz()).cuda()
+    fields = f0.unsqueeze(0).repeat(K, 1, 1, 1).contiguous()
+    helms = h0.unsqueeze(0).repeat(K, 1, 1, 1).contiguous()
+    names = ["adi_x", "adi_y", "adi_z_cyclic", "helmholtz_y"]
+    pts = [cfg.npts, cfg.npts, cfg.npts, 2 * cfg.nx * cfg.ny * cfg.nm]
+    out = {"grid": [cfg.nx, cfg.ny, cfg.nz], "points": cfg.npts, "copies_rotated": K,
+           "l2": "larger than L2" if K == 1 else "L2-resident field, %d copies rotated: GB/s informational" % K}
+    rounds = max(3, steps // 2)
+    for mname, mode in (("ppt", tdx.MODE_PPT), ("pdd", tdx.MODE_PDD)):
+        res = {}
+        for k, name in enumerate(names):
+            def launch(c):
+                if k < 3:
+                    grid.adi_sweep(k, mode, Ps[k], cfg.alpha, fields[c], stream)
+                else:
+                    grid.helmholtz_wavenumber_solve(mode, Ps[3], None, kz2, helms[c], stream)
+            for _ in range(3):
+                for c in range(K):
+                    launch(c)
+            tot = 0.0
+            for _ in range(rounds):
+                if k == 3:
+                    helms.copy_(h0.unsqueeze(0).expand_as(helms))
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                torch.cuda.synchronize()
+                e0.record()
+                for c in range(K):
+                    launch(c)
+                e1.record()
+                torch.cuda.synchronize()
+                tot += e0.elapsed_time(e1)
+            ms = tot / (rounds * K)
+            gbs = BYTES_PER_POINT * pts[k] / (ms * 1e-3) / 1e9
+            res[name] = {"ms": ms, "gpts_per_s": pts[k] / (ms * 1e-3) / 1e9, "gb_per_s": gbs, "frac_of_measured_peak": gbs / peak,
+                         "frac_of_nominal_8TBs": gbs / 8000.0, "P": Ps[k]}
+            if mname == "pdd" and k < 3:
+                res[name]["dropped_bound"] = grid.pdd_dropped_bound(k, Ps[k], cfg.alpha)
+        out[mname] = res
+    grid.close()
+    del fields, helms, f0, h0
+    return out
+
+
 def run_tdx(args, rank, world, local_rank):
     import torch
     from paper_1812_01178_b200 import binding as tdx
@@ -476,6 +533,16 @@ def run_tdx(args, rank, world, local_rank):
             del sfield
         except Exception as exc:                                 # an extra figure must never take the headline down
             out["slab_y_sweep"] = {"error": repr(exc)[:300]}
+
+    # north_star: "throughput on the five synthetic grids ... per sweep direction and as a fraction of the HBM roofline":
+    # the other BASELINE.json grids beside the headline one (same kernels, their own tuned P), rank 0 at N = 1 only.
+    if not args.no_step3 and world == 1:
+        try:
+            torch.cuda.empty_cache()
+            out["grids"] = {configs.get(c).name: grid_table(tdx, torch, c, local_rank, args.steps, peak)
+                            for c in (1, 2, 3, 4, 5) if c != args.config}
+        except Exception as exc:                                 # an extra figure must never take the headline down
+            out["grids"] = {"error": repr(exc)[:300]}
 
     # end to end through the host-buffer C-ABI calls: pinned host buffers, H2D + solve + D2H inside the timed region
     if not args.no_e2e:

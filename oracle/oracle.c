@@ -390,11 +390,85 @@ int oracle_partitioned_line(int n, int P, int mode, const double *a, const doubl
     return ORACLE_OK;
 }
 
-/* Cyclic line with partitions: outer Sherman-Morrison; y = A'^{-1} d by the partitioned solve of the given
- * mode; q = A'^{-1} u is matrix-only and is solved exactly by Thomas (reading on cyclic+PDD). */
+/* ---------------------------------------------------------------------------------------------
+ * PDD on a periodic line (reading A16; SURVEY 8(c) C2 "close the reduced system cyclically, P
+ * interfaces").  The split A = A~ + dA of PAPER.md:L78-91 now also moves the two wrap-around corners into dA:
+ * a_0 at (0, n-1) and c_{n-1} at (n-1, 0), so there are P interfaces, interface i (0 <= i < P) lying between
+ * partitions (i-1) mod P and i, and every partition p has both spikes (Eq.(6)):
+ *     v^(p) = A_p^{-1}(a_first e_first),   w^(p) = A_p^{-1}(c_last e_last).
+ * The exact interface rows read (indices of partitions mod P; s_i = x_{last_{i-1}}, t_i = x_{first_i}):
+ *     v_last^(i-1) s_{i-1} + s_i + w_last^(i-1) t_i     = xt_{last_{i-1}}
+ *     v_first^(i)  s_i     + t_i + w_first^(i)  t_{i+1} = xt_{first_i}
+ * PDD (L148-154) deletes the far spike ends v_last, w_first, which leaves P blocks [[1, w_last^(i-1)],[v_first^(i), 1]]
+ * solved by the explicit inverse (Algorithm 1 step 5, L252-254); Eq.(8): x^(p) = xt^(p) - v^(p) s_p - w^(p) t_{p+1}.
+ * spikes (optional, 2n doubles) returns v then w.
+ * ------------------------------------------------------------------------------------------- */
+int oracle_cyclic_pdd_line(int n, int P, const double *a, const double *b, const double *c,
+                           const double *d, double *x, double *spikes) {
+    if (P < 2 || n < 3) return ORACLE_ERR;
+    int *st = (int *)malloc(sizeof(int) * (P + 1));
+    if (oracle_partition_bounds(n, P, st) != ORACLE_OK) { free(st); return ORACLE_ERR; }
+    double *xt = (double *)malloc(sizeof(double) * (3 * n + 2 * P)), *v = xt + n, *w = xt + 2 * n, *sv = xt + 3 * n, *tv = sv + P;
+    for (int p = 0; p < P; ++p) {
+        int s = st[p], m = st[p + 1] - st[p];
+        double *aa = (double *)malloc(sizeof(double) * m * 3), *cc = aa + m, *e = aa + 2 * m;
+        memcpy(aa, a + s, sizeof(double) * m); memcpy(cc, c + s, sizeof(double) * m);
+        aa[0] = 0.0; cc[m - 1] = 0.0;                                   /* A_p: Alg.1 step 2, wrap corners included */
+        oracle_thomas(m, aa, b + s, cc, d + s, xt + s);                 /* Eq.(5) */
+        memset(e, 0, sizeof(double) * m); e[0] = a[s];
+        oracle_thomas(m, aa, b + s, cc, e, v + s);                      /* Eq.(6), a-corner (a[0] couples to row n-1) */
+        memset(e, 0, sizeof(double) * m); e[m - 1] = c[s + m - 1];
+        oracle_thomas(m, aa, b + s, cc, e, w + s);                      /* Eq.(6), c-corner (c[n-1] couples to row 0) */
+        free(aa);
+    }
+    for (int i = 0; i < P; ++i) {                                       /* Alg.1 step 5 on each of the P interfaces */
+        int pm = (i + P - 1) % P;
+        int last = st[pm + 1] - 1, first = st[i];
+        double wl = w[last], vf = v[first];
+        double det = 1.0 - wl * vf;
+        sv[i] = (xt[last] - wl * xt[first]) / det;
+        tv[i] = (xt[first] - vf * xt[last]) / det;
+    }
+    if (spikes) { memcpy(spikes, v, sizeof(double) * n); memcpy(spikes + n, w, sizeof(double) * n); }
+    for (int p = 0; p < P; ++p) {                                       /* Eq.(8) / Alg.1 step 7 */
+        double yl = sv[p], yr = tv[(p + 1) % P];
+        for (int j = st[p]; j < st[p + 1]; ++j) x[j] = xt[j] - v[j] * yl - w[j] * yr;
+    }
+    free(xt); free(st);
+    return ORACLE_OK;
+}
+
+/* a-priori bound of the cyclically closed PDD: max over ALL partitions of |v_last^(p)|, |w_first^(p)|. */
+double oracle_cyclic_pdd_dropped(int n, int P, const double *a, const double *b, const double *c) {
+    if (P < 2) return 0.0;
+    double *wk = (double *)malloc(sizeof(double) * n * 4), *d0 = wk, *x0 = wk + n, *sp = wk + 2 * n;
+    int *st = (int *)malloc(sizeof(int) * (P + 1));
+    double dr = -1.0;
+    memset(d0, 0, sizeof(double) * n);
+    if (oracle_partition_bounds(n, P, st) == ORACLE_OK && oracle_cyclic_pdd_line(n, P, a, b, c, d0, x0, sp) == ORACLE_OK) {
+        dr = 0.0;
+        for (int p = 0; p < P; ++p) {
+            double vl = fabs(sp[st[p + 1] - 1]), wf = fabs(sp[n + st[p]]);
+            if (vl > dr) dr = vl;
+            if (wf > dr) dr = wf;
+        }
+    }
+    free(wk); free(st);
+    return dr;
+}
+
+/* Cyclic line with partitions.  PDD: the cyclically closed reduced system above.  PPT (exact in either form):
+ * outer Sherman-Morrison; y = A'^{-1} d by the partitioned solve, q = A'^{-1} u by Thomas. */
 int oracle_cyclic_line(int n, int P, int mode, const double *a, const double *b, const double *c,
                        const double *d, double *x) {
     if (mode == MODE_THOMAS || P == 1) return oracle_cyclic_thomas(n, a, b, c, d, x);
+    if (mode == MODE_PDD) {
+        double *dd = (double *)malloc(sizeof(double) * n);
+        memcpy(dd, d, sizeof(double) * n);                               /* x may alias d */
+        int rc = oracle_cyclic_pdd_line(n, P, a, b, c, dd, x, NULL);
+        free(dd);
+        return rc;
+    }
     double *wk = (double *)malloc(sizeof(double) * n * 6);
     double *a2 = wk, *b2 = wk + n, *c2 = wk + 2 * n, *u = wk + 3 * n, *y = wk + 4 * n, *q = wk + 5 * n, g;
     cyclic_split(n, a, b, c, a2, b2, c2, u, &g);

@@ -37,6 +37,7 @@ def _chk(rc, what):
 
 
 _lib.oracle_pdd_dropped.restype = C.c_double
+_lib.oracle_cyclic_pdd_dropped.restype = C.c_double
 _lib.oracle_pdd_dropped.argtypes = [C.c_int, C.c_int, _dp, _dp, _dp]
 
 
@@ -134,6 +135,21 @@ def build_Zbar(Z):
 def pdd_dropped(P, a, b, c):
     a, b, c = _c(a), _c(b), _c(c)
     return float(_lib.oracle_pdd_dropped(C.c_int(b.size), C.c_int(P), _p(a), _p(b), _p(c)))
+
+
+def cyclic_pdd_dropped(P, a, b, c):
+    """a-priori bound of PDD on a periodic line (reduced system closed cyclically): every partition's far spike ends."""
+    a, b, c = _c(a), _c(b), _c(c)
+    return float(_lib.oracle_cyclic_pdd_dropped(C.c_int(b.size), C.c_int(P), _p(a), _p(b), _p(c)))
+
+
+def cyclic_pdd_line(P, a, b, c, d, return_spikes=False):
+    """PDD on one periodic line, P interfaces (oracle_cyclic_pdd_line); optionally the spikes v, w (each length n)."""
+    a, b, c, d = _c(a), _c(b), _c(c), _c(d)
+    x = np.empty_like(d)
+    sp = np.zeros(2 * d.size)
+    _chk(_lib.oracle_cyclic_pdd_line(C.c_int(d.size), C.c_int(P), _p(a), _p(b), _p(c), _p(d), _p(x), _p(sp)), "cyclic_pdd_line")
+    return (x, sp[:d.size].copy(), sp[d.size:].copy()) if return_spikes else x
 
 
 def partitioned_line(P, mode, a, b, c, d, return_y=False):

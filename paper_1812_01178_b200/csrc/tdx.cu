@@ -60,7 +60,7 @@ struct Plan {
     int layout = tdx::ROWS_PJ;
     int KB = 0, Scap = 0;
     bool cyc = false, thomas = false;
-    bool wrap = false;      // periodic line closed inside the reduced system (PPT, P <= 128) instead of Sherman-Morrison
+    bool wrap = false;      // periodic line closed inside the reduced system (PDD; PPT with P <= 128) instead of Sherman-Morrison
     int sms = 148;          // SM count of the grid's device
     mutable int pf = -1;    // L2 prefetch distance of the sweep kernel (CTAs), set at first launch
     mutable CUtensorMap tmap;             // x sweeps: tensor map of the field as [lines*P, M] partition rows
@@ -204,7 +204,10 @@ tdx_status_t build_plan(tdx_grid* g, Plan& pl, const double* lambda_host, const 
     CUDA_TRY(cudaMalloc(&pl.G, (size_t)nsets * 2 * pl.KB * P * 8));
     CUDA_TRY(cudaMalloc(&pl.band, (size_t)nsets * P * sizeof(int2)));
     const int ntp = nsets * P;
-    if (pl.mode == TDX_MODE_PDD) {
+    if (pl.mode == TDX_MODE_PDD && pl.wrap) {
+        k_pack_pdd_cyclic<<<(ntp + tb - 1) / tb, tb, 0, st>>>(nsets, P, pl.KB, ends.as<double>(), pl.G, pl.band);
+        LAUNCH_CHECK("k_pack_pdd_cyclic");
+    } else if (pl.mode == TDX_MODE_PDD) {
         k_pack_pdd<<<(ntp + tb - 1) / tb, tb, 0, st>>>(nsets, P, pl.KB, ends.as<double>(), pl.G, pl.band);
         LAUNCH_CHECK("k_pack_pdd");
     } else if (pl.wrap) {
@@ -246,11 +249,17 @@ tdx_status_t build_plan(tdx_grid* g, Plan& pl, const double* lambda_host, const 
     CUDA_TRY(cudaMemcpyAsync(he.data(), ends.p, he.size() * 8, cudaMemcpyDeviceToHost, st));
     CUDA_TRY(cudaStreamSynchronize(st));
     double dr = 0.0;
-    for (int s = 0; s < nsets; ++s)
+    for (int s = 0; s < nsets; ++s) {
+        if (pl.wrap) {                                              // cyclic reduced system: v_last, w_first of every partition
+            for (int p = 0; p < P; ++p)
+                dr = std::max(dr, std::max(std::fabs(he[((size_t)s * P + p) * 4 + 1]), std::fabs(he[((size_t)s * P + p) * 4 + 2])));
+            continue;
+        }
         for (int i = 1; i <= P - 1; ++i) {
             if (i >= 2) dr = std::max(dr, std::fabs(he[((size_t)s * P + i - 1) * 4 + 1]));
             if (i <= P - 2) dr = std::max(dr, std::fabs(he[((size_t)s * P + i) * 4 + 2]));
         }
+    }
     pl.dropped = dr;
     return TDX_OK;
 }
@@ -268,8 +277,10 @@ tdx_status_t get_plan(tdx_grid* g, int kind, int dir, int mode, int P, double al
     if (thomas) { P = 1; mode = TDX_MODE_THOMAS; }
     const bool periodic = (kind == KIND_USER) || (kind == KIND_ADI && g->bc[dir] == TDX_BC_PERIODIC);
     if (periodic && n < 3) return fail(TDX_ERR_INVALID_ARG, "periodic line needs n >= 3");
-    // PPT closes a periodic line inside the (then cyclic) reduced system; PDD and Thomas use Sherman-Morrison (Eq.(3), rank 1)
-    const bool wrap = periodic && !thomas && mode == TDX_MODE_PPT && P >= 2 && P <= 128;
+    // PDD and PPT close a periodic line inside the (then cyclic) reduced system: the wrap corners join Delta A, P interfaces
+    // (Eq.(3)-(4) with rank 2P; PPT needs the dense 2P x 2P inverse at plan time, hence P <= 128).  Thomas, and PPT with
+    // more partitions, use the rank-1 Sherman-Morrison split.
+    const bool wrap = periodic && !thomas && P >= 2 && (mode == TDX_MODE_PDD || P <= 128);
     const bool cyc = periodic && !wrap;
     int M = 0;
     if (!thomas) {

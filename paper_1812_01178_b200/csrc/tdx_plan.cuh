@@ -463,6 +463,36 @@ __global__ void k_pack_pdd(int nsets, int P, int KB, const double* __restrict__ 
     }
 }
 
+// PDD on a periodic line (the reduced system closed cyclically, as k_reduced_cyclic_factor does for PPT): the wrap
+// corners a_0, c_{n-1} join Delta A, so there are P interfaces -- interface i between partitions
+// (i-1) mod P and i -- and PDD (L148-154) deletes v_last^(p), w_first^(p) of EVERY partition, leaving P 2x2 blocks
+// [[1, w_last^(i-1)],[v_first^(i), 1]].  Partition p needs yL = x_last_{p-1} (interface p) and yR = x_first_{p+1}
+// (interface p+1), indices mod P.  band = cyclic window r[(2p-1) mod K .. (2p+2) mod K], K = 2P.
+__global__ void k_pack_pdd_cyclic(int nsets, int P, int KB, const double* __restrict__ ends, double* __restrict__ G, int2* __restrict__ band) {
+    int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= nsets * P) return;
+    int s = t / P, p = t % P;
+    const int K = 2 * P;
+    const double* e = ends + (size_t)s * P * 4;
+    const int pm = (p - 1 + P) % P, pp = (p + 1) % P;
+    double g[2][4] = {{0, 0, 0, 0}, {0, 0, 0, 0}};          // over r[2p-1] = xt_last^(p-1), r[2p], r[2p+1], r[2p+2] = xt_first^(p+1)
+    {
+        const double wl = e[pm * 4 + 3], vf = e[p * 4 + 0];
+        const double det = 1.0 - wl * vf;
+        g[0][0] = 1.0 / det; g[0][1] = -wl / det;
+    }
+    {
+        const double wl = e[p * 4 + 3], vf = e[pp * 4 + 0];
+        const double det = 1.0 - wl * vf;
+        g[1][2] = -vf / det; g[1][3] = 1.0 / det;
+    }
+    band[t] = make_int2((2 * p - 1 + K) % K, 4);
+    for (int k = 0; k < KB; ++k) {
+        G[g_index(s, 0, k, p, KB, P)] = k < 4 ? g[0][k] : 0.0;
+        G[g_index(s, 1, k, p, KB, P)] = k < 4 ? g[1][k] : 0.0;
+    }
+}
+
 // a5: the Sherman-Morrison scalar s = kappa (y_0 + g y_{n-1}) as a sparse linear functional of r, where y is the
 // partitioned solution of A' y = d:  y_0 = r[0] - w_first^(0) yR_0,  y_{n-1} = r[2P-1] - v_last^(P-1) yL_{P-1}.
 // Sidx/Sval[set*Scap + k], Sn[set]; Scap >= 2 + 2*KB.

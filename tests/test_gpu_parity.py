@@ -37,11 +37,10 @@ def check_sweep(grid, faces, bcs, field, direction, mode_name, P, alpha):
     if mode_name == "pdd":
         f = faces[direction]
         a, b, c = orc.adi_coeffs(f, bcs[direction], alpha)
-        if bcs[direction] == orc.BC_PERIODIC:                   # PDD acts on the Sherman-Morrison split matrix A'
-            g = a[0] / -b[0]
-            b = b.copy(); b[0] = 2 * b[0]; b[-1] = b[-1] - c[-1] * g
-            a = a.copy(); c = c.copy(); a[0] = 0.0; c[-1] = 0.0
-        dropped = orc.pdd_dropped(P, a, b, c)
+        if bcs[direction] == orc.BC_PERIODIC:                   # reduced system closed cyclically: P interfaces (A16)
+            dropped = orc.cyclic_pdd_dropped(P, a, b, c)
+        else:
+            dropped = orc.pdd_dropped(P, a, b, c)
         assert abs(grid.pdd_dropped_bound(direction, P, alpha) - dropped) <= 1e-10 * dropped + 1e-300
         ref_pdd = orc.adi_sweep(field.copy(), *faces, bcs, direction, orc.MODE_PDD, P, alpha)
         assert relerr(out, ref_pdd) < TOL_EXACT, ("pdd vs oracle pdd", direction, P, relerr(out, ref_pdd))

@@ -195,6 +195,69 @@ def test_cyclic_line_with_partitions(mode):
     assert relerr(orc.cyclic_thomas(a, b, c, d), ref) < 1e-14
 
 
+def cyclic_pdd_dense_reference(P, a, b, c, d):
+    """Independent restatement with dense LAPACK algebra: Woodbury (Eq.(3)-(4)) with the wrap corners in dA, the far
+    spike ends deleted from Z = I + E^T A~^{-1} V (L148-154), everything else exact."""
+    n = b.size
+    st = orc.partition_bounds(n, P)
+    A = orc.dense_from_tridiag(a, b, c, cyclic=True)
+    At = np.zeros_like(A)
+    for p in range(P):
+        At[st[p]:st[p + 1], st[p]:st[p + 1]] = A[st[p]:st[p + 1], st[p]:st[p + 1]]
+    dA = A - At                                              # the 2P corner entries
+    cols, V = [], []
+    for i in range(P):                                       # interface i: rows last_{i-1}, first_i
+        last, first = st[(i - 1) % P + 1] - 1, st[i]
+        cols += [last, first]
+        ea = np.zeros(n); ea[first] = dA[first, last]; ec = np.zeros(n); ec[last] = dA[last, first]
+        V += [ea, ec]                                        # column of V multiplying x_last, then x_first
+    E = np.zeros((n, 2 * P)); E[cols, np.arange(2 * P)] = 1.0
+    V = np.array(V).T
+    assert np.allclose(V @ E.T, dA, atol=0, rtol=0)
+    Y = np.linalg.solve(At, V)
+    Z = np.eye(2 * P) + E.T @ Y
+    Zp = np.zeros_like(Z)
+    for i in range(P):                                       # keep only the 2x2 diagonal blocks
+        Zp[2 * i:2 * i + 2, 2 * i:2 * i + 2] = Z[2 * i:2 * i + 2, 2 * i:2 * i + 2]
+    xt = np.linalg.solve(At, d)
+    y = np.linalg.solve(Zp, E.T @ xt)
+    return xt - Y @ y, float(np.max(np.abs(Z - Zp)))
+
+
+@pytest.mark.parametrize("n,P,margin", [(64, 4, 6.0), (60, 2, 0.3), (37, 5, 0.05), (96, 8, 0.01)])
+def test_cyclic_pdd_matches_dense_woodbury_with_far_ends_deleted(n, P, margin):
+    a = rng.uniform(-1, -0.2, n); c = rng.uniform(-1, -0.2, n); b = margin - a - c
+    d = rng.uniform(-1, 1, n)
+    ref, dropped = cyclic_pdd_dense_reference(P, a, b, c, d)
+    x = orc.cyclic_pdd_line(P, a, b, c, d)
+    assert relerr(x, ref) < 1e-12
+    assert abs(orc.cyclic_pdd_dropped(P, a, b, c) - dropped) <= 1e-12 * dropped + 1e-300
+    assert np.array_equal(orc.cyclic_line(P, orc.MODE_PDD, a, b, c, d), x)
+    exact = np.linalg.solve(orc.dense_from_tridiag(a, b, c, cyclic=True), d)
+    assert relerr(x, exact) <= 50 * dropped + 1e-13, (relerr(x, exact), dropped)
+    if dropped > 1e-6:                                       # and it IS an approximation when the spikes have not decayed
+        assert relerr(x, exact) > 1e-3 * dropped
+
+
+def test_cyclic_pdd_spikes_and_exactness_when_decayed():
+    n, P = 48, 4
+    a = rng.uniform(-1, 0, n); c = rng.uniform(-1, 0, n); b = 1.0 - a - c + 60.0
+    d = rng.uniform(-1, 1, n)
+    x, v, w = orc.cyclic_pdd_line(P, a, b, c, d, return_spikes=True)
+    st = orc.partition_bounds(n, P)
+    for p in range(P):                                       # Eq.(6): A_p v = a_first e_first, A_p w = c_last e_last, every partition
+        s, e = st[p], st[p + 1]
+        Ap = orc.dense_from_tridiag(a[s:e], b[s:e], c[s:e])
+        rv = np.zeros(e - s); rv[0] = a[s]; rw = np.zeros(e - s); rw[-1] = c[e - 1]
+        assert np.max(np.abs(Ap @ v[s:e] - rv)) < 1e-13 and np.max(np.abs(Ap @ w[s:e] - rw)) < 1e-13
+    assert orc.cyclic_pdd_dropped(P, a, b, c) < 1e-17
+    assert relerr(x, orc.cyclic_thomas(a, b, c, d)) < 1e-14
+    assert relerr(x, orc.cyclic_line(P, orc.MODE_PPT, a, b, c, d)) < 1e-14
+    # identity operator: bit-exact
+    z = np.zeros(n)
+    assert np.array_equal(orc.cyclic_pdd_line(P, z, np.ones(n), z, d), d)
+
+
 # ---------------------------------------------------------------- 3-D sweeps
 def sweep_reference(field, a, b, c, axis, cyclic):
     """independent: move the axis last and solve every line with LAPACK."""
@@ -217,7 +280,11 @@ def test_adi_sweep_every_direction_vs_lapack(direction, mode, P):
     a, b, c = orc.adi_coeffs(f, bcs[direction], alpha)
     ref = sweep_reference(field, a, b, c, axis=2 - direction, cyclic=(direction == 2))
     out = orc.adi_sweep(field.copy(), xf, yf, zf, bcs, direction, mode, P, alpha)
-    assert relerr(out, ref) < 1e-13
+    tol = 1e-13
+    if mode == orc.MODE_PDD and direction == 2:             # periodic + PDD: P interfaces, an approximation even at P = 2
+        tol += 50 * orc.cyclic_pdd_dropped(P, a, b, c)
+        assert tol < 1e-2
+    assert relerr(out, ref) < tol
 
 
 def test_sweep_one_hot_touches_only_its_line():
@@ -271,4 +338,5 @@ def test_cyclic_solve_user_coefficients():
     ref = sweep_reference(field, a, b, c, axis=0, cyclic=True)
     for mode, P in [(orc.MODE_THOMAS, 1), (orc.MODE_PPT, 3), (orc.MODE_PDD, 2)]:
         out = orc.cyclic_solve(field.copy(), 2, mode, P, a, b, c)
-        assert relerr(out, ref) < 1e-13
+        tol = 1e-13 + (50 * orc.cyclic_pdd_dropped(P, a, b, c) if mode == orc.MODE_PDD else 0.0)   # PDD: P interfaces, approximate
+        assert relerr(out, ref) < tol < 1e-2
