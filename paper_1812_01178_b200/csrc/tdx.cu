@@ -176,20 +176,21 @@ tdx_status_t build_plan(tdx_grid* g, Plan& pl, const double* lambda_host, const 
         return TDX_OK;
     }
     // partitioned modes
-    pl.layout = ROWS_PJ;
-    if (pl.dir == 0) {
-        pl.layout = ROWS_JP;
-        if (n % P == 0 && P >= 3 && nsets == 1 && !pl.wrap) {
-            DevBuf differs; CUDA_TRY(differs.alloc(4));
-            CUDA_TRY(cudaMemsetAsync(differs.p, 0, 4, st));
-            k_blocks_identical<<<(n + tb - 1) / tb, tb, 0, st>>>(n, P, a.as<double>(), b.as<double>(), c.as<double>(),
-                                                                  pl.kind == KIND_ADI ? 1e-13 : 0.0, differs.as<int>());
-            LAUNCH_CHECK("k_blocks_identical");
-            int h = 1;
-            CUDA_TRY(cudaMemcpyAsync(&h, differs.p, 4, cudaMemcpyDeviceToHost, st));
-            CUDA_TRY(cudaStreamSynchronize(st));
-            if (h == 0) pl.layout = ROWS_U;
-        }
+    pl.layout = (pl.dir == 0) ? ROWS_JP : ROWS_PJ;
+    // One table for every partition when all blocks are identical (uniform grid): x lines (Dirichlet ends, P >= 3: partition
+    // 1 has both neighbours), and strided lines of the instantiated sizes; a periodic line closed inside the reduced system
+    // (wrap) qualifies from P = 2, every partition having both neighbours.
+    const bool uni_shape = (pl.dir == 0) ? !pl.wrap : (pl.M == 8 || pl.M == 16 || pl.M == 32);
+    if (n % P == 0 && nsets == 1 && !pl.cyc && uni_shape && (pl.wrap ? P >= 2 : P >= 3) && pl.kind != KIND_HELM) {
+        DevBuf differs; CUDA_TRY(differs.alloc(4));
+        CUDA_TRY(cudaMemsetAsync(differs.p, 0, 4, st));
+        k_blocks_identical<<<(n + tb - 1) / tb, tb, 0, st>>>(n, P, pl.wrap ? 1 : 0, a.as<double>(), b.as<double>(), c.as<double>(),
+                                                              pl.kind == KIND_ADI ? 1e-13 : 0.0, differs.as<int>());
+        LAUNCH_CHECK("k_blocks_identical");
+        int h = 1;
+        CUDA_TRY(cudaMemcpyAsync(&h, differs.p, 4, cudaMemcpyDeviceToHost, st));
+        CUDA_TRY(cudaStreamSynchronize(st));
+        if (h == 0) pl.layout = ROWS_U;
     }
     const size_t rows_elems = (pl.layout == ROWS_U) ? (size_t)pl.M * 6 : (size_t)nsets * P * pl.M * 6;
     CUDA_TRY(cudaMalloc(&pl.rows, rows_elems * 8));
@@ -317,21 +318,30 @@ Tables tables_of(const Plan& pl) {
 // ---- launch selection ---------------------------------------------------------------------------------------
 namespace {
 
-template <int M, int V, bool CYC>
+template <int M, int V, bool CYC, bool UNI = false>
 tdx_status_t launch_strided_inst(const Plan& pl, StridedArgs& A, const Tables& T, dim3 grid, dim3 block, size_t smem, cudaStream_t st) {
     static bool attr_done = false;
     if (!attr_done && smem > 48 * 1024) {
-        CUDA_TRY(cudaFuncSetAttribute(k_strided<M, V, CYC>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+        CUDA_TRY(cudaFuncSetAttribute(k_strided<M, V, CYC, UNI>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
         attr_done = true;
     }
     if (pl.pf < 0) {                                               // prefetch one wave of resident CTAs ahead
         int occ = 1;
-        CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_strided<M, V, CYC>, (int)(block.x * block.y), smem));
+        CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_strided<M, V, CYC, UNI>, (int)(block.x * block.y), smem));
         pl.pf = pl.sms * (occ < 1 ? 1 : occ) * prefetch_waves();
     }
     // one tile per CTA: pf = CTAs ahead; looping CTAs (grid.x < tiles_x): pf = sets ahead for the first tile of a later CTA
     A.pf = ((int)grid.x == A.tiles_x) ? pl.pf : (pl.pf > 0 ? (pl.pf + (int)grid.x - 1) / (int)grid.x : 0);
-    k_strided<M, V, CYC><<<grid, block, smem, st>>>(A, T);
+    UniTable<UNI ? M : 1> U;
+    if (UNI) {
+        if (!pl.uni_host_ok) {
+            CUDA_TRY(cudaMemcpyAsync(pl.uni_host, pl.rows, sizeof(double) * M * 6, cudaMemcpyDeviceToHost, st));
+            CUDA_TRY(cudaStreamSynchronize(st));
+            pl.uni_host_ok = true;
+        }
+        std::memcpy(U.v, pl.uni_host, sizeof(U.v));
+    } else std::memset(U.v, 0, sizeof(U.v));
+    k_strided<M, V, CYC, UNI><<<grid, block, smem, st>>>(A, T, U);
     LAUNCH_CHECK("k_strided");
     return TDX_OK;
 }
@@ -339,6 +349,16 @@ tdx_status_t launch_strided_inst(const Plan& pl, StridedArgs& A, const Tables& T
 template <int V, bool CYC>
 tdx_status_t launch_strided_M(const Plan& pl, StridedArgs& A, const Tables& T, dim3 grid, dim3 block, size_t smem, cudaStream_t st) {
     const int M = pl.M;
+    if (pl.layout == ROWS_U) {                                     // only set for the sizes instantiated here (build_plan)
+        if (CYC) return fail(TDX_ERR_UNSUPPORTED, "uniform table with the rank-1 periodic closure");
+        switch (M) {
+            case 8: return launch_strided_inst<8, V, false, true>(pl, A, T, grid, block, smem, st);
+            case 16: return launch_strided_inst<16, V, false, true>(pl, A, T, grid, block, smem, st);
+            case 32: if (V == 2) return launch_strided_inst<32, 2, false, true>(pl, A, T, grid, block, smem, st);
+                     return launch_strided_inst<32, 1, false, true>(pl, A, T, grid, block, smem, st);
+        }
+        return fail(TDX_ERR_UNSUPPORTED, "no uniform-table strided kernel for M=%d", M);
+    }
     switch (M) {
         case 4: return launch_strided_inst<4, V, CYC>(pl, A, T, grid, block, smem, st);
         case 8: return launch_strided_inst<8, V, CYC>(pl, A, T, grid, block, smem, st);

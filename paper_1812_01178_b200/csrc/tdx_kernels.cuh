@@ -61,9 +61,15 @@ constexpr int strided_block_threads(int MAXM, int V) {            // largest CTA
     return (65536 / strided_regs(MAXM, V)) / 32 * 32 > 1024 ? 1024 : (65536 / strided_regs(MAXM, V)) / 32 * 32;
 }
 
-template <int MAXM, int V, bool CYC>
+// A row table shared by every partition (uniform grid: all blocks A_p identical) travels as a kernel parameter: with the
+// row loops fully unrolled every table value is a constant-bank operand of its DFMA -- no load instruction, no L1
+// wavefront, no register holding a table value in flight.
+template <int M> struct UniTable { double v[M * 6]; };
+
+// UNI: row table = U.v[jj*6 + f] for every partition (ROWS_U plans: periodic or interior-identical blocks, one set).
+template <int MAXM, int V, bool CYC, bool UNI>
 __global__ void __maxnreg__(strided_regs(MAXM, V))
-k_strided(StridedArgs A, Tables T) {
+k_strided(StridedArgs A, Tables T, const __grid_constant__ UniTable<UNI ? MAXM : 1> U) {
     extern __shared__ double rs[];                          // rs[(idx*LPC + tx)*V + v], idx in [0, 2P)
     const int tx = threadIdx.x, p = threadIdx.y;
     const int LPC = A.LPC, P = T.P;
@@ -127,18 +133,18 @@ k_strided(StridedArgs A, Tables T) {
     // Eq.(5): forward y_j = d_j - l_j y_{j-1}, backward xt_j = y_j inv_j - cp_j xt_{j+1}
 #pragma unroll
     for (int jj = 1; jj < MAXM; ++jj) {
-        const double l = __ldg(reinterpret_cast<const double*>(&rt[jj * 3 + 0]));
+        const double l = UNI ? U.v[UNI ? jj * 6 + F_L : 0] : __ldg(reinterpret_cast<const double*>(&rt[jj * 3 + 0]));
 #pragma unroll
         for (int v = 0; v < V; ++v) x[jj][v] = fma(-l, x[jj - 1][v], x[jj][v]);
     }
     {
-        const double inv = __ldg(reinterpret_cast<const double*>(&rt[(MAXM - 1) * 3 + 1]));
+        const double inv = UNI ? U.v[UNI ? (MAXM - 1) * 6 + F_INV : 0] : __ldg(reinterpret_cast<const double*>(&rt[(MAXM - 1) * 3 + 1]));
 #pragma unroll
         for (int v = 0; v < V; ++v) x[MAXM - 1][v] *= inv;
     }
 #pragma unroll
     for (int jj = MAXM - 2; jj >= 0; --jj) {
-        const double2 ic = __ldg(&rt[jj * 3 + 1]);          // {inv, cp}
+        const double2 ic = UNI ? make_double2(U.v[UNI ? jj * 6 + F_INV : 0], U.v[UNI ? jj * 6 + F_CP : 0]) : __ldg(&rt[jj * 3 + 1]);   // {inv, cp}
 #pragma unroll
         for (int v = 0; v < V; ++v) x[jj][v] = fma(-ic.y, x[jj + 1][v], x[jj][v] * ic.x);
     }
@@ -181,7 +187,7 @@ k_strided(StridedArgs A, Tables T) {
     // Eq.(8): x = xt - v yL - w yR (- q s for periodic lines), then store
 #pragma unroll
     for (int jj = 0; jj < MAXM; ++jj) {
-        const double2 vw = __ldg(&rt[jj * 3 + 2]);          // {v, w}
+        const double2 vw = UNI ? make_double2(U.v[UNI ? jj * 6 + F_V : 0], U.v[UNI ? jj * 6 + F_W : 0]) : __ldg(&rt[jj * 3 + 2]);     // {v, w}
         double qj = 0.0;
         if (CYC) qj = __ldg(reinterpret_cast<const double*>(&rt[jj * 3 + 0]) + 1);   // {l, q}
 #pragma unroll

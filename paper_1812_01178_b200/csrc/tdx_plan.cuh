@@ -226,19 +226,23 @@ __global__ void k_factor_line(int n, int nsets, const double* __restrict__ a, co
 // by rounding, f_j = L j / N, so the blocks differ in the 12th digit; since an ADI row has |b| = |a| + |c| + 1
 // (PAPER.md:L162), ||A^-1|| <= 1 and replacing every block by block 0 changes the solution by at most tol relative --
 // 1e-13 against the 1e-12 gate.
-__global__ void k_blocks_identical(int n, int P, const double* __restrict__ a, const double* __restrict__ b,
+// wrap: periodic line closed inside the reduced system -- a_0 and c_{n-1} are spike right-hand sides like the others.
+__global__ void k_blocks_identical(int n, int P, int wrap, const double* __restrict__ a, const double* __restrict__ b,
                                    const double* __restrict__ c, double tol, int* __restrict__ differs) {
     int j = blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= n) return;
     int m = n / P;                       // only called when n % P == 0
     int p = j / m, jj = j % m;
-    if (p == 0) return;
     bool first = (jj == 0), last = (jj == m - 1);
+    if (p == 0) {
+        if (wrap && first && !(fabs(a[0] - a[m]) <= tol)) atomicExch(differs, 1);
+        return;
+    }
     // a_first and c_last are zeroed inside every block (Alg.1 step 2), so they do not take part in the comparison
     double diff = fabs(b[j] - b[jj]) + (first ? 0.0 : fabs(a[j] - a[jj])) + (last ? 0.0 : fabs(c[j] - c[jj]));
     // the spikes' right-hand sides: a_first of p>=1 blocks and c_last of p<=P-2 blocks must agree among themselves
     if (first && p > 1) diff += fabs(a[j] - a[m]);
-    if (last && p < P - 1) diff += fabs(c[j] - c[m - 1]);
+    if (last && (p < P - 1 || wrap)) diff += fabs(c[j] - c[m - 1]);
     if (!(diff <= tol)) atomicExch(differs, 1);
 }
 

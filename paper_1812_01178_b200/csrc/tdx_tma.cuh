@@ -70,9 +70,8 @@ struct UnitTmaArgs {
 
 constexpr int unit_tma_regs(int M) { return M <= 8 ? 56 : (M <= 16 ? 80 : 128); }
 
-// The uniform row table (all partitions identical: uniform grid in x) travels as a kernel parameter: with the row loops
-// fully unrolled every table value is a constant-bank operand of its DFMA -- no load instruction, no L1 wavefront.
-template <int M> struct UniTable { double v[M * 6]; };
+// The uniform row table (all partitions identical: uniform grid in x) travels as a kernel parameter (UniTable,
+// tdx_kernels.cuh).
 
 // M = rows per partition = doubles per partition row (16 -> 128-byte rows / SWIZZLE_128B, 8 -> 64-byte / SWIZZLE_64B,
 // 32 -> two 128-byte tile rows per partition: eight lanes then hit four distinct swizzle keys, a 2-way bank conflict that
