@@ -95,7 +95,7 @@ tdx_status_t tdx_adi_step(tdx_grid_t* grid, tdx_mode_t mode, int Px, int Py, int
  * (b_0 := 1, c_0 := 0, d_0 := 0).  kz2: HOST, nm doubles.  kx2: HOST, nx doubles, or NULL for zeros
  * A kx2 with non-zero entries gives every line its own matrix (the paper's cosine-x / Fourier-z solve): factorisation,
  * spikes and reduced system are then computed on the fly per line; THOMAS takes any shape (device workspace of nx*ny*nm
- * doubles owned by the grid), PDD/PPT need ny = P*M with M in {8,12,16} (else TDX_ERR_UNSUPPORTED).  This case is
+ * doubles owned by the grid), PDD/PPT take at most 16 rows per partition, ceil(ny/P) <= 16 (else TDX_ERR_UNSUPPORTED: raise P).  This case is
  * synchronous (kx2/kz2 are read during the call).
  * rhs_inout: DEVICE, complex128 interleaved [nm][ny][nx] (x fastest) = 2*nm*ny*nx doubles; the matrix is
  * real, so re and im are two right-hand sides of one factorisation.                                       */
@@ -125,7 +125,7 @@ tdx_status_t tdx_irfft_z(tdx_grid_t* grid, const double* spec_in, double* field_
  * scratch of 2*(nz/2+1)*ny*nx doubles (caller-owned).  kx2 (HOST, nx) / kz2 (HOST, nz/2+1): the modified wavenumbers,
  * or NULL for kx2[i] = 2(1-cos(pi i/nx))/dx^2, kz2[m] = 2(1-cos(2 pi m/nz))/dz^2 of the grid's uniform x / z spacing
  * (TDX_ERR_UNSUPPORTED if that direction is not uniform).  mode / P: as tdx_helmholtz_wavenumber_solve with per-line
- * shifts (PDD/PPT need ny = P*M, M in {8,12,16}; the paper uses PPT here because PDD is inaccurate on the weakly
+ * shifts (PDD/PPT need ceil(ny/P) <= 16; the paper uses PPT here because PDD is inaccurate on the weakly
  * dominant low modes, L172).  Every argument check of every stage precedes the first launch.  Synchronous
  * (returns when the solve has finished on `stream`).                                                          */
 tdx_status_t tdx_poisson_solve(tdx_grid_t* grid, tdx_mode_t mode, int P, const double* kx2, const double* kz2,

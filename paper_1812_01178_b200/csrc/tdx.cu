@@ -373,6 +373,9 @@ tdx_status_t launch_strided_M(const Plan& pl, StridedArgs& A, const Tables& T, d
     return fail(TDX_ERR_UNSUPPORTED, "no strided kernel for M=%d V=%d", M, V);
 }
 
+// register tile of k_helm_lines for ceil(n / P) rows per partition: 8, 12 or 16 (0: does not fit)
+int helm_lines_M(int n, int P) { const int mx = (n + P - 1) / P; return mx <= 8 ? 8 : (mx <= 12 ? 12 : (mx <= 16 ? 16 : 0)); }
+
 int pow2floor(long long v) { int p = 1; while ((long long)p * 2 <= v) p *= 2; return p; }
 
 // lines of `dir` in a field whose x extent is `nxe` doubles (nx for real fields, 2 nx for complex ones)
@@ -999,11 +1002,11 @@ tdx_status_t tdx_helmholtz_wavenumber_solve(tdx_grid_t* g, tdx_mode_t mode, int 
         if (any) {
             // per-line matrices: only the on-the-fly Thomas baseline is built (PPT/PDD per line: SURVEY 8(f) N2/N4)
             const int ny = g->ny;
-            const int Mh = (mode != TDX_MODE_THOMAS && P >= 2 && ny % P == 0) ? ny / P : 0;
+            int Mh = 0;
             if (mode != TDX_MODE_THOMAS) {
                 if (P < 2 || P > TDX_MAX_P || ny / P < 2) return fail(TDX_ERR_BAD_PARTITION, "P=%d invalid for line length %d", P, ny);
-                if (Mh != 8 && Mh != 12 && Mh != 16)
-                    return fail(TDX_ERR_UNSUPPORTED, "per-line shifts (non-zero kx2) in PDD/PPT mode need ny = P*M with M in {8,12,16}; ny=%d P=%d", ny, P);
+                Mh = helm_lines_M(ny, P);
+                if (!Mh) return fail(TDX_ERR_UNSUPPORTED, "per-line shifts (non-zero kx2) in PDD/PPT mode take at most 16 rows per partition: raise P; ny=%d P=%d", ny, P);
             }
             CUDA_TRY(cudaSetDevice(g->device));
             cudaStream_t st = static_cast<cudaStream_t>(stream);
@@ -1031,14 +1034,21 @@ tdx_status_t tdx_helmholtz_wavenumber_solve(tdx_grid_t* g, tdx_mode_t mode, int 
                 double2* d2 = reinterpret_cast<double2*>(rhs);
                 static bool attr_done = false;
                 if (!attr_done) {
-                    CUDA_TRY(cudaFuncSetAttribute(k_helm_lines<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024));
-                    CUDA_TRY(cudaFuncSetAttribute(k_helm_lines<12>, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024));
-                    CUDA_TRY(cudaFuncSetAttribute(k_helm_lines<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024));
+                    CUDA_TRY(cudaFuncSetAttribute(k_helm_lines<8, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024));
+                    CUDA_TRY(cudaFuncSetAttribute(k_helm_lines<12, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024));
+                    CUDA_TRY(cudaFuncSetAttribute(k_helm_lines<16, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024));
+                    CUDA_TRY(cudaFuncSetAttribute(k_helm_lines<8, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024));
+                    CUDA_TRY(cudaFuncSetAttribute(k_helm_lines<12, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024));
+                    CUDA_TRY(cudaFuncSetAttribute(k_helm_lines<16, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024));
                     attr_done = true;
                 }
-                if (Mh == 8) k_helm_lines<8><<<grid, block, smem, st>>>(d2, g->nx, ny, P, ppt, pf, g->lo_neumann_y, g->up_neumann_y, dkx, dkz);
-                else if (Mh == 12) k_helm_lines<12><<<grid, block, smem, st>>>(d2, g->nx, ny, P, ppt, pf, g->lo_neumann_y, g->up_neumann_y, dkx, dkz);
-                else k_helm_lines<16><<<grid, block, smem, st>>>(d2, g->nx, ny, P, ppt, pf, g->lo_neumann_y, g->up_neumann_y, dkx, dkz);
+                const int hq = ny / P, hr = ny % P;
+                const bool rag = hr != 0 || hq != Mh;              // partitions shorter than the register tile: padding rows
+#define TDX_HELM_LINES(MM, RR) k_helm_lines<MM, RR><<<grid, block, smem, st>>>(d2, g->nx, ny, P, hq, hr, ppt, pf, g->lo_neumann_y, g->up_neumann_y, dkx, dkz)
+                if (Mh == 8) { if (rag) TDX_HELM_LINES(8, true); else TDX_HELM_LINES(8, false); }
+                else if (Mh == 12) { if (rag) TDX_HELM_LINES(12, true); else TDX_HELM_LINES(12, false); }
+                else { if (rag) TDX_HELM_LINES(16, true); else TDX_HELM_LINES(16, false); }
+#undef TDX_HELM_LINES
                 LAUNCH_CHECK("k_helm_lines");
                 CUDA_TRY(cudaStreamSynchronize(st));
                 return TDX_OK;
@@ -1084,9 +1094,8 @@ tdx_status_t tdx_poisson_solve(tdx_grid_t* g, tdx_mode_t mode, int P, const doub
     if ((reinterpret_cast<uintptr_t>(field) | reinterpret_cast<uintptr_t>(spec_work)) & 15) return fail(TDX_ERR_INVALID_ARG, "buffers must be 16-byte aligned");
     if (mode != TDX_MODE_THOMAS) {
         if (P < 2 || P > TDX_MAX_P || g->ny / P < 2) return fail(TDX_ERR_BAD_PARTITION, "P=%d invalid for line length %d", P, g->ny);
-        const int Mh = (g->ny % P == 0) ? g->ny / P : 0;
-        if (Mh != 8 && Mh != 12 && Mh != 16)
-            return fail(TDX_ERR_UNSUPPORTED, "per-line shifts in PDD/PPT mode need ny = P*M with M in {8,12,16}; ny=%d P=%d", g->ny, P);
+        if (!helm_lines_M(g->ny, P))
+            return fail(TDX_ERR_UNSUPPORTED, "per-line shifts in PDD/PPT mode take at most 16 rows per partition: raise P; ny=%d P=%d", g->ny, P);
     }
     std::vector<double> kx, kz;
     if (!kx2) {

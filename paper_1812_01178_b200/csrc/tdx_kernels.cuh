@@ -399,10 +399,13 @@ __global__ void k_thomas_helm_lines(double2* __restrict__ data, double* __restri
 // the interface values and spike ends go to shared memory; PDD solves its two 2x2 blocks per thread (Alg.1 step 5), PPT
 // solves the block-tridiagonal Z in natural order (2x2 diagonal blocks [[1, w_last],[v_first, 1]]; DESIGN.md reading
 // A7) by block parallel cyclic reduction over the line's P threads, ceil(log2(P-1)) steps of one division each;
-// then Eq.(8).  Requires n = P*M exactly.  HBM traffic: 32 B per complex point; lo/up/kx2/kz2 come from L1.
-template <int M>
+// then Eq.(8).  RAG = false: n = P*M exactly.  RAG = true: the partition map of tdx_partition_bounds (q = n / P rows, the
+// first rq = n % P partitions one more, all <= M); slots jj >= m of a partition are padding rows (a = -1, b = 1, c = 0,
+// d = 0), which copy xt_last, v_last and w_last along to slot M-1 so that no register array is indexed at run time.
+// HBM traffic: 32 B per complex point; lo/up/kx2/kz2 come from L1.
+template <int M, bool RAG>
 __global__ void __maxnreg__(M <= 8 ? 128 : (M <= 12 ? 168 : 208))
-k_helm_lines(double2* __restrict__ data, int nx, int ny, int P, int ppt, int pf,
+k_helm_lines(double2* __restrict__ data, int nx, int ny, int P, int q, int rq, int ppt, int pf,
              const double* __restrict__ lo, const double* __restrict__ up,
              const double* __restrict__ kx2, const double* __restrict__ kz2) {
     extern __shared__ double hs[];
@@ -412,7 +415,8 @@ k_helm_lines(double2* __restrict__ data, int nx, int ny, int P, int ppt, int pf,
     const int m = blockIdx.y;
     const double lam = valid ? __dadd_rn(__ldg(kx2 + i), __ldg(kz2 + m)) : 1.0;
     const bool pinned = lam == 0.0;
-    const int start = p * M;
+    const int start = RAG ? part_start(p, q, rq) : p * M;
+    const int mr = RAG ? q + (p < rq ? 1 : 0) : M;                  // real rows of this partition
     double2* base = data + ((size_t)m * ny + start) * nx + i;
     // shared layout, all indexed [p][tx]: xf, xl (double2), vf, vl, wf, wl; PPT adds beta, idet, r0, r1 (double2 r)
     const int S = P * LPC;
@@ -429,7 +433,7 @@ k_helm_lines(double2* __restrict__ data, int nx, int ny, int P, int ppt, int pf,
     double2 y[M];
     double f[M], cp[M];
 #pragma unroll
-    for (int jj = 0; jj < M; ++jj) y[jj] = valid ? __ldcs(base + (size_t)jj * nx) : make_double2(0.0, 0.0);
+    for (int jj = 0; jj < M; ++jj) y[jj] = (valid && (!RAG || jj < mr)) ? __ldcs(base + (size_t)jj * nx) : make_double2(0.0, 0.0);
     if (pf > 0 && (tx & 7) == 0) {                                   // L2 prefetch of the tile `pf` CTAs ahead, one lane per 128-byte line
         const long long lin = (long long)blockIdx.y * gridDim.x + blockIdx.x + pf;
         if (lin < (long long)gridDim.x * gridDim.y) {
@@ -437,7 +441,7 @@ k_helm_lines(double2* __restrict__ data, int nx, int ny, int P, int ppt, int pf,
             if (bx * LPC + tx < nx) {
                 const double2* pb = data + ((size_t)by * ny + start) * nx + bx * LPC + tx;
 #pragma unroll
-                for (int jj = 0; jj < M; ++jj) asm volatile("prefetch.global.L2 [%0];" ::"l"(pb + (size_t)jj * nx));
+                for (int jj = 0; jj < M; ++jj) if (!RAG || jj < mr) asm volatile("prefetch.global.L2 [%0];" ::"l"(pb + (size_t)jj * nx));
             }
         }
     }
@@ -448,18 +452,22 @@ k_helm_lines(double2* __restrict__ data, int nx, int ny, int P, int ppt, int pf,
 #pragma unroll
         for (int jj = 0; jj < M; ++jj) {
             const int j = start + jj;
-            double aj = __ldg(lo + j), cj = __ldg(up + j);
-            double bj = __dsub_rn(-__dadd_rn(aj, cj), lam);
-            if (j == 0) { bj = __dsub_rn(-cj, lam); aj = 0.0; }
-            if (j == ny - 1) { bj = __dsub_rn(-aj, lam); cj = 0.0; }
-            if (pinned && j == 0) { bj = 1.0; cj = 0.0; y[0] = make_double2(0.0, 0.0); }
-            const double ae = (jj == 0) ? 0.0 : aj, ce = (jj == M - 1) ? 0.0 : cj;
+            const bool pad = RAG && jj >= mr;
+            double aj = -1.0, cj = 0.0, bj = 1.0;                    // padding row: y_jj = y_{jj-1}
+            if (!pad) {
+                aj = __ldg(lo + j); cj = __ldg(up + j);
+                bj = __dsub_rn(-__dadd_rn(aj, cj), lam);
+                if (j == 0) { bj = __dsub_rn(-cj, lam); aj = 0.0; }
+                if (j == ny - 1) { bj = __dsub_rn(-aj, lam); cj = 0.0; }
+                if (pinned && j == 0) { bj = 1.0; cj = 0.0; y[0] = make_double2(0.0, 0.0); }
+            }
+            const double ae = (jj == 0) ? 0.0 : aj, ce = (RAG ? jj >= mr - 1 : jj == M - 1) ? 0.0 : cj;
             const double inv = 1.0 / (bj - ae * cprev);
             cp[jj] = ce * inv;
             y[jj].x = (y[jj].x - ae * yprev.x) * inv;
             y[jj].y = (y[jj].y - ae * yprev.y) * inv;
             f[jj] = (jj == 0) ? aj * inv : -ae * fprev * inv;       // left spike: rhs a_first e_first
-            if (jj == M - 1) wl = cj * inv;                          // right spike: rhs c_last e_last
+            if (RAG ? jj == mr - 1 : jj == M - 1) wl = cj * inv;     // right spike: rhs c_last e_last
             cprev = cp[jj]; fprev = f[jj]; yprev = y[jj];
         }
     }
@@ -472,7 +480,7 @@ k_helm_lines(double2* __restrict__ data, int nx, int ny, int P, int ppt, int pf,
             y[jj].x = y[jj].x - c1 * y[jj + 1].x;
             y[jj].y = y[jj].y - c1 * y[jj + 1].y;
             f[jj] = f[jj] - c1 * f[jj + 1];
-            wn = -c1 * wn;
+            wn = (RAG && jj >= mr - 1) ? wl : -c1 * wn;              // padding slots hold w_last
             cp[jj] = wn;
         }
     }
@@ -566,7 +574,7 @@ k_helm_lines(double2* __restrict__ data, int nx, int ny, int P, int ppt, int pf,
         double2 r = y[jj];
         r.x = fma(-f[jj], yL.x, r.x); r.y = fma(-f[jj], yL.y, r.y);
         r.x = fma(-cp[jj], yR.x, r.x); r.y = fma(-cp[jj], yR.y, r.y);
-        if (valid) __stcs(base + (size_t)jj * nx, r);
+        if (valid && (!RAG || jj < mr)) __stcs(base + (size_t)jj * nx, r);
     }
 }
 

@@ -220,9 +220,10 @@ def test_helmholtz_per_line_shift_kx2_thomas(cfg2):
     for m in range(0, c.nm, 4):                                  # per wavenumber: large low modes must not hide the rest
         assert relerr(out[m], ref[m]) < TOL_EXACT, (m, relerr(out[m], ref[m]))
     assert relerr(out, ref) < TOL_EXACT
-    with pytest.raises(tdx.TdxError) as e:                       # per-line PDD/PPT needs ny = P*M, M in {8,12,16}
+    before = t.clone()
+    with pytest.raises(tdx.TdxError) as e:                       # per-line PDD/PPT takes at most 16 rows per partition (128 / 4 = 32)
         grid.helmholtz_wavenumber_solve(tdx.MODE_PPT, 4, kx2, kz2, t)
-    assert e.value.status == tdx.ERR_UNSUPPORTED
+    assert e.value.status == tdx.ERR_UNSUPPORTED and torch.equal(t, before)
     # kx2 given but all zero is the shared-matrix fast path
     t2 = torch.from_numpy(rhs).cuda(); t3 = torch.from_numpy(rhs).cuda()
     grid.helmholtz_wavenumber_solve(tdx.MODE_PPT, 8, np.zeros(c.nx), kz2, t2)
@@ -275,4 +276,34 @@ def test_helmholtz_per_line_ragged_tile_and_12_row_partitions():
         grid.helmholtz_wavenumber_solve(tdx.MODE_PPT, P, kx2, kz2, t)
         torch.cuda.synchronize()
         assert relerr(t.cpu().numpy(), exact) < TOL_EXACT, P
+    grid.close()
+
+
+@pytest.mark.parametrize("ny,P", [(100, 8), (100, 7), (37, 3), (50, 25), (131, 9), (96, 7)])
+def test_helmholtz_per_line_ragged_partitions(ny, P):
+    """Per-line PPT / PDD when ny is not P*M: the partition map of tdx_partition_bounds (reading A5) with padding rows in
+    the register tile (k_helm_lines<M, true>); every element against the oracle, PDD against the oracle's step-by-step PDD."""
+    nx, nz = 21, 10
+    faces = (inputs.faces_uniform(nx, 1.0), inputs.faces_tanh_one_sided(ny, 2.5), inputs.faces_uniform(nz, 1.0))
+    grid = tdx.Grid(nx, ny, nz, *faces, bcs=BCS)
+    nm = nz // 2 + 1
+    rhs = inputs.rhs_complex_uniform((nm, ny, nx), 77 + ny)
+    kz2 = inputs.modified_wavenumbers_z(nz, 1.0)
+    kx2 = inputs.modified_wavenumbers_x(nx, 1.0)
+    exact = orc.helmholtz_solve(rhs.copy(), faces[1], kx2, kz2, orc.MODE_THOMAS, 1)
+    t = torch.from_numpy(rhs).cuda()
+    grid.helmholtz_wavenumber_solve(tdx.MODE_PPT, P, kx2, kz2, t)
+    torch.cuda.synchronize()
+    out = t.cpu().numpy()
+    assert out[0, 0, 0] == 0.0                                   # the pinned point of mode (0, 0)
+    assert relerr(out, exact) < TOL_EXACT, (ny, P, relerr(out, exact))
+    for m in range(nm):
+        assert relerr(out[m], exact[m]) < 1e-11, (m, relerr(out[m], exact[m]))
+    t = torch.from_numpy(rhs).cuda()
+    grid.helmholtz_wavenumber_solve(tdx.MODE_PDD, P, kx2, kz2, t)
+    torch.cuda.synchronize()
+    pdd = orc.helmholtz_solve(rhs.copy(), faces[1], kx2, kz2, orc.MODE_PDD, P)
+    out = t.cpu().numpy()
+    for m in range(nm):
+        assert relerr(out[m], pdd[m]) < 1e-11, (m, relerr(out[m], pdd[m]))
     grid.close()

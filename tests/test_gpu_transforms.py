@@ -122,8 +122,8 @@ def test_transform_error_paths_leave_data_untouched():
         grid.rfft_z(t, t)                                    # in place is not defined
     assert e.value.status == tdx.ERR_INVALID_ARG
     with pytest.raises(tdx.TdxError) as e:
-        grid.poisson_solve(tdx.MODE_PPT, 3, None, None, t, spec)   # 16 rows / 3 partitions: not P*M
-    assert e.value.status in (tdx.ERR_UNSUPPORTED, tdx.ERR_BAD_PARTITION)
+        grid.poisson_solve(tdx.MODE_PPT, 9, None, None, t, spec)   # 16 rows / 9 partitions: fewer than 2 rows each
+    assert e.value.status == tdx.ERR_BAD_PARTITION
     t.fill_(1.5)
     bad = np.full(32, 1.0); bad[7] = float("nan")
     with pytest.raises(tdx.TdxError) as e:                       # a bad wavenumber is caught before the first transform runs
@@ -198,7 +198,7 @@ def test_poisson_solve_manufactured_small_every_element():
     phi = inputs.rhs_uniform((nz, ny, nx), 31)
     f = otr.laplacian(phi, faces[1], 2.0, 1.0)
     work = torch.empty((nz // 2 + 1, ny, nx), dtype=torch.complex128, device="cuda")
-    for mode, P in ((tdx.MODE_THOMAS, 1), (tdx.MODE_PPT, 4), (tdx.MODE_PPT, 2)):
+    for mode, P in ((tdx.MODE_THOMAS, 1), (tdx.MODE_PPT, 4), (tdx.MODE_PPT, 2), (tdx.MODE_PPT, 3), (tdx.MODE_PPT, 5)):   # 3, 5: ragged partitions
         t = torch.from_numpy(f).cuda()
         grid.poisson_solve(mode, P, None, None, t, work)
         torch.cuda.synchronize()
