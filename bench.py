@@ -35,8 +35,8 @@ TUNED_P_LINE = {1: 4, 2: 16, 3: 32, 4: 32, 5: 24, 6: 16}
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures
 # (profiles/r1_ncu_cfg5_summary.md), valid for mode ppt with the tuned P of the config; bytes.
 NCU_TRAFFIC = {
-    "cfg5_4096x288x512": {"adi_x": 9.605491e9, "adi_y": 9.604487e9, "adi_z_cyclic": 9.623668e9, "helmholtz_y": 9.713430e9},
-    "cfg4_1024x512x256": {"adi_x": 2.089586e9, "adi_y": 2.088622e9, "adi_z_cyclic": 2.097331e9, "helmholtz_y": 2.110831e9},
+    "cfg5_4096x288x512": {"adi_x": 9.605791e9, "adi_y": 9.604312e9, "adi_z_cyclic": 9.622963e9, "helmholtz_y": 9.714489e9},
+    "cfg4_1024x512x256": {"adi_x": 2.089255e9, "adi_y": 2.088877e9, "adi_z_cyclic": 2.098726e9, "helmholtz_y": 2.114430e9},
 }
 
 # tuned partitions per line (x, y, z, helmholtz-y) per config; rows per partition <= 64

@@ -76,7 +76,7 @@ def test_error_paths_leave_data_untouched(small):
         grid.adi_sweep(0, tdx.MODE_PPT, 2, 1e-3, 0)              # NULL data pointer
     assert e.value.status == tdx.ERR_INVALID_ARG
     with pytest.raises(tdx.TdxError) as e:
-        grid.helmholtz_wavenumber_solve(tdx.MODE_PPT, 4, np.ones(nx), np.ones(3), t)
+        grid.helmholtz_wavenumber_solve(tdx.MODE_PPT, 2, np.ones(nx), np.ones(3), t)   # per-line shifts: 18 rows per partition > 16
     assert e.value.status == tdx.ERR_UNSUPPORTED
     torch.cuda.synchronize()
     assert np.array_equal(t.cpu().numpy(), field)
