@@ -40,7 +40,7 @@ NCU_TRAFFIC = {
 }
 
 # tuned partitions per line (x, y, z, helmholtz-y) per config; rows per partition <= 64
-TUNED_P = {1: (4, 4, 4, 4), 2: (16, 8, 8, 8), 3: (32, 8, 8, 8), 4: (64, 16, 8, 16), 5: (256, 24, 16, 12), 6: (192, 8, 24, 8)}
+TUNED_P = {1: (4, 4, 4, 4), 2: (16, 8, 8, 8), 3: (32, 8, 8, 8), 4: (64, 16, 8, 16), 5: (256, 24, 16, 12), 6: (384, 8, 24, 8)}
 
 
 def parse():

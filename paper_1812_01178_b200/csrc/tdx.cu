@@ -318,16 +318,16 @@ Tables tables_of(const Plan& pl) {
 // ---- launch selection ---------------------------------------------------------------------------------------
 namespace {
 
-template <int M, int V, bool CYC, bool UNI = false>
+template <int M, int V, bool CYC, bool UNI = false, int REGS = strided_regs(M, V)>
 tdx_status_t launch_strided_inst(const Plan& pl, StridedArgs& A, const Tables& T, dim3 grid, dim3 block, size_t smem, cudaStream_t st) {
     static bool attr_done = false;
     if (!attr_done && smem > 48 * 1024) {
-        CUDA_TRY(cudaFuncSetAttribute(k_strided<M, V, CYC, UNI>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+        CUDA_TRY(cudaFuncSetAttribute(k_strided<M, V, CYC, UNI, REGS>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
         attr_done = true;
     }
     if (pl.pf < 0) {                                               // prefetch one wave of resident CTAs ahead
         int occ = 1;
-        CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_strided<M, V, CYC, UNI>, (int)(block.x * block.y), smem));
+        CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_strided<M, V, CYC, UNI, REGS>, (int)(block.x * block.y), smem));
         pl.pf = pl.sms * (occ < 1 ? 1 : occ) * prefetch_waves();
     }
     // one tile per CTA: pf = CTAs ahead; looping CTAs (grid.x < tiles_x): pf = sets ahead for the first tile of a later CTA
@@ -341,7 +341,7 @@ tdx_status_t launch_strided_inst(const Plan& pl, StridedArgs& A, const Tables& T
         }
         std::memcpy(U.v, pl.uni_host, sizeof(U.v));
     } else std::memset(U.v, 0, sizeof(U.v));
-    k_strided<M, V, CYC, UNI><<<grid, block, smem, st>>>(A, T, U);
+    k_strided<M, V, CYC, UNI, REGS><<<grid, block, smem, st>>>(A, T, U);
     LAUNCH_CHECK("k_strided");
     return TDX_OK;
 }
@@ -354,7 +354,8 @@ tdx_status_t launch_strided_M(const Plan& pl, StridedArgs& A, const Tables& T, d
         switch (M) {
             case 8: return launch_strided_inst<8, V, false, true>(pl, A, T, grid, block, smem, st);
             case 16: return launch_strided_inst<16, V, false, true>(pl, A, T, grid, block, smem, st);
-            case 32: if (V == 2) return launch_strided_inst<32, 2, false, true>(pl, A, T, grid, block, smem, st);
+            case 32: if (V == 2 && block.x * block.y > 256) return launch_strided_inst<32, 2, false, true, 168>(pl, A, T, grid, block, smem, st);
+                     if (V == 2) return launch_strided_inst<32, 2, false, true>(pl, A, T, grid, block, smem, st);
                      return launch_strided_inst<32, 1, false, true>(pl, A, T, grid, block, smem, st);
         }
         return fail(TDX_ERR_UNSUPPORTED, "no uniform-table strided kernel for M=%d", M);
@@ -405,8 +406,11 @@ tdx_status_t run_strided(const Plan& pl, double* data, long long W, long long li
     const bool fat = set_per_outer && pl.M >= 32;             // 255-register instantiation, one table set per outer index: measured on cfg4 Helmholtz
     if (fat) row_doubles = 32;                                //   256-byte rows + 8 tiles per CTA 0.389 ms against 0.406 (128-byte rows, 4 tiles)
     if (env_row == 16 || env_row == 32 || env_row == 64) row_doubles = env_row;
+    // 32-row partitions with the table in the constant bank fit 168 registers: up to 384 threads, so 17..24 partitions
+    // still get 256-byte row segments (nz = 768 = 24 x 32, the paper's grid) where the 213-register kernel stops at 16
+    const bool slim = pl.layout == ROWS_U && pl.M == 32 && even && row_doubles == 32 && pl.P > 16 && pl.P <= 24;
     auto pick = [&](int V, int& LPC) -> bool {
-        const int bt = strided_block_threads(pl.M, V);
+        const int bt = (slim && V == 2) ? 384 : strided_block_threads(pl.M, V);
         if (bt < pl.P || (V == 2 && (!even || pl.M > 32))) return false;
         int lmax = pow2floor(bt / pl.P); if (lmax > 32) lmax = 32;
         int l = row_doubles / V;

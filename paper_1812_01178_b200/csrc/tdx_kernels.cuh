@@ -67,8 +67,9 @@ constexpr int strided_block_threads(int MAXM, int V) {            // largest CTA
 template <int M> struct UniTable { double v[M * 6]; };
 
 // UNI: row table = U.v[jj*6 + f] for every partition (ROWS_U plans: periodic or interior-identical blocks, one set).
-template <int MAXM, int V, bool CYC, bool UNI>
-__global__ void __maxnreg__(strided_regs(MAXM, V))
+// REGS: register budget; the default is the tier of the partition size, a smaller one buys a wider CTA (longer row segments).
+template <int MAXM, int V, bool CYC, bool UNI, int REGS = strided_regs(MAXM, V)>
+__global__ void __maxnreg__(REGS)
 k_strided(StridedArgs A, Tables T, const __grid_constant__ UniTable<UNI ? MAXM : 1> U) {
     extern __shared__ double rs[];                          // rs[(idx*LPC + tx)*V + v], idx in [0, 2P)
     const int tx = threadIdx.x, p = threadIdx.y;
