@@ -9,7 +9,9 @@
  *
  * Every function is pinned by tests/test_oracle_pins.py (dense Gaussian elimination, manufactured
  * solutions, eigen closed forms, the printed structure of Z and Z-bar at PAPER.md:L116/L136, the
- * dominance invariants at L162/L172).  Nothing here is "parity unpinned".
+ * dominance invariants at L162/L172) and tests/test_oracle_partition_pins.py (PDD / PPT step by step; PDD on a
+ * periodic line, oracle_cyclic_pdd_line, against a dense LAPACK Woodbury restatement with the far spike ends deleted,
+ * the block spike equations, exactness when decayed).  Nothing here is "parity unpinned".
  *
  * Layout of 3-D fields: x fastest, idx(i,j,k) = i + nx*(j + ny*k); all solves in place.
  */

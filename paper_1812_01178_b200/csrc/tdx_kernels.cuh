@@ -1,6 +1,7 @@
 // tdx_kernels.cuh -- the hot path: one launch per sweep, 8 B read + 8 B written per grid value.
 //
-//   k_strided<MAXM,V,CYC>  y / z sweeps and the Helmholtz y-solves: thread = (line, partition), a warp holds
+//   k_strided<MAXM,V,CYC,UNI,REGS>  (UNI: one row table for every partition, passed as a kernel parameter; REGS: register budget)
+//                          y / z sweeps and the Helmholtz y-solves: thread = (line, partition), a warp holds
 //                          consecutive lines of ONE partition, so every global access is a coalesced row segment and
 //                          the plan tables are warp-uniform.  Each thread keeps its partition (<= MAXM rows, V lines)
 //                          in registers: forward + backward elimination (Eq.(5)), interface values to shared memory,
