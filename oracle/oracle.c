@@ -459,6 +459,42 @@ double oracle_cyclic_pdd_dropped(int n, int P, const double *a, const double *b,
     return dr;
 }
 
+/* ---------------------------------------------------------------------------------------------
+ * The OTHER definition of PDD on a periodic line ("outer Sherman-Morrison (y and q each by the
+ * partitioned solve; q is matrix-only)" -- the definition the survey assigns to the oracle; reading A16
+ * says why the product takes the cyclically closed one above).  Rank-1 split of Eq.(3) first (cyclic_split:
+ * A' = A_cyc - u v^T, plain tridiagonal), then
+ *     y = PDD(A') d   step by step (oracle_partitioned_line, P-1 interfaces, Alg.1 steps 3, 5, 7),
+ *     q = A'^{-1} u   exactly (matrix-only, plan time),
+ *     x = y - q (y_0 + g y_{n-1}) / (1 + q_0 + g q_{n-1}).
+ * Unlike the cyclic closure this is exact at P = 1 and has P-1 interfaces; the two differ by O(dropped) (pinned in
+ * tests/test_oracle_partition_pins.py on the six config z-operators and on random weakly dominant lines).
+ * ------------------------------------------------------------------------------------------- */
+int oracle_cyclic_pdd_outer_line(int n, int P, const double *a, const double *b, const double *c,
+                                 const double *d, double *x) {
+    if (n < 3) return ORACLE_ERR;
+    double *wk = (double *)malloc(sizeof(double) * n * 7);
+    double *a2 = wk, *b2 = wk + n, *c2 = wk + 2 * n, *u = wk + 3 * n, *y = wk + 4 * n, *q = wk + 5 * n, *dd = wk + 6 * n, g;
+    memcpy(dd, d, sizeof(double) * n);                                   /* x may alias d */
+    cyclic_split(n, a, b, c, a2, b2, c2, u, &g);
+    int rc = oracle_partitioned_line(n, P, MODE_PDD, a2, b2, c2, dd, y, NULL);
+    oracle_thomas(n, a2, b2, c2, u, q);
+    double s = (y[0] + g * y[n - 1]) / (1.0 + q[0] + g * q[n - 1]);
+    for (int j = 0; j < n; ++j) x[j] = y[j] - q[j] * s;
+    free(wk);
+    return rc;
+}
+
+/* a-priori bound of the outer-split PDD: the far spike ends of A' = the non-periodic bound on the split matrix. */
+double oracle_cyclic_pdd_outer_dropped(int n, int P, const double *a, const double *b, const double *c) {
+    if (n < 3) return -1.0;
+    double *wk = (double *)malloc(sizeof(double) * n * 4), g;
+    cyclic_split(n, a, b, c, wk, wk + n, wk + 2 * n, wk + 3 * n, &g);
+    double dr = oracle_pdd_dropped(n, P, wk, wk + n, wk + 2 * n);
+    free(wk);
+    return dr;
+}
+
 /* Cyclic line with partitions.  PDD: the cyclically closed reduced system above.  PPT (exact in either form):
  * outer Sherman-Morrison; y = A'^{-1} d by the partitioned solve, q = A'^{-1} u by Thomas. */
 int oracle_cyclic_line(int n, int P, int mode, const double *a, const double *b, const double *c,

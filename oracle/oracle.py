@@ -38,6 +38,7 @@ def _chk(rc, what):
 
 _lib.oracle_pdd_dropped.restype = C.c_double
 _lib.oracle_cyclic_pdd_dropped.restype = C.c_double
+_lib.oracle_cyclic_pdd_outer_dropped.restype = C.c_double
 _lib.oracle_pdd_dropped.argtypes = [C.c_int, C.c_int, _dp, _dp, _dp]
 
 
@@ -150,6 +151,20 @@ def cyclic_pdd_line(P, a, b, c, d, return_spikes=False):
     sp = np.zeros(2 * d.size)
     _chk(_lib.oracle_cyclic_pdd_line(C.c_int(d.size), C.c_int(P), _p(a), _p(b), _p(c), _p(d), _p(x), _p(sp)), "cyclic_pdd_line")
     return (x, sp[:d.size].copy(), sp[d.size:].copy()) if return_spikes else x
+
+
+def cyclic_pdd_outer_line(P, a, b, c, d):
+    """PDD on one periodic line by the OUTER rank-1 split (SURVEY 8(c) C2's oracle definition; oracle_cyclic_pdd_outer_line)."""
+    a, b, c, d = _c(a), _c(b), _c(c), _c(d)
+    x = np.empty_like(d)
+    _chk(_lib.oracle_cyclic_pdd_outer_line(C.c_int(d.size), C.c_int(P), _p(a), _p(b), _p(c), _p(d), _p(x)), "cyclic_pdd_outer_line")
+    return x
+
+
+def cyclic_pdd_outer_dropped(P, a, b, c):
+    """a-priori bound of the outer-split PDD: the far spike ends of the split matrix A'."""
+    a, b, c = _c(a), _c(b), _c(c)
+    return float(_lib.oracle_cyclic_pdd_outer_dropped(C.c_int(b.size), C.c_int(P), _p(a), _p(b), _p(c)))
 
 
 def partitioned_line(P, mode, a, b, c, d, return_y=False):
