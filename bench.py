@@ -32,15 +32,41 @@ BYTES_PER_POINT = 16.0          # 8 B read + 8 B written per real grid value per
 # partitions per line for the per-line-shift Helmholtz solve (kx2 != 0): at most 16 rows per partition
 TUNED_P_LINE = {1: 4, 2: 16, 3: 32, 4: 32, 5: 24, 6: 16}
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed `ncu --set full` captures
-# (profiles/r1_ncu_cfg5_summary.md), valid for mode ppt with the tuned P of the config; bytes.
-NCU_TRAFFIC = {
-    "cfg5_4096x288x512": {"adi_x": 9.605791e9, "adi_y": 9.604312e9, "adi_z_cyclic": 9.622963e9, "helmholtz_y": 9.714489e9},
-    "cfg4_1024x512x256": {"adi_x": 2.089255e9, "adi_y": 2.088877e9, "adi_z_cyclic": 2.098726e9, "helmholtz_y": 2.114430e9},
-}
+PDD_GATE = 1e-11                # DESIGN.md reading A9: north_star's 1e-10 PDD bar applies where the a-priori dropped bound <= 1e-11
 
-# tuned partitions per line (x, y, z, helmholtz-y) per config; rows per partition <= 64
+NCU_TRAFFIC_FILE = os.path.join(ROOT, "profiles", "r2_ncu_traffic.csv")
+
+
+def ncu_traffic(workload, launch):
+    """roofline.traffic: dram__bytes_read.sum + dram__bytes_write.sum per launch of the committed `ncu --set full` capture
+    (profiles/r2_ncu_traffic.csv; the command is in profiles/r2_ncu_traffic.md) for exactly this workload, kernel
+    instantiation and launch shape (tdx_last_launch()).  A kernel or launch-shape change finds no row: (None, reason)."""
+    if not os.path.exists(NCU_TRAFFIC_FILE):
+        return None, "no committed capture (profiles/r2_ncu_traffic.csv missing)"
+    import csv
+    with open(NCU_TRAFFIC_FILE) as f:
+        for row in csv.DictReader(r for r in f if not r.startswith("#")):
+            if row["workload"] == workload and row["launch"] == launch:
+                return float(row["dram_bytes_read"]) + float(row["dram_bytes_write"]), "profiles/r2_ncu_traffic.csv (ncu --set full, per launch)"
+    return None, "no committed ncu capture for %s on %s" % (launch, workload)
+
+
+# tuned partitions per line (x, y, z, helmholtz-y) per config, mode PPT (exact for every P)
 TUNED_P = {1: (4, 4, 4, 4), 2: (16, 8, 8, 8), 3: (32, 8, 8, 8), 4: (64, 16, 8, 16), 5: (256, 24, 16, 12), 6: (384, 8, 24, 8)}
+
+
+def pdd_partitions(grid, cfg, direction, P_ppt):
+    """P for a PDD sweep, by rule (never by hand): the PPT-tuned P if PDD is inside its regime there (a-priori bound
+    tdx_pdd_dropped_bound <= PDD_GATE, PAPER.md:L152 'n >> p'), else the largest smaller divisor of the line length whose
+    bound passes.  Returns (P, bound)."""
+    n = (cfg.nx, cfg.ny, cfg.nz)[direction]
+    for P in [P_ppt] + [d for d in range(P_ppt - 1, 1, -1) if n % d == 0]:
+        if n // P < 2:
+            continue
+        bound = grid.pdd_dropped_bound(direction, P, cfg.alpha)
+        if bound <= PDD_GATE:
+            return P, bound
+    return 1, 0.0                                               # P = 1 is the plain Thomas recurrence
 
 
 def parse():
@@ -249,11 +275,19 @@ def grid_table(tdx, torch, cfg_no, local_rank, steps, peak):
     for mname, mode in (("ppt", tdx.MODE_PPT), ("pdd", tdx.MODE_PDD)):
         res = {}
         for k, name in enumerate(names):
+            if mname == "pdd" and k == 3:
+                # PDD is not a valid solve for the Poisson y-systems (tests assert its error > 1e-3 on the
+                # low modes): no throughput is quoted for it.  PPT is the production mode there, as in the paper.
+                res[name] = {"skipped": "PDD is inaccurate on the weakly dominant Helmholtz systems (PAPER.md:L172): PPT only"}
+                continue
+            Pk, bound = Ps[k], None
+            if mname == "pdd":
+                Pk, bound = pdd_partitions(grid, cfg, k, Ps[k])
             def launch(c):
                 if k < 3:
-                    grid.adi_sweep(k, mode, Ps[k], cfg.alpha, fields[c], stream)
+                    grid.adi_sweep(k, mode, Pk, cfg.alpha, fields[c], stream)
                 else:
-                    grid.helmholtz_wavenumber_solve(mode, Ps[3], None, kz2, helms[c], stream)
+                    grid.helmholtz_wavenumber_solve(mode, Pk, None, kz2, helms[c], stream)
             for _ in range(3):
                 for c in range(K):
                     launch(c)
@@ -272,9 +306,10 @@ def grid_table(tdx, torch, cfg_no, local_rank, steps, peak):
             ms = tot / (rounds * K)
             gbs = BYTES_PER_POINT * pts[k] / (ms * 1e-3) / 1e9
             res[name] = {"ms": ms, "gpts_per_s": pts[k] / (ms * 1e-3) / 1e9, "gb_per_s": gbs, "frac_of_measured_peak": gbs / peak,
-                         "frac_of_nominal_8TBs": gbs / 8000.0, "P": Ps[k]}
-            if mname == "pdd" and k < 3:
-                res[name]["dropped_bound"] = grid.pdd_dropped_bound(k, Ps[k], cfg.alpha)
+                         "frac_of_nominal_8TBs": gbs / 8000.0, "P": Pk, "launch": tdx.last_launch()}
+            if mname == "pdd":
+                res[name]["dropped_bound"] = bound
+                res[name]["pdd_gate_ok"] = bool(bound <= PDD_GATE)
         out[mname] = res
     grid.close()
     del fields, helms, f0, h0
@@ -295,6 +330,17 @@ def run_tdx(args, rank, world, local_rank):
     bcs = (tdx.BC_DIRICHLET, tdx.BC_DIRICHLET, tdx.BC_PERIODIC)
     grid = tdx.Grid(cfg.nx, cfg.ny, cfg.nz, *cfg.faces(), bcs=bcs, device=local_rank)
     kz2 = cfg.kz2()
+    # --mode pdd: the ADI sweeps run PDD with P chosen by rule (pdd_partitions: a-priori bound <= 1e-11, so north_star's
+    # 1e-10 bar holds); the Poisson y-solves stay PPT -- PDD is not a valid solve there
+    hmode, pdd_bounds = mode, [None, None, None]
+    if args.mode == "pdd":
+        hmode = tdx.MODE_PPT
+        if not args.P:
+            picked = [pdd_partitions(grid, cfg, d, Ps[d]) for d in range(3)]
+            Ps = tuple(p for p, _ in picked) + (Ps[3],)
+            pdd_bounds = [b for _, b in picked]
+        else:
+            pdd_bounds = [grid.pdd_dropped_bound(d, Ps[d], cfg.alpha) for d in range(3)]
 
     # inputs: seeded synthetic, generated once on the host, resident in HBM before the timed region
     host_field = cfg.rhs_field() if rank == 0 else None         # every rank solves its own field (weak scaling)
@@ -308,13 +354,17 @@ def run_tdx(args, rank, world, local_rank):
     helm = helm0.clone()
     stream = torch.cuda.current_stream().cuda_stream
 
+    launches_seen = []                                          # kernel instantiation + launch shape of the four sweeps
+
     def step(ev=None):
         # in place: re-running on its own output is the same work (same bytes); contraction keeps values bounded
         for k, d in enumerate((0, 1, 2)):
             if ev: ev[k].record()
             grid.adi_sweep(d, mode, Ps[d], cfg.alpha, field, stream)
+            if launches_seen is not None and len(launches_seen) < 3: launches_seen.append(tdx.last_launch())
         if ev: ev[3].record()
-        grid.helmholtz_wavenumber_solve(mode, Ps[3], None, kz2, helm, stream)
+        grid.helmholtz_wavenumber_solve(hmode, Ps[3], None, kz2, helm, stream)
+        if launches_seen is not None and len(launches_seen) < 4: launches_seen.append(tdx.last_launch())
         if ev: ev[4].record()
 
     def barrier():
@@ -351,13 +401,19 @@ def run_tdx(args, rank, world, local_rank):
     peak, peak_src = measured_peak()
     per_kernel = {n: {"ms": kms[k], "gpts_per_s": pts[k] / (kms[k] * 1e-3) / 1e9, "gb_per_s": BYTES_PER_POINT * pts[k] / (kms[k] * 1e-3) / 1e9,
                       "frac_of_measured_peak": BYTES_PER_POINT * pts[k] / (kms[k] * 1e-3) / 1e9 / peak,
-                      "frac_of_nominal_8TBs": BYTES_PER_POINT * pts[k] / (kms[k] * 1e-3) / 1e9 / 8000.0, "P": Ps[k]} for k, n in enumerate(names)}
+                      "frac_of_nominal_8TBs": BYTES_PER_POINT * pts[k] / (kms[k] * 1e-3) / 1e9 / 8000.0, "P": Ps[k],
+                      "launch": launches_seen[k] if k < len(launches_seen) else None} for k, n in enumerate(names)}
+    for k in range(3):
+        if pdd_bounds[k] is not None:
+            per_kernel[names[k]]["dropped_bound"] = pdd_bounds[k]
+            per_kernel[names[k]]["pdd_gate_ok"] = bool(pdd_bounds[k] <= PDD_GATE)
+    if args.mode == "pdd":
+        per_kernel[names[3]]["mode"] = "ppt (PDD is not a valid solve for the Poisson y-systems, PAPER.md:L172)"
     dom = int(np.argmax(kms))
     achieved = BYTES_PER_POINT * pts[dom] / (kms[dom] * 1e-3) / 1e9
-    tuned = (Ps == TUNED_P[args.config]) and args.mode == "ppt"
-    traffic = NCU_TRAFFIC.get(cfg.name, {}).get(names[dom]) if tuned else None
-    roofline = {"bound": "hbm", "kernel": names[dom], "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": traffic, "traffic_source": "profiles/r1_ncu_cfg5_summary.md (ncu --set full, per launch)" if traffic else None,
+    traffic, traffic_src = ncu_traffic(cfg.name, per_kernel[names[dom]]["launch"])
+    roofline = {"bound": "hbm", "kernel": names[dom], "launch": per_kernel[names[dom]]["launch"], "achieved": achieved, "peak": peak,
+                "unit": "GB/s", "frac": achieved / peak, "traffic": traffic, "traffic_source": traffic_src,
                 "peak_source": peak_src, "algorithmic_bytes_per_launch": BYTES_PER_POINT * pts[dom],
                 "share_of_step": kms[dom] / sum(kms)}
 
@@ -545,7 +601,9 @@ def run_tdx(args, rank, world, local_rank):
             out["grids"] = {"error": repr(exc)[:300]}
 
     # end to end through the host-buffer C-ABI calls: pinned host buffers, H2D + solve + D2H inside the timed region
-    if not args.no_e2e:
+    if not args.no_e2e and hmode != mode:
+        out["e2e"] = {"skipped": "tdx_step_host runs one mode for the whole step; the end-to-end figure is quoted for --mode ppt"}
+    elif not args.no_e2e:
         hf = torch.from_numpy(host_field).pin_memory().numpy()
         hh = torch.from_numpy(host_helm).pin_memory().numpy()
         hh0 = host_helm

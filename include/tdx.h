@@ -42,12 +42,16 @@ typedef enum {
     TDX_ERR_BAD_PARTITION = -2,    /* P < 1, P > TDX_MAX_P or floor(n_dir/P) < 2                          */
     TDX_ERR_ALLOC = -3,
     TDX_ERR_CUDA = -4,             /* no device / launch or runtime failure (text in tdx_last_error)      */
-    TDX_ERR_UNSUPPORTED = -5,      /* valid request this build cannot run (e.g. rows per partition > 64)  */
-    TDX_ERR_PDD_BOUND = -6         /* reserved for strict PDD checking                                    */
+    TDX_ERR_UNSUPPORTED = -5,      /* valid request this build cannot run (text in tdx_last_error)        */
+    TDX_ERR_PDD_BOUND = -6         /* strict PDD checking is on (tdx_grid_set_pdd_strict) and the a-priori bound of this
+                                      (dir, P, operator) exceeds the limit; nothing was launched           */
 } tdx_status_t;
 
 #define TDX_MAX_P 1024             /* partitions per line                                                 */
-#define TDX_MAX_ROWS_PER_PARTITION 64   /* register-resident partition length limit for PDD/PPT          */
+#define TDX_MAX_ROWS_PER_PARTITION 64   /* rows one THREAD keeps in registers.  Not a limit on the caller's P: longer
+                                           partitions are cut again into sub-partitions inside the thread block (two-level
+                                           PDD / PPT; at most 256 sub-partitions per line), with the
+                                           result of the caller's P: PPT exact, PDD = PDD with his P partitions.     */
 
 /* Create a grid.  xf/yf/zf: HOST arrays of n+1 strictly increasing face coordinates per direction (copied).
  * Metrics (reading A3): width D_j, centre spacings hm_j, hp_j, mirrored ghost at Dirichlet/Neumann
@@ -59,16 +63,26 @@ tdx_status_t tdx_grid_create(int nx, int ny, int nz,
                              int device, tdx_grid_t** out);
 tdx_status_t tdx_grid_destroy(tdx_grid_t* grid);   /* frees plan tables; NULL is accepted                 */
 
+/* Strict PDD checking ("when n >> p", L164, L172).  PDD never falls back silently: it runs as
+ * asked.  With max_dropped > 0 every later PDD solve on this grid whose a-priori bound -- the largest far spike end
+ * |v_last|, |w_first| that PDD deletes from Z, tdx_pdd_dropped_bound -- exceeds max_dropped returns TDX_ERR_PDD_BOUND
+ * before anything is launched (1e-11 keeps the result within 1e-10 of the exact solution, reading A9).
+ * Helmholtz solves with per-line shifts are judged by their least dominant line (smallest kx2 + kz2); slabs by the
+ * rank-level bound.  0 switches the check off (the default).  THOMAS / PPT are never refused.               */
+tdx_status_t tdx_grid_set_pdd_strict(tdx_grid_t* grid, double max_dropped);
+
 /* Partition map (host, integer only; bit-exact contract, reading A5): q = n/P, r = n%P,
  * starts[p] = p*q + min(p,r), p = 0..P.  The paper has only m = n/p.
  * starts: HOST array of P+1 ints.                                                                        */
 tdx_status_t tdx_partition_bounds(int n, int P, int* starts);
 
 /* ADI sweep (Algorithm 1): solve (I - alpha*delta2_dir) x = rhs on every line of
- * direction dir, in place.  Rows satisfy |b| = |a| + |c| + 1 (L162).  Periodic directions: THOMAS and PDD close the
- * line by Sherman-Morrison (Eq.(3) with a rank-1 update) around the chosen mode; PPT (P <= 128) puts the two wrap-around
- * corner entries into Delta A (L78-91), i.e. P interfaces and a cyclic reduced system Z -- Woodbury, Eq.(3)-(4), exact.
- * rhs_inout: DEVICE, nx*ny*nz doubles.  P: partitions per line (ignored for THOMAS).                    */
+ * direction dir, in place.  Rows satisfy |b| = |a| + |c| + 1 (L162).  Periodic directions: THOMAS closes the line by
+ * Sherman-Morrison (Eq.(3) with a rank-1 update); PDD and PPT (P <= 128) put the two wrap-around corner entries into
+ * Delta A (L78-91), i.e. P interfaces and a cyclic reduced system Z -- Woodbury, Eq.(3)-(4): exact for PPT, and PDD deletes
+ * the far spike ends of every partition (reading A16: an approximation already at P = 2).
+ * rhs_inout: DEVICE, nx*ny*nz doubles.  P: partitions per line (ignored for THOMAS), 1 <= P <= TDX_MAX_P,
+ * floor(n_dir / P) >= 2, any partition length (see TDX_MAX_ROWS_PER_PARTITION).                           */
 tdx_status_t tdx_adi_sweep(tdx_grid_t* grid, tdx_dir_t dir, tdx_mode_t mode, int P,
                            double alpha, double* rhs_inout, void* stream);
 
@@ -95,8 +109,10 @@ tdx_status_t tdx_adi_step(tdx_grid_t* grid, tdx_mode_t mode, int Px, int Py, int
  * (b_0 := 1, c_0 := 0, d_0 := 0).  kz2: HOST, nm doubles.  kx2: HOST, nx doubles, or NULL for zeros
  * A kx2 with non-zero entries gives every line its own matrix (the paper's cosine-x / Fourier-z solve): factorisation,
  * spikes and reduced system are then computed on the fly per line; THOMAS takes any shape (device workspace of nx*ny*nm
- * doubles owned by the grid), PDD/PPT take at most 16 rows per partition, ceil(ny/P) <= 16 (else TDX_ERR_UNSUPPORTED: raise P).  This case is
- * synchronous (kx2/kz2 are read during the call).
+ * doubles owned by the grid); PPT takes any P (partitions of more than 16 rows are cut again inside the thread block --
+ * the result is exact either way, L156); PDD takes at most 16 rows per partition, ceil(ny/P) <= 16 (else
+ * TDX_ERR_UNSUPPORTED: raise P).  Asynchronous like the shared-matrix case: kx2 / kz2 are copied to the device (and cached
+ * by content) before the call returns.
  * rhs_inout: DEVICE, complex128 interleaved [nm][ny][nx] (x fastest) = 2*nm*ny*nx doubles; the matrix is
  * real, so re and im are two right-hand sides of one factorisation.                                       */
 tdx_status_t tdx_helmholtz_wavenumber_solve(tdx_grid_t* grid, tdx_mode_t mode, int P,
@@ -109,12 +125,12 @@ tdx_status_t tdx_helmholtz_wavenumber_solve(tdx_grid_t* grid, tdx_mode_t mode, i
  *
  * tdx_dct_x: in place on field [nz][ny][nx].  inverse == 0: X_k = sum_n x_n cos(pi k (n + 1/2) / nx), k < nx
  * (cell-centred values, Neumann walls; unnormalised).  inverse != 0: x_n = (1/nx)[X_0 + 2 sum_{k>=1} X_k cos(...)],
- * the exact inverse.  nx a power of two in [16, 4096], else TDX_ERR_UNSUPPORTED.
+ * the exact inverse.  nx = 2^k in [16, 4096] or 3*2^k in [48, 3072], else TDX_ERR_UNSUPPORTED.
  *
  * tdx_rfft_z: field_in real [nz][ny][nx] -> spec_out complex128 interleaved [nz/2+1][ny][nx] (the layout
  * tdx_helmholtz_wavenumber_solve takes), F_m = sum_k f_k exp(-2 pi i m k / nz).  tdx_irfft_z: the inverse including
  * the 1/nz (imaginary parts of F_0 and F_{nz/2} do not enter).  Out of place (in == out is TDX_ERR_INVALID_ARG); the
- * input is not modified.  nz a power of two in [16, 1024] and nx even, else TDX_ERR_UNSUPPORTED.               */
+ * input is not modified.  nz = 2^k in [16, 1024] or 3*2^k in [48, 1536], and nx even, else TDX_ERR_UNSUPPORTED.  */
 tdx_status_t tdx_dct_x(tdx_grid_t* grid, int inverse, double* field_inout, void* stream);
 tdx_status_t tdx_rfft_z(tdx_grid_t* grid, const double* field_in, double* spec_out, void* stream);
 tdx_status_t tdx_irfft_z(tdx_grid_t* grid, const double* spec_in, double* field_out, void* stream);
@@ -125,9 +141,10 @@ tdx_status_t tdx_irfft_z(tdx_grid_t* grid, const double* spec_in, double* field_
  * scratch of 2*(nz/2+1)*ny*nx doubles (caller-owned).  kx2 (HOST, nx) / kz2 (HOST, nz/2+1): the modified wavenumbers,
  * or NULL for kx2[i] = 2(1-cos(pi i/nx))/dx^2, kz2[m] = 2(1-cos(2 pi m/nz))/dz^2 of the grid's uniform x / z spacing
  * (TDX_ERR_UNSUPPORTED if that direction is not uniform).  mode / P: as tdx_helmholtz_wavenumber_solve with per-line
- * shifts (PDD/PPT need ceil(ny/P) <= 16; the paper uses PPT here because PDD is inaccurate on the weakly
- * dominant low modes, L172).  Every argument check of every stage precedes the first launch.  Synchronous
- * (returns when the solve has finished on `stream`).                                                          */
+ * shifts (PDD needs ceil(ny/P) <= 16; the paper uses PPT here because PDD is inaccurate on the weakly
+ * dominant low modes, L172).  Every argument check of every stage precedes the first launch.  Asynchronous on
+ * `stream` like every device entry point: all five stages are enqueued, nothing waits for them; kx2 / kz2 (or the
+ * grid's own wavenumbers) are on the device, cached by content, when the call returns.                        */
 tdx_status_t tdx_poisson_solve(tdx_grid_t* grid, tdx_mode_t mode, int P, const double* kx2, const double* kz2,
                                double* field_inout, double* spec_work, void* stream);
 
@@ -177,8 +194,8 @@ tdx_status_t tdx_general_solve(tdx_grid_t* grid, tdx_dir_t dir, int pivoting, co
 
 /* Batched cyclic tridiagonal solve along dir with caller-given coefficients shared by every line:
  * a, b, c: HOST arrays of n_dir doubles; a[0] couples row 0 to row n-1 and c[n-1] couples row n-1 to row 0.
- * Closure as for tdx_adi_sweep on a periodic direction (Sherman-Morrison with gamma = -b[0] for THOMAS / PDD, cyclic
- * reduced system for PPT).  rhs_inout: DEVICE, nx*ny*nz doubles. */
+ * Closure as for tdx_adi_sweep on a periodic direction (Sherman-Morrison with gamma = -b[0] for THOMAS, cyclic
+ * reduced system for PDD / PPT).  rhs_inout: DEVICE, nx*ny*nz doubles. */
 tdx_status_t tdx_cyclic_solve(tdx_grid_t* grid, tdx_dir_t dir, tdx_mode_t mode, int P,
                               const double* a, const double* b, const double* c,
                               double* rhs_inout, void* stream);
@@ -205,6 +222,10 @@ tdx_status_t tdx_step_host(tdx_grid_t* grid, tdx_mode_t mode, int Px, int Py, in
 /* Diagnostics.  tdx_pdd_dropped_bound: max over interfaces of |v_last|, |w_first| for the ADI operator of
  * (dir, P, alpha) -- the entries PDD deletes from Z; the a-priori size of the PDD error.  */
 tdx_status_t tdx_pdd_dropped_bound(tdx_grid_t* grid, tdx_dir_t dir, int P, double alpha, double* out);
+/* The last PDD / PPT sweep kernel this host thread launched: name with template arguments and launch shape, e.g.
+ * "k_strided<32,2,0,0,255,1> grid=(296,1,1) block=(8,16,1)" ("" before the first).  Thread-local, static storage.
+ * bench.py keys the committed ncu captures (profiles/) by it: a changed kernel or launch shape invalidates them.  */
+const char*  tdx_last_launch(void);
 /* Number of kernels this library has launched on this process so far (all grids). */
 long long    tdx_kernel_launch_count(void);
 const char*  tdx_status_string(tdx_status_t status);

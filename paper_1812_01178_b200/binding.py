@@ -16,10 +16,10 @@ BC_DIRICHLET, BC_PERIODIC, BC_NEUMANN = 0, 1, 2
 LOC_CENTER, LOC_FACE = 0, 1
 OK, ERR_INVALID_ARG, ERR_BAD_PARTITION, ERR_ALLOC, ERR_CUDA, ERR_UNSUPPORTED, ERR_PDD_BOUND = 0, -1, -2, -3, -4, -5, -6
 
-EXPORTS = ("tdx_grid_create", "tdx_grid_destroy", "tdx_partition_bounds", "tdx_adi_sweep", "tdx_adi_sweep_at", "tdx_adi_step",
+EXPORTS = ("tdx_grid_create", "tdx_grid_destroy", "tdx_grid_set_pdd_strict", "tdx_partition_bounds", "tdx_adi_sweep", "tdx_adi_sweep_at", "tdx_adi_step",
            "tdx_helmholtz_wavenumber_solve", "tdx_dct_x", "tdx_rfft_z", "tdx_irfft_z", "tdx_poisson_solve", "tdx_general_solve", "tdx_slab_create", "tdx_slab_destroy", "tdx_slab_eliminate", "tdx_slab_correct", "tdx_slab_dropped_bound", "tdx_cyclic_solve", "tdx_adi_sweep_host", "tdx_adi_step_host",
            "tdx_helmholtz_wavenumber_solve_host", "tdx_step_host", "tdx_pdd_dropped_bound", "tdx_kernel_launch_count",
-           "tdx_status_string", "tdx_last_error", "tdx_version")
+           "tdx_status_string", "tdx_last_error", "tdx_last_launch", "tdx_version")
 
 _dp = C.POINTER(C.c_double)
 _lib = None
@@ -44,9 +44,11 @@ def lib():
         L.tdx_status_string.restype = C.c_char_p
         L.tdx_last_error.restype = C.c_char_p
         L.tdx_version.restype = C.c_char_p
+        L.tdx_last_launch.restype = C.c_char_p
         L.tdx_kernel_launch_count.restype = C.c_longlong
         L.tdx_grid_create.argtypes = [C.c_int, C.c_int, C.c_int, _dp, _dp, _dp, C.c_int, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_void_p)]
         L.tdx_grid_destroy.argtypes = [C.c_void_p]
+        L.tdx_grid_set_pdd_strict.argtypes = [C.c_void_p, C.c_double]
         L.tdx_partition_bounds.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_int)]
         L.tdx_adi_sweep.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_double, C.c_void_p, C.c_void_p]
         L.tdx_adi_sweep_at.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_double, C.c_void_p, C.c_void_p]
@@ -78,6 +80,11 @@ def status_string(status):
 
 def last_error():
     return lib().tdx_last_error().decode()
+
+
+def last_launch():
+    """Kernel name (with template arguments) and launch shape of this thread's last PDD / PPT sweep launch."""
+    return lib().tdx_last_launch().decode()
 
 
 def version():
@@ -135,6 +142,9 @@ class Grid:
             self.close()
         except Exception:
             pass
+
+    def set_pdd_strict(self, max_dropped):
+        _chk(lib().tdx_grid_set_pdd_strict(self._h, float(max_dropped)))
 
     def adi_sweep(self, direction, mode, P, alpha, rhs, stream=0):
         _chk(lib().tdx_adi_sweep(self._h, direction, mode, P, alpha, _devptr(rhs), C.c_void_p(stream)))

@@ -29,6 +29,16 @@ namespace {
 thread_local std::string g_last_error;
 std::atomic<long long> g_launches{0};
 
+// What the last sweep launch of this host thread was (tdx_last_launch): kernel name with its template arguments and the
+// launch shape -- bench.py keys the committed ncu captures by it, so a changed kernel or launch configuration invalidates them.
+struct LaunchNote { const char* fmt = ""; int t[6] = {0, 0, 0, 0, 0, 0}; unsigned g[3] = {0, 0, 0}, b[3] = {0, 0, 0}; };
+thread_local LaunchNote g_note;
+thread_local std::string g_note_text;
+inline void note_launch(const char* fmt, int t0, int t1, int t2, int t3, int t4, int t5, dim3 grid, dim3 block) {
+    g_note.fmt = fmt; g_note.t[0] = t0; g_note.t[1] = t1; g_note.t[2] = t2; g_note.t[3] = t3; g_note.t[4] = t4; g_note.t[5] = t5;
+    g_note.g[0] = grid.x; g_note.g[1] = grid.y; g_note.g[2] = grid.z; g_note.b[0] = block.x; g_note.b[1] = block.y; g_note.b[2] = block.z;
+}
+
 tdx_status_t fail(tdx_status_t st, const char* fmt, ...) {
     char buf[512];
     va_list ap; va_start(ap, fmt); vsnprintf(buf, sizeof buf, fmt, ap); va_end(ap);
@@ -54,7 +64,8 @@ struct DevBuf {
 enum PlanKind { KIND_ADI = 0, KIND_HELM = 1, KIND_USER = 2, KIND_USERNP = 3 };   // USER: cyclic caller coefficients; USERNP: the same, not periodic
 
 struct Plan {
-    int kind = 0, dir = 0, mode = 0, P = 1, n = 0, nsets = 1;
+    int kind = 0, dir = 0, mode = 0, P = 1, n = 0, nsets = 1;   // P: KERNEL partitions per line = Pu * S
+    int Pu = 1, S = 1;      // the caller's partitions, and how many sub-partitions each is cut into (long partitions: DESIGN.md 4b)
     int loc = 0;            // unknowns of this direction at cell centres (0) or faces (1); ADI only
     int M = 0;              // register rows per partition (kernel instantiation)
     int layout = tdx::ROWS_PJ;
@@ -62,7 +73,10 @@ struct Plan {
     bool cyc = false, thomas = false;
     bool wrap = false;      // periodic line closed inside the reduced system (PDD; PPT with P <= 128) instead of Sherman-Morrison
     int sms = 148;          // SM count of the grid's device
-    mutable int pf = -1;    // L2 prefetch distance of the sweep kernel (CTAs), set at first launch
+    int dev = 0;            // the grid's device ordinal (per-device one-time kernel attributes)
+    mutable int pf = -1;    // L2 prefetch distance of the sweep kernel (CTAs) for the launch shape pf_key (recomputed when the shape changes)
+    mutable long long pf_key = -1;
+    mutable int occ = 1;    // resident CTAs per SM of that launch shape
     mutable CUtensorMap tmap;             // x sweeps: tensor map of the field as [lines*P, M] partition rows
     mutable const void* tmap_ptr = nullptr;   // field the cached tensor map was encoded for
     mutable int tmap_box = 0;
@@ -85,6 +99,10 @@ const int kMInst[] = {4, 8, 12, 16, 20, 24, 32, 48, 64};
 
 // L2 prefetch distance in waves of resident CTAs: environment TDX_L2_PREFETCH (default 1; 0 switches the prefetch off).
 // A measurement knob (profiles/ compare on/off); it never changes results.
+// cudaFuncSetAttribute(MaxDynamicSharedMemorySize) is per device: one flag per (kernel instantiation, device ordinal)
+const int kMaxDev = 64;
+struct DevOnce { bool done[kMaxDev] = {}; bool need(int dev) const { return dev < 0 || dev >= kMaxDev || !done[dev]; } void set(int dev) { if (dev >= 0 && dev < kMaxDev) done[dev] = true; } };
+
 int prefetch_waves() {
     static int w = [] { const char* e = std::getenv("TDX_L2_PREFETCH"); int v = e ? std::atoi(e) : 1; return v < 0 ? 0 : (v > 64 ? 64 : v); }();
     return w;
@@ -101,6 +119,7 @@ uint64_t fnv1a(const void* data, size_t bytes, uint64_t h = 1469598103934665603u
 struct tdx_grid {
     int nx = 0, ny = 0, nz = 0, device = 0, sms = 148;
     int bc[3] = {0, 0, 0};
+    double pdd_strict = 0.0;                            // > 0: PDD solves whose a-priori bound exceeds it return TDX_ERR_PDD_BOUND
     double* faces[3] = {nullptr, nullptr, nullptr};     // device copies
     double* lo[3] = {nullptr, nullptr, nullptr};        // metrics per direction (device), unknowns at cell centres
     double* up[3] = {nullptr, nullptr, nullptr};
@@ -111,7 +130,10 @@ struct tdx_grid {
     std::deque<Plan> plans;            // deque: references stay valid across push_back
     std::mutex mu;
     double* stage = nullptr; size_t stage_bytes = 0;    // device staging for the *_host entry points
-    double* ws = nullptr; size_t ws_bytes = 0;          // per-line Helmholtz (kx2 != 0): c' workspace + device copies of kx2, kz2
+    double* ws = nullptr; size_t ws_bytes = 0;          // per-line Helmholtz (kx2 != 0), THOMAS mode: c' workspace
+    struct WaveTab { uint64_t hash; int n; double* dev; };
+    std::vector<WaveTab> wave;                          // device copies of caller wavenumber arrays, keyed by content hash
+    bool attr_helm_lines = false;                       // cudaFuncSetAttribute done for this grid's device
     double* stage2 = nullptr; size_t stage2_bytes = 0;  // second staging buffer (Helmholtz part of tdx_step_host)
     cudaStream_t s_up = nullptr, s_comp = nullptr, s_down = nullptr;   // pipeline streams of tdx_step_host
     double length[3] = {0, 0, 0};                       // domain length per direction (host copy of faces[n] - faces[0])
@@ -124,6 +146,31 @@ struct tdx_grid {
 namespace {
 
 using namespace tdx;
+
+const int kMaxKernelP = 256;      // kernel partitions per line of a two-level plan (dense 2P x 2P reduced system at plan time)
+
+// Sub-partitions per caller's partition (1 = none).  x lines: the TMA kernel takes whole partitions of 8, 16 or 32 rows, so a
+// longer partition whose length has such a divisor is cut down to it (16 measured best, then 8, then 32); strided
+// lines: at most 32 rows per thread (two lines per thread in registers; longer partitions ran one line per thread at
+// 255 registers).  TDX_SPLIT_ROWS (measurement knob): target rows for the strided directions, 64 = never split below 64.
+int choose_split(int n, int P, int dir) {
+    static const int env_rows = [] { const char* e = std::getenv("TDX_SPLIT_ROWS"); int v = e ? std::atoi(e) : 0; return (v >= 4 && v <= 64) ? v : 0; }();
+    const int q = n / P, mo = q + (n % P ? 1 : 0);
+    if (dir == 0) {
+        if (n % P == 0) {
+            if (q == 8 || q == 16 || q == 32) return 1;
+            for (int target : {16, 8, 32})
+                if (q % target == 0 && (long long)P * (q / target) <= kMaxKernelP) return q / target;
+        }
+        if (mo <= 32) return 1;
+    } else if (mo <= (env_rows ? env_rows : 32)) return 1;
+    const int targets[2] = {env_rows ? env_rows : 32, 64};
+    for (int target : targets) {
+        const int S = (mo + target - 1) / target;
+        if (S >= 1 && (long long)P * S <= kMaxKernelP && q / S >= 2) return S;
+    }
+    return mo <= 64 ? 1 : -1;
+}
 
 int pick_M(int maxlen) {
     for (int m : kMInst) if (m >= maxlen) return m;
@@ -197,15 +244,35 @@ tdx_status_t build_plan(tdx_grid* g, Plan& pl, const double* lambda_host, const 
     DevBuf ends; CUDA_TRY(ends.alloc((size_t)nsets * P * 4 * 8));
     {
         const int nt = nsets * P;
-        k_factor<TDX_MAX_ROWS_PER_PARTITION><<<(nt + 63) / 64, 64, 0, st>>>(n, nsets, P, pl.M, pl.layout, pl.wrap ? 1 : 0, a.as<double>(), b.as<double>(),
+        k_factor<TDX_MAX_ROWS_PER_PARTITION><<<(nt + 63) / 64, 64, 0, st>>>(n, nsets, P, pl.S, pl.M, pl.layout, pl.wrap ? 1 : 0, a.as<double>(), b.as<double>(),
                                                                             c.as<double>(), qptr, flags.as<int>(), pl.rows, ends.as<double>());
         LAUNCH_CHECK("k_factor");
     }
-    pl.KB = (pl.mode == TDX_MODE_PDD) ? 4 : 2 * P;
+    pl.KB = (pl.mode == TDX_MODE_PDD && pl.S == 1) ? 4 : 2 * P;
     CUDA_TRY(cudaMalloc(&pl.G, (size_t)nsets * 2 * pl.KB * P * 8));
     CUDA_TRY(cudaMalloc(&pl.band, (size_t)nsets * P * sizeof(int2)));
     const int ntp = nsets * P;
-    if (pl.mode == TDX_MODE_PDD && pl.wrap) {
+    DevBuf oends;                                               // far spike ends of the caller's partitions (two-level plans)
+    if (pl.S > 1) {
+        // long partitions: sub-level reduced system, solved exactly (PPT) or with the caller's PDD approximation carried
+        // into it (tdx_plan.cuh, "two-level plans")
+        const int K = 2 * P, Po = pl.Pu;
+        const int pdd = pl.mode == TDX_MODE_PDD ? 1 : 0;
+        DevBuf Z, Zi, piv, scratch;
+        CUDA_TRY(Z.alloc((size_t)nsets * K * K * 8)); CUDA_TRY(Zi.alloc((size_t)nsets * K * K * 8)); CUDA_TRY(piv.alloc((size_t)nsets * K * 4));
+        CUDA_TRY(oends.alloc((size_t)nsets * Po * 4 * 8)); CUDA_TRY(scratch.alloc(tot * 8));
+        k_outer_ends<<<(nsets * Po + tb - 1) / tb, tb, 0, st>>>(n, nsets, Po, pl.wrap ? 1 : 0, a.as<double>(), b.as<double>(), c.as<double>(),
+                                                                 scratch.as<double>(), oends.as<double>());
+        LAUNCH_CHECK("k_outer_ends");
+        k_composite_factor<<<nsets, 128, 0, st>>>(P, pl.S, pl.wrap ? 1 : 0, pdd, ends.as<double>(), oends.as<double>(), Z.as<double>(), piv.as<int>());
+        LAUNCH_CHECK("k_composite_factor");
+        const long nk = (long)nsets * K;
+        k_reduced_cyclic_inverse<<<(unsigned)((nk + 63) / 64), 64, 0, st>>>(nsets, P, Z.as<double>(), piv.as<int>(), Zi.as<double>());
+        LAUNCH_CHECK("k_reduced_cyclic_inverse");
+        k_pack_ppt_cyclic<<<(ntp + 63) / 64, 64, 0, st>>>(nsets, P, pl.KB, Zi.as<double>(), pl.G, pl.band, pl.wrap ? 1 : 0);
+        LAUNCH_CHECK("k_pack_ppt_cyclic");
+        CUDA_TRY(cudaStreamSynchronize(st));
+    } else if (pl.mode == TDX_MODE_PDD && pl.wrap) {
         k_pack_pdd_cyclic<<<(ntp + tb - 1) / tb, tb, 0, st>>>(nsets, P, pl.KB, ends.as<double>(), pl.G, pl.band);
         LAUNCH_CHECK("k_pack_pdd_cyclic");
     } else if (pl.mode == TDX_MODE_PDD) {
@@ -250,6 +317,19 @@ tdx_status_t build_plan(tdx_grid* g, Plan& pl, const double* lambda_host, const 
     CUDA_TRY(cudaMemcpyAsync(he.data(), ends.p, he.size() * 8, cudaMemcpyDeviceToHost, st));
     CUDA_TRY(cudaStreamSynchronize(st));
     double dr = 0.0;
+    if (pl.S > 1) {                                             // what the caller's PDD deletes: far ends of HIS partitions
+        const int Po = pl.Pu;
+        std::vector<double> ho((size_t)nsets * Po * 4);
+        CUDA_TRY(cudaMemcpyAsync(ho.data(), oends.p, ho.size() * 8, cudaMemcpyDeviceToHost, st));
+        CUDA_TRY(cudaStreamSynchronize(st));
+        for (int s = 0; s < nsets; ++s)
+            for (int p = 0; p < Po; ++p) {
+                if (pl.wrap || (p >= 1 && p <= Po - 2)) dr = std::max(dr, std::fabs(ho[((size_t)s * Po + p) * 4 + 1]));   // v_last^(p): interface p+1 >= 2
+                if (pl.wrap || (p >= 1 && p <= Po - 2)) dr = std::max(dr, std::fabs(ho[((size_t)s * Po + p) * 4 + 2]));   // w_first^(p): interface p <= Po-2
+            }
+        pl.dropped = dr;
+        return TDX_OK;
+    }
     for (int s = 0; s < nsets; ++s) {
         if (pl.wrap) {                                              // cyclic reduced system: v_last, w_first of every partition
             for (int p = 0; p < P; ++p)
@@ -265,10 +345,19 @@ tdx_status_t build_plan(tdx_grid* g, Plan& pl, const double* lambda_host, const 
     return TDX_OK;
 }
 
+// "mode = PDD never silently falls back -- it runs as asked ... optional strict flag returns TDX_ERR_PDD_BOUND
+// when the bound > 1e-11".  The bound is matrix-only (plan time), so the refusal precedes any launch.
+tdx_status_t strict_check(const tdx_grid* g, const Plan& pl, bool enforce) {
+    if (enforce && pl.mode == TDX_MODE_PDD && !pl.thomas && g->pdd_strict > 0.0 && !(pl.dropped <= g->pdd_strict))
+        return fail(TDX_ERR_PDD_BOUND, "PDD with P=%d drops couplings of size %.3e > strict limit %.3e (PAPER.md:L152: valid when n >> p): lower P or use PPT",
+                    pl.Pu, pl.dropped, g->pdd_strict);
+    return TDX_OK;
+}
+
 // find or build
 tdx_status_t get_plan(tdx_grid* g, int kind, int dir, int mode, int P, double alpha, int nsets,
                       const double* lambda_host, const double* ua, const double* ub, const double* uc,
-                      cudaStream_t st, Plan** out, int loc = 0) {
+                      cudaStream_t st, Plan** out, int loc = 0, bool enforce_strict = true) {
     const int n = (kind == KIND_HELM) ? g->ny : g->n_of(dir);
     if (n < 2) return fail(TDX_ERR_INVALID_ARG, "line length %d < 2", n);
     bool thomas = (mode == TDX_MODE_THOMAS) || P == 1;
@@ -278,38 +367,45 @@ tdx_status_t get_plan(tdx_grid* g, int kind, int dir, int mode, int P, double al
     if (thomas) { P = 1; mode = TDX_MODE_THOMAS; }
     const bool periodic = (kind == KIND_USER) || (kind == KIND_ADI && g->bc[dir] == TDX_BC_PERIODIC);
     if (periodic && n < 3) return fail(TDX_ERR_INVALID_ARG, "periodic line needs n >= 3");
+    // Long partitions (more rows than a thread keeps in registers, or a shape the fast kernels do not take): every partition is
+    // cut again into S sub-partitions and the sweep runs with P * S kernel partitions (two-level plans, tdx_plan.cuh).
+    const int Pu = P;
+    int S = 1, M = 0;
+    if (!thomas) {
+        S = choose_split(n, P, kind == KIND_HELM ? 1 : dir);
+        if (S < 1) return fail(TDX_ERR_UNSUPPORTED, "P=%d partitions of %d rows: more than %d sub-partitions per line would be needed", P, n / P + (n % P ? 1 : 0), kMaxKernelP);
+        const int q = n / P, mo = q + (n % P ? 1 : 0);
+        const int maxlen = S > 1 ? mo / S + (mo % S ? 1 : 0) : mo;
+        M = pick_M(maxlen);
+        if (M < 0) return fail(TDX_ERR_UNSUPPORTED, "rows per partition %d > %d", maxlen, TDX_MAX_ROWS_PER_PARTITION);
+        if (S > 1 && q / S < 2) return fail(TDX_ERR_BAD_PARTITION, "P=%d invalid for line length %d", P, n);
+    }
     // PDD and PPT close a periodic line inside the (then cyclic) reduced system: the wrap corners join Delta A, P interfaces
     // (Eq.(3)-(4) with rank 2P; PPT needs the dense 2P x 2P inverse at plan time, hence P <= 128).  Thomas, and PPT with
     // more partitions, use the rank-1 Sherman-Morrison split.
-    const bool wrap = periodic && !thomas && P >= 2 && (mode == TDX_MODE_PDD || P <= 128);
+    const bool wrap = periodic && !thomas && P >= 2 && (mode == TDX_MODE_PDD || P <= 128 || S > 1);
     const bool cyc = periodic && !wrap;
-    int M = 0;
-    if (!thomas) {
-        const int maxlen = n / P + (n % P ? 1 : 0);
-        M = pick_M(maxlen);
-        if (M < 0) return fail(TDX_ERR_UNSUPPORTED, "rows per partition %d > %d: raise P", maxlen, TDX_MAX_ROWS_PER_PARTITION);
-    }
     uint64_t h = 0;
     if (kind == KIND_HELM) h = fnv1a(lambda_host, (size_t)nsets * 8);
     if (kind == KIND_USER || kind == KIND_USERNP) { h = fnv1a(ua, (size_t)n * 8); h = fnv1a(ub, (size_t)n * 8, h); h = fnv1a(uc, (size_t)n * 8, h); }
     std::lock_guard<std::mutex> lk(g->mu);
     for (Plan& p : g->plans)
-        if (p.kind == kind && p.dir == dir && p.loc == loc && p.mode == mode && p.P == P && p.nsets == nsets && p.hash == h &&
-            std::memcmp(&p.alpha, &alpha, 8) == 0) { *out = &p; return TDX_OK; }
+        if (p.kind == kind && p.dir == dir && p.loc == loc && p.mode == mode && p.Pu == Pu && p.nsets == nsets && p.hash == h &&
+            std::memcmp(&p.alpha, &alpha, 8) == 0) { *out = &p; return strict_check(g, p, enforce_strict); }
     Plan pl;
-    pl.kind = kind; pl.dir = dir; pl.mode = mode; pl.P = P; pl.n = n; pl.nsets = nsets; pl.M = M; pl.cyc = cyc; pl.wrap = wrap;
-    pl.thomas = thomas; pl.alpha = alpha; pl.hash = h; pl.sms = g->sms; pl.loc = loc;
+    pl.kind = kind; pl.dir = dir; pl.mode = mode; pl.P = Pu * S; pl.Pu = Pu; pl.S = S; pl.n = n; pl.nsets = nsets; pl.M = M; pl.cyc = cyc; pl.wrap = wrap;
+    pl.thomas = thomas; pl.alpha = alpha; pl.hash = h; pl.sms = g->sms; pl.dev = g->device; pl.loc = loc;
     tdx_status_t rc = build_plan(g, pl, lambda_host, ua, ub, uc, st);
     if (rc != TDX_OK) { pl.release(); return rc; }
     g->plans.push_back(pl);
     *out = &g->plans.back();
-    return TDX_OK;
+    return strict_check(g, g->plans.back(), enforce_strict);
 }
 
 Tables tables_of(const Plan& pl) {
     Tables T;
     T.rows = pl.rows; T.G = pl.G; T.band = pl.band; T.Sidx = pl.Sidx; T.Sval = pl.Sval; T.Sn = pl.Sn;
-    T.P = pl.P; T.n = pl.n; T.q = pl.n / pl.P; T.r = pl.n % pl.P; T.KB = pl.KB; T.Scap = pl.Scap;
+    T.P = pl.P; T.n = pl.n; T.q = pl.n / pl.Pu; T.r = pl.n % pl.Pu; T.S = pl.S; T.KB = pl.KB; T.Scap = pl.Scap;
     return T;
 }
 
@@ -320,15 +416,18 @@ namespace {
 
 template <int M, int V, bool CYC, bool UNI = false, int REGS = strided_regs(M, V)>
 tdx_status_t launch_strided_inst(const Plan& pl, StridedArgs& A, const Tables& T, dim3 grid, dim3 block, size_t smem, cudaStream_t st) {
-    static bool attr_done = false;
-    if (!attr_done && smem > 48 * 1024) {
+    static DevOnce attr;
+    if (smem > 48 * 1024 && attr.need(pl.dev)) {
         CUDA_TRY(cudaFuncSetAttribute(k_strided<M, V, CYC, UNI, REGS>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
-        attr_done = true;
+        attr.set(pl.dev);
     }
-    if (pl.pf < 0) {                                               // prefetch one wave of resident CTAs ahead
+    const long long key = ((long long)(block.x * block.y) << 32) | ((long long)smem << 4) | (V << 1) | (REGS == strided_regs(M, V) ? 0 : 1);
+    if (pl.pf < 0 || pl.pf_key != key) {                           // prefetch one wave of resident CTAs ahead
         int occ = 1;
         CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_strided<M, V, CYC, UNI, REGS>, (int)(block.x * block.y), smem));
-        pl.pf = pl.sms * (occ < 1 ? 1 : occ) * prefetch_waves();
+        pl.occ = occ < 1 ? 1 : occ;
+        pl.pf = pl.sms * pl.occ * prefetch_waves();
+        pl.pf_key = key;
     }
     // one tile per CTA: pf = CTAs ahead; looping CTAs (grid.x < tiles_x): pf = sets ahead for the first tile of a later CTA
     A.pf = ((int)grid.x == A.tiles_x) ? pl.pf : (pl.pf > 0 ? (pl.pf + (int)grid.x - 1) / (int)grid.x : 0);
@@ -343,6 +442,7 @@ tdx_status_t launch_strided_inst(const Plan& pl, StridedArgs& A, const Tables& T
     } else std::memset(U.v, 0, sizeof(U.v));
     k_strided<M, V, CYC, UNI, REGS><<<grid, block, smem, st>>>(A, T, U);
     LAUNCH_CHECK("k_strided");
+    note_launch("k_strided<%d,%d,%d,%d,%d>", M, V, CYC, UNI, REGS, 0, grid, block);
     return TDX_OK;
 }
 
@@ -377,6 +477,16 @@ tdx_status_t launch_strided_M(const Plan& pl, StridedArgs& A, const Tables& T, d
 // register tile of k_helm_lines for ceil(n / P) rows per partition: 8, 12 or 16 (0: does not fit)
 int helm_lines_M(int n, int P) { const int mx = (n + P - 1) / P; return mx <= 8 ? 8 : (mx <= 12 ? 12 : (mx <= 16 ? 16 : 0)); }
 
+// kernel partitions of k_helm_lines for the caller's P: P itself when its partitions fit the 16-row register tile; PPT is exact
+// for any partitioning, so longer partitions are cut again (P * S partitions); PDD is not (0 = unsupported).
+int helm_lines_P(int n, int P, int mode) {
+    if (helm_lines_M(n, P)) return P;
+    if (mode != TDX_MODE_PPT) return 0;
+    const int mo = (n + P - 1) / P;
+    for (int S = (mo + 15) / 16; P * S <= 512 && n / (P * S) >= 2; ++S) if (helm_lines_M(n, P * S)) return P * S;
+    return 0;
+}
+
 int pow2floor(long long v) { int p = 1; while ((long long)p * 2 <= v) p *= 2; return p; }
 
 // lines of `dir` in a field whose x extent is `nxe` doubles (nx for real fields, 2 nx for complex ones)
@@ -403,7 +513,7 @@ tdx_status_t run_strided(const Plan& pl, double* data, long long W, long long li
     // Rows far apart in memory (z lines: stride = one xy-plane) like longer row segments; measured on cfg5 z.
     static const int env_row = [] { const char* e = std::getenv("TDX_ROW_DOUBLES"); return e ? std::atoi(e) : 0; }();
     int row_doubles = (line_stride * 8 >= (1 << 20)) ? 32 : 16;
-    const bool fat = set_per_outer && pl.M >= 32;             // 255-register instantiation, one table set per outer index: measured on cfg4 Helmholtz
+    const bool fat = set_per_outer && pl.M >= 32;   // 255-register instantiation, one table set per outer index: measured on cfg4 Helmholtz
     if (fat) row_doubles = 32;                                //   256-byte rows + 8 tiles per CTA 0.389 ms against 0.406 (128-byte rows, 4 tiles)
     if (env_row == 16 || env_row == 32 || env_row == 64) row_doubles = env_row;
     // 32-row partitions with the table in the constant bank fit 168 registers: up to 384 threads, so 17..24 partitions
@@ -447,29 +557,30 @@ tdx_status_t run_strided(const Plan& pl, double* data, long long W, long long li
 }
 
 template <int M, bool UNI, bool CYC>
-tdx_status_t launch_unit_inst(const UnitArgs& A, const Tables& T, unsigned grid, int threads, size_t smem, cudaStream_t st) {
-    static bool attr_done = false;
-    if (!attr_done) {
+tdx_status_t launch_unit_inst(const UnitArgs& A, const Tables& T, unsigned grid, int threads, size_t smem, cudaStream_t st, int dev) {
+    static DevOnce attr;
+    if (attr.need(dev)) {
         CUDA_TRY(cudaFuncSetAttribute(k_unit<M, UNI, CYC>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
-        attr_done = true;
+        attr.set(dev);
     }
     k_unit<M, UNI, CYC><<<grid, threads, smem, st>>>(A, T);
     LAUNCH_CHECK("k_unit");
+    note_launch("k_unit<%d,%d,%d>", M, UNI, CYC, 0, 0, 0, dim3(grid), dim3(threads));
     return TDX_OK;
 }
 
 template <bool UNI, bool CYC>
-tdx_status_t launch_unit_M(int M, const UnitArgs& A, const Tables& T, unsigned grid, int threads, size_t smem, cudaStream_t st) {
+tdx_status_t launch_unit_M(int M, const UnitArgs& A, const Tables& T, unsigned grid, int threads, size_t smem, cudaStream_t st, int dev) {
     switch (M) {
-        case 4: return launch_unit_inst<4, UNI, CYC>(A, T, grid, threads, smem, st);
-        case 8: return launch_unit_inst<8, UNI, CYC>(A, T, grid, threads, smem, st);
-        case 12: return launch_unit_inst<12, UNI, CYC>(A, T, grid, threads, smem, st);
-        case 16: return launch_unit_inst<16, UNI, CYC>(A, T, grid, threads, smem, st);
-        case 20: return launch_unit_inst<20, UNI, CYC>(A, T, grid, threads, smem, st);
-        case 24: return launch_unit_inst<24, UNI, CYC>(A, T, grid, threads, smem, st);
-        case 32: return launch_unit_inst<32, UNI, CYC>(A, T, grid, threads, smem, st);
-        case 48: return launch_unit_inst<48, UNI, CYC>(A, T, grid, threads, smem, st);
-        case 64: return launch_unit_inst<64, UNI, CYC>(A, T, grid, threads, smem, st);
+        case 4: return launch_unit_inst<4, UNI, CYC>(A, T, grid, threads, smem, st, dev);
+        case 8: return launch_unit_inst<8, UNI, CYC>(A, T, grid, threads, smem, st, dev);
+        case 12: return launch_unit_inst<12, UNI, CYC>(A, T, grid, threads, smem, st, dev);
+        case 16: return launch_unit_inst<16, UNI, CYC>(A, T, grid, threads, smem, st, dev);
+        case 20: return launch_unit_inst<20, UNI, CYC>(A, T, grid, threads, smem, st, dev);
+        case 24: return launch_unit_inst<24, UNI, CYC>(A, T, grid, threads, smem, st, dev);
+        case 32: return launch_unit_inst<32, UNI, CYC>(A, T, grid, threads, smem, st, dev);
+        case 48: return launch_unit_inst<48, UNI, CYC>(A, T, grid, threads, smem, st, dev);
+        case 64: return launch_unit_inst<64, UNI, CYC>(A, T, grid, threads, smem, st, dev);
     }
     return fail(TDX_ERR_UNSUPPORTED, "no unit-stride kernel for M=%d", M);
 }
@@ -490,15 +601,17 @@ EncodeTiledFn encode_tiled_fn() {
 
 template <int M, bool UNI, bool CYC>
 tdx_status_t launch_unit_tma_inst(const Plan& pl, UnitTmaArgs& A, const Tables& T, unsigned grid, int threads, size_t smem, cudaStream_t st) {
-    static bool attr_done = false;
-    if (!attr_done) {
+    static DevOnce attr;
+    if (attr.need(pl.dev)) {
         CUDA_TRY(cudaFuncSetAttribute(k_unit_tma<M, UNI, CYC>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
-        attr_done = true;
+        attr.set(pl.dev);
     }
-    if (pl.pf < 0) {
+    const long long key = ((long long)threads << 32) | (long long)smem;
+    if (pl.pf < 0 || pl.pf_key != key) {
         int occ = 1;
         CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_unit_tma<M, UNI, CYC>, threads, smem));
         pl.pf = pl.sms * (occ < 1 ? 1 : occ) * prefetch_waves();
+        pl.pf_key = key;
     }
     A.pf = pl.pf;
     UniTable<M> U;
@@ -512,6 +625,7 @@ tdx_status_t launch_unit_tma_inst(const Plan& pl, UnitTmaArgs& A, const Tables& 
     } else std::memset(U.v, 0, sizeof(U.v));
     k_unit_tma<M, UNI, CYC><<<grid, threads, smem, st>>>(pl.tmap, A, T, U);
     LAUNCH_CHECK("k_unit_tma");
+    note_launch("k_unit_tma<%d,%d,%d>", M, UNI, CYC, 0, 0, 0, dim3(grid), dim3(threads));
     return TDX_OK;
 }
 
@@ -599,8 +713,8 @@ tdx_status_t run_unit(const Plan& pl, double* data, long long nlines, cudaStream
     const unsigned grid = (unsigned)((nlines + A.LPB - 1) / A.LPB);
     Tables T = tables_of(pl);
     const bool uni = pl.layout == ROWS_U;
-    if (uni) return pl.cyc ? launch_unit_M<true, true>(pl.M, A, T, grid, threads, smem, st) : launch_unit_M<true, false>(pl.M, A, T, grid, threads, smem, st);
-    return pl.cyc ? launch_unit_M<false, true>(pl.M, A, T, grid, threads, smem, st) : launch_unit_M<false, false>(pl.M, A, T, grid, threads, smem, st);
+    if (uni) return pl.cyc ? launch_unit_M<true, true>(pl.M, A, T, grid, threads, smem, st, pl.dev) : launch_unit_M<true, false>(pl.M, A, T, grid, threads, smem, st, pl.dev);
+    return pl.cyc ? launch_unit_M<false, true>(pl.M, A, T, grid, threads, smem, st, pl.dev) : launch_unit_M<false, false>(pl.M, A, T, grid, threads, smem, st, pl.dev);
 }
 
 // ncomp fields of the grid's shape stored back to back are just a longer batch: more x lines, more outer planes for
@@ -620,6 +734,29 @@ void trim_plans(tdx_grid* g) {
     const size_t kMaxPlans = 64, kKeep = 48;
     if (g->plans.size() <= kMaxPlans) return;
     while (g->plans.size() > kKeep) { g->plans.front().release(); g->plans.pop_front(); }
+}
+
+// Device copy of a caller's HOST wavenumber array, cached by content (as plans are): the per-line Helmholtz solve and the
+// Poisson solve then stay asynchronous -- the array is read before the call returns only on a cache miss.
+tdx_status_t wavenumbers_on_device(tdx_grid* g, const double* host, int n, cudaStream_t st, const double** out) {
+    const uint64_t h = fnv1a(host, (size_t)n * 8);
+    std::lock_guard<std::mutex> lk(g->mu);
+    for (auto& w : g->wave) if (w.hash == h && w.n == n) { *out = w.dev; return TDX_OK; }
+    if (g->wave.size() >= 16) {                                    // oldest out; cudaFree waits for kernels that still read it
+        cudaFree(g->wave.front().dev);
+        g->wave.erase(g->wave.begin());
+    }
+    double* d = nullptr;
+    if (cudaMalloc(&d, (size_t)n * 8) != cudaSuccess) { cudaGetLastError(); return fail(TDX_ERR_ALLOC, "wavenumber table allocation failed"); }
+    // pageable source: the runtime stages the data before returning, so the caller's array is not read afterwards
+    cudaError_t e = cudaMemcpyAsync(d, host, (size_t)n * 8, cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) { cudaFree(d); return fail(TDX_ERR_CUDA, "wavenumber upload failed: %s", cudaGetErrorString(e)); }
+    // other streams may use the cached table later: make the upload complete now (once per distinct array)
+    e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) { cudaFree(d); return fail(TDX_ERR_CUDA, "wavenumber upload failed: %s", cudaGetErrorString(e)); }
+    g->wave.push_back({h, n, d});
+    *out = d;
+    return TDX_OK;
 }
 
 tdx_status_t check_common(tdx_grid* g, int dir, int mode, const void* ptr) {
@@ -648,6 +785,8 @@ tdx_status_t fft_tables(tdx_grid* g, int dir, cudaStream_t st) {
     if (dir == 0 && cudaMalloc(&w4, (size_t)(N / 2 + 1) * 16) != cudaSuccess) { cudaGetLastError(); cudaFree(tw); return fail(TDX_ERR_ALLOC, "twiddle table allocation failed"); }
     tdx::k_fft_tables<<<(N + 127) / 128, 128, 0, st>>>(tw, w4, N);
     LAUNCH_CHECK("k_fft_tables");
+    // once per grid and direction: other streams may run the next transform, so the tables are complete before they are published
+    if (cudaStreamSynchronize(st) != cudaSuccess) { cudaFree(tw); cudaFree(w4); return fail(TDX_ERR_CUDA, "twiddle table kernel failed: %s", cudaGetErrorString(cudaGetLastError())); }
     g->fft_tw[dir] = tw;
     if (dir == 0) g->fft_w4 = w4;
     return TDX_OK;
@@ -661,13 +800,13 @@ tdx_status_t launch_fft_z(tdx_grid* g, const double* in, double* out, bool inver
     const int resident = std::max(1, std::min((int)(220 * 1024 / smem), 2048 / (C * N / K)));
     const int pf = g->sms * resident * std::min(WAVES, prefetch_waves());
     if (!inverse) {
-        static bool done = false;
-        if (!done) { CUDA_TRY(cudaFuncSetAttribute(k_rfft_z<N, C, K>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); done = true; }
+        static DevOnce attr;
+        if (attr.need(g->device)) { CUDA_TRY(cudaFuncSetAttribute(k_rfft_z<N, C, K>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); attr.set(g->device); }
         k_rfft_z<N, C, K><<<grid, block, smem, st>>>(in, reinterpret_cast<double2*>(out), g->nx, g->ny, g->fft_tw[2], pf);
         LAUNCH_CHECK("k_rfft_z");
     } else {
-        static bool done = false;
-        if (!done) { CUDA_TRY(cudaFuncSetAttribute(k_irfft_z<N, C, K>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); done = true; }
+        static DevOnce attr;
+        if (attr.need(g->device)) { CUDA_TRY(cudaFuncSetAttribute(k_irfft_z<N, C, K>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); attr.set(g->device); }
         k_irfft_z<N, C, K><<<grid, block, smem, st>>>(reinterpret_cast<const double2*>(in), out, g->nx, g->ny, g->fft_tw[2], pf);
         LAUNCH_CHECK("k_irfft_z");
     }
@@ -684,13 +823,13 @@ tdx_status_t launch_fft_z3(tdx_grid* g, const double* in, double* out, bool inve
     const size_t smem = (size_t)N * C * 16;
     dim3 block(C, N / 24), grid((g->nx + 2 * C - 1) / (2 * C), g->ny);
     if (!inverse) {
-        static bool done = false;
-        if (!done) { CUDA_TRY(cudaFuncSetAttribute(k_rfft_z3<N, C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); done = true; }
+        static DevOnce attr;
+        if (attr.need(g->device)) { CUDA_TRY(cudaFuncSetAttribute(k_rfft_z3<N, C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); attr.set(g->device); }
         k_rfft_z3<N, C><<<grid, block, smem, st>>>(in, reinterpret_cast<double2*>(out), g->nx, g->ny, g->fft_tw[2]);
         LAUNCH_CHECK("k_rfft_z3");
     } else {
-        static bool done = false;
-        if (!done) { CUDA_TRY(cudaFuncSetAttribute(k_irfft_z3<N, C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); done = true; }
+        static DevOnce attr;
+        if (attr.need(g->device)) { CUDA_TRY(cudaFuncSetAttribute(k_irfft_z3<N, C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); attr.set(g->device); }
         k_irfft_z3<N, C><<<grid, block, smem, st>>>(reinterpret_cast<const double2*>(in), out, g->nx, g->ny, g->fft_tw[2]);
         LAUNCH_CHECK("k_irfft_z3");
     }
@@ -736,12 +875,12 @@ tdx_status_t launch_dct_x(tdx_grid* g, double* field, bool inverse, cudaStream_t
     const int resident = std::max(1, std::min((int)(220 * 1024 / smem), 2048 / (LP * N / K)));
     const int pf = g->sms * resident * prefetch_waves();
     if (!inverse) {
-        static bool done = false;
-        if (!done) { CUDA_TRY(cudaFuncSetAttribute(k_dct_x<N, LP, 0, K>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); done = true; }
+        static DevOnce attr;
+        if (attr.need(g->device)) { CUDA_TRY(cudaFuncSetAttribute(k_dct_x<N, LP, 0, K>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); attr.set(g->device); }
         k_dct_x<N, LP, 0, K><<<(unsigned)ctas, LP * N / K, smem, st>>>(field, lines, g->fft_tw[0], g->fft_w4, pf);
     } else {
-        static bool done = false;
-        if (!done) { CUDA_TRY(cudaFuncSetAttribute(k_dct_x<N, LP, 1, K>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); done = true; }
+        static DevOnce attr;
+        if (attr.need(g->device)) { CUDA_TRY(cudaFuncSetAttribute(k_dct_x<N, LP, 1, K>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); attr.set(g->device); }
         k_dct_x<N, LP, 1, K><<<(unsigned)ctas, LP * N / K, smem, st>>>(field, lines, g->fft_tw[0], g->fft_w4, pf);
     }
     LAUNCH_CHECK("k_dct_x");
@@ -757,12 +896,12 @@ tdx_status_t launch_dct_x3(tdx_grid* g, double* field, bool inverse, cudaStream_
     const int resident = std::max(1, std::min((int)(220 * 1024 / smem), 2048 / (LP * N / 24)));
     const int pf = g->sms * resident * prefetch_waves();
     if (!inverse) {
-        static bool done = false;
-        if (!done) { CUDA_TRY(cudaFuncSetAttribute(k_dct_x3<N, LP, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); done = true; }
+        static DevOnce attr;
+        if (attr.need(g->device)) { CUDA_TRY(cudaFuncSetAttribute(k_dct_x3<N, LP, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); attr.set(g->device); }
         k_dct_x3<N, LP, 0><<<(unsigned)ctas, LP * N / 24, smem, st>>>(field, lines, g->fft_tw[0], g->fft_w4, pf);
     } else {
-        static bool done = false;
-        if (!done) { CUDA_TRY(cudaFuncSetAttribute(k_dct_x3<N, LP, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); done = true; }
+        static DevOnce attr;
+        if (attr.need(g->device)) { CUDA_TRY(cudaFuncSetAttribute(k_dct_x3<N, LP, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); attr.set(g->device); }
         k_dct_x3<N, LP, 1><<<(unsigned)ctas, LP * N / 24, smem, st>>>(field, lines, g->fft_tw[0], g->fft_w4, pf);
     }
     LAUNCH_CHECK("k_dct_x3");
@@ -828,6 +967,13 @@ extern "C" {
 
 const char* tdx_version(void) { return "tdx 0.1 (sm_100a)"; }
 const char* tdx_last_error(void) { return g_last_error.c_str(); }
+const char* tdx_last_launch(void) {
+    char name[128], buf[256];
+    snprintf(name, sizeof name, g_note.fmt, g_note.t[0], g_note.t[1], g_note.t[2], g_note.t[3], g_note.t[4], g_note.t[5]);
+    snprintf(buf, sizeof buf, "%s grid=(%u,%u,%u) block=(%u,%u,%u)", name, g_note.g[0], g_note.g[1], g_note.g[2], g_note.b[0], g_note.b[1], g_note.b[2]);
+    g_note_text = buf;
+    return g_note_text.c_str();
+}
 long long tdx_kernel_launch_count(void) { return g_launches.load(); }
 
 const char* tdx_status_string(tdx_status_t s) {
@@ -912,12 +1058,20 @@ tdx_status_t tdx_grid_destroy(tdx_grid_t* g) {
     for (Plan& p : g->plans) p.release();
     for (int d = 0; d < 3; ++d) { cudaFree(g->faces[d]); cudaFree(g->lo[d]); cudaFree(g->up[d]); cudaFree(g->lo_face[d]); cudaFree(g->up_face[d]); }
     cudaFree(g->lo_neumann_y); cudaFree(g->up_neumann_y); cudaFree(g->stage); cudaFree(g->stage2); cudaFree(g->ws);
+    for (auto& w : g->wave) cudaFree(w.dev);
     for (int d = 0; d < 3; ++d) cudaFree(g->fft_tw[d]);
     cudaFree(g->fft_w4);
     if (g->s_up) cudaStreamDestroy(g->s_up);
     if (g->s_comp) cudaStreamDestroy(g->s_comp);
     if (g->s_down) cudaStreamDestroy(g->s_down);
     delete g;
+    return TDX_OK;
+}
+
+tdx_status_t tdx_grid_set_pdd_strict(tdx_grid_t* g, double max_dropped) {
+    if (!g) return fail(TDX_ERR_INVALID_ARG, "grid is NULL");
+    if (!(max_dropped >= 0.0)) return fail(TDX_ERR_INVALID_ARG, "max_dropped must be >= 0 (0 switches the check off)");
+    g->pdd_strict = max_dropped;
     return TDX_OK;
 }
 
@@ -1004,63 +1158,70 @@ tdx_status_t tdx_helmholtz_wavenumber_solve(tdx_grid_t* g, tdx_mode_t mode, int 
         bool any = false;
         for (int i = 0; i < g->nx; ++i) { if (!(kx2[i] >= 0.0)) return fail(TDX_ERR_INVALID_ARG, "kx2[%d] is negative or NaN", i); any |= kx2[i] != 0.0; }
         if (any) {
-            // per-line matrices: only the on-the-fly Thomas baseline is built (PPT/PDD per line: SURVEY 8(f) N2/N4)
+            // per-line matrices (the paper's cosine-x / Fourier-z solve, L45, L170-174): factorisation, spikes and reduced
+            // system on the fly in k_helm_lines (PDD / PPT) or k_thomas_helm_lines (two-pass baseline)
             const int ny = g->ny;
-            int Mh = 0;
+            int Mh = 0, Pk = P;
             if (mode != TDX_MODE_THOMAS) {
                 if (P < 2 || P > TDX_MAX_P || ny / P < 2) return fail(TDX_ERR_BAD_PARTITION, "P=%d invalid for line length %d", P, ny);
-                Mh = helm_lines_M(ny, P);
-                if (!Mh) return fail(TDX_ERR_UNSUPPORTED, "per-line shifts (non-zero kx2) in PDD/PPT mode take at most 16 rows per partition: raise P; ny=%d P=%d", ny, P);
+                Pk = helm_lines_P(ny, P, mode);
+                if (!Pk) return fail(TDX_ERR_UNSUPPORTED, "per-line shifts (non-zero kx2) in PDD mode take at most 16 rows per partition: raise P or use PPT; ny=%d P=%d", ny, P);
+                Mh = helm_lines_M(ny, Pk);
             }
             CUDA_TRY(cudaSetDevice(g->device));
             cudaStream_t st = static_cast<cudaStream_t>(stream);
-            const size_t wsb = (mode == TDX_MODE_THOMAS) ? (size_t)g->nx * g->ny * nm * 8 : 0;
-            std::lock_guard<std::mutex> lk(g->mu);
-            if (g->ws_bytes < wsb + (size_t)(g->nx + nm) * 8) {
-                cudaFree(g->ws); g->ws = nullptr; g->ws_bytes = 0;
-                if (cudaMalloc(&g->ws, wsb + (size_t)(g->nx + nm) * 8) != cudaSuccess) { cudaGetLastError(); return fail(TDX_ERR_ALLOC, "workspace allocation of %zu bytes failed", wsb); }
-                g->ws_bytes = wsb + (size_t)(g->nx + nm) * 8;
+            if (mode == TDX_MODE_PDD && g->pdd_strict > 0.0) {     // strict PDD: the least dominant line (smallest shift) has the slowest spikes
+                double lmin = *std::min_element(kx2, kx2 + g->nx) + *std::min_element(kz2, kz2 + nm);
+                Plan* pb = nullptr;
+                rc = get_plan(g, KIND_HELM, TDX_DIR_Y, TDX_MODE_PDD, P, 0.0, 1, &lmin, nullptr, nullptr, nullptr, st, &pb);
+                if (rc != TDX_OK) return rc;
             }
-            double* dkx = g->ws + wsb / 8;
-            double* dkz = dkx + g->nx;
-            CUDA_TRY(cudaMemcpyAsync(dkx, kx2, (size_t)g->nx * 8, cudaMemcpyHostToDevice, st));
-            CUDA_TRY(cudaMemcpyAsync(dkz, kz2, (size_t)nm * 8, cudaMemcpyHostToDevice, st));
+            const double *dkx = nullptr, *dkz = nullptr;
+            rc = wavenumbers_on_device(g, kx2, g->nx, st, &dkx);  if (rc != TDX_OK) return rc;
+            rc = wavenumbers_on_device(g, kz2, nm, st, &dkz);      if (rc != TDX_OK) return rc;
             if (mode != TDX_MODE_THOMAS) {
                 const int regs = Mh <= 8 ? 128 : (Mh <= 12 ? 168 : 208);
                 int lpc = 8;
-                while (lpc > 1 && (lpc * P > 1024 || lpc * P * regs > 65536)) lpc /= 2;
-                if (lpc * P > 1024 || lpc * P * regs > 65536) return fail(TDX_ERR_UNSUPPORTED, "P=%d partitions do not fit one thread block", P);
-                dim3 block(lpc, P), grid((g->nx + lpc - 1) / lpc, nm);
+                while (lpc > 1 && (lpc * Pk > 1024 || lpc * Pk * regs > 65536)) lpc /= 2;
+                if (lpc * Pk > 1024 || lpc * Pk * regs > 65536) return fail(TDX_ERR_UNSUPPORTED, "P=%d partitions do not fit one thread block", Pk);
+                dim3 block(lpc, Pk), grid((g->nx + lpc - 1) / lpc, nm);
                 if (grid.y > 65535) return fail(TDX_ERR_UNSUPPORTED, "nm > 65535");
-                const size_t smem = (size_t)30 * P * lpc * 8;          // interface values 8, y0/y1 4, PCR buffers 2 x 9 (tdx_kernels.cuh)
+                const size_t smem = (size_t)30 * Pk * lpc * 8;         // interface values 8, y0/y1 4, PCR buffers 2 x 9 (tdx_kernels.cuh)
                 const int ppt = mode == TDX_MODE_PPT ? 1 : 0;
                 const int pf = g->sms * 2 * prefetch_waves();
                 double2* d2 = reinterpret_cast<double2*>(rhs);
-                static bool attr_done = false;
-                if (!attr_done) {
+                if (!g->attr_helm_lines) {
                     CUDA_TRY(cudaFuncSetAttribute(k_helm_lines<8, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024));
                     CUDA_TRY(cudaFuncSetAttribute(k_helm_lines<12, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024));
                     CUDA_TRY(cudaFuncSetAttribute(k_helm_lines<16, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024));
                     CUDA_TRY(cudaFuncSetAttribute(k_helm_lines<8, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024));
                     CUDA_TRY(cudaFuncSetAttribute(k_helm_lines<12, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024));
                     CUDA_TRY(cudaFuncSetAttribute(k_helm_lines<16, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024));
-                    attr_done = true;
+                    g->attr_helm_lines = true;
                 }
-                const int hq = ny / P, hr = ny % P;
+                const int hq = ny / Pk, hr = ny % Pk;
                 const bool rag = hr != 0 || hq != Mh;              // partitions shorter than the register tile: padding rows
-#define TDX_HELM_LINES(MM, RR) k_helm_lines<MM, RR><<<grid, block, smem, st>>>(d2, g->nx, ny, P, hq, hr, ppt, pf, g->lo_neumann_y, g->up_neumann_y, dkx, dkz)
+#define TDX_HELM_LINES(MM, RR) k_helm_lines<MM, RR><<<grid, block, smem, st>>>(d2, g->nx, ny, Pk, hq, hr, ppt, pf, g->lo_neumann_y, g->up_neumann_y, dkx, dkz)
                 if (Mh == 8) { if (rag) TDX_HELM_LINES(8, true); else TDX_HELM_LINES(8, false); }
                 else if (Mh == 12) { if (rag) TDX_HELM_LINES(12, true); else TDX_HELM_LINES(12, false); }
                 else { if (rag) TDX_HELM_LINES(16, true); else TDX_HELM_LINES(16, false); }
 #undef TDX_HELM_LINES
                 LAUNCH_CHECK("k_helm_lines");
-                CUDA_TRY(cudaStreamSynchronize(st));
+                note_launch("k_helm_lines<%d,%d>", Mh, rag ? 1 : 0, 0, 0, 0, 0, grid, block);
                 return TDX_OK;
+            }
+            const size_t wsb = (size_t)g->nx * g->ny * nm * 8;
+            {
+                std::lock_guard<std::mutex> lk(g->mu);
+                if (g->ws_bytes < wsb) {
+                    cudaFree(g->ws); g->ws = nullptr; g->ws_bytes = 0;      // cudaFree waits for work in flight
+                    if (cudaMalloc(&g->ws, wsb) != cudaSuccess) { cudaGetLastError(); return fail(TDX_ERR_ALLOC, "workspace allocation of %zu bytes failed", wsb); }
+                    g->ws_bytes = wsb;
+                }
             }
             dim3 grid((g->nx + 127) / 128, nm);
             k_thomas_helm_lines<<<grid, 128, 0, st>>>(reinterpret_cast<double2*>(rhs), g->ws, g->nx, g->ny, g->lo_neumann_y, g->up_neumann_y, dkx, dkz);
             LAUNCH_CHECK("k_thomas_helm_lines");
-            CUDA_TRY(cudaStreamSynchronize(st));               // kx2/kz2 are read from host memory during the call
             return TDX_OK;
         }
     }
@@ -1098,8 +1259,8 @@ tdx_status_t tdx_poisson_solve(tdx_grid_t* g, tdx_mode_t mode, int P, const doub
     if ((reinterpret_cast<uintptr_t>(field) | reinterpret_cast<uintptr_t>(spec_work)) & 15) return fail(TDX_ERR_INVALID_ARG, "buffers must be 16-byte aligned");
     if (mode != TDX_MODE_THOMAS) {
         if (P < 2 || P > TDX_MAX_P || g->ny / P < 2) return fail(TDX_ERR_BAD_PARTITION, "P=%d invalid for line length %d", P, g->ny);
-        if (!helm_lines_M(g->ny, P))
-            return fail(TDX_ERR_UNSUPPORTED, "per-line shifts in PDD/PPT mode take at most 16 rows per partition: raise P; ny=%d P=%d", g->ny, P);
+        if (!helm_lines_P(g->ny, P, mode))
+            return fail(TDX_ERR_UNSUPPORTED, "per-line shifts in PDD mode take at most 16 rows per partition: raise P or use PPT; ny=%d P=%d", g->ny, P);
     }
     std::vector<double> kx, kz;
     if (!kx2) {
@@ -1189,7 +1350,10 @@ tdx_status_t tdx_slab_create(tdx_grid_t* g, tdx_dir_t dir, int rank, int nranks,
         if (rank <= nranks - 2) { hcoef[2] = he[(size_t)rank * 4 + 3]; hcoef[3] = he[(size_t)(rank + 1) * 4 + 0]; }     // w_last^(r), v_first^(r+1)
     } else {
         DevBuf Z, Zi, piv;                                                           // rank-level reduced system: the plan kernels of the intra-GPU PPT
-        CUDA_TRY(Z.alloc((size_t)K * K * 8)); CUDA_TRY(Zi.alloc((size_t)K * K * 8)); CUDA_TRY(piv.alloc((size_t)K * 4));
+        if (Z.alloc((size_t)K * K * 8) != cudaSuccess || Zi.alloc((size_t)K * K * 8) != cudaSuccess || piv.alloc((size_t)K * 4) != cudaSuccess) {
+            cudaGetLastError();
+            return bail(fail(TDX_ERR_ALLOC, "device allocation failed"));
+        }
         tdx::k_reduced_factor<<<1, 32>>>(1, nranks, ends.as<double>(), Z.as<double>(), piv.as<int>());
         g_launches.fetch_add(1);
         tdx::k_reduced_inverse<<<(K + 63) / 64, 64>>>(1, nranks, Z.as<double>(), piv.as<int>(), Zi.as<double>());
@@ -1287,7 +1451,7 @@ tdx_status_t tdx_pdd_dropped_bound(tdx_grid_t* g, tdx_dir_t dir, int P, double a
     if (dir < 0 || dir > 2) return fail(TDX_ERR_INVALID_ARG, "dir=%d", dir);
     CUDA_TRY(cudaSetDevice(g->device));
     Plan* pl = nullptr;
-    tdx_status_t rc = get_plan(g, KIND_ADI, dir, TDX_MODE_PDD, P, alpha, 1, nullptr, nullptr, nullptr, nullptr, 0, &pl);
+    tdx_status_t rc = get_plan(g, KIND_ADI, dir, TDX_MODE_PDD, P, alpha, 1, nullptr, nullptr, nullptr, nullptr, 0, &pl, 0, false);
     if (rc != TDX_OK) return rc;
     *out = pl->dropped;
     return TDX_OK;

@@ -27,7 +27,8 @@ struct Tables {
     const int* Sidx;         // cyclic closure functional (sparse), Sidx/Sval[set*Scap + k], Sn[set]
     const double* Sval;
     const int* Sn;
-    int P, n, q, r, KB, Scap;
+    int P, n, q, r, KB, Scap;   // P: kernel partitions; q, r: the CALLER's partition map (n / Pu, n % Pu)
+    int S;                      // sub-partitions per caller's partition (sub_part; 1 = plain map)
 };
 
 struct StridedArgs {
@@ -77,9 +78,9 @@ k_strided(StridedArgs A, Tables T, const __grid_constant__ UniTable<UNI ? MAXM :
     const int LPC = A.LPC, P = T.P;
     const int o = blockIdx.y;
     const int set = A.set_per_outer ? A.set0 + o : 0;
-    const int start = part_start(p, T.q, T.r);
-    const int m = T.q + (p < T.r ? 1 : 0);
-    const bool full = (T.r == 0) && (T.q == MAXM);          // every partition has exactly MAXM rows (warp-uniform)
+    int start, m;
+    sub_part(p, T.q, T.r, T.S, start, m);
+    const bool full = (T.r == 0) && (T.q == MAXM * T.S);    // every partition has exactly MAXM rows (warp-uniform)
     const long long rstride = A.line_stride * V;
     // One table set per outer index (Helmholtz: a set per wavenumber): this CTA's set is cold in L1, so pull its lines
     // in now, one prefetch per thread -- otherwise every table load on the dependent chain and in the band loop pays
@@ -233,9 +234,10 @@ k_unit(UnitArgs A, Tables T) {
     long long lines_here = A.nlines - line0; if (lines_here > A.LPB) lines_here = A.LPB;
     const int ll = tl / P, p = tl - ll * P;
     const bool valid = tl < nthreads_real && ll < lines_here;
-    const int m = valid ? T.q + (p < T.r ? 1 : 0) : 0;
+    int pst = 0, m = 0;
+    if (valid) sub_part(p, T.q, T.r, T.S, pst, m);
     const int cta_end = (int)lines_here * n;
-    const int S = valid ? ll * n + part_start(p, T.q, T.r) : cta_end;   // element offset in the CTA chunk
+    const int S = valid ? ll * n + pst : cta_end;                       // element offset in the CTA chunk
     const int e0 = __shfl_sync(0xffffffffu, S, 0);
     const int e1 = __shfl_sync(0xffffffffu, S + m, 31);
     const int count = e1 - e0;

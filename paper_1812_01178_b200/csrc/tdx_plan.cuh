@@ -27,6 +27,17 @@ enum RowLayout { ROWS_PJ = 0,      // rows[((set*P + p)*M + jj)*6 + f]   strided
 enum RowField { F_L = 0, F_Q = 1, F_INV = 2, F_CP = 3, F_V = 4, F_W = 5 };
 
 __host__ __device__ inline int part_start(int p, int q, int r) { return p * q + (p < r ? p : r); }
+// Two-level partition map (long partitions): the caller's P partitions of the map above (q = n / P rows, the
+// first r = n % P one more) are each cut again into S sub-partitions by the same rule; kernel partition p = po * S + s.
+// S = 1 is the plain map.  start / m: first row and number of rows of kernel partition p.
+__host__ __device__ inline void sub_part(int p, int q, int r, int S, int& start, int& m) {
+    if (S == 1) { start = part_start(p, q, r); m = q + (p < r ? 1 : 0); return; }
+    const int po = p / S, s = p - po * S;
+    const int mo = q + (po < r ? 1 : 0);
+    const int qs = mo / S, rs = mo - qs * S;
+    start = part_start(po, q, r) + part_start(s, qs, rs);
+    m = qs + (s < rs ? 1 : 0);
+}
 // reduced-system coefficients: pairs {gL, gR} per (set, band entry k, partition p) -- one 16-byte load per band entry
 __host__ __device__ inline size_t g_index(int set, int side, int k, int p, int KB, int P) { return ((((size_t)set * KB + k) * P + p) << 1) + side; }
 
@@ -136,15 +147,16 @@ __global__ void k_cyclic_q(int n, int nsets, const double* __restrict__ a, const
 // ends[(set*P+p)*4 + {0:v_first, 1:v_last, 2:w_first, 3:w_last}].  M = padded rows per partition (identity rows).
 // pinned sets (flags): d_0 := 0 is encoded as inv_0 := 0, l_1 := 0.
 template <int MAXROWS>
-__global__ void k_factor(int n, int nsets, int P, int M, int layout, int wrap,
+__global__ void k_factor(int n, int nsets, int P, int S, int M, int layout, int wrap,
                          const double* __restrict__ a, const double* __restrict__ b, const double* __restrict__ c,
                          const double* __restrict__ qv, const int* __restrict__ flags,
                          double* __restrict__ rows, double* __restrict__ ends) {
     int t = blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= nsets * P) return;
     int s = t / P, p = t % P;
-    int q = n / P, r = n % P;
-    int st = part_start(p, q, r), m = q + (p < r ? 1 : 0);
+    int Po = P / S;                                          // the caller's partitions; P = Po * S kernel partitions
+    int st, m;
+    sub_part(p, n / Po, n % Po, S, st, m);
     const double* as = a + (size_t)s * n + st; const double* bs = b + (size_t)s * n + st; const double* cs = c + (size_t)s * n + st;
     bool pinned = flags && flags[s] && p == 0;
     // ROWS_U (needs P >= 3): partition 1 has both neighbours and writes the one shared table; every partition still
@@ -407,7 +419,9 @@ __global__ void k_reduced_cyclic_inverse(int nsets, int P, const double* __restr
 
 // Partition p needs yL = x_{last_{p-1}} = u_{(2p-2) mod K} and yR = x_{first_{p+1}} = u_{(2p+1) mod K}.  The band is a
 // cyclic window of r indices around 2p: band = {lo, cnt}, entry k <-> r[(lo + k) mod K] <-> Z^{-1} column (lo + k - 1) mod K.
-__global__ void k_pack_ppt_cyclic(int nsets, int P, int KB, const double* __restrict__ Zi, double* __restrict__ G, int2* __restrict__ band) {
+// wrap = 0: the same cyclic bookkeeping for a line that is NOT periodic (composite plans, k_composite_factor): partition 0
+// has no left neighbour and partition P-1 no right one, their rows of Z^-1 are not used.
+__global__ void k_pack_ppt_cyclic(int nsets, int P, int KB, const double* __restrict__ Zi, double* __restrict__ G, int2* __restrict__ band, int wrap = 1) {
     int t = blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= nsets * P) return;
     int s = t / P, p = t % P;
@@ -415,12 +429,13 @@ __global__ void k_pack_ppt_cyclic(int nsets, int P, int KB, const double* __rest
     const double* zi = Zi + (size_t)s * K * K;
     const double tau = 1e-24;
     const int rowL = (2 * p - 2 + K) % K, rowR = (2 * p + 1) % K;
+    const bool useL = wrap || p > 0, useR = wrap || p < P - 1;
     double mxL = 0.0, mxR = 0.0;
     for (int cc = 0; cc < K; ++cc) { mxL = fmax(mxL, fabs(zi[(size_t)rowL * K + cc])); mxR = fmax(mxR, fabs(zi[(size_t)rowR * K + cc])); }
     int dl = 0, dr = 0;
     for (int d = -(K / 2); d < K - K / 2; ++d) {
         const int ri = ((2 * p + d) % K + K) % K, cc = (ri - 1 + K) % K;
-        if (fabs(zi[(size_t)rowL * K + cc]) > tau * mxL || fabs(zi[(size_t)rowR * K + cc]) > tau * mxR) { if (-d > dl) dl = -d; if (d > dr) dr = d; }
+        if ((useL && fabs(zi[(size_t)rowL * K + cc]) > tau * mxL) || (useR && fabs(zi[(size_t)rowR * K + cc]) > tau * mxR)) { if (-d > dl) dl = -d; if (d > dr) dr = d; }
     }
     int cnt = dl + dr + 1; if (cnt > K) cnt = K;
     const int lo = ((2 * p - dl) % K + K) % K;
@@ -429,10 +444,103 @@ __global__ void k_pack_ppt_cyclic(int nsets, int P, int KB, const double* __rest
         double gl = 0.0, gr = 0.0;
         if (k < cnt) {
             const int cc = ((lo + k) % K - 1 + K) % K;
-            gl = zi[(size_t)rowL * K + cc]; gr = zi[(size_t)rowR * K + cc];
+            gl = useL ? zi[(size_t)rowL * K + cc] : 0.0; gr = useR ? zi[(size_t)rowR * K + cc] : 0.0;
         }
         G[g_index(s, 0, k, p, KB, P)] = gl;
         G[g_index(s, 1, k, p, KB, P)] = gr;
+    }
+}
+
+// ---- long partitions: two-level plans ---------------------------------------------------------
+// A caller's partition of more than the register-resident length is cut again into S sub-partitions (sub_part), and the
+// sweep kernels run with P = Po * S kernel partitions.  Eq.(5)-(8) hold verbatim at the sub-level (every sub-partition is a
+// block of A~ with its own spikes), so
+//   PPT: the sub-level reduced system is solved exactly -- the same x as with the caller's Po partitions, to rounding
+//        ("no approximation");
+//   PDD: the caller's method drops v_last^(i-1), w_first^(i) of HIS partitions (L148-154).  With s_i, t_i the interface
+//        unknowns of his interface i, Alg.1 step 5 and Eq.(8) give  s_i = x_last^(i-1) + v_last^(i-1) s_{i-1}  and
+//        t_i = x_first^(i) + w_first^(i) t_{i+1}  (x = the PDD solution): the neighbour value a boundary sub-partition uses
+//        differs from the true neighbour row by exactly the dropped term.  In the sub-level Z (unknowns = the neighbour
+//        values every sub-partition uses) that is two extra entries per outer interface, -v_last^(i-1) and -w_first^(i)
+//        (outer spikes, k_outer_ends); for S = 1 they cancel the far spike ends, i.e. Z becomes the block-diagonal PDD
+//        matrix.  The result equals the caller's PDD with Po partitions to rounding.
+// Both use the cyclic bookkeeping of k_reduced_cyclic_factor (K = 2P unknowns u_{2p} = x_last_p, u_{(2p-1) mod K} =
+// x_first_p; the right-hand side of row k is r[(k+1) mod K]); a non-periodic line simply has zero spikes at its ends.
+
+// Far spike ends of the CALLER's partitions, any length: oends[(set*Po + p)*4 + {1: v_last, 2: w_first}] (0, 3 unused).
+// One thread per (set, partition); scratch: n doubles per set (c' of the block).
+__global__ void k_outer_ends(int n, int nsets, int Po, int wrap, const double* __restrict__ a, const double* __restrict__ b,
+                             const double* __restrict__ c, double* __restrict__ scratch, double* __restrict__ oends) {
+    int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= nsets * Po) return;
+    int s = t / Po, p = t % Po;
+    int q = n / Po, r = n % Po;
+    int st = part_start(p, q, r), m = q + (p < r ? 1 : 0);
+    const double* as = a + (size_t)s * n + st; const double* bs = b + (size_t)s * n + st; const double* cs = c + (size_t)s * n + st;
+    double* cp = scratch + (size_t)s * n + st;
+    const bool has_v = p > 0 || wrap, has_w = p < Po - 1 || wrap;
+    double cprev = 0.0, vprev = 0.0, inv = 0.0;
+    for (int j = 0; j < m; ++j) {                            // forward elimination of the block with rhs a_first e_first
+        const double ae = j == 0 ? 0.0 : as[j], ce = j == m - 1 ? 0.0 : cs[j];
+        inv = 1.0 / (bs[j] - ae * cprev);
+        cp[j] = ce * inv;
+        vprev = ((j == 0 && has_v ? as[0] : 0.0) - ae * vprev) * inv;
+        cprev = cp[j];
+    }
+    double w = has_w ? cs[m - 1] * inv : 0.0;                // w_{m-1}, then w_j = -c'_j w_{j+1}
+    for (int j = m - 2; j >= 0; --j) w = -cp[j] * w;
+    double* e = oends + (size_t)t * 4;
+    e[0] = 0.0; e[1] = vprev; e[2] = w; e[3] = 0.0;          // v_last = the last forward value (x_{m-1} = d'_{m-1})
+}
+
+// Z of the sub-level reduced system (+ the PDD entries above when pdd != 0), dense LU with partial pivoting.
+// One CTA per set; ends: sub-level spike ends [set][P][4]; oends: outer far ends [set][P/S][4] (pdd only).
+__global__ void k_composite_factor(int P, int S, int wrap, int pdd, const double* __restrict__ ends, const double* __restrict__ oends,
+                                   double* __restrict__ Z, int* __restrict__ piv) {
+    const int s = blockIdx.x, tid = threadIdx.x, nt = blockDim.x;
+    const int K = 2 * P, Po = P / S;
+    double* z = Z + (size_t)s * K * K;
+    int* pv = piv + (size_t)s * K;
+    const double* e = ends + (size_t)s * P * 4;
+    __shared__ int spr;
+    for (int i = tid; i < K * K; i += nt) z[i] = 0.0;
+    __syncthreads();
+    if (tid == 0) {
+        for (int p = 0; p < P; ++p) {
+            const int rl = 2 * p, rf = (2 * p - 1 + K) % K;
+            const int cL = (2 * p - 2 + K) % K, cR = (2 * p + 1) % K;          // x_last_{p-1}, x_first_{p+1}
+            z[(size_t)rl * K + rl] += 1.0; z[(size_t)rl * K + cL] += e[p * 4 + 1]; z[(size_t)rl * K + cR] += e[p * 4 + 3];
+            z[(size_t)rf * K + rf] += 1.0; z[(size_t)rf * K + cL] += e[p * 4 + 0]; z[(size_t)rf * K + cR] += e[p * 4 + 2];
+        }
+        if (pdd) {
+            const double* oe = oends + (size_t)s * Po * 4;
+            for (int i = wrap ? 0 : 1; i < Po; ++i) {                          // the caller's interface i: partitions im | i
+                const int im = (i - 1 + Po) % Po;
+                const int slast = im * S + S - 1, tfirst = im * S;             // s_i is defined by the row of x_last of slast ...
+                z[(size_t)(2 * slast) * K + (2 * tfirst - 2 + K) % K] -= oe[im * 4 + 1];      // ... minus v_last^(im) s_im
+                const int f = i * S, s2 = i * S + S - 1;                       // t_i: row of x_first of f, minus w_first^(i) t_{i+1}
+                z[(size_t)((2 * f - 1 + K) % K) * K + (2 * s2 + 1) % K] -= oe[i * 4 + 2];
+            }
+        }
+    }
+    __syncthreads();
+    for (int k = 0; k < K; ++k) {
+        if (tid == 0) {
+            int pr = k; double best = fabs(z[(size_t)k * K + k]);
+            for (int i = k + 1; i < K; ++i) { double t = fabs(z[(size_t)i * K + k]); if (t > best) { best = t; pr = i; } }
+            pv[k] = pr; spr = pr;
+        }
+        __syncthreads();
+        const int pr = spr;
+        if (pr != k) for (int cc = tid; cc < K; cc += nt) { double t = z[(size_t)k * K + cc]; z[(size_t)k * K + cc] = z[(size_t)pr * K + cc]; z[(size_t)pr * K + cc] = t; }
+        __syncthreads();
+        const double d = z[(size_t)k * K + k];
+        for (int i = k + 1 + tid; i < K; i += nt) {
+            const double f = z[(size_t)i * K + k] / d;
+            z[(size_t)i * K + k] = f;
+            if (f != 0.0) for (int cc = k + 1; cc < K; ++cc) z[(size_t)i * K + cc] -= f * z[(size_t)k * K + cc];
+        }
+        __syncthreads();
     }
 }
 

@@ -76,21 +76,24 @@ def test_error_paths_leave_data_untouched(small):
         grid.adi_sweep(0, tdx.MODE_PPT, 2, 1e-3, 0)              # NULL data pointer
     assert e.value.status == tdx.ERR_INVALID_ARG
     with pytest.raises(tdx.TdxError) as e:
-        grid.helmholtz_wavenumber_solve(tdx.MODE_PPT, 2, np.ones(nx), np.ones(3), t)   # per-line shifts: 18 rows per partition > 16
+        grid.helmholtz_wavenumber_solve(tdx.MODE_PDD, 2, np.ones(nx), np.ones(3), t)   # per-line shifts, PDD: 18 rows per partition > 16
     assert e.value.status == tdx.ERR_UNSUPPORTED
     torch.cuda.synchronize()
     assert np.array_equal(t.cpu().numpy(), field)
 
 
-def test_rows_per_partition_limit_is_reported():
+def test_rows_per_partition_has_no_limit():
+    """Round 1 refused more than 64 rows per partition; SURVEY 8(b) asks only 1 <= P, floor(n/P) >= 2."""
     nx = 400
     f = inputs.faces_uniform(nx, 1.0); g8 = inputs.faces_uniform(8, 1.0)
     grid = tdx.Grid(nx, 8, 8, f, g8, g8, bcs=BCS)
-    t = torch.zeros(8 * 8 * nx, dtype=torch.float64, device="cuda")
-    with pytest.raises(tdx.TdxError) as e:
-        grid.adi_sweep(0, tdx.MODE_PPT, 4, 1e-3, t)              # 100 rows per partition > 64
-    assert e.value.status == tdx.ERR_UNSUPPORTED
-    grid.adi_sweep(0, tdx.MODE_THOMAS, 4, 1e-3, t)               # Thomas has no such limit
+    field = inputs.rhs_uniform((8, 8, nx), 2)
+    ref = orc.adi_sweep(field.copy(), f, g8, g8, BCS, 0, orc.MODE_THOMAS, 1, 1e-5)
+    for mode in (tdx.MODE_PPT, tdx.MODE_THOMAS):
+        t = torch.from_numpy(field).cuda()
+        grid.adi_sweep(0, mode, 4, 1e-5, t)                      # 100 rows per partition
+        torch.cuda.synchronize()
+        assert np.max(np.abs(t.cpu().numpy() - ref)) / np.max(np.abs(ref)) < 1e-12
     grid.close()
 
 
