@@ -491,12 +491,13 @@ int pow2floor(long long v) { int p = 1; while ((long long)p * 2 <= v) p *= 2; re
 
 // lines of `dir` in a field whose x extent is `nxe` doubles (nx for real fields, 2 nx for complex ones)
 tdx_status_t run_strided(const Plan& pl, double* data, long long W, long long line_stride, long long O,
-                         long long outer_stride, bool set_per_outer, cudaStream_t st, int set0 = 0) {
+                         long long outer_stride, bool set_per_outer, cudaStream_t st, int set0 = 0, double* iface = nullptr) {
     // W, strides in doubles on entry.  16-byte accesses (V = 2 lines per thread) when everything is even.
     const bool even = W % 2 == 0 && line_stride % 2 == 0 && outer_stride % 2 == 0 && (reinterpret_cast<uintptr_t>(data) % 16) == 0;
     if (O > 65535) return fail(TDX_ERR_UNSUPPORTED, "outer extent %lld > 65535", O);
     StridedArgs A;
     A.data = data; A.set_per_outer = set_per_outer ? 1 : 0; A.set0 = set0; A.pf = 0;
+    A.iface = iface; A.iface_plane = W * O;
     if (pl.thomas) {
         const int V = even ? 2 : 1;
         A.W = W / V; A.line_stride = line_stride / V; A.outer_stride = outer_stride / V;
@@ -719,11 +720,12 @@ tdx_status_t run_unit(const Plan& pl, double* data, long long nlines, cudaStream
 
 // ncomp fields of the grid's shape stored back to back are just a longer batch: more x lines, more outer planes for
 // the y sweep, `ncomp` outer indices for the z sweep.
-tdx_status_t run_sweep(tdx_grid* g, const Plan& pl, int dir, double* data, cudaStream_t st, int ncomp = 1) {
+// iface (y / z only): the sweep also stores the first and last row of every line there (slab sweeps)
+tdx_status_t run_sweep(tdx_grid* g, const Plan& pl, int dir, double* data, cudaStream_t st, int ncomp = 1, double* iface = nullptr) {
     const long long nx = g->nx, ny = g->ny, nz = g->nz;
     if (dir == 0) return run_unit(pl, data, ny * nz * ncomp, st);
-    if (dir == 1) return run_strided(pl, data, nx, nx, nz * ncomp, nx * ny, false, st);
-    return run_strided(pl, data, nx * ny, nx * ny, ncomp, ncomp > 1 ? nx * ny * nz : 0, false, st);
+    if (dir == 1) return run_strided(pl, data, nx, nx, nz * ncomp, nx * ny, false, st, 0, iface);
+    return run_strided(pl, data, nx * ny, nx * ny, ncomp, ncomp > 1 ? nx * ny * nz : 0, false, st, 0, iface);
 }
 
 // The plan cache is keyed by (kind, dir, loc, mode, P, alpha / coefficient hash): a caller that keeps changing alpha (variable
@@ -948,7 +950,6 @@ struct tdx_slab {
     long long inner = 0, outer = 0;
     std::vector<double> a, b, c;       // the slab's cut operator (host): user coefficients of the local plan
     double *v = nullptr, *w = nullptr, *coef = nullptr;   // device: spikes of this rank, interface coefficients
-    double* ylr = nullptr;             // device [2][plane]: interface unknowns of the current sweep
     double dropped = 0.0;              // max |v_last|, |w_first| over interior ranks: what PDD across ranks deletes
 };
 
@@ -1328,7 +1329,7 @@ tdx_status_t tdx_slab_create(tdx_grid_t* g, tdx_dir_t dir, int rank, int nranks,
     s->inner = inner; s->outer = outer;
     const int K = 2 * (nranks - 1);
     if (cudaMalloc(&s->v, (size_t)n_loc * 8) != cudaSuccess || cudaMalloc(&s->w, (size_t)n_loc * 8) != cudaSuccess ||
-        cudaMalloc(&s->coef, (size_t)std::max(4, 2 * K) * 8) != cudaSuccess || cudaMalloc(&s->ylr, (size_t)2 * inner * outer * 8) != cudaSuccess) { cudaGetLastError(); return bail(fail(TDX_ERR_ALLOC, "device allocation failed")); }
+        cudaMalloc(&s->coef, (size_t)std::max(4, 2 * K) * 8) != cudaSuccess) { cudaGetLastError(); return bail(fail(TDX_ERR_ALLOC, "device allocation failed")); }
     tdx::k_slab_spikes<<<(nranks + 31) / 32, 32>>>(nranks, dst.as<int>(), a.as<double>(), b.as<double>(), c.as<double>(), rank, nmax,
                                                     scratch.as<double>(), ends.as<double>(), s->v, s->w);
     g_launches.fetch_add(1);
@@ -1344,6 +1345,8 @@ tdx_status_t tdx_slab_create(tdx_grid_t* g, tdx_dir_t dir, int rank, int nranks,
         if (i >= 2) s->dropped = std::max(s->dropped, std::fabs(he[(size_t)(i - 1) * 4 + 1]));
         if (i <= nranks - 2) s->dropped = std::max(s->dropped, std::fabs(he[(size_t)i * 4 + 2]));
     }
+    if (across == TDX_MODE_PDD && g->pdd_strict > 0.0 && !(s->dropped <= g->pdd_strict))
+        return bail(fail(TDX_ERR_PDD_BOUND, "PDD across %d ranks drops couplings of size %.3e > strict limit %.3e: use PPT across ranks", nranks, s->dropped, g->pdd_strict));
     std::vector<double> hcoef(std::max(4, 2 * K), 0.0);
     if (across == TDX_MODE_PDD || nranks == 1) {
         if (rank >= 1) { hcoef[0] = he[(size_t)(rank - 1) * 4 + 3]; hcoef[1] = he[(size_t)rank * 4 + 0]; }               // w_last^(r-1), v_first^(r)
@@ -1374,7 +1377,7 @@ tdx_status_t tdx_slab_create(tdx_grid_t* g, tdx_dir_t dir, int rank, int nranks,
 
 tdx_status_t tdx_slab_destroy(tdx_slab_t* s) {
     if (!s) return TDX_OK;
-    cudaFree(s->v); cudaFree(s->w); cudaFree(s->coef); cudaFree(s->ylr);
+    cudaFree(s->v); cudaFree(s->w); cudaFree(s->coef);
     delete s;
     return TDX_OK;
 }
@@ -1389,12 +1392,7 @@ tdx_status_t tdx_slab_eliminate(tdx_slab_t* s, double* field, double* iface_out,
     Plan* pl = nullptr;
     rc = get_plan(g, KIND_USERNP, s->dir, s->local_mode, s->P_local, 0.0, 1, nullptr, s->a.data(), s->b.data(), s->c.data(), st, &pl);
     if (rc != TDX_OK) return rc;
-    rc = run_sweep(g, *pl, s->dir, field, st);
-    if (rc != TDX_OK) return rc;
-    const long long tot = 2 * s->inner * s->outer;
-    tdx::k_slab_pack<<<(unsigned)((tot + 255) / 256), 256, 0, st>>>(field, iface_out, s->n_loc, s->inner, s->outer);
-    LAUNCH_CHECK("k_slab_pack");
-    return TDX_OK;
+    return run_sweep(g, *pl, s->dir, field, st, 1, iface_out);      // Alg.1 steps 2-4 in one launch: the store loop packs the interface rows
 }
 
 tdx_status_t tdx_slab_correct(tdx_slab_t* s, double* field, const double* iface_own, const double* iface_nbr, void* stream) {
@@ -1404,15 +1402,13 @@ tdx_status_t tdx_slab_correct(tdx_slab_t* s, double* field, const double* iface_
     if (!iface_nbr || (reinterpret_cast<uintptr_t>(iface_nbr) & 15)) return fail(TDX_ERR_INVALID_ARG, "iface_nbr is NULL or not 16-byte aligned");
     CUDA_TRY(cudaSetDevice(s->g->device));
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    const int JT = std::max(8, (s->n_loc + 7) / 8);
+    // one thread marches over all rows of its two lines when the plane alone fills the GPU; row slices otherwise
+    const long long plane = s->inner * s->outer;
+    const int JT = (plane / 2 >= (long long)s->g->sms * 2048) ? s->n_loc : std::max(8, (s->n_loc + 7) / 8);
     dim3 block(128), grid((unsigned)((s->inner / 2 + 127) / 128), (s->n_loc + JT - 1) / JT, (unsigned)s->outer);
     if (s->outer > 65535) return fail(TDX_ERR_UNSUPPORTED, "outer extent > 65535");
-    const long long plane = s->inner * s->outer;
-    const unsigned ib = (unsigned)((plane / 2 + 255) / 256);
-    if (s->across == TDX_MODE_PPT) tdx::k_slab_interface<true><<<ib, 256, 0, st>>>(iface_own, iface_nbr, s->coef, s->ylr, s->rank, s->R, plane);
-    else tdx::k_slab_interface<false><<<ib, 256, 0, st>>>(iface_own, iface_nbr, s->coef, s->ylr, s->rank, s->R, plane);
-    LAUNCH_CHECK("k_slab_interface");
-    tdx::k_slab_correct<<<grid, block, 0, st>>>(field, s->ylr, s->v, s->w, s->n_loc, s->inner, s->outer, JT);
+    if (s->across == TDX_MODE_PPT) tdx::k_slab_correct<true><<<grid, block, 0, st>>>(field, iface_own, iface_nbr, s->coef, s->v, s->w, s->rank, s->R, s->n_loc, s->inner, s->outer, JT);
+    else tdx::k_slab_correct<false><<<grid, block, 0, st>>>(field, iface_own, iface_nbr, s->coef, s->v, s->w, s->rank, s->R, s->n_loc, s->inner, s->outer, JT);
     LAUNCH_CHECK("k_slab_correct");
     return TDX_OK;
 }

@@ -41,6 +41,8 @@ struct StridedArgs {
     int LPC;                 // lines (V-vectors) per CTA = blockDim.x
     int pf;                  // L2 prefetch distance: CTAs ahead (one tile per CTA) or sets ahead (looping CTAs); 0 = off
     int tiles_x;             // column tiles per outer index
+    double* iface;           // slab sweeps (tdx_slab_eliminate): also store row 0 of every line to iface[0][outer][W*V] and its last
+    long long iface_plane;   //   row to iface[1][...] (Alg.1 step 4's pack, fused into the store); iface_plane = doubles per plane; NULL = off
 };
 
 template <int V> struct VecIO;
@@ -201,6 +203,11 @@ k_strided(StridedArgs A, Tables T, const __grid_constant__ UniTable<UNI ? MAXM :
             x[jj][v] = r;
         }
         if (valid && (full || jj < m)) VecIO<V>::st(base + jj * rstride, x[jj]);
+        if (A.iface != nullptr && valid) {                  // Alg.1 step 4: the slab's interface rows, packed for the exchange
+            double* ip = A.iface + ((long long)o * A.W + i) * V;
+            if (p == 0 && jj == 0) VecIO<V>::st(ip, x[0]);
+            if (p == P - 1 && jj == m - 1) VecIO<V>::st(ip + A.iface_plane, x[jj]);
+        }
     }
     if (xt + (int)gridDim.x < tiles_x) __syncthreads();     // rs is reused by the next tile
   }
@@ -337,6 +344,11 @@ __global__ void k_thomas_strided(StridedArgs A, const double* __restrict__ rows,
 #pragma unroll
         for (int v = 0; v < V; ++v) { cur[v] = fma(-cp, prev[v], cur[v] * inv); prev[v] = cur[v]; if (j == n - 1) ylast[v] = cur[v]; }
         VecIO<V>::st(base + j * rstride, cur);
+    }
+    if (A.iface != nullptr && !CYC) {                       // slab sweeps: pack rows 0 and n-1 (prev = x_0, ylast = x_{n-1})
+        double* ip = A.iface + ((long long)o * A.W + i) * V;
+        VecIO<V>::st(ip, prev);
+        VecIO<V>::st(ip + A.iface_plane, ylast);
     }
     if (CYC) {
         const double g = __ldg(cyc + set * 4 + 0), kappa = __ldg(cyc + set * 4 + 3);

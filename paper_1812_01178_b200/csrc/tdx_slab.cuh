@@ -6,12 +6,15 @@
 //                    (tdx_kernels.cuh / tdx_tma.cuh) with the cut operator as a user-coefficient plan; the spikes
 //                    A_r v = a_first e_first, A_r w = c_last e_last are matrix-only, so they are plan-time vectors here
 //                    (k_slab_spikes) instead of two extra right-hand sides per line (R(9M), L228-231).
-//   step 4 / 6       the interface rows xt_first, xt_last of the slab are packed into one buffer (k_slab_pack) that the
+//   step 4 / 6       the interface rows xt_first, xt_last of the slab are packed into one buffer BY THE SWEEP KERNEL's own
+//                    store loop (StridedArgs::iface: iface[0][outer][inner] = row 0, iface[1][..] = row n_loc-1) that the
 //                    caller exchanges: neighbour send/recv for PDD (L244-256), one all-gather for PPT (L156, L174).
-//   step 5           k_slab_interface: per line, the interface unknowns (PDD: the two 2x2 blocks of L148-154; PPT: two rows
-//                    of the plan-time Z^-1 of the rank-level reduced system, Eq.(7)), two planes.
-//   step 7           k_slab_correct: x = xt - v yL - w yR (Eq.(8)) over the slab.
-// The correction is a second pass over the slab (8 B read + 8 B written per value), as step 7 is in the paper.
+//   step 5 + 7       k_slab_correct: per line, the interface unknowns (PDD: the two 2x2 blocks of L148-154; PPT: two rows
+//                    of the plan-time Z^-1 of the rank-level reduced system, Eq.(7)) in the prologue, then
+//                    x = xt - v yL - w yR (Eq.(8)) over the slab.
+// One launch per phase: the messages are 2 / n_loc of the slab, so launch and exchange latency is what a sweep pays for
+// beyond its two passes.  The correction is a second pass over the slab (8 B read + 8 B written per value), as step 7 is in
+// the paper.
 #pragma once
 #include <cuda_runtime.h>
 
@@ -49,27 +52,24 @@ __global__ void k_slab_spikes(int R, const int* __restrict__ starts, const doubl
     if (r == me) for (int jj = 0; jj < n; ++jj) { v_out[jj] = v[jj]; w_out[jj] = w[jj]; }
 }
 
-// field [outer][n_loc][inner]: iface[0][o][i] = row 0, iface[1][o][i] = row n_loc-1
-__global__ void k_slab_pack(const double* __restrict__ field, double* __restrict__ iface, int n_loc, long long inner, long long outer) {
-    const long long plane = inner * outer;
-    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (t >= 2 * plane) return;
-    const int which = t >= plane;
-    const long long q = t - which * plane;
-    const long long o = q / inner, i = q - o * inner;
-    iface[t] = field[(o * n_loc + (which ? n_loc - 1 : 0)) * inner + i];
-}
-
-// Interface unknowns of every line of the slab (Alg.1 step 5 / Eq.(7)), once per sweep: y[0][plane] = yL = x_last of
-// rank-1, y[1][plane] = yR = x_first of rank+1 (zero where there is no neighbour).
-// coef (device): PDD: {wl_prev, vf_me, wl_me, vf_next}; PPT: rows of Z^-1: coef[k] (yL) and coef[K + k] (yR), k < K = 2(R-1).
-// own: [2][plane] of this rank (xt_first, xt_last); nbr: PDD [2][plane] = (xt_last of rank-1, xt_first of rank+1);
-// PPT [R][2][plane] gathered from every rank.  Thread = two adjacent values (plane is even).
+// Alg.1 steps 5 and 7 in ONE pass over the slab [outer][n_loc][inner].  Thread = two adjacent inner elements (inner is
+// even) of one outer index.  Prologue (step 5 / Eq.(7)): the two interface unknowns of the thread's lines, yL = x_last of
+// rank-1, yR = x_first of rank+1 (zero where there is no neighbour) --
+//   PDD: the two 2x2 blocks of L148-154, coef = {wl_prev, vf_me, wl_me, vf_next};
+//   PPT: two rows of the plan-time Z^-1 of the rank-level reduced system, coef[k] (yL) and coef[K + k] (yR), K = 2(R-1).
+// own: [2][plane] of this rank (xt_first, xt_last); nbr: PDD [2][plane] = (xt_last of rank-1, xt_first of rank+1); PPT
+// [R][2][plane] gathered from every rank.  Then Eq.(8) (step 7): x = xt - v yL - w yR, marching over rows [j0, j1) of the
+// slab; grid.y slices the rows only when the plane alone has too few threads to fill the GPU (each slice then repeats the
+// prologue, which reads 4 (PDD) or 2R (PPT) plane values against 2 JT slab values).
 template <bool PPT>
-__global__ void __launch_bounds__(256) k_slab_interface(const double* __restrict__ own, const double* __restrict__ nbr,
-                                                        const double* __restrict__ coef, double* __restrict__ y, int rank, int R, long long plane) {
-    const long long q = ((long long)blockIdx.x * blockDim.x + threadIdx.x) * 2;
-    if (q >= plane) return;
+__global__ void __launch_bounds__(128) k_slab_correct(double* __restrict__ field, const double* __restrict__ own, const double* __restrict__ nbr,
+                                                      const double* __restrict__ coef, const double* __restrict__ v, const double* __restrict__ w,
+                                                      int rank, int R, int n_loc, long long inner, long long outer, int JT) {
+    const long long plane = inner * outer;
+    const long long i = ((long long)blockIdx.x * blockDim.x + threadIdx.x) * 2;
+    if (i >= inner) return;
+    const long long o = blockIdx.z;
+    const long long q = o * inner + i;
     double2 yL = make_double2(0.0, 0.0), yR = make_double2(0.0, 0.0);
     if (!PPT) {
         const double2 xf = *reinterpret_cast<const double2*>(own + q), xl = *reinterpret_cast<const double2*>(own + plane + q);
@@ -93,21 +93,6 @@ __global__ void __launch_bounds__(256) k_slab_interface(const double* __restrict
             yR.x += gr0 * r0.x + gr1 * r1.x; yR.y += gr0 * r0.y + gr1 * r1.y;
         }
     }
-    *reinterpret_cast<double2*>(y + q) = yL;
-    *reinterpret_cast<double2*>(y + plane + q) = yR;
-}
-
-// Eq.(8) (Alg.1 step 7): x = xt - v yL - w yR over the slab [outer][n_loc][inner].  Thread = two adjacent inner elements
-// (inner is even) of one outer index, marching over JT rows; grid.y slices the rows to keep enough CTAs in flight.
-__global__ void __launch_bounds__(128) k_slab_correct(double* __restrict__ field, const double* __restrict__ y,
-                                                      const double* __restrict__ v, const double* __restrict__ w,
-                                                      int n_loc, long long inner, long long outer, int JT) {
-    const long long plane = inner * outer;
-    const long long i = ((long long)blockIdx.x * blockDim.x + threadIdx.x) * 2;
-    if (i >= inner) return;
-    const long long o = blockIdx.z;
-    const long long q = o * inner + i;
-    const double2 yL = *reinterpret_cast<const double2*>(y + q), yR = *reinterpret_cast<const double2*>(y + plane + q);
     const int j0 = blockIdx.y * JT, j1 = min(n_loc, j0 + JT);
     double* p = field + (o * n_loc + j0) * inner + i;
 #pragma unroll 4

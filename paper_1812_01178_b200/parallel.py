@@ -56,8 +56,12 @@ class SlabSweep:
     slab tensor [nz_loc][ny_loc][nx] (float64, CUDA).  `across` = tdx.MODE_PDD or tdx.MODE_PPT between ranks,
     `local_mode` / `P_local` inside the rank."""
 
-    def __init__(self, slab_grid, direction, rank, world, faces_global, bc_global, alpha, across, local_mode, P_local, group=None):
-        self.slab = tdx.Slab(slab_grid, direction, rank, world, faces_global, bc_global, alpha, across, local_mode, P_local)
+    def __init__(self, slab_grid, direction, rank, world, faces_global, bc_global, alpha, across, local_mode, P_local, group=None,
+                 slab=None):
+        """slab: an object with eliminate(field, iface, stream) / correct(field, iface_own, iface_nbr, stream) / close();
+        default: the CUDA kernels behind tdx.Slab.  (The CPU tests of this class's control flow and exchange pattern pass
+        a stand-in, since the kernels need a device.)"""
+        self.slab = slab if slab is not None else tdx.Slab(slab_grid, direction, rank, world, faces_global, bc_global, alpha, across, local_mode, P_local)
         self.rank, self.world, self.across, self.group = rank, world, across, group
         g = slab_grid
         self.plane = (g.nx * g.nz) if direction == 1 else (g.nx * g.ny)
@@ -66,7 +70,7 @@ class SlabSweep:
     def sweep(self, field):
         if self.iface is None or self.iface.device != field.device:
             self.iface = torch.empty((2, self.plane), dtype=torch.float64, device=field.device)
-        stream = torch.cuda.current_stream().cuda_stream
+        stream = torch.cuda.current_stream().cuda_stream if field.is_cuda else 0
         self.slab.eliminate(field, self.iface, stream)
         if self.world == 1:
             return field

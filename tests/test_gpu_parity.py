@@ -221,9 +221,13 @@ def test_helmholtz_per_line_shift_kx2_thomas(cfg2):
         assert relerr(out[m], ref[m]) < TOL_EXACT, (m, relerr(out[m], ref[m]))
     assert relerr(out, ref) < TOL_EXACT
     before = t.clone()
-    with pytest.raises(tdx.TdxError) as e:                       # per-line PDD/PPT takes at most 16 rows per partition (128 / 4 = 32)
-        grid.helmholtz_wavenumber_solve(tdx.MODE_PPT, 4, kx2, kz2, t)
+    with pytest.raises(tdx.TdxError) as e:                       # per-line PDD takes at most 16 rows per partition (128 / 4 = 32)
+        grid.helmholtz_wavenumber_solve(tdx.MODE_PDD, 4, kx2, kz2, t)
     assert e.value.status == tdx.ERR_UNSUPPORTED and torch.equal(t, before)
+    t4 = torch.from_numpy(rhs).cuda()                           # PPT is exact for any partitioning: 32-row partitions are cut again
+    grid.helmholtz_wavenumber_solve(tdx.MODE_PPT, 4, kx2, kz2, t4)
+    torch.cuda.synchronize()
+    assert relerr(t4.cpu().numpy(), ref) < TOL_EXACT
     # kx2 given but all zero is the shared-matrix fast path
     t2 = torch.from_numpy(rhs).cuda(); t3 = torch.from_numpy(rhs).cuda()
     grid.helmholtz_wavenumber_solve(tdx.MODE_PPT, 8, np.zeros(c.nx), kz2, t2)
