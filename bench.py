@@ -82,8 +82,10 @@ def parse():
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-step3", action="store_true", help="skip the extra 3-component staggered ADI step figure")
-    ap.add_argument("--slab", action="store_true", help="with --gpus N > 1: also time the y sweep of ONE field cut into y-slabs over the "
-                    "ranks (NCCL neighbour exchange / all-gather; SURVEY 8(f) N3).  At N = 1 the per-rank compute figure is always reported.")
+    ap.add_argument("--no-slab", action="store_true", help="skip `slab_y_sweep`: the y sweep of ONE field cut into y-slabs over the ranks "
+                    "(NCCL neighbour exchange / all-gather; SURVEY 8(f) N3; strong scaling).  Default at every N; at N = 1 it is the "
+                    "compute part of one rank of a 4-rank job.")
+    ap.add_argument("--slab", action="store_true", help=argparse.SUPPRESS)      # round-1 opt-in, now the default
     ap.add_argument("--psweep", default="", help="P sweep table (e.g. 8,16,32,64): per direction and mode, time, GB/s, PDD bound, "
                                                  "error of sampled lines vs the oracle; prints a markdown table, not the JSON line")
     ap.add_argument("--selftest-ranks", action="store_true",
@@ -96,13 +98,46 @@ def init_dist(world, backend, local_rank=0):
     """Process group for the barrier and the max-over-ranks reduction only. MASTER_ADDR/PORT, RANK, WORLD_SIZE from env."""
     if world <= 1:
         return None
+    import datetime
     import torch
     import torch.distributed as dist
+    # a collective that never completes (a dead peer) aborts after two minutes instead of hanging the bench
     if backend == "nccl":
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+        nccl_log_setup()
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank), timeout=datetime.timedelta(seconds=120))
     else:
-        dist.init_process_group(backend)
+        dist.init_process_group(backend, timeout=datetime.timedelta(seconds=120))
     return dist
+
+
+def nccl_log_setup():
+    """NCCL's own INIT lines (communicator size, transport, NVLS) go to a file per process, so the N > 1 line can say which
+    communicator it really ran on without polluting stdout (the JSON line).  Respects a caller's NCCL_DEBUG settings."""
+    if "NCCL_DEBUG" in os.environ:
+        return
+    d = os.path.join(ROOT, "gpurun_out")
+    try:
+        os.makedirs(d, exist_ok=True)
+    except OSError:
+        return
+    os.environ["NCCL_DEBUG"] = "INFO"
+    os.environ["NCCL_DEBUG_SUBSYS"] = "INIT,GRAPH"
+    os.environ["NCCL_DEBUG_FILE"] = os.path.join(d, "nccl_%h_%p.log")
+
+
+def nccl_log_summary():
+    """What this process's NCCL log says: communicator sizes seen, whether NVLS (in-switch reduction) was set up."""
+    import re
+    pat = os.environ.get("NCCL_DEBUG_FILE", "")
+    if not pat:
+        return None
+    path = pat.replace("%h", __import__("socket").gethostname()).replace("%p", str(os.getpid()))
+    try:
+        text = open(path, errors="replace").read()
+    except OSError:
+        return {"log": path, "error": "not written"}
+    return {"log": os.path.relpath(path, ROOT), "nranks_seen": sorted({int(v) for v in re.findall(r"nranks (\d+)", text)}),
+            "nvls": "NVLS" in text, "p2p": "P2P" in text, "lines": text.count("\n")}
 
 
 def max_over_ranks(value, dist, device="cpu"):
@@ -546,8 +581,8 @@ def run_tdx(args, rank, world, local_rank):
         # world == 1: the compute part of an interior rank of a 4-rank job (a quarter slab; the exchange is a device copy);
         # world > 1: the real thing over NCCL (strong scaling of ONE field), max over ranks.
         try:
-            if world > 1 and not args.slab:
-                raise RuntimeError("skipped: pass --slab to time the NCCL slab sweep at N > 1")
+            if args.no_slab:
+                raise RuntimeError("skipped (--no-slab)")
             from paper_1812_01178_b200 import parallel
             Rk = world if world > 1 else 4
             rk = rank if world > 1 else 1
@@ -627,6 +662,9 @@ def run_tdx(args, rank, world, local_rank):
         info["unit"] = UNIT
         out["cpu_baseline"] = info
     grid.close()
+    if world > 1:
+        out["nccl"] = nccl_log_summary()
+        out["nccl_comm_nranks_ok"] = bool(out["nccl"] and world in out["nccl"].get("nranks_seen", []))
     if rank == 0:
         print(json.dumps(out))
     if world > 1:

@@ -18,12 +18,43 @@ def _fields(shape, seed, diag_scale):
     return a, b, c
 
 
-def _matvec(a, b, c, x, axis):
+def _matvec(a, b, c, x, axis, cyclic=False):
     y = b * x
     xm = np.moveaxis(x, axis, 0); am = np.moveaxis(a, axis, 0); cm = np.moveaxis(c, axis, 0); ym = np.moveaxis(y, axis, 0)
     ym[1:] += am[1:] * xm[:-1]
     ym[:-1] += cm[:-1] * xm[1:]
+    if cyclic:
+        ym[0] += am[0] * xm[-1]
+        ym[-1] += cm[-1] * xm[0]
     return y
+
+
+def test_manufactured_solutions_along_x_and_periodic_lines():
+    shape = (5, 7, 18)
+    for axis, cyclic in ((2, False), (2, True), (1, True), (0, True)):
+        a, b, c = _fields(shape, 61 + axis, 0.3)
+        x = inputs.uniform_pm1(63, int(np.prod(shape))).reshape(shape)
+        d = _matvec(a, b, c, x, axis, cyclic)
+        got, A = ogen.general_solve(a, b, c, d, axis, cyclic)
+        cond = np.linalg.cond(A)
+        err = np.max(np.abs(np.moveaxis(got - x, axis, -1).reshape(len(cond), -1)), axis=1)
+        assert np.all(err <= 1e-14 * cond * 10), float(np.max(err / cond))
+        if cyclic:                                               # the corners really are part of the system
+            plain, _ = ogen.general_solve(a, b, c, d, axis, False)
+            assert np.max(np.abs(plain - x)) > 1e-3
+
+
+def test_periodic_dominant_systems_agree_with_the_c_cyclic_thomas():
+    shape = (2, 21, 3)
+    a, b, c = _fields(shape, 71, 1.0)
+    b = 3.0 + np.abs(b)
+    d = inputs.uniform_pm1(72, int(np.prod(shape))).reshape(shape)
+    got, _ = ogen.general_solve(a, b, c, d, 1, cyclic=True)
+    for k in range(shape[0]):
+        for i in range(shape[2]):
+            ref = orc.cyclic_thomas(np.ascontiguousarray(a[k, :, i]), np.ascontiguousarray(b[k, :, i]), np.ascontiguousarray(c[k, :, i]),
+                                    np.ascontiguousarray(d[k, :, i]))
+            assert np.max(np.abs(got[k, :, i] - ref)) < 1e-14
 
 
 def test_manufactured_solutions_non_dominant_both_axes():
