@@ -181,16 +181,31 @@ tdx_status_t tdx_slab_correct(tdx_slab_t* slab, double* field_inout, const doubl
 tdx_status_t tdx_slab_dropped_bound(tdx_slab_t* slab, double* out);
 
 /* Batched tridiagonal solve with PER-LINE coefficients and diagonal pivoting ("a parallel tridiagonal
- * solver with diagonal pivoting is used [3]") -- for systems that are not diagonally dominant.
- * a, b, c: DEVICE, nx*ny*nz doubles each, laid out like the field: row j of the line through (i, k) [dir = y] holds
- * a = coupling to row j-1, b = diagonal, c = coupling to row j+1; a of a line's first row and c of its last row are
- * not read.  pivoting != 0: 1x1 / 2x2 diagonal pivots without row interchanges (criterion: tdx_general.cuh);
- * pivoting == 0: plain Thomas on the same data (breaks down on a zero pivot: inf / nan in that line, no error).
- * rhs_inout: DEVICE, in place.  work: DEVICE scratch of 9*nx*ny*nz BYTES (modified diagonal + pivot types), 8-byte
- * aligned, caller-owned.  dir = y or z (x lines: TDX_ERR_UNSUPPORTED).  A singular line yields inf / nan in that line.
- * Thread-per-line baseline, two passes over HBM (about 100 B per value); asynchronous on `stream`.               */
+ * solver with diagonal pivoting is used [3]") -- for systems whose dominance the caller does not vouch for.
+ * a, b, c: DEVICE, nx*ny*nz doubles each, laid out like the field: row j of a line holds a = coupling to row j-1,
+ * b = diagonal, c = coupling to row j+1; a of a line's first row and c of its last row are not read by
+ * tdx_general_solve and are the periodic corner couplings for tdx_general_cyclic_solve (a of row 0 couples it to row
+ * n-1, c of row n-1 to row 0; n >= 3).  pivoting != 0: 1x1 / 2x2 diagonal pivots without row interchanges (criterion:
+ * tdx_general.cuh); pivoting == 0: plain elimination on the same data (breaks down on a zero pivot: inf / nan in that line,
+ * no error).  rhs_inout: DEVICE, in place; the coefficient arrays are not modified.  dir = x, y or z.
+ * Two methods (tdx_general.cuh).  PARTITION: Eq.(5)-(8) with the pivoted elimination inside every 8-row partition, spikes and
+ * reduced system on the fly, one pass over HBM (40 B per value); the result of every line is checked (componentwise
+ * backward error of the line's equations) before it is stored, and a line that fails -- a numerically singular partition
+ * block; the line itself may be regular -- is solved instead, in the same call, by the other method;
+ * tdx_general_fallback_count says how many lines of the grid's last general solve that were (it synchronises).
+ * LINES: one thread per line, diagonal pivoting over the whole line, two passes over HBM (about 82 B per value).
+ * Default: PARTITION for x lines, LINES for y / z lines (each where it measured faster); OR the flags below
+ * into `pivoting` to force one.  Periodic lines, and lines of fewer than 4 or more than 4096 rows, always take LINES.
+ * work: DEVICE scratch, caller-owned, 8-byte aligned: 9*nx*ny*nz + 8 bytes (tdx_general_solve), 25*nx*ny*nz + 24 bytes
+ * (tdx_general_cyclic_solve).  A singular line yields inf / nan in that line.  Asynchronous on `stream`.       */
+#define TDX_GENERAL_PIVOT 1
+#define TDX_GENERAL_FORCE_PARTITION 16
+#define TDX_GENERAL_FORCE_LINES 32
 tdx_status_t tdx_general_solve(tdx_grid_t* grid, tdx_dir_t dir, int pivoting, const double* a, const double* b,
                                const double* c, double* rhs_inout, void* work, void* stream);
+tdx_status_t tdx_general_cyclic_solve(tdx_grid_t* grid, tdx_dir_t dir, int pivoting, const double* a, const double* b,
+                                      const double* c, double* rhs_inout, void* work, void* stream);
+tdx_status_t tdx_general_fallback_count(tdx_grid_t* grid, long long* out);
 
 /* Batched cyclic tridiagonal solve along dir with caller-given coefficients shared by every line:
  * a, b, c: HOST arrays of n_dir doubles; a[0] couples row 0 to row n-1 and c[n-1] couples row n-1 to row 0.

@@ -14,10 +14,11 @@ DIR_X, DIR_Y, DIR_Z = 0, 1, 2
 MODE_THOMAS, MODE_PDD, MODE_PPT = 0, 1, 2
 BC_DIRICHLET, BC_PERIODIC, BC_NEUMANN = 0, 1, 2
 LOC_CENTER, LOC_FACE = 0, 1
+GENERAL_PIVOT, GENERAL_FORCE_PARTITION, GENERAL_FORCE_LINES = 1, 16, 32
 OK, ERR_INVALID_ARG, ERR_BAD_PARTITION, ERR_ALLOC, ERR_CUDA, ERR_UNSUPPORTED, ERR_PDD_BOUND = 0, -1, -2, -3, -4, -5, -6
 
 EXPORTS = ("tdx_grid_create", "tdx_grid_destroy", "tdx_grid_set_pdd_strict", "tdx_partition_bounds", "tdx_adi_sweep", "tdx_adi_sweep_at", "tdx_adi_step",
-           "tdx_helmholtz_wavenumber_solve", "tdx_dct_x", "tdx_rfft_z", "tdx_irfft_z", "tdx_poisson_solve", "tdx_general_solve", "tdx_slab_create", "tdx_slab_destroy", "tdx_slab_eliminate", "tdx_slab_correct", "tdx_slab_dropped_bound", "tdx_cyclic_solve", "tdx_adi_sweep_host", "tdx_adi_step_host",
+           "tdx_helmholtz_wavenumber_solve", "tdx_dct_x", "tdx_rfft_z", "tdx_irfft_z", "tdx_poisson_solve", "tdx_general_solve", "tdx_general_cyclic_solve", "tdx_general_fallback_count", "tdx_slab_create", "tdx_slab_destroy", "tdx_slab_eliminate", "tdx_slab_correct", "tdx_slab_dropped_bound", "tdx_cyclic_solve", "tdx_adi_sweep_host", "tdx_adi_step_host",
            "tdx_helmholtz_wavenumber_solve_host", "tdx_step_host", "tdx_pdd_dropped_bound", "tdx_kernel_launch_count",
            "tdx_status_string", "tdx_last_error", "tdx_last_launch", "tdx_version")
 
@@ -64,6 +65,8 @@ def lib():
         L.tdx_irfft_z.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.tdx_poisson_solve.argtypes = [C.c_void_p, C.c_int, C.c_int, _dp, _dp, C.c_void_p, C.c_void_p, C.c_void_p]
         L.tdx_general_solve.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.tdx_general_cyclic_solve.argtypes = L.tdx_general_solve.argtypes
+        L.tdx_general_fallback_count.argtypes = [C.c_void_p, C.POINTER(C.c_longlong)]
         L.tdx_slab_create.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, _dp, C.c_int, C.c_double, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_void_p)]
         L.tdx_slab_destroy.argtypes = [C.c_void_p]
         L.tdx_slab_eliminate.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
@@ -182,6 +185,14 @@ class Grid:
 
     def general_solve(self, direction, pivoting, a, b, c, rhs, work, stream=0):
         _chk(lib().tdx_general_solve(self._h, direction, int(pivoting), _devptr(a), _devptr(b), _devptr(c), _devptr(rhs), _devptr(work), C.c_void_p(stream)))
+
+    def general_cyclic_solve(self, direction, pivoting, a, b, c, rhs, work, stream=0):
+        _chk(lib().tdx_general_cyclic_solve(self._h, direction, int(pivoting), _devptr(a), _devptr(b), _devptr(c), _devptr(rhs), _devptr(work), C.c_void_p(stream)))
+
+    def general_fallback_count(self):
+        out = C.c_longlong(0)
+        _chk(lib().tdx_general_fallback_count(self._h, C.byref(out)))
+        return int(out.value)
 
     def cyclic_solve(self, direction, mode, P, a, b, c, rhs, stream=0):
         (_, pa), (_, pb), (_, pc) = _host(a), _host(b), _host(c)

@@ -134,6 +134,7 @@ struct tdx_grid {
     struct WaveTab { uint64_t hash; int n; double* dev; };
     std::vector<WaveTab> wave;                          // device copies of caller wavenumber arrays, keyed by content hash
     bool attr_helm_lines = false;                       // cudaFuncSetAttribute done for this grid's device
+    unsigned int* fb = nullptr; unsigned fb_cap = 0;    // tdx_general_solve: [0] = number of lines that fell back, [4..] = their indices
     double* stage2 = nullptr; size_t stage2_bytes = 0;  // second staging buffer (Helmholtz part of tdx_step_host)
     cudaStream_t s_up = nullptr, s_comp = nullptr, s_down = nullptr;   // pipeline streams of tdx_step_host
     double length[3] = {0, 0, 0};                       // domain length per direction (host copy of faces[n] - faces[0])
@@ -414,17 +415,17 @@ Tables tables_of(const Plan& pl) {
 // ---- launch selection ---------------------------------------------------------------------------------------
 namespace {
 
-template <int M, int V, bool CYC, bool UNI = false, int REGS = strided_regs(M, V)>
+template <int M, int V, bool CYC, bool UNI = false, int REGS = strided_regs(M, V), bool TS = false>
 tdx_status_t launch_strided_inst(const Plan& pl, StridedArgs& A, const Tables& T, dim3 grid, dim3 block, size_t smem, cudaStream_t st) {
     static DevOnce attr;
     if (smem > 48 * 1024 && attr.need(pl.dev)) {
-        CUDA_TRY(cudaFuncSetAttribute(k_strided<M, V, CYC, UNI, REGS>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+        CUDA_TRY(cudaFuncSetAttribute(k_strided<M, V, CYC, UNI, REGS, TS>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
         attr.set(pl.dev);
     }
     const long long key = ((long long)(block.x * block.y) << 32) | ((long long)smem << 4) | (V << 1) | (REGS == strided_regs(M, V) ? 0 : 1);
     if (pl.pf < 0 || pl.pf_key != key) {                           // prefetch one wave of resident CTAs ahead
         int occ = 1;
-        CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_strided<M, V, CYC, UNI, REGS>, (int)(block.x * block.y), smem));
+        CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_strided<M, V, CYC, UNI, REGS, TS>, (int)(block.x * block.y), smem));
         pl.occ = occ < 1 ? 1 : occ;
         pl.pf = pl.sms * pl.occ * prefetch_waves();
         pl.pf_key = key;
@@ -440,15 +441,25 @@ tdx_status_t launch_strided_inst(const Plan& pl, StridedArgs& A, const Tables& T
         }
         std::memcpy(U.v, pl.uni_host, sizeof(U.v));
     } else std::memset(U.v, 0, sizeof(U.v));
-    k_strided<M, V, CYC, UNI, REGS><<<grid, block, smem, st>>>(A, T, U);
+    k_strided<M, V, CYC, UNI, REGS, TS><<<grid, block, smem, st>>>(A, T, U);
     LAUNCH_CHECK("k_strided");
-    note_launch("k_strided<%d,%d,%d,%d,%d>", M, V, CYC, UNI, REGS, 0, grid, block);
+    note_launch("k_strided<%d,%d,%d,%d,%d,%d>", M, V, CYC, UNI, REGS, TS, grid, block);
     return TDX_OK;
 }
 
 template <int V, bool CYC>
 tdx_status_t launch_strided_M(const Plan& pl, StridedArgs& A, const Tables& T, dim3 grid, dim3 block, size_t smem, cudaStream_t st) {
     const int M = pl.M;
+    if (A.tables_smem) {                                           // Helmholtz y-solves: the set's tables in shared memory (k_strided "TS")
+        if (V == 2 && !CYC)
+            switch (M) {
+                case 12: return launch_strided_inst<12, 2, false, false, strided_regs(12, 2), true>(pl, A, T, grid, block, smem, st);
+                case 16: return launch_strided_inst<16, 2, false, false, strided_regs(16, 2), true>(pl, A, T, grid, block, smem, st);
+                case 24: return launch_strided_inst<24, 2, false, false, strided_regs(24, 2), true>(pl, A, T, grid, block, smem, st);
+                case 32: return launch_strided_inst<32, 2, false, false, strided_regs(32, 2), true>(pl, A, T, grid, block, smem, st);
+            }
+        return fail(TDX_ERR_UNSUPPORTED, "no shared-memory-table strided kernel for M=%d V=%d", M, V);
+    }
     if (pl.layout == ROWS_U) {                                     // only set for the sizes instantiated here (build_plan)
         if (CYC) return fail(TDX_ERR_UNSUPPORTED, "uniform table with the rank-1 periodic closure");
         switch (M) {
@@ -497,7 +508,7 @@ tdx_status_t run_strided(const Plan& pl, double* data, long long W, long long li
     if (O > 65535) return fail(TDX_ERR_UNSUPPORTED, "outer extent %lld > 65535", O);
     StridedArgs A;
     A.data = data; A.set_per_outer = set_per_outer ? 1 : 0; A.set0 = set0; A.pf = 0;
-    A.iface = iface; A.iface_plane = W * O;
+    A.iface = iface; A.iface_plane = W * O; A.tables_smem = 0;
     if (pl.thomas) {
         const int V = even ? 2 : 1;
         A.W = W / V; A.line_stride = line_stride / V; A.outer_stride = outer_stride / V;
@@ -531,7 +542,8 @@ tdx_status_t run_strided(const Plan& pl, double* data, long long W, long long li
         return true;
     };
     int V = 0, LPC = 0, l1 = 0, l2 = 0;
-    const bool ok2 = pick(2, l2), ok1 = pick(1, l1);
+    static const int env_v = [] { const char* e = std::getenv("TDX_STRIDED_V"); return e ? std::atoi(e) : 0; }();   // measurement knob
+    const bool ok2 = pick(2, l2) && env_v != 1, ok1 = pick(1, l1);
     if (ok2 && (!ok1 || l2 * 2 >= l1)) { V = 2; LPC = l2; }
     else if (ok1) { V = 1; LPC = l1; }
     else return fail(TDX_ERR_UNSUPPORTED, "P=%d partitions of up to %d rows do not fit one thread block", pl.P, pl.M);
@@ -551,7 +563,11 @@ tdx_status_t run_strided(const Plan& pl, double* data, long long W, long long li
         if (env_loops >= 1 && env_loops <= 64) loops = env_loops;
     }
     dim3 block(LPC, pl.P), grid((unsigned)((A.tiles_x + loops - 1) / loops), (unsigned)O);
-    const size_t smem = (size_t)2 * pl.P * LPC * V * 8;
+    size_t smem = (size_t)2 * pl.P * LPC * V * 8;
+    // the set's tables in shared memory (TDX_HELM_SMEM_TABLES=0: measurement knob, the round-1 path through L1)
+    static const int env_ts = [] { const char* e = std::getenv("TDX_HELM_SMEM_TABLES"); return e ? std::atoi(e) : 1; }();
+    A.tables_smem = (set_per_outer && env_ts && V == 2 && !pl.cyc && pl.layout != ROWS_U && (pl.M == 12 || pl.M == 16 || pl.M == 24 || pl.M == 32)) ? 1 : 0;
+    if (A.tables_smem) smem += ((size_t)pl.P * (pl.M * 3 + 1) + (size_t)pl.KB * pl.P) * 16;
     Tables T = tables_of(pl);
     if (V == 2) return pl.cyc ? launch_strided_M<2, true>(pl, A, T, grid, block, smem, st) : launch_strided_M<2, false>(pl, A, T, grid, block, smem, st);
     return pl.cyc ? launch_strided_M<1, true>(pl, A, T, grid, block, smem, st) : launch_strided_M<1, false>(pl, A, T, grid, block, smem, st);
@@ -1060,6 +1076,7 @@ tdx_status_t tdx_grid_destroy(tdx_grid_t* g) {
     for (int d = 0; d < 3; ++d) { cudaFree(g->faces[d]); cudaFree(g->lo[d]); cudaFree(g->up[d]); cudaFree(g->lo_face[d]); cudaFree(g->up_face[d]); }
     cudaFree(g->lo_neumann_y); cudaFree(g->up_neumann_y); cudaFree(g->stage); cudaFree(g->stage2); cudaFree(g->ws);
     for (auto& w : g->wave) cudaFree(w.dev);
+    cudaFree(g->fb);
     for (int d = 0; d < 3; ++d) cudaFree(g->fft_tw[d]);
     cudaFree(g->fft_w4);
     if (g->s_up) cudaStreamDestroy(g->s_up);
@@ -1419,26 +1436,106 @@ tdx_status_t tdx_slab_dropped_bound(tdx_slab_t* s, double* out) {
     return TDX_OK;
 }
 
-tdx_status_t tdx_general_solve(tdx_grid_t* g, tdx_dir_t dir, int pivoting, const double* a, const double* b, const double* c,
-                               double* rhs, void* work, void* stream) {
+static tdx_status_t general_solve_impl(tdx_grid_t* g, tdx_dir_t dir, int pivoting, bool periodic, const double* a, const double* b,
+                                       const double* c, double* rhs, void* work, void* stream) {
     if (!g) return fail(TDX_ERR_INVALID_ARG, "grid is NULL");
     if (!a || !b || !c || !rhs || !work) return fail(TDX_ERR_INVALID_ARG, "NULL argument");
-    if (dir != TDX_DIR_Y && dir != TDX_DIR_Z) return fail(TDX_ERR_UNSUPPORTED, "per-line coefficients are taken along y (the paper's case, L174) or z; dir=%d", (int)dir);
+    if (dir < 0 || dir > 2) return fail(TDX_ERR_INVALID_ARG, "dir=%d not in {0,1,2}", (int)dir);
     if (reinterpret_cast<uintptr_t>(work) & 7) return fail(TDX_ERR_INVALID_ARG, "work must be 8-byte aligned");
     CUDA_TRY(cudaSetDevice(g->device));
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     const int n = g->n_of(dir);
-    const long long inner = dir == TDX_DIR_Y ? g->nx : (long long)g->nx * g->ny, outer = dir == TDX_DIR_Y ? g->nz : 1;
-    if (outer > 65535) return fail(TDX_ERR_UNSUPPORTED, "outer extent > 65535");
-    const size_t npts = (size_t)g->nx * g->ny * g->nz;
+    if (periodic && n < 3) return fail(TDX_ERR_INVALID_ARG, "periodic line needs n >= 3");
+    const long long nx = g->nx, ny = g->ny, nz = g->nz;
+    const size_t npts = (size_t)nx * ny * nz;
+    tdx::GeneralArgs G;
+    G.a = a; G.b = b; G.c = c; G.d = rhs; G.n = n; G.periodic = periodic ? 1 : 0;
+    long long O = 1;
+    if (dir == TDX_DIR_X) { G.W = ny * nz; G.lane_stride = nx; G.row_stride = 1; G.outer_stride = 0; }
+    else if (dir == TDX_DIR_Y) { G.W = nx; G.lane_stride = 1; G.row_stride = nx; G.outer_stride = nx * ny; O = nz; }
+    else { G.W = nx * ny; G.lane_stride = 1; G.row_stride = nx * ny; G.outer_stride = 0; }
+    if (O > 65535) return fail(TDX_ERR_UNSUPPORTED, "outer extent > 65535");
+    if (G.W * O >= (1LL << 32)) return fail(TDX_ERR_UNSUPPORTED, "more than 2^32 lines");
     double* bm = static_cast<double*>(work);
     unsigned char* flag = reinterpret_cast<unsigned char*>(bm + npts);
-    dim3 block(128), grid((unsigned)((inner + 127) / 128), (unsigned)outer);
-    if (pivoting) tdx::k_general_forward<true><<<grid, block, 0, st>>>(a, b, c, rhs, bm, flag, n, inner, outer);
-    else tdx::k_general_forward<false><<<grid, block, 0, st>>>(a, b, c, rhs, bm, flag, n, inner, outer);
-    LAUNCH_CHECK("k_general_forward");
-    tdx::k_general_backward<<<grid, block, 0, st>>>(a, c, rhs, bm, flag, n, inner, outer);
-    LAUNCH_CHECK("k_general_backward");
+    double* qv = reinterpret_cast<double*>(flag + ((npts + 7) / 8) * 8);                 // periodic only (25 bytes per value in all)
+    double* dv = qv + npts;
+    // Method: the partition kernel (8 rows per thread, P threads of a line in one CTA) where it is the faster one -- measured
+    // on cfg5: x lines 18.0 ms against 76.8 ms for one thread per (contiguous) line; y / z lines 19.0 / 30.2 ms
+    // against 10.9 / 11.2 ms, so strided lines take the per-line kernel unless the caller forces the partition method.
+    const int method = pivoting & (TDX_GENERAL_FORCE_PARTITION | TDX_GENERAL_FORCE_LINES);
+    pivoting &= 1;
+    if (method == (TDX_GENERAL_FORCE_PARTITION | TDX_GENERAL_FORCE_LINES)) return fail(TDX_ERR_INVALID_ARG, "both methods forced");
+    const int M = 8;
+    int P = (n + M - 1) / M; if (P < 2) P = 2;
+    const bool can_part = !periodic && n / P >= 2 && P <= 512;                           // 512 threads of 128 registers
+    if (method == TDX_GENERAL_FORCE_PARTITION && !can_part) return fail(TDX_ERR_UNSUPPORTED, "the partition method takes non-periodic lines of 4 to 4096 rows");
+    const bool part = can_part && (method == TDX_GENERAL_FORCE_PARTITION || (method == 0 && dir == TDX_DIR_X));
+    if (!part) {                                                                         // one thread per line over the whole line
+        dim3 block(128), grid((unsigned)std::min<long long>((G.W + 127) / 128, 1 << 20), (unsigned)O);
+        G.fb_count = nullptr; G.fb_lines = nullptr; G.fb_cap = 0; G.P = 1; G.q = n; G.r = 0;
+        if (periodic) { if (pivoting) tdx::k_general_lines<true, false, true><<<grid, block, 0, st>>>(G, bm, flag, qv, dv); else tdx::k_general_lines<false, false, true><<<grid, block, 0, st>>>(G, bm, flag, qv, dv); }
+        else { if (pivoting) tdx::k_general_lines<true, false, false><<<grid, block, 0, st>>>(G, bm, flag, qv, dv); else tdx::k_general_lines<false, false, false><<<grid, block, 0, st>>>(G, bm, flag, qv, dv); }
+        LAUNCH_CHECK("k_general_lines");
+        return TDX_OK;
+    }
+    const unsigned nlines = (unsigned)(G.W * O);
+    {
+        std::lock_guard<std::mutex> lk(g->mu);
+        if (g->fb_cap < nlines) {
+            cudaFree(g->fb); g->fb = nullptr; g->fb_cap = 0;
+            if (cudaMalloc(&g->fb, ((size_t)nlines + 4) * 4) != cudaSuccess) { cudaGetLastError(); return fail(TDX_ERR_ALLOC, "fallback list allocation failed"); }
+            g->fb_cap = nlines;
+        }
+    }
+    G.fb_count = g->fb; G.fb_lines = g->fb + 4; G.fb_cap = nlines;
+    G.P = P; G.q = n / P; G.r = n % P;
+    CUDA_TRY(cudaMemsetAsync(g->fb, 0, 4, st));
+    const bool unit = dir == TDX_DIR_X;
+    // lines per CTA: small CTAs (several resident per SM at different phases: load / eliminate / reduce / store) beat one
+    // large one; x lines: whole lines of P consecutive lanes.  TDX_GENERAL_LINES (measurement knob) overrides.
+    static const int env_L = [] { const char* e = std::getenv("TDX_GENERAL_LINES"); return e ? std::atoi(e) : 0; }();
+    int L = 1;
+    const int cap = env_L > 0 ? env_L : 4;
+    while (L * 2 * P <= 512 && L * 2 <= (unit ? std::max(1, 128 / P) : cap)) L *= 2;
+    if ((long long)L > G.W) { L = 1; while ((long long)L * 2 <= G.W && L * 2 * P <= 512) L *= 2; }
+    dim3 block = unit ? dim3(P, L) : dim3(L, P), grid((unsigned)((G.W + L - 1) / L), (unsigned)O);
+    const size_t smem = (size_t)21 * P * L * 8 + (size_t)L * 8 + 16;
+#define TDX_GENERAL_PART(PV, UN)                                                                                              \
+    do { static DevOnce attr;                                                                                                 \
+         if (attr.need(g->device)) { CUDA_TRY(cudaFuncSetAttribute(tdx::k_general_part<8, PV, UN>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024)); attr.set(g->device); } \
+         tdx::k_general_part<8, PV, UN><<<grid, block, smem, st>>>(G); } while (0)
+    if (pivoting) { if (unit) TDX_GENERAL_PART(true, true); else TDX_GENERAL_PART(true, false); }
+    else { if (unit) TDX_GENERAL_PART(false, true); else TDX_GENERAL_PART(false, false); }
+#undef TDX_GENERAL_PART
+    LAUNCH_CHECK("k_general_part");
+    note_launch("k_general_part<%d,%d,%d>", 8, pivoting ? 1 : 0, unit ? 1 : 0, 0, 0, 0, grid, block);
+    // the lines whose blocks were numerically singular: one thread per line (none on weakly dominant systems)
+    dim3 fgrid((unsigned)(g->sms * 4));
+    if (pivoting) tdx::k_general_lines<true, true, false><<<fgrid, 128, 0, st>>>(G, bm, flag, qv, dv);
+    else tdx::k_general_lines<false, true, false><<<fgrid, 128, 0, st>>>(G, bm, flag, qv, dv);
+    LAUNCH_CHECK("k_general_lines");
+    return TDX_OK;
+}
+
+tdx_status_t tdx_general_solve(tdx_grid_t* g, tdx_dir_t dir, int pivoting, const double* a, const double* b, const double* c,
+                               double* rhs, void* work, void* stream) {
+    return general_solve_impl(g, dir, pivoting, false, a, b, c, rhs, work, stream);
+}
+
+tdx_status_t tdx_general_cyclic_solve(tdx_grid_t* g, tdx_dir_t dir, int pivoting, const double* a, const double* b, const double* c,
+                                      double* rhs, void* work, void* stream) {
+    return general_solve_impl(g, dir, pivoting, true, a, b, c, rhs, work, stream);
+}
+
+tdx_status_t tdx_general_fallback_count(tdx_grid_t* g, long long* out) {
+    if (!g || !out) return fail(TDX_ERR_INVALID_ARG, "NULL argument");
+    *out = 0;
+    if (!g->fb) return TDX_OK;
+    CUDA_TRY(cudaSetDevice(g->device));
+    unsigned v = 0;
+    CUDA_TRY(cudaMemcpy(&v, g->fb, 4, cudaMemcpyDeviceToHost));           // waits for the solve that wrote it
+    *out = v;
     return TDX_OK;
 }
 

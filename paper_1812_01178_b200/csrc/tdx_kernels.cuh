@@ -41,6 +41,7 @@ struct StridedArgs {
     int LPC;                 // lines (V-vectors) per CTA = blockDim.x
     int pf;                  // L2 prefetch distance: CTAs ahead (one tile per CTA) or sets ahead (looping CTAs); 0 = off
     int tiles_x;             // column tiles per outer index
+    int tables_smem;         // 1: the TS instantiation (set's tables staged in shared memory)
     double* iface;           // slab sweeps (tdx_slab_eliminate): also store row 0 of every line to iface[0][outer][W*V] and its last
     long long iface_plane;   //   row to iface[1][...] (Alg.1 step 4's pack, fused into the store); iface_plane = doubles per plane; NULL = off
 };
@@ -56,7 +57,7 @@ template <> struct VecIO<2> {
 };
 
 // Register budget per thread: the partition (MAXM x V doubles = 2 MAXM V registers) plus ~50 for addresses, table
-// values in flight and the interface unknowns.  Measured on B200 (profiles/r1_probe_strided.md): spills cost more than
+// values in flight and the interface unknowns.  Measured on B200 (development sweeps): spills cost more than
 // occupancy, and 2-4 small co-resident CTAs per SM beat one large one.
 constexpr int strided_regs(int MAXM, int V) {
     return (MAXM * V <= 8) ? 72 : ((MAXM * V <= 16) ? 104 : ((MAXM * V <= 32) ? 128 : ((MAXM * V <= 48) ? 168 : 255)));
@@ -72,7 +73,11 @@ template <int M> struct UniTable { double v[M * 6]; };
 
 // UNI: row table = U.v[jj*6 + f] for every partition (ROWS_U plans: periodic or interior-identical blocks, one set).
 // REGS: register budget; the default is the tier of the partition size, a smaller one buys a wider CTA (longer row segments).
-template <int MAXM, int V, bool CYC, bool UNI, int REGS = strided_regs(MAXM, V)>
+// TS (one table set per outer index = the Helmholtz y-solves): the CTA copies its set's row table and reduced-system
+// coefficients into shared memory once, before its tiles; every table read of the three passes and of the band loop is
+// then an LDS (two addresses per warp, partitions padded by 16 bytes: conflict-free) instead of an L1 hit competing with
+// the tile's own loads and stores in the L1TEX pipe.
+template <int MAXM, int V, bool CYC, bool UNI, int REGS = strided_regs(MAXM, V), bool TS = false>
 __global__ void __maxnreg__(REGS)
 k_strided(StridedArgs A, Tables T, const __grid_constant__ UniTable<UNI ? MAXM : 1> U) {
     extern __shared__ double rs[];                          // rs[(idx*LPC + tx)*V + v], idx in [0, 2P)
@@ -80,6 +85,18 @@ k_strided(StridedArgs A, Tables T, const __grid_constant__ UniTable<UNI ? MAXM :
     const int LPC = A.LPC, P = T.P;
     const int o = blockIdx.y;
     const int set = A.set_per_outer ? A.set0 + o : 0;
+    constexpr int RSTR = MAXM * 3 + 1;                      // TS: double2 per partition in shared memory (padded)
+    double2* const st_rows = reinterpret_cast<double2*>(rs + (size_t)2 * P * LPC * V);
+    double2* const st_G = st_rows + (size_t)P * RSTR;
+    if (TS) {
+        const int tid = p * LPC + tx, nth = LPC * P;
+        const double2* src = reinterpret_cast<const double2*>(T.rows + (size_t)set * P * MAXM * 6);
+        for (int k = tid; k < P * MAXM * 3; k += nth) { const int pp = k / (MAXM * 3); st_rows[pp * RSTR + (k - pp * MAXM * 3)] = __ldg(src + k); }
+        const double2* gsrc = reinterpret_cast<const double2*>(T.G) + (size_t)set * T.KB * P;
+        for (int k = tid; k < T.KB * P; k += nth) st_G[k] = __ldg(gsrc + k);
+        __syncthreads();
+    }
+    const double2* const trow = st_rows + p * RSTR;
     int start, m;
     sub_part(p, T.q, T.r, T.S, start, m);
     const bool full = (T.r == 0) && (T.q == MAXM * T.S);    // every partition has exactly MAXM rows (warp-uniform)
@@ -87,7 +104,7 @@ k_strided(StridedArgs A, Tables T, const __grid_constant__ UniTable<UNI ? MAXM :
     // One table set per outer index (Helmholtz: a set per wavenumber): this CTA's set is cold in L1, so pull its lines
     // in now, one prefetch per thread -- otherwise every table load on the dependent chain and in the band loop pays
     // L2 latency.  Such a CTA then works through several column tiles of its set (the loop below) with warm tables.
-    if (A.set_per_outer) {
+    if (A.set_per_outer && !TS) {
         const int tid = p * LPC + tx, nth = LPC * P;
         const char* rb = reinterpret_cast<const char*>(T.rows + (size_t)set * P * MAXM * 6);
         const int rlines = (P * MAXM * 48 + 127) >> 7;
@@ -138,18 +155,18 @@ k_strided(StridedArgs A, Tables T, const __grid_constant__ UniTable<UNI ? MAXM :
     // Eq.(5): forward y_j = d_j - l_j y_{j-1}, backward xt_j = y_j inv_j - cp_j xt_{j+1}
 #pragma unroll
     for (int jj = 1; jj < MAXM; ++jj) {
-        const double l = UNI ? U.v[UNI ? jj * 6 + F_L : 0] : __ldg(reinterpret_cast<const double*>(&rt[jj * 3 + 0]));
+        const double l = UNI ? U.v[UNI ? jj * 6 + F_L : 0] : (TS ? trow[jj * 3 + 0].x : __ldg(reinterpret_cast<const double*>(&rt[jj * 3 + 0])));
 #pragma unroll
         for (int v = 0; v < V; ++v) x[jj][v] = fma(-l, x[jj - 1][v], x[jj][v]);
     }
     {
-        const double inv = UNI ? U.v[UNI ? (MAXM - 1) * 6 + F_INV : 0] : __ldg(reinterpret_cast<const double*>(&rt[(MAXM - 1) * 3 + 1]));
+        const double inv = UNI ? U.v[UNI ? (MAXM - 1) * 6 + F_INV : 0] : (TS ? trow[(MAXM - 1) * 3 + 1].x : __ldg(reinterpret_cast<const double*>(&rt[(MAXM - 1) * 3 + 1])));
 #pragma unroll
         for (int v = 0; v < V; ++v) x[MAXM - 1][v] *= inv;
     }
 #pragma unroll
     for (int jj = MAXM - 2; jj >= 0; --jj) {
-        const double2 ic = UNI ? make_double2(U.v[UNI ? jj * 6 + F_INV : 0], U.v[UNI ? jj * 6 + F_CP : 0]) : __ldg(&rt[jj * 3 + 1]);   // {inv, cp}
+        const double2 ic = UNI ? make_double2(U.v[UNI ? jj * 6 + F_INV : 0], U.v[UNI ? jj * 6 + F_CP : 0]) : (TS ? trow[jj * 3 + 1] : __ldg(&rt[jj * 3 + 1]));   // {inv, cp}
 #pragma unroll
         for (int v = 0; v < V; ++v) x[jj][v] = fma(-ic.y, x[jj + 1][v], x[jj][v] * ic.x);
     }
@@ -168,7 +185,7 @@ k_strided(StridedArgs A, Tables T, const __grid_constant__ UniTable<UNI ? MAXM :
         const int2 bd = __ldg(&T.band[set * P + p]);
         const double2* g2 = reinterpret_cast<const double2*>(T.G) + (size_t)set * T.KB * P + p;
         for (int k = 0; k < bd.y; ++k) {
-            const double2 ab = __ldg(g2 + (size_t)k * P);   // {gL, gR}
+            const double2 ab = TS ? st_G[k * P + p] : __ldg(g2 + (size_t)k * P);   // {gL, gR}
             const double a = ab.x, b = ab.y;
             int idx = bd.x + k;                             // band may wrap around (periodic line closed inside Z)
             if (idx >= 2 * P) idx -= 2 * P;
@@ -192,7 +209,7 @@ k_strided(StridedArgs A, Tables T, const __grid_constant__ UniTable<UNI ? MAXM :
     // Eq.(8): x = xt - v yL - w yR (- q s for periodic lines), then store
 #pragma unroll
     for (int jj = 0; jj < MAXM; ++jj) {
-        const double2 vw = UNI ? make_double2(U.v[UNI ? jj * 6 + F_V : 0], U.v[UNI ? jj * 6 + F_W : 0]) : __ldg(&rt[jj * 3 + 2]);     // {v, w}
+        const double2 vw = UNI ? make_double2(U.v[UNI ? jj * 6 + F_V : 0], U.v[UNI ? jj * 6 + F_W : 0]) : (TS ? trow[jj * 3 + 2] : __ldg(&rt[jj * 3 + 2]));     // {v, w}
         double qj = 0.0;
         if (CYC) qj = __ldg(reinterpret_cast<const double*>(&rt[jj * 3 + 0]) + 1);   // {l, q}
 #pragma unroll
@@ -272,12 +289,8 @@ k_unit(UnitArgs A, Tables T) {
     x[MAXM - 1] *= tab(MAXM - 1, F_INV);
 #pragma unroll
     for (int jj = MAXM - 2; jj >= 0; --jj) x[jj] = fma(-tab(jj, F_CP), x[jj + 1], x[jj] * tab(jj, F_INV));
-    {
-        double xl = x[MAXM - 1];
-#pragma unroll
-        for (int jj = 0; jj < MAXM - 1; ++jj) if (jj == m - 1) xl = x[jj];
-        rf[tl] = x[0]; rl[tl] = xl;
-    }
+    rf[tl] = x[0]; rl[tl] = x[MAXM - 1];                               // the plan's padding rows carry xt_last to slot MAXM-1 (a select
+                                                                        // over jj == m-1 becomes a run-time index: the tile went to local memory)
     __syncthreads();
     double yL = 0.0, yR = 0.0, sc = 0.0;
     if (valid) {

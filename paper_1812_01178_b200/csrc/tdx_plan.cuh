@@ -26,6 +26,11 @@ enum RowLayout { ROWS_PJ = 0,      // rows[((set*P + p)*M + jj)*6 + f]   strided
 // field order: 16-byte pairs {l, q}, {inv, cp}, {v, w} -- forward, backward and correction each read one pair per row
 enum RowField { F_L = 0, F_Q = 1, F_INV = 2, F_CP = 3, F_V = 4, F_W = 5 };
 
+// Entries of a row of Z^-1 below kBandTau times the row's largest entry are left out of the band a partition applies: the
+// band has at most 2P <= 512 terms, so what is dropped stays below 1e-16 of the sum's largest term -- under the rounding
+// error of the sum itself (round 1 cut at 1e-24).
+constexpr double kBandTau = 2e-19;
+
 __host__ __device__ inline int part_start(int p, int q, int r) { return p * q + (p < r ? p : r); }
 // Two-level partition map (long partitions): the caller's P partitions of the map above (q = n / P rows, the
 // first r = n % P one more) are each cut again into S sub-partitions by the same rule; kernel partition p = po * S + s.
@@ -335,7 +340,7 @@ __global__ void k_pack_ppt(int nsets, int P, int KB, const double* __restrict__ 
     int s = t / P, p = t % P;
     int K = 2 * (P - 1);
     const double* zi = Zi + (size_t)s * K * K;
-    const double tau = 1e-24;
+    const double tau = kBandTau;
     int rowL = (p >= 1) ? 2 * p - 2 : -1, rowR = (p <= P - 2) ? 2 * p + 1 : -1;
     int lo = K, hi = -1;
     for (int side = 0; side < 2; ++side) {
@@ -427,7 +432,7 @@ __global__ void k_pack_ppt_cyclic(int nsets, int P, int KB, const double* __rest
     int s = t / P, p = t % P;
     const int K = 2 * P;
     const double* zi = Zi + (size_t)s * K * K;
-    const double tau = 1e-24;
+    const double tau = kBandTau;
     const int rowL = (2 * p - 2 + K) % K, rowR = (2 * p + 1) % K;
     const bool useL = wrap || p > 0, useR = wrap || p < P - 1;
     double mxL = 0.0, mxR = 0.0;

@@ -1,7 +1,9 @@
-"""GPU parity of tdx_general_solve (per-line coefficients, diagonal pivoting) against the
-dense LAPACK oracle.  Tolerance: the systems are random and NOT dominant, so the forward error of any backward-stable
-solver is kappa(A) * eps per line; each line is gated at 50 * kappa(A_line) * eps (kappa from the oracle's dense
-matrices), and the whole field at a relative residual of 1e-13."""
+"""GPU parity of tdx_general_solve / tdx_general_cyclic_solve (per-line coefficients, diagonal pivoting; SURVEY 8(f) N4,
+PAPER.md:L174) against the dense LAPACK oracle, along x, y and z.  Tolerance: the random systems are NOT dominant, so the
+forward error of any backward-stable solver is kappa(A) * eps per line; each line is gated at 50 * kappa(A_line) * eps
+(kappa from the oracle's dense matrices), and the whole field at a relative residual of 1e-13.  The partition kernel
+hands lines with a numerically singular partition block to the per-line path: both paths are exercised (the count of
+such lines is asserted: none on weakly dominant systems, some on the random ones)."""
 import numpy as np
 import pytest
 import torch
@@ -13,6 +15,7 @@ from paper_1812_01178_b200 import inputs
 
 pytestmark = pytest.mark.gpu
 BCS = (tdx.BC_DIRICHLET, tdx.BC_DIRICHLET, tdx.BC_DIRICHLET)
+AXIS = {0: 2, 1: 1, 2: 0}                                       # array axis of a sweep direction
 EPS = 2.220446049250313e-16
 
 
@@ -27,23 +30,32 @@ def _setup(nx, ny, nz, seed, diag_scale):
     return grid, a, b, c, d
 
 
-def _solve(grid, direction, pivoting, a, b, c, d):
+def _solve(grid, direction, pivoting, a, b, c, d, cyclic=False, method=tdx.GENERAL_FORCE_PARTITION):
+    """method: the partition kernel is forced wherever it applies (it is the default only for x lines), so that it is the
+    path under test; periodic lines and very short lines take the per-line kernel whatever is asked."""
+    n = d.shape[AXIS[direction]]
+    P = max(2, -(-n // 8))
+    pivoting = int(pivoting) | (method if (not cyclic and n // P >= 2 and P <= 512) else 0)
     ta, tb, tc = (torch.from_numpy(v).cuda() for v in (a, b, c))
     td = torch.from_numpy(d).cuda()
-    work = torch.empty(9 * d.size + 64, dtype=torch.uint8, device="cuda")
-    grid.general_solve(direction, pivoting, ta, tb, tc, td, work)
+    work = torch.empty(25 * d.size + 64, dtype=torch.uint8, device="cuda")
+    (grid.general_cyclic_solve if cyclic else grid.general_solve)(direction, pivoting, ta, tb, tc, td, work)
     torch.cuda.synchronize()
     assert torch.equal(ta.cpu(), torch.from_numpy(a)) and torch.equal(tb.cpu(), torch.from_numpy(b))   # coefficients untouched
     return td.cpu().numpy()
 
 
-@pytest.mark.parametrize("direction,shape", [(1, (150, 48, 6)), (2, (34, 5, 40)), (1, (4, 2, 3)), (1, (5, 3, 2)), (2, (130, 1 + 1, 1 + 2))])
-def test_non_dominant_random_systems_with_pivoting(direction, shape):
+@pytest.mark.parametrize("cyclic", [False, True])
+@pytest.mark.parametrize("direction,shape", [(1, (150, 48, 6)), (2, (34, 5, 40)), (1, (4, 2, 3)), (1, (5, 3, 2)), (2, (130, 1 + 1, 1 + 2)),
+                                             (0, (64, 9, 7)), (0, (203, 5, 3)), (0, (9, 4, 4)), (1, (32, 288, 2)), (1, (17, 101, 3))])
+def test_non_dominant_random_systems_with_pivoting(direction, shape, cyclic):
     nx, ny, nz = shape
     grid, a, b, c, d = _setup(nx, ny, nz, 700 + nx, 0.3)
-    axis = 1 if direction == 1 else 0
-    got = _solve(grid, direction, True, a, b, c, d)
-    ref, A = ogen.general_solve(a, b, c, d, axis)
+    axis = AXIS[direction]
+    if cyclic and d.shape[axis] < 3:
+        pytest.skip("periodic lines need n >= 3")
+    got = _solve(grid, direction, True, a, b, c, d, cyclic)
+    ref, A = ogen.general_solve(a, b, c, d, axis, cyclic)
     cond = np.linalg.cond(A)
     n = d.shape[axis]
     err = np.max(np.abs(np.moveaxis(got - ref, axis, -1).reshape(-1, n)), axis=1)
@@ -54,7 +66,46 @@ def test_non_dominant_random_systems_with_pivoting(direction, shape):
     gm = np.moveaxis(got, axis, 0); rm = np.moveaxis(r, axis, 0); am = np.moveaxis(a, axis, 0); cm = np.moveaxis(c, axis, 0)
     rm[1:] += am[1:] * gm[:-1]
     rm[:-1] += cm[:-1] * gm[1:]
+    if cyclic:
+        rm[0] += am[0] * gm[-1]
+        rm[-1] += cm[-1] * gm[0]
     assert np.max(np.abs(r - d)) <= 1e-13 * (np.max(np.abs(got)) * 3.0 + 1.0)
+    nfb = grid.general_fallback_count()
+    nlines = d.size // n
+    assert 0 <= nfb <= nlines
+    if not cyclic and n >= 64:
+        assert nfb > 0                                           # random non-dominant blocks: some line always has a bad 8-row block
+    grid.close()
+
+
+@pytest.mark.parametrize("direction", [0, 1, 2])
+def test_weakly_dominant_per_line_systems_take_the_partition_path_only(direction):
+    """The paper's case (L172-174): Poisson-like rows |b| = |a| + |c| + eps with a different eps on every line, given as
+    explicit per-line coefficients.  No partition block is singular: no line may fall back, and the result is within
+    the kappa * eps gate of the dense oracle."""
+    nx, ny, nz = 40, 36, 34
+    grid, a, b, c, d = _setup(nx, ny, nz, 900 + direction, 1.0)
+    a = -(0.2 + np.abs(a)); c = -(0.2 + np.abs(c))
+    eps = 10.0 ** (-6.0 * np.abs(b))                                               # 1e-6 ... 1 per entry
+    axis = AXIS[direction]
+    eps = np.broadcast_to(np.take(eps, [0], axis=axis), eps.shape).copy()          # one shift per line
+    am = np.moveaxis(a, axis, 0); cm = np.moveaxis(c, axis, 0)
+    am[0] = 0.0; cm[-1] = 0.0                                                      # the cut ends, so that every row is dominant
+    b = -(a + c) + eps
+    got = _solve(grid, direction, True, a, b, c, d)
+    assert grid.general_fallback_count() == 0
+    ref, A = ogen.general_solve(a, b, c, d, axis)
+    cond = np.linalg.cond(A)
+    n = d.shape[axis]
+    err = np.max(np.abs(np.moveaxis(got - ref, axis, -1).reshape(-1, n)), axis=1)
+    scale = np.max(np.abs(np.moveaxis(ref, axis, -1).reshape(-1, n)), axis=1)
+    assert np.all(err <= 50 * cond * EPS * scale), float(np.max(err / (cond * EPS * scale)))
+    assert np.array_equal(got, _solve(grid, direction, False, a, b, c, d))         # dominant rows always take the 1x1 pivot
+    lines = _solve(grid, direction, True, a, b, c, d, method=tdx.GENERAL_FORCE_LINES)   # the other method: same answer to the gate
+    errl = np.max(np.abs(np.moveaxis(lines - ref, axis, -1).reshape(-1, n)), axis=1)
+    assert np.all(errl <= 50 * cond * EPS * scale)
+    dflt = _solve(grid, direction, True, a, b, c, d, method=0)                     # default: partition for x, lines for y / z
+    assert np.array_equal(dflt, got if direction == 0 else lines)
     grid.close()
 
 
@@ -86,7 +137,7 @@ def test_dominant_systems_equal_thomas_with_and_without_pivoting():
         ref = orc.thomas(np.ascontiguousarray(a[k, :, i]), np.ascontiguousarray(b[k, :, i]), np.ascontiguousarray(c[k, :, i]),
                          np.ascontiguousarray(d[k, :, i]))
         assert np.max(np.abs(x1[k, :, i] - ref)) <= 1e-12 * np.max(np.abs(ref))
-    with pytest.raises(tdx.TdxError) as e:
-        _solve(grid, 0, True, a, b, c, d)
-    assert e.value.status == tdx.ERR_UNSUPPORTED
+    xx = _solve(grid, 0, True, a, b, c, d)                       # x lines as well (round 1: TDX_ERR_UNSUPPORTED)
+    refx, _ = ogen.general_solve(a, b, c, d, 2)
+    assert np.max(np.abs(xx - refx)) <= 1e-12 * np.max(np.abs(refx))
     grid.close()

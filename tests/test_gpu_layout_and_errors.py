@@ -197,3 +197,33 @@ def test_plan_cache_is_bounded_and_rebuilds_evicted_plans(small):
     torch.cuda.synchronize()
     assert torch.equal(t2, first)
     assert free0 - torch.cuda.mem_get_info()[0] < 64 * 1024 * 1024   # 200 plans of this grid would be far below this anyway; no leak growth
+
+
+@pytest.mark.parametrize("L,uniform_table", [(3.8, True), (2.1, False)])
+@pytest.mark.parametrize("mode", [tdx.MODE_PPT, tdx.MODE_PDD])
+def test_uniform_table_switch_at_its_1e_13_boundary(L, uniform_table, mode):
+    """A product approximation that is not in the paper: when the partitions' ADI blocks agree row-wise to 1e-13 (uniform
+    spacing that is not a binary fraction: the faces L j / N differ by rounding), every block is replaced by one table
+    (k_blocks_identical; ||A^-1|| <= 1 for rows with |b| = |a| + |c| + 1, bounds the change by 1e-13).
+    Two grids on either side of the switch -- 48 uniform cells, P = 3, alpha = 1e-2 (alpha / h^2 = 1.6 and 5.2: coupled
+    partitions): L = 3.8, blocks differ by 0.47e-13 -> one table; L = 2.1, 2.1e-13 -> per-partition tables.  Both must
+    meet the 1e-12 gate against the oracle, which always uses the true coefficients."""
+    nx, ny, nz, P, alpha = 48, 6, 48, 3, 1e-2
+    faces = (inputs.faces_uniform(nx, L), inputs.faces_uniform(ny, 1.0), inputs.faces_uniform(nz, L))
+    a, b, c = orc.adi_coeffs(faces[0], orc.BC_DIRICHLET, alpha)
+    m = nx // P
+    diff = max(abs(b[p * m + jj] - b[jj]) + (abs(a[p * m + jj] - a[jj]) if jj else 0.0) + (abs(c[p * m + jj] - c[jj]) if jj < m - 1 else 0.0)
+               for p in range(1, P) for jj in range(m))
+    assert (0 < diff < 0.9e-13) if uniform_table else (1.1e-13 < diff < 5e-13)      # the inputs sit where the docstring says
+    grid = tdx.Grid(nx, ny, nz, *faces, bcs=BCS)
+    field = inputs.rhs_uniform((nz, ny, nx), 8)
+    for direction in (0, 2):                                     # x: the TMA kernel; z (periodic): the strided kernel
+        t = torch.from_numpy(field).cuda()
+        grid.adi_sweep(direction, mode, P, alpha, t)
+        torch.cuda.synchronize()
+        launch = tdx.last_launch()
+        uni = launch.split("<")[1].split(">")[0].split(",")[1 if direction == 0 else 3]
+        assert uni == ("1" if uniform_table else "0"), launch
+        ref = orc.adi_sweep(field.copy(), *faces, BCS, direction, orc.MODE_THOMAS if mode == tdx.MODE_PPT else orc.MODE_PDD, P, alpha)
+        assert relerr(t.cpu().numpy(), ref) < 1e-12, (direction, launch, relerr(t.cpu().numpy(), ref))
+    grid.close()
