@@ -566,7 +566,9 @@ tdx_status_t run_strided(const Plan& pl, double* data, long long W, long long li
     size_t smem = (size_t)2 * pl.P * LPC * V * 8;
     // the set's tables in shared memory (TDX_HELM_SMEM_TABLES=0: measurement knob, the round-1 path through L1)
     static const int env_ts = [] { const char* e = std::getenv("TDX_HELM_SMEM_TABLES"); return e ? std::atoi(e) : 1; }();
-    A.tables_smem = (set_per_outer && env_ts && V == 2 && !pl.cyc && pl.layout != ROWS_U && (pl.M == 12 || pl.M == 16 || pl.M == 24 || pl.M == 32)) ? 1 : 0;
+    // measured (cfg4 / cfg5 / the paper's grid): a gain only for the 24-row tile (cfg5 1.586 -> 1.567 ms: the 168-register
+    // instantiation stops spilling); 32 rows: 0.388 -> 0.407 ms, 12 rows: 1.76 -> 1.94 ms (the copy and its barrier cost more)
+    A.tables_smem = (set_per_outer && env_ts && V == 2 && !pl.cyc && pl.layout != ROWS_U && (pl.M == 24 || (env_ts > 1 && (pl.M == 12 || pl.M == 16 || pl.M == 32)))) ? 1 : 0;
     if (A.tables_smem) smem += ((size_t)pl.P * (pl.M * 3 + 1) + (size_t)pl.KB * pl.P) * 16;
     Tables T = tables_of(pl);
     if (V == 2) return pl.cyc ? launch_strided_M<2, true>(pl, A, T, grid, block, smem, st) : launch_strided_M<2, false>(pl, A, T, grid, block, smem, st);
@@ -1421,7 +1423,9 @@ tdx_status_t tdx_slab_correct(tdx_slab_t* s, double* field, const double* iface_
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     // one thread marches over all rows of its two lines when the plane alone fills the GPU; row slices otherwise
     const long long plane = s->inner * s->outer;
-    const int JT = (plane / 2 >= (long long)s->g->sms * 2048) ? s->n_loc : std::max(8, (s->n_loc + 7) / 8);
+    static const int env_jt = [] { const char* e = std::getenv("TDX_SLAB_JT"); return e ? std::atoi(e) : 0; }();   // measurement knob: rows per slice
+    int JT = (plane / 2 >= (long long)s->g->sms * 2048) ? s->n_loc : std::max(8, (s->n_loc + 7) / 8);
+    if (env_jt > 0) JT = std::min(env_jt, s->n_loc);
     dim3 block(128), grid((unsigned)((s->inner / 2 + 127) / 128), (s->n_loc + JT - 1) / JT, (unsigned)s->outer);
     if (s->outer > 65535) return fail(TDX_ERR_UNSUPPORTED, "outer extent > 65535");
     if (s->across == TDX_MODE_PPT) tdx::k_slab_correct<true><<<grid, block, 0, st>>>(field, iface_own, iface_nbr, s->coef, s->v, s->w, s->rank, s->R, s->n_loc, s->inner, s->outer, JT);

@@ -184,6 +184,10 @@ k_strided(StridedArgs A, Tables T, const __grid_constant__ UniTable<UNI ? MAXM :
     {
         const int2 bd = __ldg(&T.band[set * P + p]);
         const double2* g2 = reinterpret_cast<const double2*>(T.G) + (size_t)set * T.KB * P + p;
+        // two band terms per iteration let the loads of the next term overlap the FMAs (cfg5 y 1.48 -> 1.44 ms); not for the
+        // 255-register tile, where it costs registers the recurrences need (cfg4 Helmholtz 0.387 -> 0.399 ms)
+        constexpr int kBandUnroll = (MAXM * V >= 64) ? 1 : 2;
+#pragma unroll kBandUnroll
         for (int k = 0; k < bd.y; ++k) {
             const double2 ab = TS ? st_G[k * P + p] : __ldg(g2 + (size_t)k * P);   // {gL, gR}
             const double a = ab.x, b = ab.y;
@@ -220,10 +224,24 @@ k_strided(StridedArgs A, Tables T, const __grid_constant__ UniTable<UNI ? MAXM :
             x[jj][v] = r;
         }
         if (valid && (full || jj < m)) VecIO<V>::st(base + jj * rstride, x[jj]);
-        if (A.iface != nullptr && valid) {                  // Alg.1 step 4: the slab's interface rows, packed for the exchange
+        if (MAXM * V > 8 && A.iface != nullptr && valid) {  // Alg.1 step 4 (slab sweeps): the interface rows, packed for the exchange
             double* ip = A.iface + ((long long)o * A.W + i) * V;
             if (p == 0 && jj == 0) VecIO<V>::st(ip, x[0]);
             if (p == P - 1 && jj == m - 1) VecIO<V>::st(ip + A.iface_plane, x[jj]);
+        }
+    }
+    if (MAXM * V <= 8 && A.iface != nullptr && valid) {     // Alg.1 step 4 (slab sweeps): the interface rows, packed for the exchange.
+        double* ip = A.iface + ((long long)o * A.W + i) * V;   // Tiny tiles: a chain of selects (the in-loop form below becomes a
+        if (p == 0) VecIO<V>::st(ip, x[0]);                 // run-time index there, which puts the tile into local memory)
+        if (p == P - 1) {
+            double xlast[V];
+#pragma unroll
+            for (int v = 0; v < V; ++v) xlast[v] = x[0][v];
+#pragma unroll
+            for (int jj = 1; jj < MAXM; ++jj)
+#pragma unroll
+                for (int v = 0; v < V; ++v) xlast[v] = (jj < m) ? x[jj][v] : xlast[v];
+            VecIO<V>::st(ip + A.iface_plane, xlast);
         }
     }
     if (xt + (int)gridDim.x < tiles_x) __syncthreads();     // rs is reused by the next tile
