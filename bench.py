@@ -52,7 +52,7 @@ def ncu_traffic(workload, launch):
 
 
 # tuned partitions per line (x, y, z, helmholtz-y) per config, mode PPT (exact for every P)
-TUNED_P = {1: (4, 4, 4, 4), 2: (16, 8, 8, 8), 3: (32, 8, 8, 8), 4: (64, 16, 8, 16), 5: (256, 24, 16, 12), 6: (384, 8, 24, 8)}
+TUNED_P = {1: (4, 4, 4, 4), 2: (16, 8, 8, 8), 3: (32, 8, 8, 8), 4: (128, 16, 8, 16), 5: (256, 24, 16, 12), 6: (384, 8, 24, 8)}
 
 
 def pdd_partitions(grid, cfg, direction, P_ppt):
@@ -572,22 +572,28 @@ def run_tdx(args, rank, world, local_rank):
                     else:
                         ga, gc = (torch.rand(field0.shape, dtype=torch.float64, device=field0.device, generator=gen) * 2 - 1 for _ in range(2))
                         gb = (torch.rand(field0.shape, dtype=torch.float64, device=field0.device, generator=gen) * 2 - 1) * 0.3
-                    for _ in range(2):
-                        gd.copy_(field0); grid.general_solve(1, True, ga, gb, gc, gd, gwork, stream)
-                    barrier()
-                    tot = 0.0
-                    for _ in range(args.steps):
-                        gd.copy_(field0)
-                        s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-                        s0.record(); grid.general_solve(1, True, ga, gb, gc, gd, gwork, stream); s1.record()
-                        torch.cuda.synchronize()
-                        tot += s0.elapsed_time(s1)
-                    msg = max_over_ranks(tot / args.steps, dist, "cuda")
-                    nfb = grid.general_fallback_count()
-                    gout[wname] = {"ms": msg, "gpts_per_s": cfg.npts / (msg * 1e-3) / 1e9, "gb_per_s": 40 * cfg.npts / (msg * 1e-3) / 1e9,
-                                   "frac_of_measured_peak": 40 * cfg.npts / (msg * 1e-3) / 1e9 / peak, "finite": bool(torch.isfinite(gd).all()),
-                                   "lines_solved_by_the_per_line_path": nfb, "share_of_lines": nfb / (cfg.nx * cfg.nz), "launch": tdx.last_launch()}
-                gout["what"] = "tdx_general_solve along y, per-line a, b, c, diagonal pivoting inside 8-row partitions; 40 B per value, one pass"
+                    res = {}
+                    # both methods (include/tdx.h): "lines" = one thread per line, two passes, the default for y / z lines;
+                    # "partition" = the one-pass partition kernel (forced here; the default for x lines)
+                    for meth, flag, nbytes in (("lines", tdx.GENERAL_FORCE_LINES, 82), ("partition", tdx.GENERAL_FORCE_PARTITION, 40)):
+                        for _ in range(2):
+                            gd.copy_(field0); grid.general_solve(1, 1 | flag, ga, gb, gc, gd, gwork, stream)
+                        barrier()
+                        tot = 0.0
+                        for _ in range(args.steps):
+                            gd.copy_(field0)
+                            s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                            s0.record(); grid.general_solve(1, 1 | flag, ga, gb, gc, gd, gwork, stream); s1.record()
+                            torch.cuda.synchronize()
+                            tot += s0.elapsed_time(s1)
+                        msg = max_over_ranks(tot / args.steps, dist, "cuda")
+                        nfb = grid.general_fallback_count() if meth == "partition" else 0
+                        res[meth] = {"ms": msg, "gpts_per_s": cfg.npts / (msg * 1e-3) / 1e9, "algorithmic_bytes_per_value": nbytes,
+                                     "gb_per_s": nbytes * cfg.npts / (msg * 1e-3) / 1e9,
+                                     "frac_of_measured_peak": nbytes * cfg.npts / (msg * 1e-3) / 1e9 / peak, "finite": bool(torch.isfinite(gd).all()),
+                                     "lines_re_solved_by_the_per_line_kernel": nfb, "share_of_lines": nfb / (cfg.nx * cfg.nz), "launch": tdx.last_launch()}
+                    gout[wname] = res
+                gout["what"] = "tdx_general_solve along y, per-line a, b, c, diagonal pivoting: per-line kernel (two passes, 82 B per value; default for y / z) and partition kernel (8-row partitions, one pass, 40 B per value; default for x)"
                 out["general_solve_pivoting"] = gout
                 del ga, gb, gc, gd, gwork
         except Exception as exc:

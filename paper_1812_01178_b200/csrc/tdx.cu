@@ -1481,6 +1481,7 @@ static tdx_status_t general_solve_impl(tdx_grid_t* g, tdx_dir_t dir, int pivotin
         if (periodic) { if (pivoting) tdx::k_general_lines<true, false, true><<<grid, block, 0, st>>>(G, bm, flag, qv, dv); else tdx::k_general_lines<false, false, true><<<grid, block, 0, st>>>(G, bm, flag, qv, dv); }
         else { if (pivoting) tdx::k_general_lines<true, false, false><<<grid, block, 0, st>>>(G, bm, flag, qv, dv); else tdx::k_general_lines<false, false, false><<<grid, block, 0, st>>>(G, bm, flag, qv, dv); }
         LAUNCH_CHECK("k_general_lines");
+        note_launch("k_general_lines<%d,%d,%d>", pivoting ? 1 : 0, 0, periodic ? 1 : 0, 0, 0, 0, grid, block);
         return TDX_OK;
     }
     const unsigned nlines = (unsigned)(G.W * O);

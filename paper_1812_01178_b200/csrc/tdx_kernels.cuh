@@ -184,11 +184,7 @@ k_strided(StridedArgs A, Tables T, const __grid_constant__ UniTable<UNI ? MAXM :
     {
         const int2 bd = __ldg(&T.band[set * P + p]);
         const double2* g2 = reinterpret_cast<const double2*>(T.G) + (size_t)set * T.KB * P + p;
-        // two band terms per iteration let the loads of the next term overlap the FMAs (cfg5 y 1.48 -> 1.44 ms); not for the
-        // 255-register tile, where it costs registers the recurrences need (cfg4 Helmholtz 0.387 -> 0.399 ms)
-        constexpr int kBandUnroll = (MAXM * V >= 64) ? 1 : 2;
-#pragma unroll kBandUnroll
-        for (int k = 0; k < bd.y; ++k) {
+        auto term = [&](int k) {
             const double2 ab = TS ? st_G[k * P + p] : __ldg(g2 + (size_t)k * P);   // {gL, gR}
             const double a = ab.x, b = ab.y;
             int idx = bd.x + k;                             // band may wrap around (periodic line closed inside Z)
@@ -199,6 +195,15 @@ k_strided(StridedArgs A, Tables T, const __grid_constant__ UniTable<UNI ? MAXM :
                 yL[v] = fma(a, rv, yL[v]);
                 yR[v] = fma(b, rv, yR[v]);
             }
+        };
+        // two band terms per iteration let the loads of the next term overlap the FMAs (cfg5 y 1.48 -> 1.44 ms); the
+        // 255-register tile keeps the compiler's own choice, 4 (forcing 2 there: cfg4 Helmholtz 0.388 -> 0.399 ms, 1: 0.422, 8: 0.389
+        // but cfg4 y 0.332 -> 0.345)
+        if (MAXM * V >= 64) {
+            for (int k = 0; k < bd.y; ++k) term(k);
+        } else {
+#pragma unroll 2
+            for (int k = 0; k < bd.y; ++k) term(k);
         }
         if (CYC) {
             const int ns = __ldg(&T.Sn[set]);
