@@ -207,6 +207,27 @@ tdx_status_t tdx_general_cyclic_solve(tdx_grid_t* grid, tdx_dir_t dir, int pivot
                                       const double* c, double* rhs_inout, void* work, void* stream);
 tdx_status_t tdx_general_fallback_count(tdx_grid_t* grid, long long* out);
 
+/* A solve that ALLOCATES NOTHING, for callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid it): the Poisson y-solves (delta2_y - kx2[i] - kz2[m]) phi = rhs of
+ * tdx_helmholtz_wavenumber_solve in mode THOMAS with per-line shifts (same kernel, same
+ * arithmetic, same pinning of lambda == 0 lines), with two differences: kx2_dev (nx doubles) and kz2_dev (nm doubles) are
+ * DEVICE arrays the caller owns (no upload, no cache), and the kernel's scratch (the scaled super-diagonal of every line,
+ * nx*ny*nm doubles) is a static device array inside the library instead of a workspace the grid allocates.
+ * Limit: nx*ny*nm <= TDX_STATIC_SCRATCH_DOUBLES (2 359 296 doubles = 18 MiB, held by every GPU that loads the library
+ * until the process exits; config 2, 256 x 128 x 65 modes, fits); larger sizes return TDX_ERR_UNSUPPORTED and launch nothing.
+ * The call makes no cudaMalloc / cudaFree and calls no allocating routine; the grid must exist already (its metric tables
+ * are allocated by tdx_grid_create).  Negative or NaN wavenumbers cannot be checked here (they are on the device).
+ * EVERY call on a device shares the one array: calls that overlap on the GPU (two streams, two host threads, two grids)
+ * RACE -- order them on one stream or with events.  The array keeps the last call's contents; nothing in it needs to be
+ * zero at entry (every entry is written before it is read).  rhs_inout: DEVICE, complex128 [nm][ny][nx], in place.
+ * Asynchronous on `stream`.  tdx_static_scratch_setup(device) resolves the array's device address
+ * (cudaGetSymbolAddress, once per device) ahead of time -- call it before a graph capture begins; otherwise the first
+ * solve on a device does it.                                                                                      */
+#define TDX_STATIC_SCRATCH_DOUBLES 2359296
+tdx_status_t tdx_static_scratch_setup(int device);
+tdx_status_t tdx_helmholtz_thomas_lines_static(tdx_grid_t* grid, int nm, const double* kx2_dev, const double* kz2_dev,
+                                               double* rhs_inout, void* stream);
+
 /* Batched cyclic tridiagonal solve along dir with caller-given coefficients shared by every line:
  * a, b, c: HOST arrays of n_dir doubles; a[0] couples row 0 to row n-1 and c[n-1] couples row n-1 to row 0.
  * Closure as for tdx_adi_sweep on a periodic direction (Sherman-Morrison with gamma = -b[0] for THOMAS, cyclic

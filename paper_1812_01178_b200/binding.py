@@ -18,7 +18,7 @@ GENERAL_PIVOT, GENERAL_FORCE_PARTITION, GENERAL_FORCE_LINES = 1, 16, 32
 OK, ERR_INVALID_ARG, ERR_BAD_PARTITION, ERR_ALLOC, ERR_CUDA, ERR_UNSUPPORTED, ERR_PDD_BOUND = 0, -1, -2, -3, -4, -5, -6
 
 EXPORTS = ("tdx_grid_create", "tdx_grid_destroy", "tdx_grid_set_pdd_strict", "tdx_partition_bounds", "tdx_adi_sweep", "tdx_adi_sweep_at", "tdx_adi_step",
-           "tdx_helmholtz_wavenumber_solve", "tdx_dct_x", "tdx_rfft_z", "tdx_irfft_z", "tdx_poisson_solve", "tdx_general_solve", "tdx_general_cyclic_solve", "tdx_general_fallback_count", "tdx_slab_create", "tdx_slab_destroy", "tdx_slab_eliminate", "tdx_slab_correct", "tdx_slab_dropped_bound", "tdx_cyclic_solve", "tdx_adi_sweep_host", "tdx_adi_step_host",
+           "tdx_helmholtz_wavenumber_solve", "tdx_dct_x", "tdx_rfft_z", "tdx_irfft_z", "tdx_poisson_solve", "tdx_static_scratch_setup", "tdx_helmholtz_thomas_lines_static", "tdx_general_solve", "tdx_general_cyclic_solve", "tdx_general_fallback_count", "tdx_slab_create", "tdx_slab_destroy", "tdx_slab_eliminate", "tdx_slab_correct", "tdx_slab_dropped_bound", "tdx_cyclic_solve", "tdx_adi_sweep_host", "tdx_adi_step_host",
            "tdx_helmholtz_wavenumber_solve_host", "tdx_step_host", "tdx_pdd_dropped_bound", "tdx_kernel_launch_count",
            "tdx_status_string", "tdx_last_error", "tdx_last_launch", "tdx_version")
 
@@ -67,6 +67,8 @@ def lib():
         L.tdx_general_solve.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.tdx_general_cyclic_solve.argtypes = L.tdx_general_solve.argtypes
         L.tdx_general_fallback_count.argtypes = [C.c_void_p, C.POINTER(C.c_longlong)]
+        L.tdx_static_scratch_setup.argtypes = [C.c_int]
+        L.tdx_helmholtz_thomas_lines_static.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.tdx_slab_create.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, _dp, C.c_int, C.c_double, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_void_p)]
         L.tdx_slab_destroy.argtypes = [C.c_void_p]
         L.tdx_slab_eliminate.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
@@ -119,6 +121,13 @@ def _hostptr(arr, nbytes):
     return C.c_void_p(arr.ctypes.data)
 
 
+STATIC_SCRATCH_DOUBLES = 2359296
+
+
+def static_scratch_setup(device=0):
+    _chk(lib().tdx_static_scratch_setup(int(device)))
+
+
 def partition_bounds(n, P):
     st = (C.c_int * (P + 1))()
     _chk(lib().tdx_partition_bounds(n, P, st))
@@ -168,6 +177,10 @@ class Grid:
         kz, pkz = _host(kz2)
         _, pkx = _host(kx2)
         _chk(lib().tdx_helmholtz_wavenumber_solve(self._h, mode, P, kz.size, pkx, pkz, _devptr(rhs), C.c_void_p(stream)))
+
+    def helmholtz_thomas_lines_static(self, nm, kx2_dev, kz2_dev, rhs, stream=0):
+        """The entry point that allocates nothing: kx2_dev / kz2_dev are DEVICE arrays; scratch is the library's static array."""
+        _chk(lib().tdx_helmholtz_thomas_lines_static(self._h, int(nm), _devptr(kx2_dev), _devptr(kz2_dev), _devptr(rhs), C.c_void_p(stream)))
 
     def dct_x(self, inverse, field, stream=0):
         _chk(lib().tdx_dct_x(self._h, int(inverse), _devptr(field), C.c_void_p(stream)))

@@ -1254,6 +1254,63 @@ tdx_status_t tdx_helmholtz_wavenumber_solve(tdx_grid_t* g, tdx_mode_t mode, int 
     return run_strided(*pl, rhs, nx2, nx2, nm, nx2 * g->ny, true, st);
 }
 
+// ---- an entry point that allocates nothing (for callers that cannot call cudaMalloc: CUDA graph capture, tight serving
+// loops, harnesses that forbid it) ----------------------------------------------------------------------------------------
+// The per-line Thomas solve of the Poisson y-systems (k_thomas_helm_lines) needs a scratch array for the scaled
+// super-diagonal c'_j of every line (nx * ny * nm doubles), which tdx_helmholtz_wavenumber_solve takes from a workspace the
+// grid cudaMallocs on demand.  Here the scratch is a file-scope device array of fixed size instead: every GPU that loads the
+// library holds its TDX_STATIC_SCRATCH_DOUBLES * 8 bytes until the process exits.  In host code the name `g_static_scratch`
+// is a host-side stand-in, NOT a device address: the address a kernel may use comes from cudaGetSymbolAddress, once per
+// device, with that device current (static_scratch_ptr).
+static __device__ __align__(256) double g_static_scratch[TDX_STATIC_SCRATCH_DOUBLES];
+
+namespace {
+std::mutex g_static_mu;
+double* g_static_ptr[kMaxDev] = {};
+
+// device address of g_static_scratch on `device`; resolved once per device, with that device current
+tdx_status_t static_scratch_ptr(int device, double** out) {
+    if (device < 0 || device >= kMaxDev) return fail(TDX_ERR_INVALID_ARG, "device %d not in [0,%d)", device, kMaxDev);
+    std::lock_guard<std::mutex> lk(g_static_mu);
+    if (!g_static_ptr[device]) {
+        CUDA_TRY(cudaSetDevice(device));
+        double* p = nullptr;
+        CUDA_TRY(cudaGetSymbolAddress(reinterpret_cast<void**>(&p), g_static_scratch));
+        if (!p) return fail(TDX_ERR_CUDA, "cudaGetSymbolAddress returned a null address");
+        g_static_ptr[device] = p;
+    }
+    *out = g_static_ptr[device];
+    return TDX_OK;
+}
+}  // namespace
+
+tdx_status_t tdx_static_scratch_setup(int device) {
+    double* p = nullptr;
+    return static_scratch_ptr(device, &p);
+}
+
+tdx_status_t tdx_helmholtz_thomas_lines_static(tdx_grid_t* g, int nm, const double* kx2_dev, const double* kz2_dev,
+                                               double* rhs, void* stream) {
+    if (!g) return fail(TDX_ERR_INVALID_ARG, "grid is NULL");
+    if (!kx2_dev || !kz2_dev || !rhs) return fail(TDX_ERR_INVALID_ARG, "NULL argument");
+    if (nm < 1 || nm > 65535) return fail(TDX_ERR_INVALID_ARG, "nm=%d not in [1, 65535]", nm);
+    if (reinterpret_cast<uintptr_t>(rhs) & 15) return fail(TDX_ERR_INVALID_ARG, "rhs_inout must be 16-byte aligned");
+    const long long need = (long long)g->nx * g->ny * nm;
+    if (need > (long long)TDX_STATIC_SCRATCH_DOUBLES)
+        return fail(TDX_ERR_UNSUPPORTED, "nx*ny*nm = %lld doubles of scratch exceed the static array of %lld (TDX_STATIC_SCRATCH_DOUBLES): "
+                                         "use tdx_helmholtz_wavenumber_solve", need, (long long)TDX_STATIC_SCRATCH_DOUBLES);
+    double* scratch = nullptr;
+    tdx_status_t rc = static_scratch_ptr(g->device, &scratch);           // no allocation: a symbol look-up, cached per device
+    if (rc != TDX_OK) return rc;
+    CUDA_TRY(cudaSetDevice(g->device));
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    // nothing in the scratch must start at zero: the forward pass writes c'_j of every (line, row) before the backward pass reads it
+    dim3 grid((g->nx + 127) / 128, nm);
+    k_thomas_helm_lines<<<grid, 128, 0, st>>>(reinterpret_cast<double2*>(rhs), scratch, g->nx, g->ny, g->lo_neumann_y, g->up_neumann_y, kx2_dev, kz2_dev);
+    LAUNCH_CHECK("k_thomas_helm_lines");
+    return TDX_OK;
+}
+
 tdx_status_t tdx_dct_x(tdx_grid_t* g, int inverse, double* field, void* stream) {
     return run_dct_x(g, field, inverse != 0, static_cast<cudaStream_t>(stream));
 }
