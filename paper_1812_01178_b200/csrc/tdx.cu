@@ -89,9 +89,14 @@ struct Plan {
     double *rows = nullptr, *G = nullptr, *Sval = nullptr, *cyc_tab = nullptr;
     int2* band = nullptr;
     int *Sidx = nullptr, *Sn = nullptr;
+    double* pcr = nullptr;  // PPT by plan-time cyclic reduction (k_pcr_tables); used by the strided kernels when use_pcr
+    int* pcr_n = nullptr;
+    int pcr_cap = 0;
+    bool use_pcr = false;
+    double band_mean = 0.0; // mean number of Z^-1 band terms a partition applies per line (PPT)
     void release() {
-        cudaFree(rows); cudaFree(G); cudaFree(Sval); cudaFree(cyc_tab); cudaFree(band); cudaFree(Sidx); cudaFree(Sn);
-        rows = G = Sval = cyc_tab = nullptr; band = nullptr; Sidx = Sn = nullptr;
+        cudaFree(rows); cudaFree(G); cudaFree(Sval); cudaFree(cyc_tab); cudaFree(band); cudaFree(Sidx); cudaFree(Sn); cudaFree(pcr); cudaFree(pcr_n);
+        rows = G = Sval = cyc_tab = pcr = nullptr; band = nullptr; Sidx = Sn = pcr_n = nullptr;
     }
 };
 
@@ -303,6 +308,32 @@ tdx_status_t build_plan(tdx_grid* g, Plan& pl, const double* lambda_host, const 
         k_pack_ppt<<<(ntp + 63) / 64, 64, 0, st>>>(nsets, P, pl.KB, Zi.as<double>(), pl.G, pl.band);
         LAUNCH_CHECK("k_pack_ppt");
         CUDA_TRY(cudaStreamSynchronize(st));
+        // Strided lines: the same reduced system also as plan-time cyclic-reduction tables (tdx_plan.cuh).  They replace
+        // the band where it is long -- mean band length above kPcrBandMin terms per partition (measured: DESIGN.md section 4c);
+        // TDX_PPT_PCR = 0 / 1 (measurement knob) forces the band / the reduction.
+        if ((pl.dir != 0 || pl.kind == KIND_HELM) && P >= 3 && P <= 256 && !pl.cyc) {
+            std::vector<int2> hb((size_t)ntp);
+            CUDA_TRY(cudaMemcpy(hb.data(), pl.band, hb.size() * sizeof(int2), cudaMemcpyDeviceToHost));
+            double sum = 0.0;
+            for (const int2& b2 : hb) sum += b2.y;
+            pl.band_mean = sum / (double)ntp;
+            static const int env_pcr = [] { const char* e = std::getenv("TDX_PPT_PCR"); return e ? std::atoi(e) : -1; }();
+            const double kPcrBandMin = 21.0;
+            pl.use_pcr = env_pcr < 0 ? pl.band_mean > kPcrBandMin : env_pcr != 0;
+            static const bool env_dbg = std::getenv("TDX_DEBUG_PLAN") != nullptr;
+            if (env_dbg) fprintf(stderr, "[tdx plan] kind=%d dir=%d P=%d M=%d sets=%d: mean Z^-1 band %.1f of %d terms -> %s\n", pl.kind, pl.dir, P, pl.M, nsets,
+                                 pl.band_mean, 2 * P, pl.use_pcr ? "cyclic reduction" : "band");
+            if (pl.use_pcr) {
+                pl.pcr_cap = 1;
+                for (int d = 1; d < P - 1; d <<= 1) ++pl.pcr_cap;
+                CUDA_TRY(cudaMalloc(&pl.pcr, (size_t)nsets * pl.pcr_cap * P * 6 * 8));
+                CUDA_TRY(cudaMalloc(&pl.pcr_n, (size_t)nsets * 4));
+                CUDA_TRY(cudaMemsetAsync(pl.pcr, 0, (size_t)nsets * pl.pcr_cap * P * 6 * 8, st));
+                k_pcr_tables<<<nsets, 256, 0, st>>>(P, pl.pcr_cap, ends.as<double>(), pl.pcr, pl.pcr_n);
+                LAUNCH_CHECK("k_pcr_tables");
+                CUDA_TRY(cudaStreamSynchronize(st));
+            }
+        }
     }
     if (pl.cyc) {
         pl.Scap = 2 + 2 * pl.KB;
@@ -406,6 +437,7 @@ tdx_status_t get_plan(tdx_grid* g, int kind, int dir, int mode, int P, double al
 Tables tables_of(const Plan& pl) {
     Tables T;
     T.rows = pl.rows; T.G = pl.G; T.band = pl.band; T.Sidx = pl.Sidx; T.Sval = pl.Sval; T.Sn = pl.Sn;
+    T.pcr = pl.pcr; T.pcr_n = pl.pcr_n; T.pcr_cap = pl.pcr_cap;
     T.P = pl.P; T.n = pl.n; T.q = pl.n / pl.Pu; T.r = pl.n % pl.Pu; T.S = pl.S; T.KB = pl.KB; T.Scap = pl.Scap;
     return T;
 }
@@ -415,17 +447,17 @@ Tables tables_of(const Plan& pl) {
 // ---- launch selection ---------------------------------------------------------------------------------------
 namespace {
 
-template <int M, int V, bool CYC, bool UNI = false, int REGS = strided_regs(M, V), bool TS = false>
+template <int M, int V, bool CYC, bool UNI = false, int REGS = strided_regs(M, V), bool TS = false, bool PCR = false>
 tdx_status_t launch_strided_inst(const Plan& pl, StridedArgs& A, const Tables& T, dim3 grid, dim3 block, size_t smem, cudaStream_t st) {
     static DevOnce attr;
     if (smem > 48 * 1024 && attr.need(pl.dev)) {
-        CUDA_TRY(cudaFuncSetAttribute(k_strided<M, V, CYC, UNI, REGS, TS>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+        CUDA_TRY(cudaFuncSetAttribute(k_strided<M, V, CYC, UNI, REGS, TS, PCR>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
         attr.set(pl.dev);
     }
     const long long key = ((long long)(block.x * block.y) << 32) | ((long long)smem << 4) | (V << 1) | (REGS == strided_regs(M, V) ? 0 : 1);
     if (pl.pf < 0 || pl.pf_key != key) {                           // prefetch one wave of resident CTAs ahead
         int occ = 1;
-        CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_strided<M, V, CYC, UNI, REGS, TS>, (int)(block.x * block.y), smem));
+        CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_strided<M, V, CYC, UNI, REGS, TS, PCR>, (int)(block.x * block.y), smem));
         pl.occ = occ < 1 ? 1 : occ;
         pl.pf = pl.sms * pl.occ * prefetch_waves();
         pl.pf_key = key;
@@ -441,15 +473,27 @@ tdx_status_t launch_strided_inst(const Plan& pl, StridedArgs& A, const Tables& T
         }
         std::memcpy(U.v, pl.uni_host, sizeof(U.v));
     } else std::memset(U.v, 0, sizeof(U.v));
-    k_strided<M, V, CYC, UNI, REGS, TS><<<grid, block, smem, st>>>(A, T, U);
+    k_strided<M, V, CYC, UNI, REGS, TS, PCR><<<grid, block, smem, st>>>(A, T, U);
     LAUNCH_CHECK("k_strided");
-    note_launch("k_strided<%d,%d,%d,%d,%d,%d>", M, V, CYC, UNI, REGS, TS, grid, block);
+    note_launch(PCR ? "k_strided<%d,%d,%d,%d,%d,%d,1>" : "k_strided<%d,%d,%d,%d,%d,%d>", M, V, CYC, UNI, REGS, TS, grid, block);
     return TDX_OK;
 }
 
 template <int V, bool CYC>
 tdx_status_t launch_strided_M(const Plan& pl, StridedArgs& A, const Tables& T, dim3 grid, dim3 block, size_t smem, cudaStream_t st) {
     const int M = pl.M;
+    if (A.pcr) {                                                   // PPT by plan-time cyclic reduction (k_strided "PCR"): two lines per thread
+        if (V == 2 && !CYC)
+            switch (M) {
+                case 4: return launch_strided_inst<4, 2, false, false, strided_regs(4, 2), false, true>(pl, A, T, grid, block, smem, st);
+                case 8: return launch_strided_inst<8, 2, false, false, strided_regs(8, 2), false, true>(pl, A, T, grid, block, smem, st);
+                case 12: return launch_strided_inst<12, 2, false, false, strided_regs(12, 2), false, true>(pl, A, T, grid, block, smem, st);
+                case 16: return launch_strided_inst<16, 2, false, false, strided_regs(16, 2), false, true>(pl, A, T, grid, block, smem, st);
+                case 24: return launch_strided_inst<24, 2, false, false, strided_regs(24, 2), false, true>(pl, A, T, grid, block, smem, st);
+                case 32: return launch_strided_inst<32, 2, false, false, strided_regs(32, 2), false, true>(pl, A, T, grid, block, smem, st);
+            }
+        return fail(TDX_ERR_UNSUPPORTED, "no cyclic-reduction strided kernel for M=%d V=%d", M, V);
+    }
     if (A.tables_smem) {                                           // Helmholtz y-solves: the set's tables in shared memory (k_strided "TS")
         if (V == 2 && !CYC)
             switch (M) {
@@ -508,7 +552,7 @@ tdx_status_t run_strided(const Plan& pl, double* data, long long W, long long li
     if (O > 65535) return fail(TDX_ERR_UNSUPPORTED, "outer extent %lld > 65535", O);
     StridedArgs A;
     A.data = data; A.set_per_outer = set_per_outer ? 1 : 0; A.set0 = set0; A.pf = 0;
-    A.iface = iface; A.iface_plane = W * O; A.tables_smem = 0;
+    A.iface = iface; A.iface_plane = W * O; A.tables_smem = 0; A.pcr = 0;
     if (pl.thomas) {
         const int V = even ? 2 : 1;
         A.W = W / V; A.line_stride = line_stride / V; A.outer_stride = outer_stride / V;
@@ -569,6 +613,8 @@ tdx_status_t run_strided(const Plan& pl, double* data, long long W, long long li
     // measured (cfg4 / cfg5 / the paper's grid): a gain only for the 24-row tile (cfg5 1.586 -> 1.567 ms: the 168-register
     // instantiation stops spilling); 32 rows: 0.388 -> 0.407 ms, 12 rows: 1.76 -> 1.94 ms (the copy and its barrier cost more)
     A.tables_smem = (set_per_outer && env_ts && V == 2 && !pl.cyc && pl.layout != ROWS_U && (pl.M == 24 || (env_ts > 1 && (pl.M == 12 || pl.M == 16 || pl.M == 32)))) ? 1 : 0;
+    A.pcr = (pl.use_pcr && pl.pcr && V == 2 && pl.layout != ROWS_U && (pl.M == 4 || pl.M == 8 || pl.M == 12 || pl.M == 16 || pl.M == 24 || pl.M == 32)) ? 1 : 0;
+    if (A.pcr) { A.tables_smem = 0; smem += (size_t)4 * pl.P * LPC * V * 8; }
     if (A.tables_smem) smem += ((size_t)pl.P * (pl.M * 3 + 1) + (size_t)pl.KB * pl.P) * 16;
     Tables T = tables_of(pl);
     if (V == 2) return pl.cyc ? launch_strided_M<2, true>(pl, A, T, grid, block, smem, st) : launch_strided_M<2, false>(pl, A, T, grid, block, smem, st);
@@ -1562,7 +1608,7 @@ static tdx_status_t general_solve_impl(tdx_grid_t* g, tdx_dir_t dir, int pivotin
     while (L * 2 * P <= 512 && L * 2 <= (unit ? std::max(1, 128 / P) : cap)) L *= 2;
     if ((long long)L > G.W) { L = 1; while ((long long)L * 2 <= G.W && L * 2 * P <= 512) L *= 2; }
     dim3 block = unit ? dim3(P, L) : dim3(L, P), grid((unsigned)((G.W + L - 1) / L), (unsigned)O);
-    const size_t smem = (size_t)21 * P * L * 8 + (size_t)L * 8 + 16;
+    const size_t smem = (size_t)19 * P * L * 8 + (size_t)L * 8 + 16;
 #define TDX_GENERAL_PART(PV, UN)                                                                                              \
     do { static DevOnce attr;                                                                                                 \
          if (attr.need(g->device)) { CUDA_TRY(cudaFuncSetAttribute(tdx::k_general_part<8, PV, UN>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024)); attr.set(g->device); } \

@@ -79,17 +79,24 @@ k_general_part(GeneralArgs G) {
     // Alg.1 step 2: the couplings at the partition's ends are cut; they are the right-hand sides of the spikes (Eq.(6)).
     double A_[M], B_[M], C_[M], D_[M], F_[M];
     double clast = 0.0;
+    {
+        const double *pa = G.a + e0, *pb = G.b + e0, *pcc = G.c + e0, *pd = G.d + e0;
+        const long long rs = G.row_stride;
+        double av[M], cv[M];
 #pragma unroll
-    for (int jj = 0; jj < M; ++jj) {
-        const bool real = jj < m;
-        const long long e = e0 + (long long)jj * G.row_stride;
-        const double av = (valid && real) ? __ldg(G.a + e) : 0.0, cv = (valid && real) ? __ldg(G.c + e) : 0.0;
-        A_[jj] = real ? (jj == 0 ? 0.0 : av) : -1.0;
-        B_[jj] = (valid && real) ? __ldg(G.b + e) : 1.0;
-        C_[jj] = (jj < m - 1) ? cv : 0.0;
-        D_[jj] = (valid && real) ? __ldg(G.d + e) : 0.0;
-        F_[jj] = (jj == 0 && p > 0) ? av : 0.0;
-        if (jj == m - 1 && p < P - 1) clast = cv;
+        for (int jj = 0; jj < M; ++jj) {                                // all loads first: 4 M independent requests in flight
+            const bool ld = valid && jj < m;
+            av[jj] = ld ? __ldg(pa) : 0.0; B_[jj] = ld ? __ldg(pb) : 1.0; cv[jj] = ld ? __ldg(pcc) : 0.0; D_[jj] = ld ? __ldg(pd) : 0.0;
+            pa += rs; pb += rs; pcc += rs; pd += rs;
+        }
+#pragma unroll
+        for (int jj = 0; jj < M; ++jj) {
+            const bool real = jj < m;
+            A_[jj] = real ? (jj == 0 ? 0.0 : av[jj]) : -1.0;
+            C_[jj] = (jj < m - 1) ? cv[jj] : 0.0;
+            F_[jj] = (jj == 0 && p > 0) ? av[jj] : 0.0;
+            if (jj == m - 1 && p < P - 1) clast = cv[jj];
+        }
     }
 
     // forward elimination with 1x1 / 2x2 diagonal pivots; fl: 2 bits per row (0: 1x1, 1: first row of a 2x2 pivot, 2: second).
@@ -172,10 +179,10 @@ k_general_part(GeneralArgs G) {
     const double xl = D_[M - 1], vl = F_[M - 1], wl = A_[M - 1];        // padding rows carried the last real row here
     const double xf = D_[0], vf = F_[0], wf = A_[0];
 
-    // shared memory, all indexed [me]: xf, xl, vf, vl, wf, wl, t (x_first after the solve), 2 PCR buffers x 7, flags
+    // shared memory, all indexed [me]: xf, xl, vf, vl, wf, wl, t (x_first after the solve), 2 PCR buffers x 6, flags
     double* s_xf = gs;            double* s_xl = s_xf + S;  double* s_vf = s_xl + S;  double* s_vl = s_vf + S;
     double* s_wf = s_vl + S;      double* s_wl = s_wf + S;  double* s_t = s_wl + S;   double* pc = s_t + S;
-    int* s_bad = reinterpret_cast<int*>(pc + (size_t)14 * S);           // per line of the CTA: [lt] a row failed the test, [L + lt] a block was not tame
+    int* s_bad = reinterpret_cast<int*>(pc + 12 * S);           // per line of the CTA: [lt] a row failed the test, [L + lt] a block was not tame
     if (p == 0) { s_bad[lt] = 0; s_bad[L + lt] = 0; }
     s_xf[me] = xf; s_xl[me] = xl; s_vf[me] = vf; s_vl[me] = vl; s_wf[me] = wf; s_wl[me] = wl;
     __syncthreads();
@@ -189,30 +196,36 @@ k_general_part(GeneralArgs G) {
         up_ = (p <= K - 1) ? s_wf[me] : 0.0;
         r0 = s_xl[pa]; r1 = s_xf[me];
     }
+    // Per step a block hands its neighbours three products each: to the block d to its right {u e01, q0, l idet}, to the block
+    // d to its left {l e10, q1, u idet} (e01 = beta idet, e10 = gamma idet): 6 stores and 6 loads per step, 32-bit indices.
     int buf = 0;
     double q0 = 0.0, q1 = 0.0;
+    const int S6 = 6 * S;
     for (int dd = 1;; dd <<= 1) {
         const double idet = 1.0 / (1.0 - beta * gamma);
         q0 = (r0 - beta * r1) * idet;
         q1 = (r1 - gamma * r0) * idet;
         if (dd >= K) break;                                             // uniform over the CTA
-        double* Bf = pc + (size_t)buf * 7 * S;
-        Bf[me] = idet; Bf[S + me] = beta * idet; Bf[2 * S + me] = gamma * idet; Bf[3 * S + me] = lo_; Bf[4 * S + me] = up_;
-        Bf[5 * S + me] = q0; Bf[6 * S + me] = q1;
-        __syncthreads();
+        double* Bf = pc + buf * S6 + me;
+        Bf[0] = up_ * beta * idet; Bf[S] = q0; Bf[2 * S] = lo_ * idet;
+        Bf[3 * S] = lo_ * gamma * idet; Bf[4 * S] = q1; Bf[5 * S] = up_ * idet;
+        // couplings below 1e-30 of the unit diagonal are invisible in fp64: once every block of the CTA's lines is decoupled
+        // (decayed spikes) the remaining steps would change nothing
+        if (!__syncthreads_or(fabs(lo_) > 1e-30 || fabs(up_) > 1e-30)) break;
         if (p >= 1) {
             double ln = 0.0, un = 0.0;
+            const int off = dd * pst;
             if (p - dd >= 1) {
-                const int Li = me - dd * pst;
-                beta = fma(lo_ * Bf[4 * S + Li], Bf[S + Li], beta);
-                r0 = fma(-lo_, Bf[5 * S + Li], r0);
-                ln = -lo_ * Bf[3 * S + Li] * Bf[Li];
+                const double* Lp = Bf - off;
+                beta = fma(lo_, Lp[0], beta);
+                r0 = fma(-lo_, Lp[S], r0);
+                ln = -lo_ * Lp[2 * S];
             }
             if (p + dd <= K) {
-                const int Ri = me + dd * pst;
-                gamma = fma(up_ * Bf[3 * S + Ri], Bf[2 * S + Ri], gamma);
-                r1 = fma(-up_, Bf[6 * S + Ri], r1);
-                un = -up_ * Bf[4 * S + Ri] * Bf[Ri];
+                const double* Rp = Bf + off;
+                gamma = fma(up_, Rp[3 * S], gamma);
+                r1 = fma(-up_, Rp[4 * S], r1);
+                un = -up_ * Rp[5 * S];
             }
             lo_ = ln; up_ = un;
         }
@@ -228,12 +241,14 @@ k_general_part(GeneralArgs G) {
     // more (they were read a moment ago: L1 / L2): the componentwise backward error of the line's equations in this
     // thread's rows.  NaN fails every comparison.
     s_xf[me] = D_[0]; s_xl[me] = D_[M - 1];                             // s_xf / s_xl were last read before the first barrier of the PCR
+    if (!tame && valid) s_bad[L + lt] = 1;                              // benign race: every writer stores 1
     __syncthreads();
     const double xprev = (p >= 1) ? s_xl[me - pst] : 0.0, xnext = (p <= P - 2) ? s_xf[me + pst] : 0.0;
     bool bad = false;
+    const bool check = s_bad[L + lt] != 0;                              // a line of tame blocks only is accepted as it is: no second read
 #pragma unroll
     for (int jj = 0; jj < M; ++jj) {
-        if (valid && jj < m) {
+        if (check && valid && jj < m) {
             const long long e = e0 + (long long)jj * G.row_stride;
             const double av = __ldg(G.a + e), bv = __ldg(G.b + e), cv = __ldg(G.c + e), dv = __ldg(G.d + e);
             const double xlo = (jj == 0) ? xprev : D_[jj > 0 ? jj - 1 : 0];
@@ -243,10 +258,9 @@ k_general_part(GeneralArgs G) {
             if (!(fabs(res) <= kGeneralBackwardError * (fabs(t1) + fabs(t2) + fabs(t3) + fabs(dv)))) bad = true;
         }
     }
-    if (bad) s_bad[lt] = 1;                                             // benign race: every writer stores 1
-    if (!tame && valid) s_bad[L + lt] = 1;
+    if (bad) s_bad[lt] = 1;
     __syncthreads();
-    if (s_bad[lt] != 0 && s_bad[L + lt] != 0) {
+    if (s_bad[lt] != 0) {
         if (p == 0 && valid) {
             const unsigned slot = atomicAdd(G.fb_count, 1u);
             if (slot < G.fb_cap) G.fb_lines[slot] = (unsigned)((long long)o * G.W + l);

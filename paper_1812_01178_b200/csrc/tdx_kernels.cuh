@@ -27,6 +27,9 @@ struct Tables {
     const int* Sidx;         // cyclic closure functional (sparse), Sidx/Sval[set*Scap + k], Sn[set]
     const double* Sval;
     const int* Sn;
+    const double* pcr;       // PPT by plan-time cyclic reduction (k_pcr_tables): pcr[((set*pcr_cap + step)*P + p)*6 + f]; NULL = band of Z^-1 rows
+    const int* pcr_n;        // exchange steps per set
+    int pcr_cap;
     int P, n, q, r, KB, Scap;   // P: kernel partitions; q, r: the CALLER's partition map (n / Pu, n % Pu)
     int S;                      // sub-partitions per caller's partition (sub_part; 1 = plain map)
 };
@@ -42,6 +45,7 @@ struct StridedArgs {
     int pf;                  // L2 prefetch distance: CTAs ahead (one tile per CTA) or sets ahead (looping CTAs); 0 = off
     int tiles_x;             // column tiles per outer index
     int tables_smem;         // 1: the TS instantiation (set's tables staged in shared memory)
+    int pcr;                 // 1: the PCR instantiation (Tables::pcr)
     double* iface;           // slab sweeps (tdx_slab_eliminate): also store row 0 of every line to iface[0][outer][W*V] and its last
     long long iface_plane;   //   row to iface[1][...] (Alg.1 step 4's pack, fused into the store); iface_plane = doubles per plane; NULL = off
 };
@@ -77,9 +81,13 @@ template <int M> struct UniTable { double v[M * 6]; };
 // coefficients into shared memory once, before its tiles; every table read of the three passes and of the band loop is
 // then an LDS (two addresses per warp, partitions padded by 16 bytes: conflict-free) instead of an L1 hit competing with
 // the tile's own loads and stores in the L1TEX pipe.
-template <int MAXM, int V, bool CYC, bool UNI, int REGS = strided_regs(MAXM, V), bool TS = false>
+// PCR (PPT, non-periodic lines): the reduced system is solved by block cyclic reduction with plan-time coefficients
+// (k_pcr_tables, tdx_plan.cuh) instead of the 2P-term band of Z^-1 rows: ceil(log2(P-1)) steps of six multiply-adds per line,
+// one barrier each, right-hand sides exchanged through double-buffered shared memory.
+template <int MAXM, int V, bool CYC, bool UNI, int REGS = strided_regs(MAXM, V), bool TS = false, bool PCR = false>
 __global__ void __maxnreg__(REGS)
 k_strided(StridedArgs A, Tables T, const __grid_constant__ UniTable<UNI ? MAXM : 1> U) {
+    static_assert(!(PCR && (TS || CYC || UNI)), "PCR is built for the plain per-set tables only");
     extern __shared__ double rs[];                          // rs[(idx*LPC + tx)*V + v], idx in [0, 2P)
     const int tx = threadIdx.x, p = threadIdx.y;
     const int LPC = A.LPC, P = T.P;
@@ -181,7 +189,48 @@ k_strided(StridedArgs A, Tables T, const __grid_constant__ UniTable<UNI ? MAXM :
     double yL[V], yR[V], sc[V];
 #pragma unroll
     for (int v = 0; v < V; ++v) { yL[v] = 0.0; yR[v] = 0.0; sc[v] = 0.0; }
-    {
+    if (PCR) {
+        // block p = (s_p, t_p) = (x_last of partition p-1, x_first of partition p), p = 1..P-1; thread 0 only takes part in the barriers
+        double* pb = rs + (size_t)2 * P * LPC * V;          // 2 buffers x {q0, q1} x [P][LPC*V]
+        const int S2 = P * LPC * V, me = (p * LPC + tx) * V;
+        const int nst = __ldg(&T.pcr_n[set]);
+        const double2* pc = reinterpret_cast<const double2*>(T.pcr) + ((size_t)set * T.pcr_cap * P + p) * 3;
+        double r0[V], r1[V], q0[V], q1[V];
+#pragma unroll
+        for (int v = 0; v < V; ++v) {
+            r0[v] = (p >= 1) ? rs[((2 * p - 1) * LPC + tx) * V + v] : 0.0;   // xt_last of partition p-1
+            r1[v] = (p >= 1) ? x[0][v] : 0.0;                                  // xt_first of this partition
+        }
+        for (int s = 0, d = 1;; ++s, d <<= 1) {
+            const double2 c0 = __ldg(pc + (size_t)s * P * 3), c1 = __ldg(pc + (size_t)s * P * 3 + 1), c2 = __ldg(pc + (size_t)s * P * 3 + 2);
+#pragma unroll
+            for (int v = 0; v < V; ++v) {                   // D^-1 r: {idet, -beta idet}, {-gamma idet, l}, {u, -}
+                q0[v] = fma(c0.y, r1[v], c0.x * r0[v]);
+                q1[v] = fma(c1.x, r0[v], c0.x * r1[v]);
+            }
+            double* B = pb + (size_t)(s & 1) * 2 * S2;
+            if (s == nst) {                                 // decoupled: s_p = q0 (own), t_{p+1} = q1 of the next block
+#pragma unroll
+                for (int v = 0; v < V; ++v) B[S2 + me + v] = q1[v];
+                __syncthreads();
+#pragma unroll
+                for (int v = 0; v < V; ++v) {
+                    yL[v] = q0[v];
+                    yR[v] = (p <= P - 2) ? B[S2 + me + LPC * V + v] : 0.0;
+                }
+                break;
+            }
+#pragma unroll
+            for (int v = 0; v < V; ++v) { B[me + v] = q0[v]; B[S2 + me + v] = q1[v]; }
+            __syncthreads();
+            const int mL = ((p - d > 0 ? p - d : 0) * LPC + tx) * V, mR = ((p + d < P - 1 ? p + d : P - 1) * LPC + tx) * V;   // l, u are 0 beyond the ends
+#pragma unroll
+            for (int v = 0; v < V; ++v) {
+                r0[v] = fma(-c1.y, B[mL + v], r0[v]);
+                r1[v] = fma(-c2.x, B[S2 + mR + v], r1[v]);
+            }
+        }
+    } else {
         const int2 bd = __ldg(&T.band[set * P + p]);
         const double2* g2 = reinterpret_cast<const double2*>(T.G) + (size_t)set * T.KB * P + p;
         auto term = [&](int k) {

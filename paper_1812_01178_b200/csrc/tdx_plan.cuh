@@ -549,6 +549,56 @@ __global__ void k_composite_factor(int P, int S, int wrap, int pdd, const double
     }
 }
 
+// ---- a3 for PPT without the dense Z^-1: block parallel cyclic reduction with PLAN-TIME coefficients -----------------------
+// The band of Z^-1 rows (k_pack_ppt) costs every thread up to 2P terms per line; where the spikes decay slowly (the weakly
+// dominant Poisson y-systems) the band is full and P cannot grow.  The reduced system in natural order is
+// block tridiagonal (block i = (s_i, t_i) = (x_last_{i-1}, x_first_i), i = 1..K = P-1; reading A7):
+//   l_i s_{i-1} + s_i + beta_i t_i = r0_i,      gamma_i s_i + t_i + u_i t_{i+1} = r1_i
+// and a cyclic-reduction step of distance d (substitute blocks i-d and i+d into block i) keeps that form -- the recurrences
+// are those of k_helm_lines (tdx_kernels.cuh), but here the matrix is shared by all lines, so the coefficients of every
+// step are tabulated once and a line only updates its right-hand side: per step and block
+//   q0 = idet (r0 - beta r1),  q1 = idet (r1 - gamma r0);   r0 -= l q0[i-d],  r1 -= u q1[i+d]
+// ceil(log2 K) steps of 4 + 2 multiply-adds instead of 2P-term dot products; no pivoting is needed in this order (unit
+// diagonal, |spikes| < 1).  Table: pcr[((set*cap + step)*P + i)*6 + {idet, -beta idet, -gamma idet, l, u, 0}], entry i = 0
+// all zero; nsteps[set] = exchange steps until every coupling is below 1e-30 (decayed spikes: the rest would change
+// nothing); the entry of step nsteps[set] holds the final block inverses.  One CTA per set, thread = block, P <= 256.
+__global__ void __launch_bounds__(256) k_pcr_tables(int P, int cap, const double* __restrict__ ends, double* __restrict__ pcr,
+                                                    int* __restrict__ nsteps) {
+    __shared__ double sl[2][256], su[2][256], se01[256], se10[256], sid[256];
+    const int set = blockIdx.x, i = threadIdx.x, K = P - 1;
+    const double* e = ends + (size_t)set * P * 4;
+    const bool blk = i >= 1 && i <= K;
+    double beta = 0.0, gamma = 0.0, l = 0.0, u = 0.0;
+    if (blk) {
+        beta = e[(i - 1) * 4 + 3];                          // w_last^(i-1)
+        gamma = e[i * 4 + 0];                               // v_first^(i)
+        l = (i >= 2) ? e[(i - 1) * 4 + 1] : 0.0;            // v_last^(i-1)
+        u = (i <= K - 1) ? e[i * 4 + 2] : 0.0;              // w_first^(i)
+    }
+    int cur = 0, nst = 0;
+    sl[0][i] = l; su[0][i] = u;
+    for (int d = 1, s = 0;; d <<= 1, ++s) {
+        const double idet = blk ? 1.0 / (1.0 - beta * gamma) : 0.0;
+        if (i < P) {
+            double* t = pcr + (((size_t)set * cap + s) * P + i) * 6;
+            t[0] = idet; t[1] = -beta * idet; t[2] = -gamma * idet; t[3] = l; t[4] = u; t[5] = 0.0;
+        }
+        nst = s;
+        if (d >= K || s + 1 >= cap) break;                  // uniform over the CTA
+        sid[i] = idet; se01[i] = beta * idet; se10[i] = gamma * idet;
+        if (!__syncthreads_or(fabs(l) > 1e-30 || fabs(u) > 1e-30)) break;
+        double ln = 0.0, un = 0.0;
+        if (blk) {
+            if (i - d >= 1) { const int L = i - d; beta = fma(l * su[cur][L], se01[L], beta); ln = -l * sl[cur][L] * sid[L]; }
+            if (i + d <= K) { const int R = i + d; gamma = fma(u * sl[cur][R], se10[R], gamma); un = -u * su[cur][R] * sid[R]; }
+        }
+        l = ln; u = un; cur ^= 1;
+        sl[cur][i] = l; su[cur][i] = u;
+        __syncthreads();
+    }
+    if (i == 0) nsteps[set] = nst;
+}
+
 // PDD (Alg.1 step 5): interface i block [[1, w_last^(i-1)],[v_first^(i), 1]] inverted explicitly:
 //   y_{2i-1} = (xt_last^(i-1) - w_last^(i-1) xt_first^(i))/det,  y_{2i} = (xt_first^(i) - v_first^(i) xt_last^(i-1))/det.
 // band of partition p: r[2p-1 .. 2p+2].
