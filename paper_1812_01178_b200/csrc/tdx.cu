@@ -178,6 +178,16 @@ int choose_split(int n, int P, int dir) {
     return mo <= 64 ? 1 : -1;
 }
 
+// x lines: does (n, P) reach the TMA kernel, directly or through a two-level plan (choose_split)?
+bool x_shape_is_fast(int n, int P) {
+    if (n % P != 0) return false;
+    const int q = n / P;
+    if (q == 8 || q == 16 || q == 32) return true;
+    for (int target : {16, 8, 32})
+        if (q % target == 0 && (long long)P * (q / target) <= kMaxKernelP) return true;
+    return false;
+}
+
 int pick_M(int maxlen) {
     for (int m : kMInst) if (m >= maxlen) return m;
     return -1;
@@ -397,6 +407,13 @@ tdx_status_t get_plan(tdx_grid* g, int kind, int dir, int mode, int P, double al
         if (P < 1 || P > TDX_MAX_P || n / P < 2) return fail(TDX_ERR_BAD_PARTITION, "P=%d invalid for line length %d (need 1 <= P <= %d, floor(n/P) >= 2)", P, n, TDX_MAX_P);
     }
     if (thomas) { P = 1; mode = TDX_MODE_THOMAS; }
+    // x lines in PPT: the result does not depend on the partitioning (PPT "makes no approximation"), so a
+    // shape the TMA kernel cannot take even after cutting the partitions again -- ragged partitions (n % P != 0), lengths
+    // without a divisor 8 / 16 / 32 -- is solved with partitions of 16 (8, 32) rows instead whenever the line length allows,
+    // rather than by the generic kernel (1.0-1.3 TB/s: its per-partition tables do not fit L1).  PDD keeps the caller's map.
+    if (!thomas && mode == TDX_MODE_PPT && dir == 0 && kind != KIND_HELM && !x_shape_is_fast(n, P))
+        for (int target : {16, 8, 32})
+            if (n % target == 0 && n / target >= 2 && n / target <= TDX_MAX_P) { P = n / target; break; }
     const bool periodic = (kind == KIND_USER) || (kind == KIND_ADI && g->bc[dir] == TDX_BC_PERIODIC);
     if (periodic && n < 3) return fail(TDX_ERR_INVALID_ARG, "periodic line needs n >= 3");
     // Long partitions (more rows than a thread keeps in registers, or a shape the fast kernels do not take): every partition is
@@ -432,6 +449,25 @@ tdx_status_t get_plan(tdx_grid* g, int kind, int dir, int mode, int P, double al
     g->plans.push_back(pl);
     *out = &g->plans.back();
     return strict_check(g, g->plans.back(), enforce_strict);
+}
+
+// The plan a SWEEP runs with.  As get_plan, except: PDD along x on a shape the TMA kernel cannot take (ragged partitions,
+// lengths without a divisor 8 / 16 / 32) whose dropped couplings are below fp64 visibility (a-priori bound < 1e-20: every
+// uniform x grid of the configs, bounds 1e-40 ... 1e-300) IS the exact solution to rounding -- so it runs on the
+// re-partitioned PPT plan (get_plan) instead of the generic kernel.  The strict switch and tdx_pdd_dropped_bound still see
+// the caller's PDD plan.  Looked up per call (no pointer is kept: plans may be trimmed).
+tdx_status_t get_sweep_plan(tdx_grid* g, int kind, int dir, int mode, int P, double alpha, const double* ua, const double* ub,
+                            const double* uc, cudaStream_t st, Plan** out, int loc = 0) {
+    tdx_status_t rc = get_plan(g, kind, dir, mode, P, alpha, 1, nullptr, ua, ub, uc, st, out, loc);
+    if (rc != TDX_OK) return rc;
+    const Plan& pl = **out;
+    if (dir == 0 && mode == TDX_MODE_PDD && !pl.thomas && !x_shape_is_fast(pl.n, pl.Pu) && pl.dropped < 1e-20) {
+        Plan* alt = nullptr;
+        rc = get_plan(g, kind, dir, TDX_MODE_PPT, P, alpha, 1, nullptr, ua, ub, uc, st, &alt, loc);
+        if (rc == TDX_OK && alt && x_shape_is_fast(alt->n, alt->Pu)) *out = alt;
+        else if (rc != TDX_OK) return rc;
+    }
+    return TDX_OK;
 }
 
 Tables tables_of(const Plan& pl) {
@@ -1148,7 +1184,7 @@ tdx_status_t tdx_adi_sweep(tdx_grid_t* g, tdx_dir_t dir, tdx_mode_t mode, int P,
     CUDA_TRY(cudaSetDevice(g->device));
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     Plan* pl = nullptr;
-    rc = get_plan(g, KIND_ADI, dir, mode, P, alpha, 1, nullptr, nullptr, nullptr, nullptr, st, &pl);
+    rc = get_sweep_plan(g, KIND_ADI, dir, mode, P, alpha, nullptr, nullptr, nullptr, st, &pl);
     if (rc != TDX_OK) return rc;
     return run_sweep(g, *pl, dir, rhs, st);
 }
@@ -1162,7 +1198,7 @@ tdx_status_t tdx_adi_sweep_at(tdx_grid_t* g, tdx_dir_t dir, tdx_loc_t loc, tdx_m
     CUDA_TRY(cudaSetDevice(g->device));
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     Plan* pl = nullptr;
-    rc = get_plan(g, KIND_ADI, dir, mode, P, alpha, 1, nullptr, nullptr, nullptr, nullptr, st, &pl, (int)loc);
+    rc = get_sweep_plan(g, KIND_ADI, dir, mode, P, alpha, nullptr, nullptr, nullptr, st, &pl, (int)loc);
     if (rc != TDX_OK) return rc;
     return run_sweep(g, *pl, dir, rhs, st);
 }
@@ -1185,7 +1221,7 @@ tdx_status_t tdx_adi_step(tdx_grid_t* g, tdx_mode_t mode, int Px, int Py, int Pz
             const int l = loc ? loc[c * 3 + d] : 0;
             if (l != 0 && l != 1) return fail(TDX_ERR_INVALID_ARG, "loc[%d][%d]=%d not in {0,1}", c, d, l);
             if (l == 1 && !g->lo_face[d]) return fail(TDX_ERR_UNSUPPORTED, "face-located unknowns need Dirichlet or periodic ends in direction %d", d);
-            if (!pls[d][l]) { rc = get_plan(g, KIND_ADI, d, mode, Ps[d], alpha, 1, nullptr, nullptr, nullptr, nullptr, st, &pls[d][l], l); if (rc != TDX_OK) return rc; }
+            if (!pls[d][l]) { rc = get_sweep_plan(g, KIND_ADI, d, mode, Ps[d], alpha, nullptr, nullptr, nullptr, st, &pls[d][l], l); if (rc != TDX_OK) return rc; }
         }
     for (int d = 0; d < 3; ++d) {
         int c = 0;
@@ -1209,7 +1245,7 @@ tdx_status_t tdx_cyclic_solve(tdx_grid_t* g, tdx_dir_t dir, tdx_mode_t mode, int
     CUDA_TRY(cudaSetDevice(g->device));
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     Plan* pl = nullptr;
-    rc = get_plan(g, KIND_USER, dir, mode, P, 0.0, 1, nullptr, a, b, c, st, &pl);
+    rc = get_sweep_plan(g, KIND_USER, dir, mode, P, 0.0, a, b, c, st, &pl);
     if (rc != TDX_OK) return rc;
     return run_sweep(g, *pl, dir, rhs, st);
 }
@@ -1675,7 +1711,7 @@ tdx_status_t tdx_adi_step_host(tdx_grid_t* g, tdx_mode_t mode, int Px, int Py, i
     const int Ps[3] = {Px, Py, Pz};
     Plan* pls[3];
     for (int d = 0; d < 3; ++d) {                       // validate everything before any copy
-        rc = get_plan(g, KIND_ADI, d, mode, Ps[d], alpha, 1, nullptr, nullptr, nullptr, nullptr, 0, &pls[d]);
+        rc = get_sweep_plan(g, KIND_ADI, d, mode, Ps[d], alpha, nullptr, nullptr, nullptr, 0, &pls[d]);
         if (rc != TDX_OK) return rc;
     }
     rc = ensure_stage(g, bytes);
@@ -1693,7 +1729,7 @@ tdx_status_t tdx_adi_sweep_host(tdx_grid_t* g, tdx_dir_t dir, tdx_mode_t mode, i
     CUDA_TRY(cudaSetDevice(g->device));
     const size_t bytes = (size_t)g->nx * g->ny * g->nz * 8;
     Plan* pl = nullptr;
-    rc = get_plan(g, KIND_ADI, dir, mode, P, alpha, 1, nullptr, nullptr, nullptr, nullptr, 0, &pl);
+    rc = get_sweep_plan(g, KIND_ADI, dir, mode, P, alpha, nullptr, nullptr, nullptr, 0, &pl);
     if (rc != TDX_OK) return rc;
     rc = ensure_stage(g, bytes);
     if (rc != TDX_OK) return rc;
@@ -1731,7 +1767,7 @@ tdx_status_t tdx_step_host(tdx_grid_t* g, tdx_mode_t mode, int Px, int Py, int P
     if (host_field) {
         const int Ps[3] = {Px, Py, Pz};
         for (int d = 0; d < 3; ++d) {                       // validate and build every plan before any copy
-            rc = get_plan(g, KIND_ADI, d, mode, Ps[d], alpha, 1, nullptr, nullptr, nullptr, nullptr, g->s_comp, &pls[d]);
+            rc = get_sweep_plan(g, KIND_ADI, d, mode, Ps[d], alpha, nullptr, nullptr, nullptr, g->s_comp, &pls[d]);
             if (rc != TDX_OK) return rc;
         }
         rc = ensure_stage(g, (size_t)nx * ny * nz * 8);

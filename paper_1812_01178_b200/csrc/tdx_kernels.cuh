@@ -64,7 +64,7 @@ template <> struct VecIO<2> {
 // values in flight and the interface unknowns.  Measured on B200 (development sweeps): spills cost more than
 // occupancy, and 2-4 small co-resident CTAs per SM beat one large one.
 constexpr int strided_regs(int MAXM, int V) {
-    return (MAXM * V <= 8) ? 72 : ((MAXM * V <= 16) ? 104 : ((MAXM * V <= 32) ? 128 : ((MAXM * V <= 48) ? 168 : 255)));
+    return (MAXM * V <= 8) ? 64 : ((MAXM * V <= 16) ? 104 : ((MAXM * V <= 32) ? 128 : ((MAXM * V <= 48) ? 168 : 255)));
 }
 constexpr int strided_block_threads(int MAXM, int V) {            // largest CTA the register budget allows
     return (65536 / strided_regs(MAXM, V)) / 32 * 32 > 1024 ? 1024 : (65536 / strided_regs(MAXM, V)) / 32 * 32;
@@ -629,7 +629,9 @@ k_helm_lines(double2* __restrict__ data, int nx, int ny, int P, int q, int rq, i
             u = (p <= K - 1) ? s_wf[me] : 0.0;
             r0 = s_xl[a]; r1 = s_xf[me];
         }
-        double* pc = reinterpret_cast<double*>(s_y1 + S);            // 2 buffers x {idet, e01, e10, l, u, q0 (2), q1 (2)} x S
+        // Per step a block hands its neighbours products, not raw coefficients: to the block d to its right {u e01, l idet} and
+        // q0, to the block d to its left {l e10, u idet} and q1 -- 16-byte pairs, 4 stores and 4 loads per step.
+        double2* pc = s_y1 + S;                                      // 2 buffers x {cR, q0, cL, q1} x S (16 bytes each)
         int buf = 0;
         double2 q0, q1;
         for (int d = 1;; d <<= 1) {
@@ -637,28 +639,26 @@ k_helm_lines(double2* __restrict__ data, int nx, int ny, int P, int q, int rq, i
             q0 = make_double2((r0.x - beta * r1.x) * idet, (r0.y - beta * r1.y) * idet);
             q1 = make_double2((r1.x - gamma * r0.x) * idet, (r1.y - gamma * r0.y) * idet);
             if (d >= K) break;                                       // uniform over the CTA
-            double* B = pc + (size_t)buf * 9 * S;
-            B[me] = idet; B[S + me] = beta * idet; B[2 * S + me] = gamma * idet; B[3 * S + me] = l; B[4 * S + me] = u;
-            reinterpret_cast<double2*>(B + 5 * S)[me] = q0;
-            reinterpret_cast<double2*>(B + 7 * S)[me] = q1;
+            double2* B = pc + buf * 4 * S + me;
+            B[0] = make_double2(u * beta * idet, l * idet); B[S] = q0;
+            B[2 * S] = make_double2(l * gamma * idet, u * idet); B[3 * S] = q1;
             // couplings below 1e-30 of the unit diagonal are invisible in fp64: once every block of the CTA's lines is
             // decoupled (decayed spikes: high wavenumbers away from the wall) the remaining steps would change nothing
             if (!__syncthreads_or(fabs(l) > 1e-30 || fabs(u) > 1e-30)) break;
             if (p >= 1) {
                 double ln = 0.0, un = 0.0;
+                const int off = d * LPC;
                 if (p - d >= 1) {
-                    const int L = me - d * LPC;
-                    const double2 qL = reinterpret_cast<const double2*>(B + 5 * S)[L];
-                    beta = fma(l * B[4 * S + L], B[S + L], beta);
+                    const double2 cR = B[-off], qL = B[S - off];
+                    beta = fma(l, cR.x, beta);
                     r0.x = fma(-l, qL.x, r0.x); r0.y = fma(-l, qL.y, r0.y);
-                    ln = -l * B[3 * S + L] * B[L];
+                    ln = -l * cR.y;
                 }
                 if (p + d <= K) {
-                    const int R = me + d * LPC;
-                    const double2 qR = reinterpret_cast<const double2*>(B + 7 * S)[R];
-                    gamma = fma(u * B[3 * S + R], B[2 * S + R], gamma);
+                    const double2 cL = B[2 * S + off], qR = B[3 * S + off];
+                    gamma = fma(u, cL.x, gamma);
                     r1.x = fma(-u, qR.x, r1.x); r1.y = fma(-u, qR.y, r1.y);
-                    un = -u * B[4 * S + R] * B[R];
+                    un = -u * cL.y;
                 }
                 l = ln; u = un;
             }
