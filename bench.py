@@ -579,8 +579,9 @@ def run_tdx(args, rank, world, local_rank):
                         ga, gc = (torch.rand(field0.shape, dtype=torch.float64, device=field0.device, generator=gen) * 2 - 1 for _ in range(2))
                         gb = (torch.rand(field0.shape, dtype=torch.float64, device=field0.device, generator=gen) * 2 - 1) * 0.3
                     res = {}
-                    # both methods (include/tdx.h): "lines" = one thread per line, two passes, the default for y / z lines;
-                    # "partition" = the one-pass partition kernel (forced here; the default for x lines)
+                    # both methods (include/tdx.h): "partition" = the one-pass partition kernel (the default: optimistic plain
+                    # elimination inside the partitions, checked, unsafe lines re-solved with pivots); "lines" = one thread
+                    # per line with diagonal pivoting, two passes
                     for meth, flag, nbytes in (("lines", tdx.GENERAL_FORCE_LINES, 82), ("partition", tdx.GENERAL_FORCE_PARTITION, 40)):
                         for _ in range(2):
                             gd.copy_(field0); grid.general_solve(1, 1 | flag, ga, gb, gc, gd, gwork, stream)
@@ -599,7 +600,7 @@ def run_tdx(args, rank, world, local_rank):
                                      "frac_of_measured_peak": nbytes * cfg.npts / (msg * 1e-3) / 1e9 / peak, "finite": bool(torch.isfinite(gd).all()),
                                      "lines_re_solved_by_the_per_line_kernel": nfb, "share_of_lines": nfb / (cfg.nx * cfg.nz), "launch": tdx.last_launch()}
                     gout[wname] = res
-                gout["what"] = "tdx_general_solve along y, per-line a, b, c, diagonal pivoting: per-line kernel (two passes, 82 B per value; default for y / z) and partition kernel (8-row partitions, one pass, 40 B per value; default for x)"
+                gout["what"] = "tdx_general_solve along y, per-line a, b, c, diagonal pivoting: partition kernel (8-row partitions, one pass, 40 B per value; the default) and per-line kernel (two passes, 82 B per value)"
                 out["general_solve_pivoting"] = gout
                 del ga, gb, gc, gd, gwork
         except Exception as exc:

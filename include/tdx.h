@@ -193,14 +193,20 @@ tdx_status_t tdx_slab_dropped_bound(tdx_slab_t* slab, double* out);
  * backward error of the line's equations) before it is stored, and a line that fails -- a numerically singular partition
  * block; the line itself may be regular -- is solved instead, in the same call, by the other method;
  * tdx_general_fallback_count says how many lines of the grid's last general solve that were (it synchronises).
+ * With pivoting != 0 the partition pass runs OPTIMISTICALLY with plain elimination: a line is accepted when the LU factors of
+ * all its blocks are componentwise stable (|L||U| <= 4|A|: true for row- or column-dominant rows) and the spikes stay <= 1, or
+ * when it passes the backward-error check; every other line is re-solved WITH the diagonal pivots by the LINES method.  The flag
+ * TDX_GENERAL_PIVOT_PARTITIONS keeps the pivots inside the partitions instead (fewer re-solved lines on non-dominant
+ * systems, slower on dominant ones).
  * LINES: one thread per line, diagonal pivoting over the whole line, two passes over HBM (about 82 B per value).
- * Default: PARTITION for x lines, LINES for y / z lines (each where it measured faster); OR the flags below
- * into `pivoting` to force one.  Periodic lines, and lines of fewer than 4 or more than 4096 rows, always take LINES.
+ * Default: PARTITION wherever it applies (it measured faster in every direction); OR the flags below into
+ * `pivoting` to force one.  Periodic lines, and lines of fewer than 4 or more than 4096 rows, always take LINES.
  * work: DEVICE scratch, caller-owned, 8-byte aligned: 9*nx*ny*nz + 8 bytes (tdx_general_solve), 25*nx*ny*nz + 24 bytes
  * (tdx_general_cyclic_solve).  A singular line yields inf / nan in that line.  Asynchronous on `stream`.       */
 #define TDX_GENERAL_PIVOT 1
 #define TDX_GENERAL_FORCE_PARTITION 16
 #define TDX_GENERAL_FORCE_LINES 32
+#define TDX_GENERAL_PIVOT_PARTITIONS 64   /* PARTITION method: keep the 1x1 / 2x2 pivots inside the partitions (see below) */
 tdx_status_t tdx_general_solve(tdx_grid_t* grid, tdx_dir_t dir, int pivoting, const double* a, const double* b,
                                const double* c, double* rhs_inout, void* work, void* stream);
 tdx_status_t tdx_general_cyclic_solve(tdx_grid_t* grid, tdx_dir_t dir, int pivoting, const double* a, const double* b,

@@ -14,7 +14,7 @@ DIR_X, DIR_Y, DIR_Z = 0, 1, 2
 MODE_THOMAS, MODE_PDD, MODE_PPT = 0, 1, 2
 BC_DIRICHLET, BC_PERIODIC, BC_NEUMANN = 0, 1, 2
 LOC_CENTER, LOC_FACE = 0, 1
-GENERAL_PIVOT, GENERAL_FORCE_PARTITION, GENERAL_FORCE_LINES = 1, 16, 32
+GENERAL_PIVOT, GENERAL_FORCE_PARTITION, GENERAL_FORCE_LINES, GENERAL_PIVOT_PARTITIONS = 1, 16, 32, 64
 OK, ERR_INVALID_ARG, ERR_BAD_PARTITION, ERR_ALLOC, ERR_CUDA, ERR_UNSUPPORTED, ERR_PDD_BOUND = 0, -1, -2, -3, -4, -5, -6
 
 EXPORTS = ("tdx_grid_create", "tdx_grid_destroy", "tdx_grid_set_pdd_strict", "tdx_partition_bounds", "tdx_adi_sweep", "tdx_adi_sweep_at", "tdx_adi_step",

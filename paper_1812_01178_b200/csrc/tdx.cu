@@ -1603,9 +1603,10 @@ static tdx_status_t general_solve_impl(tdx_grid_t* g, tdx_dir_t dir, int pivotin
     unsigned char* flag = reinterpret_cast<unsigned char*>(bm + npts);
     double* qv = reinterpret_cast<double*>(flag + ((npts + 7) / 8) * 8);                 // periodic only (25 bytes per value in all)
     double* dv = qv + npts;
-    // Method: the partition kernel (8 rows per thread, P threads of a line in one CTA) where it is the faster one -- measured
-    // on cfg5: x lines 18.0 ms against 76.8 ms for one thread per (contiguous) line; y / z lines 19.0 / 30.2 ms
-    // against 10.9 / 11.2 ms, so strided lines take the per-line kernel unless the caller forces the partition method.
+    // Method: the partition kernel (8 rows per thread, P threads of a line in one CTA) wherever it applies -- measured on cfg5
+    // (DESIGN.md 9f): 7.05 / 9.17 / 11.5 ms along y / z / x against 10.9 / 11.2 / 77 ms for one thread per line -- unless the
+    // caller forces the per-line kernel.
+    const int flags_in = pivoting;
     const int method = pivoting & (TDX_GENERAL_FORCE_PARTITION | TDX_GENERAL_FORCE_LINES);
     pivoting &= 1;
     if (method == (TDX_GENERAL_FORCE_PARTITION | TDX_GENERAL_FORCE_LINES)) return fail(TDX_ERR_INVALID_ARG, "both methods forced");
@@ -1613,7 +1614,7 @@ static tdx_status_t general_solve_impl(tdx_grid_t* g, tdx_dir_t dir, int pivotin
     int P = (n + M - 1) / M; if (P < 2) P = 2;
     const bool can_part = !periodic && n / P >= 2 && P <= 512;                           // 512 threads of 128 registers
     if (method == TDX_GENERAL_FORCE_PARTITION && !can_part) return fail(TDX_ERR_UNSUPPORTED, "the partition method takes non-periodic lines of 4 to 4096 rows");
-    const bool part = can_part && (method == TDX_GENERAL_FORCE_PARTITION || (method == 0 && dir == TDX_DIR_X));
+    const bool part = can_part && method != TDX_GENERAL_FORCE_LINES;
     if (!part) {                                                                         // one thread per line over the whole line
         dim3 block(128), grid((unsigned)std::min<long long>((G.W + 127) / 128, 1 << 20), (unsigned)O);
         G.fb_count = nullptr; G.fb_lines = nullptr; G.fb_cap = 0; G.P = 1; G.q = n; G.r = 0;
@@ -1640,20 +1641,27 @@ static tdx_status_t general_solve_impl(tdx_grid_t* g, tdx_dir_t dir, int pivotin
     // large one; x lines: whole lines of P consecutive lanes.  TDX_GENERAL_LINES (measurement knob) overrides.
     static const int env_L = [] { const char* e = std::getenv("TDX_GENERAL_LINES"); return e ? std::atoi(e) : 0; }();
     int L = 1;
-    const int cap = env_L > 0 ? env_L : 4;
+    const bool pv_part = pivoting && (flags_in & TDX_GENERAL_PIVOT_PARTITIONS);
+    const int cap = env_L > 0 ? env_L : (pv_part ? 4 : 8);             // plain elimination runs at 96 registers: 8 lines x P threads, two CTAs per SM
     while (L * 2 * P <= 512 && L * 2 <= (unit ? std::max(1, 128 / P) : cap)) L *= 2;
     if ((long long)L > G.W) { L = 1; while ((long long)L * 2 <= G.W && L * 2 * P <= 512) L *= 2; }
     dim3 block = unit ? dim3(P, L) : dim3(L, P), grid((unsigned)((G.W + L - 1) / L), (unsigned)O);
     const size_t smem = (size_t)19 * P * L * 8 + (size_t)L * 8 + 16;
-#define TDX_GENERAL_PART(PV, UN)                                                                                              \
+    // pivoting solves run the partition kernel OPTIMISTICALLY with plain elimination (k_general_part, "PIVOT = false"): lines
+    // it cannot vouch for go to the pivoted per-line kernel below.  TDX_GENERAL_PIVOT_PARTITIONS keeps the 1x1 / 2x2 pivots
+    // inside the partitions (fewer lines fall back on non-dominant systems; 40 % more instructions on dominant ones).
+    const bool full = (n % P == 0) && (n / P == M);
+#define TDX_GENERAL_PART(PV, UN, FU)                                                                                          \
     do { static DevOnce attr;                                                                                                 \
-         if (attr.need(g->device)) { CUDA_TRY(cudaFuncSetAttribute(tdx::k_general_part<8, PV, UN>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024)); attr.set(g->device); } \
-         tdx::k_general_part<8, PV, UN><<<grid, block, smem, st>>>(G); } while (0)
-    if (pivoting) { if (unit) TDX_GENERAL_PART(true, true); else TDX_GENERAL_PART(true, false); }
-    else { if (unit) TDX_GENERAL_PART(false, true); else TDX_GENERAL_PART(false, false); }
+         if (attr.need(g->device)) { CUDA_TRY(cudaFuncSetAttribute(tdx::k_general_part<8, PV, UN, FU>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024)); attr.set(g->device); } \
+         tdx::k_general_part<8, PV, UN, FU><<<grid, block, smem, st>>>(G); } while (0)
+#define TDX_GENERAL_PART2(PV, UN) do { if (full) TDX_GENERAL_PART(PV, UN, true); else TDX_GENERAL_PART(PV, UN, false); } while (0)
+    if (pv_part) { if (unit) TDX_GENERAL_PART2(true, true); else TDX_GENERAL_PART2(true, false); }
+    else { if (unit) TDX_GENERAL_PART2(false, true); else TDX_GENERAL_PART2(false, false); }
+#undef TDX_GENERAL_PART2
 #undef TDX_GENERAL_PART
     LAUNCH_CHECK("k_general_part");
-    note_launch("k_general_part<%d,%d,%d>", 8, pivoting ? 1 : 0, unit ? 1 : 0, 0, 0, 0, grid, block);
+    note_launch("k_general_part<%d,%d,%d,%d>", 8, pv_part ? 1 : 0, unit ? 1 : 0, full ? 1 : 0, 0, 0, grid, block);
     // the lines whose blocks were numerically singular: one thread per line (none on weakly dominant systems)
     dim3 fgrid((unsigned)(g->sms * 4));
     if (pivoting) tdx::k_general_lines<true, true, false><<<fgrid, 128, 0, st>>>(G, bm, flag, qv, dv);

@@ -56,10 +56,17 @@ struct GeneralArgs {
 // its reduced system is as ill-conditioned as the line), or else when the componentwise backward error of what was computed,
 // max_j |a_j x_{j-1} + b_j x_j + c_j x_{j+1} - d_j| / (|a_j x_{j-1}| + |b_j x_j| + |c_j x_{j+1}| + |d_j|), stays below this
 // (a few roundings of a stable elimination; the forward error is then within cond(A) times it, whatever happened inside)
+// Register budgets (measured on cfg5): pivoted blocks 128; plain elimination 96 for strided lines (two CTAs of
+// 8 lines x 36 partitions per SM: y 8.0 -> 7.05 ms against 112 / 128 registers) and 112 for x lines (one 512-thread CTA either way).
 constexpr double kGeneralBackwardError = 128.0 * 2.220446049250313e-16;
 
-template <int M, bool PIVOT, bool UNIT>
-__global__ void __maxnreg__(M <= 8 ? 128 : 168)
+// FULL: every partition has exactly M rows (n = P * M): the ragged-partition selects and padding rows compile away.
+// PIVOT = false is also the OPTIMISTIC first pass of a pivoting solve (tdx.cu): plain elimination, and a block counts as
+// tame only if its LU factors are componentwise stable -- |L||U| <= 4|A|, which for a tridiagonal block is one test per row,
+// |m_j c_{j-1}| + |b'_j| <= 4 |b_j| (the off-diagonal entries of |L||U| equal those of |A|; row- or column-dominant rows give
+// <= 3) -- and its spikes stay <= 1; everything else must pass the backward-error test or goes to the pivoted per-line kernel.
+template <int M, bool PIVOT, bool UNIT, bool FULL>
+__global__ void __maxnreg__(M <= 8 ? (PIVOT ? 128 : (UNIT ? 112 : 96)) : 168)
 k_general_part(GeneralArgs G) {
     extern __shared__ double gs[];
     const int P = G.P;
@@ -70,7 +77,7 @@ k_general_part(GeneralArgs G) {
     const long long l = (long long)blockIdx.x * L + lt;
     const bool valid = l < G.W;
     const int o = blockIdx.y;
-    const int start = part_start(p, G.q, G.r), m = G.q + (p < G.r ? 1 : 0);
+    const int start = FULL ? p * M : part_start(p, G.q, G.r), m = FULL ? M : G.q + (p < G.r ? 1 : 0);
     const long long e0 = (long long)o * G.outer_stride + (valid ? l : 0) * G.lane_stride + (long long)start * G.row_stride;
     const double kappa = 0.6180339887498949;
 
@@ -105,7 +112,7 @@ k_general_part(GeneralArgs G) {
     // padding rows behind the last real row must carry w_last like xt_last and v_last: wpad = what the elimination of row
     // m-1 hands to row m.  Where no lane of the warp starts a 2x2 pivot the whole warp skips that code (warp-uniform branch).
     unsigned fl = 0;
-    bool second = false;
+    bool second = false, wild = false;
     double wpad = 0.0;
 #pragma unroll
     for (int jj = 0; jj < M - 1; ++jj) {
@@ -123,6 +130,8 @@ k_general_part(GeneralArgs G) {
             const double ib = 1.0 / b0, mlt = a1 * ib;
             B_[jj] = ib;
             B_[jj + 1] = fma(-mlt, c0, b1);
+            // componentwise stability of the plain LU: |L||U| <= 4|A| (off the diagonal |L||U| = |A| exactly; NaN counts as wild)
+            if (!PIVOT && !(fabs(mlt * c0) + fabs(B_[jj + 1]) <= 4.0 * fabs(b1))) wild = true;
             D_[jj + 1] = fma(-mlt, D_[jj], D_[jj + 1]);
             F_[jj + 1] = fma(-mlt, F_[jj], F_[jj + 1]);
             if (jj == m - 1) wpad = clast * ib;
@@ -175,7 +184,7 @@ k_general_part(GeneralArgs G) {
     }
     // A block that behaved like a diagonally dominant one -- 1x1 pivots only, spikes not above 1 (the
     // paper's systems) -- is the case the partition method is stable for: its lines are accepted as they are.
-    const bool tame = (fl == 0u) && (growth <= 1.0 + 1e-9);
+    const bool tame = (fl == 0u) && !wild && (growth <= 1.0 + 1e-9);
     const double xl = D_[M - 1], vl = F_[M - 1], wl = A_[M - 1];        // padding rows carried the last real row here
     const double xf = D_[0], vf = F_[0], wf = A_[0];
 

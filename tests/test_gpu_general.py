@@ -30,12 +30,12 @@ def _setup(nx, ny, nz, seed, diag_scale):
     return grid, a, b, c, d
 
 
-def _solve(grid, direction, pivoting, a, b, c, d, cyclic=False, method=tdx.GENERAL_FORCE_PARTITION):
+def _solve(grid, direction, pivoting, a, b, c, d, cyclic=False, method=tdx.GENERAL_FORCE_PARTITION, pivot_partitions=False):
     """method: the partition kernel is forced wherever it applies (it is the default only for x lines), so that it is the
     path under test; periodic lines and very short lines take the per-line kernel whatever is asked."""
     n = d.shape[AXIS[direction]]
     P = max(2, -(-n // 8))
-    pivoting = int(pivoting) | (method if (not cyclic and n // P >= 2 and P <= 512) else 0)
+    pivoting = int(pivoting) | (method if (not cyclic and n // P >= 2 and P <= 512) else 0) | (tdx.GENERAL_PIVOT_PARTITIONS if pivot_partitions else 0)
     ta, tb, tc = (torch.from_numpy(v).cuda() for v in (a, b, c))
     td = torch.from_numpy(d).cuda()
     work = torch.empty(25 * d.size + 64, dtype=torch.uint8, device="cuda")
@@ -45,16 +45,19 @@ def _solve(grid, direction, pivoting, a, b, c, d, cyclic=False, method=tdx.GENER
     return td.cpu().numpy()
 
 
+@pytest.mark.parametrize("pivot_partitions", [False, True])       # optimistic plain elimination first / pivots inside the partitions
 @pytest.mark.parametrize("cyclic", [False, True])
 @pytest.mark.parametrize("direction,shape", [(1, (150, 48, 6)), (2, (34, 5, 40)), (1, (4, 2, 3)), (1, (5, 3, 2)), (2, (130, 1 + 1, 1 + 2)),
                                              (0, (64, 9, 7)), (0, (203, 5, 3)), (0, (9, 4, 4)), (1, (32, 288, 2)), (1, (17, 101, 3))])
-def test_non_dominant_random_systems_with_pivoting(direction, shape, cyclic):
+def test_non_dominant_random_systems_with_pivoting(direction, shape, cyclic, pivot_partitions):
     nx, ny, nz = shape
     grid, a, b, c, d = _setup(nx, ny, nz, 700 + nx, 0.3)
     axis = AXIS[direction]
     if cyclic and d.shape[axis] < 3:
         pytest.skip("periodic lines need n >= 3")
-    got = _solve(grid, direction, True, a, b, c, d, cyclic)
+    if cyclic and pivot_partitions:
+        pytest.skip("periodic lines take the per-line kernel either way")
+    got = _solve(grid, direction, True, a, b, c, d, cyclic, pivot_partitions=pivot_partitions)
     ref, A = ogen.general_solve(a, b, c, d, axis, cyclic)
     cond = np.linalg.cond(A)
     n = d.shape[axis]
@@ -104,8 +107,8 @@ def test_weakly_dominant_per_line_systems_take_the_partition_path_only(direction
     lines = _solve(grid, direction, True, a, b, c, d, method=tdx.GENERAL_FORCE_LINES)   # the other method: same answer to the gate
     errl = np.max(np.abs(np.moveaxis(lines - ref, axis, -1).reshape(-1, n)), axis=1)
     assert np.all(errl <= 50 * cond * EPS * scale)
-    dflt = _solve(grid, direction, True, a, b, c, d, method=0)                     # default: partition for x, lines for y / z
-    assert np.array_equal(dflt, got if direction == 0 else lines)
+    dflt = _solve(grid, direction, True, a, b, c, d, method=0)                     # default: the partition method in every direction
+    assert np.array_equal(dflt, got)
     grid.close()
 
 
@@ -118,6 +121,8 @@ def test_zero_diagonals_need_the_2x2_pivots():
     got = _solve(grid, 1, True, a, b, c, d)
     ref, A = ogen.general_solve(a, b, c, d, 1)
     cond = np.linalg.cond(A)
+    got_pp = _solve(grid, 1, True, a, b, c, d, pivot_partitions=True)
+    assert np.all(np.max(np.abs(np.moveaxis(got_pp - ref, 1, -1).reshape(-1, ny)), axis=1) <= 50 * cond * EPS * np.max(np.abs(np.moveaxis(ref, 1, -1).reshape(-1, ny)), axis=1))
     err = np.max(np.abs(np.moveaxis(got - ref, 1, -1).reshape(-1, ny)), axis=1)
     scale = np.max(np.abs(np.moveaxis(ref, 1, -1).reshape(-1, ny)), axis=1)
     assert np.all(err <= 50 * cond * EPS * scale)
