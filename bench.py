@@ -714,8 +714,8 @@ def run_psweep(args):
     field0 = torch.from_numpy(cfg.rhs_field()).cuda()
     rng = np.random.default_rng(7)
     ns = 48
-    print("| dir | mode | P | rows/partition | ms | GB/s | PDD dropped bound | rel. error of %d sampled lines vs oracle |" % ns)
-    print("|---|---|---|---|---|---|---|---|")
+    print("| dir | mode | P | rows/partition | ms | GB/s | PDD dropped bound | rel. error of %d sampled lines vs oracle | launch |" % ns)
+    print("|---|---|---|---|---|---|---|---|---|")
     for d, name in enumerate("xyz"):
         n = (cfg.nx, cfg.ny, cfg.nz)[d]
         dims = {0: (cfg.nz, cfg.ny), 1: (cfg.nz, cfg.nx), 2: (cfg.ny, cfg.nx)}[d]
@@ -742,9 +742,9 @@ def run_psweep(args):
                     e1.record(); torch.cuda.synchronize()
                     ms = e0.elapsed_time(e1) / 10
                     drop = grid.pdd_dropped_bound(d, P, cfg.alpha)
-                    print("| %s | %s | %d | %d | %.3f | %.0f | %.1e | %.1e |" % (name, mode_name, P, -(-n // P), ms, BYTES_PER_POINT * cfg.npts / ms / 1e6, drop, err))
+                    print("| %s | %s | %d | %d | %.3f | %.0f | %.1e | %.1e | `%s` |" % (name, mode_name, P, -(-n // P), ms, BYTES_PER_POINT * cfg.npts / ms / 1e6, drop, err, tdx.last_launch()))
                 except tdx.TdxError as e:
-                    print("| %s | %s | %d | %d | - | - | - | %s |" % (name, mode_name, P, -(-n // P), tdx.status_string(e.status)))
+                    print("| %s | %s | %d | %d | - | - | - | %s | - |" % (name, mode_name, P, -(-n // P), tdx.status_string(e.status)))
     grid.close()
 
 

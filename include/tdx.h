@@ -82,7 +82,10 @@ tdx_status_t tdx_partition_bounds(int n, int P, int* starts);
  * Delta A (L78-91), i.e. P interfaces and a cyclic reduced system Z -- Woodbury, Eq.(3)-(4): exact for PPT, and PDD deletes
  * the far spike ends of every partition (reading A16: an approximation already at P = 2).
  * rhs_inout: DEVICE, nx*ny*nz doubles.  P: partitions per line (ignored for THOMAS), 1 <= P <= TDX_MAX_P,
- * floor(n_dir / P) >= 2, any partition length (see TDX_MAX_ROWS_PER_PARTITION).                           */
+ * floor(n_dir / P) >= 2, any partition length (see TDX_MAX_ROWS_PER_PARTITION).  In PDD the result depends on P (the
+ * dropped couplings) and the caller's partition map is used as given; in PPT it does not, and the library
+ * may run with coarser partitions than asked for: fewer than 8 rows per partition are merged pairwise up to 8, x lines whose
+ * partition length the bulk-copy kernel cannot take are cut into 16-row ones (tdx_last_launch shows the shape used).  */
 tdx_status_t tdx_adi_sweep(tdx_grid_t* grid, tdx_dir_t dir, tdx_mode_t mode, int P,
                            double alpha, double* rhs_inout, void* stream);
 

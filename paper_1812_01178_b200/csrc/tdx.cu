@@ -414,6 +414,11 @@ tdx_status_t get_plan(tdx_grid* g, int kind, int dir, int mode, int P, double al
     if (!thomas && mode == TDX_MODE_PPT && dir == 0 && kind != KIND_HELM && !x_shape_is_fast(n, P))
         for (int target : {16, 8, 32})
             if (n % target == 0 && n / target >= 2 && n / target <= TDX_MAX_P) { P = n / target; break; }
+    // Likewise short partitions in any direction: below 8 rows per thread the interface exchange, the reduced system and the
+    // per-row table loads outweigh the two recurrences (cfg3, P = 64, 4 rows: 3.2-3.6 TB/s against 5.5 at P = 32), and in PPT
+    // nothing but speed depends on P -- so neighbouring partitions are merged pairwise until a thread has 8 rows.
+    if (!thomas && mode == TDX_MODE_PPT)
+        while (n / P < 8 && P >= 4) P = (P + 1) / 2;
     const bool periodic = (kind == KIND_USER) || (kind == KIND_ADI && g->bc[dir] == TDX_BC_PERIODIC);
     if (periodic && n < 3) return fail(TDX_ERR_INVALID_ARG, "periodic line needs n >= 3");
     // Long partitions (more rows than a thread keeps in registers, or a shape the fast kernels do not take): every partition is

@@ -74,6 +74,42 @@ def test_long_partitions_every_element(direction, n, P, mode_name, alpha):
     grid.close()
 
 
+# (direction, n, P): 4-, 3-, 2-row and ragged 5/4-row partitions
+SHORT_CASES = [(1, 256, 64), (2, 256, 64), (1, 96, 32), (2, 64, 32), (1, 150, 33), (2, 127, 42), (0, 128, 32), (0, 90, 30)]
+
+
+@pytest.mark.parametrize("direction,n,P", SHORT_CASES)
+@pytest.mark.parametrize("alpha", [1e-6, 1e-3])
+def test_short_partitions_ppt_merges_them_pdd_keeps_the_callers_map(direction, n, P, alpha):
+    """Fewer than 8 rows per partition: PPT (exact for any partitioning) runs with neighbouring partitions
+    merged pairwise until a thread has 8 rows -- the launch shows fewer partitions, the result is the exact
+    solution; PDD depends on P, keeps the caller's map and equals the oracle's PDD with that P."""
+    (nx, ny, nz), faces = grid_for(direction, n, other=(16, 10))
+    grid = tdx.Grid(nx, ny, nz, *faces, bcs=BCS)
+    field = inputs.rhs_uniform((nz, ny, nx), 23 + n + P)
+    exact = orc.adi_sweep(field.copy(), *faces, BCS, direction, orc.MODE_THOMAS, 1, alpha)
+    tol = 1e-12 if alpha < 1e-4 else 1e-11
+    t = torch.from_numpy(field).cuda()
+    grid.adi_sweep(direction, tdx.MODE_PPT, P, alpha, t)
+    torch.cuda.synchronize()
+    assert relerr(t.cpu().numpy(), exact) < tol, (direction, n, P, alpha, relerr(t.cpu().numpy(), exact))
+    Pm = P
+    while n // Pm < 8 and Pm >= 4:
+        Pm = (Pm + 1) // 2
+    launch = tdx.last_launch()
+    if direction != 0:                                           # strided kernels: block = (lines, partitions)
+        assert "block=(" in launch and launch.split("block=(")[1].split(",")[1] == str(Pm), (launch, Pm)
+    t = torch.from_numpy(field).cuda()
+    grid.adi_sweep(direction, tdx.MODE_PDD, P, alpha, t)
+    torch.cuda.synchronize()
+    ref = orc.adi_sweep(field.copy(), *faces, BCS, direction, orc.MODE_PDD, P, alpha)
+    assert relerr(t.cpu().numpy(), ref) < tol, ("pdd", direction, n, P, alpha, relerr(t.cpu().numpy(), ref))
+    if direction != 0 and dropped_of(faces, direction, P, alpha) >= 1e-20:
+        launch = tdx.last_launch()
+        assert launch.split("block=(")[1].split(",")[1] == str(P), (launch, P)
+    grid.close()
+
+
 def test_long_partition_pdd_is_the_callers_pdd_not_the_sub_partitions():
     """alpha = 1e-3 on 400 uniform rows: PDD with P = 4 (100 rows) deletes couplings of a few 1e-4; PDD with the 16
     sub-partitions the kernel runs would delete O(0.1) ones.  The result must be the former."""
