@@ -1622,7 +1622,7 @@ static tdx_status_t general_solve_impl(tdx_grid_t* g, tdx_dir_t dir, int pivotin
     const bool part = can_part && method != TDX_GENERAL_FORCE_LINES;
     if (!part) {                                                                         // one thread per line over the whole line
         dim3 block(128), grid((unsigned)std::min<long long>((G.W + 127) / 128, 1 << 20), (unsigned)O);
-        G.fb_count = nullptr; G.fb_lines = nullptr; G.fb_cap = 0; G.P = 1; G.q = n; G.r = 0;
+        G.fb_count = nullptr; G.fb_lines = nullptr; G.fb_flag = nullptr; G.fb_cap = 0; G.P = 1; G.q = n; G.r = 0;
         if (periodic) { if (pivoting) tdx::k_general_lines<true, false, true><<<grid, block, 0, st>>>(G, bm, flag, qv, dv); else tdx::k_general_lines<false, false, true><<<grid, block, 0, st>>>(G, bm, flag, qv, dv); }
         else { if (pivoting) tdx::k_general_lines<true, false, false><<<grid, block, 0, st>>>(G, bm, flag, qv, dv); else tdx::k_general_lines<false, false, false><<<grid, block, 0, st>>>(G, bm, flag, qv, dv); }
         LAUNCH_CHECK("k_general_lines");
@@ -1634,13 +1634,15 @@ static tdx_status_t general_solve_impl(tdx_grid_t* g, tdx_dir_t dir, int pivotin
         std::lock_guard<std::mutex> lk(g->mu);
         if (g->fb_cap < nlines) {
             cudaFree(g->fb); g->fb = nullptr; g->fb_cap = 0;
-            if (cudaMalloc(&g->fb, ((size_t)nlines + 4) * 4) != cudaSuccess) { cudaGetLastError(); return fail(TDX_ERR_ALLOC, "fallback list allocation failed"); }
+            if (cudaMalloc(&g->fb, ((size_t)nlines + 4) * 4 + (size_t)nlines + 16) != cudaSuccess) { cudaGetLastError(); return fail(TDX_ERR_ALLOC, "fallback list allocation failed"); }
             g->fb_cap = nlines;
         }
     }
     G.fb_count = g->fb; G.fb_lines = g->fb + 4; G.fb_cap = nlines;
+    G.fb_flag = reinterpret_cast<unsigned char*>(g->fb + 4 + (size_t)g->fb_cap);       // after the list (allocated capacity)
     G.P = P; G.q = n / P; G.r = n % P;
     CUDA_TRY(cudaMemsetAsync(g->fb, 0, 4, st));
+    CUDA_TRY(cudaMemsetAsync(G.fb_flag, 0, nlines, st));
     const bool unit = dir == TDX_DIR_X;
     // lines per CTA: small CTAs (several resident per SM at different phases: load / eliminate / reduce / store) beat one
     // large one; x lines: whole lines of P consecutive lanes.  TDX_GENERAL_LINES (measurement knob) overrides.
@@ -1668,7 +1670,7 @@ static tdx_status_t general_solve_impl(tdx_grid_t* g, tdx_dir_t dir, int pivotin
     LAUNCH_CHECK("k_general_part");
     note_launch("k_general_part<%d,%d,%d,%d>", 8, pv_part ? 1 : 0, unit ? 1 : 0, full ? 1 : 0, 0, 0, grid, block);
     // the lines whose blocks were numerically singular: one thread per line (none on weakly dominant systems)
-    dim3 fgrid((unsigned)(g->sms * 4));
+    dim3 fgrid((unsigned)(g->sms * 8));                                                  // 62 registers: 8 CTAs of 128 threads per SM
     if (pivoting) tdx::k_general_lines<true, true, false><<<fgrid, 128, 0, st>>>(G, bm, flag, qv, dv);
     else tdx::k_general_lines<false, true, false><<<fgrid, 128, 0, st>>>(G, bm, flag, qv, dv);
     LAUNCH_CHECK("k_general_lines");

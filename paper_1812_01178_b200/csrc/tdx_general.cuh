@@ -49,6 +49,7 @@ struct GeneralArgs {
     unsigned int* fb_count;              // number of lines that fell back
     unsigned int* fb_lines;              // their indices o * W + l
     unsigned int fb_cap;
+    unsigned char* fb_flag;              // the same lines as one byte per line (1 = fell back): for the dense case, see k_general_lines
 };
 
 // A line is accepted when every block was "tame" (1x1 pivots only, spikes <= 1: what a diagonally dominant block does -- the
@@ -273,6 +274,7 @@ k_general_part(GeneralArgs G) {
         if (p == 0 && valid) {
             const unsigned slot = atomicAdd(G.fb_count, 1u);
             if (slot < G.fb_cap) G.fb_lines[slot] = (unsigned)((long long)o * G.W + l);
+            G.fb_flag[(long long)o * G.W + l] = 1;
         }
         return;                                                         // nothing of this line is written: k_general_lines solves it
     }
@@ -299,11 +301,20 @@ __global__ void __launch_bounds__(128) k_general_lines(GeneralArgs G, double* __
     const double kappa = 0.6180339887498949;
     const int n = G.n;
     const long long rs = G.row_stride;
-    const long long cnt = LIST ? (long long)min(*G.fb_count, G.fb_cap) : G.W;
+    // LIST: few listed lines are taken from the list (their threads read lines far apart: about three times the cost per line
+    // of neighbouring lines); when more than a third of all lines are listed, every line is visited in memory order instead
+    // and the accepted ones skipped (one flag byte per line), so the worst case costs what the kernel costs over all lines.
+    const long long listed = LIST ? (long long)min(*G.fb_count, G.fb_cap) : 0;
+    const bool dense = LIST && listed * 3 > (long long)G.fb_cap;
+    const long long cnt = LIST ? (dense ? (long long)G.fb_cap : listed) : G.W;
     double* const rhs = CYC ? dv : G.d;                                 // where the modified right-hand side / y lives
     for (long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x; s < cnt; s += (long long)gridDim.x * blockDim.x) {
         long long o, l;
-        if (LIST) { const unsigned id = G.fb_lines[s]; o = id / G.W; l = id - o * G.W; }
+        if (LIST) {
+            const unsigned id = dense ? (unsigned)s : G.fb_lines[s];
+            if (dense && G.fb_flag[id] == 0) continue;
+            o = id / G.W; l = id - o * G.W;
+        }
         else { o = blockIdx.y; l = s; }
         const long long base = o * G.outer_stride + l * G.lane_stride;
         const long long qe = base + (long long)(n - 1) * rs;              // last row

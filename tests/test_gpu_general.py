@@ -112,6 +112,40 @@ def test_weakly_dominant_per_line_systems_take_the_partition_path_only(direction
     grid.close()
 
 
+@pytest.mark.parametrize("direction", [0, 1, 2])
+@pytest.mark.parametrize("share", [0.06, 0.6])
+def test_mixed_lines_only_the_lines_that_need_pivots_are_re_solved(direction, share):
+    """Dominant lines with a share of lines in between whose every second diagonal entry is exactly zero (plain elimination
+    divides by zero there; the 2x2 pivots solve them).  The re-solve of the lines the partition kernel does not vouch for has
+    two forms (k_general_lines: from the list when they are few, every line in memory order with the accepted ones skipped
+    when they are more than a third): both must leave the accepted lines alone and solve the others to the gate, and the
+    count of re-solved lines is exactly the number of zero-diagonal lines."""
+    nx, ny, nz = {0: (64, 24, 20), 1: (40, 64, 12), 2: (24, 20, 64)}[direction]
+    grid, a, b, c, d = _setup(nx, ny, nz, 950 + direction, 1.0)
+    axis = AXIS[direction]
+    n = d.shape[axis]
+    a = np.sign(a) * (0.5 + np.abs(a)); c = np.sign(c) * (0.5 + np.abs(c))          # couplings bounded away from zero
+    pick = inputs.uniform_pm1(77, d.size // n, stream=5)                            # one draw per line
+    shape = list(d.shape); shape[axis] = 1
+    wild = np.broadcast_to((0.5 * (pick + 1.0) < share).reshape(shape), d.shape)
+    nwild = int(wild.sum()) // n
+    assert 0 < nwild < d.size // n
+    odd = np.zeros(n, dtype=bool); odd[::2] = True
+    shp = [1, 1, 1]; shp[axis] = n
+    bz = np.where(odd.reshape(shp), 0.0, b)                                          # zero on every second row
+    b = np.where(wild, bz, np.abs(a) + np.abs(c) + 0.5 + np.abs(b))
+    got = _solve(grid, direction, True, a, b, c, d)
+    nfb = grid.general_fallback_count()
+    assert nfb == nwild, (nfb, nwild)
+    assert (nfb * 3 > d.size // n) == (share > 0.5), (nfb, d.size // n)              # the branch this case is meant to take
+    ref, A = ogen.general_solve(a, b, c, d, axis)
+    cond = np.linalg.cond(A)
+    err = np.max(np.abs(np.moveaxis(got - ref, axis, -1).reshape(-1, n)), axis=1)
+    scale = np.max(np.abs(np.moveaxis(ref, axis, -1).reshape(-1, n)), axis=1)
+    assert np.all(err <= 50 * cond * EPS * scale), float(np.max(err / (cond * EPS * scale)))
+    grid.close()
+
+
 def test_zero_diagonals_need_the_2x2_pivots():
     """Every second diagonal entry is exactly zero: plain Thomas (pivoting = 0) breaks down, the pivoting solve is exact."""
     nx, ny, nz = 64, 40, 3
