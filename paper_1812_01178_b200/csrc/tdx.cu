@@ -1609,7 +1609,7 @@ static tdx_status_t general_solve_impl(tdx_grid_t* g, tdx_dir_t dir, int pivotin
     double* qv = reinterpret_cast<double*>(flag + ((npts + 7) / 8) * 8);                 // periodic only (25 bytes per value in all)
     double* dv = qv + npts;
     // Method: the partition kernel (8 rows per thread, P threads of a line in one CTA) wherever it applies -- measured on cfg5
-    // (DESIGN.md 9f): 7.05 / 9.17 / 11.5 ms along y / z / x against 10.9 / 11.2 / 77 ms for one thread per line -- unless the
+    // (DESIGN.md 9f): 6.63 / 8.9 / 11.5 ms along y / z / x against 10.9 / 11.2 / 77 ms for one thread per line -- unless the
     // caller forces the per-line kernel.
     const int flags_in = pivoting;
     const int method = pivoting & (TDX_GENERAL_FORCE_PARTITION | TDX_GENERAL_FORCE_LINES);
