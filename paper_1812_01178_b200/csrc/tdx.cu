@@ -603,6 +603,7 @@ tdx_status_t run_strided(const Plan& pl, double* data, long long W, long long li
         if (V == 2) { if (pl.cyc) k_thomas_strided<2, true><<<grid, tb, 0, st>>>(A, pl.rows, pl.cyc_tab, pl.n); else k_thomas_strided<2, false><<<grid, tb, 0, st>>>(A, pl.rows, pl.cyc_tab, pl.n); }
         else { if (pl.cyc) k_thomas_strided<1, true><<<grid, tb, 0, st>>>(A, pl.rows, pl.cyc_tab, pl.n); else k_thomas_strided<1, false><<<grid, tb, 0, st>>>(A, pl.rows, pl.cyc_tab, pl.n); }
         LAUNCH_CHECK("k_thomas_strided");
+        note_launch("k_thomas_strided<%d,%d>", V, pl.cyc ? 1 : 0, 0, 0, 0, 0, grid, dim3(tb));
         return TDX_OK;
     }
     // CTA shape: LPC line-vectors x P partitions.  Row segments of 128 bytes (LPC*V = 16 doubles) and small CTAs (several
@@ -791,11 +792,13 @@ int unit_bt(int M) { return M <= 8 ? 1024 : (M <= 24 ? 512 : 256); }
 
 tdx_status_t run_unit(const Plan& pl, double* data, long long nlines, cudaStream_t st) {
     if (pl.thomas) {
-        const int tb = 128;
+        const int tb = 128;                                             // 4 warps of 32 lines each, 33 KB of shared memory
         unsigned grid = (unsigned)((nlines + tb - 1) / tb);
-        if (pl.cyc) k_thomas_unit<true><<<grid, tb, 0, st>>>(data, nlines, pl.rows, pl.cyc_tab, pl.n);
-        else k_thomas_unit<false><<<grid, tb, 0, st>>>(data, nlines, pl.rows, pl.cyc_tab, pl.n);
-        LAUNCH_CHECK("k_thomas_unit");
+        const size_t smem = (size_t)(tb / 32) * 32 * 33 * 8;
+        if (pl.cyc) k_thomas_unit_tiled<true><<<grid, tb, smem, st>>>(data, nlines, pl.rows, pl.cyc_tab, pl.n);
+        else k_thomas_unit_tiled<false><<<grid, tb, smem, st>>>(data, nlines, pl.rows, pl.cyc_tab, pl.n);
+        LAUNCH_CHECK("k_thomas_unit_tiled");
+        note_launch("k_thomas_unit_tiled<%d>", pl.cyc ? 1 : 0, 0, 0, 0, 0, 0, dim3(grid), dim3(tb));
         return TDX_OK;
     }
     {

@@ -11,7 +11,7 @@
 //                          lanes; a warp's 32 partitions are one contiguous chunk of memory which is loaded coalesced,
 //                          transposed through a padded per-warp shared-memory tile, and stored back the same way --
 //                          no global transpose (PAPER.md:L51-74 is what the method removes).
-//   k_thomas_strided / k_thomas_unit   mode THOMAS: one thread per line, plain recurrence, in place (GPU baseline).
+//   k_thomas_strided / k_thomas_unit_tiled   mode THOMAS: one thread per line, plain recurrence, in place (GPU baseline).
 //
 // PAPER.md references: Eq.(5)-(8) L104-124, PDD L148-154, PPT L126-146/L156, Algorithm 1 steps 3,5,7 L240-258.
 #pragma once
@@ -679,27 +679,88 @@ k_helm_lines(double2* __restrict__ data, int nx, int ny, int P, int q, int rq, i
     }
 }
 
+// THOMAS mode along x, warp-tiled: a warp owns 32 consecutive lines and walks them 32 columns at a time.  The 32 x 32 tile comes
+// in with coalesced 256-byte row reads (lane = column), is turned through shared memory (33-double rows: conflict-free both
+// ways) so that lane = line runs its recurrence over the 32 columns, and goes back the same way -- forward pass up the line,
+// backward pass down, and for periodic lines a third, purely elementwise pass (x = y - q s, s per line by shuffle).  The
+// one-thread-per-line form it replaces read 8 useful bytes per 32-byte sector (cfg5 10.8 ms against 3.1 ms for the strided
+// directions); this one moves the same 32 B per value with full sectors.  Shared memory: 32 * 33 doubles per warp.
 template <bool CYC>
-__global__ void k_thomas_unit(double* __restrict__ data, long long nlines, const double* __restrict__ rows,
-                              const double* __restrict__ cyc, int n) {
-    const long long line = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (line >= nlines) return;
-    double* base = data + line * n;
+__global__ void __launch_bounds__(128) k_thomas_unit_tiled(double* __restrict__ data, long long nlines, const double* __restrict__ rows,
+                                                          const double* __restrict__ cyc, int n) {
+    extern __shared__ double tt[];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    double* tile = tt + w * (32 * 33);
+    const long long line0 = ((long long)blockIdx.x * (blockDim.x >> 5) + w) * 32;
+    if (line0 >= nlines) return;
+    const int nl = (int)min((long long)32, nlines - line0);
+    double* base = data + line0 * n;
+    // the tile of the NEXT step is in flight (32 loads per lane, in registers) while the current one is computed
+    double nxt[32];
+    auto fetch = [&](int c0) {
+        const bool in = c0 >= 0 && c0 + lane < n;
+#pragma unroll
+        for (int r = 0; r < 32; ++r) nxt[r] = (in && r < nl) ? base[(long long)r * n + c0 + lane] : 0.0;
+    };
+    auto land = [&]() {
+#pragma unroll
+        for (int r = 0; r < 32; ++r) tile[r * 33 + lane] = nxt[r];
+    };
+    auto put = [&](int c0) {
+        if (c0 + lane < n) {
+#pragma unroll
+            for (int r = 0; r < 32; ++r) if (r < nl) base[(long long)r * n + c0 + lane] = tile[r * 33 + lane];
+        }
+    };
     double prev = 0.0;
-    for (int j = 0; j < n; ++j) {
-        const double cur = fma(-__ldg(rows + (size_t)j * 6 + F_L), prev, base[j]);
-        base[j] = cur; prev = cur;
+    fetch(0);
+    for (int c0 = 0; c0 < n; c0 += 32) {                            // forward: y_j = d_j - l_j y_{j-1}
+        const int nc = min(32, n - c0);
+        land();
+        fetch(c0 + 32 < n ? c0 + 32 : -1);
+        __syncwarp();
+        if (lane < nl) {
+#pragma unroll 8
+            for (int k = 0; k < nc; ++k) {
+                const double cur = fma(-__ldg(rows + (size_t)(c0 + k) * 6 + F_L), prev, tile[lane * 33 + k]);
+                tile[lane * 33 + k] = cur; prev = cur;
+            }
+        }
+        __syncwarp();
+        put(c0);
+        __syncwarp();
     }
     prev = 0.0;
     double ylast = 0.0;
-    for (int j = n - 1; j >= 0; --j) {
-        const double cur = fma(-__ldg(rows + (size_t)j * 6 + F_CP), prev, base[j] * __ldg(rows + (size_t)j * 6 + F_INV));
-        base[j] = cur; prev = cur;
-        if (j == n - 1) ylast = cur;
+    const int clast = ((n - 1) / 32) * 32;
+    // The backward pass re-reads what the forward pass has just written through this same warp: ordinary loads after the
+    // stores of the same thread are ordered, and a lane only reads columns it wrote itself (lane = column in both).
+    fetch(clast);
+    for (int c0 = clast; c0 >= 0; c0 -= 32) {                        // backward: x_j = y_j inv_j - c'_j x_{j+1}
+        const int nc = min(32, n - c0);
+        land();
+        fetch(c0 - 32);
+        __syncwarp();
+        if (lane < nl) {
+#pragma unroll 8
+            for (int k = nc - 1; k >= 0; --k) {
+                const int j = c0 + k;
+                const double cur = fma(-__ldg(rows + (size_t)j * 6 + F_CP), prev, tile[lane * 33 + k] * __ldg(rows + (size_t)j * 6 + F_INV));
+                tile[lane * 33 + k] = cur; prev = cur;
+                if (j == n - 1) ylast = cur;
+            }
+        }
+        __syncwarp();
+        put(c0);                                                     // (periodic lines: y, the closure needs all of it first)
+        __syncwarp();
     }
-    if (CYC) {
-        const double s = __ldg(cyc + 3) * fma(__ldg(cyc + 0), ylast, prev);
-        for (int j = 0; j < n; ++j) base[j] = fma(-__ldg(rows + (size_t)j * 6 + F_Q), s, base[j]);
+    if (CYC) {                                                       // x = y - q (y_0 + g y_{n-1}) kappa   (Sherman-Morrison, Eq.(3))
+        const double s = __ldg(cyc + 3) * fma(__ldg(cyc + 0), ylast, prev);     // prev = y_0 of this lane's line
+        for (int r = 0; r < nl; ++r) {
+            const double sr = __shfl_sync(0xffffffffu, s, r);
+            double* row = base + (long long)r * n;
+            for (int j = lane; j < n; j += 32) row[j] = fma(-__ldg(rows + (size_t)j * 6 + F_Q), sr, row[j]);
+        }
     }
 }
 

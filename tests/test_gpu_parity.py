@@ -187,6 +187,22 @@ def test_other_boundary_conditions(bcs, mode_name):
     grid.close()
 
 
+@pytest.mark.parametrize("bcx", [tdx.BC_DIRICHLET, tdx.BC_PERIODIC, tdx.BC_NEUMANN])
+@pytest.mark.parametrize("nx,ny,nz", [(33, 5, 3), (64, 8, 8), (100, 7, 11), (7, 9, 5), (32, 4, 8), (257, 6, 6), (31, 13, 5)])
+def test_thomas_along_x_warp_tiles(bcx, nx, ny, nz):
+    """THOMAS mode along x walks 32 lines x 32 columns per warp through shared memory (k_thomas_unit_tiled): line counts that
+    are not multiples of 32 (15, 77, 45, 65 lines), line lengths below, at and across the 32-column tile, last tiles of
+    1 and 31 columns; Dirichlet, Neumann and periodic (third pass) ends.  Stretched x so that every row has its own table
+    entry."""
+    faces = (inputs.faces_tanh_two_sided(nx, 1.2), inputs.faces_uniform(ny, 1.0), inputs.faces_uniform(nz, 1.0))
+    bcs = (bcx, tdx.BC_DIRICHLET, tdx.BC_PERIODIC)
+    grid = tdx.Grid(nx, ny, nz, *faces, bcs=bcs)
+    field = inputs.rhs_uniform((nz, ny, nx), 31 + nx)
+    check_sweep(grid, faces, bcs, field, 0, "thomas", 1, 3e-4)
+    assert tdx.last_launch().startswith("k_thomas_unit_tiled<%d>" % (1 if bcx == tdx.BC_PERIODIC else 0))
+    grid.close()
+
+
 @pytest.mark.parametrize("nx,ny,nz,P", [(64, 48, 40, 2), (96, 16, 16, 12), (256, 8, 8, 64), (512, 6, 6, 8), (40, 36, 200, 25)])
 def test_tile_and_partition_extremes(nx, ny, nz, P):
     """P=2 (no uniform table), many short partitions, 64-row partitions, lines spanning several warps."""
