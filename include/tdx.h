@@ -264,6 +264,20 @@ tdx_status_t tdx_helmholtz_wavenumber_solve_host(tdx_grid_t* grid, tdx_mode_t mo
 tdx_status_t tdx_step_host(tdx_grid_t* grid, tdx_mode_t mode, int Px, int Py, int Pz, double alpha, double* host_field,
                            int Ph, int nm, const double* kz2, double* host_helm);
 
+/* The same step, enqueued only: returns as soon as its copies and kernels are in the three pipeline streams; the results are
+ * in the host buffers once tdx_step_host_wait(grid, slot) has returned TDX_OK.  Two steps may be in flight, one per slot
+ * (slot in {0, 1}; each slot has its own device staging, so the grid then holds two fields and two Helmholtz arrays).  One
+ * call alone cannot beat three transfer times (the field must be up completely before any of it comes down -- the z sweep
+ * needs every plane -- and the Helmholtz array shares the link with it); with two steps in flight the download of one
+ * runs beside the upload of the next and the pair of PCIe directions stays busy: two transfer times per step.  The host
+ * buffers of a slot must not be touched between the call and its wait; they must be page-locked for the call to be
+ * asynchronous at all.  A slot that still holds a step returns TDX_ERR_INVALID_ARG; tdx_step_host is slot 0 followed by
+ * its wait; the other *_host entry points wait for slot 0 first (they share its staging).  Calls on one grid from one
+ * host thread at a time. */
+tdx_status_t tdx_step_host_async(tdx_grid_t* grid, int slot, tdx_mode_t mode, int Px, int Py, int Pz, double alpha,
+                                 double* host_field, int Ph, int nm, const double* kz2, double* host_helm);
+tdx_status_t tdx_step_host_wait(tdx_grid_t* grid, int slot);
+
 /* Diagnostics.  tdx_pdd_dropped_bound: max over interfaces of |v_last|, |w_first| for the ADI operator of
  * (dir, P, alpha) -- the entries PDD deletes from Z; the a-priori size of the PDD error.  */
 tdx_status_t tdx_pdd_dropped_bound(tdx_grid_t* grid, tdx_dir_t dir, int P, double alpha, double* out);

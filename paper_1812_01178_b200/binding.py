@@ -19,7 +19,7 @@ OK, ERR_INVALID_ARG, ERR_BAD_PARTITION, ERR_ALLOC, ERR_CUDA, ERR_UNSUPPORTED, ER
 
 EXPORTS = ("tdx_grid_create", "tdx_grid_destroy", "tdx_grid_set_pdd_strict", "tdx_partition_bounds", "tdx_adi_sweep", "tdx_adi_sweep_at", "tdx_adi_step",
            "tdx_helmholtz_wavenumber_solve", "tdx_dct_x", "tdx_rfft_z", "tdx_irfft_z", "tdx_poisson_solve", "tdx_static_scratch_setup", "tdx_helmholtz_thomas_lines_static", "tdx_general_solve", "tdx_general_cyclic_solve", "tdx_general_fallback_count", "tdx_slab_create", "tdx_slab_destroy", "tdx_slab_eliminate", "tdx_slab_correct", "tdx_slab_dropped_bound", "tdx_cyclic_solve", "tdx_adi_sweep_host", "tdx_adi_step_host",
-           "tdx_helmholtz_wavenumber_solve_host", "tdx_step_host", "tdx_pdd_dropped_bound", "tdx_kernel_launch_count",
+           "tdx_helmholtz_wavenumber_solve_host", "tdx_step_host", "tdx_step_host_async", "tdx_step_host_wait", "tdx_pdd_dropped_bound", "tdx_kernel_launch_count",
            "tdx_status_string", "tdx_last_error", "tdx_last_launch", "tdx_version")
 
 _dp = C.POINTER(C.c_double)
@@ -60,6 +60,8 @@ def lib():
         L.tdx_adi_step_host.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_double, C.c_void_p]
         L.tdx_helmholtz_wavenumber_solve_host.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, _dp, _dp, C.c_void_p]
         L.tdx_step_host.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_double, C.c_void_p, C.c_int, C.c_int, _dp, C.c_void_p]
+        L.tdx_step_host_async.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_double, C.c_void_p, C.c_int, C.c_int, _dp, C.c_void_p]
+        L.tdx_step_host_wait.argtypes = [C.c_void_p, C.c_int]
         L.tdx_dct_x.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p]
         L.tdx_rfft_z.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.tdx_irfft_z.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
@@ -229,6 +231,16 @@ class Grid:
         pf = _hostptr(host_field, self.nx * self.ny * self.nz * 8) if host_field is not None else None
         ph = _hostptr(host_helm, self.nx * self.ny * kz.size * 16) if host_helm is not None else None
         _chk(lib().tdx_step_host(self._h, mode, Px, Py, Pz, alpha, pf, Ph, kz.size if kz is not None else 0, pkz, ph))
+
+    def step_host_async(self, slot, mode, Px, Py, Pz, alpha, host_field, Ph, kz2, host_helm):
+        """The pipelined step enqueued only (slot 0 or 1); the host buffers are valid after step_host_wait(slot)."""
+        kz, pkz = _host(kz2) if host_helm is not None else (None, None)
+        pf = _hostptr(host_field, self.nx * self.ny * self.nz * 8) if host_field is not None else None
+        ph = _hostptr(host_helm, self.nx * self.ny * kz.size * 16) if host_helm is not None else None
+        _chk(lib().tdx_step_host_async(self._h, slot, mode, Px, Py, Pz, alpha, pf, Ph, kz.size if kz is not None else 0, pkz, ph))
+
+    def step_host_wait(self, slot):
+        _chk(lib().tdx_step_host_wait(self._h, slot))
 
     def pdd_dropped_bound(self, direction, P, alpha):
         out = C.c_double(0.0)

@@ -141,6 +141,13 @@ struct tdx_grid {
     bool attr_helm_lines = false;                       // cudaFuncSetAttribute done for this grid's device
     unsigned int* fb = nullptr; unsigned fb_cap = 0;    // tdx_general_solve: [0] = number of lines that fell back, [4..] = their indices
     double* stage2 = nullptr; size_t stage2_bytes = 0;  // second staging buffer (Helmholtz part of tdx_step_host)
+    // tdx_step_host_async: two slots, each with its own staging pair (slot 0 = stage / stage2 above), the events of the step in
+    // flight and the event that marks its last download
+    double* stage_b = nullptr; size_t stage_b_bytes = 0;
+    double* stage2_b = nullptr; size_t stage2_b_bytes = 0;
+    std::vector<cudaEvent_t> slot_evs[2];
+    cudaEvent_t slot_done[2] = {nullptr, nullptr};
+    bool slot_busy[2] = {false, false};
     cudaStream_t s_up = nullptr, s_comp = nullptr, s_down = nullptr;   // pipeline streams of tdx_step_host
     double length[3] = {0, 0, 0};                       // domain length per direction (host copy of faces[n] - faces[0])
     bool uniform[3] = {false, false, false};            // spacing uniform to 1e-12 relative (the transforms need it in x, z)
@@ -1164,6 +1171,12 @@ tdx_status_t tdx_grid_create(int nx, int ny, int nz, const double* xf, const dou
 tdx_status_t tdx_grid_destroy(tdx_grid_t* g) {
     if (!g) return TDX_OK;
     cudaSetDevice(g->device);
+    for (int slot = 0; slot < 2; ++slot)                       // a pipelined step still in flight: let it finish
+        if (g->slot_busy[slot]) {
+            if (g->slot_done[slot]) { cudaEventSynchronize(g->slot_done[slot]); cudaEventDestroy(g->slot_done[slot]); }
+            for (cudaEvent_t ev : g->slot_evs[slot]) if (ev) cudaEventDestroy(ev);
+        }
+    cudaFree(g->stage_b); cudaFree(g->stage2_b);
     for (Plan& p : g->plans) p.release();
     for (int d = 0; d < 3; ++d) { cudaFree(g->faces[d]); cudaFree(g->lo[d]); cudaFree(g->up[d]); cudaFree(g->lo_face[d]); cudaFree(g->up_face[d]); }
     cudaFree(g->lo_neumann_y); cudaFree(g->up_neumann_y); cudaFree(g->stage); cudaFree(g->stage2); cudaFree(g->ws);
@@ -1713,7 +1726,9 @@ tdx_status_t tdx_pdd_dropped_bound(tdx_grid_t* g, tdx_dir_t dir, int P, double a
 }
 
 // ---- host-buffer entry points (end-to-end: H2D + solve + D2H, synchronous) ----------------------------------
+static tdx_status_t step_slot_wait(tdx_grid* g, int slot);
 static tdx_status_t ensure_stage(tdx_grid* g, size_t bytes) {
+    if (g->slot_busy[0]) { tdx_status_t rc = step_slot_wait(g, 0); if (rc != TDX_OK) return rc; }   // slot 0 shares this buffer
     if (g->stage_bytes >= bytes) return TDX_OK;
     cudaFree(g->stage); g->stage = nullptr; g->stage_bytes = 0;
     if (cudaMalloc(&g->stage, bytes) != cudaSuccess) { cudaGetLastError(); return fail(TDX_ERR_ALLOC, "staging allocation of %zu bytes failed", bytes); }
@@ -1764,10 +1779,33 @@ tdx_status_t tdx_adi_sweep_host(tdx_grid_t* g, tdx_dir_t dir, tdx_mode_t mode, i
 //   field: z-slabs go up; each slab is swept in x and y as soon as it has arrived; when the last one is in, the z sweep
 //          runs y-slab by y-slab and every finished y-slab goes down (strided 2-D copy) while
 //   helm : the wavenumber slabs go up behind the field, are solved as they arrive and go down behind the field.
-tdx_status_t tdx_step_host(tdx_grid_t* g, tdx_mode_t mode, int Px, int Py, int Pz, double alpha, double* host_field,
-                           int Ph, int nm, const double* kz2, double* host_helm) {
+// Waits for the step in flight in `slot` (if any) and releases its events.
+static tdx_status_t step_slot_wait(tdx_grid* g, int slot) {
+    if (!g->slot_busy[slot]) return TDX_OK;
+    cudaError_t e = g->slot_done[slot] ? cudaEventSynchronize(g->slot_done[slot]) : cudaDeviceSynchronize();
+    for (cudaEvent_t ev : g->slot_evs[slot]) if (ev) cudaEventDestroy(ev);
+    g->slot_evs[slot].clear();
+    if (g->slot_done[slot]) { cudaEventDestroy(g->slot_done[slot]); g->slot_done[slot] = nullptr; }
+    g->slot_busy[slot] = false;
+    if (e != cudaSuccess) return fail(TDX_ERR_CUDA, "pipelined step failed: %s", cudaGetErrorString(e));
+    return TDX_OK;
+}
+
+static tdx_status_t grow(double** p, size_t* have, size_t want) {
+    if (*have >= want) return TDX_OK;
+    cudaFree(*p); *p = nullptr; *have = 0;
+    if (cudaMalloc(p, want) != cudaSuccess) { cudaGetLastError(); return fail(TDX_ERR_ALLOC, "staging allocation of %zu bytes failed", want); }
+    *have = want;
+    return TDX_OK;
+}
+
+// Enqueues one whole step on the three pipeline streams; returns without waiting (tdx_step_host_async).
+static tdx_status_t step_host_enqueue(tdx_grid_t* g, int slot, tdx_mode_t mode, int Px, int Py, int Pz, double alpha, double* host_field,
+                                      int Ph, int nm, const double* kz2, double* host_helm) {
     if (!g) return fail(TDX_ERR_INVALID_ARG, "grid is NULL");
-    trim_plans(g);
+    if (slot < 0 || slot > 1) return fail(TDX_ERR_INVALID_ARG, "slot=%d not in {0,1}", slot);
+    if (g->slot_busy[slot]) return fail(TDX_ERR_INVALID_ARG, "slot %d still holds a step in flight: call tdx_step_host_wait first", slot);
+    if (!g->slot_busy[0] && !g->slot_busy[1]) trim_plans(g);          // never while another step still uses its plans
     if (mode < 0 || mode > 2) return fail(TDX_ERR_INVALID_ARG, "mode=%d not in {0,1,2}", (int)mode);
     if (!host_field && !host_helm) return fail(TDX_ERR_INVALID_ARG, "both host buffers are NULL");
     if (host_helm && (nm < 1 || !kz2)) return fail(TDX_ERR_INVALID_ARG, "nm=%d / kz2 invalid", nm);
@@ -1782,33 +1820,31 @@ tdx_status_t tdx_step_host(tdx_grid_t* g, tdx_mode_t mode, int Px, int Py, int P
     tdx_status_t rc;
     Plan* pls[3] = {nullptr, nullptr, nullptr};
     Plan* plh = nullptr;
+    double** st1 = slot ? &g->stage_b : &g->stage;   size_t* st1b = slot ? &g->stage_b_bytes : &g->stage_bytes;
+    double** st2 = slot ? &g->stage2_b : &g->stage2; size_t* st2b = slot ? &g->stage2_b_bytes : &g->stage2_bytes;
     if (host_field) {
         const int Ps[3] = {Px, Py, Pz};
         for (int d = 0; d < 3; ++d) {                       // validate and build every plan before any copy
             rc = get_sweep_plan(g, KIND_ADI, d, mode, Ps[d], alpha, nullptr, nullptr, nullptr, g->s_comp, &pls[d]);
             if (rc != TDX_OK) return rc;
         }
-        rc = ensure_stage(g, (size_t)nx * ny * nz * 8);
+        rc = grow(st1, st1b, (size_t)nx * ny * nz * 8);
         if (rc != TDX_OK) return rc;
     }
     if (host_helm) {
         rc = get_plan(g, KIND_HELM, TDX_DIR_Y, mode, Ph, 0.0, nm, kz2, nullptr, nullptr, nullptr, g->s_comp, &plh);
         if (rc != TDX_OK) return rc;
-        const size_t hb = (size_t)nx * ny * nm * 16;
-        if (g->stage2_bytes < hb) {
-            cudaFree(g->stage2); g->stage2 = nullptr; g->stage2_bytes = 0;
-            if (cudaMalloc(&g->stage2, hb) != cudaSuccess) { cudaGetLastError(); return fail(TDX_ERR_ALLOC, "staging allocation of %zu bytes failed", hb); }
-            g->stage2_bytes = hb;
-        }
+        rc = grow(st2, st2b, (size_t)nx * ny * nm * 16);
+        if (rc != TDX_OK) return rc;
     }
-    std::vector<cudaEvent_t> evs;
+    std::vector<cudaEvent_t>& evs = g->slot_evs[slot];
     auto new_event = [&]() -> cudaEvent_t { cudaEvent_t e = nullptr; cudaEventCreateWithFlags(&e, cudaEventDisableTiming); evs.push_back(e); return e; };
-    auto cleanup = [&]() { for (cudaEvent_t e : evs) if (e) cudaEventDestroy(e); };
+    auto cleanup = [&]() { for (cudaEvent_t e : evs) if (e) cudaEventDestroy(e); evs.clear(); };
 #define STEP_TRY(expr) do { cudaError_t e_ = (expr); if (e_ != cudaSuccess) { cudaDeviceSynchronize(); cleanup(); return fail(TDX_ERR_CUDA, "%s failed: %s", #expr, cudaGetErrorString(e_)); } } while (0)
 #define STEP_RC(expr) do { rc = (expr); if (rc != TDX_OK) { cudaDeviceSynchronize(); cleanup(); return rc; } } while (0)
     const int kSlabs = 16;
     if (host_field) {
-        double* dev = g->stage;
+        double* dev = *st1;
         const int sz = (int)std::min<long long>(kSlabs, nz);
         for (int s = 0; s < sz; ++s) {                      // z-slabs up; x and y sweeps as they arrive
             const long long k0 = nz * s / sz, k1 = nz * (s + 1) / sz;
@@ -1833,7 +1869,7 @@ tdx_status_t tdx_step_host(tdx_grid_t* g, tdx_mode_t mode, int Px, int Py, int P
         }
     }
     if (host_helm) {
-        double* dev = g->stage2;
+        double* dev = *st2;
         const int sm = std::min(kSlabs, nm);
         for (int s = 0; s < sm; ++s) {
             const long long m0 = (long long)nm * s / sm, m1 = (long long)nm * (s + 1) / sm;
@@ -1850,13 +1886,32 @@ tdx_status_t tdx_step_host(tdx_grid_t* g, tdx_mode_t mode, int Px, int Py, int P
             STEP_TRY(cudaMemcpyAsync(host_helm + off, dev + off, bytes, cudaMemcpyDeviceToHost, g->s_down));
         }
     }
-    STEP_TRY(cudaStreamSynchronize(g->s_down));
-    STEP_TRY(cudaStreamSynchronize(g->s_comp));
-    STEP_TRY(cudaStreamSynchronize(g->s_up));
+    // every copy and kernel of the step precedes its last download in dependency order: one event on the download stream
+    STEP_TRY(cudaEventCreateWithFlags(&g->slot_done[slot], cudaEventDisableTiming));
+    STEP_TRY(cudaEventRecord(g->slot_done[slot], g->s_down));
 #undef STEP_TRY
 #undef STEP_RC
-    cleanup();
+    g->slot_busy[slot] = true;
     return TDX_OK;
+}
+
+tdx_status_t tdx_step_host_async(tdx_grid_t* g, int slot, tdx_mode_t mode, int Px, int Py, int Pz, double alpha, double* host_field,
+                                 int Ph, int nm, const double* kz2, double* host_helm) {
+    return step_host_enqueue(g, slot, mode, Px, Py, Pz, alpha, host_field, Ph, nm, kz2, host_helm);
+}
+
+tdx_status_t tdx_step_host_wait(tdx_grid_t* g, int slot) {
+    if (!g) return fail(TDX_ERR_INVALID_ARG, "grid is NULL");
+    if (slot < 0 || slot > 1) return fail(TDX_ERR_INVALID_ARG, "slot=%d not in {0,1}", slot);
+    CUDA_TRY(cudaSetDevice(g->device));
+    return step_slot_wait(g, slot);
+}
+
+tdx_status_t tdx_step_host(tdx_grid_t* g, tdx_mode_t mode, int Px, int Py, int Pz, double alpha, double* host_field,
+                           int Ph, int nm, const double* kz2, double* host_helm) {
+    tdx_status_t rc = step_host_enqueue(g, 0, mode, Px, Py, Pz, alpha, host_field, Ph, nm, kz2, host_helm);
+    if (rc != TDX_OK) return rc;
+    return step_slot_wait(g, 0);
 }
 
 tdx_status_t tdx_helmholtz_wavenumber_solve_host(tdx_grid_t* g, tdx_mode_t mode, int P, int nm, const double* kx2,

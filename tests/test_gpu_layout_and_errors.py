@@ -178,6 +178,51 @@ def test_pipelined_step_host_equals_device_path_bit_exact():
     grid.close()
 
 
+def test_two_steps_in_flight_equal_the_synchronous_step_bit_exact():
+    """tdx_step_host_async: two steps in flight on two slots (different data), then a third on the first slot again, give
+    exactly what tdx_step_host gives one at a time; a busy slot is refused; the other host entry points wait for slot 0."""
+    nx, ny, nz = 96, 40, 36
+    faces = (inputs.faces_uniform(nx, 2.0), inputs.faces_tanh_two_sided(ny, 2.0), inputs.faces_uniform(nz, 1.0))
+    grid = tdx.Grid(nx, ny, nz, *faces, bcs=BCS)
+    nm = nz // 2 + 1
+    kz2 = inputs.modified_wavenumbers_z(nz, 1.0)
+    alpha = 3e-4
+    args = (tdx.MODE_PPT, 6, 5, 4, alpha)
+    fields = [inputs.rhs_uniform((nz, ny, nx), 50 + k) for k in range(3)]
+    helms = [inputs.rhs_complex_uniform((nm, ny, nx), 60 + k) for k in range(3)]
+    want = []
+    for f, h in zip(fields, helms):
+        hf = torch.from_numpy(f.copy()).pin_memory().numpy(); hh = torch.from_numpy(h.copy()).pin_memory().numpy()
+        grid.step_host(*args, hf, 4, kz2, hh)
+        want.append((hf.copy(), hh.copy()))
+    bufs = [(torch.from_numpy(f.copy()).pin_memory().numpy(), torch.from_numpy(h.copy()).pin_memory().numpy()) for f, h in zip(fields, helms)]
+    grid.step_host_async(0, *args, bufs[0][0], 4, kz2, bufs[0][1])
+    grid.step_host_async(1, *args, bufs[1][0], 4, kz2, bufs[1][1])
+    with pytest.raises(tdx.TdxError) as e:                       # slot 1 holds a step
+        grid.step_host_async(1, *args, bufs[2][0], 4, kz2, bufs[2][1])
+    assert e.value.status == tdx.ERR_INVALID_ARG
+    grid.step_host_wait(0)
+    grid.step_host_async(0, *args, bufs[2][0], 4, kz2, bufs[2][1])    # slot 0 again while slot 1 is still out
+    grid.step_host_wait(1)
+    grid.step_host_wait(0)
+    grid.step_host_wait(0)                                       # an idle slot: nothing to wait for
+    for k in range(3):
+        assert np.array_equal(bufs[k][0], want[k][0]), k
+        assert np.array_equal(bufs[k][1], want[k][1]), k
+    # a step in flight in slot 0, then a synchronous host call that shares its staging: it must wait, both must be right
+    b0 = (torch.from_numpy(fields[0].copy()).pin_memory().numpy(), torch.from_numpy(helms[0].copy()).pin_memory().numpy())
+    grid.step_host_async(0, *args, b0[0], 4, kz2, b0[1])
+    other = fields[1].copy()
+    grid.adi_step_host(tdx.MODE_PPT, 6, 5, 4, alpha, other)
+    grid.step_host_wait(0)
+    assert np.array_equal(b0[0], want[0][0]) and np.array_equal(b0[1], want[0][1])
+    assert np.array_equal(other, want[1][0])
+    with pytest.raises(tdx.TdxError):
+        grid.step_host_wait(2)
+    grid.step_host_async(1, *args, b0[0], 4, kz2, b0[1])         # destroyed with a step in flight: must not crash or leak
+    grid.close()
+
+
 def test_plan_cache_is_bounded_and_rebuilds_evicted_plans(small):
     """A caller that keeps changing alpha (variable time step) must not grow the plan cache without bound, and a plan
     that was dropped is rebuilt to the same bits."""
