@@ -352,6 +352,44 @@ def grid_table(tdx, torch, cfg_no, local_rank, steps, peak):
                 res[name]["dropped_bound"] = bound
                 res[name]["pdd_gate_ok"] = bool(bound <= PDD_GATE)
         out[mname] = res
+    if K > 1 or fbytes < 126e6:
+        # Launch-bound grids: the whole step (x, y, cyclic z, Helmholtz; PPT) of all K copies captured ONCE in a CUDA graph
+        # (the sweeps are plain stream work once their plans exist: no allocation, no synchronisation) and replayed.
+        try:
+            def step(c, st):
+                for d in range(3):
+                    grid.adi_sweep(d, tdx.MODE_PPT, Ps[d], cfg.alpha, fields[c], st)
+                grid.helmholtz_wavenumber_solve(tdx.MODE_PPT, Ps[3], None, kz2, helms[c], st)
+            side = torch.cuda.Stream()
+            side.wait_stream(torch.cuda.current_stream())
+            with torch.cuda.stream(side):
+                for c in range(K):
+                    step(c, side.cuda_stream)
+                side.synchronize()
+                n0 = tdx.kernel_launch_count()
+                cg = torch.cuda.CUDAGraph()
+                with torch.cuda.graph(cg, stream=side):
+                    for c in range(K):
+                        step(c, side.cuda_stream)
+                captured = tdx.kernel_launch_count() - n0
+            torch.cuda.synchronize()
+            for _ in range(3):
+                cg.replay()
+            R = 50
+            helms.copy_(h0.unsqueeze(0).expand_as(helms))
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            e0.record()
+            for _ in range(R):
+                cg.replay()
+            e1.record()
+            torch.cuda.synchronize()
+            eager = sum(out["ppt"][n]["ms"] for n in names)
+            out["step_cuda_graph"] = {"ms_per_step": e0.elapsed_time(e1) / (R * K), "eager_ms_per_step": eager, "kernels_in_graph": int(captured),
+                                      "what": "x + y + cyclic z + Helmholtz (PPT) of the %d rotated copies captured in one CUDA graph, %d replays" % (K, R)}
+            del cg
+        except Exception as exc:                                 # an extra figure must never take the table down
+            out["step_cuda_graph"] = {"error": repr(exc)[:300]}
     grid.close()
     del fields, helms, f0, h0
     return out

@@ -178,6 +178,56 @@ def test_pipelined_step_host_equals_device_path_bit_exact():
     grid.close()
 
 
+def test_step_is_capturable_in_a_cuda_graph_and_replays_bit_exact():
+    """Once their plans exist the sweeps are plain stream work (no allocation, no synchronisation): x, y, cyclic z and the
+    Helmholtz solve are captured in one CUDA graph on a side stream and the replay gives the bits of the eager calls --
+    on new data written into the captured buffers.  Small grids are launch-bound (cfg1: 7 us per sweep); this is how a
+    caller removes the launch overhead."""
+    nx, ny, nz = 64, 32, 32
+    faces = (inputs.faces_uniform(nx, 2.0), inputs.faces_tanh_two_sided(ny, 2.0), inputs.faces_uniform(nz, 1.0))
+    grid = tdx.Grid(nx, ny, nz, *faces, bcs=BCS)
+    nm = nz // 2 + 1
+    kz2 = inputs.modified_wavenumbers_z(nz, 1.0)
+    alpha = 5e-7
+
+    def step(t, th, st):
+        for d in range(3):
+            grid.adi_sweep(d, tdx.MODE_PPT, 4, alpha, t, st)
+        grid.helmholtz_wavenumber_solve(tdx.MODE_PPT, 4, None, kz2, th, st)
+
+    f1, f2 = inputs.rhs_uniform((nz, ny, nx), 1), inputs.rhs_uniform((nz, ny, nx), 2)
+    h1, h2 = inputs.rhs_complex_uniform((nm, ny, nx), 3), inputs.rhs_complex_uniform((nm, ny, nx), 4)
+    want = []
+    for f, h in ((f1, h1), (f2, h2)):                            # eager, default stream: builds the plans too
+        t, th = torch.from_numpy(f).cuda(), torch.from_numpy(h).cuda()
+        step(t, th, 0)
+        torch.cuda.synchronize()
+        want.append((t.clone(), th.clone()))
+    buf, bufh = torch.from_numpy(f1).cuda(), torch.from_numpy(h1).cuda()
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        scratch, scratchh = buf.clone(), bufh.clone()
+        step(scratch, scratchh, side.cuda_stream)                # once on this stream outside capture
+        side.synchronize()
+        n0 = tdx.kernel_launch_count()
+        cg = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(cg, stream=side):
+            step(buf, bufh, side.cuda_stream)
+        assert tdx.kernel_launch_count() - n0 == 4               # four kernels recorded, none run yet
+    torch.cuda.synchronize()
+    assert torch.equal(buf.cpu(), torch.from_numpy(f1))           # capture does not execute
+    cg.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(buf, want[0][0]) and torch.equal(bufh, want[0][1])
+    buf.copy_(torch.from_numpy(f2)); bufh.copy_(torch.from_numpy(h2))
+    cg.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(buf, want[1][0]) and torch.equal(bufh, want[1][1])
+    del cg
+    grid.close()
+
+
 def test_two_steps_in_flight_equal_the_synchronous_step_bit_exact():
     """tdx_step_host_async: two steps in flight on two slots (different data), then a third on the first slot again, give
     exactly what tdx_step_host gives one at a time; a busy slot is refused; the other host entry points wait for slot 0."""
