@@ -12,7 +12,9 @@
  *   - Pointers marked HOST are read during the call and never retained; pointers marked DEVICE must be valid on
  *     the grid's device and belong to the caller (e.g. torch.Tensor.data_ptr()).  The library never frees them.
  *   - `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  Device entry points are
- *     asynchronous with respect to the host; plan tables are built on first use on the same stream.
+ *     asynchronous with respect to the host; plan tables are built on first use on the same stream (that first call
+ *     allocates and synchronises).  With its plan in the cache a sweep or Helmholtz solve is plain stream work -- no
+ *     allocation, no synchronisation -- and may be recorded by CUDA stream capture (one warm-up call outside the capture).
  *   - Every call returns tdx_status_t.  Argument validation precedes any launch: on an argument error nothing
  *     is written.  tdx_last_error() gives a thread-local message for the last failure on this thread.
  *   - There is no CPU fallback and no other backend: without a CUDA device every solve returns TDX_ERR_CUDA.
