@@ -230,14 +230,14 @@ def sample_shapes(cfg):
     return kx, jz, mh
 
 
-def run_oracle_sample(cfg, repeats=1):
+def run_oracle_sample(cfg, repeats=1, shrink=1):
     """Times the oracle as it stands (Thomas / cyclic Thomas per line, OpenMP over lines). Returns (Gpts/s, info)."""
     sys.path.insert(0, os.path.join(ROOT, "oracle"))
     import oracle as orc
     from paper_1812_01178_b200 import inputs
     xf, yf, zf = cfg.faces()
     bcs = (orc.BC_DIRICHLET, orc.BC_DIRICHLET, orc.BC_PERIODIC)
-    kx, jz, mh = sample_shapes(cfg)
+    kx, jz, mh = (max(1, v // shrink) for v in sample_shapes(cfg))
     fxy = inputs.rhs_uniform((kx, cfg.ny, cfg.nx), cfg.seed)
     fz = inputs.rhs_uniform((cfg.nz, jz, cfg.nx), cfg.seed + 100)
     fh = inputs.rhs_complex_uniform((mh, cfg.ny, cfg.nx), cfg.seed)
@@ -747,6 +747,18 @@ def run_tdx(args, rank, world, local_rank):
         v, _, info = run_oracle_sample(cfg)
         info["value"] = v
         info["unit"] = UNIT
+        try:                                                       # a 1-thread figure beside it (an eighth of the sample)
+            sys.path.insert(0, os.path.join(ROOT, "oracle"))
+            import oracle as orc
+            ncores = orc.num_threads()
+            orc.set_num_threads(1)
+            v1, _, info1 = run_oracle_sample(cfg, shrink=8)
+            orc.set_num_threads(ncores)
+            info["value_1_thread"] = v1
+            info["sample_1_thread"] = info1["sample"]
+        except Exception as exc:
+            info["value_1_thread"] = None
+            info["sample_1_thread"] = repr(exc)[:200]
         out["cpu_baseline"] = info
     grid.close()
     if world > 1:

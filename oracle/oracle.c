@@ -36,6 +36,18 @@ int oracle_num_threads(void) {
 #endif
 }
 
+/* Thread count of the OpenMP loops over lines (bench.py's cpu_baseline quotes an all-cores and a 1-thread figure,
+ * SURVEY 8(d)); no arithmetic depends on it: every line is solved by one thread, start to end. */
+int oracle_set_num_threads(int n) {
+#ifdef _OPENMP
+    if (n >= 1) omp_set_num_threads(n);
+    return omp_get_max_threads();
+#else
+    (void)n;
+    return 1;
+#endif
+}
+
 /* ---------------------------------------------------------------------------------------------
  * Partition map (reading A5; the paper only has m = n/p).
  * q = floor(n/P), r = n mod P, start_p = p*q + min(p,r); partition p owns rows [start_p, start_{p+1}).

@@ -46,6 +46,11 @@ def num_threads():
     return int(_lib.oracle_num_threads())
 
 
+def set_num_threads(n):
+    """OpenMP threads of the loops over lines (timing only: no result depends on it).  Returns the count now in force."""
+    return int(_lib.oracle_set_num_threads(C.c_int(int(n))))
+
+
 def partition_bounds(n, P):
     st = np.zeros(P + 1, dtype=np.int32)
     _chk(_lib.oracle_partition_bounds(C.c_int(n), C.c_int(P), st.ctypes.data_as(_ip)), "partition_bounds")
