@@ -239,8 +239,15 @@ tdx_status_t build_plan(tdx_grid* g, Plan& pl, const double* lambda_host, const 
     const double* qptr = pl.cyc ? qv.as<double>() : nullptr;
     if (pl.thomas) {
         CUDA_TRY(cudaMalloc(&pl.rows, tot * 6 * 8));
+        DevBuf zv;
+        if (pl.cyc) {                                           // the closure's functional on the right-hand side (k_cyclic_z)
+            CUDA_TRY(zv.alloc(tot * 8));
+            k_cyclic_z<<<(nsets + tb - 1) / tb, tb, 0, st>>>(n, nsets, a.as<double>(), b.as<double>(), c.as<double>(), pl.cyc_tab,
+                                                             zv.as<double>(), work.as<double>());
+            LAUNCH_CHECK("k_cyclic_z");
+        }
         k_factor_line<<<(nsets + tb - 1) / tb, tb, 0, st>>>(n, nsets, a.as<double>(), b.as<double>(), c.as<double>(), qptr,
-                                                            flags.as<int>(), pl.rows);
+                                                            pl.cyc ? zv.as<double>() : nullptr, flags.as<int>(), pl.rows);
         LAUNCH_CHECK("k_factor_line");
         CUDA_TRY(cudaStreamSynchronize(st));
         return TDX_OK;

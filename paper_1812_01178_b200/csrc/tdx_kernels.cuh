@@ -410,43 +410,40 @@ __global__ void k_thomas_strided(StridedArgs A, const double* __restrict__ rows,
     double* base = A.data + ((long long)o * A.outer_stride + i) * V;
     const long long rstride = A.line_stride * V;
     const double* rt = rows + (size_t)set * n * 6;
-    double prev[V], cur[V];
+    double prev[V], cur[V], dot[V];
 #pragma unroll
-    for (int v = 0; v < V; ++v) prev[v] = 0.0;
+    for (int v = 0; v < V; ++v) { prev[v] = 0.0; dot[v] = 0.0; }
     for (int j = 0; j < n; ++j) {
         const double l = __ldg(rt + (size_t)j * 6 + F_L);
         VecIO<V>::ld(base + j * rstride, cur);
+        if (CYC) {                                           // z.d = y_0 + g y_{n-1} (k_cyclic_z): the closure's scalar, one pass early
+            const double zj = __ldg(rt + (size_t)j * 6 + F_V);
+#pragma unroll
+            for (int v = 0; v < V; ++v) dot[v] = fma(zj, cur[v], dot[v]);
+        }
 #pragma unroll
         for (int v = 0; v < V; ++v) { cur[v] = fma(-l, prev[v], cur[v]); prev[v] = cur[v]; }
         VecIO<V>::st(base + j * rstride, cur);
     }
-    double ylast[V];
+    double ylast[V], sc[V];
 #pragma unroll
-    for (int v = 0; v < V; ++v) prev[v] = 0.0;
+    for (int v = 0; v < V; ++v) { prev[v] = 0.0; sc[v] = CYC ? __ldg(cyc + set * 4 + 3) * dot[v] : 0.0; }
     for (int j = n - 1; j >= 0; --j) {
         const double inv = __ldg(rt + (size_t)j * 6 + F_INV), cp = __ldg(rt + (size_t)j * 6 + F_CP);
         VecIO<V>::ld(base + j * rstride, cur);
 #pragma unroll
         for (int v = 0; v < V; ++v) { cur[v] = fma(-cp, prev[v], cur[v] * inv); prev[v] = cur[v]; if (j == n - 1) ylast[v] = cur[v]; }
+        if (CYC) {                                           // x_j = y_j - q_j s (Sherman-Morrison, Eq.(3)); prev keeps y_j
+            const double qj = __ldg(rt + (size_t)j * 6 + F_Q);
+#pragma unroll
+            for (int v = 0; v < V; ++v) cur[v] = fma(-qj, sc[v], cur[v]);
+        }
         VecIO<V>::st(base + j * rstride, cur);
     }
     if (A.iface != nullptr && !CYC) {                       // slab sweeps: pack rows 0 and n-1 (prev = x_0, ylast = x_{n-1})
         double* ip = A.iface + ((long long)o * A.W + i) * V;
         VecIO<V>::st(ip, prev);
         VecIO<V>::st(ip + A.iface_plane, ylast);
-    }
-    if (CYC) {
-        const double g = __ldg(cyc + set * 4 + 0), kappa = __ldg(cyc + set * 4 + 3);
-        double s[V];
-#pragma unroll
-        for (int v = 0; v < V; ++v) s[v] = kappa * fma(g, ylast[v], prev[v]);     // prev = y_0 after the backward pass
-        for (int j = 0; j < n; ++j) {
-            const double qj = __ldg(rt + (size_t)j * 6 + F_Q);
-            VecIO<V>::ld(base + j * rstride, cur);
-#pragma unroll
-            for (int v = 0; v < V; ++v) cur[v] = fma(-qj, s[v], cur[v]);
-            VecIO<V>::st(base + j * rstride, cur);
-        }
     }
 }
 
@@ -682,7 +679,7 @@ k_helm_lines(double2* __restrict__ data, int nx, int ny, int P, int q, int rq, i
 // THOMAS mode along x, warp-tiled: a warp owns 32 consecutive lines and walks them 32 columns at a time.  The 32 x 32 tile comes
 // in with coalesced 256-byte row reads (lane = column), is turned through shared memory (33-double rows: conflict-free both
 // ways) so that lane = line runs its recurrence over the 32 columns, and goes back the same way -- forward pass up the line,
-// backward pass down, and for periodic lines a third, purely elementwise pass (x = y - q s, s per line by shuffle).  The
+// backward pass down (periodic lines: the closure's scalar s comes out of the forward pass, k_cyclic_z).  The
 // one-thread-per-line form it replaces read 8 useful bytes per 32-byte sector (cfg5 10.8 ms against 3.1 ms for the strided
 // directions); this one moves the same 32 B per value with full sectors.  Shared memory: 32 * 33 doubles per warp.
 template <bool CYC>
@@ -712,7 +709,7 @@ __global__ void __launch_bounds__(128) k_thomas_unit_tiled(double* __restrict__ 
             for (int r = 0; r < 32; ++r) if (r < nl) base[(long long)r * n + c0 + lane] = tile[r * 33 + lane];
         }
     };
-    double prev = 0.0;
+    double prev = 0.0, dot = 0.0;
     fetch(0);
     for (int c0 = 0; c0 < n; c0 += 32) {                            // forward: y_j = d_j - l_j y_{j-1}
         const int nc = min(32, n - c0);
@@ -722,7 +719,9 @@ __global__ void __launch_bounds__(128) k_thomas_unit_tiled(double* __restrict__ 
         if (lane < nl) {
 #pragma unroll 8
             for (int k = 0; k < nc; ++k) {
-                const double cur = fma(-__ldg(rows + (size_t)(c0 + k) * 6 + F_L), prev, tile[lane * 33 + k]);
+                const double dj = tile[lane * 33 + k];
+                if (CYC) dot = fma(__ldg(rows + (size_t)(c0 + k) * 6 + F_V), dj, dot);      // z.d (k_cyclic_z)
+                const double cur = fma(-__ldg(rows + (size_t)(c0 + k) * 6 + F_L), prev, dj);
                 tile[lane * 33 + k] = cur; prev = cur;
             }
         }
@@ -731,7 +730,7 @@ __global__ void __launch_bounds__(128) k_thomas_unit_tiled(double* __restrict__ 
         __syncwarp();
     }
     prev = 0.0;
-    double ylast = 0.0;
+    const double sc = CYC ? __ldg(cyc + 3) * dot : 0.0;               // s = kappa (y_0 + g y_{n-1}) = kappa z.d of this lane's line
     const int clast = ((n - 1) / 32) * 32;
     // The backward pass re-reads what the forward pass has just written through this same warp: ordinary loads after the
     // stores of the same thread are ordered, and a lane only reads columns it wrote itself (lane = column in both).
@@ -746,21 +745,13 @@ __global__ void __launch_bounds__(128) k_thomas_unit_tiled(double* __restrict__ 
             for (int k = nc - 1; k >= 0; --k) {
                 const int j = c0 + k;
                 const double cur = fma(-__ldg(rows + (size_t)j * 6 + F_CP), prev, tile[lane * 33 + k] * __ldg(rows + (size_t)j * 6 + F_INV));
-                tile[lane * 33 + k] = cur; prev = cur;
-                if (j == n - 1) ylast = cur;
+                prev = cur;                                                                      // y_j; x_j = y_j - q_j s (Eq.(3))
+                tile[lane * 33 + k] = CYC ? fma(-__ldg(rows + (size_t)j * 6 + F_Q), sc, cur) : cur;
             }
         }
         __syncwarp();
-        put(c0);                                                     // (periodic lines: y, the closure needs all of it first)
+        put(c0);
         __syncwarp();
-    }
-    if (CYC) {                                                       // x = y - q (y_0 + g y_{n-1}) kappa   (Sherman-Morrison, Eq.(3))
-        const double s = __ldg(cyc + 3) * fma(__ldg(cyc + 0), ylast, prev);     // prev = y_0 of this lane's line
-        for (int r = 0; r < nl; ++r) {
-            const double sr = __shfl_sync(0xffffffffu, s, r);
-            double* row = base + (long long)r * n;
-            for (int j = lane; j < n; j += 32) row[j] = fma(-__ldg(rows + (size_t)j * 6 + F_Q), sr, row[j]);
-        }
     }
 }
 

@@ -147,6 +147,29 @@ __global__ void k_cyclic_q(int n, int nsets, const double* __restrict__ a, const
     cyc[s * 4 + 3] = 1.0 / (1.0 + q[0] + g * q[n - 1]);
 }
 
+// z = A'^{-T} v, v = (1, 0, ..., 0, g): the functional of the Sherman-Morrison closure taken to the right-hand side,
+// v.y = v.A'^{-1} d = z.d -- so the THOMAS-mode kernels know s = kappa (y_0 + g y_{n-1}) = kappa z.d at the end of their FORWARD
+// pass (which reads every d_j anyway) and the backward pass writes x_j = y_j - s q_j at once: two passes over HBM
+// instead of three.  Thomas recurrence on the transpose (sub-diagonal c_{j-1}, super-diagonal a_{j+1}), one thread per set.
+__global__ void k_cyclic_z(int n, int nsets, const double* __restrict__ a, const double* __restrict__ b,
+                           const double* __restrict__ c, const double* __restrict__ cyc, double* __restrict__ zv,
+                           double* __restrict__ work) {
+    int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= nsets) return;
+    const double* as = a + (size_t)s * n; const double* bs = b + (size_t)s * n; const double* cs = c + (size_t)s * n;
+    double* cp = work + (size_t)s * 2 * n; double* dp = cp + n; double* z = zv + (size_t)s * n;
+    const double g = cyc[s * 4 + 0];
+    cp[0] = (n > 1 ? as[1] : 0.0) / bs[0]; dp[0] = ((n == 1) ? 1.0 + g : 1.0) / bs[0];
+    for (int j = 1; j < n; ++j) {
+        double den = bs[j] - cs[j - 1] * cp[j - 1];
+        cp[j] = (j < n - 1 ? as[j + 1] : 0.0) / den;
+        double vj = (j == n - 1) ? g : 0.0;
+        dp[j] = (vj - cs[j - 1] * dp[j - 1]) / den;
+    }
+    z[n - 1] = dp[n - 1];
+    for (int j = n - 2; j >= 0; --j) z[j] = dp[j] - cp[j] * z[j + 1];
+}
+
 // ---- a2 (matrix part): block factors and spikes. One thread per (set, partition). --------------------------
 // Forward y_j = d_j - l_j y_{j-1};  backward x_j = y_j inv_j - cp_j x_{j+1}  (Thomas with plan-time pivots).
 // ends[(set*P+p)*4 + {0:v_first, 1:v_last, 2:w_first, 3:w_last}].  M = padded rows per partition (identity rows).
@@ -214,16 +237,17 @@ __global__ void k_factor(int n, int nsets, int P, int S, int M, int layout, int 
 }
 
 // Thomas-mode table (P = 1, any n): rows[(set*n + j)*6 + f], one thread per set, no local arrays.
+// F_V carries z_j (k_cyclic_z) for periodic lines, 0 otherwise; F_W is unused.
 __global__ void k_factor_line(int n, int nsets, const double* __restrict__ a, const double* __restrict__ b,
-                              const double* __restrict__ c, const double* __restrict__ qv, const int* __restrict__ flags,
-                              double* __restrict__ rows) {
+                              const double* __restrict__ c, const double* __restrict__ qv, const double* __restrict__ zv,
+                              const int* __restrict__ flags, double* __restrict__ rows) {
     int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= nsets) return;
     const double* as = a + (size_t)s * n; const double* bs = b + (size_t)s * n; const double* cs = c + (size_t)s * n;
     double* rt = rows + (size_t)s * n * 6;
     bool pinned = flags && flags[s];
     double inv_prev = 1.0 / bs[0], cp_prev = (n > 1) ? cs[0] * inv_prev : 0.0;
-    rt[F_L] = 0.0; rt[F_INV] = pinned ? 0.0 : inv_prev; rt[F_CP] = cp_prev; rt[F_V] = 0.0; rt[F_W] = 0.0;
+    rt[F_L] = 0.0; rt[F_INV] = pinned ? 0.0 : inv_prev; rt[F_CP] = cp_prev; rt[F_V] = zv ? zv[(size_t)s * n] : 0.0; rt[F_W] = 0.0;
     rt[F_Q] = qv ? qv[(size_t)s * n] : 0.0;
     for (int j = 1; j < n; ++j) {
         double lj = as[j] * inv_prev;
@@ -231,7 +255,7 @@ __global__ void k_factor_line(int n, int nsets, const double* __restrict__ a, co
         double invj = 1.0 / den;
         double cpj = (j < n - 1) ? cs[j] * invj : 0.0;
         double* rj = rt + (size_t)j * 6;
-        rj[F_L] = (pinned && j == 1) ? 0.0 : lj; rj[F_INV] = invj; rj[F_CP] = cpj; rj[F_V] = 0.0; rj[F_W] = 0.0;
+        rj[F_L] = (pinned && j == 1) ? 0.0 : lj; rj[F_INV] = invj; rj[F_CP] = cpj; rj[F_V] = zv ? zv[(size_t)s * n + j] : 0.0; rj[F_W] = 0.0;
         rj[F_Q] = qv ? qv[(size_t)s * n + j] : 0.0;
         inv_prev = invj; cp_prev = cpj;
     }
