@@ -52,7 +52,7 @@ def ncu_traffic(workload, launch):
 
 
 # tuned partitions per line (x, y, z, helmholtz-y) per config, mode PPT (exact for every P)
-TUNED_P = {1: (4, 4, 4, 4), 2: (16, 8, 8, 8), 3: (32, 8, 8, 8), 4: (128, 16, 8, 16), 5: (256, 24, 16, 12), 6: (384, 8, 24, 8)}
+TUNED_P = {1: (4, 4, 4, 4), 2: (16, 8, 8, 8), 3: (32, 8, 8, 8), 4: (128, 32, 8, 16), 5: (256, 12, 16, 12), 6: (384, 8, 24, 8)}
 
 
 def pdd_partitions(grid, cfg, direction, P_ppt):

@@ -86,14 +86,14 @@ def test_adi_sweeps_fullsize_sampled_lines(cfg_no, mode_name):
 
 
 def test_pdd_outside_its_regime_errs_by_the_bound_and_strict_refuses():
-    """NOT the bench configuration: cfg4's y sweep with the PPT-tuned P = 16, where the spikes of the near-wall partitions
+    """NOT the bench configuration: cfg4's y sweep with P = 16 (a good PPT choice: 32-row partitions), where the spikes of the near-wall partitions
     have not decayed (a-priori bound 3.6e-7).  PDD runs as asked (never a silent fallback), is wrong by about the bound --
     three orders outside north_star's 1e-10 -- and the strict switch refuses it."""
     c = configs.get(4)
     _need(int(c.npts * 8 * 1.3))
     faces = c.faces()
     grid = tdx.Grid(c.nx, c.ny, c.nz, *faces, bcs=BCS)
-    P = bench.TUNED_P[4][1]
+    P = 16
     dropped = grid.pdd_dropped_bound(1, P, c.alpha)
     assert dropped > 1e-8
     t = torch.from_numpy(c.rhs_field()).cuda()
