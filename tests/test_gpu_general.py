@@ -112,6 +112,35 @@ def test_weakly_dominant_per_line_systems_take_the_partition_path_only(direction
     grid.close()
 
 
+@pytest.mark.parametrize("nx", [256, 512, 768, 1024, 2048])
+@pytest.mark.parametrize("kind", ["weak", "strong", "random"])
+def test_x_lines_of_many_partitions(nx, kind):
+    """Long x lines: 32 to 256 partitions per line (1 to 8 warps of one CTA work on a line; 5 to 8 reduction steps), several
+    lines per CTA with a partly filled last CTA.  'weak': |b| = |a| + |c| + eps, eps down to 1e-6 (couplings that do not
+    decay: every reduction step runs; lines of tame blocks are accepted WITHOUT a residual check, so only the oracle sees a
+    wrong reduced solve); 'strong': decayed spikes (the early exit); 'random': non-dominant lines, re-solved ones included.
+    Gate: kappa * eps per line against the dense LAPACK oracle."""
+    ny, nz = 3, 2
+    grid, a, b, c, d = _setup(nx, ny, nz, 1200 + nx, 0.3 if kind == "random" else 1.0)
+    if kind != "random":
+        a = -(0.2 + np.abs(a)); c = -(0.2 + np.abs(c))
+        eps = 10.0 ** (-6.0 * np.abs(b)) if kind == "weak" else 2.0 + np.abs(b)
+        eps = np.broadcast_to(eps[:, :, :1], eps.shape).copy()                      # one shift per line
+        a[:, :, 0] = 0.0; c[:, :, -1] = 0.0
+        b = -(a + c) + eps
+    got = _solve(grid, 0, True, a, b, c, d)
+    assert tdx.last_launch().startswith("k_general_part<8,0,1,1>") and "block=(%d," % (nx // 8) in tdx.last_launch().replace(" ", "")
+    nfb = grid.general_fallback_count()
+    if kind != "random":
+        assert nfb == 0
+    ref, A = ogen.general_solve(a, b, c, d, 2)
+    cond = np.linalg.cond(A)
+    err = np.max(np.abs(got - ref).reshape(-1, nx), axis=1)
+    scale = np.max(np.abs(ref).reshape(-1, nx), axis=1)
+    assert np.all(err <= 50 * cond * EPS * scale), float(np.max(err / (cond * EPS * scale)))
+    grid.close()
+
+
 @pytest.mark.parametrize("direction", [0, 1, 2])
 @pytest.mark.parametrize("share", [0.06, 0.6])
 def test_mixed_lines_only_the_lines_that_need_pivots_are_re_solved(direction, share):
