@@ -620,7 +620,9 @@ def run_tdx(args, rank, world, local_rank):
                     # both methods (include/tdx.h): "partition" = the one-pass partition kernel (the default: optimistic plain
                     # elimination inside the partitions, checked, unsafe lines re-solved with pivots); "lines" = one thread
                     # per line with diagonal pivoting, two passes
-                    for meth, flag, nbytes in (("lines", tdx.GENERAL_FORCE_LINES, 82), ("partition", tdx.GENERAL_FORCE_PARTITION, 40)):
+                    # "default" = no method forced: a sample of the rows decides on the device (mostly non-dominant rows: the
+                    # per-line kernel on every line; else the partition kernel)
+                    for meth, flag, nbytes in (("lines", tdx.GENERAL_FORCE_LINES, 82), ("partition", tdx.GENERAL_FORCE_PARTITION, 40), ("default", 0, 40)):
                         for _ in range(2):
                             gd.copy_(field0); grid.general_solve(1, 1 | flag, ga, gb, gc, gd, gwork, stream)
                         barrier()
@@ -632,13 +634,18 @@ def run_tdx(args, rank, world, local_rank):
                             torch.cuda.synchronize()
                             tot += s0.elapsed_time(s1)
                         msg = max_over_ranks(tot / args.steps, dist, "cuda")
-                        nfb = grid.general_fallback_count() if meth == "partition" else 0
+                        nfb = grid.general_fallback_count()
+                        launch = tdx.last_launch()
+                        if meth == "default" and nfb == cfg.nx * cfg.nz:
+                            nbytes = 82                                    # the device chose the per-line kernel for every line
+                            launch = "k_general_lines<1,0,0> on every line (chosen on the device; the partition kernel returned at once)"
                         res[meth] = {"ms": msg, "gpts_per_s": cfg.npts / (msg * 1e-3) / 1e9, "algorithmic_bytes_per_value": nbytes,
                                      "gb_per_s": nbytes * cfg.npts / (msg * 1e-3) / 1e9,
                                      "frac_of_measured_peak": nbytes * cfg.npts / (msg * 1e-3) / 1e9 / peak, "finite": bool(torch.isfinite(gd).all()),
-                                     "lines_re_solved_by_the_per_line_kernel": nfb, "share_of_lines": nfb / (cfg.nx * cfg.nz), "launch": tdx.last_launch()}
+                                     "lines_re_solved_by_the_per_line_kernel": nfb, "share_of_lines": nfb / (cfg.nx * cfg.nz), "launch": launch}
                     gout[wname] = res
-                gout["what"] = "tdx_general_solve along y, per-line a, b, c, diagonal pivoting: partition kernel (8-row partitions, one pass, 40 B per value; the default) and per-line kernel (two passes, 82 B per value)"
+                gout["what"] = ("tdx_general_solve along y, per-line a, b, c, diagonal pivoting: partition kernel (8-row partitions, one pass, 40 B per value), "
+                                "per-line kernel (two passes, 82 B per value), and the default (the device picks one of the two from a sample of the rows)")
                 out["general_solve_pivoting"] = gout
                 del ga, gb, gc, gd, gwork
         except Exception as exc:

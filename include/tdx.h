@@ -204,8 +204,11 @@ tdx_status_t tdx_slab_dropped_bound(tdx_slab_t* slab, double* out);
  * TDX_GENERAL_PIVOT_PARTITIONS keeps the pivots inside the partitions instead (fewer re-solved lines on non-dominant
  * systems, slower on dominant ones).
  * LINES: one thread per line, diagonal pivoting over the whole line, two passes over HBM (about 82 B per value).
- * Default: PARTITION wherever it applies (it measured faster in every direction); OR the flags below into
- * `pivoting` to force one.  Periodic lines, and lines of fewer than 4 or more than 4096 rows, always take LINES.
+ * Default: PARTITION wherever it applies (it measured faster in every direction on dominant systems) -- except
+ * that a pivoting solve along y or z first samples 32768 rows ON THE DEVICE (no host synchronisation; the same choice for
+ * the same input): where more than a quarter of them are not diagonally dominant, most lines would be re-solved anyway
+ * and LINES runs on every line straight away (tdx_general_fallback_count then reports every line).  OR the flags below
+ * into `pivoting` to force a method.  Periodic lines, and lines of fewer than 4 or more than 4096 rows, always take LINES.
  * work: DEVICE scratch, caller-owned, 8-byte aligned: 9*nx*ny*nz + 8 bytes (tdx_general_solve), 25*nx*ny*nz + 24 bytes
  * (tdx_general_cyclic_solve).  A singular line yields inf / nan in that line.  Asynchronous on `stream`.       */
 #define TDX_GENERAL_PIVOT 1

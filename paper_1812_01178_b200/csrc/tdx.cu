@@ -139,7 +139,9 @@ struct tdx_grid {
     struct WaveTab { uint64_t hash; int n; double* dev; };
     std::vector<WaveTab> wave;                          // device copies of caller wavenumber arrays, keyed by content hash
     bool attr_helm_lines = false;                       // cudaFuncSetAttribute done for this grid's device
-    unsigned int* fb = nullptr; unsigned fb_cap = 0;    // tdx_general_solve: [0] = number of lines that fell back, [4..] = their indices
+    unsigned int* fb = nullptr; unsigned fb_cap = 0;    // tdx_general_solve: [0] = number of lines that fell back, [1] = non-dominant rows of the sample, [4..] = their indices
+    unsigned fb_nsamp = 0, fb_nlines = 0;               // last general solve: sample size (0 = no method choice) and its line count
+    bool fb_valid = false;                              // the last general solve went through the partition method
     double* stage2 = nullptr; size_t stage2_bytes = 0;  // second staging buffer (Helmholtz part of tdx_step_host)
     // tdx_step_host_async: two slots, each with its own staging pair (slot 0 = stage / stage2 above), the events of the step in
     // flight and the event that marks its last download
@@ -1646,6 +1648,8 @@ static tdx_status_t general_solve_impl(tdx_grid_t* g, tdx_dir_t dir, int pivotin
     if (!part) {                                                                         // one thread per line over the whole line
         dim3 block(128), grid((unsigned)std::min<long long>((G.W + 127) / 128, 1 << 20), (unsigned)O);
         G.fb_count = nullptr; G.fb_lines = nullptr; G.fb_flag = nullptr; G.fb_cap = 0; G.P = 1; G.q = n; G.r = 0;
+        G.sel = nullptr; G.nsamp = 0; G.sel_lines = 0;
+        g->fb_nsamp = 0; g->fb_valid = false;
         if (periodic) { if (pivoting) tdx::k_general_lines<true, false, true><<<grid, block, 0, st>>>(G, bm, flag, qv, dv); else tdx::k_general_lines<false, false, true><<<grid, block, 0, st>>>(G, bm, flag, qv, dv); }
         else { if (pivoting) tdx::k_general_lines<true, false, false><<<grid, block, 0, st>>>(G, bm, flag, qv, dv); else tdx::k_general_lines<false, false, false><<<grid, block, 0, st>>>(G, bm, flag, qv, dv); }
         LAUNCH_CHECK("k_general_lines");
@@ -1664,8 +1668,21 @@ static tdx_status_t general_solve_impl(tdx_grid_t* g, tdx_dir_t dir, int pivotin
     G.fb_count = g->fb; G.fb_lines = g->fb + 4; G.fb_cap = nlines;
     G.fb_flag = reinterpret_cast<unsigned char*>(g->fb + 4 + (size_t)g->fb_cap);       // after the list (allocated capacity)
     G.P = P; G.q = n / P; G.r = n % P;
-    CUDA_TRY(cudaMemsetAsync(g->fb, 0, 4, st));
+    CUDA_TRY(cudaMemsetAsync(g->fb, 0, 8, st));
     CUDA_TRY(cudaMemsetAsync(G.fb_flag, 0, nlines, st));
+    // Default method of a pivoting solve along y / z: chosen on the device from a sample of the rows (tdx_general.cuh,
+    // k_general_sample) -- no host synchronisation, the same choice for the same input.  Where most rows are not diagonally
+    // dominant the optimistic partition pass would hand most lines to the per-line kernel anyway (cfg5, |b| <= 0.3 |a|:
+    // 22.5 ms against 12.7 for the per-line kernel alone), so that kernel runs on all lines straight away.  x lines always
+    // take the partition method (one thread per line reads 8 useful bytes per sector there: 77 ms).
+    G.sel = nullptr; G.nsamp = 0; G.sel_lines = 0;
+    const bool choose = pivoting && method == 0 && dir != TDX_DIR_X && !(flags_in & TDX_GENERAL_PIVOT_PARTITIONS);
+    if (choose) {
+        G.nsamp = 32768; G.sel = g->fb + 1;
+        tdx::k_general_sample<<<G.nsamp / 128, 128, 0, st>>>(a, b, c, (unsigned long long)npts, G.nsamp, g->fb + 1);
+        LAUNCH_CHECK("k_general_sample");
+    }
+    g->fb_nsamp = G.nsamp; g->fb_nlines = nlines; g->fb_valid = true;
     const bool unit = dir == TDX_DIR_X;
     // lines per CTA: small CTAs (several resident per SM at different phases: load / eliminate / reduce / store) beat one
     // large one; x lines: whole lines of P consecutive lanes.  TDX_GENERAL_LINES (measurement knob) overrides.
@@ -1697,6 +1714,13 @@ static tdx_status_t general_solve_impl(tdx_grid_t* g, tdx_dir_t dir, int pivotin
     if (pivoting) tdx::k_general_lines<true, true, false><<<fgrid, 128, 0, st>>>(G, bm, flag, qv, dv);
     else tdx::k_general_lines<false, true, false><<<fgrid, 128, 0, st>>>(G, bm, flag, qv, dv);
     LAUNCH_CHECK("k_general_lines");
+    if (choose) {                                                                        // the other branch of the choice: every line, one thread each
+        tdx::GeneralArgs GL = G;
+        GL.sel_lines = 1; GL.P = 1; GL.q = n; GL.r = 0;
+        dim3 lgrid((unsigned)std::min<long long>((G.W + 127) / 128, 1 << 20), (unsigned)O);
+        tdx::k_general_lines<true, false, false><<<lgrid, 128, 0, st>>>(GL, bm, flag, qv, dv);
+        LAUNCH_CHECK("k_general_lines");
+    }
     return TDX_OK;
 }
 
@@ -1713,11 +1737,12 @@ tdx_status_t tdx_general_cyclic_solve(tdx_grid_t* g, tdx_dir_t dir, int pivoting
 tdx_status_t tdx_general_fallback_count(tdx_grid_t* g, long long* out) {
     if (!g || !out) return fail(TDX_ERR_INVALID_ARG, "NULL argument");
     *out = 0;
-    if (!g->fb) return TDX_OK;
+    if (!g->fb || !g->fb_valid) return TDX_OK;                            // (a call that was forced to the per-line kernel: 0)
     CUDA_TRY(cudaSetDevice(g->device));
-    unsigned v = 0;
-    CUDA_TRY(cudaMemcpy(&v, g->fb, 4, cudaMemcpyDeviceToHost));           // waits for the solve that wrote it
-    *out = v;
+    unsigned v[2] = {0, 0};
+    CUDA_TRY(cudaMemcpy(v, g->fb, 8, cudaMemcpyDeviceToHost));            // waits for the solve that wrote it
+    // the device chose the per-line kernel for every line (method choice of the default, general_solve_impl)
+    *out = (g->fb_nsamp && v[1] * 4u > g->fb_nsamp) ? (long long)g->fb_nlines : (long long)v[0];
     return TDX_OK;
 }
 

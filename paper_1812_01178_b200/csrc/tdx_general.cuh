@@ -50,7 +50,34 @@ struct GeneralArgs {
     unsigned int* fb_lines;              // their indices o * W + l
     unsigned int fb_cap;
     unsigned char* fb_flag;              // the same lines as one byte per line (1 = fell back): for the dense case, see k_general_lines
+    // method choice on the device (default method of a pivoting solve along y / z, tdx.cu): sel[0] = rows of k_general_sample's
+    // sample that are not diagonally dominant.  More than a quarter of nsamp: the optimistic partition pass would be wasted
+    // work (most lines would be re-solved), so the kernels of the PARTITION method return at once and the all-lines launch of
+    // k_general_lines (sel_lines = 1) does the work; else the other way round.  sel = NULL: no choice, every kernel runs.
+    const unsigned int* sel;
+    unsigned int nsamp;
+    int sel_lines;
 };
+
+__device__ __forceinline__ bool general_deselected(const GeneralArgs& G) {
+    if (G.sel == nullptr) return false;
+    const bool lines = __ldg(G.sel) * 4u > G.nsamp;
+    return lines != (G.sel_lines != 0);
+}
+
+// The sample: nsamp rows spread over the whole field (a multiplicative hash of the thread index), counted when
+// |b| < |a| + |c|.  One launch of a few microseconds; the count is final when the kernels behind it on the stream start.
+__global__ void k_general_sample(const double* __restrict__ a, const double* __restrict__ b, const double* __restrict__ c,
+                                 unsigned long long npts, unsigned int nsamp, unsigned int* __restrict__ count) {
+    const unsigned int t = blockIdx.x * blockDim.x + threadIdx.x;
+    bool nd = false;
+    if (t < nsamp) {
+        const unsigned long long e = ((unsigned long long)t * 0x9E3779B97F4A7C15ull >> 11) % npts;
+        nd = !(fabs(__ldg(b + e)) >= fabs(__ldg(a + e)) + fabs(__ldg(c + e)));
+    }
+    const unsigned m = __ballot_sync(0xffffffffu, nd);
+    if ((threadIdx.x & 31) == 0 && m) atomicAdd(count, (unsigned)__popc(m));
+}
 
 // A line is accepted when every block was "tame" (1x1 pivots only, spikes <= 1: what a diagonally dominant block does -- the
 // partition method is stable there, and a nearly singular dominant line, eps ~ 1e-6, cannot meet a backward-error test:
@@ -69,6 +96,7 @@ constexpr double kGeneralBackwardError = 128.0 * 2.220446049250313e-16;
 template <int M, bool PIVOT, bool UNIT, bool FULL>
 __global__ void __maxnreg__(M <= 8 ? (PIVOT ? 128 : (UNIT ? 112 : 96)) : 168)
 k_general_part(GeneralArgs G) {
+    if (general_deselected(G)) return;
     extern __shared__ double gs[];
     const int P = G.P;
     const int p = UNIT ? threadIdx.x : threadIdx.y, lt = UNIT ? threadIdx.y : threadIdx.x;
@@ -298,6 +326,7 @@ k_general_part(GeneralArgs G) {
 template <bool PIVOT, bool LIST, bool CYC>
 __global__ void __launch_bounds__(128) k_general_lines(GeneralArgs G, double* __restrict__ bm, unsigned char* __restrict__ fg, double* __restrict__ qv,
                                                        double* __restrict__ dv) {
+    if (general_deselected(G)) return;
     const double kappa = 0.6180339887498949;
     const int n = G.n;
     const long long rs = G.row_stride;

@@ -112,6 +112,38 @@ def test_weakly_dominant_per_line_systems_take_the_partition_path_only(direction
     grid.close()
 
 
+@pytest.mark.parametrize("direction", [0, 1, 2])
+def test_default_method_is_chosen_on_the_device_from_a_sample_of_the_rows(direction):
+    """method = 0 with pivoting: along y and z a sample of the rows decides on the device (no host synchronisation) --
+    mostly non-dominant rows: the per-line kernel solves every line at once (bit-equal to TDX_GENERAL_FORCE_LINES, the count
+    of lines that left the partition method = all); dominant rows, also with a few wild lines in between: the optimistic
+    partition pass (bit-equal to TDX_GENERAL_FORCE_PARTITION).  x lines always take the partition method."""
+    nx, ny, nz = 72, 64, 40
+    grid, a, b, c, d = _setup(nx, ny, nz, 1300 + direction, 0.3)
+    nlines = d.size // d.shape[AXIS[direction]]
+    dflt = _solve(grid, direction, True, a, b, c, d, method=0)
+    n_dflt = grid.general_fallback_count()
+    forced_l = _solve(grid, direction, True, a, b, c, d, method=tdx.GENERAL_FORCE_LINES)
+    forced_p = _solve(grid, direction, True, a, b, c, d, method=tdx.GENERAL_FORCE_PARTITION)
+    n_part = grid.general_fallback_count()
+    if direction == 0:
+        assert np.array_equal(dflt, forced_p) and n_dflt == n_part and 0 < n_part < nlines
+    else:
+        assert np.array_equal(dflt, forced_l) and n_dflt == nlines
+    # dominant rows with 5 % wild lines: the partition pass, whatever the direction
+    axis = AXIS[direction]
+    n = d.shape[axis]
+    pick = inputs.uniform_pm1(78, nlines, stream=5)
+    shape = list(d.shape); shape[axis] = 1
+    wild = np.broadcast_to((0.5 * (pick + 1.0) < 0.05).reshape(shape), d.shape)
+    b2 = np.where(wild, b, np.abs(a) + np.abs(c) + 0.5 + np.abs(b))
+    dflt = _solve(grid, direction, True, a, b2, c, d, method=0)
+    n_dflt = grid.general_fallback_count()
+    forced_p = _solve(grid, direction, True, a, b2, c, d, method=tdx.GENERAL_FORCE_PARTITION)
+    assert np.array_equal(dflt, forced_p) and n_dflt == grid.general_fallback_count() <= int(wild.sum()) // n
+    grid.close()
+
+
 @pytest.mark.parametrize("nx", [256, 512, 768, 1024, 2048])
 @pytest.mark.parametrize("kind", ["weak", "strong", "random"])
 def test_x_lines_of_many_partitions(nx, kind):
