@@ -205,7 +205,7 @@ tdx_status_t tdx_slab_dropped_bound(tdx_slab_t* slab, double* out);
  * systems, slower on dominant ones).
  * LINES: one thread per line, diagonal pivoting over the whole line, two passes over HBM (about 82 B per value).
  * Default: PARTITION wherever it applies (it measured faster in every direction on dominant systems) -- except
- * that a pivoting solve along y or z first samples 32768 rows ON THE DEVICE (no host synchronisation; the same choice for
+ * that a pivoting solve first samples 32768 rows ON THE DEVICE (no host synchronisation; the same choice for
  * the same input): where more than a quarter of them are not diagonally dominant, most lines would be re-solved anyway
  * and LINES runs on every line straight away (tdx_general_fallback_count then reports every line).  OR the flags below
  * into `pivoting` to force a method.  Periodic lines, and lines of fewer than 4 or more than 4096 rows, always take LINES.

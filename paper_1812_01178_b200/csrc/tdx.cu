@@ -1634,7 +1634,7 @@ static tdx_status_t general_solve_impl(tdx_grid_t* g, tdx_dir_t dir, int pivotin
     double* qv = reinterpret_cast<double*>(flag + ((npts + 7) / 8) * 8);                 // periodic only (25 bytes per value in all)
     double* dv = qv + npts;
     // Method: the partition kernel (8 rows per thread, P threads of a line in one CTA) wherever it applies -- measured on cfg5
-    // (DESIGN.md 9f): 6.63 / 8.9 / 11.5 ms along y / z / x against 10.9 / 11.2 / 77 ms for one thread per line -- unless the
+    // (DESIGN.md 9f): 6.5 / 8.7 / 11.0 ms along y / z / x against 10.9 / 11.2 / 41 ms for one thread per line -- unless the
     // caller forces the per-line kernel.
     const int flags_in = pivoting;
     const int method = pivoting & (TDX_GENERAL_FORCE_PARTITION | TDX_GENERAL_FORCE_LINES);
@@ -1647,6 +1647,7 @@ static tdx_status_t general_solve_impl(tdx_grid_t* g, tdx_dir_t dir, int pivotin
     const bool part = can_part && method != TDX_GENERAL_FORCE_LINES;
     if (!part) {                                                                         // one thread per line over the whole line
         dim3 block(128), grid((unsigned)std::min<long long>((G.W + 127) / 128, 1 << 20), (unsigned)O);
+        if (dir == TDX_DIR_X) grid.x = (unsigned)std::min<long long>(grid.x, (long long)g->sms * 4);   // x lines: few lines in flight per SM (see the re-solve below)
         G.fb_count = nullptr; G.fb_lines = nullptr; G.fb_flag = nullptr; G.fb_cap = 0; G.P = 1; G.q = n; G.r = 0;
         G.sel = nullptr; G.nsamp = 0; G.sel_lines = 0;
         g->fb_nsamp = 0; g->fb_valid = false;
@@ -1670,13 +1671,13 @@ static tdx_status_t general_solve_impl(tdx_grid_t* g, tdx_dir_t dir, int pivotin
     G.P = P; G.q = n / P; G.r = n % P;
     CUDA_TRY(cudaMemsetAsync(g->fb, 0, 8, st));
     CUDA_TRY(cudaMemsetAsync(G.fb_flag, 0, nlines, st));
-    // Default method of a pivoting solve along y / z: chosen on the device from a sample of the rows (tdx_general.cuh,
+    // Default method of a pivoting solve: chosen on the device from a sample of the rows (tdx_general.cuh,
     // k_general_sample) -- no host synchronisation, the same choice for the same input.  Where most rows are not diagonally
-    // dominant the optimistic partition pass would hand most lines to the per-line kernel anyway (cfg5, |b| <= 0.3 |a|:
-    // 22.5 ms against 12.7 for the per-line kernel alone), so that kernel runs on all lines straight away.  x lines always
-    // take the partition method (one thread per line reads 8 useful bytes per sector there: 77 ms).
+    // dominant the optimistic partition pass would hand most lines to the per-line kernel anyway (cfg5, |b| <= 0.3 |a|, along
+    // y: 22.5 ms against 12.7 for the per-line kernel alone; along x: 55 against 41), so that kernel runs on all lines
+    // straight away.
     G.sel = nullptr; G.nsamp = 0; G.sel_lines = 0;
-    const bool choose = pivoting && method == 0 && dir != TDX_DIR_X && !(flags_in & TDX_GENERAL_PIVOT_PARTITIONS);
+    const bool choose = pivoting && method == 0 && !(flags_in & TDX_GENERAL_PIVOT_PARTITIONS);
     if (choose) {
         G.nsamp = 32768; G.sel = g->fb + 1;
         tdx::k_general_sample<<<G.nsamp / 128, 128, 0, st>>>(a, b, c, (unsigned long long)npts, G.nsamp, g->fb + 1);
@@ -1710,7 +1711,10 @@ static tdx_status_t general_solve_impl(tdx_grid_t* g, tdx_dir_t dir, int pivotin
     LAUNCH_CHECK("k_general_part");
     note_launch("k_general_part<%d,%d,%d,%d>", 8, pv_part ? 1 : 0, unit ? 1 : 0, full ? 1 : 0, 0, 0, grid, block);
     // the lines whose blocks were numerically singular: one thread per line (none on weakly dominant systems)
-    dim3 fgrid((unsigned)(g->sms * 8));                                                  // 62 registers: 8 CTAs of 128 threads per SM
+    // 62 registers: 8 CTAs of 128 threads per SM -- but 4 for x lines: every lane walks its own contiguous line there, 8 bytes
+    // of a 32-byte sector per access, and the sectors survive in L1 until the next three accesses only if few enough lines
+    // are in flight per SM (cfg5, every x line re-solved: 103 ms at 8 CTAs per SM, 55 at 4, 60 at 2)
+    dim3 fgrid((unsigned)(g->sms * (dir == TDX_DIR_X ? 4 : 8)));
     if (pivoting) tdx::k_general_lines<true, true, false><<<fgrid, 128, 0, st>>>(G, bm, flag, qv, dv);
     else tdx::k_general_lines<false, true, false><<<fgrid, 128, 0, st>>>(G, bm, flag, qv, dv);
     LAUNCH_CHECK("k_general_lines");
@@ -1718,6 +1722,7 @@ static tdx_status_t general_solve_impl(tdx_grid_t* g, tdx_dir_t dir, int pivotin
         tdx::GeneralArgs GL = G;
         GL.sel_lines = 1; GL.P = 1; GL.q = n; GL.r = 0;
         dim3 lgrid((unsigned)std::min<long long>((G.W + 127) / 128, 1 << 20), (unsigned)O);
+        if (dir == TDX_DIR_X) lgrid.x = (unsigned)std::min<long long>(lgrid.x, (long long)g->sms * 4);
         tdx::k_general_lines<true, false, false><<<lgrid, 128, 0, st>>>(GL, bm, flag, qv, dv);
         LAUNCH_CHECK("k_general_lines");
     }

@@ -114,10 +114,10 @@ def test_weakly_dominant_per_line_systems_take_the_partition_path_only(direction
 
 @pytest.mark.parametrize("direction", [0, 1, 2])
 def test_default_method_is_chosen_on_the_device_from_a_sample_of_the_rows(direction):
-    """method = 0 with pivoting: along y and z a sample of the rows decides on the device (no host synchronisation) --
-    mostly non-dominant rows: the per-line kernel solves every line at once (bit-equal to TDX_GENERAL_FORCE_LINES, the count
-    of lines that left the partition method = all); dominant rows, also with a few wild lines in between: the optimistic
-    partition pass (bit-equal to TDX_GENERAL_FORCE_PARTITION).  x lines always take the partition method."""
+    """method = 0 with pivoting: a sample of the rows decides on the device (no host synchronisation) -- mostly non-dominant
+    rows: the per-line kernel solves every line at once (bit-equal to TDX_GENERAL_FORCE_LINES, the count of lines that left
+    the partition method = all); dominant rows, also with a few wild lines in between: the optimistic partition pass
+    (bit-equal to TDX_GENERAL_FORCE_PARTITION)."""
     nx, ny, nz = 72, 64, 40
     grid, a, b, c, d = _setup(nx, ny, nz, 1300 + direction, 0.3)
     nlines = d.size // d.shape[AXIS[direction]]
@@ -126,10 +126,7 @@ def test_default_method_is_chosen_on_the_device_from_a_sample_of_the_rows(direct
     forced_l = _solve(grid, direction, True, a, b, c, d, method=tdx.GENERAL_FORCE_LINES)
     forced_p = _solve(grid, direction, True, a, b, c, d, method=tdx.GENERAL_FORCE_PARTITION)
     n_part = grid.general_fallback_count()
-    if direction == 0:
-        assert np.array_equal(dflt, forced_p) and n_dflt == n_part and 0 < n_part < nlines
-    else:
-        assert np.array_equal(dflt, forced_l) and n_dflt == nlines
+    assert np.array_equal(dflt, forced_l) and n_dflt == nlines and 0 < n_part < nlines
     # dominant rows with 5 % wild lines: the partition pass, whatever the direction
     axis = AXIS[direction]
     n = d.shape[axis]
