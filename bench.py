@@ -716,7 +716,14 @@ def run_tdx(args, rank, world, local_rank):
     elif not args.no_e2e:
         # two independent pinned buffer pairs: consecutive steps go through tdx_step_host_async in alternating slots, so one
         # step's download runs beside the next step's upload (one call alone is bound to three transfer times)
-        pairs = [(torch.from_numpy(host_field).pin_memory().numpy(), torch.from_numpy(host_helm).pin_memory().numpy()) for _ in range(2)]
+        pairs, two = [], 1.0
+        try:
+            for _ in range(2):
+                pairs.append((torch.from_numpy(host_field).pin_memory().numpy(), torch.from_numpy(host_helm).pin_memory().numpy()))
+        except RuntimeError:                                                       # no room to page-lock a second pair on this host
+            two = 0.0
+        two = -max_over_ranks(-two, dist, "cuda") > 0.5                            # every rank or none
+        nslots = 2 if two else 1
         hf, hh = pairs[0]
         grid.step_host(mode, Ps[0], Ps[1], Ps[2], cfg.alpha, hf, Ps[3], kz2, hh)   # warm-up (staging allocation, streams)
         np.copyto(hh, host_helm)
@@ -725,21 +732,21 @@ def run_tdx(args, rank, world, local_rank):
         grid.step_host(mode, Ps[0], Ps[1], Ps[2], cfg.alpha, hf, Ps[3], kz2, hh)
         torch.cuda.synchronize()
         t_single = time.perf_counter() - t0
-        for slot in (0, 1):                                                        # warm-up of the second slot's staging
+        for slot in range(nslots):                                                 # warm-up of the second slot's staging
             grid.step_host_async(slot, mode, Ps[0], Ps[1], Ps[2], cfg.alpha, pairs[slot][0], Ps[3], kz2, pairs[slot][1])
-        for slot in (0, 1):
+        for slot in range(nslots):
             grid.step_host_wait(slot)
-        for slot in (0, 1):
+        for slot in range(nslots):
             np.copyto(pairs[slot][1], host_helm)
         nsteps = max(8, 2 * args.e2e_steps)                                        # fill and drain cost one transfer time in all
         barrier()
         t0 = time.perf_counter()
         for k in range(nsteps):
-            slot = k % 2
-            if k >= 2:
+            slot = k % nslots
+            if k >= nslots:
                 grid.step_host_wait(slot)                                          # the step that used this slot's buffers is home
             grid.step_host_async(slot, mode, Ps[0], Ps[1], Ps[2], cfg.alpha, pairs[slot][0], Ps[3], kz2, pairs[slot][1])
-        for slot in (0, 1):
+        for slot in range(nslots):
             grid.step_host_wait(slot)
         torch.cuda.synchronize()
         te = max_over_ranks((time.perf_counter() - t0) / nsteps, dist, "cuda")
@@ -747,6 +754,7 @@ def run_tdx(args, rank, world, local_rank):
         out["e2e"] = {"value": world * step_points(cfg) / te / 1e9, "unit": UNIT, "h2d_bytes_per_step": int(hf.nbytes + hh.nbytes),
                       "d2h_bytes_per_step": int(hf.nbytes + hh.nbytes), "ms_per_step": te * 1e3, "steps": nsteps,
                       "single_call_ms": t_single * 1e3, "single_call_value": world * step_points(cfg) / t_single / 1e9,
+                      "steps_in_flight": nslots,
                       "api": "tdx_step_host_async / tdx_step_host_wait, two steps in flight on two pinned buffer pairs (every step's "
                              "inputs go up and its results come down inside the timed region); single_call = one synchronous "
                              "tdx_step_host"}
